@@ -1,0 +1,21 @@
+"""CPU oracle for the dfrg loop integrals -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package.  It compiles oracle/dfrg_oracle.cpp with g++ (plain C++,
+OpenMP across outputs) and exposes it through ctypes on numpy arrays.  It imports
+nothing from paper_2412_13043_b200 and the CUDA path imports nothing from here.
+"""
+from .binding import (  # noqa: F401
+    build,
+    gl_rule,
+    regulator,
+    table_lookup,
+    lpa,
+    loop4d_twopoint,
+    loop4d_threepoint,
+    matsubara3d,
+    num_threads,
+    set_num_threads,
+    REG_LITIM,
+    REG_EXP_POLY,
+)

@@ -1,0 +1,179 @@
+"""ctypes wrapper around oracle/dfrg_oracle.cpp (test infrastructure; see oracle/__init__.py)."""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "dfrg_oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+REG_LITIM = 0
+REG_EXP_POLY = 1
+
+_lib = None
+
+
+def build(force=False):
+    """g++ -O2 -fopenmp; no fast-math (libm exp/log, IEEE order of operations)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["g++", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c++17", "-ffp-contract=off",
+               "-o", _LIB, _SRC]
+        subprocess.check_call(cmd)
+    return _LIB
+
+
+_dp = C.POINTER(C.c_double)
+_lp = C.POINTER(C.c_longlong)
+
+
+def _d(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def _arr(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_table_lookup.restype = C.c_double
+        _lib.orc_table_lookup.argtypes = [_dp, C.c_int, C.c_double, C.c_double, C.c_int, C.c_double]
+        _lib.orc_regulator.restype = None
+        _lib.orc_regulator.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, _dp, _dp]
+        _lib.orc_gl_rule.argtypes = [C.c_int, C.c_double, C.c_double, _dp, _dp]
+        _lib.orc_lpa.argtypes = [C.c_int, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
+                                 C.c_int, C.c_int, C.c_double,
+                                 C.c_int, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp]
+        _lib.orc_loop4d_twopoint.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double,
+                                             C.c_int, _dp, _dp, C.c_int, _dp, _dp,
+                                             _dp, C.c_int, C.c_double, C.c_double, C.c_int,
+                                             _dp, C.c_int, C.c_int, _dp, C.c_int, _dp,
+                                             C.c_longlong, _lp, _dp, _dp]
+        _lib.orc_loop4d_threepoint.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double,
+                                               C.c_int, _dp, _dp, C.c_int, _dp, _dp,
+                                               C.c_int, _dp, _dp, C.c_int, _dp, _dp,
+                                               _dp, _dp, _dp, C.c_int, C.c_double, C.c_double, C.c_int,
+                                               _dp, C.c_int, C.c_int, _dp,
+                                               C.c_longlong, _lp, C.c_int, _dp, _dp]
+        _lib.orc_matsubara3d.argtypes = [C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, C.c_double,
+                                         C.c_int, _dp, _dp, C.c_int, _dp, _dp,
+                                         _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
+                                         _dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int,
+                                         C.c_longlong, _lp, _dp, _dp]
+    return _lib
+
+
+def num_threads():
+    return int(_load().orc_num_threads())
+
+
+def set_num_threads(n):
+    _load().orc_set_num_threads(int(n))
+
+
+def gl_rule(n, a, b):
+    x = np.empty(n)
+    w = np.empty(n)
+    rc = _load().orc_gl_rule(int(n), float(a), float(b), _d(x), _d(w))
+    if rc:
+        raise ValueError("orc_gl_rule: bad arguments")
+    return x, w
+
+
+def regulator(kind, order, k, s):
+    R = C.c_double()
+    Rd = C.c_double()
+    _load().orc_regulator(int(kind), int(order), float(k), float(s), C.byref(R), C.byref(Rd))
+    return R.value, Rd.value
+
+
+def table_lookup(v, lnq_lo, lnq_hi, interp, s):
+    v = _arr(v)
+    return float(_load().orc_table_lookup(_d(v), int(v.size), float(lnq_lo), float(lnq_hi), int(interp), float(s)))
+
+
+def _sel(sel):
+    if sel is None:
+        return 0, None, None
+    sel = np.ascontiguousarray(sel, dtype=np.int64)
+    return int(sel.size), sel.ctypes.data_as(_lp), sel
+
+
+def lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, xq, wq, rho, u, du):
+    """Returns (flow[n_field], chan[2, n_field], dmin[n_field])."""
+    xq, wq, rho, u, du = map(_arr, (xq, wq, rho, u, du))
+    nf = rho.size
+    flow = np.empty(nf)
+    chan = np.empty((2, nf))
+    dmin = np.empty(nf)
+    rc = _load().orc_lpa(int(d), float(T), int(n_max), int(reg_arg4d), float(N), float(prefactor),
+                         int(reg_kind), int(reg_order), float(k), int(xq.size), _d(xq), _d(wq),
+                         int(nf), _d(rho), _d(u), _d(du), _d(flow), _d(chan), _d(dmin))
+    if rc:
+        raise ValueError("orc_lpa: bad arguments")
+    return flow, chan, dmin
+
+
+def loop4d_twopoint(prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Z, lnq_lo, lnq_hi, interp,
+                    coef, m2, pext, sel=None):
+    """Returns (out, dmin): shape [n_ext, n_field], or [n_sel] for flat indices e*n_field+f in sel."""
+    xq, wq, xc, wc, Z, coef, m2, pext = map(_arr, (xq, wq, xc, wc, Z, coef, m2, pext))
+    ns, selp, _keep = _sel(sel)
+    shape = (ns,) if sel is not None else (pext.size, m2.size)
+    out = np.empty(shape)
+    dmin = np.empty(shape)
+    rc = _load().orc_loop4d_twopoint(float(prefactor), int(reg_kind), int(reg_order), float(k),
+                                     int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
+                                     _d(Z), int(Z.size), float(lnq_lo), float(lnq_hi), int(interp),
+                                     _d(coef), int(coef.size), int(m2.size), _d(m2), int(pext.size), _d(pext),
+                                     ns, selp, _d(out), _d(dmin))
+    if rc:
+        raise ValueError("orc_loop4d_twopoint: bad arguments")
+    return out, dmin
+
+
+def loop4d_threepoint(prefactor, reg_kind, reg_order, k, xq, wq, x1, w1, x2, w2, xphi, wphi,
+                      ZA, Zc, L3, lnq_lo, lnq_hi, interp, coef, ext, sel=None, literal_phi=False):
+    """ext: [n_ext, 3] = (|p1|, |p2|, alpha).  Returns (out[n_ext or n_sel], dmin)."""
+    xq, wq, x1, w1, x2, w2, xphi, wphi, ZA, Zc, L3, coef, ext = map(
+        _arr, (xq, wq, x1, w1, x2, w2, xphi, wphi, ZA, Zc, L3, coef, ext))
+    n_ext = ext.size // 3
+    ns, selp, _keep = _sel(sel)
+    n_out = ns if sel is not None else n_ext
+    out = np.empty(n_out)
+    dmin = np.empty(n_out)
+    rc = _load().orc_loop4d_threepoint(float(prefactor), int(reg_kind), int(reg_order), float(k),
+                                       int(xq.size), _d(xq), _d(wq), int(x1.size), _d(x1), _d(w1),
+                                       int(x2.size), _d(x2), _d(w2), int(xphi.size), _d(xphi), _d(wphi),
+                                       _d(ZA), _d(Zc), _d(L3), int(ZA.size), float(lnq_lo), float(lnq_hi),
+                                       int(interp), _d(coef), int(coef.size), int(n_ext), _d(ext),
+                                       ns, selp, int(bool(literal_phi)), _d(out), _d(dmin))
+    if rc:
+        raise ValueError("orc_loop4d_threepoint: bad arguments")
+    return out, dmin
+
+
+def matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zpsi, Zphi,
+                lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None):
+    """Zpsi, Zphi: [n_freq, n_q].  Returns (out, dmin): [n_p, n_jext, n_field] or [n_sel]
+    for flat indices (e*n_jext + j)*n_field + f in sel."""
+    xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext = map(
+        _arr, (xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext))
+    assert Zpsi.ndim == 2 and Zpsi.shape == Zphi.shape
+    nfreq, tnq = Zpsi.shape
+    ns, selp, _keep = _sel(sel)
+    shape = (ns,) if sel is not None else (pext.size, int(n_jext), m2psi.size)
+    out = np.empty(shape)
+    dmin = np.empty(shape)
+    rc = _load().orc_matsubara3d(float(T), int(n_max), float(prefactor), int(reg_kind), int(reg_order), float(k),
+                                 int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
+                                 _d(Zpsi), _d(Zphi), int(tnq), int(nfreq), float(lnq_lo), float(lnq_hi), int(interp),
+                                 _d(coef), int(coef.size), int(m2psi.size), _d(m2psi), _d(m2phi),
+                                 int(pext.size), _d(pext), int(n_jext), ns, selp, _d(out), _d(dmin))
+    if rc:
+        raise ValueError("orc_matsubara3d: bad arguments")
+    return out, dmin

@@ -1,0 +1,464 @@
+// dfrg_oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, double-precision CPU implementation of the momentum-loop
+// integrals on the right-hand side of fRG flow equations (the hot path of
+// arxiv 2412.13043, "DiFfRG"), written from the paper text and the workload
+// definitions of BASELINE.json / SURVEY.md section 8(c).  It exists to check
+// the CUDA library; only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may build, load or call it.  It shares
+// no code, header, table or constant with paper_2412_13043_b200/csrc.
+//
+// What it follows (PAPER.md line : passage):
+//   * fixed tensor-product quadrature "of arbitrary order", radial x angles in
+//     the vacuum, Matsubara sum in the time direction at finite T
+//     (sec. 5.3.2, integrator types Quadrature / Quadraturex0);
+//   * angle variables cos1, cos2, phi (App. F.1);
+//   * polynomial exponential regulator s_N(x) = k^2 exp(-sum_{i<=N} x^i/i)
+//     (eq. 14) and its RG-time derivative through
+//     k d/dk = -2x d/dx on the shape (Fig. 2 caption);
+//   * flat (Litim) regulator, shape (1/x - 1) Theta(1 - x);
+//   * propagator G = 1/(p^2 + m^2 + R_k) (eq. G.1);
+//   * dressing functions as tables on a logarithmic momentum grid
+//      and stacks of such tables indexed by an integer
+//     Matsubara index with no interpolation across it.
+// Everything concrete (integrands, measures, prefactors, loop order) is the
+// reading listed in DESIGN.md section "Readings".
+//
+// Style: one full integrand evaluation per quadrature node, nothing shared
+// between field points or external momenta, libm exp/log/sqrt, accumulation in
+// long double in exactly the loop order written, OpenMP only across outputs.
+//
+// Pins (tests/test_oracle_pins.py): Gauss-Legendre closed forms and
+// polynomial exactness; Litim threshold functions d=3,4; finite-T Litim
+// truncated Matsubara sum vs coth/digamma closed form; exponential-regulator
+// weight integrals; regulator derivative vs mpmath differentiation; cubic
+// interpolator exactness on cubics; p=0 identity; coefficient linearity;
+// dimensional scaling; brute-force convergence; an independent mpmath
+// restatement on tiny inputs.
+// Parity unpinned: the *readings* of config 3 and config 4 (which integrand
+// the words of BASELINE.json mean) have no value outside this text to compare
+// with; their arithmetic is pinned by the independent mpmath restatement only.
+
+#include <cmath>
+#include <cstddef>
+#include <cstdint>
+#include <limits>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+typedef long double acc_t;
+
+const double kInf = std::numeric_limits<double>::infinity();
+
+// ---- regulators: PAPER.md:192 (eq. 14), PAPER.md:178 ---------------------------------
+// kind 0: Litim      R = (k^2 - s) Theta(k^2 - s),  Rdot = 2 k^2 Theta(k^2 - s), Theta(0)=0
+// kind 1: EXP_POLY(N) R = k^2 exp(-sum_{i=1..N} x^i / i), Rdot = 2 R (1 + sum_{i=1..N} x^i)
+// s is the squared momentum, x = s/k^2, Rdot = k dR/dk.
+void regulator(int kind, int order, double k, double s, double* R, double* Rdot) {
+  const double k2 = k * k;
+  if (kind == 0) {
+    if (s < k2) { *R = k2 - s; *Rdot = 2.0 * k2; }
+    else        { *R = 0.0;    *Rdot = 0.0; }
+    return;
+  }
+  const double x = s / k2;
+  double expo = 0.0, geo = 0.0, xi = 1.0;
+  for (int i = 1; i <= order; ++i) {
+    xi *= x;
+    expo += xi / (double)i;
+    geo += xi;
+  }
+  const double r = k2 * std::exp(-expo);
+  *R = r;
+  *Rdot = 2.0 * r * (1.0 + geo);
+}
+
+// ---- log-grid table look-up: PAPER.md:1854-1880; stacks PAPER.md:1898-1905 -----------
+// v[0..n-1] sits on ln q_i = lo + i h, h = (hi - lo)/(n - 1).  The argument is the
+// SQUARED momentum s; l = log(s)/2; t = clamp((l - lo)/h, 0, n-1).
+//   interp 3: i0 = clamp(floor(t) - 1, 0, n - 4), sg = t - i0, 4-point Lagrange on 0,1,2,3
+//   interp 1: i = min(floor(t), n - 2), linear
+// Outside the grid the end value is returned (clamp-to-edge).
+double table_lookup(const double* v, int n, double lo, double hi, int interp, double s) {
+  const double h = (hi - lo) / (double)(n - 1);
+  const double l = 0.5 * std::log(s);  // s == 0 -> -inf -> clamps low
+  double t = (l - lo) / h;
+  if (!(t > 0.0)) t = 0.0;             // also catches NaN
+  if (t > (double)(n - 1)) t = (double)(n - 1);
+  if (interp == 3) {
+    int i0 = (int)std::floor(t) - 1;
+    if (i0 < 0) i0 = 0;
+    if (i0 > n - 4) i0 = n - 4;
+    const double sg = t - (double)i0;
+    const double L0 = -(sg - 1.0) * (sg - 2.0) * (sg - 3.0) / 6.0;
+    const double L1 = sg * (sg - 2.0) * (sg - 3.0) / 2.0;
+    const double L2 = -sg * (sg - 1.0) * (sg - 3.0) / 2.0;
+    const double L3 = sg * (sg - 1.0) * (sg - 2.0) / 6.0;
+    return v[i0] * L0 + v[i0 + 1] * L1 + v[i0 + 2] * L2 + v[i0 + 3] * L3;
+  }
+  int i = (int)std::floor(t);
+  if (i > n - 2) i = n - 2;
+  const double tau = t - (double)i;
+  return v[i] * (1.0 - tau) + v[i + 1] * tau;
+}
+
+inline double ipow(double x, int e) {
+  double r = 1.0;
+  for (int i = 0; i < e; ++i) r *= x;
+  return r;
+}
+
+inline double clamp0(double s) { return s > 0.0 ? s : 0.0; }  // reading A16
+
+}  // namespace
+
+extern "C" {
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+void orc_set_num_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
+// Gauss-Legendre rule GL(n;[a,b]): x_i = (b-a)/2 xi_i + (a+b)/2, w_i = (b-a)/2 om_i with
+// xi_i the roots of P_n ascending and om_i = 2/((1 - xi_i^2) P_n'(xi_i)^2).
+// Newton on the three-term recurrence (j+1)P_{j+1} = (2j+1) x P_j - j P_{j-1}, every root
+// on its own from the guess cos(pi (i - 1/4)/(n + 1/2)), all in long double.
+int orc_gl_rule(int n, double a, double b, double* x, double* w) {
+  if (n < 1 || !x || !w) return -1;
+  const long double pi = 3.141592653589793238462643383279502884L;
+  const long double half = 0.5L * ((long double)b - (long double)a);
+  const long double mid = 0.5L * ((long double)b + (long double)a);
+  for (int i = 1; i <= n; ++i) {
+    long double z = cosl(pi * ((long double)i - 0.25L) / ((long double)n + 0.5L));
+    long double dp = 1.0L;
+    for (int it = 0; it < 100; ++it) {
+      long double p0 = 1.0L, p1 = z;  // P_0, P_1
+      for (int j = 1; j < n; ++j) {
+        const long double p2 = ((2.0L * j + 1.0L) * z * p1 - (long double)j * p0) / ((long double)j + 1.0L);
+        p0 = p1;
+        p1 = p2;
+      }
+      // n == 1: p1 = z = P_1, p0 = 1 = P_0
+      dp = (long double)n * (z * p1 - p0) / (z * z - 1.0L);  // P_n'(z)
+      const long double dz = p1 / dp;
+      z -= dz;
+      if (fabsl(dz) < 2e-19L) break;
+    }
+    {  // derivative at the converged root
+      long double p0 = 1.0L, p1 = z;
+      for (int j = 1; j < n; ++j) {
+        const long double p2 = ((2.0L * j + 1.0L) * z * p1 - (long double)j * p0) / ((long double)j + 1.0L);
+        p0 = p1;
+        p1 = p2;
+      }
+      dp = (long double)n * (z * p1 - p0) / (z * z - 1.0L);
+    }
+    if (2 * i == n + 1) z = 0.0L;  // middle root of odd n is exactly 0
+    const long double om = 2.0L / ((1.0L - z * z) * dp * dp);
+    // the guess enumerates roots descending; store ascending
+    x[n - i] = (double)(mid + half * z);
+    w[n - i] = (double)(half * om);
+  }
+  return 0;
+}
+
+void orc_regulator(int kind, int order, double k, double s, double* R, double* Rdot) {
+  regulator(kind, order, k, s, R, Rdot);
+}
+
+double orc_table_lookup(const double* v, int n_q, double lnq_lo, double lnq_hi, int interp, double s) {
+  return table_lookup(v, n_q, lnq_lo, lnq_hi, interp, s);
+}
+
+// ---- LPA O(N) flow right-hand side (configs 0 and 1) ---------------------------------
+// T == 0:  I(m2) = C sum_i w_i q_i^(d-1) Rdot(q_i^2) / (q_i^2 + R(q_i^2) + m2)
+// T  > 0:  I(m2) = C T sum_{n=-n_max..n_max} sum_i w_i q_i^(d-1) Rdot(sR) / (s + R(sR) + m2),
+//          s = w_n^2 + q_i^2, w_n = 2 pi n T, sR = s if reg_arg4d else q_i^2
+// flow[f] = (N-1) I(u[f]) + I(u[f] + 2 rho[f] du[f]);  chan = [I_pi | I_sigma] (nullable);
+// dmin[f] = signed min over nodes and both channels of (denominator / k^2) (nullable).
+int orc_lpa(int d, double T, int n_max, int reg_arg4d, double N, double prefactor,
+            int reg_kind, int reg_order, double k,
+            int nq, const double* xq, const double* wq,
+            int n_field, const double* rho, const double* u, const double* du,
+            double* flow, double* chan, double* dmin) {
+  if (d < 1 || nq < 1 || n_field < 0 || T < 0 || n_max < 0 || k <= 0) return -1;
+  const double pi = 3.14159265358979323846;
+  const double k2 = k * k;
+#pragma omp parallel for schedule(static)
+  for (int f = 0; f < n_field; ++f) {
+    const double m2c[2] = {u[f], u[f] + 2.0 * rho[f] * du[f]};
+    double I[2];
+    double dm = kInf;
+    for (int ch = 0; ch < 2; ++ch) {
+      const double m2 = m2c[ch];
+      acc_t acc = 0.0L;
+      if (T == 0.0) {
+        for (int i = 0; i < nq; ++i) {
+          const double q = xq[i];
+          const double s = q * q;
+          double R, Rd;
+          regulator(reg_kind, reg_order, k, s, &R, &Rd);
+          const double D = s + R + m2;
+          if (D / k2 < dm) dm = D / k2;
+          acc += (acc_t)(wq[i] * ipow(q, d - 1) * Rd / D);
+        }
+        I[ch] = (double)((acc_t)prefactor * acc);
+      } else {
+        for (int n = -n_max; n <= n_max; ++n) {
+          const double wn = 2.0 * pi * (double)n * T;
+          for (int i = 0; i < nq; ++i) {
+            const double q = xq[i];
+            const double s = wn * wn + q * q;
+            const double sR = reg_arg4d ? s : q * q;
+            double R, Rd;
+            regulator(reg_kind, reg_order, k, sR, &R, &Rd);
+            const double D = s + R + m2;
+            if (D / k2 < dm) dm = D / k2;
+            acc += (acc_t)(wq[i] * ipow(q, d - 1) * Rd / D);
+          }
+        }
+        I[ch] = (double)((acc_t)prefactor * (acc_t)T * acc);
+      }
+    }
+    flow[f] = (N - 1.0) * I[0] + I[1];
+    if (chan) { chan[f] = I[0]; chan[n_field + f] = I[1]; }
+    if (dmin) dmin[f] = dm;
+  }
+  return 0;
+}
+
+// ---- 4-D vacuum two-point loop (config 2) --------------------------------------------
+// out[e][f] = C sum_i wq_i q_i^3 Rdot(q_i^2) G(q_i^2;f)^2
+//               sum_j wc_j sqrt(1-c_j^2) (coef0 + coef1 q_i p_e c_j / k^2) G(s_ij;f),
+// s_ij = q_i^2 + p_e^2 + 2 q_i p_e c_j,  G(s;f) = 1/(Z(sqrt s) s + R(s) + m2_f).
+// sel (nullable): flat output indices e*n_field+f to compute; out/dmin then have n_sel entries.
+int orc_loop4d_twopoint(double prefactor, int reg_kind, int reg_order, double k,
+                        int nq, const double* xq, const double* wq,
+                        int nc, const double* xc, const double* wc,
+                        const double* Zv, int Z_nq, double Z_lo, double Z_hi, int Z_interp,
+                        const double* coef, int n_coef,
+                        int n_field, const double* m2, int n_ext, const double* pext,
+                        long long n_sel, const long long* sel,
+                        double* out, double* dmin) {
+  if (n_coef != 2 || nq < 1 || nc < 1 || n_field < 1 || n_ext < 1 || k <= 0) return -1;
+  const double k2 = k * k;
+  const long long n_out = sel ? n_sel : (long long)n_ext * n_field;
+#pragma omp parallel for schedule(static)
+  for (long long o = 0; o < n_out; ++o) {
+    const long long flat = sel ? sel[o] : o;
+    const int e = (int)(flat / n_field), f = (int)(flat % n_field);
+    const double p = pext[e], mm = m2[f];
+    double dm = kInf;
+    acc_t acc_q = 0.0L;
+    for (int i = 0; i < nq; ++i) {
+      const double q = xq[i];
+      const double sq = q * q;
+      double Rq, Rdq;
+      regulator(reg_kind, reg_order, k, sq, &Rq, &Rdq);
+      const double Dq = table_lookup(Zv, Z_nq, Z_lo, Z_hi, Z_interp, sq) * sq + Rq + mm;
+      if (Dq / k2 < dm) dm = Dq / k2;
+      const double Gq = 1.0 / Dq;
+      acc_t acc_c = 0.0L;
+      for (int j = 0; j < nc; ++j) {
+        const double c = xc[j];
+        const double s = clamp0(sq + p * p + 2.0 * q * p * c);
+        double R, Rd;
+        regulator(reg_kind, reg_order, k, s, &R, &Rd);
+        const double D = table_lookup(Zv, Z_nq, Z_lo, Z_hi, Z_interp, s) * s + R + mm;
+        if (D / k2 < dm) dm = D / k2;
+        const double poly = coef[0] + coef[1] * (q * p * c / k2);
+        acc_c += (acc_t)(wc[j] * std::sqrt((1.0 - c) * (1.0 + c)) * poly / D);
+      }
+      acc_q += (acc_t)(wq[i] * q * q * q * Rdq * Gq * Gq) * acc_c;
+    }
+    out[o] = (double)((acc_t)prefactor * acc_q);
+    if (dmin) dmin[o] = dm;
+  }
+  return 0;
+}
+
+// ---- 4-D vacuum three-point vertex loop (config 3) -----------------------------------
+// ext = (|p1|, |p2|, alpha)[e];  p1 = |p1|(1,0,0,0), p2 = |p2|(cos a, sin a, 0, 0).
+// q.p1 = q|p1|c1,  q.p2 = q|p2|(cos a c1 + sin a sqrt(1-c1^2) c2),
+// s_a = |q+p1|^2, s_b = |q-p2|^2, s_c = |p1+p2|^2,  G_A(s) = 1/(Z_A(sqrt s) s + R(s)),
+// Lam = l3((p1^2+q^2+s_a)/3) l3((p2^2+q^2+s_b)/3) l3((s_c+s_a+s_b)/3)   (table argument = squared momentum),
+// P = sum_{a+b+c<=4} kap_abc (q^2/k^2)^a (q.p1/k^2)^b (q.p2/k^2)^c, a outermost, then b, then c.
+// out[e] = C sum_q w q^3 Rdot(q^2) G_A(q^2) sum_c1 w sqrt(1-c1^2) sum_c2 w sum_phi w G_A(s_a) G_A(s_b) Lam P
+// The integrand does not depend on phi; literal_phi != 0 evaluates it inside the phi loop
+// anyway (tiny inputs only), literal_phi == 0 evaluates it once and multiplies by sum_phi w.
+int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double k,
+                          int nq, const double* xq, const double* wq,
+                          int n1, const double* x1, const double* w1,
+                          int n2, const double* x2, const double* w2,
+                          int nphi, const double* xphi, const double* wphi,
+                          const double* ZA, const double* Zc, const double* L3,
+                          int t_nq, double t_lo, double t_hi, int t_interp,
+                          const double* coef, int n_coef,
+                          int n_ext, const double* ext,
+                          long long n_sel, const long long* sel, int literal_phi,
+                          double* out, double* dmin) {
+  (void)Zc;    // accepted, not used by this integrand (reading A14)
+  (void)xphi;  // the integrand has no phi dependence
+  if (n_coef != 35 || nq < 1 || n1 < 1 || n2 < 1 || nphi < 1 || n_ext < 1 || k <= 0) return -1;
+  const double k2 = k * k;
+  const long long n_out = sel ? n_sel : (long long)n_ext;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (long long o = 0; o < n_out; ++o) {
+    const long long e = sel ? sel[o] : o;
+    const double p1 = ext[3 * e], p2 = ext[3 * e + 1], al = ext[3 * e + 2];
+    const double ca = std::cos(al), sa = std::sin(al);
+    const double sc = clamp0(p1 * p1 + p2 * p2 + 2.0 * p1 * p2 * ca);
+    double dm = kInf;
+    acc_t acc_q = 0.0L;
+    for (int i = 0; i < nq; ++i) {
+      const double q = xq[i];
+      const double sq = q * q;
+      double Rq, Rdq;
+      regulator(reg_kind, reg_order, k, sq, &Rq, &Rdq);
+      const double Dq = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, sq) * sq + Rq;
+      if (Dq / k2 < dm) dm = Dq / k2;
+      acc_t acc_1 = 0.0L;
+      for (int j1 = 0; j1 < n1; ++j1) {
+        const double c1 = x1[j1];
+        const double sin1 = std::sqrt((1.0 - c1) * (1.0 + c1));
+        acc_t acc_2 = 0.0L;
+        for (int j2 = 0; j2 < n2; ++j2) {
+          const double c2 = x2[j2];
+          const double qp1 = q * p1 * c1;
+          const double qp2 = q * p2 * (ca * c1 + sa * sin1 * c2);
+          const double s_a = clamp0(sq + p1 * p1 + 2.0 * qp1);
+          const double s_b = clamp0(sq + p2 * p2 - 2.0 * qp2);
+          acc_t acc_phi = 0.0L;
+          const int nphi_eval = literal_phi ? nphi : 1;
+          double F = 0.0;
+          for (int jp = 0; jp < nphi_eval; ++jp) {
+            double Ra, Rda, Rb, Rdb;
+            regulator(reg_kind, reg_order, k, s_a, &Ra, &Rda);
+            regulator(reg_kind, reg_order, k, s_b, &Rb, &Rdb);
+            const double Da = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, s_a) * s_a + Ra;
+            const double Db = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, s_b) * s_b + Rb;
+            if (Da / k2 < dm) dm = Da / k2;
+            if (Db / k2 < dm) dm = Db / k2;
+            const double lam =
+                table_lookup(L3, t_nq, t_lo, t_hi, t_interp, (p1 * p1 + sq + s_a) / 3.0) *
+                table_lookup(L3, t_nq, t_lo, t_hi, t_interp, (p2 * p2 + sq + s_b) / 3.0) *
+                table_lookup(L3, t_nq, t_lo, t_hi, t_interp, (sc + s_a + s_b) / 3.0);
+            double P = 0.0;
+            int idx = 0;
+            for (int a = 0; a <= 4; ++a)
+              for (int b = 0; a + b <= 4; ++b)
+                for (int c = 0; a + b + c <= 4; ++c)
+                  P += coef[idx++] * ipow(sq / k2, a) * ipow(qp1 / k2, b) * ipow(qp2 / k2, c);
+            F = (1.0 / Da) * (1.0 / Db) * lam * P;
+            if (literal_phi) acc_phi += (acc_t)(wphi[jp] * F);
+          }
+          if (!literal_phi) {
+            acc_t sw = 0.0L;
+            for (int jp = 0; jp < nphi; ++jp) sw += (acc_t)wphi[jp];
+            acc_phi = sw * (acc_t)F;
+          }
+          acc_2 += (acc_t)w2[j2] * acc_phi;
+        }
+        acc_1 += (acc_t)(w1[j1] * sin1) * acc_2;
+      }
+      acc_q += (acc_t)(wq[i] * q * q * q * Rdq / Dq) * acc_1;
+    }
+    out[o] = (double)((acc_t)prefactor * acc_q);
+    if (dmin) dmin[o] = dm;
+  }
+  return 0;
+}
+
+// ---- 3-D spatial + Matsubara loop (config 4) -----------------------------------------
+// nu_n = (2n+1) pi T (fermionic, loop n = -n_max..n_max, external j = 0..n_jext-1),
+// boson line (nu_j - nu_n, p - q): m = j - n, om_m = 2 pi m T, r^2 = p^2 + q^2 - 2 p q c.
+// s_psi = nu_n^2 + q^2,  s_phi = om_m^2 + r^2
+// G_psi = 1/(Z_psi(q, nbar) s_psi + R(s_psi) + m2_psi),  nbar = n >= 0 ? n : -n-1
+// G_phi = 1/(Z_phi(r, |m|) s_phi + R(s_phi) + m2_phi)
+// P = sum_{a+b+c<=3} kap_abc y1^a y2^b y3^c, y1 = nu_n nu_j/k^2, y2 = p q c/k^2, y3 = s_psi/k^2
+// out[p][j][f] = C T sum_n sum_q w q^2 Rdot(s_psi) G_psi^2 sum_c w P G_phi
+// Tables are row-major [n_freq][n_q]; the momentum argument is the spatial one (q^2, r^2).
+int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg_order, double k,
+                    int nq, const double* xq, const double* wq,
+                    int nc, const double* xc, const double* wc,
+                    const double* Zpsi, const double* Zphi, int t_nq, int t_nfreq,
+                    double t_lo, double t_hi, int t_interp,
+                    const double* coef, int n_coef,
+                    int n_field, const double* m2psi, const double* m2phi,
+                    int n_p, const double* pext, int n_jext,
+                    long long n_sel, const long long* sel,
+                    double* out, double* dmin) {
+  if (n_coef != 20 || nq < 1 || nc < 1 || n_field < 1 || n_p < 1 || n_jext < 1 || k <= 0 || T <= 0) return -1;
+  if (n_max + 1 > t_nfreq || n_jext - 1 + n_max + 1 > t_nfreq) return -1;
+  const double pi = 3.14159265358979323846;
+  const double k2 = k * k;
+  const long long n_out = sel ? n_sel : (long long)n_p * n_jext * n_field;
+#pragma omp parallel for schedule(static)
+  for (long long o = 0; o < n_out; ++o) {
+    const long long flat = sel ? sel[o] : o;
+    const int f = (int)(flat % n_field);
+    const int j = (int)((flat / n_field) % n_jext);
+    const int e = (int)(flat / ((long long)n_field * n_jext));
+    const double p = pext[e];
+    const double nuj = (2.0 * j + 1.0) * pi * T;
+    double dm = kInf;
+    acc_t acc_n = 0.0L;
+    for (int n = -n_max; n <= n_max; ++n) {
+      const double nun = (2.0 * n + 1.0) * pi * T;
+      const int nbar = n >= 0 ? n : -n - 1;
+      const int m = j - n;
+      const int mabs = m >= 0 ? m : -m;
+      const double om = 2.0 * pi * (double)m * T;
+      for (int i = 0; i < nq; ++i) {
+        const double q = xq[i];
+        const double spsi = nun * nun + q * q;
+        double Rp, Rdp;
+        regulator(reg_kind, reg_order, k, spsi, &Rp, &Rdp);
+        const double Dpsi =
+            table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q) * spsi + Rp + m2psi[f];
+        if (Dpsi / k2 < dm) dm = Dpsi / k2;
+        const double Gpsi = 1.0 / Dpsi;
+        acc_t acc_c = 0.0L;
+        for (int jc = 0; jc < nc; ++jc) {
+          const double c = xc[jc];
+          const double r2 = clamp0(p * p + q * q - 2.0 * p * q * c);
+          const double sphi = om * om + r2;
+          double Rb, Rdb;
+          regulator(reg_kind, reg_order, k, sphi, &Rb, &Rdb);
+          const double Dphi =
+              table_lookup(Zphi + (size_t)mabs * t_nq, t_nq, t_lo, t_hi, t_interp, r2) * sphi + Rb + m2phi[f];
+          if (Dphi / k2 < dm) dm = Dphi / k2;
+          const double y1 = nun * nuj / k2, y2 = p * q * c / k2, y3 = spsi / k2;
+          double P = 0.0;
+          int idx = 0;
+          for (int a = 0; a <= 3; ++a)
+            for (int b = 0; a + b <= 3; ++b)
+              for (int cc = 0; a + b + cc <= 3; ++cc)
+                P += coef[idx++] * ipow(y1, a) * ipow(y2, b) * ipow(y3, cc);
+          acc_c += (acc_t)(wc[jc] * P / Dphi);
+        }
+        acc_n += (acc_t)(wq[i] * q * q * Rdp * Gpsi * Gpsi) * acc_c;
+      }
+    }
+    out[o] = (double)((acc_t)prefactor * (acc_t)T * acc_n);
+    if (dmin) dmin[o] = dm;
+  }
+  return 0;
+}
+
+}  // extern "C"
