@@ -1,0 +1,188 @@
+/* dfrg.h -- C ABI of the B200-native loop-integral library (FP64 only).
+ *
+ * What it computes: the momentum-loop integrals on the right-hand side of functional
+ * renormalisation group flow equations, the "momentum integration of flow kernels"
+ * of arxiv 2412.13043 (DiFfRG), sec. 5.3.2: fixed tensor-product
+ * Gauss-Legendre quadrature over a radial loop momentum and 1-3 angles in the vacuum
+ * (integrator type "Quadrature"), or over a spatial radial momentum, one angle and a
+ * truncated Matsubara sum at finite temperature (type "Quadraturex0"), of
+ *     d_t R_k  x  products of propagators G = 1/(Z s + R_k(s) + m^2)  x  dressings,
+ * with the regulator shapes of PAPER.md:190-194 (eq. 14) and PAPER.md:178 (flat),
+ * the propagator of PAPER.md:1915-1918 (eq. G.1) and dressing functions tabulated on
+ * a logarithmic momentum grid.  Where the paper's interface
+ * returns ONE integral per call (integrator.get<double>(k, args...))
+ * this library evaluates a whole batch -- every field-grid point times every external
+ * momentum -- per call.  The integrand families, measures, prefactors and loop
+ * conventions are the readings listed in DESIGN.md ("Readings").
+ *
+ * Conventions common to all entry points
+ *  - Arrays are FP64, contiguous.  In the `dfrg_integrate_*` functions every pointer inside
+ *    the descriptors and in the argument list is a CUDA DEVICE pointer on the current device,
+ *    owned by the caller; the library never allocates, frees or retains them.  In the
+ *    `dfrg_integrate_*_host` functions the same pointers are HOST pointers (pinned memory
+ *    gives asynchronous copies); the library stages them through a per-thread device arena.
+ *  - Device entry points are asynchronous: they validate on the host, enqueue on `cuda_stream`
+ *    (a cudaStream_t passed as void*, NULL = default stream) and return.  No hidden
+ *    synchronisation.  Host entry points return after the outputs have landed in host memory.
+ *  - Return value: a dfrg_status.  Nothing is written to any output on DFRG_EINVAL /
+ *    DFRG_EUNSUPPORTED.  The library never throws across the ABI and has no CPU fallback.
+ *  - Device pointers must be 8-byte aligned.  Tables and node arrays that are 16-byte aligned
+ *    with a size that is a multiple of 16 bytes are staged into shared memory with TMA bulk
+ *    copies; others with plain loads (same results).
+ *  - Numerical special cases are not errors: a vanishing or negative propagator denominator
+ *    gives whatever IEEE arithmetic gives; `dmin` reports it (signed minimum over all quadrature
+ *    nodes and all propagators of an output of denominator / k^2; reading A4 in DESIGN.md).
+ *    An exactly zero denominator yields NaN (the reciprocal is a Newton iteration on a hardware seed).
+ *  - Deterministic: fixed thread -> node mapping, fixed reduction trees, no atomics.
+ *  - Re-entrant; concurrent calls on different streams are allowed.
+ */
+#ifndef DFRG_H_
+#define DFRG_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  DFRG_OK = 0,
+  DFRG_EINVAL = -1,       /* null required pointer, non-positive size, T < 0, k <= 0, bad interp, wrong n_coef ... */
+  DFRG_EUNSUPPORTED = -2, /* sizes beyond the shared-memory budget, unsupported dimension, not an sm_100 device */
+  DFRG_ECUDA = -3,        /* CUDA runtime / launch error; see dfrg_last_cuda_error() */
+  DFRG_ENOMEM = -4        /* device arena allocation failed (host entry points only) */
+} dfrg_status;
+
+const char* dfrg_strerror(int status);  /* static string */
+int dfrg_last_cuda_error(void);         /* cudaError_t of the last DFRG_ECUDA on the calling thread */
+int dfrg_version(void);                 /* 100*major + minor */
+void dfrg_shutdown(void);               /* frees the calling thread's device arena (host entry points) */
+
+/* Regulator R_k(s), s = squared momentum, x = s/k^2; Rdot = k dR/dk (k d/dk = -2x d/dx).
+ *   DFRG_REG_LITIM:    R = (k^2 - s) Theta(k^2 - s),            Rdot = 2 k^2 Theta(k^2 - s), Theta(0) = 0
+ *   DFRG_REG_EXP_POLY: R = k^2 exp(-sum_{i=1..order} x^i / i),  Rdot = 2 R (1 + sum_{i=1..order} x^i)       (eq. 14)
+ * order in [1, 16] for EXP_POLY; ignored for LITIM. */
+typedef enum { DFRG_REG_LITIM = 0, DFRG_REG_EXP_POLY = 1 } dfrg_reg_kind;
+typedef struct {
+  int kind;
+  int order;
+  double k;
+} dfrg_regulator;
+
+/* S1 (host): Gauss-Legendre rule of order n mapped to [a, b]: x ascending, w > 0, sum w = b - a
+ * ("quadrature rules of arbitrary order").  x_host, w_host: caller-owned HOST arrays of n doubles.
+ * 1 <= n <= 4096.  Nodes and weights are correct to 1 ulp. */
+typedef enum { DFRG_RULE_GAUSS_LEGENDRE = 0 } dfrg_rule_kind;
+int dfrg_quad_nodes(int rule_kind, int n, double a, double b, double* x_host, double* w_host);
+
+typedef struct {
+  const double* x; /* nodes   [n] */
+  const double* w; /* weights [n] */
+  int n;           /* 0 = axis unused */
+} dfrg_rule;
+
+/* Dressing function tabulated on a uniform grid in ln q:
+ *   ln q_i = lnq_lo + i (lnq_hi - lnq_lo)/(n_q - 1),  v row-major [n_freq][n_q]; n_freq = 1 for 1-D tables.
+ * Evaluated at a squared momentum s through l = log(s)/2, t = clamp((l - lnq_lo)/h, 0, n_q - 1):
+ *   interp 3: 4-point Lagrange on the stencil i0..i0+3, i0 = clamp(floor(t) - 1, 0, n_q - 4)
+ *   interp 1: linear between floor(t) and floor(t)+1 (the paper's interpolators)
+ * Outside the grid the end value is returned.  The frequency index of a stacked table selects a row
+ * exactly; there is no interpolation across it. */
+typedef struct {
+  const double* v;
+  int n_q;
+  int n_freq;
+  double lnq_lo, lnq_hi;
+  int interp;
+} dfrg_table;
+
+/* ---- LPA O(N) flow right-hand side (BASELINE.json configs 0 and 1) -------------------------------------
+ *   flow[f] = (N - 1) I(u[f]) + I(u[f] + 2 rho[f] du[f])
+ *   T == 0: I(m2) = prefactor sum_i w_i q_i^(d-1) Rdot(q_i^2) / (q_i^2 + R(q_i^2) + m2)
+ *   T  > 0: I(m2) = prefactor T sum_{n=-n_max..n_max} sum_i w_i q_i^(d-1) Rdot(sR) / (s + R(sR) + m2),
+ *           s = (2 pi n T)^2 + q_i^2,  sR = s if reg_arg4d else q_i^2      (Matsubara sum)
+ * d = dimension of the radial integral (1..8): 4 in the vacuum config, 3 at finite T.
+ * flow [n_field]; chan nullable [2][n_field] = I_pi, I_sigma; dmin nullable [n_field].
+ * Limits: (n_max + 1) * q.n <= 12288. */
+typedef struct {
+  int d;
+  double T;
+  int n_max;
+  int reg_arg4d;
+  double N;
+  double prefactor;
+  dfrg_regulator reg;
+  dfrg_rule q;
+} dfrg_lpa_desc;
+
+int dfrg_integrate_lpa(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u, const double* du,
+                       double* flow, double* chan, double* dmin, void* cuda_stream);
+int dfrg_integrate_lpa_host(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u,
+                            const double* du, double* flow, double* chan, double* dmin);
+
+/* ---- 4-D vacuum loops (BASELINE.json configs 2 and 3; angles cos1, cos2, phi of PAPER.md:1837-1840) ------
+ * DFRG_LOOP_TWOPOINT (tab[0] = Z, n_coef = 2, axes q, cos1; cos2/phi unused, their measure is in prefactor):
+ *   out[e][f] = prefactor sum_i wq_i q_i^3 Rdot(q_i^2) G(q_i^2; f)^2
+ *                 sum_j wc_j sqrt(1 - c_j^2) (coef[0] + coef[1] q_i p_e c_j / k^2) G(s_ij; f)
+ *   s_ij = max(q_i^2 + p_e^2 + 2 q_i p_e c_j, 0),   G(s; f) = 1/(Z(s) s + R(s) + m2[f]);  ext = |p|[n_ext]
+ * DFRG_LOOP_THREEPOINT (tab = Z_A, Z_c, lambda3 sharing one grid, n_coef = 35, axes q, cos1, cos2, phi; n_field = 0):
+ *   ext = (|p1|, |p2|, alpha)[n_ext];  q.p1 = q |p1| c1,  q.p2 = q |p2| (cos(alpha) c1 + sin(alpha) sqrt(1-c1^2) c2)
+ *   s_a = |q + p1|^2, s_b = |q - p2|^2, s_c = |p1 + p2|^2,  G_A(s) = 1/(Z_A(s) s + R(s))
+ *   Lam = l3((p1^2+q^2+s_a)/3) l3((p2^2+q^2+s_b)/3) l3((s_c+s_a+s_b)/3)
+ *   P = sum_{a+b+c<=4} coef[idx(a,b,c)] (q^2/k^2)^a (q.p1/k^2)^b (q.p2/k^2)^c,  idx: a outermost, then b, then c, ascending
+ *   out[e] = prefactor sum_q w q^3 Rdot(q^2) G_A(q^2) sum_c1 w sqrt(1-c1^2) sum_c2 w sum_phi w  G_A(s_a) G_A(s_b) Lam P
+ *   (the integrand is phi-independent: the phi axis contributes sum_phi w; Z_c is accepted and not used.)
+ * out, dmin (nullable): [n_ext][max(n_field, 1)].
+ * Limits: two-point q.n * cos1.n <= 12288; three-point q.n * cos1.n <= 65536, every tab[i].n_q <= 1024. */
+typedef enum { DFRG_LOOP_TWOPOINT = 0, DFRG_LOOP_THREEPOINT = 1 } dfrg_loop_family;
+typedef struct {
+  int family;
+  double prefactor;
+  dfrg_regulator reg;
+  dfrg_rule q, cos1, cos2, phi;
+  dfrg_table tab[3];
+  const double* coef;
+  int n_coef;
+} dfrg_loop4d_desc;
+
+int dfrg_integrate_loop4d(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext, const double* ext,
+                          double* out, double* dmin, void* cuda_stream);
+int dfrg_integrate_loop4d_host(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext,
+                               const double* ext, double* out, double* dmin);
+
+/* ---- 3-D spatial momentum + Matsubara sum (BASELINE.json config 4; "Quadraturex0") -------
+ *   nu_n = (2n+1) pi T (loop fermion, n = -n_max..n_max; external fermion index j = 0..n_jext-1)
+ *   boson line (nu_j - nu_n, p - q): m = j - n, om_m = 2 pi m T, r^2 = max(p^2 + q^2 - 2 p q c, 0)
+ *   s_psi = nu_n^2 + q^2,  s_phi = om_m^2 + r^2
+ *   G_psi = 1/(Z_psi(q^2; row nbar) s_psi + R(s_psi) + m2_psi[f]),  nbar = n >= 0 ? n : -n-1
+ *   G_phi = 1/(Z_phi(r^2; row |m|) s_phi + R(s_phi) + m2_phi[f])
+ *   P = sum_{a+b+c<=3} coef[idx(a,b,c)] y1^a y2^b y3^c,  y1 = nu_n nu_j/k^2, y2 = p q c/k^2, y3 = s_psi/k^2   (n_coef = 20)
+ *   out[p][j][f] = prefactor T sum_n sum_q w q^2 Rdot(s_psi) G_psi^2 sum_c w P G_phi
+ * tab_psi and tab_phi share n_q, lnq_lo, lnq_hi, interp; rows needed: tab_psi.n_freq > n_max,
+ * tab_phi.n_freq > n_jext - 1 + n_max.  out, dmin (nullable): [n_p][n_jext][n_field].
+ * Limits: q.n * cos1.n <= 6144, table n_q <= 1024. */
+typedef struct {
+  double T;
+  int n_max;
+  double prefactor;
+  dfrg_regulator reg;
+  dfrg_rule q, cos1;
+  dfrg_table tab_psi, tab_phi;
+  const double* coef;
+  int n_coef;
+} dfrg_mats3d_desc;
+
+int dfrg_integrate_matsubara3d(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi, const double* m2_phi,
+                               int n_p, const double* p, int n_jext, double* out, double* dmin, void* cuda_stream);
+int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi,
+                                    const double* m2_phi, int n_p, const double* p, int n_jext, double* out,
+                                    double* dmin);
+
+/* ---- measurement aid (bench.py roofline denominator; not part of the paper's path) -----------------------
+ * Runs a register-only kernel of independent DFMA chains (n_iter x 64 DFMA per thread, one CTA of 512 threads
+ * per SM x ctas_per_sm) on cuda_stream; *flops_out (host) receives the number of FP64 flops it executes
+ * (2 per DFMA).  sink: device array of at least 1 double. */
+int dfrg_fp64_peak_probe(int n_iter, int ctas_per_sm, double* sink, double* flops_out, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DFRG_H_ */

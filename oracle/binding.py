@@ -47,23 +47,23 @@ def _load():
         _lib.orc_gl_rule.argtypes = [C.c_int, C.c_double, C.c_double, _dp, _dp]
         _lib.orc_lpa.argtypes = [C.c_int, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
                                  C.c_int, C.c_int, C.c_double,
-                                 C.c_int, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp]
+                                 C.c_int, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _dp]
         _lib.orc_loop4d_twopoint.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double,
                                              C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                              _dp, C.c_int, C.c_double, C.c_double, C.c_int,
                                              _dp, C.c_int, C.c_int, _dp, C.c_int, _dp,
-                                             C.c_longlong, _lp, _dp, _dp]
+                                             C.c_longlong, _lp, _dp, _dp, _dp]
         _lib.orc_loop4d_threepoint.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double,
                                                C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                                C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                                _dp, _dp, _dp, C.c_int, C.c_double, C.c_double, C.c_int,
                                                _dp, C.c_int, C.c_int, _dp,
-                                               C.c_longlong, _lp, C.c_int, _dp, _dp]
+                                               C.c_longlong, _lp, C.c_int, _dp, _dp, _dp]
         _lib.orc_matsubara3d.argtypes = [C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, C.c_double,
                                          C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                          _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
                                          _dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int,
-                                         C.c_longlong, _lp, _dp, _dp]
+                                         C.c_longlong, _lp, _dp, _dp, _dp]
     return _lib
 
 
@@ -103,41 +103,43 @@ def _sel(sel):
     return int(sel.size), sel.ctypes.data_as(_lp), sel
 
 
-def lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, xq, wq, rho, u, du):
-    """Returns (flow[n_field], chan[2, n_field], dmin[n_field])."""
+def lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, xq, wq, rho, u, du, want_sens=False):
+    """Returns (flow[n_field], chan[2, n_field], dmin[n_field]) (+ sens[2, n_field] if want_sens)."""
     xq, wq, rho, u, du = map(_arr, (xq, wq, rho, u, du))
     nf = rho.size
     flow = np.empty(nf)
     chan = np.empty((2, nf))
     dmin = np.empty(nf)
+    sens = np.empty((2, nf))
     rc = _load().orc_lpa(int(d), float(T), int(n_max), int(reg_arg4d), float(N), float(prefactor),
                          int(reg_kind), int(reg_order), float(k), int(xq.size), _d(xq), _d(wq),
-                         int(nf), _d(rho), _d(u), _d(du), _d(flow), _d(chan), _d(dmin))
+                         int(nf), _d(rho), _d(u), _d(du), _d(flow), _d(chan), _d(dmin), _d(sens))
     if rc:
         raise ValueError("orc_lpa: bad arguments")
-    return flow, chan, dmin
+    return (flow, chan, dmin, sens) if want_sens else (flow, chan, dmin)
 
 
 def loop4d_twopoint(prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Z, lnq_lo, lnq_hi, interp,
-                    coef, m2, pext, sel=None):
+                    coef, m2, pext, sel=None, want_sens=False):
     """Returns (out, dmin): shape [n_ext, n_field], or [n_sel] for flat indices e*n_field+f in sel."""
     xq, wq, xc, wc, Z, coef, m2, pext = map(_arr, (xq, wq, xc, wc, Z, coef, m2, pext))
     ns, selp, _keep = _sel(sel)
     shape = (ns,) if sel is not None else (pext.size, m2.size)
     out = np.empty(shape)
     dmin = np.empty(shape)
+    sens = np.empty(shape)
     rc = _load().orc_loop4d_twopoint(float(prefactor), int(reg_kind), int(reg_order), float(k),
                                      int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
                                      _d(Z), int(Z.size), float(lnq_lo), float(lnq_hi), int(interp),
                                      _d(coef), int(coef.size), int(m2.size), _d(m2), int(pext.size), _d(pext),
-                                     ns, selp, _d(out), _d(dmin))
+                                     ns, selp, _d(out), _d(dmin), _d(sens))
     if rc:
         raise ValueError("orc_loop4d_twopoint: bad arguments")
-    return out, dmin
+    return (out, dmin, sens) if want_sens else (out, dmin)
 
 
 def loop4d_threepoint(prefactor, reg_kind, reg_order, k, xq, wq, x1, w1, x2, w2, xphi, wphi,
-                      ZA, Zc, L3, lnq_lo, lnq_hi, interp, coef, ext, sel=None, literal_phi=False):
+                      ZA, Zc, L3, lnq_lo, lnq_hi, interp, coef, ext, sel=None, literal_phi=False, want_sens=False):
     """ext: [n_ext, 3] = (|p1|, |p2|, alpha).  Returns (out[n_ext or n_sel], dmin)."""
     xq, wq, x1, w1, x2, w2, xphi, wphi, ZA, Zc, L3, coef, ext = map(
         _arr, (xq, wq, x1, w1, x2, w2, xphi, wphi, ZA, Zc, L3, coef, ext))
@@ -146,19 +148,20 @@ def loop4d_threepoint(prefactor, reg_kind, reg_order, k, xq, wq, x1, w1, x2, w2,
     n_out = ns if sel is not None else n_ext
     out = np.empty(n_out)
     dmin = np.empty(n_out)
+    sens = np.empty(n_out)
     rc = _load().orc_loop4d_threepoint(float(prefactor), int(reg_kind), int(reg_order), float(k),
                                        int(xq.size), _d(xq), _d(wq), int(x1.size), _d(x1), _d(w1),
                                        int(x2.size), _d(x2), _d(w2), int(xphi.size), _d(xphi), _d(wphi),
                                        _d(ZA), _d(Zc), _d(L3), int(ZA.size), float(lnq_lo), float(lnq_hi),
                                        int(interp), _d(coef), int(coef.size), int(n_ext), _d(ext),
-                                       ns, selp, int(bool(literal_phi)), _d(out), _d(dmin))
+                                       ns, selp, int(bool(literal_phi)), _d(out), _d(dmin), _d(sens))
     if rc:
         raise ValueError("orc_loop4d_threepoint: bad arguments")
-    return out, dmin
+    return (out, dmin, sens) if want_sens else (out, dmin)
 
 
 def matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zpsi, Zphi,
-                lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None):
+                lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, want_sens=False):
     """Zpsi, Zphi: [n_freq, n_q].  Returns (out, dmin): [n_p, n_jext, n_field] or [n_sel]
     for flat indices (e*n_jext + j)*n_field + f in sel."""
     xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext = map(
@@ -169,11 +172,12 @@ def matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zps
     shape = (ns,) if sel is not None else (pext.size, int(n_jext), m2psi.size)
     out = np.empty(shape)
     dmin = np.empty(shape)
+    sens = np.empty(shape)
     rc = _load().orc_matsubara3d(float(T), int(n_max), float(prefactor), int(reg_kind), int(reg_order), float(k),
                                  int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
                                  _d(Zpsi), _d(Zphi), int(tnq), int(nfreq), float(lnq_lo), float(lnq_hi), int(interp),
                                  _d(coef), int(coef.size), int(m2psi.size), _d(m2psi), _d(m2phi),
-                                 int(pext.size), _d(pext), int(n_jext), ns, selp, _d(out), _d(dmin))
+                                 int(pext.size), _d(pext), int(n_jext), ns, selp, _d(out), _d(dmin), _d(sens))
     if rc:
         raise ValueError("orc_matsubara3d: bad arguments")
-    return out, dmin
+    return (out, dmin, sens) if want_sens else (out, dmin)

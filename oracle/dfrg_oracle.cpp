@@ -24,6 +24,12 @@
 // Everything concrete (integrands, measures, prefactors, loop order) is the
 // reading listed in DESIGN.md section "Readings".
 //
+// Every integrator also returns, per output, dmin (signed minimum over nodes and propagators of
+// denominator/k^2, reading A4) and sens: the sum over nodes of |term| -- with |P| replaced by the sum of
+// |monomials| -- times (1 + sum over propagators of (|D - m2| + |m2|)/|D| per power), i.e. the first-order
+// bound on the output's change under relative perturbations of every input of a term.  The parity tests
+// use eps*sens as the condition-aware tolerance for outputs whose denominators vanish or change sign.
+//
 // Style: one full integrand evaluation per quadrature node, nothing shared
 // between field points or external momenta, libm exp/log/sqrt, accumulation in
 // long double in exactly the loop order written, OpenMP only across outputs.
@@ -195,7 +201,7 @@ int orc_lpa(int d, double T, int n_max, int reg_arg4d, double N, double prefacto
             int reg_kind, int reg_order, double k,
             int nq, const double* xq, const double* wq,
             int n_field, const double* rho, const double* u, const double* du,
-            double* flow, double* chan, double* dmin) {
+            double* flow, double* chan, double* dmin, double* sens) {
   if (d < 1 || nq < 1 || n_field < 0 || T < 0 || n_max < 0 || k <= 0) return -1;
   const double pi = 3.14159265358979323846;
   const double k2 = k * k;
@@ -204,6 +210,7 @@ int orc_lpa(int d, double T, int n_max, int reg_arg4d, double N, double prefacto
     const double m2c[2] = {u[f], u[f] + 2.0 * rho[f] * du[f]};
     double I[2];
     double dm = kInf;
+    acc_t sn[2] = {0.0L, 0.0L};
     for (int ch = 0; ch < 2; ++ch) {
       const double m2 = m2c[ch];
       acc_t acc = 0.0L;
@@ -215,7 +222,9 @@ int orc_lpa(int d, double T, int n_max, int reg_arg4d, double N, double prefacto
           regulator(reg_kind, reg_order, k, s, &R, &Rd);
           const double D = s + R + m2;
           if (D / k2 < dm) dm = D / k2;
-          acc += (acc_t)(wq[i] * ipow(q, d - 1) * Rd / D);
+          const double term = wq[i] * ipow(q, d - 1) * Rd / D;
+          acc += (acc_t)term;
+          sn[ch] += (acc_t)(std::fabs(term) * (1.0 + (std::fabs(s + R) + std::fabs(m2)) / std::fabs(D)));
         }
         I[ch] = (double)((acc_t)prefactor * acc);
       } else {
@@ -229,7 +238,9 @@ int orc_lpa(int d, double T, int n_max, int reg_arg4d, double N, double prefacto
             regulator(reg_kind, reg_order, k, sR, &R, &Rd);
             const double D = s + R + m2;
             if (D / k2 < dm) dm = D / k2;
-            acc += (acc_t)(wq[i] * ipow(q, d - 1) * Rd / D);
+            const double term = wq[i] * ipow(q, d - 1) * Rd / D;
+            acc += (acc_t)term;
+            sn[ch] += (acc_t)(std::fabs(term) * (1.0 + (std::fabs(s + R) + std::fabs(m2)) / std::fabs(D)));
           }
         }
         I[ch] = (double)((acc_t)prefactor * (acc_t)T * acc);
@@ -238,6 +249,11 @@ int orc_lpa(int d, double T, int n_max, int reg_arg4d, double N, double prefacto
     flow[f] = (N - 1.0) * I[0] + I[1];
     if (chan) { chan[f] = I[0]; chan[n_field + f] = I[1]; }
     if (dmin) dmin[f] = dm;
+    if (sens) {
+      const acc_t sc = (acc_t)std::fabs(prefactor) * (T == 0.0 ? (acc_t)1.0 : (acc_t)T);
+      sens[f] = (double)(sc * sn[0]);
+      sens[n_field + f] = (double)(sc * sn[1]);
+    }
   }
   return 0;
 }
@@ -254,7 +270,7 @@ int orc_loop4d_twopoint(double prefactor, int reg_kind, int reg_order, double k,
                         const double* coef, int n_coef,
                         int n_field, const double* m2, int n_ext, const double* pext,
                         long long n_sel, const long long* sel,
-                        double* out, double* dmin) {
+                        double* out, double* dmin, double* sens) {
   if (n_coef != 2 || nq < 1 || nc < 1 || n_field < 1 || n_ext < 1 || k <= 0) return -1;
   const double k2 = k * k;
   const long long n_out = sel ? n_sel : (long long)n_ext * n_field;
@@ -264,7 +280,7 @@ int orc_loop4d_twopoint(double prefactor, int reg_kind, int reg_order, double k,
     const int e = (int)(flat / n_field), f = (int)(flat % n_field);
     const double p = pext[e], mm = m2[f];
     double dm = kInf;
-    acc_t acc_q = 0.0L;
+    acc_t acc_q = 0.0L, sn = 0.0L;
     for (int i = 0; i < nq; ++i) {
       const double q = xq[i];
       const double sq = q * q;
@@ -273,7 +289,8 @@ int orc_loop4d_twopoint(double prefactor, int reg_kind, int reg_order, double k,
       const double Dq = table_lookup(Zv, Z_nq, Z_lo, Z_hi, Z_interp, sq) * sq + Rq + mm;
       if (Dq / k2 < dm) dm = Dq / k2;
       const double Gq = 1.0 / Dq;
-      acc_t acc_c = 0.0L;
+      const double condq = 2.0 * (std::fabs(Dq - mm) + std::fabs(mm)) / std::fabs(Dq);
+      acc_t acc_c = 0.0L, sn_c = 0.0L;
       for (int j = 0; j < nc; ++j) {
         const double c = xc[j];
         const double s = clamp0(sq + p * p + 2.0 * q * p * c);
@@ -283,11 +300,16 @@ int orc_loop4d_twopoint(double prefactor, int reg_kind, int reg_order, double k,
         if (D / k2 < dm) dm = D / k2;
         const double poly = coef[0] + coef[1] * (q * p * c / k2);
         acc_c += (acc_t)(wc[j] * std::sqrt((1.0 - c) * (1.0 + c)) * poly / D);
+        const double apoly = std::fabs(coef[0]) + std::fabs(coef[1] * (q * p * c / k2));
+        sn_c += (acc_t)(std::fabs(wc[j] * std::sqrt((1.0 - c) * (1.0 + c)) * apoly / D) *
+                        (1.0 + condq + (std::fabs(D - mm) + std::fabs(mm)) / std::fabs(D)));
       }
       acc_q += (acc_t)(wq[i] * q * q * q * Rdq * Gq * Gq) * acc_c;
+      sn += (acc_t)std::fabs(wq[i] * q * q * q * Rdq * Gq * Gq) * sn_c;
     }
     out[o] = (double)((acc_t)prefactor * acc_q);
     if (dmin) dmin[o] = dm;
+    if (sens) sens[o] = (double)((acc_t)std::fabs(prefactor) * sn);
   }
   return 0;
 }
@@ -311,7 +333,7 @@ int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double 
                           const double* coef, int n_coef,
                           int n_ext, const double* ext,
                           long long n_sel, const long long* sel, int literal_phi,
-                          double* out, double* dmin) {
+                          double* out, double* dmin, double* sens) {
   (void)Zc;    // accepted, not used by this integrand (reading A14)
   (void)xphi;  // the integrand has no phi dependence
   if (n_coef != 35 || nq < 1 || n1 < 1 || n2 < 1 || nphi < 1 || n_ext < 1 || k <= 0) return -1;
@@ -324,7 +346,7 @@ int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double 
     const double ca = std::cos(al), sa = std::sin(al);
     const double sc = clamp0(p1 * p1 + p2 * p2 + 2.0 * p1 * p2 * ca);
     double dm = kInf;
-    acc_t acc_q = 0.0L;
+    acc_t acc_q = 0.0L, sn_q = 0.0L;
     for (int i = 0; i < nq; ++i) {
       const double q = xq[i];
       const double sq = q * q;
@@ -332,11 +354,11 @@ int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double 
       regulator(reg_kind, reg_order, k, sq, &Rq, &Rdq);
       const double Dq = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, sq) * sq + Rq;
       if (Dq / k2 < dm) dm = Dq / k2;
-      acc_t acc_1 = 0.0L;
+      acc_t acc_1 = 0.0L, sn_1 = 0.0L;
       for (int j1 = 0; j1 < n1; ++j1) {
         const double c1 = x1[j1];
         const double sin1 = std::sqrt((1.0 - c1) * (1.0 + c1));
-        acc_t acc_2 = 0.0L;
+        acc_t acc_2 = 0.0L, sn_2 = 0.0L;
         for (int j2 = 0; j2 < n2; ++j2) {
           const double c2 = x2[j2];
           const double qp1 = q * p1 * c1;
@@ -345,7 +367,7 @@ int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double 
           const double s_b = clamp0(sq + p2 * p2 - 2.0 * qp2);
           acc_t acc_phi = 0.0L;
           const int nphi_eval = literal_phi ? nphi : 1;
-          double F = 0.0;
+          double F = 0.0, Fabs = 0.0;
           for (int jp = 0; jp < nphi_eval; ++jp) {
             double Ra, Rda, Rb, Rdb;
             regulator(reg_kind, reg_order, k, s_a, &Ra, &Rda);
@@ -358,13 +380,17 @@ int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double 
                 table_lookup(L3, t_nq, t_lo, t_hi, t_interp, (p1 * p1 + sq + s_a) / 3.0) *
                 table_lookup(L3, t_nq, t_lo, t_hi, t_interp, (p2 * p2 + sq + s_b) / 3.0) *
                 table_lookup(L3, t_nq, t_lo, t_hi, t_interp, (sc + s_a + s_b) / 3.0);
-            double P = 0.0;
+            double P = 0.0, Pabs = 0.0;
             int idx = 0;
             for (int a = 0; a <= 4; ++a)
               for (int b = 0; a + b <= 4; ++b)
-                for (int c = 0; a + b + c <= 4; ++c)
-                  P += coef[idx++] * ipow(sq / k2, a) * ipow(qp1 / k2, b) * ipow(qp2 / k2, c);
+                for (int c = 0; a + b + c <= 4; ++c) {
+                  const double mono = coef[idx++] * ipow(sq / k2, a) * ipow(qp1 / k2, b) * ipow(qp2 / k2, c);
+                  P += mono;
+                  Pabs += std::fabs(mono);
+                }
             F = (1.0 / Da) * (1.0 / Db) * lam * P;
+            Fabs = std::fabs((1.0 / Da) * (1.0 / Db) * lam) * Pabs;
             if (literal_phi) acc_phi += (acc_t)(wphi[jp] * F);
           }
           if (!literal_phi) {
@@ -373,13 +399,21 @@ int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double 
             acc_phi = sw * (acc_t)F;
           }
           acc_2 += (acc_t)w2[j2] * acc_phi;
+          sn_2 += (acc_t)(w2[j2] * Fabs);
         }
         acc_1 += (acc_t)(w1[j1] * sin1) * acc_2;
+        sn_1 += (acc_t)(w1[j1] * sin1) * sn_2;
       }
       acc_q += (acc_t)(wq[i] * q * q * q * Rdq / Dq) * acc_1;
+      sn_q += (acc_t)std::fabs(wq[i] * q * q * q * Rdq / Dq) * sn_1;
     }
     out[o] = (double)((acc_t)prefactor * acc_q);
     if (dmin) dmin[o] = dm;
+    if (sens) {  // sum of |terms| with |P| replaced by the sum of |monomials|, times sum_phi w
+      acc_t sw = 0.0L;
+      for (int jp = 0; jp < nphi; ++jp) sw += (acc_t)wphi[jp];
+      sens[o] = (double)((acc_t)std::fabs(prefactor) * sw * sn_q);
+    }
   }
   return 0;
 }
@@ -402,7 +436,7 @@ int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg
                     int n_field, const double* m2psi, const double* m2phi,
                     int n_p, const double* pext, int n_jext,
                     long long n_sel, const long long* sel,
-                    double* out, double* dmin) {
+                    double* out, double* dmin, double* sens) {
   if (n_coef != 20 || nq < 1 || nc < 1 || n_field < 1 || n_p < 1 || n_jext < 1 || k <= 0 || T <= 0) return -1;
   if (n_max + 1 > t_nfreq || n_jext - 1 + n_max + 1 > t_nfreq) return -1;
   const double pi = 3.14159265358979323846;
@@ -417,7 +451,7 @@ int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg
     const double p = pext[e];
     const double nuj = (2.0 * j + 1.0) * pi * T;
     double dm = kInf;
-    acc_t acc_n = 0.0L;
+    acc_t acc_n = 0.0L, sn_n = 0.0L;
     for (int n = -n_max; n <= n_max; ++n) {
       const double nun = (2.0 * n + 1.0) * pi * T;
       const int nbar = n >= 0 ? n : -n - 1;
@@ -433,7 +467,8 @@ int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg
             table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q) * spsi + Rp + m2psi[f];
         if (Dpsi / k2 < dm) dm = Dpsi / k2;
         const double Gpsi = 1.0 / Dpsi;
-        acc_t acc_c = 0.0L;
+        const double condpsi = 2.0 * (std::fabs(Dpsi - m2psi[f]) + std::fabs(m2psi[f])) / std::fabs(Dpsi);
+        acc_t acc_c = 0.0L, sn_c = 0.0L;
         for (int jc = 0; jc < nc; ++jc) {
           const double c = xc[jc];
           const double r2 = clamp0(p * p + q * q - 2.0 * p * q * c);
@@ -444,19 +479,26 @@ int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg
               table_lookup(Zphi + (size_t)mabs * t_nq, t_nq, t_lo, t_hi, t_interp, r2) * sphi + Rb + m2phi[f];
           if (Dphi / k2 < dm) dm = Dphi / k2;
           const double y1 = nun * nuj / k2, y2 = p * q * c / k2, y3 = spsi / k2;
-          double P = 0.0;
+          double P = 0.0, Pabs = 0.0;
           int idx = 0;
           for (int a = 0; a <= 3; ++a)
             for (int b = 0; a + b <= 3; ++b)
-              for (int cc = 0; a + b + cc <= 3; ++cc)
-                P += coef[idx++] * ipow(y1, a) * ipow(y2, b) * ipow(y3, cc);
+              for (int cc = 0; a + b + cc <= 3; ++cc) {
+                const double mono = coef[idx++] * ipow(y1, a) * ipow(y2, b) * ipow(y3, cc);
+                P += mono;
+                Pabs += std::fabs(mono);
+              }
           acc_c += (acc_t)(wc[jc] * P / Dphi);
+          sn_c += (acc_t)(std::fabs(wc[jc] * Pabs / Dphi) *
+                          (1.0 + condpsi + (std::fabs(Dphi - m2phi[f]) + std::fabs(m2phi[f])) / std::fabs(Dphi)));
         }
         acc_n += (acc_t)(wq[i] * q * q * Rdp * Gpsi * Gpsi) * acc_c;
+        sn_n += (acc_t)std::fabs(wq[i] * q * q * Rdp * Gpsi * Gpsi) * sn_c;
       }
     }
     out[o] = (double)((acc_t)prefactor * (acc_t)T * acc_n);
     if (dmin) dmin[o] = dm;
+    if (sens) sens[o] = (double)((acc_t)std::fabs(prefactor) * (acc_t)T * sn_n);
   }
   return 0;
 }

@@ -1,0 +1,178 @@
+// api_common.cu -- status strings, error slot, device check, Gauss-Legendre nodes (S1, host),
+// the host-entry-point arena, and the FP64 peak probe kernel used by bench.py.
+#include <math.h>
+#include <stdint.h>
+
+#include "dfrg_internal.h"
+
+namespace dfrg {
+
+static thread_local int g_last_cuda_error = 0;
+void set_last_cuda_error(int e) { g_last_cuda_error = e; }
+
+int require_sm100(int* sm_count) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) { set_last_cuda_error((int)e); return DFRG_ECUDA; }
+  int major = 0, sms = 0;
+  e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e != cudaSuccess) { set_last_cuda_error((int)e); return DFRG_ECUDA; }
+  e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) { set_last_cuda_error((int)e); return DFRG_ECUDA; }
+  if (major != 10) return DFRG_EUNSUPPORTED;
+  if (sm_count) *sm_count = sms;
+  return DFRG_OK;
+}
+
+// ---- arena ---------------------------------------------------------------------------------------
+static size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
+
+int Arena::begin(size_t bytes_needed) {
+  status_ = DFRG_OK;
+  off_ = 0;
+  if (!stream_) {
+    cudaError_t e = cudaStreamCreateWithFlags(&stream_, cudaStreamNonBlocking);
+    if (e != cudaSuccess) { set_last_cuda_error((int)e); return status_ = DFRG_ECUDA; }
+  }
+  if (bytes_needed > cap_) {
+    if (base_) cudaFree(base_);
+    base_ = nullptr;
+    cap_ = 0;
+    const size_t want = align256(bytes_needed + (bytes_needed >> 2));
+    cudaError_t e = cudaMalloc((void**)&base_, want);
+    if (e != cudaSuccess) { set_last_cuda_error((int)e); cudaGetLastError(); return status_ = DFRG_ENOMEM; }
+    cap_ = want;
+  }
+  return DFRG_OK;
+}
+double* Arena::reserve(size_t n) {
+  const size_t b = align256(n * sizeof(double));
+  if (off_ + b > cap_) { status_ = DFRG_ENOMEM; return nullptr; }
+  double* p = (double*)(base_ + off_);
+  off_ += b;
+  return p;
+}
+double* Arena::put(const double* host, size_t n) {
+  double* p = reserve(n);
+  if (!p) return nullptr;
+  cudaError_t e = cudaMemcpyAsync(p, host, n * sizeof(double), cudaMemcpyHostToDevice, stream_);
+  if (e != cudaSuccess) { set_last_cuda_error((int)e); status_ = DFRG_ECUDA; return nullptr; }
+  return p;
+}
+int Arena::fetch(double* host, const double* dev, size_t n) {
+  cudaError_t e = cudaMemcpyAsync(host, dev, n * sizeof(double), cudaMemcpyDeviceToHost, stream_);
+  if (e != cudaSuccess) { set_last_cuda_error((int)e); return status_ = DFRG_ECUDA; }
+  return DFRG_OK;
+}
+int Arena::finish() {
+  cudaError_t e = cudaStreamSynchronize(stream_);
+  if (e != cudaSuccess) { set_last_cuda_error((int)e); return status_ = DFRG_ECUDA; }
+  return status_;
+}
+void Arena::release() {
+  if (base_) cudaFree(base_);
+  if (stream_) cudaStreamDestroy(stream_);
+  base_ = nullptr; cap_ = off_ = 0; stream_ = nullptr;
+}
+Arena& thread_arena() {
+  static thread_local Arena a;
+  return a;
+}
+
+// ---- FP64 peak probe ---------------------------------------------------------------------------
+// 8 independent DFMA chains per thread, 8 DFMA per chain per iteration: register-only, no memory.
+__global__ void __launch_bounds__(512) fp64_peak_kernel(int n_iter, double* sink) {
+  double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 0.1, a2 = a0 + 0.2, a3 = a0 + 0.3;
+  double a4 = a0 + 0.4, a5 = a0 + 0.5, a6 = a0 + 0.6, a7 = a0 + 0.7;
+  const double m = 0.999999, c = 1e-7;
+  for (int it = 0; it < n_iter; ++it) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+      a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+  }
+  const double s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  if (s == 123456.789) sink[0] = s;  // never true; keeps the chains alive
+}
+
+}  // namespace dfrg
+
+using namespace dfrg;
+
+extern "C" {
+
+const char* dfrg_strerror(int status) {
+  switch (status) {
+    case DFRG_OK: return "ok";
+    case DFRG_EINVAL: return "invalid argument";
+    case DFRG_EUNSUPPORTED: return "unsupported size, dimension or device";
+    case DFRG_ECUDA: return "CUDA runtime error (see dfrg_last_cuda_error)";
+    case DFRG_ENOMEM: return "device arena allocation failed";
+    default: return "unknown status";
+  }
+}
+int dfrg_last_cuda_error(void) { return g_last_cuda_error; }
+int dfrg_version(void) { return 100; }
+void dfrg_shutdown(void) { thread_arena().release(); }
+
+// S1: Gauss-Legendre nodes.  Half the roots from the Tricomi initial guess, Newton on P_n with the
+// three-term recurrence in long double, mirrored; derivative from P_n' = n (P_{n-1} - x P_n)/(1 - x^2).
+int dfrg_quad_nodes(int rule_kind, int n, double a, double b, double* x_host, double* w_host) {
+  if (rule_kind != DFRG_RULE_GAUSS_LEGENDRE || n < 1 || n > 4096 || !x_host || !w_host) return DFRG_EINVAL;
+  if (!(b > a) || !isfinite(a) || !isfinite(b)) return DFRG_EINVAL;
+  const long double PI_L = 3.14159265358979323846264338327950288L;
+  const long double hw = ((long double)b - (long double)a) / 2.0L, mid = ((long double)b + (long double)a) / 2.0L;
+  const int half = (n + 1) / 2;
+  const long double nn = (long double)n;
+  for (int r = 0; r < half; ++r) {  // r-th largest root
+    const long double theta = PI_L * (4.0L * r + 3.0L) / (4.0L * nn + 2.0L);
+    const long double sn = sinl(theta);
+    long double x = (1.0L - (nn - 1.0L) / (8.0L * nn * nn * nn) -
+                     (39.0L - 28.0L / (sn * sn)) / (384.0L * nn * nn * nn * nn)) * cosl(theta);
+    long double pn = 0.0L, pm = 0.0L, dpn = 1.0L;
+    for (int it = 0; it < 64; ++it) {
+      pm = 1.0L;  // P_0
+      pn = x;     // P_1
+      for (int j = 2; j <= n; ++j) {
+        const long double pj = ((2.0L * j - 1.0L) * x * pn - (j - 1.0L) * pm) / (long double)j;
+        pm = pn;
+        pn = pj;
+      }
+      if (n == 1) pm = 1.0L;
+      dpn = nn * (pm - x * pn) / ((1.0L - x) * (1.0L + x));
+      const long double step = pn / dpn;
+      x -= step;
+      if (fabsl(step) <= 4e-20L) break;
+    }
+    if (n % 2 == 1 && r == half - 1) x = 0.0L;
+    {  // P_{n-1} at the final x for the weight
+      pm = 1.0L; pn = x;
+      for (int j = 2; j <= n; ++j) {
+        const long double pj = ((2.0L * j - 1.0L) * x * pn - (j - 1.0L) * pm) / (long double)j;
+        pm = pn; pn = pj;
+      }
+      if (n == 1) pm = 1.0L;
+      dpn = nn * (pm - x * pn) / ((1.0L - x) * (1.0L + x));
+    }
+    const long double w = 2.0L / ((1.0L - x) * (1.0L + x) * dpn * dpn);
+    x_host[n - 1 - r] = (double)(mid + hw * x);
+    w_host[n - 1 - r] = (double)(hw * w);
+    x_host[r] = (double)(mid - hw * x);
+    w_host[r] = (double)(hw * w);
+  }
+  return DFRG_OK;
+}
+
+int dfrg_fp64_peak_probe(int n_iter, int ctas_per_sm, double* sink, double* flops_out, void* cuda_stream) {
+  if (n_iter < 1 || ctas_per_sm < 1 || ctas_per_sm > 4 || !sink) return DFRG_EINVAL;
+  int sms = 0;
+  int rc = require_sm100(&sms);
+  if (rc != DFRG_OK) return rc;
+  const int grid = sms * ctas_per_sm;
+  fp64_peak_kernel<<<grid, 512, 0, (cudaStream_t)cuda_stream>>>(n_iter, sink);
+  if (flops_out) *flops_out = 2.0 * 64.0 * (double)n_iter * 512.0 * (double)grid;
+  return check_cuda(cudaGetLastError());
+}
+
+}  // extern "C"

@@ -1,0 +1,57 @@
+// dfrg_internal.h -- host-side helpers shared by the C-ABI translation units (not installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+#include "../../include/dfrg.h"
+
+namespace dfrg {
+
+void set_last_cuda_error(int e);
+
+// Records the error and returns DFRG_ECUDA if e != cudaSuccess, else DFRG_OK.
+inline int check_cuda(cudaError_t e) {
+  if (e == cudaSuccess) return DFRG_OK;
+  set_last_cuda_error((int)e);
+  return DFRG_ECUDA;
+}
+
+// DFRG_EUNSUPPORTED unless the current device is compute capability 10.x.
+int require_sm100(int* sm_count);
+
+inline bool valid_regulator(const dfrg_regulator& r) {
+  if (!(r.k > 0.0)) return false;
+  if (r.kind == DFRG_REG_LITIM) return true;
+  return r.kind == DFRG_REG_EXP_POLY && r.order >= 1 && r.order <= 16;
+}
+inline bool valid_rule(const dfrg_rule& r) { return r.n >= 1 && r.x && r.w; }
+inline bool valid_table(const dfrg_table& t, int min_rows) {
+  if (!t.v || t.n_freq < min_rows || !(t.lnq_hi > t.lnq_lo)) return false;
+  if (t.interp == 3) return t.n_q >= 4;
+  if (t.interp == 1) return t.n_q >= 2;
+  return false;
+}
+
+// Per-thread device arena used by the *_host entry points: one growing cudaMalloc block plus a
+// private stream.  reset() rewinds; put() copies a host array in (async on the arena stream) and
+// returns the device address; get() reserves device space for an output.
+class Arena {
+ public:
+  int begin(size_t bytes_needed);  // DFRG_OK / DFRG_ENOMEM / DFRG_ECUDA
+  double* put(const double* host, size_t n);
+  double* reserve(size_t n);
+  int fetch(double* host, const double* dev, size_t n);  // async D2H
+  int finish();                                          // synchronise the arena stream
+  cudaStream_t stream() const { return stream_; }
+  void release();
+  int status() const { return status_; }
+
+ private:
+  char* base_ = nullptr;
+  size_t cap_ = 0, off_ = 0;
+  cudaStream_t stream_ = nullptr;
+  int status_ = DFRG_OK;
+};
+Arena& thread_arena();
+
+}  // namespace dfrg

@@ -1,0 +1,369 @@
+// loop4d.cu -- dfrg_integrate_loop4d: 4-D vacuum loops (BASELINE.json configs 2 and 3).
+//
+// Two-point family.  CTA = (external momentum p_e, tile of TP_FTILE field points).
+//   S2: nodes, weights and the Z table are staged into shared memory by TMA bulk copies.
+//   S3: the block builds, once per p_e, everything that does not depend on the field point:
+//         inner[i][j] = (D0, W'),  D0 = Z(s_ij) s_ij + R(s_ij),  W' = wc_j sqrt(1-c_j^2) (coef0 + coef1 q_i p c_j/k^2)
+//         outer[i]    = (D0q, Wq), D0q = Z(q_i^2) q_i^2 + R(q_i^2), Wq = wq_i q_i^3 Rdot(q_i^2)
+//   S4: lane = field point, warp = q-slice; per radial node the angular sum
+//         A = sum_j W'_ij / (D0_ij + m2_f) runs on four independent accumulators (add -> rcp -> FMA),
+//       then acc += Wq_i G(q_i)^2 A.  Every lane of a warp reads the same table entry (broadcast).
+//   S5: the q-slices are combined through shared memory in fixed order.
+//
+// Three-point family.  CTA = one external configuration (|p1|, |p2|, alpha); no field axis.
+//   thread = (q, c1) pairs, strided; per pair the c2-independent part (s_a, G_A(s_a), first vertex
+//   factor, the five coefficients of P as a quartic in q.p2) is hoisted out of the c2 loop.
+//   The integrand has no phi dependence: the phi axis contributes sum_phi w.  Fixed-order block sum.
+#include "dfrg_device.cuh"
+#include "dfrg_internal.h"
+
+namespace dfrg {
+
+// =====================================================================================================
+// two-point
+// =====================================================================================================
+constexpr int TP_FTILE = 128;
+constexpr int TP_SLICES = 4;
+constexpr int TP_THREADS = TP_FTILE * TP_SLICES;  // 512
+constexpr int TP_MAX_PAIRS = 12288;
+
+struct TwoPointParams {
+  int nq, nc, n_field, n_ext;
+  double prefactor;
+  RegParams reg;
+  GridParams grid;
+  const double *xq, *wq, *xc, *wc, *Z, *coef, *m2, *pext;
+  double *out, *dmin;
+};
+
+__global__ void __launch_bounds__(TP_THREADS) twopoint_kernel(const TwoPointParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t bar;
+  __shared__ double red[32];
+
+  const int nq = P.nq, nc = P.nc, npairs = nq * nc;
+  double2* inner = reinterpret_cast<double2*>(smem_raw);  // [nq*nc]
+  double2* outer = inner + npairs;                         // [nq]
+  double* sxq = reinterpret_cast<double*>(outer + nq);
+  double* swq = sxq + ((nq + 1) & ~1);
+  double* sxc = swq + ((nq + 1) & ~1);
+  double* swc = sxc + ((nc + 1) & ~1);
+  double* sZ = swc + ((nc + 1) & ~1);
+  double* part = sZ + ((P.grid.n + 1) & ~1);  // [TP_SLICES][TP_FTILE]
+
+  if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
+  __syncthreads();
+  StageList L;
+  L.add(sxq, P.xq, nq); L.add(swq, P.wq, nq);
+  L.add(sxc, P.xc, nc); L.add(swc, P.wc, nc);
+  L.add(sZ, P.Z, P.grid.n);
+  stage_to_smem(L, &bar, 0);
+
+  const double p = P.pext[blockIdx.x];
+  const double coef0 = P.coef[0], coef1 = P.coef[1];
+  const double inf = __longlong_as_double(0x7ff0000000000000LL);
+  double dmin0 = inf;
+
+  // ---- S3 ----
+  for (int t = threadIdx.x; t < npairs; t += TP_THREADS) {
+    const int i = t / nc, j = t - i * nc;
+    const double q = sxq[i], c = sxc[j];
+    double s = q * q + p * p + 2.0 * q * p * c;
+    s = s > 0.0 ? s : 0.0;
+    double R, Rd;
+    regulator(P.reg, s, R, Rd);
+    const double D0 = table_lookup(sZ, P.grid, s) * s + R;
+    const double poly = coef0 + coef1 * (q * p * c * P.reg.inv_k2);
+    inner[t] = make_double2(D0, swc[j] * sqrt((1.0 - c) * (1.0 + c)) * poly);
+    dmin0 = fmin(dmin0, D0);
+  }
+  for (int i = threadIdx.x; i < nq; i += TP_THREADS) {
+    const double q = sxq[i], s = q * q;
+    double R, Rd;
+    regulator(P.reg, s, R, Rd);
+    const double D0 = table_lookup(sZ, P.grid, s) * s + R;
+    outer[i] = make_double2(D0, swq[i] * q * q * q * Rd);
+    dmin0 = fmin(dmin0, D0);
+  }
+  dmin0 = block_min(dmin0, red);
+
+  // ---- S4 ----
+  const int lane_f = threadIdx.x % TP_FTILE, slice = threadIdx.x / TP_FTILE;
+  const int f = blockIdx.y * TP_FTILE + lane_f;
+  const bool live = f < P.n_field;
+  const double m2 = live ? P.m2[f] : 1.0;
+  double acc = 0.0;
+  for (int i = slice; i < nq; i += TP_SLICES) {
+    const double2* row = inner + i * nc;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    int j = 0;
+    for (; j + 3 < nc; j += 4) {
+      const double2 p0 = row[j], p1 = row[j + 1], p2 = row[j + 2], p3 = row[j + 3];
+      a0 = fma(p0.y, fast_rcp(p0.x + m2), a0);
+      a1 = fma(p1.y, fast_rcp(p1.x + m2), a1);
+      a2 = fma(p2.y, fast_rcp(p2.x + m2), a2);
+      a3 = fma(p3.y, fast_rcp(p3.x + m2), a3);
+    }
+    for (; j < nc; ++j) {
+      const double2 p0 = row[j];
+      a0 = fma(p0.y, fast_rcp(p0.x + m2), a0);
+    }
+    const double2 o = outer[i];
+    const double g = fast_rcp(o.x + m2);
+    acc = fma(o.y * (g * g), (a0 + a1) + (a2 + a3), acc);
+  }
+  part[slice * TP_FTILE + lane_f] = acc;
+  __syncthreads();
+
+  // ---- S5/S6 ----
+  if (slice == 0 && live) {
+    double r = part[lane_f];
+#pragma unroll
+    for (int sidx = 1; sidx < TP_SLICES; ++sidx) r += part[sidx * TP_FTILE + lane_f];
+    const size_t o = (size_t)blockIdx.x * P.n_field + f;
+    P.out[o] = P.prefactor * r;
+    if (P.dmin) P.dmin[o] = (dmin0 + m2) * P.reg.inv_k2;
+  }
+}
+
+static size_t twopoint_smem(int nq, int nc, int ntab) {
+  return (size_t)nq * nc * 16 + (size_t)nq * 16 +
+         8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((nc + 1) & ~1) + ((ntab + 1) & ~1) + TP_SLICES * TP_FTILE);
+}
+
+// =====================================================================================================
+// three-point
+// =====================================================================================================
+constexpr int T3_THREADS = 256;
+
+struct ThreePointParams {
+  int nq, n1, n2, nphi, n_ext;
+  double prefactor;
+  RegParams reg;
+  GridParams grid;
+  const double *xq, *wq, *x1, *w1, *x2, *w2, *wphi, *ZA, *L3, *coef, *ext;
+  double *out, *dmin;
+};
+
+__global__ void __launch_bounds__(T3_THREADS) threepoint_kernel(const ThreePointParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t bar;
+  __shared__ double red[32];
+
+  const int nq = P.nq, n1 = P.n1, n2 = P.n2, nt = P.grid.n;
+  double* sxq = reinterpret_cast<double*>(smem_raw);
+  double* swq = sxq + ((nq + 1) & ~1);
+  double* sx1 = swq + ((nq + 1) & ~1);
+  double* sw1 = sx1 + ((n1 + 1) & ~1);
+  double* sx2 = sw1 + ((n1 + 1) & ~1);
+  double* sw2 = sx2 + ((n2 + 1) & ~1);
+  double* sZA = sw2 + ((n2 + 1) & ~1);
+  double* sL3 = sZA + ((nt + 1) & ~1);
+  double* skap = sL3 + ((nt + 1) & ~1);  // 36
+
+  if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
+  __syncthreads();
+  {
+    StageList L;
+    L.add(sxq, P.xq, nq); L.add(swq, P.wq, nq);
+    L.add(sx1, P.x1, n1); L.add(sw1, P.w1, n1);
+    L.add(sx2, P.x2, n2); L.add(sw2, P.w2, n2);
+    L.add(sZA, P.ZA, nt); L.add(sL3, P.L3, nt);
+    stage_to_smem(L, &bar, 0);
+  }
+  if (threadIdx.x < 35) skap[threadIdx.x] = P.coef[threadIdx.x];
+  __syncthreads();
+
+  const int e = blockIdx.x;
+  const double p1 = P.ext[3 * e], p2 = P.ext[3 * e + 1], al = P.ext[3 * e + 2];
+  double sa_, ca_;
+  sincos(al, &sa_, &ca_);
+  const double ik2 = P.reg.inv_k2;
+  double scc = p1 * p1 + p2 * p2 + 2.0 * p1 * p2 * ca_;
+  scc = scc > 0.0 ? scc : 0.0;
+  const double inf = __longlong_as_double(0x7ff0000000000000LL);
+  double dm = inf;
+  double acc = 0.0;
+
+  const int npairs = nq * n1;
+  for (int t = threadIdx.x; t < npairs; t += T3_THREADS) {
+    const int i = t / n1, j1 = t - i * n1;
+    const double q = sxq[i], c1 = sx1[j1];
+    const double sq = q * q;
+    const double sin1 = sqrt((1.0 - c1) * (1.0 + c1));
+    // q-only pieces (recomputed per pair: cheap next to the c2 loop)
+    double Rq, Rdq;
+    regulator(P.reg, sq, Rq, Rdq);
+    const double Dq = table_lookup(sZA, P.grid, sq) * sq + Rq;
+    dm = fmin(dm, Dq);
+    const double wpair = (swq[i] * q * q * q * Rdq) * fast_rcp(Dq) * (sw1[j1] * sin1);
+    // (q, c1) pieces
+    const double qp1 = q * p1 * c1;
+    double s_a = sq + p1 * p1 + 2.0 * qp1;
+    s_a = s_a > 0.0 ? s_a : 0.0;
+    double Ra, Rda;
+    regulator(P.reg, s_a, Ra, Rda);
+    const double Da = table_lookup(sZA, P.grid, s_a) * s_a + Ra;
+    dm = fmin(dm, Da);
+    const double Ga = fast_rcp(Da);
+    const double lam1 = table_lookup(sL3, P.grid, (p1 * p1 + sq + s_a) * (1.0 / 3.0));
+    // P as a quartic in z = q.p2/k^2: gam[c] = sum_{a+b<=4-c} kap_abc X^a Y^b
+    const double X = sq * ik2, Y = qp1 * ik2;
+    double gam[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    {
+      int idx = 0;
+      double Xa = 1.0;
+#pragma unroll
+      for (int a = 0; a <= 4; ++a) {
+        double XaYb = Xa;
+#pragma unroll
+        for (int b = 0; b <= 4 - a; ++b) {
+#pragma unroll
+          for (int c = 0; c <= 4 - a - b; ++c) gam[c] = fma(skap[idx++], XaYb, gam[c]);
+          XaYb *= Y;
+        }
+        Xa *= X;
+      }
+    }
+    const double zc = q * p2 * ca_ * c1;       // q.p2 = zc + zs * c2
+    const double zs = q * p2 * sa_ * sin1;
+    double acc2 = 0.0;
+    for (int j2 = 0; j2 < n2; ++j2) {
+      const double qp2 = fma(zs, sx2[j2], zc);
+      double s_b = sq + p2 * p2 - 2.0 * qp2;
+      s_b = s_b > 0.0 ? s_b : 0.0;
+      double Rb, Rdb;
+      regulator(P.reg, s_b, Rb, Rdb);
+      const double Db = table_lookup(sZA, P.grid, s_b) * s_b + Rb;
+      dm = fmin(dm, Db);
+      const double lam2 = table_lookup(sL3, P.grid, (p2 * p2 + sq + s_b) * (1.0 / 3.0));
+      const double lam3 = table_lookup(sL3, P.grid, (scc + s_a + s_b) * (1.0 / 3.0));
+      const double z = qp2 * ik2;
+      const double poly = fma(fma(fma(fma(gam[4], z, gam[3]), z, gam[2]), z, gam[1]), z, gam[0]);
+      acc2 = fma(sw2[j2], fast_rcp(Db) * (lam2 * lam3) * poly, acc2);
+    }
+    acc = fma(wpair, (Ga * lam1) * acc2, acc);
+  }
+  const double total = block_sum(acc, red);
+  const double dmin_b = P.dmin ? block_min(dm, red) : 0.0;
+  if (threadIdx.x == 0) {
+    double sum_wphi = 0.0;  // the integrand has no phi dependence: the axis contributes sum_phi w
+    for (int jp = 0; jp < P.nphi; ++jp) sum_wphi += P.wphi[jp];
+    P.out[e] = P.prefactor * sum_wphi * total;
+    if (P.dmin) P.dmin[e] = dmin_b * ik2;
+  }
+}
+
+static size_t threepoint_smem(int nq, int n1, int n2, int nt) {
+  return 8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((n1 + 1) & ~1) + 2 * ((n2 + 1) & ~1) + 2 * ((nt + 1) & ~1) + 36);
+}
+
+// =====================================================================================================
+// host side
+// =====================================================================================================
+static int loop4d_validate(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext, const double* ext,
+                           double* out) {
+  if (!D || !ext || !out || n_ext < 1) return DFRG_EINVAL;
+  if (!valid_regulator(D->reg) || !valid_rule(D->q) || !valid_rule(D->cos1) || !D->coef) return DFRG_EINVAL;
+  if (D->family == DFRG_LOOP_TWOPOINT) {
+    if (n_field < 1 || !m2 || D->n_coef != 2 || !valid_table(D->tab[0], 1)) return DFRG_EINVAL;
+    if ((long long)D->q.n * D->cos1.n > TP_MAX_PAIRS || D->tab[0].n_q > 1024) return DFRG_EUNSUPPORTED;
+    if ((n_field + TP_FTILE - 1) / TP_FTILE > 65535) return DFRG_EUNSUPPORTED;
+    return DFRG_OK;
+  }
+  if (D->family == DFRG_LOOP_THREEPOINT) {
+    if (n_field != 0 || D->n_coef != 35 || !valid_rule(D->cos2) || !valid_rule(D->phi)) return DFRG_EINVAL;
+    for (int t = 0; t < 3; ++t)
+      if (!valid_table(D->tab[t], 1)) return DFRG_EINVAL;
+    for (int t = 1; t < 3; ++t)
+      if (D->tab[t].n_q != D->tab[0].n_q || D->tab[t].lnq_lo != D->tab[0].lnq_lo ||
+          D->tab[t].lnq_hi != D->tab[0].lnq_hi || D->tab[t].interp != D->tab[0].interp)
+        return DFRG_EINVAL;
+    if ((long long)D->q.n * D->cos1.n > 65536 || D->tab[0].n_q > 1024 || D->q.n > 4096 || D->cos1.n > 4096 ||
+        D->cos2.n > 4096)
+      return DFRG_EUNSUPPORTED;
+    return DFRG_OK;
+  }
+  return DFRG_EINVAL;
+}
+
+static void fill_common(const dfrg_regulator& r, const dfrg_table& t, RegParams* rp, GridParams* gp) {
+  rp->kind = r.kind; rp->order = r.order; rp->k2 = r.k * r.k; rp->inv_k2 = 1.0 / rp->k2;
+  gp->lo = t.lnq_lo; gp->inv_h = (double)(t.n_q - 1) / (t.lnq_hi - t.lnq_lo); gp->n = t.n_q; gp->interp = t.interp;
+}
+
+static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext, const double* ext,
+                         double* out, double* dmin, cudaStream_t stream) {
+  if (D->family == DFRG_LOOP_TWOPOINT) {
+    TwoPointParams P;
+    P.nq = D->q.n; P.nc = D->cos1.n; P.n_field = n_field; P.n_ext = n_ext;
+    P.prefactor = D->prefactor;
+    fill_common(D->reg, D->tab[0], &P.reg, &P.grid);
+    P.xq = D->q.x; P.wq = D->q.w; P.xc = D->cos1.x; P.wc = D->cos1.w; P.Z = D->tab[0].v;
+    P.coef = D->coef; P.m2 = m2; P.pext = ext; P.out = out; P.dmin = dmin;
+    const size_t smem = twopoint_smem(P.nq, P.nc, P.grid.n);
+    cudaError_t e = cudaFuncSetAttribute(twopoint_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return check_cuda(e);
+    dim3 grid(n_ext, (n_field + TP_FTILE - 1) / TP_FTILE);
+    twopoint_kernel<<<grid, TP_THREADS, smem, stream>>>(P);
+    return check_cuda(cudaGetLastError());
+  }
+  ThreePointParams P;
+  P.nq = D->q.n; P.n1 = D->cos1.n; P.n2 = D->cos2.n; P.nphi = D->phi.n; P.n_ext = n_ext;
+  P.prefactor = D->prefactor;
+  fill_common(D->reg, D->tab[0], &P.reg, &P.grid);
+  P.xq = D->q.x; P.wq = D->q.w; P.x1 = D->cos1.x; P.w1 = D->cos1.w; P.x2 = D->cos2.x; P.w2 = D->cos2.w; P.wphi = D->phi.w;
+  P.ZA = D->tab[0].v; P.L3 = D->tab[2].v; P.coef = D->coef; P.ext = ext; P.out = out; P.dmin = dmin;
+  const size_t smem = threepoint_smem(P.nq, P.n1, P.n2, P.grid.n);
+  cudaError_t e = cudaFuncSetAttribute(threepoint_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return check_cuda(e);
+  threepoint_kernel<<<n_ext, T3_THREADS, smem, stream>>>(P);
+  return check_cuda(cudaGetLastError());
+}
+
+}  // namespace dfrg
+
+using namespace dfrg;
+
+extern "C" int dfrg_integrate_loop4d(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext,
+                                     const double* ext, double* out, double* dmin, void* cuda_stream) {
+  int rc = loop4d_validate(D, n_field, m2, n_ext, ext, out);
+  if (rc != DFRG_OK) return rc;
+  rc = require_sm100(nullptr);
+  if (rc != DFRG_OK) return rc;
+  return loop4d_launch(D, n_field, m2, n_ext, ext, out, dmin, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int dfrg_integrate_loop4d_host(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext,
+                                          const double* ext, double* out, double* dmin) {
+  int rc = loop4d_validate(D, n_field, m2, n_ext, ext, out);
+  if (rc != DFRG_OK) return rc;
+  rc = require_sm100(nullptr);
+  if (rc != DFRG_OK) return rc;
+  Arena& A = thread_arena();
+  const bool two = D->family == DFRG_LOOP_TWOPOINT;
+  const size_t nf = two ? (size_t)n_field : 1, ne = (size_t)n_ext, next_d = two ? ne : 3 * ne;
+  size_t need = 2 * ((size_t)D->q.n + D->cos1.n + D->cos2.n + D->phi.n) + 3 * (size_t)D->tab[0].n_q + 64 + nf + next_d +
+                2 * ne * nf;
+  rc = A.begin(need * sizeof(double) + 32 * 256);
+  if (rc != DFRG_OK) return rc;
+  dfrg_loop4d_desc Dd = *D;
+  Dd.q.x = A.put(D->q.x, D->q.n); Dd.q.w = A.put(D->q.w, D->q.n);
+  Dd.cos1.x = A.put(D->cos1.x, D->cos1.n); Dd.cos1.w = A.put(D->cos1.w, D->cos1.n);
+  if (!two) {
+    Dd.cos2.x = A.put(D->cos2.x, D->cos2.n); Dd.cos2.w = A.put(D->cos2.w, D->cos2.n);
+    Dd.phi.x = A.put(D->phi.x, D->phi.n); Dd.phi.w = A.put(D->phi.w, D->phi.n);
+  }
+  for (int t = 0; t < (two ? 1 : 3); ++t) Dd.tab[t].v = A.put(D->tab[t].v, D->tab[t].n_q);
+  Dd.coef = A.put(D->coef, D->n_coef);
+  const double* d_m2 = two ? A.put(m2, nf) : nullptr;
+  const double* d_ext = A.put(ext, next_d);
+  double* d_out = A.reserve(ne * nf);
+  double* d_dmin = dmin ? A.reserve(ne * nf) : nullptr;
+  if (A.status() != DFRG_OK) return A.status();
+  rc = loop4d_launch(&Dd, n_field, d_m2, n_ext, d_ext, d_out, d_dmin, A.stream());
+  if (rc != DFRG_OK) return rc;
+  A.fetch(out, d_out, ne * nf);
+  if (dmin) A.fetch(dmin, d_dmin, ne * nf);
+  return A.finish();
+}

@@ -1,0 +1,175 @@
+// lpa.cu -- dfrg_integrate_lpa: LPA O(N) flow right-hand side (BASELINE.json configs 0, 1).
+//
+// One CTA per tile of 32 field points.  Prologue (S2/S3): the radial rule is staged into shared
+// memory with a TMA bulk copy; the block builds the field-independent table of (D0, W) pairs,
+//     D0 = s + R(sR),  W = fold * w_i q_i^(d-1) Rdot(sR),
+// over (Matsubara index n >= 0) x (radial node i); the terms are even in n, so n and -n are folded
+// (fold = 2 for n > 0).  Hot loop (S4): lane = field point, warp = (channel, node slice); every lane
+// of a warp reads the same (D0, W) pair (shared-memory broadcast) and does add -> reciprocal -> FMA
+// into four independent accumulators.  S5: fixed-order combination of the slices through shared
+// memory.  dmin needs no work in the hot loop: fl(D0 + m2) is monotone in D0, so
+// min_nodes fl(D0 + m2) = fl(min_nodes D0 + m2) exactly.
+#include "dfrg_device.cuh"
+#include "dfrg_internal.h"
+
+namespace dfrg {
+
+constexpr int LPA_THREADS = 256;   // 8 warps: 2 channels x 4 node slices
+constexpr int LPA_SLICES = 4;
+constexpr int LPA_FTILE = 32;
+constexpr int LPA_MAX_PAIRS = 12288;
+
+struct LpaParams {
+  int d, n_max, reg_arg4d, nq, n_field;
+  double T, N, prefactor;
+  RegParams reg;
+  const double *xq, *wq, *rho, *u, *du;
+  double *flow, *chan, *dmin;
+};
+
+__global__ void __launch_bounds__(LPA_THREADS) lpa_kernel(const LpaParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t bar;
+  __shared__ double red[32];
+  __shared__ double part[2][LPA_SLICES][LPA_FTILE];
+
+  const int n_terms = (P.T > 0.0) ? P.n_max + 1 : 1;
+  const int n_pairs = n_terms * P.nq;
+  double2* tab = reinterpret_cast<double2*>(smem_raw);                 // [n_pairs] (D0, W)
+  double* sx = reinterpret_cast<double*>(smem_raw + (size_t)n_pairs * 16);  // [nq]
+  double* sw = sx + ((P.nq + 1) & ~1);                                      // [nq]
+
+  if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
+  __syncthreads();
+  StageList L;
+  L.add(sx, P.xq, P.nq);
+  L.add(sw, P.wq, P.nq);
+  stage_to_smem(L, &bar, 0);
+
+  // ---- S3: field-independent table ----
+  const double two_pi_T = 2.0 * 3.14159265358979323846 * P.T;
+  double dmin0 = __longlong_as_double(0x7ff0000000000000LL);
+  for (int t = threadIdx.x; t < n_pairs; t += LPA_THREADS) {
+    const int n = t / P.nq, i = t - n * P.nq;
+    const double q = sx[i];
+    const double wn = two_pi_T * (double)n;
+    const double s = wn * wn + q * q;
+    const double sR = P.reg_arg4d ? s : q * q;
+    double R, Rd;
+    regulator(P.reg, sR, R, Rd);
+    const double D0 = s + R;
+    const double fold = (n > 0) ? 2.0 : 1.0;
+    tab[t] = make_double2(D0, fold * (sw[i] * ipow(q, P.d - 1) * Rd));
+    dmin0 = fmin(dmin0, D0);
+  }
+  dmin0 = block_min(dmin0, red);  // includes the barriers that publish tab[]
+
+  // ---- S4: hot loop ----
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int ch = wid & 1, slice = wid >> 1;
+  const int f = blockIdx.x * LPA_FTILE + lane;
+  const bool live = f < P.n_field;
+  double m2 = 1.0, m2pi = 1.0, m2sig = 1.0;
+  if (live) {
+    m2pi = P.u[f];
+    m2sig = m2pi + 2.0 * P.rho[f] * P.du[f];
+    m2 = ch ? m2sig : m2pi;
+  }
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  int t = slice;
+  for (; t + 3 * LPA_SLICES < n_pairs; t += 4 * LPA_SLICES) {
+    const double2 p0 = tab[t], p1 = tab[t + LPA_SLICES], p2 = tab[t + 2 * LPA_SLICES], p3 = tab[t + 3 * LPA_SLICES];
+    a0 = fma(p0.y, fast_rcp(p0.x + m2), a0);
+    a1 = fma(p1.y, fast_rcp(p1.x + m2), a1);
+    a2 = fma(p2.y, fast_rcp(p2.x + m2), a2);
+    a3 = fma(p3.y, fast_rcp(p3.x + m2), a3);
+  }
+  for (; t < n_pairs; t += LPA_SLICES) {
+    const double2 p0 = tab[t];
+    a0 = fma(p0.y, fast_rcp(p0.x + m2), a0);
+  }
+  part[ch][slice][lane] = (a0 + a1) + (a2 + a3);
+  __syncthreads();
+
+  // ---- S5/S6 ----
+  if (wid == 0 && live) {
+    const double scale = (P.T > 0.0) ? P.prefactor * P.T : P.prefactor;
+    double I[2];
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+      I[c] = scale * ((part[c][0][lane] + part[c][1][lane]) + (part[c][2][lane] + part[c][3][lane]));
+    P.flow[f] = (P.N - 1.0) * I[0] + I[1];
+    if (P.chan) { P.chan[f] = I[0]; P.chan[P.n_field + f] = I[1]; }
+    if (P.dmin) P.dmin[f] = fmin(dmin0 + m2pi, dmin0 + m2sig) * P.reg.inv_k2;
+  }
+}
+
+static int lpa_launch(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u, const double* du,
+                      double* flow, double* chan, double* dmin, cudaStream_t stream) {
+  LpaParams P;
+  P.d = D->d; P.n_max = D->n_max; P.reg_arg4d = D->reg_arg4d; P.nq = D->q.n; P.n_field = n_field;
+  P.T = D->T; P.N = D->N; P.prefactor = D->prefactor;
+  P.reg.kind = D->reg.kind; P.reg.order = D->reg.order;
+  P.reg.k2 = D->reg.k * D->reg.k; P.reg.inv_k2 = 1.0 / P.reg.k2;
+  P.xq = D->q.x; P.wq = D->q.w; P.rho = rho; P.u = u; P.du = du;
+  P.flow = flow; P.chan = chan; P.dmin = dmin;
+  const int n_terms = (D->T > 0.0) ? D->n_max + 1 : 1;
+  const size_t smem = (size_t)n_terms * D->q.n * 16 + 2 * (size_t)((D->q.n + 1) & ~1) * 8;
+  cudaError_t e = cudaFuncSetAttribute(lpa_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return check_cuda(e);
+  const int grid = (n_field + LPA_FTILE - 1) / LPA_FTILE;
+  lpa_kernel<<<grid, LPA_THREADS, smem, stream>>>(P);
+  return check_cuda(cudaGetLastError());
+}
+
+static int lpa_validate(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u, const double* du,
+                        double* flow) {
+  if (!D || !rho || !u || !du || !flow || n_field < 1) return DFRG_EINVAL;
+  if (!valid_regulator(D->reg) || !valid_rule(D->q)) return DFRG_EINVAL;
+  if (!(D->T >= 0.0) || D->n_max < 0 || !(D->N == D->N)) return DFRG_EINVAL;
+  if (D->d < 1 || D->d > 8) return DFRG_EUNSUPPORTED;
+  const long long n_terms = (D->T > 0.0) ? (long long)D->n_max + 1 : 1;
+  if (n_terms * D->q.n > LPA_MAX_PAIRS) return DFRG_EUNSUPPORTED;
+  return DFRG_OK;
+}
+
+}  // namespace dfrg
+
+using namespace dfrg;
+
+extern "C" int dfrg_integrate_lpa(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u,
+                                  const double* du, double* flow, double* chan, double* dmin, void* cuda_stream) {
+  int rc = lpa_validate(D, n_field, rho, u, du, flow);
+  if (rc != DFRG_OK) return rc;
+  rc = require_sm100(nullptr);
+  if (rc != DFRG_OK) return rc;
+  return lpa_launch(D, n_field, rho, u, du, flow, chan, dmin, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int dfrg_integrate_lpa_host(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u,
+                                       const double* du, double* flow, double* chan, double* dmin) {
+  int rc = lpa_validate(D, n_field, rho, u, du, flow);
+  if (rc != DFRG_OK) return rc;
+  rc = require_sm100(nullptr);
+  if (rc != DFRG_OK) return rc;
+  Arena& A = thread_arena();
+  const size_t nf = (size_t)n_field, nq = (size_t)D->q.n;
+  rc = A.begin((2 * nq + 3 * nf + 4 * nf) * sizeof(double) + 16 * 256);
+  if (rc != DFRG_OK) return rc;
+  dfrg_lpa_desc Dd = *D;
+  Dd.q.x = A.put(D->q.x, nq);
+  Dd.q.w = A.put(D->q.w, nq);
+  const double* d_rho = A.put(rho, nf);
+  const double* d_u = A.put(u, nf);
+  const double* d_du = A.put(du, nf);
+  double* d_flow = A.reserve(nf);
+  double* d_chan = chan ? A.reserve(2 * nf) : nullptr;
+  double* d_dmin = dmin ? A.reserve(nf) : nullptr;
+  if (A.status() != DFRG_OK) return A.status();
+  rc = lpa_launch(&Dd, n_field, d_rho, d_u, d_du, d_flow, d_chan, d_dmin, A.stream());
+  if (rc != DFRG_OK) return rc;
+  A.fetch(flow, d_flow, nf);
+  if (chan) A.fetch(chan, d_chan, 2 * nf);
+  if (dmin) A.fetch(dmin, d_dmin, nf);
+  return A.finish();
+}

@@ -1,0 +1,132 @@
+"""Shared test plumbing: run one workload dict (paper_2412_13043_b200.inputs) through the CPU oracle
+or through the CUDA library, and the parity criterion of DESIGN.md ("Parity bar")."""
+import numpy as np
+
+import oracle
+from paper_2412_13043_b200 import inputs  # noqa: F401
+
+REGULAR_DMIN = 1e-6      # an output is regular iff the oracle's dmin >= this (reading A4)
+RTOL = 1e-12             # north_star: relative error <= 1e-12 per output on the same nodes
+SENS_EPS = 1e-13         # condition-aware bound for singular outputs: |gpu - oracle| <= SENS_EPS * sens
+
+
+def kind_of(c):
+    n = c["name"]
+    return "lpa" if n.startswith(("cfg0", "cfg1")) else n.split("_", 1)[1]
+
+
+def make_rules(c, gen):
+    """gen(n, a, b) -> (x, w); returns {axis: (x, w)} for every rule_* entry of the workload."""
+    return {key[5:]: gen(*val) for key, val in c.items() if key.startswith("rule_")}
+
+
+def oracle_run(c, R, sel=None):
+    """-> (out, dmin, sens); lpa: out = flow[n_field], extra channels under key 'chan' are returned via dict."""
+    kd = kind_of(c)
+    if kd == "lpa":
+        flow, chan, dmin, sens = oracle.lpa(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["N"], c["prefactor"],
+                                            c["reg_kind"], c["reg_order"], c["k"], *R["q"], c["rho"], c["u"], c["du"],
+                                            want_sens=True)
+        return dict(out=flow, chan=chan, dmin=dmin, sens=(c["N"] - 1.0) * sens[0] + sens[1], sens_chan=sens)
+    if kd == "twopoint":
+        out, dmin, sens = oracle.loop4d_twopoint(c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], *R["q"], *R["c"],
+                                                 c["Z"], c["lnq_lo"], c["lnq_hi"], c["interp"], c["coef"], c["m2"],
+                                                 c["pext"], sel=sel, want_sens=True)
+    elif kd == "threepoint":
+        out, dmin, sens = oracle.loop4d_threepoint(c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], *R["q"],
+                                                   *R["c1"], *R["c2"], *R["phi"], c["ZA"], c["Zc"], c["L3"],
+                                                   c["lnq_lo"], c["lnq_hi"], c["interp"], c["coef"], c["ext"],
+                                                   sel=sel, want_sens=True)
+    else:
+        out, dmin, sens = oracle.matsubara3d(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
+                                             *R["q"], *R["c"], c["Zpsi"], c["Zphi"], c["lnq_lo"], c["lnq_hi"],
+                                             c["interp"], c["coef"], c["m2psi"], c["m2phi"], c["pext"], c["n_jext"],
+                                             sel=sel, want_sens=True)
+    return dict(out=out, dmin=dmin, sens=sens)
+
+
+def gpu_run(c, R, host=False, want_dmin=True):
+    """Runs the workload through the C ABI (device entry point on torch CUDA tensors, or the *_host entry
+    point on numpy arrays).  -> dict(out=, dmin=, [chan=]) of numpy arrays."""
+    import torch
+    from paper_2412_13043_b200 import binding as B
+
+    if host:
+        up = lambda a: np.ascontiguousarray(a, dtype=np.float64)
+        new = lambda *shape: np.full(shape, np.nan)
+        down = lambda a: a
+    else:
+        up = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+        new = lambda *shape: torch.full(shape, float("nan"), dtype=torch.float64, device="cuda")
+        down = lambda a: a.cpu().numpy()
+    rule = lambda key: (up(R[key][0]), up(R[key][1]))
+    kd = kind_of(c)
+    res = {}
+    if kd == "lpa":
+        nf = c["rho"].size
+        flow, chan, dmin = new(nf), new(2, nf), new(nf) if want_dmin else None
+        fn = B.dfrg_integrate_lpa_host if host else B.dfrg_integrate_lpa
+        fn(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["N"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
+           rule("q"), up(c["rho"]), up(c["u"]), up(c["du"]), flow, chan, dmin)
+        res = dict(out=flow, chan=chan, dmin=dmin)
+    elif kd == "twopoint":
+        out = new(c["pext"].size, c["m2"].size)
+        dmin = new(c["pext"].size, c["m2"].size) if want_dmin else None
+        fn = B.dfrg_integrate_loop4d_host if host else B.dfrg_integrate_loop4d
+        fn(B.LOOP_TWOPOINT, c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], rule("q"), rule("c"), None, None,
+           (up(c["Z"]),), c["lnq_lo"], c["lnq_hi"], c["interp"], up(c["coef"]), up(c["m2"]), up(c["pext"]), out, dmin)
+        res = dict(out=out, dmin=dmin)
+    elif kd == "threepoint":
+        ne = c["ext"].shape[0]
+        out, dmin = new(ne), new(ne) if want_dmin else None
+        fn = B.dfrg_integrate_loop4d_host if host else B.dfrg_integrate_loop4d
+        fn(B.LOOP_THREEPOINT, c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], rule("q"), rule("c1"),
+           rule("c2"), rule("phi"), (up(c["ZA"]), up(c["Zc"]), up(c["L3"])), c["lnq_lo"], c["lnq_hi"], c["interp"],
+           up(c["coef"]), None, up(c["ext"]), out, dmin)
+        res = dict(out=out, dmin=dmin)
+    else:
+        shape = (c["pext"].size, c["n_jext"], c["m2psi"].size)
+        out, dmin = new(*shape), new(*shape) if want_dmin else None
+        fn = B.dfrg_integrate_matsubara3d_host if host else B.dfrg_integrate_matsubara3d
+        fn(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], rule("q"), rule("c"),
+           up(c["Zpsi"]), up(c["Zphi"]), c["lnq_lo"], c["lnq_hi"], c["interp"], up(c["coef"]), up(c["m2psi"]),
+           up(c["m2phi"]), up(c["pext"]), c["n_jext"], out, dmin)
+        res = dict(out=out, dmin=dmin)
+    if not host:
+        torch.cuda.synchronize()
+    return {k_: (None if v is None else down(v)) for k_, v in res.items()}
+
+
+def parity_report(gpu, orc, dmin_orc, sens):
+    """Element-by-element comparison.  Regular outputs (oracle dmin >= REGULAR_DMIN): relative error.
+    Singular outputs: |diff| / sens.  Returns a dict of worst cases; assert_parity() applies the bars."""
+    gpu, orc, dmin_orc, sens = (np.asarray(a, dtype=np.float64).ravel() for a in (gpu, orc, dmin_orc, sens))
+    regular = dmin_orc >= REGULAR_DMIN
+    diff = np.abs(gpu - orc)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        rel = np.where(orc != 0, diff / np.abs(orc), np.where(diff == 0, 0.0, np.inf))
+        ratio = diff / sens
+    both_nonfinite = ~np.isfinite(gpu) & ~np.isfinite(orc)
+    rep = dict(n=gpu.size, n_regular=int(regular.sum()), n_singular=int((~regular).sum()),
+               max_rel_regular=float(rel[regular].max()) if regular.any() else 0.0,
+               max_sens_ratio_regular=float(np.nanmax(ratio[regular])) if regular.any() else 0.0,
+               max_sens_ratio_singular=float(np.nanmax(np.where(both_nonfinite, 0.0, ratio)[~regular]))
+               if (~regular).any() else 0.0,
+               n_nonfinite_gpu=int((~np.isfinite(gpu)).sum()), n_nonfinite_oracle=int((~np.isfinite(orc)).sum()))
+    rep["_rel"] = rel
+    rep["_regular"] = regular
+    return rep
+
+
+def assert_parity(gpu, orc, dmin_orc, sens, what=""):
+    rep = parity_report(gpu, orc, dmin_orc, sens)
+    msg = {k_: v for k_, v in rep.items() if not k_.startswith("_")}
+    assert rep["max_rel_regular"] <= RTOL, (what, msg)
+    assert rep["max_sens_ratio_singular"] <= SENS_EPS, (what, msg)
+    return msg
+
+
+def assert_dmin(gpu_dmin, orc_dmin, scale=1.0):
+    """dmin is a min over the same node set on both sides; the sides differ by the rounding of D0 only."""
+    g, o = np.asarray(gpu_dmin).ravel(), np.asarray(orc_dmin).ravel()
+    assert np.all(np.abs(g - o) <= 1e-12 * (scale + np.abs(o))), float(np.max(np.abs(g - o)))

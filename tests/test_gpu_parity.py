@@ -1,0 +1,201 @@
+"""GPU parity: the CUDA library (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs and the same quadrature nodes (those dfrg_quad_nodes produces).  Bars:
+regular outputs <= 1e-12 relative; outputs whose denominators vanish or change sign (oracle dmin < 1e-6):
+|gpu - oracle| <= 1e-13 * sens; closed forms <= 1e-10.  Small cases span several tiles and a ragged tail;
+full BASELINE.json sizes are compared on every output where the oracle finishes in seconds, else on a
+deterministic sample of outputs."""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_2412_13043_b200 import inputs
+
+from helpers import assert_dmin, assert_parity, gpu_run, make_rules, oracle_run
+
+pytestmark = pytest.mark.gpu
+
+PI = math.pi
+REPORT = {}
+
+
+def nodes(n, a, b):
+    from paper_2412_13043_b200 import binding as B
+    return B.dfrg_quad_nodes(n, a, b)
+
+
+def run_both(c, sel=None, what=None, check_dmin=True):
+    R = make_rules(c, nodes)
+    g = gpu_run(c, R)
+    o = oracle_run(c, R, sel=sel)
+    gout, gdm = g["out"], g["dmin"]
+    if sel is not None:
+        gout, gdm = gout.ravel()[sel], gdm.ravel()[sel]
+    rep = assert_parity(gout, o["out"], o["dmin"], o["sens"], what or c["name"])
+    if check_dmin:
+        assert_dmin(gdm, o["dmin"], scale=1.0 + float(np.max(np.abs(o["dmin"][np.isfinite(o["dmin"])]))))
+    REPORT[what or c["name"]] = rep
+    return g, o, rep
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _write_report():
+    yield
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open("gpurun_out/parity_report.json", "w") as fh:
+        json.dump(REPORT, fh, indent=1, sort_keys=True)
+
+
+# ---- LPA -------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_field,n_q", [(1, 5), (31, 8), (33, 17), (1000, 64)])
+def test_lpa_T0_small(n_field, n_q):
+    c = inputs.config0(n_field=n_field, n_q=n_q)
+    g, o, _ = run_both(c, what="lpa_T0_%d_%d" % (n_field, n_q))
+    assert_parity(g["chan"], o["chan"], np.stack([o["dmin"]] * 2), o["sens_chan"], "chan")
+
+
+@pytest.mark.parametrize("T", inputs.CONFIG1_TEMPERATURES)
+def test_lpa_finite_T_small(T):
+    c = inputs.config1(T, n_field=777, n_q=33)
+    run_both(c, what="lpa_T%g_small" % T)
+
+
+def test_lpa_litim_closed_forms_on_gpu():
+    # P2 / P3 closed forms straight against the CUDA path (<= 1e-10)
+    for d in (3, 4):
+        c = inputs.config0(n_field=513, litim=True, d=d)
+        R = make_rules(c, nodes)
+        g = gpu_run(c, R)
+        m2 = np.stack([c["u"], c["u"] + 2 * c["rho"] * c["du"]])
+        E2 = 1.0 + m2
+        ok = np.abs(E2) > 1e-3
+        ref = c["prefactor"] * 2.0 / (d * E2)
+        assert np.max(np.abs(g["chan"][ok] / ref[ok] - 1)) < 1e-10
+    import mpmath as mp
+    mp.mp.dps = 30
+    c = inputs.config1(0.1, n_field=65, litim=True)
+    R = make_rules(c, nodes)
+    g = gpu_run(c, R)
+    T, N = c["T"], c["n_max"]
+    for f in range(0, 65, 4):
+        E2 = 1.0 + c["u"][f]
+        if E2 < 1e-2:
+            continue
+        E = mp.sqrt(E2)
+        a = E / (2 * mp.pi * T)
+        S = mp.coth(E / (2 * T)) / (2 * E * T) - 2 / (2 * mp.pi * T) ** 2 * mp.im(mp.digamma(N + 1 + 1j * a)) / a
+        assert abs(g["chan"][0, f] / float(c["prefactor"] * T * (2.0 / 3) * S) - 1) < 1e-10
+
+
+def test_lpa_k_and_regulator_order():
+    c = inputs.config0(n_field=100, k=1.7)
+    run_both(c, what="lpa_k1.7")
+    c = inputs.config1(0.2, n_field=100, k=0.6)
+    c["reg_order"] = 8          # the paper's default shape s_8
+    run_both(c, what="lpa_s8")
+    c = inputs.config1(0.2, n_field=100, litim=True)
+    run_both(c, what="lpa_litim_spatial")
+
+
+def test_lpa_full_config0_and_config1():
+    run_both(inputs.config0(), what="cfg0_full")
+    for T in inputs.CONFIG1_TEMPERATURES:
+        run_both(inputs.config1(T), what="cfg1_full_T%g" % T)
+
+
+# ---- two-point --------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_field,n_ext,n_q,n_c,interp", [(1, 1, 4, 4, 3), (150, 5, 37, 7, 3), (129, 3, 40, 12, 1),
+                                                           (300, 2, 128, 32, 3)])
+def test_twopoint_small(n_field, n_ext, n_q, n_c, interp):
+    c = inputs.config2(n_field=n_field, n_ext=n_ext, n_q=n_q, n_c=n_c, interp=interp)
+    run_both(c, what="twopoint_%d_%d_%d_%d_i%d" % (n_field, n_ext, n_q, n_c, interp))
+
+
+def test_twopoint_p0_identity_and_edge_momenta():
+    # P7 on the GPU: p = 0 collapses the angular sum; very large p pushes |q+p| off the table (clamp high)
+    c = inputs.config2(n_field=64, n_ext=3)
+    c["pext"] = np.array([0.0, 1e-3, 5e2])
+    g, o, _ = run_both(c, what="twopoint_edges")
+    c["m2"] = np.abs(c["m2"]) + 0.1
+    R = make_rules(c, nodes)
+    g = gpu_run(c, R)
+    xq, wq = R["q"]
+    xc, wc = R["c"]
+    Sc = float(np.sum(wc * np.sqrt((1 - xc) * (1 + xc))))
+    import oracle
+    Zq = np.array([oracle.table_lookup(c["Z"], c["lnq_lo"], c["lnq_hi"], 3, q * q) for q in xq])
+    Rq = np.exp(-xq ** 2)
+    G = 1.0 / (Zq[None, :] * xq[None, :] ** 2 + Rq[None, :] + c["m2"][:, None])
+    ref = c["prefactor"] * Sc * np.sum(wq * xq ** 3 * 2 * Rq * (1 + xq ** 2) * G ** 3, axis=1)
+    assert np.max(np.abs(g["out"][0] / ref - 1)) < 1e-12
+
+
+def test_twopoint_full_config2():
+    g, o, rep = run_both(inputs.config2(), what="cfg2_full")
+    assert rep["n"] == 16384
+
+
+# ---- three-point ------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_p,n_alpha,n_q,n1,n2,interp", [(1, 1, 3, 3, 2, 3), (3, 2, 20, 10, 6, 3), (2, 3, 33, 9, 5, 1)])
+def test_threepoint_small(n_p, n_alpha, n_q, n1, n2, interp):
+    c = inputs.config3(n_p=n_p, n_alpha=n_alpha, n_q=n_q, n_c1=n1, n_c2=n2, n_phi=5, interp=interp)
+    run_both(c, what="threepoint_%d_%d_%d_%d_%d_i%d" % (n_p, n_alpha, n_q, n1, n2, interp))
+
+
+def test_threepoint_full_config3_sampled():
+    c = inputs.config3()
+    sel = np.arange(0, 8192, 131)                        # 63 outputs spread over (|p1|, |p2|, alpha)
+    g, o, rep = run_both(c, sel=sel, what="cfg3_full_sampled")
+    assert g["out"].shape == (8192,) and np.all(np.isfinite(g["out"]))
+
+
+# ---- Matsubara --------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_field,n_p,n_jext,n_q,n_c,n_max,interp", [(1, 1, 1, 3, 2, 0, 3), (100, 3, 3, 24, 8, 3, 3),
+                                                                      (300, 2, 2, 17, 5, 2, 3), (600, 1, 2, 12, 6, 1, 1)])
+def test_matsubara_small(n_field, n_p, n_jext, n_q, n_c, n_max, interp):
+    c = inputs.config4(n_field=n_field, n_p=n_p, n_jext=n_jext, n_q=n_q, n_c=n_c, interp=interp)
+    c["n_max"] = n_max
+    run_both(c, what="mats_%d_%d_%d_%d_%d_%d_i%d" % (n_field, n_p, n_jext, n_q, n_c, n_max, interp))
+
+
+def test_matsubara_full_config4_sampled():
+    c = inputs.config4()
+    n_out = 64 * 16 * 512
+    sel = np.arange(0, n_out, 257)                        # 2041 outputs, all (p, j, f) residues
+    g, o, rep = run_both(c, sel=sel, what="cfg4_full_sampled")
+    assert g["out"].shape == (64, 16, 512)
+
+
+# ---- ABI behaviour ----------------------------------------------------------------------------------
+def test_host_entry_points_match_device_entry_points_bitwise():
+    for c in (inputs.config0(n_field=100), inputs.config1(0.2, n_field=100),
+              inputs.config2(n_field=140, n_ext=3, n_q=24, n_c=8),
+              inputs.config3(n_p=2, n_alpha=2, n_q=12, n_c1=6, n_c2=4),
+              inputs.config4(n_field=70, n_p=2, n_jext=2, n_q=12, n_c=6)):
+        R = make_rules(c, nodes)
+        d = gpu_run(c, R)
+        h = gpu_run(c, R, host=True)
+        for key in d:
+            assert np.array_equal(d[key], h[key], equal_nan=True), (c["name"], key)
+
+
+def test_deterministic_and_dmin_optional():
+    c = inputs.config4(n_field=300, n_p=2, n_jext=2, n_q=17, n_c=5)
+    R = make_rules(c, nodes)
+    a = gpu_run(c, R)
+    b = gpu_run(c, R)
+    n = gpu_run(c, R, want_dmin=False)
+    assert np.array_equal(a["out"], b["out"]) and np.array_equal(a["out"], n["out"]) and n["dmin"] is None
+
+
+def test_runs_on_a_side_stream():
+    import torch
+    c = inputs.config2(n_field=64, n_ext=2, n_q=16, n_c=8)
+    R = make_rules(c, nodes)
+    ref = gpu_run(c, R)["out"]
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        out = gpu_run(c, R)["out"]
+    assert np.array_equal(ref, out)
