@@ -1,0 +1,367 @@
+#!/usr/bin/env python
+"""bench.py -- measures the loop-integral hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-others]
+
+A step is one pass of the whole hot path (S1..S6) over one batch: BASELINE.json configs[4], the
+finite-T momentum-dependent loop (64 p x 16 Matsubara indices x 512 field points = 524 288 integrals,
+52 992 quadrature nodes each), the largest single-GPU configuration.  `value` = nominal integrand
+evaluations per second with inputs resident in HBM; `e2e` = the same through the host-buffer C-ABI
+call (node generation + H2D + kernel + D2H in the timed region).  One JSON line on stdout.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+sys.path.insert(0, os.path.join(ROOT, "tests"))
+
+METRIC = "fp64_integrand_evals_per_s"
+UNIT = "evals/s"
+WORKLOAD = "cfg4_matsubara3d: 64 p x 16 j x 512 field points, 23 Matsubara terms x 96 q x 24 cos nodes, FP64"
+
+# FP64 roofline denominator: 148 SMs x 64 FP64 lanes x 2 flop/DFMA x 1.965 GHz
+FP64_LANES_PER_SM = 64
+
+
+def cfg4_counts(c, rules):
+    n_out = c["pext"].size * c["n_jext"] * c["m2psi"].size
+    n_terms = 2 * c["n_max"] + 1
+    nq, nc = rules["q"][0].size, rules["c"][0].size
+    evals = n_out * n_terms * nq * nc
+    # algorithmic FP64 work: per nominal evaluation add + reciprocal (3 FMA) + FMA = 9 flop in
+    # 5 instructions; per (output, n, q) the fermion line add + reciprocal + 2 mul + FMA = 11 flop in 7.
+    flops = n_out * n_terms * nq * (9 * nc + 11)
+    return n_out, evals, flops
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        self.p.wait()
+        self.f.flush()
+        self.f.seek(0)
+        rows = [r.split(",") for r in self.f.read().strip().splitlines() if r.count(",") >= 6]
+        os.unlink(self.f.name)
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [nm for i, nm in enumerate(names) if any("Active" in r[3 + i] and "Not" not in r[3 + i] for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "samples": len(rows),
+                "power_w_max": max(float(r[2]) for r in rows), "reasons": reasons}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands on the host cores, a bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    from helpers import make_rules, oracle_run
+    from paper_2412_13043_b200 import inputs
+    c = inputs.config4()
+    R = make_rules(c, oracle.gl_rule)
+    n_out, evals, _ = cfg4_counts(c, R)
+    stride = 512
+    sel = np.arange(0, n_out, stride)                       # 1024 outputs per step
+    per_out = evals // n_out
+    for _ in range(args.warmup):
+        oracle_run(c, R, sel=sel[:64])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_run(c, R, sel=sel)
+    dt = (time.perf_counter() - t0) / args.steps
+    val = sel.size * per_out / dt
+    cores = oracle.num_threads()
+    sample = "%d of %d outputs per step (every %dth), %d nodes each" % (sel.size, n_out, stride, per_out)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "integrals_per_s": sel.size / dt}
+    print(json.dumps(line))
+    return 0
+
+
+def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
+    """Device-resident timings of configs 0-3 (context for the flagship loop4d kernels; not the bench line)."""
+    out = {}
+
+    def timeit(fn, n=iters):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(n):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            b.synchronize()
+            ts.append(a.elapsed_time(b))
+        return float(np.median(ts))
+
+    up = lambda a: torch.as_tensor(np.ascontiguousarray(a)).cuda()
+    # cfg0 / cfg1
+    for name, cs in (("cfg0", [inputs.config0()]), ("cfg1", [inputs.config1(T) for T in inputs.CONFIG1_TEMPERATURES])):
+        calls, evals, integrals = [], 0, 0
+        for c in cs:
+            R = make_rules(c, B.dfrg_quad_nodes)
+            rq = (up(R["q"][0]), up(R["q"][1]))
+            rho, u, du = up(c["rho"]), up(c["u"]), up(c["du"])
+            flow = torch.empty_like(rho)
+            calls.append((c, rq, rho, u, du, flow))
+            terms = (2 * c["n_max"] + 1) if c["T"] > 0 else 1
+            evals += 2 * rho.numel() * terms * rq[0].numel()
+            integrals += 2 * rho.numel()
+
+        def fn():
+            for c, rq, rho, u, du, flow in calls:
+                B.dfrg_integrate_lpa(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["N"], c["prefactor"], c["reg_kind"],
+                                     c["reg_order"], c["k"], rq, rho, u, du, flow)
+        ms = timeit(fn)
+        out[name] = {"ms": ms, "evals_per_s": evals / ms * 1e3, "integrals_per_s": integrals / ms * 1e3,
+                     "launches": len(calls)}
+    # cfg2
+    c = inputs.config2()
+    R = make_rules(c, B.dfrg_quad_nodes)
+    rq, rc = (up(R["q"][0]), up(R["q"][1])), (up(R["c"][0]), up(R["c"][1]))
+    Z, coef, m2, pext = up(c["Z"]), up(c["coef"]), up(c["m2"]), up(c["pext"])
+    o2 = torch.empty(pext.numel(), m2.numel(), dtype=torch.float64, device="cuda")
+    ms = timeit(lambda: B.dfrg_integrate_loop4d(B.LOOP_TWOPOINT, c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
+                                                rq, rc, None, None, (Z,), c["lnq_lo"], c["lnq_hi"], c["interp"], coef,
+                                                m2, pext, o2))
+    ev = o2.numel() * rq[0].numel() * rc[0].numel()
+    fl = o2.numel() * rq[0].numel() * (9 * rc[0].numel() + 11)
+    out["cfg2"] = {"ms": ms, "evals_per_s": ev / ms * 1e3, "integrals_per_s": o2.numel() / ms * 1e3,
+                   "alg_tflops": fl / ms * 1e-9, "launches": 1}
+    # cfg3
+    c = inputs.config3()
+    R = make_rules(c, B.dfrg_quad_nodes)
+    rr = {k_: (up(v[0]), up(v[1])) for k_, v in R.items()}
+    tabs = (up(c["ZA"]), up(c["Zc"]), up(c["L3"]))
+    coef, ext = up(c["coef"]), up(c["ext"])
+    o3 = torch.empty(ext.shape[0], dtype=torch.float64, device="cuda")
+    ms = timeit(lambda: B.dfrg_integrate_loop4d(B.LOOP_THREEPOINT, c["prefactor"], c["reg_kind"], c["reg_order"],
+                                                c["k"], rr["q"], rr["c1"], rr["c2"], rr["phi"], tabs, c["lnq_lo"],
+                                                c["lnq_hi"], c["interp"], coef, None, ext, o3), n=3)
+    uniq = o3.numel() * rr["q"][0].numel() * rr["c1"][0].numel() * rr["c2"][0].numel()
+    out["cfg3"] = {"ms": ms, "unique_evals_per_s": uniq / ms * 1e3,
+                   "nominal_evals_per_s": uniq * rr["phi"][0].numel() / ms * 1e3,
+                   "integrals_per_s": o3.numel() / ms * 1e3, "launches": 1}
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-others", action="store_true", help="skip the context timings of configs 0-3")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from helpers import make_rules, oracle_run
+    from paper_2412_13043_b200 import binding as B
+    from paper_2412_13043_b200 import inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.lib()  # fail loudly if libdfrg.so is missing
+
+    # ---- workload (weak scaling: every rank integrates its own full batch; no data-path collective) ----
+    c = inputs.config4()
+    t_s1 = time.perf_counter()
+    R = make_rules(c, B.dfrg_quad_nodes)                     # S1, host
+    t_s1 = time.perf_counter() - t_s1
+    n_out, evals, flops = cfg4_counts(c, R)
+    up = lambda a: torch.as_tensor(np.ascontiguousarray(a)).cuda()
+    rq, rc = (up(R["q"][0]), up(R["q"][1])), (up(R["c"][0]), up(R["c"][1]))
+    Zpsi, Zphi, coef = up(c["Zpsi"]), up(c["Zphi"]), up(c["coef"])
+    m2psi, m2phi, pext = up(c["m2psi"]), up(c["m2phi"]), up(c["pext"])
+    out = torch.empty(pext.numel(), c["n_jext"], m2psi.numel(), dtype=torch.float64, device="cuda")
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def step():
+        B.dfrg_integrate_matsubara3d(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], rq, rc,
+                                     Zpsi, Zphi, c["lnq_lo"], c["lnq_hi"], c["interp"], coef, m2psi, m2phi, pext,
+                                     c["n_jext"], out)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- FP64 peak probe (register-only DFMA chains), before the timed region ----
+    sink = torch.zeros(8, dtype=torch.float64, device="cuda")
+    B.dfrg_fp64_peak_probe(2000, 2, sink)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    probe_flops = B.dfrg_fp64_peak_probe(40000, 2, sink)
+    b.record()
+    b.synchronize()
+    probe_tflops = probe_flops / (a.elapsed_time(b) * 1e-3) * 1e-12
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    evs = []
+    barrier()
+    t_wall = time.perf_counter()
+    for _ in range(args.steps):
+        flush.fill_(1)                                        # L2 flush between timed iterations (not timed)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        step()
+        e1.record()
+        evs.append((e0, e1))
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    clocks = sampler.stop()
+    ms_local = sum(e0.elapsed_time(e1) for e0, e1 in evs) / args.steps
+    ms = ms_local
+    if dist is not None:
+        t = torch.tensor([ms_local], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * evals / (ms * 1e-3)
+
+    # ---- e2e: host buffers through the C ABI, S1 + H2D + kernel + D2H inside the timed region ----
+    pin = lambda a: torch.as_tensor(np.ascontiguousarray(a)).pin_memory()
+    h = {k_: pin(c[k_]) for k_ in ("Zpsi", "Zphi", "coef", "m2psi", "m2phi", "pext")}
+    h_out = torch.empty(out.shape, dtype=torch.float64).pin_memory()
+    hx = {ax: (torch.empty(R[ax][0].size, dtype=torch.float64).pin_memory(),
+               torch.empty(R[ax][0].size, dtype=torch.float64).pin_memory()) for ax in ("q", "c")}
+
+    def e2e_step():
+        for ax in ("q", "c"):                                  # S1 on the host, into pinned buffers
+            n_, a_, b_ = c["rule_" + ax]
+            rc_ = B.lib().dfrg_quad_nodes(0, n_, a_, b_, hx[ax][0].data_ptr(), hx[ax][1].data_ptr())
+            assert rc_ == 0
+        B.dfrg_integrate_matsubara3d_host(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
+                                          hx["q"], hx["c"], h["Zpsi"], h["Zphi"], c["lnq_lo"], c["lnq_hi"], c["interp"],
+                                          h["coef"], h["m2psi"], h["m2phi"], h["pext"], c["n_jext"], h_out)
+    e2e_steps = max(3, min(args.steps, 10))
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    rows_psi, rows_phi = c["n_max"] + 1, c["n_jext"] + c["n_max"]
+    h2d = 8 * (2 * (R["q"][0].size + R["c"][0].size) + (rows_psi + rows_phi) * c["Zpsi"].shape[1] + 20 +
+               2 * c["m2psi"].size + c["pext"].size)
+    d2h = 8 * n_out
+    assert torch.equal(h_out.cuda(), out), "host and device entry points disagree"
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    sm_max_mhz = clocks.get("sm_max_mhz") or 1965.0
+    sms = torch.cuda.get_device_properties(local).multi_processor_count
+    peak = sms * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 * 1e-12          # TFLOP/s at max clock
+    achieved = flops / (ms_local * 1e-3) * 1e-12
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": WORKLOAD, "l2": "flushed between timed steps (256 MiB fill)",
+                       "parallelism": "independent batches per GPU, no collective", "integrals_per_step": n_out,
+                       "nominal_evals_per_step": evals},
+            "integrals_per_s": world * n_out / (ms * 1e-3),
+            "clocks": clocks, "gpu_launches": args.steps,
+            "e2e": {"value": world * evals / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": e2e_s * 1e3, "s1_host_ms": t_s1 * 1e3},
+            "roofline": {"bound": "alu", "kernel": "mats3d_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                         "frac": achieved / peak, "traffic": None,
+                         "peak_kind": "nominal FP64: %d SMs x %d lanes x 2 x %.0f MHz (MEASURED_PEAKS.json has no FP64 "
+                                      "entry)" % (sms, FP64_LANES_PER_SM, sm_max_mhz),
+                         "peak_probe_tflops": probe_tflops, "frac_of_probe": achieved / probe_tflops,
+                         "alg_flops_per_launch": flops},
+            "wall_s_timed_region": t_wall}
+
+    if not args.no_others and world == 1:
+        line["other_configs"] = time_other_configs(torch, B, inputs, make_rules, None)
+
+    if not args.no_cpu_baseline and world == 1:
+        import oracle
+        Ro = make_rules(c, oracle.gl_rule)
+        per_out = evals // n_out
+        probe_sel = np.arange(0, n_out, n_out // 256)[:256]
+        t0 = time.perf_counter()
+        oracle_run(c, Ro, sel=probe_sel)
+        rate = probe_sel.size / (time.perf_counter() - t0)                 # outputs per second
+        n_s = int(min(8192, max(256, rate * 15.0)))
+        sel = np.arange(n_s, dtype=np.int64) * (n_out // n_s)
+        t0 = time.perf_counter()
+        o = oracle_run(c, Ro, sel=sel)
+        dt = time.perf_counter() - t0
+        got = out.cpu().numpy().ravel()[sel]
+        reg = o["dmin"] >= 1e-6
+        line["cpu_baseline"] = {"value": n_s * per_out / dt, "unit": UNIT, "cores": oracle.num_threads(),
+                                "kind": "oracle", "seconds": dt,
+                                "sample": "%d of %d outputs (every %dth), %d nodes each" % (n_s, n_out, n_out // n_s,
+                                                                                           per_out),
+                                "max_rel_err_vs_gpu_regular": float(np.max(np.abs(got[reg] / o["out"][reg] - 1)))}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
