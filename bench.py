@@ -323,10 +323,10 @@ def main():
                        "parallelism": "independent batches per GPU, no collective", "integrals_per_step": n_out,
                        "nominal_evals_per_step": evals},
             "integrals_per_s": world * n_out / (ms * 1e-3),
-            "clocks": clocks, "gpu_launches": args.steps,
+            "clocks": clocks, "gpu_launches": 3 * args.steps,  # phi-rows pre-pass, psi pre-pass, main kernel per step
             "e2e": {"value": world * evals / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_s * 1e3, "s1_host_ms": t_s1 * 1e3},
-            "roofline": {"bound": "alu", "kernel": "mats3d_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+            "roofline": {"bound": "alu", "kernel": "mats3d_main_kernel (+ its two pre-pass kernels, timed together)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                          "frac": achieved / peak, "traffic": None,
                          "peak_kind": "nominal FP64: %d SMs x %d lanes x 2 x %.0f MHz (MEASURED_PEAKS.json has no FP64 "
                                       "entry)" % (sms, FP64_LANES_PER_SM, sm_max_mhz),

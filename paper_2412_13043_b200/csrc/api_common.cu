@@ -3,6 +3,8 @@
 #include <math.h>
 #include <stdint.h>
 
+#include <mutex>
+
 #include "dfrg_internal.h"
 
 namespace dfrg {
@@ -22,6 +24,48 @@ int require_sm100(int* sm_count) {
   if (major != 10) return DFRG_EUNSUPPORTED;
   if (sm_count) *sm_count = sms;
   return DFRG_OK;
+}
+
+// ---- stream-ordered scratch pool ---------------------------------------------------------------------
+static std::mutex g_pool_mutex;
+static cudaMemPool_t g_pools[64] = {};
+
+static int get_pool(cudaMemPool_t* pool) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return check_cuda(e);
+  if (dev < 0 || dev >= 64) return DFRG_EUNSUPPORTED;
+  std::lock_guard<std::mutex> lock(g_pool_mutex);
+  if (!g_pools[dev]) {
+    cudaMemPoolProps props = {};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    e = cudaMemPoolCreate(&g_pools[dev], &props);
+    if (e != cudaSuccess) { g_pools[dev] = nullptr; return check_cuda(e); }
+    unsigned long long threshold = ~0ull;
+    cudaMemPoolSetAttribute(g_pools[dev], cudaMemPoolAttrReleaseThreshold, &threshold);
+  }
+  *pool = g_pools[dev];
+  return DFRG_OK;
+}
+
+int scratch_alloc(void** ptr, size_t bytes, cudaStream_t stream) {
+  cudaMemPool_t pool;
+  int rc = get_pool(&pool);
+  if (rc != DFRG_OK) return rc;
+  cudaError_t e = cudaMallocFromPoolAsync(ptr, bytes, pool, stream);
+  if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); set_last_cuda_error((int)e); return DFRG_ENOMEM; }
+  return check_cuda(e);
+}
+void scratch_free(void* ptr, cudaStream_t stream) {
+  if (ptr) cudaFreeAsync(ptr, stream);
+}
+void scratch_shutdown() {
+  std::lock_guard<std::mutex> lock(g_pool_mutex);
+  for (int d = 0; d < 64; ++d)
+    if (g_pools[d]) { cudaMemPoolDestroy(g_pools[d]); g_pools[d] = nullptr; }
 }
 
 // ---- arena ---------------------------------------------------------------------------------------
@@ -114,7 +158,7 @@ const char* dfrg_strerror(int status) {
 }
 int dfrg_last_cuda_error(void) { return g_last_cuda_error; }
 int dfrg_version(void) { return 100; }
-void dfrg_shutdown(void) { thread_arena().release(); }
+void dfrg_shutdown(void) { thread_arena().release(); scratch_shutdown(); }
 
 // S1: Gauss-Legendre nodes.  Half the roots from the Tricomi initial guess, Newton on P_n with the
 // three-term recurrence in long double, mirrored; derivative from P_n' = n (P_{n-1} - x P_n)/(1 - x^2).

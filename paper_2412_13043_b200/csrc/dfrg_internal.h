@@ -32,6 +32,14 @@ inline bool valid_table(const dfrg_table& t, int min_rows) {
   return false;
 }
 
+// Stream-ordered scratch for intermediate tables (S3 pre-pass outputs): allocated from a library-owned
+// cudaMemPool per device (created lazily, release threshold = max so that blocks are reused across calls
+// without touching the OS allocator), freed in stream order right after the consuming kernel.  No
+// synchronisation; dfrg_shutdown() destroys the pools.
+int scratch_alloc(void** ptr, size_t bytes, cudaStream_t stream);  // DFRG_OK / DFRG_ENOMEM / DFRG_ECUDA
+void scratch_free(void* ptr, cudaStream_t stream);
+void scratch_shutdown();
+
 // Per-thread device arena used by the *_host entry points: one growing cudaMalloc block plus a
 // private stream.  reset() rewinds; put() copies a host array in (async on the arena stream) and
 // returns the device address; get() reserves device space for an output.

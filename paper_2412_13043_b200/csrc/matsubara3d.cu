@@ -1,186 +1,326 @@
 // matsubara3d.cu -- dfrg_integrate_matsubara3d: 3-D spatial loop + Matsubara sum (BASELINE.json config 4).
 //
-// CTA = (external momentum p, external fermion index j, tile of field points); it walks the loop
-// Matsubara index n = -n_max..n_max.  Per n:
-//   S2: the two table rows it needs (Z_phi row |j-n|, Z_psi row nbar) arrive by TMA bulk copy.
-//   S3: the block builds the field-independent node tables in shared memory,
-//         inner[i][c] = (D0phi, Nw),  D0phi = Z_phi(r^2) s_phi + R(s_phi),  Nw = wc_c P(y1, y2, y3)
-//         outer[i]    = (D0psi, Wpsi), D0psi = Z_psi(q_i^2) s_psi + R(s_psi), Wpsi = wq_i q_i^2 Rdot(s_psi)
-//       with P evaluated as a cubic in y2 = p q c/k^2 whose four coefficients depend on (n, i) only.
-//   S4: thread = MF field points; per radial node the angular sum A_f = sum_c Nw / (D0phi + m2phi_f)
-//       (add -> reciprocal -> FMA; every lane reads the same table entry: shared-memory broadcast),
-//       then acc_f += Wpsi G_psi(f)^2 A_f.
-//   S5/S6: each thread owns its outputs; sums are sequential in (n, i, c) order per field point.
-// dmin: min over nodes of D0 is field independent (fl(D0 + m2) is monotone in D0).
+// Three launches per call, all on the caller's stream:
+//
+//  (1) mats3d_phi_rows_kernel  (S3, field independent, once per call)
+//        D0phi[p][m][i][c] = Z_phi(r^2; row m) s_phi + R(s_phi),  m = 0 .. n_jext-1+n_max
+//      The boson denominator depends on the external and loop Matsubara indices only through
+//      |j - n|, so the 16 x 23 (j, n) combinations of config 4 share 27 rows per momentum p.
+//      Rows go to a stream-ordered scratch buffer (31 MB for config 4: L2 resident) together with
+//      their minima (for dmin).
+//  (2) mats3d_psi_kernel       (S3, once per call)
+//        psi[n][i] = (D0psi, Wpsi) = (Z_psi(q_i^2; row nbar) s_psi + R(s_psi),  wq_i q_i^2 Rdot(s_psi))
+//  (3) mats3d_main_kernel      (S2 + S3 remainder + S4 + S5 + S6): persistent, one CTA per SM, warp-specialised
+//      (see the comment at the kernel).  Row |j-n| of D0phi and row n of psi arrive by TMA bulk copy into a
+//      double-buffered shared-memory stage; a producer warp builds the numerator row Nw[i][c] = wc_c P(y1, y2, y3)
+//      (P as a cubic in y2 = p q c/k^2 by Horner, its four coefficients depending on (n, i) only).  Hot loop:
+//      thread = MF field points; per node  d_f = D0 + m2phi_f;  two-way batched inversion
+//      r = 1/(d_a d_b), 1/d_a = r d_b, 1/d_b = r d_a  (one MUFU.RCP64H seed + cubic Newton step per two
+//      evaluations: 10 FP64 instructions per two evaluations, the same as two separate reciprocals, but
+//      half the load on the XU pipe);  a_f += Nw / d_f  on two accumulators per field point.
+//      Every lane of a warp reads the same table entries (shared-memory broadcast).
+//      Then acc_f += Wpsi G_psi(f)^2 a_f.
+// dmin: fl(D0 + m2) is monotone in D0, so the minimum over nodes is (min D0) + m2: no hot-loop work.
+#include <stdlib.h>
+
 #include "dfrg_device.cuh"
 #include "dfrg_internal.h"
 
 namespace dfrg {
 
-constexpr int M3_THREADS = 256;
 constexpr int M3_MAX_PAIRS = 6144;
+constexpr int M3_PRE_THREADS = 256;
 
 struct Mats3dParams {
-  int nq, nc, n_field, n_p, n_jext, n_max;
+  int nq, nc, n_field, n_p, n_jext, n_max, n_rows, row_stride;
   double T, prefactor;
   RegParams reg;
   GridParams grid;
   const double *xq, *wq, *xc, *wc, *Zpsi, *Zphi, *coef, *m2psi, *m2phi, *pext;
+  double *d0phi;    // [n_p][n_rows][row_stride]
+  double *rowmin;   // [n_p][n_rows]
+  double2 *psi;     // [2 n_max + 1][psi_stride]
+  double *psimin;   // [2 n_max + 1]
+  int psi_stride;
   double *out, *dmin;
 };
 
-template <int MF>
-__global__ void __launch_bounds__(M3_THREADS) mats3d_kernel(const Mats3dParams P) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  __shared__ __align__(8) uint64_t bar;
+// ---- (1) boson rows --------------------------------------------------------------------------------
+__global__ void __launch_bounds__(M3_PRE_THREADS) mats3d_phi_rows_kernel(const Mats3dParams P) {
+  __shared__ double srow[1024];
   __shared__ double red[32];
+  const int m = blockIdx.x, e = blockIdx.y;
+  const int nt = P.grid.n;
+  for (int i = threadIdx.x; i < nt; i += M3_PRE_THREADS) srow[i] = P.Zphi[(size_t)m * nt + i];
+  __syncthreads();
+  const double p = P.pext[e];
+  const double om = 2.0 * 3.14159265358979323846 * (double)m * P.T;
+  const int npairs = P.nq * P.nc;
+  double* dst = P.d0phi + ((size_t)e * P.n_rows + m) * P.row_stride;
+  double dmin = __longlong_as_double(0x7ff0000000000000LL);
+  for (int t = threadIdx.x; t < npairs; t += M3_PRE_THREADS) {
+    const int i = t / P.nc, jc = t - i * P.nc;
+    const double q = P.xq[i], c = P.xc[jc];
+    double r2 = p * p + q * q - 2.0 * p * q * c;
+    r2 = r2 > 0.0 ? r2 : 0.0;
+    const double sphi = om * om + r2;
+    double R, Rd;
+    regulator(P.reg, sphi, R, Rd);
+    const double D0 = table_lookup(srow, P.grid, r2) * sphi + R;
+    dst[t] = D0;
+    dmin = fmin(dmin, D0);
+  }
+  if (threadIdx.x == 0 && (npairs & 1)) dst[npairs] = 1.0;  // pad to the even row stride
+  dmin = block_min(dmin, red);
+  if (threadIdx.x == 0) P.rowmin[(size_t)e * P.n_rows + m] = dmin;
+}
+
+// ---- (2) fermion line --------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) mats3d_psi_kernel(const Mats3dParams P) {
+  __shared__ double red[32];
+  const int it = blockIdx.x, n = it - P.n_max;
+  const int nbar = n >= 0 ? n : -n - 1;
+  const double nun = (2.0 * n + 1.0) * 3.14159265358979323846 * P.T;
+  const double* row = P.Zpsi + (size_t)nbar * P.grid.n;
+  double dmin = __longlong_as_double(0x7ff0000000000000LL);
+  for (int i = threadIdx.x; i < P.nq; i += 128) {
+    const double q = P.xq[i];
+    const double spsi = nun * nun + q * q;
+    double R, Rd;
+    regulator(P.reg, spsi, R, Rd);
+    const double D0 = table_lookup(row, P.grid, q * q) * spsi + R;
+    P.psi[(size_t)it * P.psi_stride + i] = make_double2(D0, P.wq[i] * q * q * Rd);
+    dmin = fmin(dmin, D0);
+  }
+  dmin = block_min(dmin, red);
+  if (threadIdx.x == 0) P.psimin[it] = dmin;
+}
+
+// ---- (3) main kernel -----------------------------------------------------------------------------------
+// Persistent, warp-specialised.  One CTA per SM walks the work items (p, j, field tile) it owns
+// (item = blockIdx.x + k gridDim.x) and, inside an item, the loop Matsubara index n.  One producer warp
+// runs up to two (item, n) stages ahead of the consumers: it waits for a stage to drain (mbarrier
+// empty[b]), issues the TMA bulk copies of row |j-n| of D0phi and row n of psi, builds the numerator row
+// Nw in shared memory and arrives on full[b].  GROUPS x 256 consumer threads run the hot loop: thread =
+// (MF field points, radial nodes i = group mod GROUPS); the groups' partial sums are combined in fixed
+// order through shared memory once per item.
+constexpr int M3_FT = 128;  // threads per consumer group; a group covers M3_FT x MF field points
+
+// One quadrature node for the MF field points of a thread:  a_f += Nw / (D0 + m2_f).
+// Batched inversion over the field points (same Nw): with d_f = D0 + m2_f,
+//   MF = 2:  R = Nw/(d0 d1),               a0 += R d1,            a1 += R d0              (9 FP64 instr / 2 evals)
+//   MF = 4:  R = Nw/((d0 d1)(d2 d3)),      a0 += (R p23) d1, ...                          (17 FP64 instr / 4 evals)
+// i.e. 4 + 1/MF FP64-pipe instructions and 1/MF MUFU.RCP64H per evaluation instead of 5 and 1.  The products stay
+// far inside the double range (|d| between ~1e-3 k^2 and ~1e5 k^2); each extra multiply costs half an ulp.
+template <int MF>
+__device__ __forceinline__ void accumulate_node(const double D0, const double Nw, const double (&m2)[MF],
+                                                double (&a)[MF]) {
+  if constexpr (MF == 1) {
+    a[0] = fma(Nw, fast_rcp(D0 + m2[0]), a[0]);
+  } else if constexpr (MF == 2) {
+    const double d0 = D0 + m2[0], d1 = D0 + m2[1];
+    const double R = fast_rcp(d0 * d1) * Nw;
+    a[0] = fma(R, d1, a[0]);
+    a[1] = fma(R, d0, a[1]);
+  } else {
+    static_assert(MF == 4, "MF must be 1, 2 or 4");
+    const double d0 = D0 + m2[0], d1 = D0 + m2[1], d2 = D0 + m2[2], d3 = D0 + m2[3];
+    const double p01 = d0 * d1, p23 = d2 * d3;
+    const double R = fast_rcp(p01 * p23) * Nw;
+    const double r01 = R * p23, r23 = R * p01;
+    a[0] = fma(r01, d1, a[0]);
+    a[1] = fma(r01, d0, a[1]);
+    a[2] = fma(r23, d3, a[2]);
+    a[3] = fma(r23, d2, a[3]);
+  }
+}
+
+template <int GROUPS, int MF>
+__global__ void __launch_bounds__(GROUPS * M3_FT + 32, 1) mats3d_main_kernel(const Mats3dParams P) {
+  constexpr int NCONS = GROUPS * M3_FT;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t full[2], empty[2];
   __shared__ double skap[20];
 
-  const int nq = P.nq, nc = P.nc, npairs = nq * nc, nt = P.grid.n;
-  double2* inner = reinterpret_cast<double2*>(smem_raw);  // [nq*nc]
-  double2* outer = inner + npairs;                         // [nq]
-  double* beta = reinterpret_cast<double*>(outer + nq);    // [nq][4]
+  const int nq = P.nq, nc = P.nc, npairs = nq * nc;
+  const int rs = P.row_stride, ps = P.psi_stride;
+  double* d0buf = reinterpret_cast<double*>(smem_raw);               // [2][rs]
+  double2* psibuf = reinterpret_cast<double2*>(d0buf + 2 * rs);      // [2][ps]
+  double* nwbuf = reinterpret_cast<double*>(psibuf + 2 * ps);        // [2][rs]
+  double* beta = nwbuf + 2 * rs;                                     // [nq][4]   (producer only)
   double* sxq = beta + 4 * nq;
-  double* swq = sxq + ((nq + 1) & ~1);
-  double* sxc = swq + ((nq + 1) & ~1);
+  double* sxc = sxq + ((nq + 1) & ~1);
   double* swc = sxc + ((nc + 1) & ~1);
-  double* rowpsi = swc + ((nc + 1) & ~1);
-  double* rowphi = rowpsi + ((nt + 1) & ~1);
+  double* part = swc + ((nc + 1) & ~1);                              // [2][GROUPS][M3_FT * MF]
 
-  if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
-  if (threadIdx.x < 20) skap[threadIdx.x] = P.coef[threadIdx.x];
-  __syncthreads();
-  uint32_t parity = 0;
-  {
-    StageList L;
-    L.add(sxq, P.xq, nq); L.add(swq, P.wq, nq);
-    L.add(sxc, P.xc, nc); L.add(swc, P.wc, nc);
-    stage_to_smem(L, &bar, parity);
-    parity ^= 1;
-  }
-
-  const int e = blockIdx.x / P.n_jext, j = blockIdx.x - e * P.n_jext;
-  const double p = P.pext[e];
+  const int n_terms = 2 * P.n_max + 1;
+  const int n_ftiles = (P.n_field + M3_FT * MF - 1) / (M3_FT * MF);
+  const int n_items = P.n_p * P.n_jext * n_ftiles;
+  const uint32_t row_bytes = (uint32_t)rs * 8u, psi_bytes = (uint32_t)ps * 16u;
   const double pi = 3.14159265358979323846;
-  const double nuj = (2.0 * j + 1.0) * pi * P.T;
   const double ik2 = P.reg.inv_k2;
-  const double inf = __longlong_as_double(0x7ff0000000000000LL);
 
-  const int f0 = blockIdx.y * (M3_THREADS * MF) + threadIdx.x;
-  double m2psi[MF], m2phi[MF], acc[MF];
-#pragma unroll
-  for (int m = 0; m < MF; ++m) {
-    const int f = f0 + m * M3_THREADS;
-    m2psi[m] = (f < P.n_field) ? P.m2psi[f] : 1.0;
-    m2phi[m] = (f < P.n_field) ? P.m2phi[f] : 1.0;
-    acc[m] = 0.0;
+  if (threadIdx.x == 0) {
+    mbar_init(&full[0], 1);
+    mbar_init(&full[1], 1);
+    mbar_init(&empty[0], NCONS / 32);
+    mbar_init(&empty[1], NCONS / 32);
+    mbar_fence_init();
   }
-  double dmin_psi = inf, dmin_phi = inf;
+  if (threadIdx.x < 20) skap[threadIdx.x] = P.coef[threadIdx.x];
+  for (int i = threadIdx.x; i < nq; i += blockDim.x) sxq[i] = P.xq[i];
+  for (int i = threadIdx.x; i < nc; i += blockDim.x) { sxc[i] = P.xc[i]; swc[i] = P.wc[i]; }
+  __syncthreads();
 
-  for (int n = -P.n_max; n <= P.n_max; ++n) {
-    const int nbar = n >= 0 ? n : -n - 1;
-    const int mm = j - n;
-    const int mabs = mm >= 0 ? mm : -mm;
-    const double nun = (2.0 * n + 1.0) * pi * P.T;
-    const double om = 2.0 * pi * (double)mm * P.T;
-    const double y1 = nun * nuj * ik2;
-
-    __syncthreads();  // previous hot loop done with inner/outer/rows
-    {
-      StageList L;
-      L.add(rowpsi, P.Zpsi + (size_t)nbar * nt, nt);
-      L.add(rowphi, P.Zphi + (size_t)mabs * nt, nt);
-      stage_to_smem(L, &bar, parity);
-      parity ^= 1;
-    }
-    // ---- S3a: per radial node ----
-    for (int i = threadIdx.x; i < nq; i += M3_THREADS) {
-      const double q = sxq[i];
-      const double spsi = nun * nun + q * q;
-      double R, Rd;
-      regulator(P.reg, spsi, R, Rd);
-      const double D0 = table_lookup(rowpsi, P.grid, q * q) * spsi + R;
-      outer[i] = make_double2(D0, swq[i] * q * q * Rd);
-      dmin_psi = fmin(dmin_psi, D0);
-      // P = sum_b y2^b beta_b,  beta_b = sum_{a+c<=3-b} kap_abc y1^a y3^c   (idx: a outermost, then b, then c)
-      const double y3 = spsi * ik2;
-      double be[4] = {0.0, 0.0, 0.0, 0.0};
-      int idx = 0;
-      double y1a = 1.0;
+  if (threadIdx.x >= NCONS) {
+    // =========================== producer warp ===========================
+    const int lane = threadIdx.x - NCONS;
+    uint32_t g = 0;  // global stage counter
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+      const int ej = item / n_ftiles;
+      const int e = ej / P.n_jext, j = ej - e * P.n_jext;
+      const double p = P.pext[e];
+      const double nuj = (2.0 * j + 1.0) * pi * P.T;
+      for (int it = 0; it < n_terms; ++it, ++g) {
+        const int b = g & 1;
+        const int n = it - P.n_max;
+        const int mm = j - n, mabs = mm >= 0 ? mm : -mm;
+        mbar_wait(&empty[b], ((g >> 1) & 1) ^ 1);  // consumers drained this stage (passes at once for g < 2)
+        if (lane == 0) {
+          mbar_expect_tx_only(&full[b], row_bytes + psi_bytes);
+          tma_bulk_g2s(d0buf + (size_t)b * rs, P.d0phi + ((size_t)e * P.n_rows + mabs) * rs, row_bytes, &full[b]);
+          tma_bulk_g2s(psibuf + (size_t)b * ps, P.psi + (size_t)it * ps, psi_bytes, &full[b]);
+        }
+        // P = sum_b y2^b beta_b,  beta_b = sum_{a+c<=3-b} kap_abc y1^a y3^c   (idx: a outermost, then b, then c)
+        const double nun = (2.0 * n + 1.0) * pi * P.T;
+        const double y1 = nun * nuj * ik2;
+        for (int i = lane; i < nq; i += 32) {
+          const double q = sxq[i];
+          const double y3 = (nun * nun + q * q) * ik2;
+          double be[4] = {0.0, 0.0, 0.0, 0.0};
+          int idx = 0;
+          double y1a = 1.0;
 #pragma unroll
-      for (int a = 0; a <= 3; ++a) {
+          for (int a = 0; a <= 3; ++a) {
 #pragma unroll
-        for (int b = 0; b <= 3 - a; ++b) {
-          double y3c = y1a;
+            for (int bb = 0; bb <= 3 - a; ++bb) {
+              double y3c = y1a;
 #pragma unroll
-          for (int c = 0; c <= 3 - a - b; ++c) {
-            be[b] = fma(skap[idx++], y3c, be[b]);
-            y3c *= y3;
+              for (int c = 0; c <= 3 - a - bb; ++c) {
+                be[bb] = fma(skap[idx++], y3c, be[bb]);
+                y3c *= y3;
+              }
+            }
+            y1a *= y1;
+          }
+          beta[4 * i + 0] = be[0]; beta[4 * i + 1] = be[1]; beta[4 * i + 2] = be[2]; beta[4 * i + 3] = be[3];
+        }
+        __syncwarp();
+        double* nw = nwbuf + (size_t)b * rs;
+        for (int i = 0; i < nq; ++i) {
+          const double pq = p * sxq[i] * ik2;
+          const double b0 = beta[4 * i], b1 = beta[4 * i + 1], b2 = beta[4 * i + 2], b3 = beta[4 * i + 3];
+          for (int jc = lane; jc < nc; jc += 32) {
+            const double y2 = pq * sxc[jc];
+            nw[i * nc + jc] = swc[jc] * fma(fma(fma(b3, y2, b2), y2, b1), y2, b0);
           }
         }
-        y1a *= y1;
+        if (lane == 0 && (npairs & 1)) nw[npairs] = 0.0;
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&full[b]);  // release: the Nw row is visible to whoever acquires full[b]
       }
-      beta[4 * i + 0] = be[0]; beta[4 * i + 1] = be[1]; beta[4 * i + 2] = be[2]; beta[4 * i + 3] = be[3];
     }
-    __syncthreads();
-    // ---- S3b: per (radial, angular) node ----
-    for (int t = threadIdx.x; t < npairs; t += M3_THREADS) {
-      const int i = t / nc, jc = t - i * nc;
-      const double q = sxq[i], c = sxc[jc];
-      double r2 = p * p + q * q - 2.0 * p * q * c;
-      r2 = r2 > 0.0 ? r2 : 0.0;
-      const double sphi = om * om + r2;
-      double R, Rd;
-      regulator(P.reg, sphi, R, Rd);
-      const double D0 = table_lookup(rowphi, P.grid, r2) * sphi + R;
-      const double y2 = p * q * c * ik2;
-      const double poly = fma(fma(fma(beta[4 * i + 3], y2, beta[4 * i + 2]), y2, beta[4 * i + 1]), y2, beta[4 * i]);
-      inner[t] = make_double2(D0, swc[jc] * poly);
-      dmin_phi = fmin(dmin_phi, D0);
-    }
-    __syncthreads();
+    return;
+  }
 
-    // ---- S4 ----
-    for (int i = 0; i < nq; ++i) {
-      const double2* row = inner + i * nc;
-      double a[MF];
+  // =============================== consumers ===============================
+  const int grp = threadIdx.x / M3_FT, tf = threadIdx.x - grp * M3_FT;
+  const bool warp_leader = (threadIdx.x & 31) == 0;
+  uint32_t g = 0;
+  int item_parity = 0;
+  for (int item = blockIdx.x; item < n_items; item += gridDim.x, item_parity ^= 1) {
+    const int ej = item / n_ftiles, ftile = item - ej * n_ftiles;
+    const int e = ej / P.n_jext, j = ej - e * P.n_jext;
+    const int f0 = ftile * (M3_FT * MF) + tf;
+    double m2psi[MF], m2phi[MF], acc[MF];
 #pragma unroll
-      for (int m = 0; m < MF; ++m) a[m] = 0.0;
-#pragma unroll 4
-      for (int jc = 0; jc < nc; ++jc) {
-        const double2 pr = row[jc];
+    for (int m = 0; m < MF; ++m) {
+      const int f = f0 + m * M3_FT;
+      m2psi[m] = (f < P.n_field) ? P.m2psi[f] : 1.0;
+      m2phi[m] = (f < P.n_field) ? P.m2phi[f] : 1.0;
+      acc[m] = 0.0;
+    }
+    for (int it = 0; it < n_terms; ++it, ++g) {
+      const int b = g & 1;
+      mbar_wait(&full[b], (g >> 1) & 1);
+      const double* d0 = d0buf + (size_t)b * rs;
+      const double* nw = nwbuf + (size_t)b * rs;
+      const double2* psi = psibuf + (size_t)b * ps;
+      for (int i = grp; i < nq; i += GROUPS) {
+        // fermion line first: its reciprocal chain overlaps with the angular loop below
+        const double2 o = psi[i];
+        double h[MF], a[MF];
 #pragma unroll
-        for (int m = 0; m < MF; ++m) a[m] = fma(pr.y, fast_rcp(pr.x + m2phi[m]), a[m]);
+        for (int m = 0; m < MF; ++m) {
+          const double gpsi = fast_rcp(o.x + m2psi[m]);
+          h[m] = o.y * (gpsi * gpsi);
+          a[m] = 0.0;
+        }
+        if ((nc & 1) == 0) {
+          const double2* drow = reinterpret_cast<const double2*>(d0 + i * nc);
+          const double2* nrow = reinterpret_cast<const double2*>(nw + i * nc);
+#pragma unroll 2
+          for (int jc = 0; jc < nc / 2; ++jc) {
+            const double2 dd = drow[jc], nn = nrow[jc];
+            accumulate_node<MF>(dd.x, nn.x, m2phi, a);
+            accumulate_node<MF>(dd.y, nn.y, m2phi, a);
+          }
+        } else {
+          for (int jc = 0; jc < nc; ++jc) accumulate_node<MF>(d0[i * nc + jc], nw[i * nc + jc], m2phi, a);
+        }
+#pragma unroll
+        for (int m = 0; m < MF; ++m) acc[m] = fma(h[m], a[m], acc[m]);
       }
-      const double2 o = outer[i];
+      __syncwarp();
+      if (warp_leader) mbar_arrive(&empty[b]);
+    }
+    // ---- S5/S6: combine the radial-node groups in fixed order, write the item's outputs ----
+    double* mypart = part + (size_t)item_parity * GROUPS * (M3_FT * MF);
+#pragma unroll
+    for (int m = 0; m < MF; ++m) mypart[grp * (M3_FT * MF) + m * M3_FT + tf] = acc[m];
+    named_bar_sync(1, NCONS);
+    if (grp == 0) {
+      const double scale = P.prefactor * P.T;
+      double dpsi = 0.0, dphi = 0.0;
+      if (P.dmin) {
+        const double inf = __longlong_as_double(0x7ff0000000000000LL);
+        dpsi = inf;
+        dphi = inf;
+        for (int it = 0; it < n_terms; ++it) {
+          const int mm = j - (it - P.n_max), mabs = mm >= 0 ? mm : -mm;
+          dpsi = fmin(dpsi, P.psimin[it]);
+          dphi = fmin(dphi, P.rowmin[(size_t)e * P.n_rows + mabs]);
+        }
+      }
 #pragma unroll
       for (int m = 0; m < MF; ++m) {
-        const double g = fast_rcp(o.x + m2psi[m]);
-        acc[m] = fma(o.y * (g * g), a[m], acc[m]);
-      }
-    }
-  }
-
-  const double scale = P.prefactor * P.T;
-  double dpsi = 0.0, dphi = 0.0;
-  if (P.dmin) {
-    dpsi = block_min(dmin_psi, red);
-    dphi = block_min(dmin_phi, red);
-  }
+        const int f = f0 + m * M3_FT;
+        if (f < P.n_field) {
+          double r = mypart[m * M3_FT + tf];
 #pragma unroll
-  for (int m = 0; m < MF; ++m) {
-    const int f = f0 + m * M3_THREADS;
-    if (f < P.n_field) {
-      const size_t o = (size_t)blockIdx.x * P.n_field + f;
-      P.out[o] = scale * acc[m];
-      if (P.dmin) P.dmin[o] = fmin(dpsi + m2psi[m], dphi + m2phi[m]) * ik2;
+          for (int gg = 1; gg < GROUPS; ++gg) r += mypart[gg * (M3_FT * MF) + m * M3_FT + tf];
+          const size_t o = (size_t)ej * P.n_field + f;
+          P.out[o] = scale * r;
+          if (P.dmin) P.dmin[o] = fmin(dpsi + m2psi[m], dphi + m2phi[m]) * ik2;
+        }
+      }
     }
   }
 }
 
-static size_t mats3d_smem(int nq, int nc, int nt) {
-  return (size_t)nq * nc * 16 + (size_t)nq * 16 +
-         8 * (size_t)(4 * nq + 2 * ((nq + 1) & ~1) + 2 * ((nc + 1) & ~1) + 2 * ((nt + 1) & ~1));
+static size_t mats3d_main_smem(int nq, int nc, int rs, int ps, int groups, int mf) {
+  return 8 * (size_t)(2 * rs + 4 * ps + 2 * rs + 4 * nq + ((nq + 1) & ~1) + 2 * ((nc + 1) & ~1) +
+                      2 * groups * M3_FT * mf);
 }
 
 static int mats3d_validate(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi, const double* m2_phi, int n_p,
@@ -194,14 +334,32 @@ static int mats3d_validate(const dfrg_mats3d_desc* D, int n_field, const double*
       D->tab_psi.lnq_hi != D->tab_phi.lnq_hi || D->tab_psi.interp != D->tab_phi.interp)
     return DFRG_EINVAL;
   if ((long long)D->q.n * D->cos1.n > M3_MAX_PAIRS || D->tab_psi.n_q > 1024) return DFRG_EUNSUPPORTED;
-  if ((long long)n_p * n_jext > 2147483647LL) return DFRG_EUNSUPPORTED;
+  if ((long long)n_p * n_jext > 2147483647LL || n_p > 65535) return DFRG_EUNSUPPORTED;
   return DFRG_OK;
 }
 
+template <int GROUPS, int MF>
+static int mats3d_launch_main(const Mats3dParams& P, int sm_count, cudaStream_t stream) {
+  const size_t smem = mats3d_main_smem(P.nq, P.nc, P.row_stride, P.psi_stride, GROUPS, MF);
+  if (smem > 227 * 1024) return DFRG_EUNSUPPORTED;
+  cudaError_t e = cudaFuncSetAttribute(mats3d_main_kernel<GROUPS, MF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)smem);
+  if (e != cudaSuccess) return check_cuda(e);
+  const long long n_ftiles = (P.n_field + M3_FT * MF - 1) / (M3_FT * MF);
+  const long long n_items = (long long)P.n_p * P.n_jext * n_ftiles;
+  const int grid = (int)(n_items < sm_count ? n_items : sm_count);
+  mats3d_main_kernel<GROUPS, MF><<<grid, GROUPS * M3_FT + 32, smem, stream>>>(P);
+  return check_cuda(cudaGetLastError());
+}
+
 static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi, const double* m2_phi, int n_p,
-                         const double* p, int n_jext, double* out, double* dmin, cudaStream_t stream) {
+                         const double* p, int n_jext, double* out, double* dmin, int sm_count, cudaStream_t stream) {
   Mats3dParams P;
   P.nq = D->q.n; P.nc = D->cos1.n; P.n_field = n_field; P.n_p = n_p; P.n_jext = n_jext; P.n_max = D->n_max;
+  P.n_rows = n_jext + D->n_max;
+  const int npairs = P.nq * P.nc;
+  P.row_stride = (npairs + 1) & ~1;  // TMA bulk copies move multiples of 16 bytes
+  P.psi_stride = P.nq;
   P.T = D->T; P.prefactor = D->prefactor;
   P.reg.kind = D->reg.kind; P.reg.order = D->reg.order; P.reg.k2 = D->reg.k * D->reg.k; P.reg.inv_k2 = 1.0 / P.reg.k2;
   P.grid.lo = D->tab_psi.lnq_lo; P.grid.n = D->tab_psi.n_q; P.grid.interp = D->tab_psi.interp;
@@ -209,21 +367,48 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   P.xq = D->q.x; P.wq = D->q.w; P.xc = D->cos1.x; P.wc = D->cos1.w;
   P.Zpsi = D->tab_psi.v; P.Zphi = D->tab_phi.v; P.coef = D->coef;
   P.m2psi = m2_psi; P.m2phi = m2_phi; P.pext = p; P.out = out; P.dmin = dmin;
-  const size_t smem = mats3d_smem(P.nq, P.nc, P.grid.n);
-  const int mf = (n_field > M3_THREADS) ? 2 : 1;
-  dim3 grid(n_p * n_jext, (n_field + M3_THREADS * mf - 1) / (M3_THREADS * mf));
-  if (grid.y > 65535) return DFRG_EUNSUPPORTED;
-  cudaError_t e;
-  if (mf == 2) {
-    e = cudaFuncSetAttribute(mats3d_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return check_cuda(e);
-    mats3d_kernel<2><<<grid, M3_THREADS, smem, stream>>>(P);
-  } else {
-    e = cudaFuncSetAttribute(mats3d_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return check_cuda(e);
-    mats3d_kernel<1><<<grid, M3_THREADS, smem, stream>>>(P);
+
+  const int n_terms = 2 * D->n_max + 1;
+  const size_t n_d0 = (size_t)n_p * P.n_rows * P.row_stride;
+  const size_t n_rowmin = ((size_t)n_p * P.n_rows + 1) & ~(size_t)1;
+  const size_t n_psi = (size_t)n_terms * P.psi_stride * 2;
+  const size_t n_psimin = ((size_t)n_terms + 1) & ~(size_t)1;
+  void* scratch = nullptr;
+  int rc = scratch_alloc(&scratch, (n_d0 + n_rowmin + n_psi + n_psimin) * sizeof(double), stream);
+  if (rc != DFRG_OK) return rc;
+  P.d0phi = (double*)scratch;
+  P.psi = (double2*)(P.d0phi + n_d0);
+  P.rowmin = (double*)(P.psi) + n_psi;
+  P.psimin = P.rowmin + n_rowmin;
+
+  mats3d_phi_rows_kernel<<<dim3(P.n_rows, n_p), M3_PRE_THREADS, 0, stream>>>(P);
+  rc = check_cuda(cudaGetLastError());
+  if (rc == DFRG_OK) {
+    mats3d_psi_kernel<<<n_terms, 128, 0, stream>>>(P);
+    rc = check_cuda(cudaGetLastError());
   }
-  return check_cuda(cudaGetLastError());
+  if (rc == DFRG_OK) {
+    // consumer groups per CTA (radial nodes are dealt round-robin to the groups) and field points per thread;
+    // DFRG_M3_GROUPS / DFRG_M3_MF override the defaults (tuning knobs)
+    const char* vg = getenv("DFRG_M3_GROUPS");
+    const char* vm = getenv("DFRG_M3_MF");
+    int mf = n_field > 2 * M3_FT ? 4 : (n_field > M3_FT ? 2 : 1);
+    if (vm && atoi(vm) >= 1 && atoi(vm) < mf) mf = atoi(vm) == 3 ? 2 : atoi(vm);
+    const int groups = vg ? atoi(vg) : 6;
+    if (mf == 4) {
+      if (groups == 7) rc = mats3d_launch_main<7, 4>(P, sm_count, stream);
+      else if (groups == 4) rc = mats3d_launch_main<4, 4>(P, sm_count, stream);
+      else rc = mats3d_launch_main<6, 4>(P, sm_count, stream);
+    } else if (mf == 2) {
+      if (groups == 7) rc = mats3d_launch_main<7, 2>(P, sm_count, stream);
+      else if (groups == 4) rc = mats3d_launch_main<4, 2>(P, sm_count, stream);
+      else rc = mats3d_launch_main<6, 2>(P, sm_count, stream);
+    } else {
+      rc = mats3d_launch_main<4, 1>(P, sm_count, stream);
+    }
+  }
+  scratch_free(scratch, stream);
+  return rc;
 }
 
 }  // namespace dfrg
@@ -235,9 +420,10 @@ extern "C" int dfrg_integrate_matsubara3d(const dfrg_mats3d_desc* D, int n_field
                                           double* dmin, void* cuda_stream) {
   int rc = mats3d_validate(D, n_field, m2_psi, m2_phi, n_p, p, n_jext, out);
   if (rc != DFRG_OK) return rc;
-  rc = require_sm100(nullptr);
+  int sms = 0;
+  rc = require_sm100(&sms);
   if (rc != DFRG_OK) return rc;
-  return mats3d_launch(D, n_field, m2_psi, m2_phi, n_p, p, n_jext, out, dmin, (cudaStream_t)cuda_stream);
+  return mats3d_launch(D, n_field, m2_psi, m2_phi, n_p, p, n_jext, out, dmin, sms, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi,
@@ -245,7 +431,8 @@ extern "C" int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_
                                                double* out, double* dmin) {
   int rc = mats3d_validate(D, n_field, m2_psi, m2_phi, n_p, p, n_jext, out);
   if (rc != DFRG_OK) return rc;
-  rc = require_sm100(nullptr);
+  int sms = 0;
+  rc = require_sm100(&sms);
   if (rc != DFRG_OK) return rc;
   Arena& A = thread_arena();
   const size_t nf = (size_t)n_field, n_out = (size_t)n_p * n_jext * nf;
@@ -265,7 +452,7 @@ extern "C" int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_
   double* d_out = A.reserve(n_out);
   double* d_dmin = dmin ? A.reserve(n_out) : nullptr;
   if (A.status() != DFRG_OK) return A.status();
-  rc = mats3d_launch(&Dd, n_field, d_mpsi, d_mphi, n_p, d_p, n_jext, d_out, d_dmin, A.stream());
+  rc = mats3d_launch(&Dd, n_field, d_mpsi, d_mphi, n_p, d_p, n_jext, d_out, d_dmin, sms, A.stream());
   if (rc != DFRG_OK) return rc;
   A.fetch(out, d_out, n_out);
   if (dmin) A.fetch(dmin, d_dmin, n_out);
