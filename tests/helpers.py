@@ -5,9 +5,10 @@ import numpy as np
 import oracle
 from paper_2412_13043_b200 import inputs  # noqa: F401
 
-REGULAR_DMIN = 1e-6      # an output is regular iff the oracle's dmin >= this (reading A4)
-RTOL = 1e-12             # north_star: relative error <= 1e-12 per output on the same nodes
-SENS_EPS = 1e-13         # condition-aware bound for singular outputs: |gpu - oracle| <= SENS_EPS * sens
+REGULAR_DMIN = 1e-6      # an output is regular iff the oracle's dmin >= this (reading A4) ...
+COND_MAX = 1e4           # ... and its terms do not cancel by more than this: sens / |out| <= COND_MAX
+RTOL = 1e-12             # north_star: relative error <= 1e-12 per output on the same nodes (regular outputs)
+SENS_EPS = 1e-14         # every output, regular or not: |gpu - oracle| <= SENS_EPS * sens (condition-aware bound)
 
 
 def kind_of(c):
@@ -98,16 +99,19 @@ def gpu_run(c, R, host=False, want_dmin=True):
 
 
 def parity_report(gpu, orc, dmin_orc, sens):
-    """Element-by-element comparison.  Regular outputs (oracle dmin >= REGULAR_DMIN): relative error.
-    Singular outputs: |diff| / sens.  Returns a dict of worst cases; assert_parity() applies the bars."""
+    """Element-by-element comparison.  Regular outputs (oracle dmin >= REGULAR_DMIN and sens/|out| <= COND_MAX):
+    relative error.  All outputs: |diff| / sens.  Returns a dict of worst cases; assert_parity() applies the bars."""
     gpu, orc, dmin_orc, sens = (np.asarray(a, dtype=np.float64).ravel() for a in (gpu, orc, dmin_orc, sens))
-    regular = dmin_orc >= REGULAR_DMIN
+    with np.errstate(divide="ignore", invalid="ignore"):
+        cond = np.where(orc != 0, sens / np.abs(orc), np.inf)
+    regular = (dmin_orc >= REGULAR_DMIN) & (cond <= COND_MAX)
     diff = np.abs(gpu - orc)
     with np.errstate(divide="ignore", invalid="ignore"):
         rel = np.where(orc != 0, diff / np.abs(orc), np.where(diff == 0, 0.0, np.inf))
         ratio = diff / sens
     both_nonfinite = ~np.isfinite(gpu) & ~np.isfinite(orc)
     rep = dict(n=gpu.size, n_regular=int(regular.sum()), n_singular=int((~regular).sum()),
+               n_pole=int((dmin_orc < REGULAR_DMIN).sum()), n_cancelling=int(((dmin_orc >= REGULAR_DMIN) & ~regular).sum()),
                max_rel_regular=float(rel[regular].max()) if regular.any() else 0.0,
                max_sens_ratio_regular=float(np.nanmax(ratio[regular])) if regular.any() else 0.0,
                max_sens_ratio_singular=float(np.nanmax(np.where(both_nonfinite, 0.0, ratio)[~regular]))
@@ -122,6 +126,7 @@ def assert_parity(gpu, orc, dmin_orc, sens, what=""):
     rep = parity_report(gpu, orc, dmin_orc, sens)
     msg = {k_: v for k_, v in rep.items() if not k_.startswith("_")}
     assert rep["max_rel_regular"] <= RTOL, (what, msg)
+    assert rep["max_sens_ratio_regular"] <= SENS_EPS, (what, msg)
     assert rep["max_sens_ratio_singular"] <= SENS_EPS, (what, msg)
     return msg
 
