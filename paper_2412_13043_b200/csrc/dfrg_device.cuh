@@ -1,7 +1,7 @@
 // dfrg_device.cuh -- device-side building blocks shared by the integration kernels (sm_100a).
 //   * FP64 reciprocal from the hardware seed (MUFU.RCP64H) + one cubic Newton step
-//   * regulators (eq. 14)
-//   * log-grid cubic / linear interpolation reading shared-memory tables
+//   * table-driven FP64 log / exp (shared-memory tables), regulators (eq. 14)
+//   * log-grid cubic / linear interpolation reading per-cell cubics in shared memory
 //   * TMA 1-D bulk copies global -> shared with an mbarrier (cp.async.bulk; SASS: UBLKCP)
 //   * deterministic block reductions (fixed shuffle tree, fixed warp order)
 #pragma once
@@ -27,6 +27,70 @@ __device__ __forceinline__ double fast_rcp(double d) {
   return fma(r0, t, r0);
 }
 
+// ---- table-driven FP64 log and exp --------------------------------------------------------------------------
+// The S3 pre-computation is dominated by log (table coordinate) and exp (regulator).  libdevice's versions
+// cost ~100 SASS instructions each, two thirds of them integer/constant traffic.  These versions keep two small
+// tables in shared memory (built once per CTA from libdevice log/exp2, fm_build) and need ~10 FP64 instructions:
+//   fm_log(s):  s = 2^e m, m in [1,2); j = top 7 mantissa bits; r = m * (1/c_j) - 1, |r| <= 2^-8;
+//               ln s = e ln2 + ln c_j + (r - r^2/2 + ... - r^6/6)          abs. error <~ 3e-16 for |e| < 64
+//   fm_exp_neg(x) = e^-x, 0 <= x: n = rint(-64 x / ln2), r = -x - n ln2/64, |r| <= ln2/128;
+//               e^-x = 2^(n>>6) 2^((n&63)/64) (1 + r + ... + r^5/120)       rel. error <~ 2 ulp; x > 700 is clamped
+//               (e^-700 = 1e-304: the regulator is then 300 orders of magnitude below anything it is added to).
+// fm_log(0) = -709.8 (exponent field 0): every table coordinate derived from it clamps to the first grid point.
+struct FastMath {
+  const double2* logtab;  // [128] (1/c_j, ln c_j)
+  const double* exptab;   // [64]  2^(j/64)
+};
+constexpr int FM_DOUBLES = 2 * 128 + 64;
+
+// All threads of the CTA; the caller synchronises before first use.  mem: FM_DOUBLES doubles, 16-byte aligned.
+__device__ __forceinline__ FastMath fm_build(double* mem) {
+  double2* lt = reinterpret_cast<double2*>(mem);
+  double* et = mem + 256;
+  for (int j = threadIdx.x; j < 128; j += blockDim.x) {
+    const double c = 1.0 + ((double)j + 0.5) * (1.0 / 128.0);
+    const double inv = 1.0 / c;
+    lt[j] = make_double2(inv, -log(inv));  // ln of the centre the rounded reciprocal stands for
+  }
+  for (int j = threadIdx.x; j < 64; j += blockDim.x) et[j] = exp2((double)j * (1.0 / 64.0));
+  FastMath fm;
+  fm.logtab = lt;
+  fm.exptab = et;
+  return fm;
+}
+
+__device__ __forceinline__ double fm_log(const FastMath& fm, double s) {
+  const int hi = __double2hiint(s);
+  const int e = (hi >> 20) - 1023;
+  const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(s));
+  const double2 T = fm.logtab[(hi >> 13) & 127];
+  const double r = fma(m, T.x, -1.0);
+  double q = fma(r, -1.0 / 6.0, 1.0 / 5.0);
+  q = fma(r, q, -0.25);
+  q = fma(r, q, 1.0 / 3.0);
+  q = fma(r, q, -0.5);
+  const double lm = fma(r * r, q, r);  // ln(1 + r)
+  const double ed = (double)e;
+  return fma(ed, 0.6931471805592082, T.y) + fma(ed, 7.371002565167799e-13, lm);
+}
+
+__device__ __forceinline__ double fm_exp_neg(const FastMath& fm, double x) {
+  x = fmin(x, 700.0);
+  const double MAGIC = 6755399441055744.0;  // 1.5 * 2^52: the low word of y holds rint(-x * 64/ln2)
+  const double y = fma(x, -92.33248261689366, MAGIC);
+  const int n = __double2loint(y);
+  const double nd = y - MAGIC;
+  double r = fma(nd, -0.01083042469326756, -x);
+  r = fma(nd, -2.9815858269852933e-12, r);
+  double p = fma(r, 1.0 / 120.0, 1.0 / 24.0);
+  p = fma(r, p, 1.0 / 6.0);
+  p = fma(r, p, 0.5);
+  p = fma(r, p, 1.0);
+  p = fma(r, p, 1.0);
+  const double v = fm.exptab[n & 63] * p;
+  return __hiloint2double(__double2hiint(v) + ((n >> 6) << 20), __double2loint(v));
+}
+
 // ---- regulators --------------------------------------------------------------------------------
 struct RegParams {
   int kind;   // 0 Litim, 1 EXP_POLY
@@ -35,7 +99,7 @@ struct RegParams {
   double inv_k2;  // 1/k^2
 };
 
-__device__ __forceinline__ void regulator(const RegParams& rp, double s, double& R, double& Rdot) {
+__device__ __forceinline__ void regulator(const RegParams& rp, const FastMath& fm, double s, double& R, double& Rdot) {
   if (rp.kind == 0) {
     const bool in = s < rp.k2;
     R = in ? rp.k2 - s : 0.0;
@@ -43,56 +107,64 @@ __device__ __forceinline__ void regulator(const RegParams& rp, double s, double&
     return;
   }
   const double x = s * rp.inv_k2;
-  double r;
-  double geo;
-  if (rp.order == 1) {
-    r = rp.k2 * exp(-x);
-    geo = x;
-  } else {
-    double expo = 0.0, xi = 1.0;
-    geo = 0.0;
-    for (int i = 1; i <= rp.order; ++i) {
+  double expo = x, geo = x;
+  if (rp.order > 1) {
+    double xi = x;
+    for (int i = 2; i <= rp.order; ++i) {
       xi *= x;
       expo += xi / (double)i;
       geo += xi;
     }
-    r = rp.k2 * exp(-expo);
   }
+  const double r = rp.k2 * fm_exp_neg(fm, expo);
   R = r;
   Rdot = 2.0 * r * (1.0 + geo);
 }
 
 // ---- log-grid table look-up --------------------------------------------------------------------
+// A table row v[0..n-1] on ln q_i = lo + i h is turned, once per CTA, into per-cell cubics in shared memory:
+//   cubic mode (interp 3): cell c = stencil i0 = c, anchored at node c+1:  p(tau) = v[c+1] + tau (d1 + tau (d2 + tau d3)),
+//     the 4-point Lagrange interpolant through v[c..c+3] written in tau = t - (c+1)   (n-3 cells)
+//   linear mode (interp 1): cell c anchored at node c: p(tau) = v[c] + tau (v[c+1] - v[c])          (n-1 cells)
+// so a look-up is fm_log, one FMA, two clamps, an index, two LDS.128 and three FMAs.
 struct GridParams {
   double lo;     // ln q_0
   double inv_h;  // (n-1)/(hi-lo)
   int n;
   int interp;    // 1 or 3
+  __device__ __forceinline__ int ncell() const { return interp == 3 ? n - 3 : n - 1; }
+  __device__ __forceinline__ int off() const { return interp == 3 ? 1 : 0; }
 };
 
-// Value of the table row `v` (shared or global memory) at squared momentum s.
-__device__ __forceinline__ double table_lookup(const double* __restrict__ v, const GridParams& g, double s) {
-  const double l = 0.5 * log(s);  // s == 0 -> -inf -> clamps to the first entry
-  double t = (l - g.lo) * g.inv_h;
-  t = (t > 0.0) ? t : 0.0;  // NaN -> 0
-  const double tmax = (double)(g.n - 1);
-  t = (t < tmax) ? t : tmax;
-  if (g.interp == 3) {
-    int i0 = (int)t - 1;  // t >= 0: truncation == floor
-    i0 = max(i0, 0);
-    i0 = min(i0, g.n - 4);
-    const double sg = t - (double)i0;
-    const double a0 = sg, a1 = sg - 1.0, a2 = sg - 2.0, a3 = sg - 3.0;
-    const double L0 = -(a1 * a2 * a3) * (1.0 / 6.0);
-    const double L1 = (a0 * a2 * a3) * 0.5;
-    const double L2 = -(a0 * a1 * a3) * 0.5;
-    const double L3 = (a0 * a1 * a2) * (1.0 / 6.0);
-    return fma(v[i0], L0, fma(v[i0 + 1], L1, fma(v[i0 + 2], L2, v[i0 + 3] * L3)));
+// cells: ncell() double4, 32-byte aligned; v may live in shared or global memory.  All threads; caller synchronises.
+__device__ __forceinline__ void cells_build(double4* cells, const double* __restrict__ v, const GridParams& g) {
+  const int nc_ = g.ncell();
+  for (int c = threadIdx.x; c < nc_; c += blockDim.x) {
+    if (g.interp == 3) {
+      const double v0 = v[c], v1 = v[c + 1], v2 = v[c + 2], v3 = v[c + 3];
+      const double d1 = (-2.0 * v0 - 3.0 * v1 + 6.0 * v2 - v3) * (1.0 / 6.0);
+      const double d2 = (v0 - 2.0 * v1 + v2) * 0.5;
+      const double d3 = ((v3 - v0) + 3.0 * (v1 - v2)) * (1.0 / 6.0);
+      cells[c] = make_double4(v1, d1, d2, d3);
+    } else {
+      cells[c] = make_double4(v[c], v[c + 1] - v[c], 0.0, 0.0);
+    }
   }
-  int i = (int)t;
-  i = min(i, g.n - 2);
-  const double tau = t - (double)i;
-  return fma(v[i + 1], tau, v[i] * (1.0 - tau));
+}
+
+// Value of the table at squared momentum s.
+__device__ __forceinline__ double table_lookup(const double4* __restrict__ cells, const GridParams& g,
+                                               const FastMath& fm, double s) {
+  const double l = 0.5 * fm_log(fm, s);
+  double t = (l - g.lo) * g.inv_h;
+  t = fmax(t, 0.0);  // NaN -> 0
+  t = fmin(t, (double)(g.n - 1));
+  int c = (int)t - g.off();  // t >= 0: truncation == floor
+  c = max(c, 0);
+  c = min(c, g.ncell() - 1);
+  const double tau = t - (double)(c + g.off());
+  const double4 k = cells[c];
+  return fma(fma(fma(k.w, tau, k.z), tau, k.y), tau, k.x);
 }
 
 __device__ __forceinline__ double ipow(double x, int e) {

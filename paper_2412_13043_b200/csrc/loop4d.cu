@@ -10,10 +10,12 @@
 //       then acc += Wq_i G(q_i)^2 A.  Every lane of a warp reads the same table entry (broadcast).
 //   S5: the q-slices are combined through shared memory in fixed order.
 //
-// Three-point family.  CTA = one external configuration (|p1|, |p2|, alpha); no field axis.
-//   thread = (q, c1) pairs, strided; per pair the c2-independent part (s_a, G_A(s_a), first vertex
-//   factor, the five coefficients of P as a quartic in q.p2) is hoisted out of the c2 loop.
-//   The integrand has no phi dependence: the phi axis contributes sum_phi w.  Fixed-order block sum.
+// Three-point family.  No field axis: S3 is the evaluation.  Persistent CTAs (2 per SM) walk the external
+//   configurations (|p1|, |p2|, alpha); tables (per-cell cubics of Z_A and lambda3, log/exp tables, the radial
+//   factor wq q^3 Rdot G_A(q^2)) are built once per CTA.  thread = (q, c1) pairs, strided; per pair the
+//   c2-independent part (s_a, G_A(s_a), first vertex factor, the five coefficients of P as a quartic in q.p2)
+//   is hoisted out of the c2 loop.  The integrand has no phi dependence: the phi axis contributes sum_phi w.
+//   Fixed-order block sum per external configuration.
 #include "dfrg_device.cuh"
 #include "dfrg_internal.h"
 
@@ -48,8 +50,10 @@ __global__ void __launch_bounds__(TP_THREADS) twopoint_kernel(const TwoPointPara
   double* swq = sxq + ((nq + 1) & ~1);
   double* sxc = swq + ((nq + 1) & ~1);
   double* swc = sxc + ((nc + 1) & ~1);
-  double* sZ = swc + ((nc + 1) & ~1);
-  double* part = sZ + ((P.grid.n + 1) & ~1);  // [TP_SLICES][TP_FTILE]
+  double* sZ = swc + ((nc + 1) & ~1);                                   // raw table (TMA target)
+  double* part = sZ + ((P.grid.n + 1) & ~1);                            // [TP_SLICES][TP_FTILE]
+  double* fmmem = part + TP_SLICES * TP_FTILE;                          // [FM_DOUBLES]
+  double4* cZ = reinterpret_cast<double4*>(fmmem + FM_DOUBLES);         // per-cell cubics of Z
 
   if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
   __syncthreads();
@@ -57,7 +61,10 @@ __global__ void __launch_bounds__(TP_THREADS) twopoint_kernel(const TwoPointPara
   L.add(sxq, P.xq, nq); L.add(swq, P.wq, nq);
   L.add(sxc, P.xc, nc); L.add(swc, P.wc, nc);
   L.add(sZ, P.Z, P.grid.n);
+  const FastMath fm = fm_build(fmmem);
   stage_to_smem(L, &bar, 0);
+  cells_build(cZ, sZ, P.grid);
+  __syncthreads();
 
   const double p = P.pext[blockIdx.x];
   const double coef0 = P.coef[0], coef1 = P.coef[1];
@@ -71,8 +78,8 @@ __global__ void __launch_bounds__(TP_THREADS) twopoint_kernel(const TwoPointPara
     double s = q * q + p * p + 2.0 * q * p * c;
     s = s > 0.0 ? s : 0.0;
     double R, Rd;
-    regulator(P.reg, s, R, Rd);
-    const double D0 = table_lookup(sZ, P.grid, s) * s + R;
+    regulator(P.reg, fm, s, R, Rd);
+    const double D0 = table_lookup(cZ, P.grid, fm, s) * s + R;
     const double poly = coef0 + coef1 * (q * p * c * P.reg.inv_k2);
     inner[t] = make_double2(D0, swc[j] * sqrt((1.0 - c) * (1.0 + c)) * poly);
     dmin0 = fmin(dmin0, D0);
@@ -80,8 +87,8 @@ __global__ void __launch_bounds__(TP_THREADS) twopoint_kernel(const TwoPointPara
   for (int i = threadIdx.x; i < nq; i += TP_THREADS) {
     const double q = sxq[i], s = q * q;
     double R, Rd;
-    regulator(P.reg, s, R, Rd);
-    const double D0 = table_lookup(sZ, P.grid, s) * s + R;
+    regulator(P.reg, fm, s, R, Rd);
+    const double D0 = table_lookup(cZ, P.grid, fm, s) * s + R;
     outer[i] = make_double2(D0, swq[i] * q * q * q * Rd);
     dmin0 = fmin(dmin0, D0);
   }
@@ -128,7 +135,8 @@ __global__ void __launch_bounds__(TP_THREADS) twopoint_kernel(const TwoPointPara
 
 static size_t twopoint_smem(int nq, int nc, int ntab) {
   return (size_t)nq * nc * 16 + (size_t)nq * 16 +
-         8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((nc + 1) & ~1) + ((ntab + 1) & ~1) + TP_SLICES * TP_FTILE);
+         8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((nc + 1) & ~1) + ((ntab + 1) & ~1) + TP_SLICES * TP_FTILE + FM_DOUBLES +
+                      4 * ntab);
 }
 
 // =====================================================================================================
@@ -145,7 +153,7 @@ struct ThreePointParams {
   double *out, *dmin;
 };
 
-__global__ void __launch_bounds__(T3_THREADS) threepoint_kernel(const ThreePointParams P) {
+__global__ void __launch_bounds__(T3_THREADS, 2) threepoint_kernel(const ThreePointParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar;
   __shared__ double red[32];
@@ -160,6 +168,10 @@ __global__ void __launch_bounds__(T3_THREADS) threepoint_kernel(const ThreePoint
   double* sZA = sw2 + ((n2 + 1) & ~1);
   double* sL3 = sZA + ((nt + 1) & ~1);
   double* skap = sL3 + ((nt + 1) & ~1);  // 36
+  double* fmmem = skap + 36;             // [FM_DOUBLES]
+  double4* cZA = reinterpret_cast<double4*>(fmmem + FM_DOUBLES);
+  double4* cL3 = cZA + nt;
+  double2* qtab = reinterpret_cast<double2*>(cL3 + nt);  // [nq] (wq q^3 Rdot(q^2) G_A(q^2), D(q^2))
 
   if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
   __syncthreads();
@@ -171,91 +183,106 @@ __global__ void __launch_bounds__(T3_THREADS) threepoint_kernel(const ThreePoint
     L.add(sZA, P.ZA, nt); L.add(sL3, P.L3, nt);
     stage_to_smem(L, &bar, 0);
   }
+  const FastMath fm = fm_build(fmmem);
+  cells_build(cZA, sZA, P.grid);
+  cells_build(cL3, sL3, P.grid);
   if (threadIdx.x < 35) skap[threadIdx.x] = P.coef[threadIdx.x];
   __syncthreads();
 
-  const int e = blockIdx.x;
-  const double p1 = P.ext[3 * e], p2 = P.ext[3 * e + 1], al = P.ext[3 * e + 2];
-  double sa_, ca_;
-  sincos(al, &sa_, &ca_);
   const double ik2 = P.reg.inv_k2;
-  double scc = p1 * p1 + p2 * p2 + 2.0 * p1 * p2 * ca_;
-  scc = scc > 0.0 ? scc : 0.0;
   const double inf = __longlong_as_double(0x7ff0000000000000LL);
-  double dm = inf;
-  double acc = 0.0;
+  // ---- S3, once per CTA: the part that depends on the radial node only (not on the external point) ----
+  double dmq = inf;
+  for (int i = threadIdx.x; i < nq; i += T3_THREADS) {
+    const double q = sxq[i], sq = q * q;
+    double Rq, Rdq;
+    regulator(P.reg, fm, sq, Rq, Rdq);
+    const double Dq = table_lookup(cZA, P.grid, fm, sq) * sq + Rq;
+    qtab[i] = make_double2((swq[i] * q * q * q * Rdq) * fast_rcp(Dq), Dq);
+    dmq = fmin(dmq, Dq);
+  }
+  dmq = block_min(dmq, red);  // also publishes qtab
+  double sum_wphi = 0.0;      // the integrand has no phi dependence: the axis contributes sum_phi w
+  for (int jp = 0; jp < P.nphi; ++jp) sum_wphi += P.wphi[jp];
 
   const int npairs = nq * n1;
-  for (int t = threadIdx.x; t < npairs; t += T3_THREADS) {
-    const int i = t / n1, j1 = t - i * n1;
-    const double q = sxq[i], c1 = sx1[j1];
-    const double sq = q * q;
-    const double sin1 = sqrt((1.0 - c1) * (1.0 + c1));
-    // q-only pieces (recomputed per pair: cheap next to the c2 loop)
-    double Rq, Rdq;
-    regulator(P.reg, sq, Rq, Rdq);
-    const double Dq = table_lookup(sZA, P.grid, sq) * sq + Rq;
-    dm = fmin(dm, Dq);
-    const double wpair = (swq[i] * q * q * q * Rdq) * fast_rcp(Dq) * (sw1[j1] * sin1);
-    // (q, c1) pieces
-    const double qp1 = q * p1 * c1;
-    double s_a = sq + p1 * p1 + 2.0 * qp1;
-    s_a = s_a > 0.0 ? s_a : 0.0;
-    double Ra, Rda;
-    regulator(P.reg, s_a, Ra, Rda);
-    const double Da = table_lookup(sZA, P.grid, s_a) * s_a + Ra;
-    dm = fmin(dm, Da);
-    const double Ga = fast_rcp(Da);
-    const double lam1 = table_lookup(sL3, P.grid, (p1 * p1 + sq + s_a) * (1.0 / 3.0));
-    // P as a quartic in z = q.p2/k^2: gam[c] = sum_{a+b<=4-c} kap_abc X^a Y^b
-    const double X = sq * ik2, Y = qp1 * ik2;
-    double gam[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-    {
-      int idx = 0;
-      double Xa = 1.0;
+  // persistent: this CTA owns the external points e = blockIdx.x, blockIdx.x + gridDim.x, ...
+  for (int e = blockIdx.x; e < P.n_ext; e += gridDim.x) {
+    const double p1 = P.ext[3 * e], p2 = P.ext[3 * e + 1], al = P.ext[3 * e + 2];
+    double sa_, ca_;
+    sincos(al, &sa_, &ca_);
+    double scc = p1 * p1 + p2 * p2 + 2.0 * p1 * p2 * ca_;
+    scc = scc > 0.0 ? scc : 0.0;
+    double dm = dmq;
+    double acc = 0.0;
+    for (int t = threadIdx.x; t < npairs; t += T3_THREADS) {
+      const int i = t / n1, j1 = t - i * n1;
+      const double q = sxq[i], c1 = sx1[j1];
+      const double sq = q * q;
+      const double sin1 = sqrt((1.0 - c1) * (1.0 + c1));
+      const double wpair = qtab[i].x * (sw1[j1] * sin1);
+      // (q, c1) pieces
+      const double qp1 = q * p1 * c1;
+      double s_a = sq + p1 * p1 + 2.0 * qp1;
+      s_a = s_a > 0.0 ? s_a : 0.0;
+      double Ra, Rda;
+      regulator(P.reg, fm, s_a, Ra, Rda);
+      const double Da = table_lookup(cZA, P.grid, fm, s_a) * s_a + Ra;
+      dm = fmin(dm, Da);
+      const double Ga = fast_rcp(Da);
+      const double lam1 = table_lookup(cL3, P.grid, fm, (p1 * p1 + sq + s_a) * (1.0 / 3.0));
+      // P as a quartic in z = q.p2/k^2: gam[c] = sum_{a+b<=4-c} kap_abc X^a Y^b
+      const double X = sq * ik2, Y = qp1 * ik2;
+      double gam[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      {
+        int idx = 0;
+        double Xa = 1.0;
 #pragma unroll
-      for (int a = 0; a <= 4; ++a) {
-        double XaYb = Xa;
+        for (int a = 0; a <= 4; ++a) {
+          double XaYb = Xa;
 #pragma unroll
-        for (int b = 0; b <= 4 - a; ++b) {
+          for (int b = 0; b <= 4 - a; ++b) {
 #pragma unroll
-          for (int c = 0; c <= 4 - a - b; ++c) gam[c] = fma(skap[idx++], XaYb, gam[c]);
-          XaYb *= Y;
+            for (int c = 0; c <= 4 - a - b; ++c) gam[c] = fma(skap[idx++], XaYb, gam[c]);
+            XaYb *= Y;
+          }
+          Xa *= X;
         }
-        Xa *= X;
       }
+      const double zc = q * p2 * ca_ * c1;  // q.p2 = zc + zs * c2
+      const double zs = q * p2 * sa_ * sin1;
+      const double sb0 = sq + p2 * p2;      // s_b = sb0 - 2 q.p2
+      const double l20 = p2 * p2 + sq, l30 = scc + s_a;
+      double acc2 = 0.0;
+#pragma unroll 2
+      for (int j2 = 0; j2 < n2; ++j2) {
+        const double qp2 = fma(zs, sx2[j2], zc);
+        double s_b = fma(-2.0, qp2, sb0);
+        s_b = s_b > 0.0 ? s_b : 0.0;
+        double Rb, Rdb;
+        regulator(P.reg, fm, s_b, Rb, Rdb);
+        const double Db = table_lookup(cZA, P.grid, fm, s_b) * s_b + Rb;
+        dm = fmin(dm, Db);
+        const double lam2 = table_lookup(cL3, P.grid, fm, (l20 + s_b) * (1.0 / 3.0));
+        const double lam3 = table_lookup(cL3, P.grid, fm, (l30 + s_b) * (1.0 / 3.0));
+        const double z = qp2 * ik2;
+        const double poly = fma(fma(fma(fma(gam[4], z, gam[3]), z, gam[2]), z, gam[1]), z, gam[0]);
+        acc2 = fma(sw2[j2], fast_rcp(Db) * (lam2 * lam3) * poly, acc2);
+      }
+      acc = fma(wpair, (Ga * lam1) * acc2, acc);
     }
-    const double zc = q * p2 * ca_ * c1;       // q.p2 = zc + zs * c2
-    const double zs = q * p2 * sa_ * sin1;
-    double acc2 = 0.0;
-    for (int j2 = 0; j2 < n2; ++j2) {
-      const double qp2 = fma(zs, sx2[j2], zc);
-      double s_b = sq + p2 * p2 - 2.0 * qp2;
-      s_b = s_b > 0.0 ? s_b : 0.0;
-      double Rb, Rdb;
-      regulator(P.reg, s_b, Rb, Rdb);
-      const double Db = table_lookup(sZA, P.grid, s_b) * s_b + Rb;
-      dm = fmin(dm, Db);
-      const double lam2 = table_lookup(sL3, P.grid, (p2 * p2 + sq + s_b) * (1.0 / 3.0));
-      const double lam3 = table_lookup(sL3, P.grid, (scc + s_a + s_b) * (1.0 / 3.0));
-      const double z = qp2 * ik2;
-      const double poly = fma(fma(fma(fma(gam[4], z, gam[3]), z, gam[2]), z, gam[1]), z, gam[0]);
-      acc2 = fma(sw2[j2], fast_rcp(Db) * (lam2 * lam3) * poly, acc2);
+    const double total = block_sum(acc, red);
+    const double dmin_b = P.dmin ? block_min(dm, red) : 0.0;
+    if (threadIdx.x == 0) {
+      P.out[e] = P.prefactor * sum_wphi * total;
+      if (P.dmin) P.dmin[e] = dmin_b * ik2;
     }
-    acc = fma(wpair, (Ga * lam1) * acc2, acc);
-  }
-  const double total = block_sum(acc, red);
-  const double dmin_b = P.dmin ? block_min(dm, red) : 0.0;
-  if (threadIdx.x == 0) {
-    double sum_wphi = 0.0;  // the integrand has no phi dependence: the axis contributes sum_phi w
-    for (int jp = 0; jp < P.nphi; ++jp) sum_wphi += P.wphi[jp];
-    P.out[e] = P.prefactor * sum_wphi * total;
-    if (P.dmin) P.dmin[e] = dmin_b * ik2;
   }
 }
 
 static size_t threepoint_smem(int nq, int n1, int n2, int nt) {
-  return 8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((n1 + 1) & ~1) + 2 * ((n2 + 1) & ~1) + 2 * ((nt + 1) & ~1) + 36);
+  return 8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((n1 + 1) & ~1) + 2 * ((n2 + 1) & ~1) + 2 * ((nt + 1) & ~1) + 36 +
+                      FM_DOUBLES + 8 * nt + 2 * nq);
 }
 
 // =====================================================================================================
@@ -293,7 +320,7 @@ static void fill_common(const dfrg_regulator& r, const dfrg_table& t, RegParams*
 }
 
 static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext, const double* ext,
-                         double* out, double* dmin, cudaStream_t stream) {
+                         double* out, double* dmin, int sm_count, cudaStream_t stream) {
   if (D->family == DFRG_LOOP_TWOPOINT) {
     TwoPointParams P;
     P.nq = D->q.n; P.nc = D->cos1.n; P.n_field = n_field; P.n_ext = n_ext;
@@ -317,7 +344,8 @@ static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m
   const size_t smem = threepoint_smem(P.nq, P.n1, P.n2, P.grid.n);
   cudaError_t e = cudaFuncSetAttribute(threepoint_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return check_cuda(e);
-  threepoint_kernel<<<n_ext, T3_THREADS, smem, stream>>>(P);
+  const int grid = n_ext < 2 * sm_count ? n_ext : 2 * sm_count;  // persistent: 2 CTAs per SM
+  threepoint_kernel<<<grid, T3_THREADS, smem, stream>>>(P);
   return check_cuda(cudaGetLastError());
 }
 
@@ -329,16 +357,18 @@ extern "C" int dfrg_integrate_loop4d(const dfrg_loop4d_desc* D, int n_field, con
                                      const double* ext, double* out, double* dmin, void* cuda_stream) {
   int rc = loop4d_validate(D, n_field, m2, n_ext, ext, out);
   if (rc != DFRG_OK) return rc;
-  rc = require_sm100(nullptr);
+  int sms = 0;
+  rc = require_sm100(&sms);
   if (rc != DFRG_OK) return rc;
-  return loop4d_launch(D, n_field, m2, n_ext, ext, out, dmin, (cudaStream_t)cuda_stream);
+  return loop4d_launch(D, n_field, m2, n_ext, ext, out, dmin, sms, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int dfrg_integrate_loop4d_host(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext,
                                           const double* ext, double* out, double* dmin) {
   int rc = loop4d_validate(D, n_field, m2, n_ext, ext, out);
   if (rc != DFRG_OK) return rc;
-  rc = require_sm100(nullptr);
+  int sms = 0;
+  rc = require_sm100(&sms);
   if (rc != DFRG_OK) return rc;
   Arena& A = thread_arena();
   const bool two = D->family == DFRG_LOOP_TWOPOINT;
@@ -361,7 +391,7 @@ extern "C" int dfrg_integrate_loop4d_host(const dfrg_loop4d_desc* D, int n_field
   double* d_out = A.reserve(ne * nf);
   double* d_dmin = dmin ? A.reserve(ne * nf) : nullptr;
   if (A.status() != DFRG_OK) return A.status();
-  rc = loop4d_launch(&Dd, n_field, d_m2, n_ext, d_ext, d_out, d_dmin, A.stream());
+  rc = loop4d_launch(&Dd, n_field, d_m2, n_ext, d_ext, d_out, d_dmin, sms, A.stream());
   if (rc != DFRG_OK) return rc;
   A.fetch(out, d_out, ne * nf);
   if (dmin) A.fetch(dmin, d_dmin, ne * nf);

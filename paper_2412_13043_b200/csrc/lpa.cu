@@ -38,6 +38,7 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_kernel(const LpaParams P) {
   double2* tab = reinterpret_cast<double2*>(smem_raw);                 // [n_pairs] (D0, W)
   double* sx = reinterpret_cast<double*>(smem_raw + (size_t)n_pairs * 16);  // [nq]
   double* sw = sx + ((P.nq + 1) & ~1);                                      // [nq]
+  const FastMath fm = fm_build(sw + ((P.nq + 1) & ~1));                     // [FM_DOUBLES]
 
   if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
   __syncthreads();
@@ -56,7 +57,7 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_kernel(const LpaParams P) {
     const double s = wn * wn + q * q;
     const double sR = P.reg_arg4d ? s : q * q;
     double R, Rd;
-    regulator(P.reg, sR, R, Rd);
+    regulator(P.reg, fm, sR, R, Rd);
     const double D0 = s + R;
     const double fold = (n > 0) ? 2.0 : 1.0;
     tab[t] = make_double2(D0, fold * (sw[i] * ipow(q, P.d - 1) * Rd));
@@ -114,7 +115,7 @@ static int lpa_launch(const dfrg_lpa_desc* D, int n_field, const double* rho, co
   P.xq = D->q.x; P.wq = D->q.w; P.rho = rho; P.u = u; P.du = du;
   P.flow = flow; P.chan = chan; P.dmin = dmin;
   const int n_terms = (D->T > 0.0) ? D->n_max + 1 : 1;
-  const size_t smem = (size_t)n_terms * D->q.n * 16 + 2 * (size_t)((D->q.n + 1) & ~1) * 8;
+  const size_t smem = (size_t)n_terms * D->q.n * 16 + (2 * (size_t)((D->q.n + 1) & ~1) + FM_DOUBLES) * 8;
   cudaError_t e = cudaFuncSetAttribute(lpa_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return check_cuda(e);
   const int grid = (n_field + LPA_FTILE - 1) / LPA_FTILE;

@@ -47,11 +47,12 @@ struct Mats3dParams {
 
 // ---- (1) boson rows --------------------------------------------------------------------------------
 __global__ void __launch_bounds__(M3_PRE_THREADS) mats3d_phi_rows_kernel(const Mats3dParams P) {
-  __shared__ double srow[1024];
+  __shared__ __align__(32) double4 cells[1024];
+  __shared__ __align__(16) double fmmem[FM_DOUBLES];
   __shared__ double red[32];
   const int m = blockIdx.x, e = blockIdx.y;
-  const int nt = P.grid.n;
-  for (int i = threadIdx.x; i < nt; i += M3_PRE_THREADS) srow[i] = P.Zphi[(size_t)m * nt + i];
+  const FastMath fm = fm_build(fmmem);
+  cells_build(cells, P.Zphi + (size_t)m * P.grid.n, P.grid);
   __syncthreads();
   const double p = P.pext[e];
   const double om = 2.0 * 3.14159265358979323846 * (double)m * P.T;
@@ -65,8 +66,8 @@ __global__ void __launch_bounds__(M3_PRE_THREADS) mats3d_phi_rows_kernel(const M
     r2 = r2 > 0.0 ? r2 : 0.0;
     const double sphi = om * om + r2;
     double R, Rd;
-    regulator(P.reg, sphi, R, Rd);
-    const double D0 = table_lookup(srow, P.grid, r2) * sphi + R;
+    regulator(P.reg, fm, sphi, R, Rd);
+    const double D0 = table_lookup(cells, P.grid, fm, r2) * sphi + R;
     dst[t] = D0;
     dmin = fmin(dmin, D0);
   }
@@ -77,18 +78,22 @@ __global__ void __launch_bounds__(M3_PRE_THREADS) mats3d_phi_rows_kernel(const M
 
 // ---- (2) fermion line --------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) mats3d_psi_kernel(const Mats3dParams P) {
+  __shared__ __align__(32) double4 cells[1024];
+  __shared__ __align__(16) double fmmem[FM_DOUBLES];
   __shared__ double red[32];
   const int it = blockIdx.x, n = it - P.n_max;
   const int nbar = n >= 0 ? n : -n - 1;
   const double nun = (2.0 * n + 1.0) * 3.14159265358979323846 * P.T;
-  const double* row = P.Zpsi + (size_t)nbar * P.grid.n;
+  const FastMath fm = fm_build(fmmem);
+  cells_build(cells, P.Zpsi + (size_t)nbar * P.grid.n, P.grid);
+  __syncthreads();
   double dmin = __longlong_as_double(0x7ff0000000000000LL);
   for (int i = threadIdx.x; i < P.nq; i += 128) {
     const double q = P.xq[i];
     const double spsi = nun * nun + q * q;
     double R, Rd;
-    regulator(P.reg, spsi, R, Rd);
-    const double D0 = table_lookup(row, P.grid, q * q) * spsi + R;
+    regulator(P.reg, fm, spsi, R, Rd);
+    const double D0 = table_lookup(cells, P.grid, fm, q * q) * spsi + R;
     P.psi[(size_t)it * P.psi_stride + i] = make_double2(D0, P.wq[i] * q * q * Rd);
     dmin = fmin(dmin, D0);
   }
