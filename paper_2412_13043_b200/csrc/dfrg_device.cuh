@@ -40,11 +40,38 @@ __device__ __forceinline__ double fast_rcp(double d) {
 struct FastMath {
   const double2* logtab;  // [128] (1/c_j, ln c_j)
   const double* exptab;   // [64]  2^(j/64)
+  const double* k;        // FastMathConsts::c inside the kernel parameters
 };
+// Polynomial coefficients travel inside the kernel parameter struct (constant bank c[0x0]) so that DFMA reads
+// them as constant operands; as compile-time literals the compiler rebuilds each 64-bit immediate in uniform
+// registers (two UMOV) before every use.
+struct FastMathConsts {
+  double c[16];
+};
+inline FastMathConsts fm_consts() {
+  FastMathConsts k = {{
+      -1.0 / 6.0, 1.0 / 5.0, -0.25, 1.0 / 3.0, -0.5,  // 0-4  ln(1+r) = r + r^2 (-1/2 + r/3 - r^2/4 + r^3/5 - r^4/6)
+      0.6931471805592082, 7.371002565167799e-13,      // 5,6  ln2 hi / lo (40-bit split)
+      -92.33248261689366, 6755399441055744.0,         // 7,8  -64/ln2, 1.5 * 2^52
+      -0.01083042469326756, -2.9815858269852933e-12,  // 9,10 -(ln2/64) hi / lo (32-bit split)
+      1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0, 0.5, 1.0}};  // 11-15 exp series
+  return k;
+}
+// Branch-free clamps as one DSETP + two SEL (CUDA's fmin/fmax add NaN fix-ups: seven instructions each).
+__device__ __forceinline__ double clamp_lo(double x, double lo) {  // x > lo ? x : lo   (NaN -> lo)
+  double r;
+  asm("{\n.reg .pred p;\nsetp.gt.f64 p, %1, %2;\nselp.f64 %0, %1, %2, p;\n}" : "=d"(r) : "d"(x), "d"(lo));
+  return r;
+}
+__device__ __forceinline__ double clamp_hi(double x, double hi) {  // x < hi ? x : hi   (NaN -> hi)
+  double r;
+  asm("{\n.reg .pred p;\nsetp.lt.f64 p, %1, %2;\nselp.f64 %0, %1, %2, p;\n}" : "=d"(r) : "d"(x), "d"(hi));
+  return r;
+}
 constexpr int FM_DOUBLES = 2 * 128 + 64;
 
 // All threads of the CTA; the caller synchronises before first use.  mem: FM_DOUBLES doubles, 16-byte aligned.
-__device__ __forceinline__ FastMath fm_build(double* mem) {
+__device__ __forceinline__ FastMath fm_build(double* mem, const FastMathConsts& consts) {
   double2* lt = reinterpret_cast<double2*>(mem);
   double* et = mem + 256;
   for (int j = threadIdx.x; j < 128; j += blockDim.x) {
@@ -56,6 +83,7 @@ __device__ __forceinline__ FastMath fm_build(double* mem) {
   FastMath fm;
   fm.logtab = lt;
   fm.exptab = et;
+  fm.k = consts.c;
   return fm;
 }
 
@@ -65,28 +93,28 @@ __device__ __forceinline__ double fm_log(const FastMath& fm, double s) {
   const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(s));
   const double2 T = fm.logtab[(hi >> 13) & 127];
   const double r = fma(m, T.x, -1.0);
-  double q = fma(r, -1.0 / 6.0, 1.0 / 5.0);
-  q = fma(r, q, -0.25);
-  q = fma(r, q, 1.0 / 3.0);
-  q = fma(r, q, -0.5);
+  double q = fma(r, fm.k[0], fm.k[1]);
+  q = fma(r, q, fm.k[2]);
+  q = fma(r, q, fm.k[3]);
+  q = fma(r, q, fm.k[4]);
   const double lm = fma(r * r, q, r);  // ln(1 + r)
   const double ed = (double)e;
-  return fma(ed, 0.6931471805592082, T.y) + fma(ed, 7.371002565167799e-13, lm);
+  return fma(ed, fm.k[5], T.y) + fma(ed, fm.k[6], lm);
 }
 
 __device__ __forceinline__ double fm_exp_neg(const FastMath& fm, double x) {
-  x = fmin(x, 700.0);
-  const double MAGIC = 6755399441055744.0;  // 1.5 * 2^52: the low word of y holds rint(-x * 64/ln2)
-  const double y = fma(x, -92.33248261689366, MAGIC);
+  x = clamp_hi(x, 700.0);
+  const double MAGIC = fm.k[8];  // 1.5 * 2^52: the low word of y holds rint(-x * 64/ln2)
+  const double y = fma(x, fm.k[7], MAGIC);
   const int n = __double2loint(y);
   const double nd = y - MAGIC;
-  double r = fma(nd, -0.01083042469326756, -x);
-  r = fma(nd, -2.9815858269852933e-12, r);
-  double p = fma(r, 1.0 / 120.0, 1.0 / 24.0);
-  p = fma(r, p, 1.0 / 6.0);
-  p = fma(r, p, 0.5);
-  p = fma(r, p, 1.0);
-  p = fma(r, p, 1.0);
+  double r = fma(nd, fm.k[9], -x);
+  r = fma(nd, fm.k[10], r);
+  double p = fma(r, fm.k[11], fm.k[12]);
+  p = fma(r, p, fm.k[13]);
+  p = fma(r, p, fm.k[14]);
+  p = fma(r, p, fm.k[15]);
+  p = fma(r, p, fm.k[15]);
   const double v = fm.exptab[n & 63] * p;
   return __hiloint2double(__double2hiint(v) + ((n >> 6) << 20), __double2loint(v));
 }
@@ -157,8 +185,8 @@ __device__ __forceinline__ double table_lookup(const double4* __restrict__ cells
                                                const FastMath& fm, double s) {
   const double l = 0.5 * fm_log(fm, s);
   double t = (l - g.lo) * g.inv_h;
-  t = fmax(t, 0.0);  // NaN -> 0
-  t = fmin(t, (double)(g.n - 1));
+  t = clamp_lo(t, 0.0);  // NaN -> 0
+  t = clamp_hi(t, (double)(g.n - 1));
   int c = (int)t - g.off();  // t >= 0: truncation == floor
   c = max(c, 0);
   c = min(c, g.ncell() - 1);

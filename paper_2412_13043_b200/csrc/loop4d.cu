@@ -34,6 +34,7 @@ struct TwoPointParams {
   double prefactor;
   RegParams reg;
   GridParams grid;
+  FastMathConsts fmc;
   const double *xq, *wq, *xc, *wc, *Z, *coef, *m2, *pext;
   double *out, *dmin;
 };
@@ -61,7 +62,7 @@ __global__ void __launch_bounds__(TP_THREADS) twopoint_kernel(const TwoPointPara
   L.add(sxq, P.xq, nq); L.add(swq, P.wq, nq);
   L.add(sxc, P.xc, nc); L.add(swc, P.wc, nc);
   L.add(sZ, P.Z, P.grid.n);
-  const FastMath fm = fm_build(fmmem);
+  const FastMath fm = fm_build(fmmem, P.fmc);
   stage_to_smem(L, &bar, 0);
   cells_build(cZ, sZ, P.grid);
   __syncthreads();
@@ -76,7 +77,7 @@ __global__ void __launch_bounds__(TP_THREADS) twopoint_kernel(const TwoPointPara
     const int i = t / nc, j = t - i * nc;
     const double q = sxq[i], c = sxc[j];
     double s = q * q + p * p + 2.0 * q * p * c;
-    s = s > 0.0 ? s : 0.0;
+    s = clamp_lo(s, 0.0);
     double R, Rd;
     regulator(P.reg, fm, s, R, Rd);
     const double D0 = table_lookup(cZ, P.grid, fm, s) * s + R;
@@ -149,10 +150,12 @@ struct ThreePointParams {
   double prefactor;
   RegParams reg;
   GridParams grid;
+  FastMathConsts fmc;
   const double *xq, *wq, *x1, *w1, *x2, *w2, *wphi, *ZA, *L3, *coef, *ext;
   double *out, *dmin;
 };
 
+template <bool WANT_DMIN>
 __global__ void __launch_bounds__(T3_THREADS, 2) threepoint_kernel(const ThreePointParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar;
@@ -183,7 +186,7 @@ __global__ void __launch_bounds__(T3_THREADS, 2) threepoint_kernel(const ThreePo
     L.add(sZA, P.ZA, nt); L.add(sL3, P.L3, nt);
     stage_to_smem(L, &bar, 0);
   }
-  const FastMath fm = fm_build(fmmem);
+  const FastMath fm = fm_build(fmmem, P.fmc);
   cells_build(cZA, sZA, P.grid);
   cells_build(cL3, sL3, P.grid);
   if (threadIdx.x < 35) skap[threadIdx.x] = P.coef[threadIdx.x];
@@ -224,11 +227,11 @@ __global__ void __launch_bounds__(T3_THREADS, 2) threepoint_kernel(const ThreePo
       // (q, c1) pieces
       const double qp1 = q * p1 * c1;
       double s_a = sq + p1 * p1 + 2.0 * qp1;
-      s_a = s_a > 0.0 ? s_a : 0.0;
+      s_a = clamp_lo(s_a, 0.0);
       double Ra, Rda;
       regulator(P.reg, fm, s_a, Ra, Rda);
       const double Da = table_lookup(cZA, P.grid, fm, s_a) * s_a + Ra;
-      dm = fmin(dm, Da);
+      if (WANT_DMIN) dm = fmin(dm, Da);
       const double Ga = fast_rcp(Da);
       const double lam1 = table_lookup(cL3, P.grid, fm, (p1 * p1 + sq + s_a) * (1.0 / 3.0));
       // P as a quartic in z = q.p2/k^2: gam[c] = sum_{a+b<=4-c} kap_abc X^a Y^b
@@ -258,11 +261,11 @@ __global__ void __launch_bounds__(T3_THREADS, 2) threepoint_kernel(const ThreePo
       for (int j2 = 0; j2 < n2; ++j2) {
         const double qp2 = fma(zs, sx2[j2], zc);
         double s_b = fma(-2.0, qp2, sb0);
-        s_b = s_b > 0.0 ? s_b : 0.0;
+        s_b = clamp_lo(s_b, 0.0);
         double Rb, Rdb;
         regulator(P.reg, fm, s_b, Rb, Rdb);
         const double Db = table_lookup(cZA, P.grid, fm, s_b) * s_b + Rb;
-        dm = fmin(dm, Db);
+        if (WANT_DMIN) dm = fmin(dm, Db);
         const double lam2 = table_lookup(cL3, P.grid, fm, (l20 + s_b) * (1.0 / 3.0));
         const double lam3 = table_lookup(cL3, P.grid, fm, (l30 + s_b) * (1.0 / 3.0));
         const double z = qp2 * ik2;
@@ -272,10 +275,10 @@ __global__ void __launch_bounds__(T3_THREADS, 2) threepoint_kernel(const ThreePo
       acc = fma(wpair, (Ga * lam1) * acc2, acc);
     }
     const double total = block_sum(acc, red);
-    const double dmin_b = P.dmin ? block_min(dm, red) : 0.0;
+    const double dmin_b = WANT_DMIN ? block_min(dm, red) : 0.0;
     if (threadIdx.x == 0) {
       P.out[e] = P.prefactor * sum_wphi * total;
-      if (P.dmin) P.dmin[e] = dmin_b * ik2;
+      if (WANT_DMIN) P.dmin[e] = dmin_b * ik2;
     }
   }
 }
@@ -326,6 +329,7 @@ static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m
     P.nq = D->q.n; P.nc = D->cos1.n; P.n_field = n_field; P.n_ext = n_ext;
     P.prefactor = D->prefactor;
     fill_common(D->reg, D->tab[0], &P.reg, &P.grid);
+    P.fmc = fm_consts();
     P.xq = D->q.x; P.wq = D->q.w; P.xc = D->cos1.x; P.wc = D->cos1.w; P.Z = D->tab[0].v;
     P.coef = D->coef; P.m2 = m2; P.pext = ext; P.out = out; P.dmin = dmin;
     const size_t smem = twopoint_smem(P.nq, P.nc, P.grid.n);
@@ -339,13 +343,15 @@ static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m
   P.nq = D->q.n; P.n1 = D->cos1.n; P.n2 = D->cos2.n; P.nphi = D->phi.n; P.n_ext = n_ext;
   P.prefactor = D->prefactor;
   fill_common(D->reg, D->tab[0], &P.reg, &P.grid);
+  P.fmc = fm_consts();
   P.xq = D->q.x; P.wq = D->q.w; P.x1 = D->cos1.x; P.w1 = D->cos1.w; P.x2 = D->cos2.x; P.w2 = D->cos2.w; P.wphi = D->phi.w;
   P.ZA = D->tab[0].v; P.L3 = D->tab[2].v; P.coef = D->coef; P.ext = ext; P.out = out; P.dmin = dmin;
   const size_t smem = threepoint_smem(P.nq, P.n1, P.n2, P.grid.n);
-  cudaError_t e = cudaFuncSetAttribute(threepoint_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  auto kern = dmin ? threepoint_kernel<true> : threepoint_kernel<false>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return check_cuda(e);
   const int grid = n_ext < 2 * sm_count ? n_ext : 2 * sm_count;  // persistent: 2 CTAs per SM
-  threepoint_kernel<<<grid, T3_THREADS, smem, stream>>>(P);
+  kern<<<grid, T3_THREADS, smem, stream>>>(P);
   return check_cuda(cudaGetLastError());
 }
 

@@ -23,6 +23,7 @@ struct LpaParams {
   int d, n_max, reg_arg4d, nq, n_field;
   double T, N, prefactor;
   RegParams reg;
+  FastMathConsts fmc;
   const double *xq, *wq, *rho, *u, *du;
   double *flow, *chan, *dmin;
 };
@@ -38,7 +39,7 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_kernel(const LpaParams P) {
   double2* tab = reinterpret_cast<double2*>(smem_raw);                 // [n_pairs] (D0, W)
   double* sx = reinterpret_cast<double*>(smem_raw + (size_t)n_pairs * 16);  // [nq]
   double* sw = sx + ((P.nq + 1) & ~1);                                      // [nq]
-  const FastMath fm = fm_build(sw + ((P.nq + 1) & ~1));                     // [FM_DOUBLES]
+  const FastMath fm = fm_build(sw + ((P.nq + 1) & ~1), P.fmc);                     // [FM_DOUBLES]
 
   if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
   __syncthreads();
@@ -112,6 +113,7 @@ static int lpa_launch(const dfrg_lpa_desc* D, int n_field, const double* rho, co
   P.T = D->T; P.N = D->N; P.prefactor = D->prefactor;
   P.reg.kind = D->reg.kind; P.reg.order = D->reg.order;
   P.reg.k2 = D->reg.k * D->reg.k; P.reg.inv_k2 = 1.0 / P.reg.k2;
+  P.fmc = fm_consts();
   P.xq = D->q.x; P.wq = D->q.w; P.rho = rho; P.u = u; P.du = du;
   P.flow = flow; P.chan = chan; P.dmin = dmin;
   const int n_terms = (D->T > 0.0) ? D->n_max + 1 : 1;

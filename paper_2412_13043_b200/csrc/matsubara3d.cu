@@ -36,6 +36,7 @@ struct Mats3dParams {
   double T, prefactor;
   RegParams reg;
   GridParams grid;
+  FastMathConsts fmc;
   const double *xq, *wq, *xc, *wc, *Zpsi, *Zphi, *coef, *m2psi, *m2phi, *pext;
   double *d0phi;    // [n_p][n_rows][row_stride]
   double *rowmin;   // [n_p][n_rows]
@@ -51,7 +52,7 @@ __global__ void __launch_bounds__(M3_PRE_THREADS) mats3d_phi_rows_kernel(const M
   __shared__ __align__(16) double fmmem[FM_DOUBLES];
   __shared__ double red[32];
   const int m = blockIdx.x, e = blockIdx.y;
-  const FastMath fm = fm_build(fmmem);
+  const FastMath fm = fm_build(fmmem, P.fmc);
   cells_build(cells, P.Zphi + (size_t)m * P.grid.n, P.grid);
   __syncthreads();
   const double p = P.pext[e];
@@ -63,7 +64,7 @@ __global__ void __launch_bounds__(M3_PRE_THREADS) mats3d_phi_rows_kernel(const M
     const int i = t / P.nc, jc = t - i * P.nc;
     const double q = P.xq[i], c = P.xc[jc];
     double r2 = p * p + q * q - 2.0 * p * q * c;
-    r2 = r2 > 0.0 ? r2 : 0.0;
+    r2 = clamp_lo(r2, 0.0);
     const double sphi = om * om + r2;
     double R, Rd;
     regulator(P.reg, fm, sphi, R, Rd);
@@ -84,7 +85,7 @@ __global__ void __launch_bounds__(128) mats3d_psi_kernel(const Mats3dParams P) {
   const int it = blockIdx.x, n = it - P.n_max;
   const int nbar = n >= 0 ? n : -n - 1;
   const double nun = (2.0 * n + 1.0) * 3.14159265358979323846 * P.T;
-  const FastMath fm = fm_build(fmmem);
+  const FastMath fm = fm_build(fmmem, P.fmc);
   cells_build(cells, P.Zpsi + (size_t)nbar * P.grid.n, P.grid);
   __syncthreads();
   double dmin = __longlong_as_double(0x7ff0000000000000LL);
@@ -369,6 +370,7 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   P.reg.kind = D->reg.kind; P.reg.order = D->reg.order; P.reg.k2 = D->reg.k * D->reg.k; P.reg.inv_k2 = 1.0 / P.reg.k2;
   P.grid.lo = D->tab_psi.lnq_lo; P.grid.n = D->tab_psi.n_q; P.grid.interp = D->tab_psi.interp;
   P.grid.inv_h = (double)(P.grid.n - 1) / (D->tab_psi.lnq_hi - D->tab_psi.lnq_lo);
+  P.fmc = fm_consts();
   P.xq = D->q.x; P.wq = D->q.w; P.xc = D->cos1.x; P.wc = D->cos1.w;
   P.Zpsi = D->tab_psi.v; P.Zphi = D->tab_phi.v; P.coef = D->coef;
   P.m2psi = m2_psi; P.m2phi = m2_phi; P.pext = p; P.out = out; P.dmin = dmin;
