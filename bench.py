@@ -33,16 +33,21 @@ FP64_LANES_PER_SM = 64
 
 
 def cfg4_counts(c, rules):
-    n_out = c["pext"].size * c["n_jext"] * c["m2psi"].size
+    n_p, n_j, n_f = c["pext"].size, c["n_jext"], c["m2psi"].size
+    n_out = n_p * n_j * n_f
     n_terms = 2 * c["n_max"] + 1
     nq, nc = rules["q"][0].size, rules["c"][0].size
     evals = n_out * n_terms * nq * nc
-    # algorithmic FP64 work: 4.25 FP64-pipe instructions per nominal evaluation (four-way
-    # batched inversion: 4 DADD + 6 DMUL + 7 DFMA per 4 evaluations) + 8 per (output, n, q) for the fermion line.
-    # flops = DFMA-slot equivalents (2 per instruction); strict = FMA 2, add/mul 1 (6 per evaluation + 11).
-    instr = n_out * n_terms * nq * (4.25 * nc + 8)
-    strict = n_out * n_terms * nq * (6 * nc + 11)
-    return n_out, evals, (2.0 * instr, float(strict))
+    # algorithmic FP64 work of the moment factorisation, per (p, radial node, field point):
+    #   (n_j + n_max) nc x 8   angular moments of the boson line   (DADD, 3 DFMA reciprocal, 4 DFMA)
+    # + (n_max + 1) x 5        fermion line G_psi^2                (DADD, 3 DFMA, DMUL)
+    # + n_j n_terms x 5        acc_j += H (beta' . M)              (DMUL, 3 DFMA, DFMA)
+    # flops = DFMA-slot equivalents (2 per instruction); strict = FMA 2, add/mul 1.
+    rows = n_j + c["n_max"]
+    per_pif = rows * nc * 8 + (c["n_max"] + 1) * 5 + n_j * n_terms * 5
+    per_pif_strict = rows * nc * 15 + (c["n_max"] + 1) * 8 + n_j * n_terms * 9
+    units = n_p * nq * n_f
+    return n_out, evals, (2.0 * units * per_pif, float(units * per_pif_strict))
 
 
 class ClockSampler:
@@ -329,10 +334,10 @@ def main():
                        "parallelism": "external momenta sharded over GPUs (64 per GPU), no collective",
                        "integrals_per_step_per_gpu": n_out, "nominal_evals_per_step_per_gpu": evals},
             "integrals_per_s": world * n_out / (ms * 1e-3),
-            "clocks": clocks, "gpu_launches": 3 * args.steps,  # phi-rows pre-pass, psi pre-pass, main kernel per step
+            "clocks": clocks, "gpu_launches": 4 * args.steps,  # phi-rows pre-pass, psi pre-pass, moment kernel, fix-up kernel per step
             "e2e": {"value": world * evals / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_s * 1e3, "s1_host_ms": t_s1 * 1e3},
-            "roofline": {"bound": "alu", "kernel": "mats3d_main_kernel (+ its two pre-pass kernels, timed together)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+            "roofline": {"bound": "alu", "kernel": "mats3d_moment_kernel (+ the two pre-pass kernels and the fix-up kernel, timed together)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                          "frac": achieved / peak, "traffic": None,
                          "achieved_kind": "algorithmic FP64 instructions x 2 (DFMA-slot equivalents) / event time",
                          "achieved_strict": flops_strict / (ms_local * 1e-3) * 1e-12,

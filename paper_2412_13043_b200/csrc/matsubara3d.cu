@@ -44,6 +44,13 @@ struct Mats3dParams {
   double *psimin;   // [2 n_max + 1]
   int psi_stride;
   double *out, *dmin;
+  // moment path (mats3d_moment_kernel): D0phi is laid out [p][i][m][c] in chunks of chunk_stride doubles
+  int phi_layout;    // 0: [p][m][i*nc + c] (row_stride), 1: [p][i][m*nc + c] (chunk_stride)
+  int chunk_stride;
+  int tile_fields;   // field points per CTA tile of the moment kernel
+  int max_slots;     // partial sums per (field tile, p) in part[]
+  int grid_main;     // CTAs of the moment kernel (the fix-up kernel re-derives the unit ownership from it)
+  double *part;      // [max_slots][n_p][n_jext][n_field]
 };
 
 // ---- (1) boson rows --------------------------------------------------------------------------------
@@ -59,6 +66,7 @@ __global__ void __launch_bounds__(M3_PRE_THREADS) mats3d_phi_rows_kernel(const M
   const double om = 2.0 * 3.14159265358979323846 * (double)m * P.T;
   const int npairs = P.nq * P.nc;
   double* dst = P.d0phi + ((size_t)e * P.n_rows + m) * P.row_stride;
+  double* dst1 = P.d0phi + (size_t)e * P.nq * P.chunk_stride + (size_t)m * P.nc;
   double dmin = __longlong_as_double(0x7ff0000000000000LL);
   for (int t = threadIdx.x; t < npairs; t += M3_PRE_THREADS) {
     const int i = t / P.nc, jc = t - i * P.nc;
@@ -69,10 +77,16 @@ __global__ void __launch_bounds__(M3_PRE_THREADS) mats3d_phi_rows_kernel(const M
     double R, Rd;
     regulator(P.reg, fm, sphi, R, Rd);
     const double D0 = table_lookup(cells, P.grid, fm, r2) * sphi + R;
-    dst[t] = D0;
+    if (P.phi_layout == 0) dst[t] = D0;
+    else dst1[(size_t)i * P.chunk_stride + jc] = D0;
     dmin = fmin(dmin, D0);
   }
-  if (threadIdx.x == 0 && (npairs & 1)) dst[npairs] = 1.0;  // pad to the even row stride
+  if (P.phi_layout == 0) {
+    if (threadIdx.x == 0 && (npairs & 1)) dst[npairs] = 1.0;  // pad to the even row stride
+  } else if (m == 0 && ((P.n_rows * P.nc) & 1)) {
+    for (int i = threadIdx.x; i < P.nq; i += M3_PRE_THREADS)
+      P.d0phi[((size_t)e * P.nq + i) * P.chunk_stride + P.n_rows * P.nc] = 1.0;  // pad to the even chunk stride
+  }
   dmin = block_min(dmin, red);
   if (threadIdx.x == 0) P.rowmin[(size_t)e * P.n_rows + m] = dmin;
 }
@@ -329,6 +343,249 @@ static size_t mats3d_main_smem(int nq, int nc, int rs, int ps, int groups, int m
                       2 * groups * M3_FT * mf);
 }
 
+// ---- (3b) moment kernel ---------------------------------------------------------------------------------
+// The numerator polynomial is a cubic in y2 = p q c / k^2 whose coefficients depend on (j, n, i) only, and the
+// boson denominator depends on (j, n) only through m = |j - n|.  Hence
+//     sum_c wc_c P G_phi  =  sum_{b=0..3} beta_b(j,n,i) (p q_i/k^2)^b  M_b(m, i; f),
+//     M_b(m, i; f) = sum_c wc_c c^b / (D0phi[p][m][i][c] + m2phi_f)              (angular moments of the boson line)
+// and the moments are shared by every (j, n) with |j - n| = m: n_jext + n_max rows of moments serve
+// n_jext (2 n_max + 1) (j, n) pairs (27 for 368 in config 4).  Likewise G_psi depends on n only through
+// nbar (nu_{-n-1} = -nu_n): n_max + 1 fermion reciprocals serve 2 n_max + 1 terms.  Per (p, i, f):
+//     (n_jext + n_max) nc  x (DADD + reciprocal (3 DFMA) + 4 DFMA)        moments
+//   + (n_max + 1)          x (DADD + reciprocal + DMUL)                    H_nbar = G_psi^2
+//   + n_jext (2 n_max + 1) x (DMUL + 3 DFMA + DFMA)                        acc_j += H_nbar (beta' . M)
+// = 7084 FP64 instructions for config 4 instead of 16 x 23 x (24 x 4.25 + 8) = 40 480.
+//
+// Mapping.  Work unit = (field tile, p, radial node i); the units are dealt to the CTAs (one per SM, persistent)
+// in contiguous ranges, so a CTA keeps its NJ accumulators per field point in registers while it walks the radial
+// nodes of one p, and writes them as a partial sum when p (or its range) ends; mats3d_fixup_kernel adds the
+// <= max_slots partial sums of an output in fixed order (deterministic: the ownership of units is a pure
+// function of the grid size).  A producer warp runs one unit ahead: TMA bulk copy of the unit's D0phi chunk
+// [m][c] (5 KB), the fermion denominators, and beta'[j][n] = Wpsi (p q/k^2)^b beta_b (12 KB, field independent).
+// NTC consumer threads x MF field points: everything they read in the hot loop is a shared-memory broadcast.
+// The loops over m and j are unrolled at compile time (NMAX, NJ are template parameters) so that the
+// accumulators, the moments and H stay in registers.
+template <int NMAX, int NJ, int MF, int NTC>
+__global__ void __launch_bounds__(NTC + 32, 1) mats3d_moment_kernel(const Mats3dParams P) {
+  constexpr int NT = 2 * NMAX + 1, NROWS = NJ + NMAX, NB = NJ * NT * 4, NPS = NMAX + 1;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t full[2], empty[2];
+  __shared__ double skap[20];
+
+  const int nq = P.nq, nc = P.nc, cs = P.chunk_stride, ps = P.psi_stride;
+  double* d0buf = reinterpret_cast<double*>(smem_raw);           // [2][cs]
+  double* betabuf = d0buf + 2 * cs;                              // [2][NB]
+  double2* psibuf = reinterpret_cast<double2*>(betabuf + 2 * NB);  // [2][NPS] (D0psi, Wpsi)
+  double* numbuf = reinterpret_cast<double*>(psibuf + 2 * NPS);  // [nc][4]  wc c^b
+  double* sxq = numbuf + 4 * nc;                                 // [nq]
+
+  const int tile = NTC * MF;
+  const int n_ftiles = (P.n_field + tile - 1) / tile;
+  const long long upp = (long long)P.n_p * nq;                   // units per field tile
+  const long long U = (long long)n_ftiles * upp;
+  const long long u0 = (long long)blockIdx.x * U / gridDim.x, u1 = (long long)(blockIdx.x + 1) * U / gridDim.x;
+  const double pi = 3.14159265358979323846;
+  const double ik2 = P.reg.inv_k2;
+
+  if (threadIdx.x == 0) {
+    mbar_init(&full[0], 1);
+    mbar_init(&full[1], 1);
+    mbar_init(&empty[0], NTC / 32);
+    mbar_init(&empty[1], NTC / 32);
+    mbar_fence_init();
+  }
+  if (threadIdx.x < 20) skap[threadIdx.x] = P.coef[threadIdx.x];
+  for (int i = threadIdx.x; i < nq; i += blockDim.x) sxq[i] = P.xq[i];
+  for (int c = threadIdx.x; c < nc; c += blockDim.x) {
+    const double x = P.xc[c], w = P.wc[c];
+    numbuf[4 * c] = w; numbuf[4 * c + 1] = w * x; numbuf[4 * c + 2] = w * x * x; numbuf[4 * c + 3] = w * x * x * x;
+  }
+  __syncthreads();
+
+  if (threadIdx.x >= NTC) {
+    // =========================== producer warp ===========================
+    const int lane = threadIdx.x - NTC;
+    uint32_t g = 0;
+    for (long long u = u0; u < u1; ++u, ++g) {
+      const long long rem = u % upp;
+      const int e = (int)(rem / nq), i = (int)(rem - (long long)e * nq);
+      const int b = g & 1;
+      mbar_wait(&empty[b], ((g >> 1) & 1) ^ 1);
+      if (lane == 0) {
+        mbar_expect_tx_only(&full[b], (uint32_t)cs * 8u);
+        tma_bulk_g2s(d0buf + (size_t)b * cs, P.d0phi + ((size_t)e * nq + i) * cs, (uint32_t)cs * 8u, &full[b]);
+      }
+      double2* psb = psibuf + b * NPS;
+      if (lane < NPS) psb[lane] = P.psi[(size_t)(lane + P.n_max) * ps + i];   // rows n >= 0: nbar = n
+      __syncwarp();
+      const double q = sxq[i];
+      const double pq = P.pext[e] * q * ik2;
+      double* bet = betabuf + (size_t)b * NB;
+      for (int t = lane; t < NJ * NT; t += 32) {
+        const int j = t / NT, n = t - j * NT - NMAX;
+        const int nbar = n >= 0 ? n : -n - 1;
+        const double nun = (2.0 * n + 1.0) * pi * P.T, nuj = (2.0 * j + 1.0) * pi * P.T;
+        const double y1 = nun * nuj * ik2;
+        const double y3 = (nun * nun + q * q) * ik2;
+        // P = sum_b y2^b beta_b,  beta_b = sum_{a+c<=3-b} kap_abc y1^a y3^c   (idx: a outermost, then b, then c)
+        double be[4] = {0.0, 0.0, 0.0, 0.0};
+        int idx = 0;
+        double y1a = 1.0;
+#pragma unroll
+        for (int a = 0; a <= 3; ++a) {
+#pragma unroll
+          for (int bb = 0; bb <= 3 - a; ++bb) {
+            double y3c = y1a;
+#pragma unroll
+            for (int c = 0; c <= 3 - a - bb; ++c) {
+              be[bb] = fma(skap[idx++], y3c, be[bb]);
+              y3c *= y3;
+            }
+          }
+          y1a *= y1;
+        }
+        const double W = psb[nbar].y;
+        const double s1 = W * pq, s2 = s1 * pq, s3 = s2 * pq;
+        bet[4 * t] = be[0] * W; bet[4 * t + 1] = be[1] * s1; bet[4 * t + 2] = be[2] * s2; bet[4 * t + 3] = be[3] * s3;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&full[b]);
+    }
+    return;
+  }
+
+  // =============================== consumers ===============================
+  const int tid = threadIdx.x;
+  const bool warp_leader = (tid & 31) == 0;
+  const double4* num4 = reinterpret_cast<const double4*>(numbuf);
+  double m2psi[MF], m2phi[MF], acc[NJ][MF];
+  int cur_ft = -1;
+  uint32_t g = 0;
+  for (long long u = u0; u < u1; ++u, ++g) {
+    const int ft = (int)(u / upp);
+    const long long rem = u - (long long)ft * upp;
+    const int e = (int)(rem / nq), i = (int)(rem - (long long)e * nq);
+    const int f0 = ft * tile + tid;
+    if (ft != cur_ft) {
+      cur_ft = ft;
+#pragma unroll
+      for (int k = 0; k < MF; ++k) {
+        const int f = f0 + k * NTC;
+        m2psi[k] = (f < P.n_field) ? P.m2psi[f] : 1.0;
+        m2phi[k] = (f < P.n_field) ? P.m2phi[f] : 1.0;
+      }
+    }
+    if (u == u0 || i == 0) {
+#pragma unroll
+      for (int j = 0; j < NJ; ++j)
+#pragma unroll
+        for (int k = 0; k < MF; ++k) acc[j][k] = 0.0;
+    }
+    const int b = g & 1;
+    mbar_wait(&full[b], (g >> 1) & 1);
+    const double* d0 = d0buf + (size_t)b * cs;
+    const double4* bet4 = reinterpret_cast<const double4*>(betabuf + (size_t)b * NB);
+    const double2* psb = psibuf + b * NPS;
+
+    double H[NPS][MF];
+#pragma unroll
+    for (int nb = 0; nb < NPS; ++nb) {
+      const double D0 = psb[nb].x;
+#pragma unroll
+      for (int k = 0; k < MF; ++k) {
+        const double gp = fast_rcp(D0 + m2psi[k]);
+        H[nb][k] = gp * gp;
+      }
+    }
+#pragma unroll
+    for (int m = 0; m < NROWS; ++m) {
+      double M[4][MF];
+#pragma unroll
+      for (int k = 0; k < MF; ++k) { M[0][k] = 0.0; M[1][k] = 0.0; M[2][k] = 0.0; M[3][k] = 0.0; }
+      const double* drow = d0 + m * nc;
+#pragma unroll 2
+      for (int c = 0; c < nc; ++c) {
+        const double D0 = drow[c];
+        const double4 w = num4[c];
+#pragma unroll
+        for (int k = 0; k < MF; ++k) {
+          const double r = fast_rcp(D0 + m2phi[k]);
+          M[0][k] = fma(w.x, r, M[0][k]);
+          M[1][k] = fma(w.y, r, M[1][k]);
+          M[2][k] = fma(w.z, r, M[2][k]);
+          M[3][k] = fma(w.w, r, M[3][k]);
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) {
+#pragma unroll
+        for (int sgn = 0; sgn < 2; ++sgn) {
+          const int n = sgn == 0 ? j - m : j + m;
+          const bool valid = sgn == 0 ? (n >= -NMAX && n <= NMAX) : (m > 0 && n <= NMAX);
+          if (valid) {
+            const int nbar = n >= 0 ? n : -n - 1;
+            const double4 B = bet4[j * NT + n + NMAX];
+#pragma unroll
+            for (int k = 0; k < MF; ++k) {
+              double t = B.x * M[0][k];
+              t = fma(B.y, M[1][k], t);
+              t = fma(B.z, M[2][k], t);
+              t = fma(B.w, M[3][k], t);
+              acc[j][k] = fma(H[nbar][k], t, acc[j][k]);
+            }
+          }
+        }
+      }
+    }
+    __syncwarp();
+    if (warp_leader) mbar_arrive(&empty[b]);
+
+    if (i == nq - 1 || u == u1 - 1) {
+      // partial sum of this CTA for (field tile, p): slot = rank of this CTA among the owners of the p's units
+      const long long ufirst = (long long)ft * upp + (long long)e * nq;
+      const int c_first = (int)(((ufirst + 1) * gridDim.x - 1) / U);
+      const int slot = (int)blockIdx.x - c_first;
+#pragma unroll
+      for (int j = 0; j < NJ; ++j)
+#pragma unroll
+        for (int k = 0; k < MF; ++k) {
+          const int f = f0 + k * NTC;
+          if (f < P.n_field)
+            P.part[(((size_t)slot * P.n_p + e) * NJ + j) * P.n_field + f] = acc[j][k];
+        }
+    }
+  }
+}
+
+// S5/S6 of the moment path: out = prefactor T sum_slots part, dmin from the row minima.
+__global__ void __launch_bounds__(256) mats3d_fixup_kernel(const Mats3dParams P) {
+  const long long idx = (long long)blockIdx.x * 256 + threadIdx.x;
+  const long long n_out = (long long)P.n_p * P.n_jext * P.n_field;
+  if (idx >= n_out) return;
+  const int f = (int)(idx % P.n_field);
+  const long long ej = idx / P.n_field;
+  const int e = (int)(ej / P.n_jext), j = (int)(ej - (long long)e * P.n_jext);
+  const int n_ftiles = (P.n_field + P.tile_fields - 1) / P.tile_fields;
+  const long long upp = (long long)P.n_p * P.nq, U = (long long)n_ftiles * upp;
+  const long long ufirst = (long long)(f / P.tile_fields) * upp + (long long)e * P.nq, ulast = ufirst + P.nq - 1;
+  const int c_first = (int)(((ufirst + 1) * P.grid_main - 1) / U), c_last = (int)(((ulast + 1) * P.grid_main - 1) / U);
+  const size_t stride = (size_t)P.n_p * P.n_jext * P.n_field;
+  double r = P.part[idx];
+  for (int s = 1; s <= c_last - c_first; ++s) r += P.part[(size_t)s * stride + idx];
+  P.out[idx] = P.prefactor * P.T * r;
+  if (P.dmin) {
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    double dpsi = inf, dphi = inf;
+    for (int it = 0; it < 2 * P.n_max + 1; ++it) {
+      const int mm = j - (it - P.n_max), mabs = mm >= 0 ? mm : -mm;
+      dpsi = fmin(dpsi, P.psimin[it]);
+      dphi = fmin(dphi, P.rowmin[(size_t)e * P.n_rows + mabs]);
+    }
+    P.dmin[idx] = fmin(dpsi + P.m2psi[f], dphi + P.m2phi[f]) * P.reg.inv_k2;
+  }
+}
+
+
 static int mats3d_validate(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi, const double* m2_phi, int n_p,
                            const double* p, int n_jext, double* out) {
   if (!D || !m2_psi || !m2_phi || !p || !out || n_field < 1 || n_p < 1 || n_jext < 1) return DFRG_EINVAL;
@@ -358,6 +615,44 @@ static int mats3d_launch_main(const Mats3dParams& P, int sm_count, cudaStream_t 
   return check_cuda(cudaGetLastError());
 }
 
+// ---- moment-path dispatch: (n_max, n_jext) pairs with a compiled instantiation ---------------------------
+struct MomentPlan {
+  int variant;     // 0: MF 2 x 256 threads, 1: MF 1 x 512 threads, 2: MF 1 x 256 threads
+  int tile, grid, max_slots;
+  size_t smem;
+};
+
+template <int NMAX, int NJ>
+static int mats3d_moment_go(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream) {
+  cudaError_t e;
+#define DFRG_M3_GO(MF, NTC)                                                                                          \
+  e = cudaFuncSetAttribute(mats3d_moment_kernel<NMAX, NJ, MF, NTC>, cudaFuncAttributeMaxDynamicSharedMemorySize,     \
+                           (int)pl.smem);                                                                            \
+  if (e != cudaSuccess) return check_cuda(e);                                                                        \
+  mats3d_moment_kernel<NMAX, NJ, MF, NTC><<<pl.grid, NTC + 32, pl.smem, stream>>>(P);
+  if (pl.variant == 0) { DFRG_M3_GO(2, 256) }
+  else if (pl.variant == 1) { DFRG_M3_GO(1, 512) }
+  else { DFRG_M3_GO(1, 256) }
+#undef DFRG_M3_GO
+  return check_cuda(cudaGetLastError());
+}
+
+// X(NMAX, NJ) for every compiled instantiation: BASELINE.json config 4 and the small shapes of the test-suite.
+#define DFRG_M3_SHAPES(X) X(11, 16) X(11, 2) X(3, 3) X(2, 2)
+
+static bool mats3d_moment_shape(int n_max, int n_jext) {
+#define X(a, b) if (n_max == a && n_jext == b) return true;
+  DFRG_M3_SHAPES(X)
+#undef X
+  return false;
+}
+static int mats3d_moment_dispatch(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream) {
+#define X(a, b) if (P.n_max == a && P.n_jext == b) return mats3d_moment_go<a, b>(P, pl, stream);
+  DFRG_M3_SHAPES(X)
+#undef X
+  return DFRG_EUNSUPPORTED;
+}
+
 static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi, const double* m2_phi, int n_p,
                          const double* p, int n_jext, double* out, double* dmin, int sm_count, cudaStream_t stream) {
   Mats3dParams P;
@@ -365,6 +660,7 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   P.n_rows = n_jext + D->n_max;
   const int npairs = P.nq * P.nc;
   P.row_stride = (npairs + 1) & ~1;  // TMA bulk copies move multiples of 16 bytes
+  P.chunk_stride = (P.n_rows * P.nc + 1) & ~1;
   P.psi_stride = P.nq;
   P.T = D->T; P.prefactor = D->prefactor;
   P.reg.kind = D->reg.kind; P.reg.order = D->reg.order; P.reg.k2 = D->reg.k * D->reg.k; P.reg.inv_k2 = 1.0 / P.reg.k2;
@@ -374,19 +670,45 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   P.xq = D->q.x; P.wq = D->q.w; P.xc = D->cos1.x; P.wc = D->cos1.w;
   P.Zpsi = D->tab_psi.v; P.Zphi = D->tab_phi.v; P.coef = D->coef;
   P.m2psi = m2_psi; P.m2phi = m2_phi; P.pext = p; P.out = out; P.dmin = dmin;
+  P.part = nullptr; P.tile_fields = 0; P.max_slots = 0; P.grid_main = 0;
+
+  // ---- path: moment factorisation where an instantiation exists (DFRG_M3_PATH=generic forces the other one) ----
+  const char* vpath = getenv("DFRG_M3_PATH");
+  bool moment = mats3d_moment_shape(D->n_max, n_jext) && !(vpath && vpath[0] == 'g');
+  MomentPlan pl = {};
+  if (moment) {
+    const char* vm = getenv("DFRG_M3_MF");
+    pl.variant = n_field <= 256 ? 2 : ((vm && atoi(vm) == 1) ? 1 : 0);
+    pl.tile = pl.variant == 0 ? 512 : (pl.variant == 1 ? 512 : 256);
+    const int n_ftiles = (n_field + pl.tile - 1) / pl.tile;
+    const long long upp = (long long)n_p * P.nq, U = (long long)n_ftiles * upp;
+    pl.grid = (int)(U < sm_count ? U : sm_count);
+    pl.max_slots = 1;
+    for (long long seg = 0; seg < (long long)n_ftiles * n_p; ++seg) {
+      const long long ufirst = seg * P.nq, ulast = ufirst + P.nq - 1;
+      const int c0 = (int)(((ufirst + 1) * pl.grid - 1) / U), c1 = (int)(((ulast + 1) * pl.grid - 1) / U);
+      if (c1 - c0 + 1 > pl.max_slots) pl.max_slots = c1 - c0 + 1;
+    }
+    pl.smem = 8 * (size_t)(2 * P.chunk_stride + 2 * n_jext * (2 * D->n_max + 1) * 4 + 4 * (D->n_max + 1) + 4 * P.nc + P.nq);
+    if (pl.smem > 220 * 1024) moment = false;
+  }
+  P.phi_layout = moment ? 1 : 0;
+  P.tile_fields = pl.tile; P.max_slots = pl.max_slots; P.grid_main = pl.grid;
 
   const int n_terms = 2 * D->n_max + 1;
-  const size_t n_d0 = (size_t)n_p * P.n_rows * P.row_stride;
+  const size_t n_d0 = moment ? (size_t)n_p * P.nq * P.chunk_stride : (size_t)n_p * P.n_rows * P.row_stride;
   const size_t n_rowmin = ((size_t)n_p * P.n_rows + 1) & ~(size_t)1;
   const size_t n_psi = (size_t)n_terms * P.psi_stride * 2;
   const size_t n_psimin = ((size_t)n_terms + 1) & ~(size_t)1;
+  const size_t n_part = moment ? (size_t)pl.max_slots * n_p * n_jext * n_field : 0;
   void* scratch = nullptr;
-  int rc = scratch_alloc(&scratch, (n_d0 + n_rowmin + n_psi + n_psimin) * sizeof(double), stream);
+  int rc = scratch_alloc(&scratch, (n_d0 + n_rowmin + n_psi + n_psimin + n_part) * sizeof(double), stream);
   if (rc != DFRG_OK) return rc;
   P.d0phi = (double*)scratch;
   P.psi = (double2*)(P.d0phi + n_d0);
   P.rowmin = (double*)(P.psi) + n_psi;
   P.psimin = P.rowmin + n_rowmin;
+  P.part = P.psimin + n_psimin;
 
   mats3d_phi_rows_kernel<<<dim3(P.n_rows, n_p), M3_PRE_THREADS, 0, stream>>>(P);
   rc = check_cuda(cudaGetLastError());
@@ -394,9 +716,16 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
     mats3d_psi_kernel<<<n_terms, 128, 0, stream>>>(P);
     rc = check_cuda(cudaGetLastError());
   }
-  if (rc == DFRG_OK) {
-    // consumer groups per CTA (radial nodes are dealt round-robin to the groups) and field points per thread;
-    // DFRG_M3_GROUPS / DFRG_M3_MF override the defaults (tuning knobs)
+  if (rc == DFRG_OK && moment) {
+    rc = mats3d_moment_dispatch(P, pl, stream);
+    if (rc == DFRG_OK) {
+      const long long n_out = (long long)n_p * n_jext * n_field;
+      mats3d_fixup_kernel<<<(unsigned)((n_out + 255) / 256), 256, 0, stream>>>(P);
+      rc = check_cuda(cudaGetLastError());
+    }
+  } else if (rc == DFRG_OK) {
+    // generic path: consumer groups per CTA (radial nodes are dealt round-robin to the groups) and field points per
+    // thread; DFRG_M3_GROUPS / DFRG_M3_MF override the defaults (tuning knobs)
     const char* vg = getenv("DFRG_M3_GROUPS");
     const char* vm = getenv("DFRG_M3_MF");
     int mf = n_field > 2 * M3_FT ? 4 : (n_field > M3_FT ? 2 : 1);

@@ -160,6 +160,28 @@ def test_matsubara_small(n_field, n_p, n_jext, n_q, n_c, n_max, interp):
     run_both(c, what="mats_%d_%d_%d_%d_%d_%d_i%d" % (n_field, n_p, n_jext, n_q, n_c, n_max, interp))
 
 
+@pytest.mark.parametrize("n_field,n_p,n_jext,n_q,n_c,n_max,interp", [(1100, 3, 2, 13, 5, 11, 3), (700, 2, 3, 24, 7, 3, 3),
+                                                                      (257, 5, 2, 150, 4, 2, 1), (40, 70, 2, 3, 6, 2, 3)])
+def test_matsubara_moment_path_small(n_field, n_p, n_jext, n_q, n_c, n_max, interp):
+    # shapes with a compiled moment-kernel instantiation: several field tiles, a ragged tail, an odd chunk
+    # stride, more units than CTAs and fewer; the generic kernel must give the same answer on the same inputs
+    c = inputs.config4(n_field=n_field, n_p=n_p, n_jext=n_jext, n_q=n_q, n_c=n_c, interp=interp)
+    c["n_max"] = n_max
+    what = "mats_moment_%d_%d_%d_%d_%d_%d_i%d" % (n_field, n_p, n_jext, n_q, n_c, n_max, interp)
+    g, o, _ = run_both(c, what=what)
+    os.environ["DFRG_M3_PATH"] = "generic"
+    try:
+        g2, _, _ = run_both(c, what=what + "_generic")
+    finally:
+        del os.environ["DFRG_M3_PATH"]
+    assert not np.array_equal(g["out"], g2["out"]) or n_field == 1      # two different kernels ran
+    os.environ["DFRG_M3_MF"] = "1"
+    try:
+        run_both(c, what=what + "_mf1")
+    finally:
+        del os.environ["DFRG_M3_MF"]
+
+
 def test_matsubara_full_config4_sampled():
     c = inputs.config4()
     n_out = 64 * 16 * 512
