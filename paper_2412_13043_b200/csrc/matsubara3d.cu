@@ -365,6 +365,73 @@ static size_t mats3d_main_smem(int nq, int nc, int rs, int ps, int groups, int m
 // NTC consumer threads x MF field points: everything they read in the hot loop is a shared-memory broadcast.
 // The loops over m and j are unrolled at compile time (NMAX, NJ are template parameters) so that the
 // accumulators, the moments and H stay in registers.
+// Reciprocals 1/(D0[t] + m2[k]) of M3_NBAT consecutive nodes for the MF field points of a thread, stage by stage.
+// MF = 2: one hardware seed per node serves both field points, 1/(d0 d1) then r0 = R d1, r1 = R d0 -- the same
+// FP64 instruction count as two separate Newton reciprocals (8 per node) and half the MUFU.RCP64H.
+constexpr int M3_NBAT = 4;
+template <int MF>
+__device__ __forceinline__ void mats3d_recip_batch(const double* __restrict__ dptr, const double (&m2)[MF],
+                                                   double (&r)[M3_NBAT][MF]) {
+  double d[M3_NBAT][MF];
+  static_assert(M3_NBAT % 2 == 0, "vector loads of D0");
+#pragma unroll
+  for (int t = 0; t < M3_NBAT; t += 2) {
+    const double2 D0 = *reinterpret_cast<const double2*>(dptr + t);   // dptr is 16-byte aligned (even node index)
+#pragma unroll
+    for (int k = 0; k < MF; ++k) { d[t][k] = D0.x + m2[k]; d[t + 1][k] = D0.y + m2[k]; }
+  }
+  if constexpr (MF == 2) {
+    double pr[M3_NBAT], R[M3_NBAT];
+#pragma unroll
+    for (int t = 0; t < M3_NBAT; ++t) pr[t] = d[t][0] * d[t][1];
+#pragma unroll
+    for (int t = 0; t < M3_NBAT; ++t) R[t] = rcp_seed(pr[t]);
+#pragma unroll
+    for (int t = 0; t < M3_NBAT; ++t) pr[t] = fma(-pr[t], R[t], 1.0);
+#pragma unroll
+    for (int t = 0; t < M3_NBAT; ++t) pr[t] = fma(pr[t], pr[t], pr[t]);
+#pragma unroll
+    for (int t = 0; t < M3_NBAT; ++t) R[t] = fma(R[t], pr[t], R[t]);
+#pragma unroll
+    for (int t = 0; t < M3_NBAT; ++t) { r[t][0] = R[t] * d[t][1]; r[t][1] = R[t] * d[t][0]; }
+  } else {
+#pragma unroll
+    for (int t = 0; t < M3_NBAT; ++t)
+#pragma unroll
+      for (int k = 0; k < MF; ++k) r[t][k] = rcp_seed(d[t][k]);
+#pragma unroll
+    for (int t = 0; t < M3_NBAT; ++t)
+#pragma unroll
+      for (int k = 0; k < MF; ++k) d[t][k] = fma(-d[t][k], r[t][k], 1.0);
+#pragma unroll
+    for (int t = 0; t < M3_NBAT; ++t)
+#pragma unroll
+      for (int k = 0; k < MF; ++k) d[t][k] = fma(d[t][k], d[t][k], d[t][k]);
+#pragma unroll
+    for (int t = 0; t < M3_NBAT; ++t)
+#pragma unroll
+      for (int k = 0; k < MF; ++k) r[t][k] = fma(r[t][k], d[t][k], r[t][k]);
+  }
+}
+
+// M_b += sum_t w[t].b r[t]  for a batch of M3_NBAT nodes (w = wc c^b, broadcast from shared memory).
+template <int MF>
+__device__ __forceinline__ void mats3d_moment_accumulate(const double4* __restrict__ w4, const double (&r)[M3_NBAT][MF],
+                                                         double (&M)[4][MF]) {
+  double4 w[M3_NBAT];
+#pragma unroll
+  for (int t = 0; t < M3_NBAT; ++t) w[t] = w4[t];
+#pragma unroll
+  for (int t = 0; t < M3_NBAT; ++t)
+#pragma unroll
+    for (int k = 0; k < MF; ++k) {
+      M[0][k] = fma(w[t].x, r[t][k], M[0][k]);
+      M[1][k] = fma(w[t].y, r[t][k], M[1][k]);
+      M[2][k] = fma(w[t].z, r[t][k], M[2][k]);
+      M[3][k] = fma(w[t].w, r[t][k], M[3][k]);
+    }
+}
+
 // The (j, n) pairs with |j - n| = m of the moment kernel:  acc[j] += H[nbar(n)] (beta'[j][n] . M),  in groups of
 // four (two j x two signs), written stage by stage so that each stage is a set of independent instructions.
 template <int m, int NMAX, int NJ, int MF>
@@ -547,64 +614,45 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
         H[nb][k] = gp * gp;
       }
     }
+    const bool pipelined = (nc % (2 * M3_NBAT)) == 0;
+    const int l_last = NROWS * nc - M3_NBAT;
+    double ra[M3_NBAT][MF], rb[M3_NBAT][MF];
+    if (pipelined) mats3d_recip_batch<MF>(d0, m2phi, ra);
 #pragma unroll 1
     for (int m = 0; m < NROWS; ++m) {
-      // ---- angular moments of row m.  Written stage by stage over a batch of NBAT nodes x MF field points so that
-      // every stage holds NBAT*MF independent instructions: with two warps per scheduler the FP64 pipe is fed by
-      // instruction-level parallelism, not by occupancy. ----
+      // ---- angular moments of row m.  Written stage by stage over a batch of M3_NBAT nodes x MF field points so
+      // that every stage holds independent instructions, and software-pipelined: the reciprocals of the next batch
+      // (which may belong to the next row: the chunk is contiguous in [m][c]) are computed while the current batch
+      // is accumulated.  With two warps per scheduler the FP64 pipe is fed by instruction-level parallelism. ----
       double M[4][MF];
 #pragma unroll
       for (int k = 0; k < MF; ++k) { M[0][k] = 0.0; M[1][k] = 0.0; M[2][k] = 0.0; M[3][k] = 0.0; }
-      const double* drow = d0 + m * nc;
-      constexpr int NBAT = 4;
-      int c = 0;
-      for (; c + NBAT <= nc; c += NBAT) {
-        double4 w[NBAT];
-        double d[NBAT][MF], r[NBAT][MF];
-#pragma unroll
-        for (int t = 0; t < NBAT; ++t) {
-          const double D0 = drow[c + t];
-#pragma unroll
-          for (int k = 0; k < MF; ++k) d[t][k] = D0 + m2phi[k];
+      if (pipelined) {
+        // two batches per trip, the reciprocals ping-ponging between ra and rb (no register moves):
+        //   ra = batch at c (ready), rb <- batch at c+4 while ra is accumulated, ra <- batch at c+8 while rb is ...
+        for (int c = 0; c < nc; c += 2 * M3_NBAT) {
+          const int L = m * nc + c;
+          mats3d_recip_batch<MF>(d0 + L + M3_NBAT, m2phi, rb);
+          mats3d_moment_accumulate<MF>(num4 + c, ra, M);
+          int Ln = L + 2 * M3_NBAT;
+          Ln = Ln < l_last ? Ln : l_last;   // past the end of the chunk: recompute the last batch (result unused)
+          mats3d_recip_batch<MF>(d0 + Ln, m2phi, ra);
+          mats3d_moment_accumulate<MF>(num4 + c + M3_NBAT, rb, M);
         }
-#pragma unroll
-        for (int t = 0; t < NBAT; ++t) w[t] = num4[c + t];
-#pragma unroll
-        for (int t = 0; t < NBAT; ++t)
-#pragma unroll
-          for (int k = 0; k < MF; ++k) r[t][k] = rcp_seed(d[t][k]);
-#pragma unroll
-        for (int t = 0; t < NBAT; ++t)
-#pragma unroll
-          for (int k = 0; k < MF; ++k) d[t][k] = fma(-d[t][k], r[t][k], 1.0);
-#pragma unroll
-        for (int t = 0; t < NBAT; ++t)
-#pragma unroll
-          for (int k = 0; k < MF; ++k) d[t][k] = fma(d[t][k], d[t][k], d[t][k]);
-#pragma unroll
-        for (int t = 0; t < NBAT; ++t)
-#pragma unroll
-          for (int k = 0; k < MF; ++k) r[t][k] = fma(r[t][k], d[t][k], r[t][k]);
-#pragma unroll
-        for (int t = 0; t < NBAT; ++t)
+      } else {
+        const double* drow = d0 + m * nc;
+#pragma unroll 1
+        for (int c = 0; c < nc; ++c) {
+          const double D0 = drow[c];
+          const double4 w = num4[c];
 #pragma unroll
           for (int k = 0; k < MF; ++k) {
-            M[0][k] = fma(w[t].x, r[t][k], M[0][k]);
-            M[1][k] = fma(w[t].y, r[t][k], M[1][k]);
-            M[2][k] = fma(w[t].z, r[t][k], M[2][k]);
-            M[3][k] = fma(w[t].w, r[t][k], M[3][k]);
+            const double r = fast_rcp(D0 + m2phi[k]);
+            M[0][k] = fma(w.x, r, M[0][k]);
+            M[1][k] = fma(w.y, r, M[1][k]);
+            M[2][k] = fma(w.z, r, M[2][k]);
+            M[3][k] = fma(w.w, r, M[3][k]);
           }
-      }
-      for (; c < nc; ++c) {
-        const double D0 = drow[c];
-        const double4 w = num4[c];
-#pragma unroll
-        for (int k = 0; k < MF; ++k) {
-          const double r = fast_rcp(D0 + m2phi[k]);
-          M[0][k] = fma(w.x, r, M[0][k]);
-          M[1][k] = fma(w.y, r, M[1][k]);
-          M[2][k] = fma(w.z, r, M[2][k]);
-          M[3][k] = fma(w.w, r, M[3][k]);
         }
       }
       // ---- the (j, n) pairs with |j - n| = m: compile-time code per m (static register indices), reached through
