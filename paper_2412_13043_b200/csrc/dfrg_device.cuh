@@ -46,7 +46,7 @@ struct FastMath {
 // them as constant operands; as compile-time literals the compiler rebuilds each 64-bit immediate in uniform
 // registers (two UMOV) before every use.
 struct FastMathConsts {
-  double c[16];
+  double c[20];
 };
 inline FastMathConsts fm_consts() {
   FastMathConsts k = {{
@@ -54,7 +54,10 @@ inline FastMathConsts fm_consts() {
       0.6931471805592082, 7.371002565167799e-13,      // 5,6  ln2 hi / lo (40-bit split)
       -92.33248261689366, 6755399441055744.0,         // 7,8  -64/ln2, 1.5 * 2^52
       -0.01083042469326756, -2.9815858269852933e-12,  // 9,10 -(ln2/64) hi / lo (32-bit split)
-      1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0, 0.5, 1.0}};  // 11-15 exp series
+      1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0, 0.5, 1.0,   // 11-15 exp series
+      -369.3299304675746,                             // 16    -256/ln2                  (fx_exp_neg, 256-entry table)
+      -0.01083042469326756 / 4.0, -2.9815858269852933e-12 / 4.0,  // 17,18 -(ln2/256) hi / lo
+      0.0}};
   return k;
 }
 // Branch-free clamps as one DSETP + two SEL (CUDA's fmin/fmax add NaN fix-ups: seven instructions each).
@@ -193,6 +196,136 @@ __device__ __forceinline__ double table_lookup(const double4* __restrict__ cells
   const double tau = t - (double)(c + g.off());
   const double4 k = cells[c];
   return fma(fma(fma(k.w, tau, k.z), tau, k.y), tau, k.x);
+}
+
+// ---- fused log-grid coordinate and guarded cells (the S3 look-up of the hot three-point loop) -----------------
+// t(s) = (ln(s)/2 - lo)/h = A ln s + B straight from the bits of s, without a separate logarithm:
+//   s = 2^e m,  j = top 9 mantissa bits,  r = m inv_j - 1 (|r| <= 2^-10),  ln(1+r) = r - r^2/2 + r^3/3 - r^4/4
+//   (truncation r^5/5 < 1.8e-16 absolute in ln s: far below the rounding of t itself, ulp(127) = 1.4e-14)
+//   t = fma(ln(1+r), A, mant[j].y) + fma(E, A ln2, B - 1023 A ln2),   mant[j] = (inv_j, A ln c_j)
+// E = the exponent field of s >= 0 (callers clamp s at 0): zero and subnormal s land far below the grid (the table's
+// first value, as log(0) = -inf would give), inf/NaN far above.  7 FP64 instructions, one conversion, one LDS.128.
+// The cells carry guards: index F + 1 with F = clamp(floor(t), -1, n-1); F = -1 and F = n-1 are constant cells
+// (clamp-to-edge), the others hold the interpolant of SURVEY 8(c) (4-point Lagrange on the stencil
+// i0 = clamp(F-1, 0, n-4), or the linear one) re-expanded in tau = t - F.  Integer clamps replace the FP64 ones.
+// Threads of a warp look up unrelated entries, so both tables are replicated LG_REP = 8 times, one copy per
+// lane-slot (lane & 7) confined to its own 16-byte bank group: a 128-bit shared-memory load is served in
+// quarter-warps of 8 consecutive lanes, hence every look-up is conflict free (4 wavefronts) wherever it points.
+constexpr int LG_NM = 512, LG_REP = 8;
+constexpr int LG_DOUBLES = 2 * LG_NM * LG_REP;  // 64 KB
+struct LogGrid {
+  const double2* mant;  // this thread's copy: entry j at mant[j * LG_REP]
+  double A, ex1, ex0;   // A = 1/(2h); exponent term = fma((double)E, ex1, ex0)
+  int nm1;              // n - 1
+};
+// All threads of the CTA; the caller synchronises before first use.  mem: LG_DOUBLES doubles, 16-byte aligned.
+__device__ __forceinline__ LogGrid lg_build(double* mem, const double lo, const double inv_h, const int n) {
+  double2* mt = reinterpret_cast<double2*>(mem);
+  const double A = 0.5 * inv_h, B = -lo * inv_h;
+  for (int j = threadIdx.x; j < LG_NM; j += blockDim.x) {
+    const double c = 1.0 + ((double)j + 0.5) * (1.0 / (double)LG_NM);
+    const double inv = 1.0 / c;
+    const double2 ent = make_double2(inv, -A * log(inv));
+#pragma unroll
+    for (int r = 0; r < LG_REP; ++r) mt[j * LG_REP + r] = ent;
+  }
+  LogGrid L;
+  L.mant = mt + (threadIdx.x & (LG_REP - 1));
+  L.A = A;
+  L.ex1 = A * 0.6931471805599453;
+  L.ex0 = fma(-1023.0, L.ex1, B);
+  L.nm1 = n - 1;
+  return L;
+}
+__device__ __forceinline__ double lg_coord(const LogGrid& L, const double* __restrict__ kc, const double s) {
+  const unsigned hi = (unsigned)__double2hiint(s);
+  const double m = __hiloint2double((int)((hi & 0x000fffffu) | 0x3ff00000u), __double2loint(s));
+  const double2 T = L.mant[((hi >> 11) & (LG_NM - 1)) * LG_REP];
+  const double ex = fma((double)(int)(hi >> 20), L.ex1, L.ex0);
+  const double r = fma(m, T.x, -1.0);
+  double q = fma(r, kc[2], kc[3]);          // 1/3 - r/4
+  q = fma(r, q, kc[4]);                     // -1/2 + r/3 - r^2/4
+  const double lm = fma(r * r, q, r);       // ln(1 + r)
+  return fma(lm, L.A, T.y) + ex;
+}
+// Guarded cells of one table row, replicated: n + 1 cells x 2 halves x LG_REP double2.  cells_guarded_size(n) double2.
+// v may live in shared or global memory.  All threads; caller synchronises.  Returns this thread's copy.
+__device__ __host__ constexpr int cells_guarded_size(int n) { return (n + 1) * 2 * LG_REP; }
+__device__ __forceinline__ const double2* cells_build_guarded(double2* cells, const double* __restrict__ v,
+                                                              const int n, const int interp) {
+  for (int c = threadIdx.x; c <= n; c += blockDim.x) {
+    const int F = c - 1;
+    double4 k;
+    if (F < 0) k = make_double4(v[0], 0.0, 0.0, 0.0);
+    else if (F >= n - 1) k = make_double4(v[n - 1], 0.0, 0.0, 0.0);
+    else if (interp == 3) {
+      int i0 = F - 1;
+      i0 = i0 < 0 ? 0 : i0;
+      i0 = i0 > n - 4 ? n - 4 : i0;
+      const int dl = F - i0;  // anchor node inside the stencil: 0, 1 or 2
+      const double v0 = v[i0], v1 = v[i0 + 1], v2 = v[i0 + 2], v3 = v[i0 + 3];
+      const double d3 = ((v3 - v0) + 3.0 * (v1 - v2)) * (1.0 / 6.0);
+      if (dl == 0)
+        k = make_double4(v0, (-11.0 * v0 + 18.0 * v1 - 9.0 * v2 + 2.0 * v3) * (1.0 / 6.0),
+                         (2.0 * v0 - 5.0 * v1 + 4.0 * v2 - v3) * 0.5, d3);
+      else if (dl == 1)
+        k = make_double4(v1, (-2.0 * v0 - 3.0 * v1 + 6.0 * v2 - v3) * (1.0 / 6.0), (v0 - 2.0 * v1 + v2) * 0.5, d3);
+      else
+        k = make_double4(v2, (v0 - 6.0 * v1 + 3.0 * v2 + 2.0 * v3) * (1.0 / 6.0), (v1 - 2.0 * v2 + v3) * 0.5, d3);
+    } else {
+      k = make_double4(v[F], v[F + 1] - v[F], 0.0, 0.0);
+    }
+#pragma unroll
+    for (int r = 0; r < LG_REP; ++r) {
+      cells[(2 * c) * LG_REP + r] = make_double2(k.x, k.y);
+      cells[(2 * c + 1) * LG_REP + r] = make_double2(k.z, k.w);
+    }
+  }
+  return cells + (threadIdx.x & (LG_REP - 1));
+}
+// cells: this thread's copy (the pointer cells_build_guarded returns)
+__device__ __forceinline__ double lg_cell_eval(const double2* __restrict__ cells, const LogGrid& L, const double t) {
+  int F = __double2int_rd(t);  // F2I.FLOOR: saturates, NaN -> 0
+  F = max(F, -1);
+  F = min(F, L.nm1);
+  const double tau = t - (double)F;
+  const double2* cp = cells + (F + 1) * (2 * LG_REP);
+  const double2 k0 = cp[0], k1 = cp[LG_REP];
+  return fma(fma(fma(k1.y, tau, k1.x), tau, k0.y), tau, k0.x);
+}
+__device__ __forceinline__ double lg_lookup(const double2* __restrict__ cells, const LogGrid& L,
+                                            const double* __restrict__ kc, const double s) {
+  return lg_cell_eval(cells, L, lg_coord(L, kc, s));
+}
+
+// k^2 e^-x from a table of k^2 2^(j/64), replicated 16 times (one copy per lane & 15: a 64-bit shared-memory load is
+// served in half-warps, so the look-up is conflict free):  n = rint(-64 x / ln2), r = -x - n ln2/64, |r| <= ln2/128,
+// e^r by its series to r^5/120.  x is clamped to 700 (e^-700 = 1e-304).
+constexpr int FX_REP = 16;
+constexpr int FX_DOUBLES = 64 * FX_REP;
+__device__ __forceinline__ const double* fx_build(double* mem, const double k2) {
+  for (int j = threadIdx.x; j < 64; j += blockDim.x) {
+    const double v = k2 * exp2((double)j * (1.0 / 64.0));
+#pragma unroll
+    for (int r = 0; r < FX_REP; ++r) mem[j * FX_REP + r] = v;
+  }
+  return mem + (threadIdx.x & (FX_REP - 1));
+}
+__device__ __forceinline__ double fx_exp_neg(const double* __restrict__ tab, const double* __restrict__ kc, double x) {
+  x = clamp_hi(x, 700.0);
+  const double MAGIC = kc[8];
+  const double y = fma(x, kc[7], MAGIC);
+  const int n = __double2loint(y);
+  const double nd = y - MAGIC;
+  double r = fma(nd, kc[9], -x);
+  r = fma(nd, kc[10], r);
+  double p = fma(r, kc[11], kc[12]);
+  p = fma(r, p, kc[13]);
+  p = fma(r, p, kc[14]);
+  p = fma(r, p, kc[15]);
+  p = fma(r, p, kc[15]);
+  const double v = tab[(n & 63) * FX_REP] * p;
+  return __hiloint2double(__double2hiint(v) + ((n >> 6) << 20), __double2loint(v));
 }
 
 __device__ __forceinline__ double ipow(double x, int e) {
