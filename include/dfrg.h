@@ -141,6 +141,11 @@ typedef struct {
   dfrg_table tab[3];
   const double* coef;
   int n_coef;
+  int ext_outer; /* three-point only; 0 or 1: no layout promised.  G >= 2: the caller promises a product grid,
+                    n_ext = G S and ext[a S + r] = (|p1|_a, |p2|_r, alpha_r) for a < G, r < S (the paper's vertex
+                    grids), which lets the library share everything that depends on |p1| alone or on
+                    (|p2|, alpha) alone.  The promise is checked on the device; if it does not hold the general
+                    path runs and the results are the same.  Ignored (general path) if G > 256 or cos2.n > 512. */
 } dfrg_loop4d_desc;
 
 int dfrg_integrate_loop4d(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext, const double* ext,

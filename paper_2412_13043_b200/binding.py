@@ -49,7 +49,7 @@ class LpaDesc(C.Structure):
 class Loop4dDesc(C.Structure):
     _fields_ = [("family", C.c_int), ("prefactor", C.c_double), ("reg", Regulator),
                 ("q", Rule), ("cos1", Rule), ("cos2", Rule), ("phi", Rule),
-                ("tab", Table * 3), ("coef", _vp), ("n_coef", C.c_int)]
+                ("tab", Table * 3), ("coef", _vp), ("n_coef", C.c_int), ("ext_outer", C.c_int)]
 
 
 class Mats3dDesc(C.Structure):
@@ -175,13 +175,13 @@ def dfrg_integrate_lpa_host(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_
 
 # ---- loop4d ---------------------------------------------------------------------------------------
 def _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
-                 lnq_hi, interp, coef, device):
+                 lnq_hi, interp, coef, device, ext_outer=0):
     T3 = Table * 3
     tt = [_table(t, lnq_lo, lnq_hi, interp, device) for t in tabs] + [_table(None, 0, 0, 0, device)] * (3 - len(tabs))
     n_coef = coef.numel() if hasattr(coef, "numel") else coef.size
     return Loop4dDesc(int(family), float(prefactor), Regulator(int(reg_kind), int(reg_order), float(k)),
                       _rule(rule_q, device), _rule(rule_c1, device), _rule(rule_c2, device), _rule(rule_phi, device),
-                      T3(*tt), _ptr(coef, device), int(n_coef))
+                      T3(*tt), _ptr(coef, device), int(n_coef), int(ext_outer))
 
 
 def _n(a):
@@ -189,11 +189,11 @@ def _n(a):
 
 
 def dfrg_integrate_loop4d(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs,
-                          lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None):
+                          lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0):
     """two-point: tabs=(Z,), m2=[n_field], ext=[n_ext] -> out [n_ext, n_field];
-    three-point: tabs=(Z_A, Z_c, lambda3), m2=None, ext=[n_ext, 3] -> out [n_ext]."""
+    three-point: tabs=(Z_A, Z_c, lambda3), m2=None, ext=[n_ext, 3] -> out [n_ext]; ext_outer: dfrg_loop4d_desc."""
     D = _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
-                     lnq_hi, interp, coef, True)
+                     lnq_hi, interp, coef, True, ext_outer)
     n_ext = _n(ext) if family == LOOP_TWOPOINT else _n(ext) // 3
     _check(lib().dfrg_integrate_loop4d(C.byref(D), _n(m2), _ptr(m2, True), n_ext, _ptr(ext, True),
                                        _ptr(out, True), _ptr(dmin, True), _stream()), "dfrg_integrate_loop4d")
@@ -201,9 +201,9 @@ def dfrg_integrate_loop4d(family, prefactor, reg_kind, reg_order, k, rule_q, rul
 
 
 def dfrg_integrate_loop4d_host(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs,
-                               lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None):
+                               lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0):
     D = _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
-                     lnq_hi, interp, coef, False)
+                     lnq_hi, interp, coef, False, ext_outer)
     n_ext = _n(ext) if family == LOOP_TWOPOINT else _n(ext) // 3
     _check(lib().dfrg_integrate_loop4d_host(C.byref(D), _n(m2), _ptr(m2, False), n_ext, _ptr(ext, False),
                                             _ptr(out, False), _ptr(dmin, False)), "dfrg_integrate_loop4d_host")

@@ -155,6 +155,7 @@ struct ThreePointParams {
   FastMathConsts fmc;
   const double *xq, *wq, *x1, *w1, *x2, *w2, *wphi, *ZA, *L3, *coef, *ext;
   double *out, *dmin;
+  const int* skip_flag;  // nullable; the general kernel returns at once if *skip_flag == 0 (product-grid path did the work)
 };
 
 template <bool WANT_DMIN>
@@ -313,6 +314,7 @@ __global__ void __launch_bounds__(T3V2_THREADS, 1) threepoint_kernel_v2(const Th
   __shared__ __align__(8) uint64_t bar;
   __shared__ double red[32];
 
+  if (P.skip_flag && *P.skip_flag == 0) return;
   const int nq = P.nq, n1 = P.n1, n2 = P.n2, nt = P.grid.n;
   double* sxq = reinterpret_cast<double*>(smem_raw);
   double* swq = sxq + ((nq + 1) & ~1);
@@ -448,6 +450,337 @@ static size_t threepoint_v2_smem(int nq, int n1, int n2, int nt) {
                       FM_DOUBLES + FX_DOUBLES + LG_DOUBLES + 2 * cells_guarded_size(nt) * 2 + 2 * nq + 2 * n2);
 }
 
+// =====================================================================================================
+// three-point on a product grid of external momenta
+// =====================================================================================================
+// When the external configurations form a product  ext[a S + r] = (|p1|_a, |p2|_r, alpha_r),  a < G, r < S
+// (BASELINE.json config 3: 32 |p1| x (32 |p2| x 8 alpha); the paper's vertex grids are of this kind,
+// PAPER.md:336), almost everything in a node is shared:
+//   depends on (|p2|, alpha) only -- shared by the G values of |p1|:   s_b, G_A(s_b), lambda3((p2^2+q^2+s_b)/3), z = q.p2/k^2
+//   depends on |p1| only          -- shared by the S pairs (|p2|, alpha): s_a, G_A(s_a), lambda3((p1^2+q^2+s_a)/3), the five
+//                                                                       coefficients of P as a quartic in z
+// and only  lambda3((s_c + s_a + s_b)/3)  and the Horner evaluation of P are left per (a, r, node): 19 FP64 instructions
+// instead of 66.  The caller promises the layout through dfrg_loop4d_desc::ext_outer = G; the pre-pass kernel checks it
+// on the device and, if it does not hold, the product-grid kernels return at once and the general kernel runs instead
+// (both are enqueued; the one that is not needed exits after reading one flag).
+//
+//  (1) t3g_prepass_kernel: promise check; tabR[r] = (|p2|, cos alpha, sin alpha); tabA[pair][0..7][a] for every (q, c1) pair:
+//        w0 = wq q^3 Rdot(q^2) G_A(q^2) w1 sqrt(1-c1^2) G_A(s_a) lambda3(.),  s_a/3,  the five quartic coefficients,  D_a.
+//  (2) t3g_main_kernel: persistent, one CTA per SM.  Work unit = (r, chunk of KP pairs); the units are dealt to the
+//      CTAs in contiguous ranges.  Phase 1 (all threads, one unit ahead, double buffered): the shared node data
+//      (w2 G_A(s_b) lambda3(.), s_b/3, z) of the unit's KP x n2 nodes into shared memory.  Phase 2: thread = (a, pair
+//      slot); per node one look-up, one Horner, two multiply-adds; the shared node data are warp-uniform broadcasts.
+//      A thread keeps the running sum of its a while the CTA stays inside one r; the partial sums of an output are
+//      written per CTA ("slot") and added in fixed order by
+//  (3) t3g_fixup_kernel (deterministic: the ownership of units is a pure function of the grid size).
+struct ThreeGridParams {
+  ThreePointParams B;
+  int G, S;        // n_ext = G S
+  int KP, NCH;     // pairs per chunk, chunks per r
+  int grid_main, max_slots;
+  double* tabA;    // [npairs][8][G]
+  double* tabR;    // [S][4]
+  double* qmin;    // [1]   min over radial nodes of D(q^2)
+  int* flag;       // [1]   != 0: the layout promise does not hold
+  double* part;    // [max_slots][n_ext]
+  double* partB;   // [max_slots][S]  min over the slot's nodes of D_b
+};
+
+constexpr int T3G_THREADS = 256;
+constexpr int T3G_NODES = 512;  // shared nodes per unit buffer
+
+// common shared-memory carve-up of the two product-grid kernels
+struct T3GShared {
+  double *sxq, *swq, *sx1, *sw1, *sx2, *sw2, *sZA, *sL3, *skap, *fmmem, *fxmem, *lgmem;
+  double2 *cZA_all, *cL3_all, *qtab, *xw2, *nodeA;
+  double *nodeZ, *red;
+};
+__device__ __forceinline__ T3GShared t3g_carve(unsigned char* raw, int nq, int n1, int n2, int nt) {
+  T3GShared s;
+  s.sxq = reinterpret_cast<double*>(raw);
+  s.swq = s.sxq + ((nq + 1) & ~1);
+  s.sx1 = s.swq + ((nq + 1) & ~1);
+  s.sw1 = s.sx1 + ((n1 + 1) & ~1);
+  s.sx2 = s.sw1 + ((n1 + 1) & ~1);
+  s.sw2 = s.sx2 + ((n2 + 1) & ~1);
+  s.sZA = s.sw2 + ((n2 + 1) & ~1);
+  s.sL3 = s.sZA + ((nt + 1) & ~1);
+  s.skap = s.sL3 + ((nt + 1) & ~1);  // 36
+  s.fmmem = s.skap + 36;
+  s.fxmem = s.fmmem + FM_DOUBLES;
+  s.lgmem = s.fxmem + FX_DOUBLES;
+  s.cZA_all = reinterpret_cast<double2*>(s.lgmem + LG_DOUBLES);
+  s.cL3_all = s.cZA_all + cells_guarded_size(nt);
+  s.qtab = s.cL3_all + cells_guarded_size(nt);
+  s.xw2 = s.qtab + nq;
+  s.nodeA = s.xw2 + n2;                                          // [2][T3G_NODES]
+  s.nodeZ = reinterpret_cast<double*>(s.nodeA + 2 * T3G_NODES);  // [2][T3G_NODES]
+  s.red = s.nodeZ + 2 * T3G_NODES;                               // [T3G_THREADS]
+  return s;
+}
+static size_t t3g_smem(int nq, int n1, int n2, int nt) {
+  return 8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((n1 + 1) & ~1) + 2 * ((n2 + 1) & ~1) + 2 * ((nt + 1) & ~1) + 36 +
+                      FM_DOUBLES + FX_DOUBLES + LG_DOUBLES + 2 * cells_guarded_size(nt) * 2 + 2 * nq + 2 * n2 +
+                      2 * 2 * T3G_NODES + 2 * T3G_NODES + T3G_THREADS);
+}
+
+template <int REGK>
+__global__ void __launch_bounds__(T3G_THREADS, 1) t3g_prepass_kernel(const ThreeGridParams Q) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t bar;
+  __shared__ double red[32];
+  const ThreePointParams& P = Q.B;
+  const int nq = P.nq, n1 = P.n1, n2 = P.n2, nt = P.grid.n, G = Q.G, S = Q.S;
+  const T3GShared sm = t3g_carve(smem_raw, nq, n1, n2, nt);
+
+  if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
+  __syncthreads();
+  {
+    StageList L;
+    L.add(sm.sxq, P.xq, nq); L.add(sm.swq, P.wq, nq);
+    L.add(sm.sx1, P.x1, n1); L.add(sm.sw1, P.w1, n1);
+    L.add(sm.sZA, P.ZA, nt); L.add(sm.sL3, P.L3, nt);
+    stage_to_smem(L, &bar, 0);
+  }
+  const FastMath fm = fm_build(sm.fmmem, P.fmc);
+  const double* fxtab = fx_build(sm.fxmem, P.reg.k2);
+  const LogGrid lg = lg_build(sm.lgmem, P.grid.lo, P.grid.inv_h, nt);
+  const double* kc = P.fmc.c;
+  const double2* cZA = cells_build_guarded(sm.cZA_all, sm.sZA, nt, P.grid.interp);
+  const double2* cL3 = cells_build_guarded(sm.cL3_all, sm.sL3, nt, P.grid.interp);
+  if (threadIdx.x < 35) sm.skap[threadIdx.x] = P.coef[threadIdx.x];
+  __syncthreads();
+
+  const double ik2 = P.reg.inv_k2, third = 1.0 / 3.0;
+  const long long gtid = (long long)blockIdx.x * T3G_THREADS + threadIdx.x, gstride = (long long)gridDim.x * T3G_THREADS;
+  // promise check
+  for (long long e = gtid; e < P.n_ext; e += gstride) {
+    const long long a = e / S, r = e - a * S;
+    const bool ok = P.ext[3 * e] == P.ext[3 * (a * S)] && P.ext[3 * e + 1] == P.ext[3 * r + 1] &&
+                    P.ext[3 * e + 2] == P.ext[3 * r + 2];
+    if (!ok) *Q.flag = 1;
+  }
+  for (long long r = gtid; r < S; r += gstride) {
+    double sa_, ca_;
+    sincos(P.ext[3 * r + 2], &sa_, &ca_);
+    Q.tabR[4 * r] = P.ext[3 * r + 1]; Q.tabR[4 * r + 1] = ca_; Q.tabR[4 * r + 2] = sa_; Q.tabR[4 * r + 3] = 0.0;
+  }
+  // radial table (every CTA builds its own copy)
+  double dmq = __longlong_as_double(0x7ff0000000000000LL);
+  for (int i = threadIdx.x; i < nq; i += T3G_THREADS) {
+    const double q = sm.sxq[i], sq = q * q;
+    double Rq, Rdq;
+    regulator(P.reg, fm, sq, Rq, Rdq);
+    const double Dq = lg_lookup(cZA, lg, kc, sq) * sq + Rq;
+    sm.qtab[i] = make_double2((sm.swq[i] * q * q * q * Rdq) * fast_rcp(Dq), Dq);
+    dmq = fmin(dmq, Dq);
+  }
+  dmq = block_min(dmq, red);  // also publishes qtab
+  if (blockIdx.x == 0 && threadIdx.x == 0) *Q.qmin = dmq;
+
+  const long long n_items = (long long)nq * n1 * G;
+  for (long long it = gtid; it < n_items; it += gstride) {
+    const int pair = (int)(it / G), a = (int)(it - (long long)pair * G);
+    const int i = pair / n1, j1 = pair - i * n1;
+    const double p1 = P.ext[3 * ((long long)a * S)];
+    const double q = sm.sxq[i], c1 = sm.sx1[j1];
+    const double sq = q * q;
+    const double sin1 = sqrt((1.0 - c1) * (1.0 + c1));
+    const double wpair = sm.qtab[i].x * (sm.sw1[j1] * sin1);
+    const double qp1 = q * p1 * c1;
+    double s_a = sq + p1 * p1 + 2.0 * qp1;
+    s_a = clamp_lo(s_a, 0.0);
+    const double Da = fma(lg_lookup(cZA, lg, kc, s_a), s_a, t3_reg_R<REGK>(P.reg, fxtab, kc, s_a));
+    const double Ga = fast_rcp(Da);
+    const double lam1 = lg_lookup(cL3, lg, kc, (p1 * p1 + sq + s_a) * third);
+    const double X = sq * ik2, Y = qp1 * ik2;
+    double gam[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    {
+      int idx = 0;
+      double Xa = 1.0;
+#pragma unroll
+      for (int aa = 0; aa <= 4; ++aa) {
+        double XaYb = Xa;
+#pragma unroll
+        for (int b = 0; b <= 4 - aa; ++b) {
+#pragma unroll
+          for (int c = 0; c <= 4 - aa - b; ++c) gam[c] = fma(sm.skap[idx++], XaYb, gam[c]);
+          XaYb *= Y;
+        }
+        Xa *= X;
+      }
+    }
+    double* ta = Q.tabA + ((size_t)pair * 8) * G + a;
+    ta[0] = wpair * (Ga * lam1);
+    ta[(size_t)G] = s_a * third;
+#pragma unroll
+    for (int c = 0; c < 5; ++c) ta[(size_t)(2 + c) * G] = gam[c];
+    ta[(size_t)7 * G] = Da;
+  }
+}
+
+template <int REGK>
+__global__ void __launch_bounds__(T3G_THREADS, 1) t3g_main_kernel(const ThreeGridParams Q) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t bar;
+  __shared__ double red32[32];
+  if (*Q.flag != 0) return;  // the layout promise does not hold: the general kernel does the work
+  const ThreePointParams& P = Q.B;
+  const int nq = P.nq, n1 = P.n1, n2 = P.n2, nt = P.grid.n, G = Q.G, S = Q.S, KP = Q.KP, NCH = Q.NCH;
+  const int npairs = nq * n1;
+  const T3GShared sm = t3g_carve(smem_raw, nq, n1, n2, nt);
+  const int tid = threadIdx.x;
+
+  if (tid == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
+  __syncthreads();
+  {
+    StageList L;
+    L.add(sm.sxq, P.xq, nq);
+    L.add(sm.sx1, P.x1, n1);
+    L.add(sm.sx2, P.x2, n2); L.add(sm.sw2, P.w2, n2);
+    L.add(sm.sZA, P.ZA, nt); L.add(sm.sL3, P.L3, nt);
+    stage_to_smem(L, &bar, 0);
+  }
+  const double* fxtab = fx_build(sm.fxmem, P.reg.k2);
+  const LogGrid lg = lg_build(sm.lgmem, P.grid.lo, P.grid.inv_h, nt);
+  const double* kc = P.fmc.c;
+  const double2* cZA = cells_build_guarded(sm.cZA_all, sm.sZA, nt, P.grid.interp);
+  const double2* cL3 = cells_build_guarded(sm.cL3_all, sm.sL3, nt, P.grid.interp);
+  for (int j = tid; j < n2; j += T3G_THREADS) sm.xw2[j] = make_double2(sm.sx2[j], sm.sw2[j]);
+  __syncthreads();
+
+  const double ik2 = P.reg.inv_k2, third = 1.0 / 3.0, m2k2 = -2.0 * P.reg.k2;
+  const double inf = __longlong_as_double(0x7ff0000000000000LL);
+  const long long U = (long long)S * NCH;
+  const long long u0 = (long long)blockIdx.x * U / gridDim.x, u1 = (long long)(blockIdx.x + 1) * U / gridDim.x;
+  const int nw = T3G_THREADS / G;                 // pair slots
+  const bool active = tid < nw * G;
+  const int a = tid % G, w = tid / G;
+  const double p1 = P.ext[3 * ((long long)a * S)];
+
+  double dmB_cur = inf, dmB_nxt = inf;
+  // Phase 1: shared node data of unit u into buffer b
+  auto phase1 = [&](long long u, int b, double& dmB) {
+    const int r = (int)(u / NCH), ch = (int)(u - (long long)r * NCH);
+    const int pair0 = ch * KP;
+    const int npl = min(KP, npairs - pair0);
+    const double p2 = Q.tabR[4 * r], ca_ = Q.tabR[4 * r + 1], sa_ = Q.tabR[4 * r + 2];
+    double2* nA = sm.nodeA + b * T3G_NODES;
+    double* nZ = sm.nodeZ + b * T3G_NODES;
+    for (int n = tid; n < npl * n2; n += T3G_THREADS) {
+      const int pl = n / n2, j2 = n - pl * n2;
+      const int pair = pair0 + pl;
+      const int i = pair / n1, j1 = pair - i * n1;
+      const double q = sm.sxq[i], c1 = sm.sx1[j1];
+      const double sq = q * q;
+      const double sin1 = sqrt((1.0 - c1) * (1.0 + c1));
+      const double zc = q * p2 * ca_ * c1 * ik2;
+      const double zs = q * p2 * sa_ * sin1 * ik2;
+      const double sb0 = sq + p2 * p2;
+      const double2 xw = sm.xw2[j2];
+      const double z = fma(zs, xw.x, zc);
+      double s_b = fma(m2k2, z, sb0);
+      s_b = clamp_lo(s_b, 0.0);
+      const double Db = fma(lg_lookup(cZA, lg, kc, s_b), s_b, t3_reg_R<REGK>(P.reg, fxtab, kc, s_b));
+      dmB = fmin(dmB, Db);
+      const double lam2 = lg_lookup(cL3, lg, kc, fma(s_b, third, sb0 * third));
+      nA[n] = make_double2(xw.y * (fast_rcp(Db) * lam2), s_b * third);
+      nZ[n] = z;
+    }
+  };
+
+  double acc = 0.0;
+  if (u0 < u1) phase1(u0, 0, dmB_cur);
+  __syncthreads();
+  for (long long u = u0; u < u1; ++u) {
+    const int b = (int)((u - u0) & 1);
+    const int r = (int)(u / NCH), ch = (int)(u - (long long)r * NCH);
+    const bool last_of_r = (u + 1 == u1) || ((u + 1) / NCH != r);
+    if (u + 1 < u1) phase1(u + 1, b ^ 1, last_of_r ? dmB_nxt : dmB_cur);
+    // ---- phase 2 ----
+    const int pair0 = ch * KP;
+    const int npl = min(KP, npairs - pair0);
+    if (active) {
+      const double p2 = Q.tabR[4 * r], ca_ = Q.tabR[4 * r + 1];
+      double scc = p1 * p1 + p2 * p2 + 2.0 * p1 * p2 * ca_;
+      scc = scc > 0.0 ? scc : 0.0;
+      const double scc3 = scc * third;
+      const double2* nA = sm.nodeA + b * T3G_NODES;
+      const double* nZ = sm.nodeZ + b * T3G_NODES;
+      double cur[7], nxt[7];
+      if (w < npl) {
+        const double* ta = Q.tabA + ((size_t)(pair0 + w) * 8) * G + a;
+#pragma unroll
+        for (int c = 0; c < 7; ++c) cur[c] = ta[(size_t)c * G];
+      }
+      for (int pl = w; pl < npl; pl += nw) {
+        if (pl + nw < npl) {
+          const double* ta = Q.tabA + ((size_t)(pair0 + pl + nw) * 8) * G + a;
+#pragma unroll
+          for (int c = 0; c < 7; ++c) nxt[c] = ta[(size_t)c * G];
+        }
+        const double l30 = cur[1] + scc3;
+        const double2* na = nA + pl * n2;
+        const double* nz = nZ + pl * n2;
+        double acc2 = 0.0;
+#pragma unroll 8
+        for (int j2 = 0; j2 < n2; ++j2) {
+          const double2 bs = na[j2];
+          const double z = nz[j2];
+          const double lam3 = lg_lookup(cL3, lg, kc, bs.y + l30);
+          const double poly = fma(fma(fma(fma(cur[6], z, cur[5]), z, cur[4]), z, cur[3]), z, cur[2]);
+          acc2 = fma(bs.x * poly, lam3, acc2);
+        }
+        acc = fma(cur[0], acc2, acc);
+#pragma unroll
+        for (int c = 0; c < 7; ++c) cur[c] = nxt[c];
+      }
+    }
+    if (last_of_r) {
+      // partial sums of this CTA for r: slot = rank of this CTA among the owners of r's units
+      const long long ufirst = (long long)r * NCH;
+      const int c_first = (int)(((ufirst + 1) * gridDim.x - 1) / U);
+      const int slot = (int)blockIdx.x - c_first;
+      sm.red[tid] = active ? acc : 0.0;
+      const double dB = block_min(dmB_cur, red32);  // two barriers: also publishes sm.red
+      if (tid < G) {
+        double t = sm.red[tid];
+        for (int ww = 1; ww < nw; ++ww) t += sm.red[tid + ww * G];
+        Q.part[(size_t)slot * P.n_ext + (size_t)tid * S + r] = t;
+      }
+      if (tid == 0) Q.partB[(size_t)slot * S + r] = dB;
+      acc = 0.0;
+      dmB_cur = dmB_nxt;
+      dmB_nxt = inf;
+    }
+    __syncthreads();  // unit u is drained: its buffer may be refilled; the stage of unit u+1 is complete
+  }
+}
+
+__global__ void __launch_bounds__(256) t3g_fixup_kernel(const ThreeGridParams Q) {
+  if (*Q.flag != 0) return;
+  const ThreePointParams& P = Q.B;
+  const long long e = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (e >= P.n_ext) return;
+  const int S = Q.S, G = Q.G, NCH = Q.NCH;
+  const int a = (int)(e / S), r = (int)(e - (long long)a * S);
+  const long long U = (long long)S * NCH;
+  const long long ufirst = (long long)r * NCH, ulast = ufirst + NCH - 1;
+  const int c_first = (int)(((ufirst + 1) * Q.grid_main - 1) / U), c_last = (int)(((ulast + 1) * Q.grid_main - 1) / U);
+  double t = Q.part[e];
+  for (int s = 1; s <= c_last - c_first; ++s) t += Q.part[(size_t)s * P.n_ext + e];
+  double sum_wphi = 0.0;
+  for (int jp = 0; jp < P.nphi; ++jp) sum_wphi += P.wphi[jp];
+  P.out[e] = P.prefactor * sum_wphi * t;
+  if (P.dmin) {
+    double dm = *Q.qmin;
+    for (int s = 0; s <= c_last - c_first; ++s) dm = fmin(dm, Q.partB[(size_t)s * S + r]);
+    const int npairs = P.nq * P.n1;
+    for (int pair = 0; pair < npairs; ++pair) dm = fmin(dm, Q.tabA[((size_t)pair * 8 + 7) * G + a]);
+    P.dmin[e] = dm * P.reg.inv_k2;
+  }
+}
+
 static size_t threepoint_smem(int nq, int n1, int n2, int nt) {
   return 8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((n1 + 1) & ~1) + 2 * ((n2 + 1) & ~1) + 2 * ((nt + 1) & ~1) + 36 +
                       FM_DOUBLES + 8 * nt + 2 * nq);
@@ -511,6 +844,51 @@ static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m
   P.fmc = fm_consts();
   P.xq = D->q.x; P.wq = D->q.w; P.x1 = D->cos1.x; P.w1 = D->cos1.w; P.x2 = D->cos2.x; P.w2 = D->cos2.w; P.wphi = D->phi.w;
   P.ZA = D->tab[0].v; P.L3 = D->tab[2].v; P.coef = D->coef; P.ext = ext; P.out = out; P.dmin = dmin;
+  P.skip_flag = nullptr;
+  const int regk = D->reg.kind == DFRG_REG_LITIM ? 0 : (D->reg.order == 1 ? 1 : 2);
+  void* scratch = nullptr;
+  // ---- product-grid path (ext_outer = G promised by the caller, checked on the device) ----
+  const char* vgrid = getenv("DFRG_T3_GRID");
+  const int G = D->ext_outer;
+  if (G >= 2 && G <= T3G_THREADS && n_ext % G == 0 && P.n2 <= T3G_NODES && !(vgrid && vgrid[0] == '0')) {
+    ThreeGridParams Q;
+    Q.B = P;
+    Q.G = G; Q.S = n_ext / G;
+    const int npairs = P.nq * P.n1;
+    Q.KP = T3G_NODES / P.n2 < npairs ? T3G_NODES / P.n2 : npairs;
+    Q.NCH = (npairs + Q.KP - 1) / Q.KP;
+    const long long U = (long long)Q.S * Q.NCH;
+    Q.grid_main = (int)(U < sm_count ? U : sm_count);
+    Q.max_slots = 1;
+    for (int r = 0; r < Q.S; ++r) {
+      const long long ufirst = (long long)r * Q.NCH, ulast = ufirst + Q.NCH - 1;
+      const int c0 = (int)(((ufirst + 1) * Q.grid_main - 1) / U), c1 = (int)(((ulast + 1) * Q.grid_main - 1) / U);
+      if (c1 - c0 + 1 > Q.max_slots) Q.max_slots = c1 - c0 + 1;
+    }
+    const size_t n_tabA = (size_t)npairs * 8 * G, n_tabR = 4 * (size_t)Q.S, n_part = (size_t)Q.max_slots * n_ext,
+                 n_partB = (size_t)Q.max_slots * Q.S;
+    int rc = scratch_alloc(&scratch, (n_tabA + n_tabR + n_part + n_partB + 4) * sizeof(double), stream);
+    if (rc != DFRG_OK) return rc;
+    Q.tabA = (double*)scratch;
+    Q.tabR = Q.tabA + n_tabA;
+    Q.part = Q.tabR + n_tabR;
+    Q.partB = Q.part + n_part;
+    Q.qmin = Q.partB + n_partB;
+    Q.flag = (int*)(Q.qmin + 2);
+    cudaError_t e = cudaMemsetAsync(Q.flag, 0, sizeof(int), stream);
+    const size_t smem_g = t3g_smem(P.nq, P.n1, P.n2, P.grid.n);
+    void (*kpre)(const ThreeGridParams) = regk == 0 ? t3g_prepass_kernel<0> : (regk == 1 ? t3g_prepass_kernel<1> : t3g_prepass_kernel<2>);
+    void (*kmain)(const ThreeGridParams) = regk == 0 ? t3g_main_kernel<0> : (regk == 1 ? t3g_main_kernel<1> : t3g_main_kernel<2>);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kpre, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kmain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g);
+    if (e != cudaSuccess) { scratch_free(scratch, stream); return check_cuda(e); }
+    kpre<<<sm_count, T3G_THREADS, smem_g, stream>>>(Q);
+    kmain<<<Q.grid_main, T3G_THREADS, smem_g, stream>>>(Q);
+    t3g_fixup_kernel<<<(n_ext + 255) / 256, 256, 0, stream>>>(Q);
+    rc = check_cuda(cudaGetLastError());
+    if (rc != DFRG_OK) { scratch_free(scratch, stream); return rc; }
+    P.skip_flag = Q.flag;  // the general kernel below runs only if the promise turned out false
+  }
   int grid = n_ext < 2 * sm_count ? n_ext : 2 * sm_count;  // persistent: 2 CTAs per SM
   const char* vpath = getenv("DFRG_T3_PATH");
   if (vpath && vpath[0] == 'o') {
@@ -522,17 +900,18 @@ static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m
     return check_cuda(cudaGetLastError());
   }
   const size_t smem = threepoint_v2_smem(P.nq, P.n1, P.n2, P.grid.n);
-  const int regk = D->reg.kind == DFRG_REG_LITIM ? 0 : (D->reg.order == 1 ? 1 : 2);
   void (*kern)(const ThreePointParams) = nullptr;
 #define DFRG_T3_PICK(K) if (regk == K) kern = dmin ? threepoint_kernel_v2<K, true, 256, 8> : threepoint_kernel_v2<K, false, 256, 8>;
   DFRG_T3_PICK(0) DFRG_T3_PICK(1) DFRG_T3_PICK(2)
 #undef DFRG_T3_PICK
   const int nthreads = 256;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return check_cuda(e);
+  if (e != cudaSuccess) { scratch_free(scratch, stream); return check_cuda(e); }
   grid = n_ext < sm_count ? n_ext : sm_count;  // persistent: 1 CTA of 256 threads x 240 registers per SM (replicated tables: 140 KB)
   kern<<<grid, nthreads, smem, stream>>>(P);
-  return check_cuda(cudaGetLastError());
+  const int rc_last = check_cuda(cudaGetLastError());
+  scratch_free(scratch, stream);
+  return rc_last;
 }
 
 }  // namespace dfrg

@@ -132,7 +132,7 @@ def config3(n_p=32, n_alpha=8, n_q=96, n_c1=32, n_c2=16, n_phi=16, n_tab=128, k=
                 rule_q=(n_q, 0.0, 8.0 * k), rule_c1=(n_c1, -1.0, 1.0), rule_c2=(n_c2, -1.0, 1.0),
                 rule_phi=(n_phi, 0.0, 2.0 * math.pi),
                 ZA=ZA, Zc=Zc, L3=L3, lnq_lo=lo, lnq_hi=hi, interp=interp,
-                coef=coef, ext=ext.reshape(-1, 3))
+                coef=coef, ext=ext.reshape(-1, 3), ext_outer=n_p)  # product grid: |p1| outermost
 
 
 def config4(n_field=512, n_p=64, n_jext=16, n_q=96, n_c=24, n_tab=128, n_freq=64,

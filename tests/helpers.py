@@ -83,7 +83,7 @@ def gpu_run(c, R, host=False, want_dmin=True):
         fn = B.dfrg_integrate_loop4d_host if host else B.dfrg_integrate_loop4d
         fn(B.LOOP_THREEPOINT, c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], rule("q"), rule("c1"),
            rule("c2"), rule("phi"), (up(c["ZA"]), up(c["Zc"]), up(c["L3"])), c["lnq_lo"], c["lnq_hi"], c["interp"],
-           up(c["coef"]), None, up(c["ext"]), out, dmin)
+           up(c["coef"]), None, up(c["ext"]), out, dmin, ext_outer=c.get("ext_outer", 0))
         res = dict(out=out, dmin=dmin)
     else:
         shape = (c["pext"].size, c["n_jext"], c["m2psi"].size)

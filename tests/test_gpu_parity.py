@@ -144,6 +144,26 @@ def test_threepoint_small(n_p, n_alpha, n_q, n1, n2, interp):
     run_both(c, what="threepoint_%d_%d_%d_%d_%d_i%d" % (n_p, n_alpha, n_q, n1, n2, interp))
 
 
+@pytest.mark.parametrize("n_p,n_alpha,n_q,n1,n2,interp", [(3, 2, 20, 10, 6, 3), (5, 3, 33, 9, 5, 1), (7, 1, 40, 12, 16, 3),
+                                                          (2, 2, 6, 3, 200, 3)])
+def test_threepoint_product_grid_path(n_p, n_alpha, n_q, n1, n2, interp):
+    # the product-grid kernels (ext_outer = n_p promised), the general kernel on the same inputs (no promise), and a
+    # false promise (shuffled ext): all three against the oracle; the first two must come from different kernels
+    c = inputs.config3(n_p=n_p, n_alpha=n_alpha, n_q=n_q, n_c1=n1, n_c2=n2, n_phi=5, interp=interp)
+    what = "threepoint_grid_%d_%d_%d_%d_%d_i%d" % (n_p, n_alpha, n_q, n1, n2, interp)
+    assert c["ext_outer"] == n_p
+    g, o, _ = run_both(c, what=what)
+    c0 = dict(c, ext_outer=0)
+    g0, _, _ = run_both(c0, what=what + "_general")
+    assert not np.array_equal(g["out"], g0["out"])
+    perm = np.random.default_rng(5).permutation(c["ext"].shape[0])
+    cs = dict(c, ext=np.ascontiguousarray(c["ext"][perm]))
+    gs, _, _ = run_both(cs, what=what + "_false_promise")
+    assert np.array_equal(gs["out"], g0["out"][perm]) and np.array_equal(gs["dmin"], g0["dmin"][perm])
+    gn = gpu_run(c, make_rules(c, nodes), want_dmin=False)
+    assert np.array_equal(gn["out"], g["out"])
+
+
 def test_threepoint_full_config3_sampled():
     c = inputs.config3()
     sel = np.arange(0, 8192, 131)                        # 63 outputs spread over (|p1|, |p2|, alpha)
