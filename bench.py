@@ -126,7 +126,9 @@ def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
     """Device-resident timings of configs 0-3 (context for the flagship loop4d kernels; not the bench line)."""
     out = {}
 
-    def timeit(fn, n=iters):
+    def timeit(fn, n=iters, reps=1):
+        """median over n timings of `reps` back-to-back calls (reps > 1 keeps the host launch latency of a
+        tens-of-microseconds kernel out of the device time); ms per call"""
         for _ in range(2):
             fn()
         torch.cuda.synchronize()
@@ -134,10 +136,11 @@ def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
         for _ in range(n):
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record()
-            fn()
+            for _ in range(reps):
+                fn()
             b.record()
             b.synchronize()
-            ts.append(a.elapsed_time(b))
+            ts.append(a.elapsed_time(b) / reps)
         return float(np.median(ts))
 
     up = lambda a: torch.as_tensor(np.ascontiguousarray(a)).cuda()
@@ -158,7 +161,7 @@ def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
             for c, rq, rho, u, du, flow in calls:
                 B.dfrg_integrate_lpa(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["N"], c["prefactor"], c["reg_kind"],
                                      c["reg_order"], c["k"], rq, rho, u, du, flow)
-        ms = timeit(fn)
+        ms = timeit(fn, reps=20)
         out[name] = {"ms": ms, "evals_per_s": evals / ms * 1e3, "integrals_per_s": integrals / ms * 1e3,
                      "launches": len(calls)}
     # cfg2
@@ -169,7 +172,7 @@ def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
     o2 = torch.empty(pext.numel(), m2.numel(), dtype=torch.float64, device="cuda")
     ms = timeit(lambda: B.dfrg_integrate_loop4d(B.LOOP_TWOPOINT, c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
                                                 rq, rc, None, None, (Z,), c["lnq_lo"], c["lnq_hi"], c["interp"], coef,
-                                                m2, pext, o2))
+                                                m2, pext, o2), reps=20)
     ev = o2.numel() * rq[0].numel() * rc[0].numel()
     fl = o2.numel() * rq[0].numel() * (9 * rc[0].numel() + 11)
     out["cfg2"] = {"ms": ms, "evals_per_s": ev / ms * 1e3, "integrals_per_s": o2.numel() / ms * 1e3,
@@ -183,11 +186,13 @@ def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
     o3 = torch.empty(ext.shape[0], dtype=torch.float64, device="cuda")
     ms = timeit(lambda: B.dfrg_integrate_loop4d(B.LOOP_THREEPOINT, c["prefactor"], c["reg_kind"], c["reg_order"],
                                                 c["k"], rr["q"], rr["c1"], rr["c2"], rr["phi"], tabs, c["lnq_lo"],
-                                                c["lnq_hi"], c["interp"], coef, None, ext, o3), n=3)
+                                                c["lnq_hi"], c["interp"], coef, None, ext, o3,
+                                                ext_outer=c["ext_outer"]), n=3)
     uniq = o3.numel() * rr["q"][0].numel() * rr["c1"][0].numel() * rr["c2"][0].numel()
     out["cfg3"] = {"ms": ms, "unique_evals_per_s": uniq / ms * 1e3,
                    "nominal_evals_per_s": uniq * rr["phi"][0].numel() / ms * 1e3,
-                   "integrals_per_s": o3.numel() / ms * 1e3, "launches": 1}
+                   "integrals_per_s": o3.numel() / ms * 1e3,
+                   "launches": 4}   # product-grid path: pre-pass, main, fix-up, and the general kernel returning at once
     return out
 
 
@@ -358,7 +363,7 @@ def main():
         t0 = time.perf_counter()
         oracle_run(c, Ro, sel=probe_sel)
         rate = probe_sel.size / (time.perf_counter() - t0)                 # outputs per second
-        n_s = int(min(8192, max(256, rate * 15.0)))
+        n_s = int(min(n_out // 4, max(256, rate * 15.0)))               # about 15 s of host time
         sel = np.arange(n_s, dtype=np.int64) * (n_out // n_s)
         t0 = time.perf_counter()
         o = oracle_run(c, Ro, sel=sel)

@@ -202,9 +202,9 @@ __device__ __forceinline__ double table_lookup(const double4* __restrict__ cells
 // t(s) = (ln(s)/2 - lo)/h = A ln s + B straight from the bits of s, without a separate logarithm:
 //   s = 2^e m,  j = top 9 mantissa bits,  r = m inv_j - 1 (|r| <= 2^-10),  ln(1+r) = r - r^2/2 + r^3/3 - r^4/4
 //   (truncation r^5/5 < 1.8e-16 absolute in ln s: far below the rounding of t itself, ulp(127) = 1.4e-14)
-//   t = fma(ln(1+r), A, mant[j].y) + fma(E, A ln2, B - 1023 A ln2),   mant[j] = (inv_j, A ln c_j)
+//   t = e A ln2 + (A ln(1+r) + mant[j].y),   mant[j] = (A inv_j, A ln c_j + B),  everything in r' = A r
 // E = the exponent field of s >= 0 (callers clamp s at 0): zero and subnormal s land far below the grid (the table's
-// first value, as log(0) = -inf would give), inf/NaN far above.  7 FP64 instructions, one conversion, one LDS.128.
+// first value, as log(0) = -inf would give), inf/NaN far above.  6 FP64 instructions, one conversion, one LDS.128.
 // The cells carry guards: index F + 1 with F = clamp(floor(t), -1, n-1); F = -1 and F = n-1 are constant cells
 // (clamp-to-edge), the others hold the interpolant of SURVEY 8(c) (4-point Lagrange on the stencil
 // i0 = clamp(F-1, 0, n-4), or the linear one) re-expanded in tau = t - F.  Integer clamps replace the FP64 ones.
@@ -214,39 +214,42 @@ __device__ __forceinline__ double table_lookup(const double4* __restrict__ cells
 constexpr int LG_NM = 512, LG_REP = 8;
 constexpr int LG_DOUBLES = 2 * LG_NM * LG_REP;  // 64 KB
 struct LogGrid {
-  const double2* mant;  // this thread's copy: entry j at mant[j * LG_REP]
-  double A, ex1, ex0;   // A = 1/(2h); exponent term = fma((double)E, ex1, ex0)
-  int nm1;              // n - 1
+  const double2* mant;   // this thread's copy: entry j at mant[j * LG_REP] = (A inv_j, A ln c_j + B)
+  double negA, ex1;      // -A, A ln2         (A = 1/(2h))
+  double c1, c2, c3;     // -1/(2A), 1/(3A^2), -1/(4A^3): ln(1+r) = r (1 + r'(c1 + r'(c2 + r' c3))) / ... in r' = A r
+  int nm1;               // n - 1
 };
 // All threads of the CTA; the caller synchronises before first use.  mem: LG_DOUBLES doubles, 16-byte aligned.
 __device__ __forceinline__ LogGrid lg_build(double* mem, const double lo, const double inv_h, const int n) {
   double2* mt = reinterpret_cast<double2*>(mem);
   const double A = 0.5 * inv_h, B = -lo * inv_h;
+  const double ex1 = A * 0.6931471805599453;
+  const double lnA = log(A);
   for (int j = threadIdx.x; j < LG_NM; j += blockDim.x) {
     const double c = 1.0 + ((double)j + 0.5) * (1.0 / (double)LG_NM);
-    const double inv = 1.0 / c;
-    const double2 ent = make_double2(inv, -A * log(inv));
+    const double ainv = A / c;                       // the rounded value defines the centre: c_j := A / ainv
+    const double2 ent = make_double2(ainv, fma(A, lnA - log(ainv), B));
 #pragma unroll
     for (int r = 0; r < LG_REP; ++r) mt[j * LG_REP + r] = ent;
   }
   LogGrid L;
   L.mant = mt + (threadIdx.x & (LG_REP - 1));
-  L.A = A;
-  L.ex1 = A * 0.6931471805599453;
-  L.ex0 = fma(-1023.0, L.ex1, B);
+  L.negA = -A;
+  L.ex1 = ex1;
+  L.c1 = -0.5 / A;
+  L.c2 = 1.0 / (3.0 * A * A);
+  L.c3 = -0.25 / (A * A * A);
   L.nm1 = n - 1;
   return L;
 }
-__device__ __forceinline__ double lg_coord(const LogGrid& L, const double* __restrict__ kc, const double s) {
+// t(s): six FP64 instructions (r' = A r;  A ln(1+r) = r' (1 + r' (c1 + r' (c2 + r' c3)));  exponent term by FMA).
+__device__ __forceinline__ double lg_coord(const LogGrid& L, const double* __restrict__, const double s) {
   const unsigned hi = (unsigned)__double2hiint(s);
   const double m = __hiloint2double((int)((hi & 0x000fffffu) | 0x3ff00000u), __double2loint(s));
   const double2 T = L.mant[((hi >> 11) & (LG_NM - 1)) * LG_REP];
-  const double ex = fma((double)(int)(hi >> 20), L.ex1, L.ex0);
-  const double r = fma(m, T.x, -1.0);
-  double q = fma(r, kc[2], kc[3]);          // 1/3 - r/4
-  q = fma(r, q, kc[4]);                     // -1/2 + r/3 - r^2/4
-  const double lm = fma(r * r, q, r);       // ln(1 + r)
-  return fma(lm, L.A, T.y) + ex;
+  const double rp = fma(m, T.x, L.negA);
+  const double P = fma(rp, fma(rp, fma(rp, L.c3, L.c2), L.c1), 1.0);
+  return fma((double)((int)(hi >> 20) - 1023), L.ex1, fma(rp, P, T.y));
 }
 // Guarded cells of one table row, replicated: n + 1 cells x 2 halves x LG_REP double2.  cells_guarded_size(n) double2.
 // v may live in shared or global memory.  All threads; caller synchronises.  Returns this thread's copy.

@@ -10,14 +10,14 @@
 //       then acc += Wq_i G(q_i)^2 A.  Every lane of a warp reads the same table entry (broadcast).
 //   S5: the q-slices are combined through shared memory in fixed order.
 //
-// Three-point family.  No field axis: S3 is the evaluation.  Persistent CTAs (2 per SM) walk the external
-//   configurations (|p1|, |p2|, alpha); tables (per-cell cubics of Z_A and lambda3, log/exp tables, the radial
-//   factor wq q^3 Rdot G_A(q^2)) are built once per CTA.  thread = (q, c1) pairs, strided; per pair the
-//   c2-independent part (s_a, G_A(s_a), first vertex factor, the five coefficients of P as a quartic in q.p2)
-//   is hoisted out of the c2 loop.  The integrand has no phi dependence: the phi axis contributes sum_phi w.
-//   Fixed-order block sum per external configuration.
-#include <stdlib.h>
-
+// Three-point family.  No field axis: S3 is the evaluation.  Two paths (see the comments at the kernels):
+//   general  -- any list of external configurations (|p1|, |p2|, alpha): persistent CTAs walk the list; thread =
+//               (q, c1) pairs, c2 loop inside; the c2-independent part (s_a, G_A(s_a), first vertex factor, the five
+//               coefficients of P as a quartic in q.p2) is hoisted out of the c2 loop.
+//   product grid -- ext[a S + r] = (|p1|_a, |p2|_r, alpha_r) (dfrg_loop4d_desc::ext_outer): what depends on |p1| alone
+//               comes from a pre-pass table, what depends on (|p2|, alpha) alone is built once per work unit in shared
+//               memory; one look-up and one Horner evaluation remain per (a, r, node).
+//   The integrand has no phi dependence: the phi axis contributes sum_phi w.  Fixed-order sums.
 #include "dfrg_device.cuh"
 #include "dfrg_internal.h"
 
@@ -145,7 +145,6 @@ static size_t twopoint_smem(int nq, int nc, int ntab) {
 // =====================================================================================================
 // three-point
 // =====================================================================================================
-constexpr int T3_THREADS = 256;
 
 struct ThreePointParams {
   int nq, n1, n2, nphi, n_ext;
@@ -158,138 +157,10 @@ struct ThreePointParams {
   const int* skip_flag;  // nullable; the general kernel returns at once if *skip_flag == 0 (product-grid path did the work)
 };
 
-template <bool WANT_DMIN>
-__global__ void __launch_bounds__(T3_THREADS, 2) threepoint_kernel(const ThreePointParams P) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  __shared__ __align__(8) uint64_t bar;
-  __shared__ double red[32];
-
-  const int nq = P.nq, n1 = P.n1, n2 = P.n2, nt = P.grid.n;
-  double* sxq = reinterpret_cast<double*>(smem_raw);
-  double* swq = sxq + ((nq + 1) & ~1);
-  double* sx1 = swq + ((nq + 1) & ~1);
-  double* sw1 = sx1 + ((n1 + 1) & ~1);
-  double* sx2 = sw1 + ((n1 + 1) & ~1);
-  double* sw2 = sx2 + ((n2 + 1) & ~1);
-  double* sZA = sw2 + ((n2 + 1) & ~1);
-  double* sL3 = sZA + ((nt + 1) & ~1);
-  double* skap = sL3 + ((nt + 1) & ~1);  // 36
-  double* fmmem = skap + 36;             // [FM_DOUBLES]
-  double4* cZA = reinterpret_cast<double4*>(fmmem + FM_DOUBLES);
-  double4* cL3 = cZA + nt;
-  double2* qtab = reinterpret_cast<double2*>(cL3 + nt);  // [nq] (wq q^3 Rdot(q^2) G_A(q^2), D(q^2))
-
-  if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
-  __syncthreads();
-  {
-    StageList L;
-    L.add(sxq, P.xq, nq); L.add(swq, P.wq, nq);
-    L.add(sx1, P.x1, n1); L.add(sw1, P.w1, n1);
-    L.add(sx2, P.x2, n2); L.add(sw2, P.w2, n2);
-    L.add(sZA, P.ZA, nt); L.add(sL3, P.L3, nt);
-    stage_to_smem(L, &bar, 0);
-  }
-  const FastMath fm = fm_build(fmmem, P.fmc);
-  cells_build(cZA, sZA, P.grid);
-  cells_build(cL3, sL3, P.grid);
-  if (threadIdx.x < 35) skap[threadIdx.x] = P.coef[threadIdx.x];
-  __syncthreads();
-
-  const double ik2 = P.reg.inv_k2;
-  const double inf = __longlong_as_double(0x7ff0000000000000LL);
-  // ---- S3, once per CTA: the part that depends on the radial node only (not on the external point) ----
-  double dmq = inf;
-  for (int i = threadIdx.x; i < nq; i += T3_THREADS) {
-    const double q = sxq[i], sq = q * q;
-    double Rq, Rdq;
-    regulator(P.reg, fm, sq, Rq, Rdq);
-    const double Dq = table_lookup(cZA, P.grid, fm, sq) * sq + Rq;
-    qtab[i] = make_double2((swq[i] * q * q * q * Rdq) * fast_rcp(Dq), Dq);
-    dmq = fmin(dmq, Dq);
-  }
-  dmq = block_min(dmq, red);  // also publishes qtab
-  double sum_wphi = 0.0;      // the integrand has no phi dependence: the axis contributes sum_phi w
-  for (int jp = 0; jp < P.nphi; ++jp) sum_wphi += P.wphi[jp];
-
-  const int npairs = nq * n1;
-  // persistent: this CTA owns the external points e = blockIdx.x, blockIdx.x + gridDim.x, ...
-  for (int e = blockIdx.x; e < P.n_ext; e += gridDim.x) {
-    const double p1 = P.ext[3 * e], p2 = P.ext[3 * e + 1], al = P.ext[3 * e + 2];
-    double sa_, ca_;
-    sincos(al, &sa_, &ca_);
-    double scc = p1 * p1 + p2 * p2 + 2.0 * p1 * p2 * ca_;
-    scc = scc > 0.0 ? scc : 0.0;
-    double dm = dmq;
-    double acc = 0.0;
-    for (int t = threadIdx.x; t < npairs; t += T3_THREADS) {
-      const int i = t / n1, j1 = t - i * n1;
-      const double q = sxq[i], c1 = sx1[j1];
-      const double sq = q * q;
-      const double sin1 = sqrt((1.0 - c1) * (1.0 + c1));
-      const double wpair = qtab[i].x * (sw1[j1] * sin1);
-      // (q, c1) pieces
-      const double qp1 = q * p1 * c1;
-      double s_a = sq + p1 * p1 + 2.0 * qp1;
-      s_a = clamp_lo(s_a, 0.0);
-      double Ra, Rda;
-      regulator(P.reg, fm, s_a, Ra, Rda);
-      const double Da = table_lookup(cZA, P.grid, fm, s_a) * s_a + Ra;
-      if (WANT_DMIN) dm = fmin(dm, Da);
-      const double Ga = fast_rcp(Da);
-      const double lam1 = table_lookup(cL3, P.grid, fm, (p1 * p1 + sq + s_a) * (1.0 / 3.0));
-      // P as a quartic in z = q.p2/k^2: gam[c] = sum_{a+b<=4-c} kap_abc X^a Y^b
-      const double X = sq * ik2, Y = qp1 * ik2;
-      double gam[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-      {
-        int idx = 0;
-        double Xa = 1.0;
-#pragma unroll
-        for (int a = 0; a <= 4; ++a) {
-          double XaYb = Xa;
-#pragma unroll
-          for (int b = 0; b <= 4 - a; ++b) {
-#pragma unroll
-            for (int c = 0; c <= 4 - a - b; ++c) gam[c] = fma(skap[idx++], XaYb, gam[c]);
-            XaYb *= Y;
-          }
-          Xa *= X;
-        }
-      }
-      const double zc = q * p2 * ca_ * c1;  // q.p2 = zc + zs * c2
-      const double zs = q * p2 * sa_ * sin1;
-      const double sb0 = sq + p2 * p2;      // s_b = sb0 - 2 q.p2
-      const double l20 = p2 * p2 + sq, l30 = scc + s_a;
-      double acc2 = 0.0;
-#pragma unroll 2
-      for (int j2 = 0; j2 < n2; ++j2) {
-        const double qp2 = fma(zs, sx2[j2], zc);
-        double s_b = fma(-2.0, qp2, sb0);
-        s_b = clamp_lo(s_b, 0.0);
-        double Rb, Rdb;
-        regulator(P.reg, fm, s_b, Rb, Rdb);
-        const double Db = table_lookup(cZA, P.grid, fm, s_b) * s_b + Rb;
-        if (WANT_DMIN) dm = fmin(dm, Db);
-        const double lam2 = table_lookup(cL3, P.grid, fm, (l20 + s_b) * (1.0 / 3.0));
-        const double lam3 = table_lookup(cL3, P.grid, fm, (l30 + s_b) * (1.0 / 3.0));
-        const double z = qp2 * ik2;
-        const double poly = fma(fma(fma(fma(gam[4], z, gam[3]), z, gam[2]), z, gam[1]), z, gam[0]);
-        acc2 = fma(sw2[j2], fast_rcp(Db) * (lam2 * lam3) * poly, acc2);
-      }
-      acc = fma(wpair, (Ga * lam1) * acc2, acc);
-    }
-    const double total = block_sum(acc, red);
-    const double dmin_b = WANT_DMIN ? block_min(dm, red) : 0.0;
-    if (threadIdx.x == 0) {
-      P.out[e] = P.prefactor * sum_wphi * total;
-      if (WANT_DMIN) P.dmin[e] = dmin_b * ik2;
-    }
-  }
-}
-
-// ---- three-point, second version: fused log-grid coordinate, guarded cells, regulator kind at compile time ----
-// Same mapping as above (persistent CTAs, thread = (q, c1) pairs, c2 loop inside).  What changed is the cost of a
-// node: the three table look-ups go through lg_coord / lg_cell_eval (no separate logarithm, no FP64 clamps, no
-// exponent conversion), e^-x through the 256-entry table, and every affine step is a single FMA.
+// ---- three-point, general kernel (any list of external configurations) ----
+// Persistent CTAs, thread = (q, c1) pairs, c2 loop inside.  The three table look-ups of a node go through lg_coord /
+// lg_cell_eval (no separate logarithm, no FP64 clamps), e^-x through the replicated 64-entry table, every affine
+// step is a single FMA, and the regulator kind is a template parameter.
 template <int REGK>  // 0 Litim, 1 EXP_POLY(1), 2 EXP_POLY(order)
 __device__ __forceinline__ double t3_reg_R(const RegParams& rp, const double* __restrict__ fxtab,
                                            const double* __restrict__ kc, const double s) {
@@ -488,6 +359,7 @@ struct ThreeGridParams {
 
 constexpr int T3G_THREADS = 256;
 constexpr int T3G_NODES = 512;  // shared nodes per unit buffer
+constexpr int T3G_MAXT = 512;   // threads of the main kernel (126 registers each)
 
 // common shared-memory carve-up of the two product-grid kernels
 struct T3GShared {
@@ -515,13 +387,13 @@ __device__ __forceinline__ T3GShared t3g_carve(unsigned char* raw, int nq, int n
   s.xw2 = s.qtab + nq;
   s.nodeA = s.xw2 + n2;                                          // [2][T3G_NODES]
   s.nodeZ = reinterpret_cast<double*>(s.nodeA + 2 * T3G_NODES);  // [2][T3G_NODES]
-  s.red = s.nodeZ + 2 * T3G_NODES;                               // [T3G_THREADS]
+  s.red = s.nodeZ + 2 * T3G_NODES;                               // [T3G_MAXT]
   return s;
 }
 static size_t t3g_smem(int nq, int n1, int n2, int nt) {
   return 8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((n1 + 1) & ~1) + 2 * ((n2 + 1) & ~1) + 2 * ((nt + 1) & ~1) + 36 +
                       FM_DOUBLES + FX_DOUBLES + LG_DOUBLES + 2 * cells_guarded_size(nt) * 2 + 2 * nq + 2 * n2 +
-                      2 * 2 * T3G_NODES + 2 * T3G_NODES + T3G_THREADS);
+                      2 * 2 * T3G_NODES + 2 * T3G_NODES + T3G_MAXT);
 }
 
 template <int REGK>
@@ -619,8 +491,8 @@ __global__ void __launch_bounds__(T3G_THREADS, 1) t3g_prepass_kernel(const Three
   }
 }
 
-template <int REGK>
-__global__ void __launch_bounds__(T3G_THREADS, 1) t3g_main_kernel(const ThreeGridParams Q) {
+template <int REGK, int NT, int UNR>
+__global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar;
   __shared__ double red32[32];
@@ -646,14 +518,14 @@ __global__ void __launch_bounds__(T3G_THREADS, 1) t3g_main_kernel(const ThreeGri
   const double* kc = P.fmc.c;
   const double2* cZA = cells_build_guarded(sm.cZA_all, sm.sZA, nt, P.grid.interp);
   const double2* cL3 = cells_build_guarded(sm.cL3_all, sm.sL3, nt, P.grid.interp);
-  for (int j = tid; j < n2; j += T3G_THREADS) sm.xw2[j] = make_double2(sm.sx2[j], sm.sw2[j]);
+  for (int j = tid; j < n2; j += NT) sm.xw2[j] = make_double2(sm.sx2[j], sm.sw2[j]);
   __syncthreads();
 
   const double ik2 = P.reg.inv_k2, third = 1.0 / 3.0, m2k2 = -2.0 * P.reg.k2;
   const double inf = __longlong_as_double(0x7ff0000000000000LL);
   const long long U = (long long)S * NCH;
   const long long u0 = (long long)blockIdx.x * U / gridDim.x, u1 = (long long)(blockIdx.x + 1) * U / gridDim.x;
-  const int nw = T3G_THREADS / G;                 // pair slots
+  const int nw = NT / G;                 // pair slots
   const bool active = tid < nw * G;
   const int a = tid % G, w = tid / G;
   const double p1 = P.ext[3 * ((long long)a * S)];
@@ -667,7 +539,7 @@ __global__ void __launch_bounds__(T3G_THREADS, 1) t3g_main_kernel(const ThreeGri
     const double p2 = Q.tabR[4 * r], ca_ = Q.tabR[4 * r + 1], sa_ = Q.tabR[4 * r + 2];
     double2* nA = sm.nodeA + b * T3G_NODES;
     double* nZ = sm.nodeZ + b * T3G_NODES;
-    for (int n = tid; n < npl * n2; n += T3G_THREADS) {
+    for (int n = tid; n < npl * n2; n += NT) {
       const int pl = n / n2, j2 = n - pl * n2;
       const int pair = pair0 + pl;
       const int i = pair / n1, j1 = pair - i * n1;
@@ -723,7 +595,7 @@ __global__ void __launch_bounds__(T3G_THREADS, 1) t3g_main_kernel(const ThreeGri
         const double2* na = nA + pl * n2;
         const double* nz = nZ + pl * n2;
         double acc2 = 0.0;
-#pragma unroll 8
+#pragma unroll UNR
         for (int j2 = 0; j2 < n2; ++j2) {
           const double2 bs = na[j2];
           const double z = nz[j2];
@@ -779,11 +651,6 @@ __global__ void __launch_bounds__(256) t3g_fixup_kernel(const ThreeGridParams Q)
     for (int pair = 0; pair < npairs; ++pair) dm = fmin(dm, Q.tabA[((size_t)pair * 8 + 7) * G + a]);
     P.dmin[e] = dm * P.reg.inv_k2;
   }
-}
-
-static size_t threepoint_smem(int nq, int n1, int n2, int nt) {
-  return 8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((n1 + 1) & ~1) + 2 * ((n2 + 1) & ~1) + 2 * ((nt + 1) & ~1) + 36 +
-                      FM_DOUBLES + 8 * nt + 2 * nq);
 }
 
 // =====================================================================================================
@@ -848,9 +715,8 @@ static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m
   const int regk = D->reg.kind == DFRG_REG_LITIM ? 0 : (D->reg.order == 1 ? 1 : 2);
   void* scratch = nullptr;
   // ---- product-grid path (ext_outer = G promised by the caller, checked on the device) ----
-  const char* vgrid = getenv("DFRG_T3_GRID");
   const int G = D->ext_outer;
-  if (G >= 2 && G <= T3G_THREADS && n_ext % G == 0 && P.n2 <= T3G_NODES && !(vgrid && vgrid[0] == '0')) {
+  if (G >= 2 && G <= 256 && n_ext % G == 0 && P.n2 <= T3G_NODES) {
     ThreeGridParams Q;
     Q.B = P;
     Q.G = G; Q.S = n_ext / G;
@@ -878,26 +744,17 @@ static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m
     cudaError_t e = cudaMemsetAsync(Q.flag, 0, sizeof(int), stream);
     const size_t smem_g = t3g_smem(P.nq, P.n1, P.n2, P.grid.n);
     void (*kpre)(const ThreeGridParams) = regk == 0 ? t3g_prepass_kernel<0> : (regk == 1 ? t3g_prepass_kernel<1> : t3g_prepass_kernel<2>);
-    void (*kmain)(const ThreeGridParams) = regk == 0 ? t3g_main_kernel<0> : (regk == 1 ? t3g_main_kernel<1> : t3g_main_kernel<2>);
+    void (*kmain)(const ThreeGridParams) = regk == 0 ? t3g_main_kernel<0, T3G_MAXT, 8> : (regk == 1 ? t3g_main_kernel<1, T3G_MAXT, 8> : t3g_main_kernel<2, T3G_MAXT, 8>);
+    const int nt_main = T3G_MAXT;
     if (e == cudaSuccess) e = cudaFuncSetAttribute(kpre, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(kmain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g);
     if (e != cudaSuccess) { scratch_free(scratch, stream); return check_cuda(e); }
     kpre<<<sm_count, T3G_THREADS, smem_g, stream>>>(Q);
-    kmain<<<Q.grid_main, T3G_THREADS, smem_g, stream>>>(Q);
+    kmain<<<Q.grid_main, nt_main, smem_g, stream>>>(Q);
     t3g_fixup_kernel<<<(n_ext + 255) / 256, 256, 0, stream>>>(Q);
     rc = check_cuda(cudaGetLastError());
     if (rc != DFRG_OK) { scratch_free(scratch, stream); return rc; }
     P.skip_flag = Q.flag;  // the general kernel below runs only if the promise turned out false
-  }
-  int grid = n_ext < 2 * sm_count ? n_ext : 2 * sm_count;  // persistent: 2 CTAs per SM
-  const char* vpath = getenv("DFRG_T3_PATH");
-  if (vpath && vpath[0] == 'o') {
-    const size_t smem = threepoint_smem(P.nq, P.n1, P.n2, P.grid.n);
-    auto kern = dmin ? threepoint_kernel<true> : threepoint_kernel<false>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return check_cuda(e);
-    kern<<<grid, T3_THREADS, smem, stream>>>(P);
-    return check_cuda(cudaGetLastError());
   }
   const size_t smem = threepoint_v2_smem(P.nq, P.n1, P.n2, P.grid.n);
   void (*kern)(const ThreePointParams) = nullptr;
@@ -907,7 +764,7 @@ static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m
   const int nthreads = 256;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) { scratch_free(scratch, stream); return check_cuda(e); }
-  grid = n_ext < sm_count ? n_ext : sm_count;  // persistent: 1 CTA of 256 threads x 240 registers per SM (replicated tables: 140 KB)
+  const int grid = n_ext < sm_count ? n_ext : sm_count;  // persistent: 1 CTA of 256 threads x 240 registers per SM (replicated tables: 140 KB)
   kern<<<grid, nthreads, smem, stream>>>(P);
   const int rc_last = check_cuda(cudaGetLastError());
   scratch_free(scratch, stream);
