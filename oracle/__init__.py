@@ -14,6 +14,9 @@ from .binding import (  # noqa: F401
     loop4d_twopoint,
     loop4d_threepoint,
     matsubara3d,
+    lpa_dm2,
+    loop4d_twopoint_dm2,
+    matsubara3d_dm2,
     num_threads,
     set_num_threads,
     REG_LITIM,

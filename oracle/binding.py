@@ -64,6 +64,19 @@ def _load():
                                          _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
                                          _dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int,
                                          C.c_longlong, _lp, _dp, _dp, _dp]
+        _lib.orc_lpa_dm2.argtypes = [C.c_int, C.c_double, C.c_int, C.c_int, C.c_double,
+                                     C.c_int, C.c_int, C.c_double,
+                                     C.c_int, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp]
+        _lib.orc_loop4d_twopoint_dm2.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double,
+                                                 C.c_int, _dp, _dp, C.c_int, _dp, _dp,
+                                                 _dp, C.c_int, C.c_double, C.c_double, C.c_int,
+                                                 _dp, C.c_int, C.c_int, _dp, C.c_int, _dp,
+                                                 C.c_longlong, _lp, _dp, _dp]
+        _lib.orc_matsubara3d_dm2.argtypes = [C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, C.c_double,
+                                             C.c_int, _dp, _dp, C.c_int, _dp, _dp,
+                                             _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
+                                             _dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int,
+                                             C.c_longlong, _lp, _dp, _dp, _dp, _dp]
     return _lib
 
 
@@ -181,3 +194,56 @@ def matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zps
     if rc:
         raise ValueError("orc_matsubara3d: bad arguments")
     return (out, dmin, sens) if want_sens else (out, dmin)
+
+
+# ---- mass derivatives (Jacobian support) ------------------------------------------------------------
+def lpa_dm2(d, T, n_max, reg_arg4d, prefactor, reg_kind, reg_order, k, xq, wq, rho, u, du):
+    """Returns (dchan[2, n_field], sens[2, n_field]): dI/dm2 at the pion and sigma masses."""
+    xq, wq, rho, u, du = map(_arr, (xq, wq, rho, u, du))
+    nf = rho.size
+    dchan = np.empty((2, nf))
+    sens = np.empty((2, nf))
+    rc = _load().orc_lpa_dm2(int(d), float(T), int(n_max), int(reg_arg4d), float(prefactor),
+                             int(reg_kind), int(reg_order), float(k), int(xq.size), _d(xq), _d(wq),
+                             int(nf), _d(rho), _d(u), _d(du), _d(dchan), _d(sens))
+    if rc:
+        raise ValueError("orc_lpa_dm2: bad arguments")
+    return dchan, sens
+
+
+def loop4d_twopoint_dm2(prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Z, lnq_lo, lnq_hi, interp,
+                        coef, m2, pext, sel=None):
+    """Returns (dout, sens): d out[e][f] / d m2[f], shape [n_ext, n_field] or [n_sel]."""
+    xq, wq, xc, wc, Z, coef, m2, pext = map(_arr, (xq, wq, xc, wc, Z, coef, m2, pext))
+    ns, selp, _keep = _sel(sel)
+    shape = (ns,) if sel is not None else (pext.size, m2.size)
+    dout = np.empty(shape)
+    sens = np.empty(shape)
+    rc = _load().orc_loop4d_twopoint_dm2(float(prefactor), int(reg_kind), int(reg_order), float(k),
+                                         int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
+                                         _d(Z), int(Z.size), float(lnq_lo), float(lnq_hi), int(interp),
+                                         _d(coef), int(coef.size), int(m2.size), _d(m2), int(pext.size), _d(pext),
+                                         ns, selp, _d(dout), _d(sens))
+    if rc:
+        raise ValueError("orc_loop4d_twopoint_dm2: bad arguments")
+    return dout, sens
+
+
+def matsubara3d_dm2(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zpsi, Zphi,
+                    lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None):
+    """Returns (dpsi, dphi, sens_psi, sens_phi): d out / d m2_psi[f] and d out / d m2_phi[f]."""
+    xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext = map(
+        _arr, (xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext))
+    nfreq, tnq = Zpsi.shape
+    ns, selp, _keep = _sel(sel)
+    shape = (ns,) if sel is not None else (pext.size, int(n_jext), m2psi.size)
+    dpsi, dphi, spsi, sphi = (np.empty(shape) for _ in range(4))
+    rc = _load().orc_matsubara3d_dm2(float(T), int(n_max), float(prefactor), int(reg_kind), int(reg_order), float(k),
+                                     int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
+                                     _d(Zpsi), _d(Zphi), int(tnq), int(nfreq), float(lnq_lo), float(lnq_hi),
+                                     int(interp), _d(coef), int(coef.size), int(m2psi.size), _d(m2psi), _d(m2phi),
+                                     int(pext.size), _d(pext), int(n_jext), ns, selp, _d(dpsi), _d(dphi), _d(spsi),
+                                     _d(sphi))
+    if rc:
+        raise ValueError("orc_matsubara3d_dm2: bad arguments")
+    return dpsi, dphi, spsi, sphi

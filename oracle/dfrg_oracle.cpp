@@ -41,6 +41,9 @@
 // interpolator exactness on cubics; p=0 identity; coefficient linearity;
 // dimensional scaling; brute-force convergence; an independent mpmath
 // restatement on tiny inputs.
+// Mass derivatives (orc_*_dm2, at the end of the file): pinned by the derivatives of the Litim closed forms
+// (T = 0 and truncated Matsubara sum), the m2 -> inf weight integrals, and five-point finite differences of
+// the pinned value functions.
 // Parity unpinned: the *readings* of config 3 and config 4 (which integrand
 // the words of BASELINE.json mean) have no value outside this text to compare
 // with; their arithmetic is pinned by the independent mpmath restatement only.
@@ -499,6 +502,187 @@ int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg
     out[o] = (double)((acc_t)prefactor * (acc_t)T * acc_n);
     if (dmin) dmin[o] = dm;
     if (sens) sens[o] = (double)((acc_t)std::fabs(prefactor) * (acc_t)T * sn_n);
+  }
+  return 0;
+}
+
+// =====================================================================================================
+// Mass derivatives (Jacobian support).  Implicit time-steppers need dR_i/du_j (eq. 27;
+// kernel option "AD"): for the loop integrals that is the derivative of the quadrature
+// sum with respect to the mass term of its propagators.  Each function below is the term-by-term
+// derivative of the sum its value twin above computes, d/dm2 (1/D^p) = -p/D^(p+1), written out plainly.
+// sens_* = sum |term| (1 + sum over propagators of power (|D - m2| + |m2|)/|D|), as for the values.
+// =====================================================================================================
+
+// dchan[ch][f] = dI/dm2 at m2 = m2_channel:  -C [T] sum w q^(d-1) Rdot / D^2
+int orc_lpa_dm2(int d, double T, int n_max, int reg_arg4d, double prefactor,
+                int reg_kind, int reg_order, double k,
+                int nq, const double* xq, const double* wq,
+                int n_field, const double* rho, const double* u, const double* du,
+                double* dchan, double* sens) {
+  if (d < 1 || nq < 1 || n_field < 0 || T < 0 || n_max < 0 || k <= 0 || !dchan) return -1;
+  const double pi = 3.14159265358979323846;
+#pragma omp parallel for schedule(static)
+  for (int f = 0; f < n_field; ++f) {
+    const double m2c[2] = {u[f], u[f] + 2.0 * rho[f] * du[f]};
+    for (int ch = 0; ch < 2; ++ch) {
+      const double m2 = m2c[ch];
+      acc_t acc = 0.0L, sn = 0.0L;
+      const int n_lo = (T == 0.0) ? 0 : -n_max, n_hi = (T == 0.0) ? 0 : n_max;
+      for (int n = n_lo; n <= n_hi; ++n) {
+        const double wn = 2.0 * pi * (double)n * T;
+        for (int i = 0; i < nq; ++i) {
+          const double q = xq[i];
+          const double s = wn * wn + q * q;
+          const double sR = (T == 0.0 || reg_arg4d) ? s : q * q;
+          double R, Rd;
+          regulator(reg_kind, reg_order, k, sR, &R, &Rd);
+          const double D = s + R + m2;
+          const double term = -wq[i] * ipow(q, d - 1) * Rd / (D * D);
+          acc += (acc_t)term;
+          sn += (acc_t)(std::fabs(term) * (1.0 + 2.0 * (std::fabs(s + R) + std::fabs(m2)) / std::fabs(D)));
+        }
+      }
+      const acc_t sc = (acc_t)prefactor * (T == 0.0 ? (acc_t)1.0 : (acc_t)T);
+      dchan[(size_t)ch * n_field + f] = (double)(sc * acc);
+      if (sens) sens[(size_t)ch * n_field + f] = (double)(fabsl(sc) * sn);
+    }
+  }
+  return 0;
+}
+
+// dout[e][f] = d out / d m2_f with the same m2 in all three propagators:
+//   C sum_i wq q^3 Rdot [ -2 G(q)^3 sum_j W'_ij G(s_ij) - G(q)^2 sum_j W'_ij G(s_ij)^2 ]
+int orc_loop4d_twopoint_dm2(double prefactor, int reg_kind, int reg_order, double k,
+                            int nq, const double* xq, const double* wq,
+                            int nc, const double* xc, const double* wc,
+                            const double* Zv, int Z_nq, double Z_lo, double Z_hi, int Z_interp,
+                            const double* coef, int n_coef,
+                            int n_field, const double* m2, int n_ext, const double* pext,
+                            long long n_sel, const long long* sel,
+                            double* dout, double* sens) {
+  if (n_coef != 2 || nq < 1 || nc < 1 || n_field < 1 || n_ext < 1 || k <= 0 || !dout) return -1;
+  const double k2 = k * k;
+  const long long n_out = sel ? n_sel : (long long)n_ext * n_field;
+#pragma omp parallel for schedule(static)
+  for (long long o = 0; o < n_out; ++o) {
+    const long long flat = sel ? sel[o] : o;
+    const int e = (int)(flat / n_field), f = (int)(flat % n_field);
+    const double p = pext[e], mm = m2[f];
+    acc_t acc_q = 0.0L, sn = 0.0L;
+    for (int i = 0; i < nq; ++i) {
+      const double q = xq[i];
+      const double sq = q * q;
+      double Rq, Rdq;
+      regulator(reg_kind, reg_order, k, sq, &Rq, &Rdq);
+      const double Dq = table_lookup(Zv, Z_nq, Z_lo, Z_hi, Z_interp, sq) * sq + Rq + mm;
+      const double Gq = 1.0 / Dq;
+      const double condq = (std::fabs(Dq - mm) + std::fabs(mm)) / std::fabs(Dq);
+      acc_t acc_c = 0.0L, sn_c = 0.0L;
+      for (int j = 0; j < nc; ++j) {
+        const double c = xc[j];
+        const double s = clamp0(sq + p * p + 2.0 * q * p * c);
+        double R, Rd;
+        regulator(reg_kind, reg_order, k, s, &R, &Rd);
+        const double D = table_lookup(Zv, Z_nq, Z_lo, Z_hi, Z_interp, s) * s + R + mm;
+        const double G = 1.0 / D;
+        const double poly = coef[0] + coef[1] * (q * p * c / k2);
+        const double Wp = wc[j] * std::sqrt((1.0 - c) * (1.0 + c));
+        const double t1 = -2.0 * Gq * Gq * Gq * G, t2 = -Gq * Gq * G * G;
+        acc_c += (acc_t)(Wp * poly * (t1 + t2));
+        const double apoly = std::fabs(coef[0]) + std::fabs(coef[1] * (q * p * c / k2));
+        const double condc = (std::fabs(D - mm) + std::fabs(mm)) / std::fabs(D);
+        sn_c += (acc_t)(std::fabs(Wp * apoly) * (std::fabs(t1) * (1.0 + 3.0 * condq + condc) +
+                                                 std::fabs(t2) * (1.0 + 2.0 * condq + 2.0 * condc)));
+      }
+      acc_q += (acc_t)(wq[i] * q * q * q * Rdq) * acc_c;
+      sn += (acc_t)std::fabs(wq[i] * q * q * q * Rdq) * sn_c;
+    }
+    dout[o] = (double)((acc_t)prefactor * acc_q);
+    if (sens) sens[o] = (double)((acc_t)std::fabs(prefactor) * sn);
+  }
+  return 0;
+}
+
+// dpsi[p][j][f] = d out / d m2_psi_f = C T sum_n sum_q w q^2 Rdot (-2 G_psi^3) sum_c w P G_phi
+// dphi[p][j][f] = d out / d m2_phi_f = C T sum_n sum_q w q^2 Rdot G_psi^2 sum_c w P (-G_phi^2)
+int orc_matsubara3d_dm2(double T, int n_max, double prefactor, int reg_kind, int reg_order, double k,
+                        int nq, const double* xq, const double* wq,
+                        int nc, const double* xc, const double* wc,
+                        const double* Zpsi, const double* Zphi, int t_nq, int t_nfreq,
+                        double t_lo, double t_hi, int t_interp,
+                        const double* coef, int n_coef,
+                        int n_field, const double* m2psi, const double* m2phi,
+                        int n_p, const double* pext, int n_jext,
+                        long long n_sel, const long long* sel,
+                        double* dpsi, double* dphi, double* sens_psi, double* sens_phi) {
+  if (n_coef != 20 || nq < 1 || nc < 1 || n_field < 1 || n_p < 1 || n_jext < 1 || k <= 0 || T <= 0) return -1;
+  if (n_max + 1 > t_nfreq || n_jext - 1 + n_max + 1 > t_nfreq || !dpsi || !dphi) return -1;
+  const double pi = 3.14159265358979323846;
+  const double k2 = k * k;
+  const long long n_out = sel ? n_sel : (long long)n_p * n_jext * n_field;
+#pragma omp parallel for schedule(static)
+  for (long long o = 0; o < n_out; ++o) {
+    const long long flat = sel ? sel[o] : o;
+    const int f = (int)(flat % n_field);
+    const int j = (int)((flat / n_field) % n_jext);
+    const int e = (int)(flat / ((long long)n_field * n_jext));
+    const double p = pext[e];
+    const double nuj = (2.0 * j + 1.0) * pi * T;
+    acc_t a_psi = 0.0L, a_phi = 0.0L, s_psi = 0.0L, s_phi = 0.0L;
+    for (int n = -n_max; n <= n_max; ++n) {
+      const double nun = (2.0 * n + 1.0) * pi * T;
+      const int nbar = n >= 0 ? n : -n - 1;
+      const int m = j - n;
+      const int mabs = m >= 0 ? m : -m;
+      const double om = 2.0 * pi * (double)m * T;
+      for (int i = 0; i < nq; ++i) {
+        const double q = xq[i];
+        const double spsi = nun * nun + q * q;
+        double Rp, Rdp;
+        regulator(reg_kind, reg_order, k, spsi, &Rp, &Rdp);
+        const double Dpsi =
+            table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q) * spsi + Rp + m2psi[f];
+        const double Gpsi = 1.0 / Dpsi;
+        const double condpsi = (std::fabs(Dpsi - m2psi[f]) + std::fabs(m2psi[f])) / std::fabs(Dpsi);
+        acc_t c_psi = 0.0L, c_phi = 0.0L, sc_psi = 0.0L, sc_phi = 0.0L;
+        for (int jc = 0; jc < nc; ++jc) {
+          const double c = xc[jc];
+          const double r2 = clamp0(p * p + q * q - 2.0 * p * q * c);
+          const double sphi = om * om + r2;
+          double Rb, Rdb;
+          regulator(reg_kind, reg_order, k, sphi, &Rb, &Rdb);
+          const double Dphi =
+              table_lookup(Zphi + (size_t)mabs * t_nq, t_nq, t_lo, t_hi, t_interp, r2) * sphi + Rb + m2phi[f];
+          const double Gphi = 1.0 / Dphi;
+          const double condphi = (std::fabs(Dphi - m2phi[f]) + std::fabs(m2phi[f])) / std::fabs(Dphi);
+          const double y1 = nun * nuj / k2, y2 = p * q * c / k2, y3 = spsi / k2;
+          double P = 0.0, Pabs = 0.0;
+          int idx = 0;
+          for (int a = 0; a <= 3; ++a)
+            for (int b = 0; a + b <= 3; ++b)
+              for (int cc = 0; a + b + cc <= 3; ++cc) {
+                const double mono = coef[idx++] * ipow(y1, a) * ipow(y2, b) * ipow(y3, cc);
+                P += mono;
+                Pabs += std::fabs(mono);
+              }
+          c_psi += (acc_t)(wc[jc] * P * Gphi);
+          c_phi += (acc_t)(-wc[jc] * P * Gphi * Gphi);
+          sc_psi += (acc_t)(std::fabs(wc[jc] * Pabs * Gphi) * (1.0 + 3.0 * condpsi + condphi));
+          sc_phi += (acc_t)(std::fabs(wc[jc] * Pabs * Gphi * Gphi) * (1.0 + 2.0 * condpsi + 2.0 * condphi));
+        }
+        const double W = wq[i] * q * q * Rdp;
+        a_psi += (acc_t)(-2.0 * W * Gpsi * Gpsi * Gpsi) * c_psi;
+        a_phi += (acc_t)(W * Gpsi * Gpsi) * c_phi;
+        s_psi += (acc_t)std::fabs(2.0 * W * Gpsi * Gpsi * Gpsi) * sc_psi;
+        s_phi += (acc_t)std::fabs(W * Gpsi * Gpsi) * sc_phi;
+      }
+    }
+    const acc_t sc = (acc_t)prefactor * (acc_t)T;
+    dpsi[o] = (double)(sc * a_psi);
+    dphi[o] = (double)(sc * a_phi);
+    if (sens_psi) sens_psi[o] = (double)(fabsl(sc) * s_psi);
+    if (sens_phi) sens_phi[o] = (double)(fabsl(sc) * s_phi);
   }
   return 0;
 }
