@@ -33,6 +33,10 @@
  *    gives whatever IEEE arithmetic gives; `dmin` reports it (signed minimum over all quadrature
  *    nodes and all propagators of an output of denominator / k^2; reading A4 in DESIGN.md).
  *    An exactly zero denominator yields NaN (the reciprocal is a Newton iteration on a hardware seed).
+ *  - Mass derivatives (Jacobian support; the paper's "AD" kernels for implicit time-steppers, PAPER.md:713-723
+ *    eq. 27 and PAPER.md:1842): every descriptor of a family with a field axis carries nullable output pointers
+ *    for the derivative of each integral with respect to the mass term of its propagators,
+ *    d/dm2 (1/D^p) = -p/D^(p+1) term by term on the same nodes.  NULL = not computed, no cost.
  *  - Deterministic: fixed thread -> node mapping, fixed reduction trees, no atomics.
  *  - Re-entrant; concurrent calls on different streams are allowed.
  */
@@ -101,6 +105,8 @@ typedef struct {
  *           s = (2 pi n T)^2 + q_i^2,  sR = s if reg_arg4d else q_i^2      (Matsubara sum)
  * d = dimension of the radial integral (1..8): 4 in the vacuum config, 3 at finite T.
  * flow [n_field]; chan nullable [2][n_field] = I_pi, I_sigma; dmin nullable [n_field].
+ * dchan (in the descriptor, nullable) [2][n_field] = dI/dm2 at m2 = u and at m2 = u + 2 rho du, from which
+ *   dflow/du = (N-1) dchan[0] + dchan[1],  dflow/d(du) = 2 rho dchan[1].
  * Limits: (n_max + 1) * q.n <= 12288. */
 typedef struct {
   int d;
@@ -111,6 +117,7 @@ typedef struct {
   double prefactor;
   dfrg_regulator reg;
   dfrg_rule q;
+  double* dchan; /* nullable output [2][n_field] */
 } dfrg_lpa_desc;
 
 int dfrg_integrate_lpa(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u, const double* du,
@@ -146,6 +153,9 @@ typedef struct {
                     grids), which lets the library share everything that depends on |p1| alone or on
                     (|p2|, alpha) alone.  The promise is checked on the device; if it does not hold the general
                     path runs and the results are the same.  Ignored (general path) if G > 256 or cos2.n > 512. */
+  double* dout_dm2; /* two-point only, nullable output [n_ext][n_field]: d out[e][f] / d m2[f] (the same m2 sits in all
+                       three propagators):  prefactor sum_i wq q^3 Rdot [-2 G(q)^3 A_i - G(q)^2 B_i],
+                       A_i = sum_j W'_ij G(s_ij), B_i = sum_j W'_ij G(s_ij)^2.  Must be NULL for the three-point family. */
 } dfrg_loop4d_desc;
 
 int dfrg_integrate_loop4d(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext, const double* ext,
@@ -173,6 +183,8 @@ typedef struct {
   dfrg_table tab_psi, tab_phi;
   const double* coef;
   int n_coef;
+  double* dout_dm2_psi; /* nullable output [n_p][n_jext][n_field]: d out / d m2_psi[f]  (G_psi^2 -> -2 G_psi^3) */
+  double* dout_dm2_phi; /* nullable output [n_p][n_jext][n_field]: d out / d m2_phi[f]  (G_phi   -> -G_phi^2)   */
 } dfrg_mats3d_desc;
 
 int dfrg_integrate_matsubara3d(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi, const double* m2_phi,

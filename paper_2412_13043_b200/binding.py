@@ -43,19 +43,20 @@ class Table(C.Structure):
 
 class LpaDesc(C.Structure):
     _fields_ = [("d", C.c_int), ("T", C.c_double), ("n_max", C.c_int), ("reg_arg4d", C.c_int), ("N", C.c_double),
-                ("prefactor", C.c_double), ("reg", Regulator), ("q", Rule)]
+                ("prefactor", C.c_double), ("reg", Regulator), ("q", Rule), ("dchan", _vp)]
 
 
 class Loop4dDesc(C.Structure):
     _fields_ = [("family", C.c_int), ("prefactor", C.c_double), ("reg", Regulator),
                 ("q", Rule), ("cos1", Rule), ("cos2", Rule), ("phi", Rule),
-                ("tab", Table * 3), ("coef", _vp), ("n_coef", C.c_int), ("ext_outer", C.c_int)]
+                ("tab", Table * 3), ("coef", _vp), ("n_coef", C.c_int), ("ext_outer", C.c_int),
+                ("dout_dm2", _vp)]
 
 
 class Mats3dDesc(C.Structure):
     _fields_ = [("T", C.c_double), ("n_max", C.c_int), ("prefactor", C.c_double), ("reg", Regulator),
                 ("q", Rule), ("cos1", Rule), ("tab_psi", Table), ("tab_phi", Table),
-                ("coef", _vp), ("n_coef", C.c_int)]
+                ("coef", _vp), ("n_coef", C.c_int), ("dout_dm2_psi", _vp), ("dout_dm2_phi", _vp)]
 
 
 class DfrgError(RuntimeError):
@@ -149,14 +150,15 @@ def dfrg_quad_nodes(n, a, b, rule_kind=RULE_GAUSS_LEGENDRE):
 
 
 # ---- LPA ------------------------------------------------------------------------------------------
-def _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, device):
+def _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, device, dchan=None):
     return LpaDesc(int(d), float(T), int(n_max), int(reg_arg4d), float(N), float(prefactor),
-                   Regulator(int(reg_kind), int(reg_order), float(k)), _rule(rule_q, device))
+                   Regulator(int(reg_kind), int(reg_order), float(k)), _rule(rule_q, device), _ptr(dchan, device))
 
 
 def dfrg_integrate_lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, rho, u, du,
-                       flow, chan=None, dmin=None):
-    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, True)
+                       flow, chan=None, dmin=None, dchan=None):
+    """dchan (optional, [2, n_field]): dI/dm2 per channel (include/dfrg.h, "Mass derivatives")."""
+    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, True, dchan)
     _check(lib().dfrg_integrate_lpa(C.byref(D), int(rho.numel()), _ptr(rho, True), _ptr(u, True), _ptr(du, True),
                                     _ptr(flow, True), _ptr(chan, True), _ptr(dmin, True), _stream()),
            "dfrg_integrate_lpa")
@@ -164,8 +166,8 @@ def dfrg_integrate_lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order
 
 
 def dfrg_integrate_lpa_host(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, rho, u, du,
-                            flow, chan=None, dmin=None):
-    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, False)
+                            flow, chan=None, dmin=None, dchan=None):
+    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, False, dchan)
     n_field = rho.numel() if hasattr(rho, "numel") else rho.size
     _check(lib().dfrg_integrate_lpa_host(C.byref(D), int(n_field), _ptr(rho, False), _ptr(u, False),
                                          _ptr(du, False), _ptr(flow, False), _ptr(chan, False), _ptr(dmin, False)),
@@ -175,13 +177,13 @@ def dfrg_integrate_lpa_host(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_
 
 # ---- loop4d ---------------------------------------------------------------------------------------
 def _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
-                 lnq_hi, interp, coef, device, ext_outer=0):
+                 lnq_hi, interp, coef, device, ext_outer=0, dout_dm2=None):
     T3 = Table * 3
     tt = [_table(t, lnq_lo, lnq_hi, interp, device) for t in tabs] + [_table(None, 0, 0, 0, device)] * (3 - len(tabs))
     n_coef = coef.numel() if hasattr(coef, "numel") else coef.size
     return Loop4dDesc(int(family), float(prefactor), Regulator(int(reg_kind), int(reg_order), float(k)),
                       _rule(rule_q, device), _rule(rule_c1, device), _rule(rule_c2, device), _rule(rule_phi, device),
-                      T3(*tt), _ptr(coef, device), int(n_coef), int(ext_outer))
+                      T3(*tt), _ptr(coef, device), int(n_coef), int(ext_outer), _ptr(dout_dm2, device))
 
 
 def _n(a):
@@ -189,11 +191,11 @@ def _n(a):
 
 
 def dfrg_integrate_loop4d(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs,
-                          lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0):
+                          lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0, dout_dm2=None):
     """two-point: tabs=(Z,), m2=[n_field], ext=[n_ext] -> out [n_ext, n_field];
     three-point: tabs=(Z_A, Z_c, lambda3), m2=None, ext=[n_ext, 3] -> out [n_ext]; ext_outer: dfrg_loop4d_desc."""
     D = _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
-                     lnq_hi, interp, coef, True, ext_outer)
+                     lnq_hi, interp, coef, True, ext_outer, dout_dm2)
     n_ext = _n(ext) if family == LOOP_TWOPOINT else _n(ext) // 3
     _check(lib().dfrg_integrate_loop4d(C.byref(D), _n(m2), _ptr(m2, True), n_ext, _ptr(ext, True),
                                        _ptr(out, True), _ptr(dmin, True), _stream()), "dfrg_integrate_loop4d")
@@ -201,9 +203,9 @@ def dfrg_integrate_loop4d(family, prefactor, reg_kind, reg_order, k, rule_q, rul
 
 
 def dfrg_integrate_loop4d_host(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs,
-                               lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0):
+                               lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0, dout_dm2=None):
     D = _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
-                     lnq_hi, interp, coef, False, ext_outer)
+                     lnq_hi, interp, coef, False, ext_outer, dout_dm2)
     n_ext = _n(ext) if family == LOOP_TWOPOINT else _n(ext) // 3
     _check(lib().dfrg_integrate_loop4d_host(C.byref(D), _n(m2), _ptr(m2, False), n_ext, _ptr(ext, False),
                                             _ptr(out, False), _ptr(dmin, False)), "dfrg_integrate_loop4d_host")
@@ -212,18 +214,19 @@ def dfrg_integrate_loop4d_host(family, prefactor, reg_kind, reg_order, k, rule_q
 
 # ---- matsubara3d ----------------------------------------------------------------------------------
 def _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp, coef,
-               device):
+               device, dpsi=None, dphi=None):
     return Mats3dDesc(float(T), int(n_max), float(prefactor), Regulator(int(reg_kind), int(reg_order), float(k)),
                       _rule(rule_q, device), _rule(rule_c, device),
                       _table(Zpsi, lnq_lo, lnq_hi, interp, device), _table(Zphi, lnq_lo, lnq_hi, interp, device),
-                      _ptr(coef, device), _n(coef))
+                      _ptr(coef, device), _n(coef), _ptr(dpsi, device), _ptr(dphi, device))
 
 
 def dfrg_integrate_matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo,
-                               lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, out, dmin=None):
+                               lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, out, dmin=None,
+                               dout_dm2_psi=None, dout_dm2_phi=None):
     """out: [n_p, n_jext, n_field]."""
     D = _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp,
-                   coef, True)
+                   coef, True, dout_dm2_psi, dout_dm2_phi)
     _check(lib().dfrg_integrate_matsubara3d(C.byref(D), _n(m2psi), _ptr(m2psi, True), _ptr(m2phi, True), _n(pext),
                                             _ptr(pext, True), int(n_jext), _ptr(out, True), _ptr(dmin, True),
                                             _stream()), "dfrg_integrate_matsubara3d")
@@ -231,9 +234,10 @@ def dfrg_integrate_matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, rule
 
 
 def dfrg_integrate_matsubara3d_host(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo,
-                                    lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, out, dmin=None):
+                                    lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, out, dmin=None,
+                               dout_dm2_psi=None, dout_dm2_phi=None):
     D = _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp,
-                   coef, False)
+                   coef, False, dout_dm2_psi, dout_dm2_phi)
     _check(lib().dfrg_integrate_matsubara3d_host(C.byref(D), _n(m2psi), _ptr(m2psi, False), _ptr(m2phi, False),
                                                  _n(pext), _ptr(pext, False), int(n_jext), _ptr(out, False),
                                                  _ptr(dmin, False)), "dfrg_integrate_matsubara3d_host")

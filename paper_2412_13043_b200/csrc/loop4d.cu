@@ -38,9 +38,11 @@ struct TwoPointParams {
   GridParams grid;
   FastMathConsts fmc;
   const double *xq, *wq, *xc, *wc, *Z, *coef, *m2, *pext;
-  double *out, *dmin;
+  double *out, *dmin, *dout;
 };
 
+// WANT_D: also d out / d m2 = -sum_i Wq G(q)^2 (2 G(q) A_i + B_i),  B_i = sum_j W'_ij G(s_ij)^2
+template <bool WANT_D>
 __global__ void __launch_bounds__(TP_THREADS) twopoint_kernel(const TwoPointParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar;
@@ -54,8 +56,8 @@ __global__ void __launch_bounds__(TP_THREADS) twopoint_kernel(const TwoPointPara
   double* sxc = swq + ((nq + 1) & ~1);
   double* swc = sxc + ((nc + 1) & ~1);
   double* sZ = swc + ((nc + 1) & ~1);                                   // raw table (TMA target)
-  double* part = sZ + ((P.grid.n + 1) & ~1);                            // [TP_SLICES][TP_FTILE]
-  double* fmmem = part + TP_SLICES * TP_FTILE;                          // [FM_DOUBLES]
+  double* part = sZ + ((P.grid.n + 1) & ~1);                            // [2][TP_SLICES][TP_FTILE]
+  double* fmmem = part + 2 * TP_SLICES * TP_FTILE;                      // [FM_DOUBLES]
   double4* cZ = reinterpret_cast<double4*>(fmmem + FM_DOUBLES);         // per-cell cubics of Z
 
   if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
@@ -102,27 +104,41 @@ __global__ void __launch_bounds__(TP_THREADS) twopoint_kernel(const TwoPointPara
   const int f = blockIdx.y * TP_FTILE + lane_f;
   const bool live = f < P.n_field;
   const double m2 = live ? P.m2[f] : 1.0;
-  double acc = 0.0;
+  double acc = 0.0, dacc = 0.0;
   for (int i = slice; i < nq; i += TP_SLICES) {
     const double2* row = inner + i * nc;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    double b0 = 0.0, b1 = 0.0, b2 = 0.0, b3 = 0.0;
     int j = 0;
     for (; j + 3 < nc; j += 4) {
       const double2 p0 = row[j], p1 = row[j + 1], p2 = row[j + 2], p3 = row[j + 3];
-      a0 = fma(p0.y, fast_rcp(p0.x + m2), a0);
-      a1 = fma(p1.y, fast_rcp(p1.x + m2), a1);
-      a2 = fma(p2.y, fast_rcp(p2.x + m2), a2);
-      a3 = fma(p3.y, fast_rcp(p3.x + m2), a3);
+      const double r0 = fast_rcp(p0.x + m2), r1 = fast_rcp(p1.x + m2), r2 = fast_rcp(p2.x + m2), r3 = fast_rcp(p3.x + m2);
+      a0 = fma(p0.y, r0, a0);
+      a1 = fma(p1.y, r1, a1);
+      a2 = fma(p2.y, r2, a2);
+      a3 = fma(p3.y, r3, a3);
+      if constexpr (WANT_D) {
+        b0 = fma(p0.y * r0, r0, b0);
+        b1 = fma(p1.y * r1, r1, b1);
+        b2 = fma(p2.y * r2, r2, b2);
+        b3 = fma(p3.y * r3, r3, b3);
+      }
     }
     for (; j < nc; ++j) {
       const double2 p0 = row[j];
-      a0 = fma(p0.y, fast_rcp(p0.x + m2), a0);
+      const double r0 = fast_rcp(p0.x + m2);
+      a0 = fma(p0.y, r0, a0);
+      if constexpr (WANT_D) b0 = fma(p0.y * r0, r0, b0);
     }
     const double2 o = outer[i];
     const double g = fast_rcp(o.x + m2);
-    acc = fma(o.y * (g * g), (a0 + a1) + (a2 + a3), acc);
+    const double wg2 = o.y * (g * g);
+    const double A = (a0 + a1) + (a2 + a3);
+    acc = fma(wg2, A, acc);
+    if constexpr (WANT_D) dacc = fma(wg2, fma(2.0 * g, A, (b0 + b1) + (b2 + b3)), dacc);
   }
   part[slice * TP_FTILE + lane_f] = acc;
+  if constexpr (WANT_D) part[(TP_SLICES + slice) * TP_FTILE + lane_f] = dacc;
   __syncthreads();
 
   // ---- S5/S6 ----
@@ -133,12 +149,18 @@ __global__ void __launch_bounds__(TP_THREADS) twopoint_kernel(const TwoPointPara
     const size_t o = (size_t)blockIdx.x * P.n_field + f;
     P.out[o] = P.prefactor * r;
     if (P.dmin) P.dmin[o] = (dmin0 + m2) * P.reg.inv_k2;
+    if constexpr (WANT_D) {
+      double dr = part[TP_SLICES * TP_FTILE + lane_f];
+#pragma unroll
+      for (int sidx = 1; sidx < TP_SLICES; ++sidx) dr += part[(TP_SLICES + sidx) * TP_FTILE + lane_f];
+      P.dout[o] = -P.prefactor * dr;
+    }
   }
 }
 
 static size_t twopoint_smem(int nq, int nc, int ntab) {
   return (size_t)nq * nc * 16 + (size_t)nq * 16 +
-         8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((nc + 1) & ~1) + ((ntab + 1) & ~1) + TP_SLICES * TP_FTILE + FM_DOUBLES +
+         8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((nc + 1) & ~1) + ((ntab + 1) & ~1) + 2 * TP_SLICES * TP_FTILE + FM_DOUBLES +
                       4 * ntab);
 }
 
@@ -667,7 +689,7 @@ static int loop4d_validate(const dfrg_loop4d_desc* D, int n_field, const double*
     return DFRG_OK;
   }
   if (D->family == DFRG_LOOP_THREEPOINT) {
-    if (n_field != 0 || D->n_coef != 35 || !valid_rule(D->cos2) || !valid_rule(D->phi)) return DFRG_EINVAL;
+    if (n_field != 0 || D->n_coef != 35 || !valid_rule(D->cos2) || !valid_rule(D->phi) || D->dout_dm2) return DFRG_EINVAL;
     for (int t = 0; t < 3; ++t)
       if (!valid_table(D->tab[t], 1)) return DFRG_EINVAL;
     for (int t = 1; t < 3; ++t)
@@ -696,12 +718,13 @@ static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m
     fill_common(D->reg, D->tab[0], &P.reg, &P.grid);
     P.fmc = fm_consts();
     P.xq = D->q.x; P.wq = D->q.w; P.xc = D->cos1.x; P.wc = D->cos1.w; P.Z = D->tab[0].v;
-    P.coef = D->coef; P.m2 = m2; P.pext = ext; P.out = out; P.dmin = dmin;
+    P.coef = D->coef; P.m2 = m2; P.pext = ext; P.out = out; P.dmin = dmin; P.dout = D->dout_dm2;
     const size_t smem = twopoint_smem(P.nq, P.nc, P.grid.n);
-    cudaError_t e = cudaFuncSetAttribute(twopoint_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    auto kern2 = D->dout_dm2 ? twopoint_kernel<true> : twopoint_kernel<false>;
+    cudaError_t e = cudaFuncSetAttribute(kern2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return check_cuda(e);
     dim3 grid(n_ext, (n_field + TP_FTILE - 1) / TP_FTILE);
-    twopoint_kernel<<<grid, TP_THREADS, smem, stream>>>(P);
+    kern2<<<grid, TP_THREADS, smem, stream>>>(P);
     return check_cuda(cudaGetLastError());
   }
   ThreePointParams P;
@@ -796,7 +819,7 @@ extern "C" int dfrg_integrate_loop4d_host(const dfrg_loop4d_desc* D, int n_field
   const bool two = D->family == DFRG_LOOP_TWOPOINT;
   const size_t nf = two ? (size_t)n_field : 1, ne = (size_t)n_ext, next_d = two ? ne : 3 * ne;
   size_t need = 2 * ((size_t)D->q.n + D->cos1.n + D->cos2.n + D->phi.n) + 3 * (size_t)D->tab[0].n_q + 64 + nf + next_d +
-                2 * ne * nf;
+                3 * ne * nf;
   rc = A.begin(need * sizeof(double) + 32 * 256);
   if (rc != DFRG_OK) return rc;
   dfrg_loop4d_desc Dd = *D;
@@ -812,10 +835,12 @@ extern "C" int dfrg_integrate_loop4d_host(const dfrg_loop4d_desc* D, int n_field
   const double* d_ext = A.put(ext, next_d);
   double* d_out = A.reserve(ne * nf);
   double* d_dmin = dmin ? A.reserve(ne * nf) : nullptr;
+  Dd.dout_dm2 = D->dout_dm2 ? A.reserve(ne * nf) : nullptr;
   if (A.status() != DFRG_OK) return A.status();
   rc = loop4d_launch(&Dd, n_field, d_m2, n_ext, d_ext, d_out, d_dmin, sms, A.stream());
   if (rc != DFRG_OK) return rc;
   A.fetch(out, d_out, ne * nf);
   if (dmin) A.fetch(dmin, d_dmin, ne * nf);
+  if (D->dout_dm2) A.fetch(D->dout_dm2, Dd.dout_dm2, ne * nf);
   return A.finish();
 }

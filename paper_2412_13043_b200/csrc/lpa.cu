@@ -25,14 +25,17 @@ struct LpaParams {
   RegParams reg;
   FastMathConsts fmc;
   const double *xq, *wq, *rho, *u, *du;
-  double *flow, *chan, *dmin;
+  double *flow, *chan, *dmin, *dchan;
 };
 
+// WANT_D: also dI/dm2 = -sum W / D^2 per channel (two more FP64 instructions per evaluation)
+template <bool WANT_D>
 __global__ void __launch_bounds__(LPA_THREADS) lpa_kernel(const LpaParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar;
   __shared__ double red[32];
   __shared__ double part[2][LPA_SLICES][LPA_FTILE];
+  __shared__ double dpart[WANT_D ? 2 : 1][LPA_SLICES][LPA_FTILE];
 
   const int n_terms = (P.T > 0.0) ? P.n_max + 1 : 1;
   const int n_pairs = n_terms * P.nq;
@@ -78,17 +81,36 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_kernel(const LpaParams P) {
     m2 = ch ? m2sig : m2pi;
   }
   double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  double d0 = 0.0, d1 = 0.0, d2 = 0.0, d3 = 0.0;
   int t = slice;
-  for (; t + 3 * LPA_SLICES < n_pairs; t += 4 * LPA_SLICES) {
-    const double2 p0 = tab[t], p1 = tab[t + LPA_SLICES], p2 = tab[t + 2 * LPA_SLICES], p3 = tab[t + 3 * LPA_SLICES];
-    a0 = fma(p0.y, fast_rcp(p0.x + m2), a0);
-    a1 = fma(p1.y, fast_rcp(p1.x + m2), a1);
-    a2 = fma(p2.y, fast_rcp(p2.x + m2), a2);
-    a3 = fma(p3.y, fast_rcp(p3.x + m2), a3);
-  }
-  for (; t < n_pairs; t += LPA_SLICES) {
-    const double2 p0 = tab[t];
-    a0 = fma(p0.y, fast_rcp(p0.x + m2), a0);
+  if constexpr (!WANT_D) {
+    for (; t + 3 * LPA_SLICES < n_pairs; t += 4 * LPA_SLICES) {
+      const double2 p0 = tab[t], p1 = tab[t + LPA_SLICES], p2 = tab[t + 2 * LPA_SLICES], p3 = tab[t + 3 * LPA_SLICES];
+      a0 = fma(p0.y, fast_rcp(p0.x + m2), a0);
+      a1 = fma(p1.y, fast_rcp(p1.x + m2), a1);
+      a2 = fma(p2.y, fast_rcp(p2.x + m2), a2);
+      a3 = fma(p3.y, fast_rcp(p3.x + m2), a3);
+    }
+    for (; t < n_pairs; t += LPA_SLICES) {
+      const double2 p0 = tab[t];
+      a0 = fma(p0.y, fast_rcp(p0.x + m2), a0);
+    }
+  } else {
+    for (; t + 3 * LPA_SLICES < n_pairs; t += 4 * LPA_SLICES) {
+      const double2 p0 = tab[t], p1 = tab[t + LPA_SLICES], p2 = tab[t + 2 * LPA_SLICES], p3 = tab[t + 3 * LPA_SLICES];
+      const double r0 = fast_rcp(p0.x + m2), r1 = fast_rcp(p1.x + m2), r2 = fast_rcp(p2.x + m2), r3 = fast_rcp(p3.x + m2);
+      const double w0 = p0.y * r0, w1 = p1.y * r1, w2 = p2.y * r2, w3 = p3.y * r3;
+      a0 = fma(p0.y, r0, a0); a1 = fma(p1.y, r1, a1); a2 = fma(p2.y, r2, a2); a3 = fma(p3.y, r3, a3);  // as without WANT_D
+      d0 = fma(w0, r0, d0); d1 = fma(w1, r1, d1); d2 = fma(w2, r2, d2); d3 = fma(w3, r3, d3);
+    }
+    for (; t < n_pairs; t += LPA_SLICES) {
+      const double2 p0 = tab[t];
+      const double r0 = fast_rcp(p0.x + m2);
+      const double w0 = p0.y * r0;
+      a0 = fma(p0.y, r0, a0);
+      d0 = fma(w0, r0, d0);
+    }
+    dpart[ch][slice][lane] = (d0 + d1) + (d2 + d3);
   }
   part[ch][slice][lane] = (a0 + a1) + (a2 + a3);
   __syncthreads();
@@ -103,6 +125,12 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_kernel(const LpaParams P) {
     P.flow[f] = (P.N - 1.0) * I[0] + I[1];
     if (P.chan) { P.chan[f] = I[0]; P.chan[P.n_field + f] = I[1]; }
     if (P.dmin) P.dmin[f] = fmin(dmin0 + m2pi, dmin0 + m2sig) * P.reg.inv_k2;
+    if constexpr (WANT_D) {
+#pragma unroll
+      for (int c = 0; c < 2; ++c)
+        P.dchan[c * P.n_field + f] =
+            -scale * ((dpart[c][0][lane] + dpart[c][1][lane]) + (dpart[c][2][lane] + dpart[c][3][lane]));
+    }
   }
 }
 
@@ -115,13 +143,14 @@ static int lpa_launch(const dfrg_lpa_desc* D, int n_field, const double* rho, co
   P.reg.k2 = D->reg.k * D->reg.k; P.reg.inv_k2 = 1.0 / P.reg.k2;
   P.fmc = fm_consts();
   P.xq = D->q.x; P.wq = D->q.w; P.rho = rho; P.u = u; P.du = du;
-  P.flow = flow; P.chan = chan; P.dmin = dmin;
+  P.flow = flow; P.chan = chan; P.dmin = dmin; P.dchan = D->dchan;
   const int n_terms = (D->T > 0.0) ? D->n_max + 1 : 1;
   const size_t smem = (size_t)n_terms * D->q.n * 16 + (2 * (size_t)((D->q.n + 1) & ~1) + FM_DOUBLES) * 8;
-  cudaError_t e = cudaFuncSetAttribute(lpa_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  auto kern = D->dchan ? lpa_kernel<true> : lpa_kernel<false>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return check_cuda(e);
   const int grid = (n_field + LPA_FTILE - 1) / LPA_FTILE;
-  lpa_kernel<<<grid, LPA_THREADS, smem, stream>>>(P);
+  kern<<<grid, LPA_THREADS, smem, stream>>>(P);
   return check_cuda(cudaGetLastError());
 }
 
@@ -157,7 +186,7 @@ extern "C" int dfrg_integrate_lpa_host(const dfrg_lpa_desc* D, int n_field, cons
   if (rc != DFRG_OK) return rc;
   Arena& A = thread_arena();
   const size_t nf = (size_t)n_field, nq = (size_t)D->q.n;
-  rc = A.begin((2 * nq + 3 * nf + 4 * nf) * sizeof(double) + 16 * 256);
+  rc = A.begin((2 * nq + 3 * nf + 6 * nf) * sizeof(double) + 16 * 256);
   if (rc != DFRG_OK) return rc;
   dfrg_lpa_desc Dd = *D;
   Dd.q.x = A.put(D->q.x, nq);
@@ -168,11 +197,13 @@ extern "C" int dfrg_integrate_lpa_host(const dfrg_lpa_desc* D, int n_field, cons
   double* d_flow = A.reserve(nf);
   double* d_chan = chan ? A.reserve(2 * nf) : nullptr;
   double* d_dmin = dmin ? A.reserve(nf) : nullptr;
+  Dd.dchan = D->dchan ? A.reserve(2 * nf) : nullptr;
   if (A.status() != DFRG_OK) return A.status();
   rc = lpa_launch(&Dd, n_field, d_rho, d_u, d_du, d_flow, d_chan, d_dmin, A.stream());
   if (rc != DFRG_OK) return rc;
   A.fetch(flow, d_flow, nf);
   if (chan) A.fetch(chan, d_chan, 2 * nf);
   if (dmin) A.fetch(dmin, d_dmin, nf);
+  if (D->dchan) A.fetch(D->dchan, Dd.dchan, 2 * nf);
   return A.finish();
 }

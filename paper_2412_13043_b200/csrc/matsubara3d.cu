@@ -51,6 +51,7 @@ struct Mats3dParams {
   int max_slots;     // partial sums per (field tile, p) in part[]
   int grid_main;     // CTAs of the moment kernel (the fix-up kernel re-derives the unit ownership from it)
   double *part;      // [max_slots][n_p][n_jext][n_field]
+  int mode;          // 0: value;  1: d/dm2_psi (G_psi^2 -> -2 G_psi^3);  2: d/dm2_phi (G_phi -> -G_phi^2, kernels with SQ)
 };
 
 // ---- (1) boson rows --------------------------------------------------------------------------------
@@ -132,10 +133,16 @@ constexpr int M3_FT = 128;  // threads per consumer group; a group covers M3_FT 
 //   MF = 4:  R = Nw/((d0 d1)(d2 d3)),      a0 += (R p23) d1, ...                          (17 FP64 instr / 4 evals)
 // i.e. 4 + 1/MF FP64-pipe instructions and 1/MF MUFU.RCP64H per evaluation instead of 5 and 1.  The products stay
 // far inside the double range (|d| between ~1e-3 k^2 and ~1e5 k^2); each extra multiply costs half an ulp.
-template <int MF>
+template <int MF, bool SQ>
 __device__ __forceinline__ void accumulate_node(const double D0, const double Nw, const double (&m2)[MF],
                                                 double (&a)[MF]) {
-  if constexpr (MF == 1) {
+  if constexpr (SQ) {  // a_f -= Nw / (D0 + m2_f)^2   (mass derivative of the boson line)
+#pragma unroll
+    for (int m = 0; m < MF; ++m) {
+      const double r = fast_rcp(D0 + m2[m]);
+      a[m] = fma(-(Nw * r), r, a[m]);
+    }
+  } else if constexpr (MF == 1) {
     a[0] = fma(Nw, fast_rcp(D0 + m2[0]), a[0]);
   } else if constexpr (MF == 2) {
     const double d0 = D0 + m2[0], d1 = D0 + m2[1];
@@ -155,7 +162,7 @@ __device__ __forceinline__ void accumulate_node(const double D0, const double Nw
   }
 }
 
-template <int GROUPS, int MF>
+template <int GROUPS, int MF, bool SQ>
 __global__ void __launch_bounds__(GROUPS * M3_FT + 32, 1) mats3d_main_kernel(const Mats3dParams P) {
   constexpr int NCONS = GROUPS * M3_FT;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -283,7 +290,8 @@ __global__ void __launch_bounds__(GROUPS * M3_FT + 32, 1) mats3d_main_kernel(con
 #pragma unroll
         for (int m = 0; m < MF; ++m) {
           const double gpsi = fast_rcp(o.x + m2psi[m]);
-          h[m] = o.y * (gpsi * gpsi);
+          const double g2 = gpsi * gpsi;
+          h[m] = o.y * (P.mode == 1 ? -2.0 * g2 * gpsi : g2);
           a[m] = 0.0;
         }
         if ((nc & 1) == 0) {
@@ -292,11 +300,11 @@ __global__ void __launch_bounds__(GROUPS * M3_FT + 32, 1) mats3d_main_kernel(con
 #pragma unroll 2
           for (int jc = 0; jc < nc / 2; ++jc) {
             const double2 dd = drow[jc], nn = nrow[jc];
-            accumulate_node<MF>(dd.x, nn.x, m2phi, a);
-            accumulate_node<MF>(dd.y, nn.y, m2phi, a);
+            accumulate_node<MF, SQ>(dd.x, nn.x, m2phi, a);
+            accumulate_node<MF, SQ>(dd.y, nn.y, m2phi, a);
           }
         } else {
-          for (int jc = 0; jc < nc; ++jc) accumulate_node<MF>(d0[i * nc + jc], nw[i * nc + jc], m2phi, a);
+          for (int jc = 0; jc < nc; ++jc) accumulate_node<MF, SQ>(d0[i * nc + jc], nw[i * nc + jc], m2phi, a);
         }
 #pragma unroll
         for (int m = 0; m < MF; ++m) acc[m] = fma(h[m], a[m], acc[m]);
@@ -369,7 +377,7 @@ static size_t mats3d_main_smem(int nq, int nc, int rs, int ps, int groups, int m
 // MF = 2: one hardware seed per node serves both field points, 1/(d0 d1) then r0 = R d1, r1 = R d0 -- the same
 // FP64 instruction count as two separate Newton reciprocals (8 per node) and half the MUFU.RCP64H.
 constexpr int M3_NBAT = 4;
-template <int MF>
+template <int MF, bool SQ>
 __device__ __forceinline__ void mats3d_recip_batch(const double* __restrict__ dptr, const double (&m2)[MF],
                                                    double (&r)[M3_NBAT][MF]) {
   double d[M3_NBAT][MF];
@@ -411,6 +419,12 @@ __device__ __forceinline__ void mats3d_recip_batch(const double* __restrict__ dp
     for (int t = 0; t < M3_NBAT; ++t)
 #pragma unroll
       for (int k = 0; k < MF; ++k) r[t][k] = fma(r[t][k], d[t][k], r[t][k]);
+  }
+  if constexpr (SQ) {  // mass derivative of the boson line: the moments are taken of -G_phi^2
+#pragma unroll
+    for (int t = 0; t < M3_NBAT; ++t)
+#pragma unroll
+      for (int k = 0; k < MF; ++k) r[t][k] = -(r[t][k] * r[t][k]);
   }
 }
 
@@ -493,7 +507,7 @@ __device__ __forceinline__ void mats3d_pairs(const double4* __restrict__ bet4, c
   }
 }
 
-template <int NMAX, int NJ, int MF, int NTC>
+template <int NMAX, int NJ, int MF, int NTC, bool SQ>
 __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParams P) {
   constexpr int NT = 2 * NMAX + 1, NROWS = NJ + NMAX, NB = NJ * NT * 4, NPS = NMAX + 1;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -611,13 +625,14 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
 #pragma unroll
       for (int k = 0; k < MF; ++k) {
         const double gp = fast_rcp(D0 + m2psi[k]);
-        H[nb][k] = gp * gp;
+        const double g2 = gp * gp;
+        H[nb][k] = P.mode == 1 ? -2.0 * g2 * gp : g2;
       }
     }
     const bool pipelined = (nc % (2 * M3_NBAT)) == 0;
     const int l_last = NROWS * nc - M3_NBAT;
     double ra[M3_NBAT][MF], rb[M3_NBAT][MF];
-    if (pipelined) mats3d_recip_batch<MF>(d0, m2phi, ra);
+    if (pipelined) mats3d_recip_batch<MF, SQ>(d0, m2phi, ra);
 #pragma unroll 1
     for (int m = 0; m < NROWS; ++m) {
       // ---- angular moments of row m.  Written stage by stage over a batch of M3_NBAT nodes x MF field points so
@@ -632,11 +647,11 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
         //   ra = batch at c (ready), rb <- batch at c+4 while ra is accumulated, ra <- batch at c+8 while rb is ...
         for (int c = 0; c < nc; c += 2 * M3_NBAT) {
           const int L = m * nc + c;
-          mats3d_recip_batch<MF>(d0 + L + M3_NBAT, m2phi, rb);
+          mats3d_recip_batch<MF, SQ>(d0 + L + M3_NBAT, m2phi, rb);
           mats3d_moment_accumulate<MF>(num4 + c, ra, M);
           int Ln = L + 2 * M3_NBAT;
           Ln = Ln < l_last ? Ln : l_last;   // past the end of the chunk: recompute the last batch (result unused)
-          mats3d_recip_batch<MF>(d0 + Ln, m2phi, ra);
+          mats3d_recip_batch<MF, SQ>(d0 + Ln, m2phi, ra);
           mats3d_moment_accumulate<MF>(num4 + c + M3_NBAT, rb, M);
         }
       } else {
@@ -647,7 +662,8 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
           const double4 w = num4[c];
 #pragma unroll
           for (int k = 0; k < MF; ++k) {
-            const double r = fast_rcp(D0 + m2phi[k]);
+            double r = fast_rcp(D0 + m2phi[k]);
+            if constexpr (SQ) r = -(r * r);
             M[0][k] = fma(w.x, r, M[0][k]);
             M[1][k] = fma(w.y, r, M[1][k]);
             M[2][k] = fma(w.z, r, M[2][k]);
@@ -734,13 +750,13 @@ template <int GROUPS, int MF>
 static int mats3d_launch_main(const Mats3dParams& P, int sm_count, cudaStream_t stream) {
   const size_t smem = mats3d_main_smem(P.nq, P.nc, P.row_stride, P.psi_stride, GROUPS, MF);
   if (smem > 227 * 1024) return DFRG_EUNSUPPORTED;
-  cudaError_t e = cudaFuncSetAttribute(mats3d_main_kernel<GROUPS, MF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)smem);
+  auto kern = P.mode == 2 ? mats3d_main_kernel<GROUPS, MF, true> : mats3d_main_kernel<GROUPS, MF, false>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return check_cuda(e);
   const long long n_ftiles = (P.n_field + M3_FT * MF - 1) / (M3_FT * MF);
   const long long n_items = (long long)P.n_p * P.n_jext * n_ftiles;
   const int grid = (int)(n_items < sm_count ? n_items : sm_count);
-  mats3d_main_kernel<GROUPS, MF><<<grid, GROUPS * M3_FT + 32, smem, stream>>>(P);
+  kern<<<grid, GROUPS * M3_FT + 32, smem, stream>>>(P);
   return check_cuda(cudaGetLastError());
 }
 
@@ -755,10 +771,13 @@ template <int NMAX, int NJ>
 static int mats3d_moment_go(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream) {
   cudaError_t e;
 #define DFRG_M3_GO(MF, NTC)                                                                                          \
-  e = cudaFuncSetAttribute(mats3d_moment_kernel<NMAX, NJ, MF, NTC>, cudaFuncAttributeMaxDynamicSharedMemorySize,     \
-                           (int)pl.smem);                                                                            \
-  if (e != cudaSuccess) return check_cuda(e);                                                                        \
-  mats3d_moment_kernel<NMAX, NJ, MF, NTC><<<pl.grid, NTC, pl.smem, stream>>>(P);
+  {                                                                                                                  \
+    auto kern = P.mode == 2 ? mats3d_moment_kernel<NMAX, NJ, MF, NTC, true>                                          \
+                            : mats3d_moment_kernel<NMAX, NJ, MF, NTC, false>;                                        \
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);                       \
+    if (e != cudaSuccess) return check_cuda(e);                                                                      \
+    kern<<<pl.grid, NTC, pl.smem, stream>>>(P);                                                                      \
+  }
   if (pl.variant == 0) { DFRG_M3_GO(2, 256) }
   else if (pl.variant == 1) { DFRG_M3_GO(1, 512) }
   else { DFRG_M3_GO(1, 256) }
@@ -803,7 +822,7 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   P.xq = D->q.x; P.wq = D->q.w; P.xc = D->cos1.x; P.wc = D->cos1.w;
   P.Zpsi = D->tab_psi.v; P.Zphi = D->tab_phi.v; P.coef = D->coef;
   P.m2psi = m2_psi; P.m2phi = m2_phi; P.pext = p; P.out = out; P.dmin = dmin;
-  P.part = nullptr; P.tile_fields = 0; P.max_slots = 0; P.grid_main = 0;
+  P.part = nullptr; P.tile_fields = 0; P.max_slots = 0; P.grid_main = 0; P.mode = 0;
 
   // ---- path: moment factorisation where an instantiation exists (DFRG_M3_PATH=generic forces the other one) ----
   const char* vpath = getenv("DFRG_M3_PATH");
@@ -849,31 +868,39 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
     mats3d_psi_kernel<<<n_terms, 128, 0, stream>>>(P);
     rc = check_cuda(cudaGetLastError());
   }
-  if (rc == DFRG_OK && moment) {
-    rc = mats3d_moment_dispatch(P, pl, stream);
-    if (rc == DFRG_OK) {
-      const long long n_out = (long long)n_p * n_jext * n_field;
-      mats3d_fixup_kernel<<<(unsigned)((n_out + 255) / 256), 256, 0, stream>>>(P);
-      rc = check_cuda(cudaGetLastError());
-    }
-  } else if (rc == DFRG_OK) {
-    // generic path: consumer groups per CTA (radial nodes are dealt round-robin to the groups) and field points per
-    // thread; DFRG_M3_GROUPS / DFRG_M3_MF override the defaults (tuning knobs)
-    const char* vg = getenv("DFRG_M3_GROUPS");
-    const char* vm = getenv("DFRG_M3_MF");
-    int mf = n_field > 2 * M3_FT ? 4 : (n_field > M3_FT ? 2 : 1);
-    if (vm && atoi(vm) >= 1 && atoi(vm) < mf) mf = atoi(vm) == 3 ? 2 : atoi(vm);
-    const int groups = vg ? atoi(vg) : 6;
-    if (mf == 4) {
-      if (groups == 7) rc = mats3d_launch_main<7, 4>(P, sm_count, stream);
-      else if (groups == 4) rc = mats3d_launch_main<4, 4>(P, sm_count, stream);
-      else rc = mats3d_launch_main<6, 4>(P, sm_count, stream);
-    } else if (mf == 2) {
-      if (groups == 7) rc = mats3d_launch_main<7, 2>(P, sm_count, stream);
-      else if (groups == 4) rc = mats3d_launch_main<4, 2>(P, sm_count, stream);
-      else rc = mats3d_launch_main<6, 2>(P, sm_count, stream);
+  // one pass for the values, one more for each requested mass derivative (same kernels, mode 1 / 2)
+  double* const pass_out[3] = {out, D->dout_dm2_psi, D->dout_dm2_phi};
+  for (int mode = 0; mode < 3 && rc == DFRG_OK; ++mode) {
+    if (!pass_out[mode]) continue;
+    P.mode = mode;
+    P.out = pass_out[mode];
+    P.dmin = mode == 0 ? dmin : nullptr;
+    if (moment) {
+      rc = mats3d_moment_dispatch(P, pl, stream);
+      if (rc == DFRG_OK) {
+        const long long n_out = (long long)n_p * n_jext * n_field;
+        mats3d_fixup_kernel<<<(unsigned)((n_out + 255) / 256), 256, 0, stream>>>(P);
+        rc = check_cuda(cudaGetLastError());
+      }
     } else {
-      rc = mats3d_launch_main<4, 1>(P, sm_count, stream);
+      // generic path: consumer groups per CTA (radial nodes are dealt round-robin to the groups) and field points per
+      // thread; DFRG_M3_GROUPS / DFRG_M3_MF override the defaults (tuning knobs)
+      const char* vg = getenv("DFRG_M3_GROUPS");
+      const char* vm = getenv("DFRG_M3_MF");
+      int mf = n_field > 2 * M3_FT ? 4 : (n_field > M3_FT ? 2 : 1);
+      if (vm && atoi(vm) >= 1 && atoi(vm) < mf) mf = atoi(vm) == 3 ? 2 : atoi(vm);
+      const int groups = vg ? atoi(vg) : 6;
+      if (mf == 4) {
+        if (groups == 7) rc = mats3d_launch_main<7, 4>(P, sm_count, stream);
+        else if (groups == 4) rc = mats3d_launch_main<4, 4>(P, sm_count, stream);
+        else rc = mats3d_launch_main<6, 4>(P, sm_count, stream);
+      } else if (mf == 2) {
+        if (groups == 7) rc = mats3d_launch_main<7, 2>(P, sm_count, stream);
+        else if (groups == 4) rc = mats3d_launch_main<4, 2>(P, sm_count, stream);
+        else rc = mats3d_launch_main<6, 2>(P, sm_count, stream);
+      } else {
+        rc = mats3d_launch_main<4, 1>(P, sm_count, stream);
+      }
     }
   }
   scratch_free(scratch, stream);
@@ -906,7 +933,7 @@ extern "C" int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_
   Arena& A = thread_arena();
   const size_t nf = (size_t)n_field, n_out = (size_t)n_p * n_jext * nf;
   const size_t rows_psi = (size_t)D->n_max + 1, rows_phi = (size_t)n_jext + D->n_max, nt = (size_t)D->tab_psi.n_q;
-  const size_t need = 2 * ((size_t)D->q.n + D->cos1.n) + (rows_psi + rows_phi) * nt + 20 + 2 * nf + n_p + 2 * n_out;
+  const size_t need = 2 * ((size_t)D->q.n + D->cos1.n) + (rows_psi + rows_phi) * nt + 20 + 2 * nf + n_p + 4 * n_out;
   rc = A.begin(need * sizeof(double) + 32 * 256);
   if (rc != DFRG_OK) return rc;
   dfrg_mats3d_desc Dd = *D;
@@ -920,10 +947,14 @@ extern "C" int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_
   const double* d_p = A.put(p, n_p);
   double* d_out = A.reserve(n_out);
   double* d_dmin = dmin ? A.reserve(n_out) : nullptr;
+  Dd.dout_dm2_psi = D->dout_dm2_psi ? A.reserve(n_out) : nullptr;
+  Dd.dout_dm2_phi = D->dout_dm2_phi ? A.reserve(n_out) : nullptr;
   if (A.status() != DFRG_OK) return A.status();
   rc = mats3d_launch(&Dd, n_field, d_mpsi, d_mphi, n_p, d_p, n_jext, d_out, d_dmin, sms, A.stream());
   if (rc != DFRG_OK) return rc;
   A.fetch(out, d_out, n_out);
   if (dmin) A.fetch(dmin, d_dmin, n_out);
+  if (D->dout_dm2_psi) A.fetch(D->dout_dm2_psi, Dd.dout_dm2_psi, n_out);
+  if (D->dout_dm2_phi) A.fetch(D->dout_dm2_phi, Dd.dout_dm2_phi, n_out);
   return A.finish();
 }

@@ -46,9 +46,28 @@ def oracle_run(c, R, sel=None):
     return dict(out=out, dmin=dmin, sens=sens)
 
 
-def gpu_run(c, R, host=False, want_dmin=True):
+def oracle_run_dm2(c, R, sel=None):
+    """Mass derivatives from the oracle: dict of (value, sens) arrays keyed like gpu_run(..., want_d=True)."""
+    kd = kind_of(c)
+    if kd == "lpa":
+        d, s = oracle.lpa_dm2(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["prefactor"], c["reg_kind"], c["reg_order"],
+                              c["k"], *R["q"], c["rho"], c["u"], c["du"])
+        return dict(dchan=(d, s))
+    if kd == "twopoint":
+        d, s = oracle.loop4d_twopoint_dm2(c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], *R["q"], *R["c"],
+                                          c["Z"], c["lnq_lo"], c["lnq_hi"], c["interp"], c["coef"], c["m2"], c["pext"],
+                                          sel=sel)
+        return dict(dout=(d, s))
+    assert kd == "matsubara3d"
+    a, b, sa, sb = oracle.matsubara3d_dm2(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
+                                          *R["q"], *R["c"], c["Zpsi"], c["Zphi"], c["lnq_lo"], c["lnq_hi"], c["interp"],
+                                          c["coef"], c["m2psi"], c["m2phi"], c["pext"], c["n_jext"], sel=sel)
+    return dict(dpsi=(a, sa), dphi=(b, sb))
+
+
+def gpu_run(c, R, host=False, want_dmin=True, want_d=False):
     """Runs the workload through the C ABI (device entry point on torch CUDA tensors, or the *_host entry
-    point on numpy arrays).  -> dict(out=, dmin=, [chan=]) of numpy arrays."""
+    point on numpy arrays).  -> dict(out=, dmin=, [chan=], [dchan= | dout= | dpsi=, dphi=]) of numpy arrays."""
     import torch
     from paper_2412_13043_b200 import binding as B
 
@@ -66,17 +85,20 @@ def gpu_run(c, R, host=False, want_dmin=True):
     if kd == "lpa":
         nf = c["rho"].size
         flow, chan, dmin = new(nf), new(2, nf), new(nf) if want_dmin else None
+        dchan = new(2, nf) if want_d else None
         fn = B.dfrg_integrate_lpa_host if host else B.dfrg_integrate_lpa
         fn(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["N"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
-           rule("q"), up(c["rho"]), up(c["u"]), up(c["du"]), flow, chan, dmin)
-        res = dict(out=flow, chan=chan, dmin=dmin)
+           rule("q"), up(c["rho"]), up(c["u"]), up(c["du"]), flow, chan, dmin, dchan=dchan)
+        res = dict(out=flow, chan=chan, dmin=dmin, dchan=dchan)
     elif kd == "twopoint":
         out = new(c["pext"].size, c["m2"].size)
         dmin = new(c["pext"].size, c["m2"].size) if want_dmin else None
+        dout = new(c["pext"].size, c["m2"].size) if want_d else None
         fn = B.dfrg_integrate_loop4d_host if host else B.dfrg_integrate_loop4d
         fn(B.LOOP_TWOPOINT, c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], rule("q"), rule("c"), None, None,
-           (up(c["Z"]),), c["lnq_lo"], c["lnq_hi"], c["interp"], up(c["coef"]), up(c["m2"]), up(c["pext"]), out, dmin)
-        res = dict(out=out, dmin=dmin)
+           (up(c["Z"]),), c["lnq_lo"], c["lnq_hi"], c["interp"], up(c["coef"]), up(c["m2"]), up(c["pext"]), out, dmin,
+           dout_dm2=dout)
+        res = dict(out=out, dmin=dmin, dout=dout)
     elif kd == "threepoint":
         ne = c["ext"].shape[0]
         out, dmin = new(ne), new(ne) if want_dmin else None
@@ -88,14 +110,15 @@ def gpu_run(c, R, host=False, want_dmin=True):
     else:
         shape = (c["pext"].size, c["n_jext"], c["m2psi"].size)
         out, dmin = new(*shape), new(*shape) if want_dmin else None
+        dpsi, dphi = (new(*shape), new(*shape)) if want_d else (None, None)
         fn = B.dfrg_integrate_matsubara3d_host if host else B.dfrg_integrate_matsubara3d
         fn(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], rule("q"), rule("c"),
            up(c["Zpsi"]), up(c["Zphi"]), c["lnq_lo"], c["lnq_hi"], c["interp"], up(c["coef"]), up(c["m2psi"]),
-           up(c["m2phi"]), up(c["pext"]), c["n_jext"], out, dmin)
-        res = dict(out=out, dmin=dmin)
+           up(c["m2phi"]), up(c["pext"]), c["n_jext"], out, dmin, dout_dm2_psi=dpsi, dout_dm2_phi=dphi)
+        res = dict(out=out, dmin=dmin, dpsi=dpsi, dphi=dphi)
     if not host:
         torch.cuda.synchronize()
-    return {k_: (None if v is None else down(v)) for k_, v in res.items()}
+    return {k_: (None if v is None else down(v)) for k_, v in res.items() if v is not None or k_ == "dmin"}
 
 
 def parity_report(gpu, orc, dmin_orc, sens):
