@@ -193,6 +193,19 @@ def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
                    "nominal_evals_per_s": uniq * rr["phi"][0].numel() / ms * 1e3,
                    "integrals_per_s": o3.numel() / ms * 1e3,
                    "launches": 4}   # product-grid path: pre-pass, main, fix-up, and the general kernel returning at once
+    # cfg4 with both mass derivatives (three passes of the moment kernel: value, d/dm2_psi, d/dm2_phi)
+    c = inputs.config4()
+    R = make_rules(c, B.dfrg_quad_nodes)
+    rq, rc = (up(R["q"][0]), up(R["q"][1])), (up(R["c"][0]), up(R["c"][1]))
+    Zpsi, Zphi, coef = up(c["Zpsi"]), up(c["Zphi"]), up(c["coef"])
+    m2psi, m2phi, pext = up(c["m2psi"]), up(c["m2phi"]), up(c["pext"])
+    o4 = [torch.empty(pext.numel(), c["n_jext"], m2psi.numel(), dtype=torch.float64, device="cuda") for _ in range(3)]
+    ms = timeit(lambda: B.dfrg_integrate_matsubara3d(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"],
+                                                     c["k"], rq, rc, Zpsi, Zphi, c["lnq_lo"], c["lnq_hi"], c["interp"],
+                                                     coef, m2psi, m2phi, pext, c["n_jext"], o4[0], dout_dm2_psi=o4[1],
+                                                     dout_dm2_phi=o4[2]), n=3)
+    out["cfg4_with_mass_derivatives"] = {"ms": ms, "integrals_and_derivatives_per_s": 3 * o4[0].numel() / ms * 1e3,
+                                         "launches": 8}
     return out
 
 
