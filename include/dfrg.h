@@ -63,12 +63,19 @@ void dfrg_shutdown(void);               /* frees the calling thread's device are
 /* Regulator R_k(s), s = squared momentum, x = s/k^2; Rdot = k dR/dk (k d/dk = -2x d/dx).
  *   DFRG_REG_LITIM:    R = (k^2 - s) Theta(k^2 - s),            Rdot = 2 k^2 Theta(k^2 - s), Theta(0) = 0
  *   DFRG_REG_EXP_POLY: R = k^2 exp(-sum_{i=1..order} x^i / i),  Rdot = 2 R (1 + sum_{i=1..order} x^i)       (eq. 14)
- * order in [1, 16] for EXP_POLY; ignored for LITIM. */
+ * order in [1, 16] for EXP_POLY; ignored for LITIM.
+ * Dressed regulator (the paper's RB / RBdot with a wave-function renormalisation; "only the
+ * eta_i = -d_t Z_i/Z_i enter the flow equations"):  with Z_k = zk and eta = -k dZ_k/dk / Z_k
+ *   R = zk R_shape,   Rdot = k d(Z_k R_shape)/dk = zk (Rdot_shape - eta R_shape)
+ * in every propagator and in the insertion.  zk > 0 is required (DFRG_EINVAL otherwise: a zero-initialised struct is
+ * rejected); zk = 1, eta = 0 gives the plain shapes.  Z_k dresses the regulator only, not the s term (reading A12/A20). */
 typedef enum { DFRG_REG_LITIM = 0, DFRG_REG_EXP_POLY = 1 } dfrg_reg_kind;
 typedef struct {
   int kind;
   int order;
   double k;
+  double zk;
+  double eta;
 } dfrg_regulator;
 
 /* S1 (host): Gauss-Legendre rule of order n mapped to [a, b]: x ascending, w > 0, sum w = b - a

@@ -43,36 +43,36 @@ def _load():
         _lib.orc_table_lookup.restype = C.c_double
         _lib.orc_table_lookup.argtypes = [_dp, C.c_int, C.c_double, C.c_double, C.c_int, C.c_double]
         _lib.orc_regulator.restype = None
-        _lib.orc_regulator.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, _dp, _dp]
+        _lib.orc_regulator.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, _dp, _dp]
         _lib.orc_gl_rule.argtypes = [C.c_int, C.c_double, C.c_double, _dp, _dp]
         _lib.orc_lpa.argtypes = [C.c_int, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
-                                 C.c_int, C.c_int, C.c_double,
+                                 C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                  C.c_int, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _dp]
-        _lib.orc_loop4d_twopoint.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double,
+        _lib.orc_loop4d_twopoint.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                              C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                              _dp, C.c_int, C.c_double, C.c_double, C.c_int,
                                              _dp, C.c_int, C.c_int, _dp, C.c_int, _dp,
                                              C.c_longlong, _lp, _dp, _dp, _dp]
-        _lib.orc_loop4d_threepoint.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double,
+        _lib.orc_loop4d_threepoint.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                                C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                                C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                                _dp, _dp, _dp, C.c_int, C.c_double, C.c_double, C.c_int,
                                                _dp, C.c_int, C.c_int, _dp,
                                                C.c_longlong, _lp, C.c_int, _dp, _dp, _dp]
-        _lib.orc_matsubara3d.argtypes = [C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, C.c_double,
+        _lib.orc_matsubara3d.argtypes = [C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                          C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                          _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
                                          _dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int,
                                          C.c_longlong, _lp, _dp, _dp, _dp]
         _lib.orc_lpa_dm2.argtypes = [C.c_int, C.c_double, C.c_int, C.c_int, C.c_double,
-                                     C.c_int, C.c_int, C.c_double,
+                                     C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                      C.c_int, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp]
-        _lib.orc_loop4d_twopoint_dm2.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double,
+        _lib.orc_loop4d_twopoint_dm2.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                                  C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                                  _dp, C.c_int, C.c_double, C.c_double, C.c_int,
                                                  _dp, C.c_int, C.c_int, _dp, C.c_int, _dp,
                                                  C.c_longlong, _lp, _dp, _dp]
-        _lib.orc_matsubara3d_dm2.argtypes = [C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, C.c_double,
+        _lib.orc_matsubara3d_dm2.argtypes = [C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                              C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                              _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
                                              _dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int,
@@ -97,10 +97,10 @@ def gl_rule(n, a, b):
     return x, w
 
 
-def regulator(kind, order, k, s):
+def regulator(kind, order, k, s, zk=1.0, eta=0.0):
     R = C.c_double()
     Rd = C.c_double()
-    _load().orc_regulator(int(kind), int(order), float(k), float(s), C.byref(R), C.byref(Rd))
+    _load().orc_regulator(int(kind), int(order), float(k), float(zk), float(eta), float(s), C.byref(R), C.byref(Rd))
     return R.value, Rd.value
 
 
@@ -116,7 +116,7 @@ def _sel(sel):
     return int(sel.size), sel.ctypes.data_as(_lp), sel
 
 
-def lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, xq, wq, rho, u, du, want_sens=False):
+def lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, xq, wq, rho, u, du, want_sens=False, zk=1.0, eta=0.0):
     """Returns (flow[n_field], chan[2, n_field], dmin[n_field]) (+ sens[2, n_field] if want_sens)."""
     xq, wq, rho, u, du = map(_arr, (xq, wq, rho, u, du))
     nf = rho.size
@@ -125,7 +125,7 @@ def lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, xq, wq, rh
     dmin = np.empty(nf)
     sens = np.empty((2, nf))
     rc = _load().orc_lpa(int(d), float(T), int(n_max), int(reg_arg4d), float(N), float(prefactor),
-                         int(reg_kind), int(reg_order), float(k), int(xq.size), _d(xq), _d(wq),
+                         int(reg_kind), int(reg_order), float(k), float(zk), float(eta), int(xq.size), _d(xq), _d(wq),
                          int(nf), _d(rho), _d(u), _d(du), _d(flow), _d(chan), _d(dmin), _d(sens))
     if rc:
         raise ValueError("orc_lpa: bad arguments")
@@ -133,7 +133,7 @@ def lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, xq, wq, rh
 
 
 def loop4d_twopoint(prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Z, lnq_lo, lnq_hi, interp,
-                    coef, m2, pext, sel=None, want_sens=False):
+                    coef, m2, pext, sel=None, want_sens=False, zk=1.0, eta=0.0):
     """Returns (out, dmin): shape [n_ext, n_field], or [n_sel] for flat indices e*n_field+f in sel."""
     xq, wq, xc, wc, Z, coef, m2, pext = map(_arr, (xq, wq, xc, wc, Z, coef, m2, pext))
     ns, selp, _keep = _sel(sel)
@@ -141,7 +141,7 @@ def loop4d_twopoint(prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Z, lnq_lo
     out = np.empty(shape)
     dmin = np.empty(shape)
     sens = np.empty(shape)
-    rc = _load().orc_loop4d_twopoint(float(prefactor), int(reg_kind), int(reg_order), float(k),
+    rc = _load().orc_loop4d_twopoint(float(prefactor), int(reg_kind), int(reg_order), float(k), float(zk), float(eta),
                                      int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
                                      _d(Z), int(Z.size), float(lnq_lo), float(lnq_hi), int(interp),
                                      _d(coef), int(coef.size), int(m2.size), _d(m2), int(pext.size), _d(pext),
@@ -152,7 +152,7 @@ def loop4d_twopoint(prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Z, lnq_lo
 
 
 def loop4d_threepoint(prefactor, reg_kind, reg_order, k, xq, wq, x1, w1, x2, w2, xphi, wphi,
-                      ZA, Zc, L3, lnq_lo, lnq_hi, interp, coef, ext, sel=None, literal_phi=False, want_sens=False):
+                      ZA, Zc, L3, lnq_lo, lnq_hi, interp, coef, ext, sel=None, literal_phi=False, want_sens=False, zk=1.0, eta=0.0):
     """ext: [n_ext, 3] = (|p1|, |p2|, alpha).  Returns (out[n_ext or n_sel], dmin)."""
     xq, wq, x1, w1, x2, w2, xphi, wphi, ZA, Zc, L3, coef, ext = map(
         _arr, (xq, wq, x1, w1, x2, w2, xphi, wphi, ZA, Zc, L3, coef, ext))
@@ -162,7 +162,7 @@ def loop4d_threepoint(prefactor, reg_kind, reg_order, k, xq, wq, x1, w1, x2, w2,
     out = np.empty(n_out)
     dmin = np.empty(n_out)
     sens = np.empty(n_out)
-    rc = _load().orc_loop4d_threepoint(float(prefactor), int(reg_kind), int(reg_order), float(k),
+    rc = _load().orc_loop4d_threepoint(float(prefactor), int(reg_kind), int(reg_order), float(k), float(zk), float(eta),
                                        int(xq.size), _d(xq), _d(wq), int(x1.size), _d(x1), _d(w1),
                                        int(x2.size), _d(x2), _d(w2), int(xphi.size), _d(xphi), _d(wphi),
                                        _d(ZA), _d(Zc), _d(L3), int(ZA.size), float(lnq_lo), float(lnq_hi),
@@ -174,7 +174,7 @@ def loop4d_threepoint(prefactor, reg_kind, reg_order, k, xq, wq, x1, w1, x2, w2,
 
 
 def matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zpsi, Zphi,
-                lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, want_sens=False):
+                lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, want_sens=False, zk=1.0, eta=0.0):
     """Zpsi, Zphi: [n_freq, n_q].  Returns (out, dmin): [n_p, n_jext, n_field] or [n_sel]
     for flat indices (e*n_jext + j)*n_field + f in sel."""
     xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext = map(
@@ -186,7 +186,7 @@ def matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zps
     out = np.empty(shape)
     dmin = np.empty(shape)
     sens = np.empty(shape)
-    rc = _load().orc_matsubara3d(float(T), int(n_max), float(prefactor), int(reg_kind), int(reg_order), float(k),
+    rc = _load().orc_matsubara3d(float(T), int(n_max), float(prefactor), int(reg_kind), int(reg_order), float(k), float(zk), float(eta),
                                  int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
                                  _d(Zpsi), _d(Zphi), int(tnq), int(nfreq), float(lnq_lo), float(lnq_hi), int(interp),
                                  _d(coef), int(coef.size), int(m2psi.size), _d(m2psi), _d(m2phi),
@@ -197,14 +197,14 @@ def matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zps
 
 
 # ---- mass derivatives (Jacobian support) ------------------------------------------------------------
-def lpa_dm2(d, T, n_max, reg_arg4d, prefactor, reg_kind, reg_order, k, xq, wq, rho, u, du):
+def lpa_dm2(d, T, n_max, reg_arg4d, prefactor, reg_kind, reg_order, k, xq, wq, rho, u, du, zk=1.0, eta=0.0):
     """Returns (dchan[2, n_field], sens[2, n_field]): dI/dm2 at the pion and sigma masses."""
     xq, wq, rho, u, du = map(_arr, (xq, wq, rho, u, du))
     nf = rho.size
     dchan = np.empty((2, nf))
     sens = np.empty((2, nf))
     rc = _load().orc_lpa_dm2(int(d), float(T), int(n_max), int(reg_arg4d), float(prefactor),
-                             int(reg_kind), int(reg_order), float(k), int(xq.size), _d(xq), _d(wq),
+                             int(reg_kind), int(reg_order), float(k), float(zk), float(eta), int(xq.size), _d(xq), _d(wq),
                              int(nf), _d(rho), _d(u), _d(du), _d(dchan), _d(sens))
     if rc:
         raise ValueError("orc_lpa_dm2: bad arguments")
@@ -212,14 +212,14 @@ def lpa_dm2(d, T, n_max, reg_arg4d, prefactor, reg_kind, reg_order, k, xq, wq, r
 
 
 def loop4d_twopoint_dm2(prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Z, lnq_lo, lnq_hi, interp,
-                        coef, m2, pext, sel=None):
+                        coef, m2, pext, sel=None, zk=1.0, eta=0.0):
     """Returns (dout, sens): d out[e][f] / d m2[f], shape [n_ext, n_field] or [n_sel]."""
     xq, wq, xc, wc, Z, coef, m2, pext = map(_arr, (xq, wq, xc, wc, Z, coef, m2, pext))
     ns, selp, _keep = _sel(sel)
     shape = (ns,) if sel is not None else (pext.size, m2.size)
     dout = np.empty(shape)
     sens = np.empty(shape)
-    rc = _load().orc_loop4d_twopoint_dm2(float(prefactor), int(reg_kind), int(reg_order), float(k),
+    rc = _load().orc_loop4d_twopoint_dm2(float(prefactor), int(reg_kind), int(reg_order), float(k), float(zk), float(eta),
                                          int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
                                          _d(Z), int(Z.size), float(lnq_lo), float(lnq_hi), int(interp),
                                          _d(coef), int(coef.size), int(m2.size), _d(m2), int(pext.size), _d(pext),
@@ -230,7 +230,7 @@ def loop4d_twopoint_dm2(prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Z, ln
 
 
 def matsubara3d_dm2(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zpsi, Zphi,
-                    lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None):
+                    lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, zk=1.0, eta=0.0):
     """Returns (dpsi, dphi, sens_psi, sens_phi): d out / d m2_psi[f] and d out / d m2_phi[f]."""
     xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext = map(
         _arr, (xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext))
@@ -238,7 +238,7 @@ def matsubara3d_dm2(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc,
     ns, selp, _keep = _sel(sel)
     shape = (ns,) if sel is not None else (pext.size, int(n_jext), m2psi.size)
     dpsi, dphi, spsi, sphi = (np.empty(shape) for _ in range(4))
-    rc = _load().orc_matsubara3d_dm2(float(T), int(n_max), float(prefactor), int(reg_kind), int(reg_order), float(k),
+    rc = _load().orc_matsubara3d_dm2(float(T), int(n_max), float(prefactor), int(reg_kind), int(reg_order), float(k), float(zk), float(eta),
                                      int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
                                      _d(Zpsi), _d(Zphi), int(tnq), int(nfreq), float(lnq_lo), float(lnq_hi),
                                      int(interp), _d(coef), int(coef.size), int(m2psi.size), _d(m2psi), _d(m2phi),

@@ -67,7 +67,17 @@ const double kInf = std::numeric_limits<double>::infinity();
 // kind 0: Litim      R = (k^2 - s) Theta(k^2 - s),  Rdot = 2 k^2 Theta(k^2 - s), Theta(0)=0
 // kind 1: EXP_POLY(N) R = k^2 exp(-sum_{i=1..N} x^i / i), Rdot = 2 R (1 + sum_{i=1..N} x^i)
 // s is the squared momentum, x = s/k^2, Rdot = k dR/dk.
-void regulator(int kind, int order, double k, double s, double* R, double* Rdot) {
+// Dressed regulator (wave-function renormalisation Z_k with anomalous dimension eta = -k dZ_k/dk / Z_k,
+// PAPER.md:367 "only the eta_i = -d_t Z_i/Z_i enter the flow equations"):
+//   R = zk R_shape,  Rdot = k d(Z_k R_shape)/dk = zk (Rdot_shape - eta R_shape);  zk = 1, eta = 0: the plain shapes.
+void regulator_shape(int kind, int order, double k, double s, double* R, double* Rdot);
+void regulator(int kind, int order, double k, double zk, double eta, double s, double* R, double* Rdot) {
+  double Rs, Rds;
+  regulator_shape(kind, order, k, s, &Rs, &Rds);
+  *R = zk * Rs;
+  *Rdot = zk * (Rds - eta * Rs);
+}
+void regulator_shape(int kind, int order, double k, double s, double* R, double* Rdot) {
   const double k2 = k * k;
   if (kind == 0) {
     if (s < k2) { *R = k2 - s; *Rdot = 2.0 * k2; }
@@ -186,8 +196,8 @@ int orc_gl_rule(int n, double a, double b, double* x, double* w) {
   return 0;
 }
 
-void orc_regulator(int kind, int order, double k, double s, double* R, double* Rdot) {
-  regulator(kind, order, k, s, R, Rdot);
+void orc_regulator(int kind, int order, double k, double zk, double eta, double s, double* R, double* Rdot) {
+  regulator(kind, order, k, zk, eta, s, R, Rdot);
 }
 
 double orc_table_lookup(const double* v, int n_q, double lnq_lo, double lnq_hi, int interp, double s) {
@@ -201,7 +211,7 @@ double orc_table_lookup(const double* v, int n_q, double lnq_lo, double lnq_hi, 
 // flow[f] = (N-1) I(u[f]) + I(u[f] + 2 rho[f] du[f]);  chan = [I_pi | I_sigma] (nullable);
 // dmin[f] = signed min over nodes and both channels of (denominator / k^2) (nullable).
 int orc_lpa(int d, double T, int n_max, int reg_arg4d, double N, double prefactor,
-            int reg_kind, int reg_order, double k,
+            int reg_kind, int reg_order, double k, double zk, double eta,
             int nq, const double* xq, const double* wq,
             int n_field, const double* rho, const double* u, const double* du,
             double* flow, double* chan, double* dmin, double* sens) {
@@ -222,7 +232,7 @@ int orc_lpa(int d, double T, int n_max, int reg_arg4d, double N, double prefacto
           const double q = xq[i];
           const double s = q * q;
           double R, Rd;
-          regulator(reg_kind, reg_order, k, s, &R, &Rd);
+          regulator(reg_kind, reg_order, k, zk, eta, s, &R, &Rd);
           const double D = s + R + m2;
           if (D / k2 < dm) dm = D / k2;
           const double term = wq[i] * ipow(q, d - 1) * Rd / D;
@@ -238,7 +248,7 @@ int orc_lpa(int d, double T, int n_max, int reg_arg4d, double N, double prefacto
             const double s = wn * wn + q * q;
             const double sR = reg_arg4d ? s : q * q;
             double R, Rd;
-            regulator(reg_kind, reg_order, k, sR, &R, &Rd);
+            regulator(reg_kind, reg_order, k, zk, eta, sR, &R, &Rd);
             const double D = s + R + m2;
             if (D / k2 < dm) dm = D / k2;
             const double term = wq[i] * ipow(q, d - 1) * Rd / D;
@@ -266,7 +276,7 @@ int orc_lpa(int d, double T, int n_max, int reg_arg4d, double N, double prefacto
 //               sum_j wc_j sqrt(1-c_j^2) (coef0 + coef1 q_i p_e c_j / k^2) G(s_ij;f),
 // s_ij = q_i^2 + p_e^2 + 2 q_i p_e c_j,  G(s;f) = 1/(Z(sqrt s) s + R(s) + m2_f).
 // sel (nullable): flat output indices e*n_field+f to compute; out/dmin then have n_sel entries.
-int orc_loop4d_twopoint(double prefactor, int reg_kind, int reg_order, double k,
+int orc_loop4d_twopoint(double prefactor, int reg_kind, int reg_order, double k, double zk, double eta,
                         int nq, const double* xq, const double* wq,
                         int nc, const double* xc, const double* wc,
                         const double* Zv, int Z_nq, double Z_lo, double Z_hi, int Z_interp,
@@ -288,7 +298,7 @@ int orc_loop4d_twopoint(double prefactor, int reg_kind, int reg_order, double k,
       const double q = xq[i];
       const double sq = q * q;
       double Rq, Rdq;
-      regulator(reg_kind, reg_order, k, sq, &Rq, &Rdq);
+      regulator(reg_kind, reg_order, k, zk, eta, sq, &Rq, &Rdq);
       const double Dq = table_lookup(Zv, Z_nq, Z_lo, Z_hi, Z_interp, sq) * sq + Rq + mm;
       if (Dq / k2 < dm) dm = Dq / k2;
       const double Gq = 1.0 / Dq;
@@ -298,7 +308,7 @@ int orc_loop4d_twopoint(double prefactor, int reg_kind, int reg_order, double k,
         const double c = xc[j];
         const double s = clamp0(sq + p * p + 2.0 * q * p * c);
         double R, Rd;
-        regulator(reg_kind, reg_order, k, s, &R, &Rd);
+        regulator(reg_kind, reg_order, k, zk, eta, s, &R, &Rd);
         const double D = table_lookup(Zv, Z_nq, Z_lo, Z_hi, Z_interp, s) * s + R + mm;
         if (D / k2 < dm) dm = D / k2;
         const double poly = coef[0] + coef[1] * (q * p * c / k2);
@@ -326,7 +336,7 @@ int orc_loop4d_twopoint(double prefactor, int reg_kind, int reg_order, double k,
 // out[e] = C sum_q w q^3 Rdot(q^2) G_A(q^2) sum_c1 w sqrt(1-c1^2) sum_c2 w sum_phi w G_A(s_a) G_A(s_b) Lam P
 // The integrand does not depend on phi; literal_phi != 0 evaluates it inside the phi loop
 // anyway (tiny inputs only), literal_phi == 0 evaluates it once and multiplies by sum_phi w.
-int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double k,
+int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double k, double zk, double eta,
                           int nq, const double* xq, const double* wq,
                           int n1, const double* x1, const double* w1,
                           int n2, const double* x2, const double* w2,
@@ -354,7 +364,7 @@ int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double 
       const double q = xq[i];
       const double sq = q * q;
       double Rq, Rdq;
-      regulator(reg_kind, reg_order, k, sq, &Rq, &Rdq);
+      regulator(reg_kind, reg_order, k, zk, eta, sq, &Rq, &Rdq);
       const double Dq = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, sq) * sq + Rq;
       if (Dq / k2 < dm) dm = Dq / k2;
       acc_t acc_1 = 0.0L, sn_1 = 0.0L;
@@ -373,8 +383,8 @@ int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double 
           double F = 0.0, Fabs = 0.0;
           for (int jp = 0; jp < nphi_eval; ++jp) {
             double Ra, Rda, Rb, Rdb;
-            regulator(reg_kind, reg_order, k, s_a, &Ra, &Rda);
-            regulator(reg_kind, reg_order, k, s_b, &Rb, &Rdb);
+            regulator(reg_kind, reg_order, k, zk, eta, s_a, &Ra, &Rda);
+            regulator(reg_kind, reg_order, k, zk, eta, s_b, &Rb, &Rdb);
             const double Da = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, s_a) * s_a + Ra;
             const double Db = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, s_b) * s_b + Rb;
             if (Da / k2 < dm) dm = Da / k2;
@@ -430,7 +440,7 @@ int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double 
 // P = sum_{a+b+c<=3} kap_abc y1^a y2^b y3^c, y1 = nu_n nu_j/k^2, y2 = p q c/k^2, y3 = s_psi/k^2
 // out[p][j][f] = C T sum_n sum_q w q^2 Rdot(s_psi) G_psi^2 sum_c w P G_phi
 // Tables are row-major [n_freq][n_q]; the momentum argument is the spatial one (q^2, r^2).
-int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg_order, double k,
+int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg_order, double k, double zk, double eta,
                     int nq, const double* xq, const double* wq,
                     int nc, const double* xc, const double* wc,
                     const double* Zpsi, const double* Zphi, int t_nq, int t_nfreq,
@@ -465,7 +475,7 @@ int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg
         const double q = xq[i];
         const double spsi = nun * nun + q * q;
         double Rp, Rdp;
-        regulator(reg_kind, reg_order, k, spsi, &Rp, &Rdp);
+        regulator(reg_kind, reg_order, k, zk, eta, spsi, &Rp, &Rdp);
         const double Dpsi =
             table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q) * spsi + Rp + m2psi[f];
         if (Dpsi / k2 < dm) dm = Dpsi / k2;
@@ -477,7 +487,7 @@ int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg
           const double r2 = clamp0(p * p + q * q - 2.0 * p * q * c);
           const double sphi = om * om + r2;
           double Rb, Rdb;
-          regulator(reg_kind, reg_order, k, sphi, &Rb, &Rdb);
+          regulator(reg_kind, reg_order, k, zk, eta, sphi, &Rb, &Rdb);
           const double Dphi =
               table_lookup(Zphi + (size_t)mabs * t_nq, t_nq, t_lo, t_hi, t_interp, r2) * sphi + Rb + m2phi[f];
           if (Dphi / k2 < dm) dm = Dphi / k2;
@@ -516,7 +526,7 @@ int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg
 
 // dchan[ch][f] = dI/dm2 at m2 = m2_channel:  -C [T] sum w q^(d-1) Rdot / D^2
 int orc_lpa_dm2(int d, double T, int n_max, int reg_arg4d, double prefactor,
-                int reg_kind, int reg_order, double k,
+                int reg_kind, int reg_order, double k, double zk, double eta,
                 int nq, const double* xq, const double* wq,
                 int n_field, const double* rho, const double* u, const double* du,
                 double* dchan, double* sens) {
@@ -536,7 +546,7 @@ int orc_lpa_dm2(int d, double T, int n_max, int reg_arg4d, double prefactor,
           const double s = wn * wn + q * q;
           const double sR = (T == 0.0 || reg_arg4d) ? s : q * q;
           double R, Rd;
-          regulator(reg_kind, reg_order, k, sR, &R, &Rd);
+          regulator(reg_kind, reg_order, k, zk, eta, sR, &R, &Rd);
           const double D = s + R + m2;
           const double term = -wq[i] * ipow(q, d - 1) * Rd / (D * D);
           acc += (acc_t)term;
@@ -553,7 +563,7 @@ int orc_lpa_dm2(int d, double T, int n_max, int reg_arg4d, double prefactor,
 
 // dout[e][f] = d out / d m2_f with the same m2 in all three propagators:
 //   C sum_i wq q^3 Rdot [ -2 G(q)^3 sum_j W'_ij G(s_ij) - G(q)^2 sum_j W'_ij G(s_ij)^2 ]
-int orc_loop4d_twopoint_dm2(double prefactor, int reg_kind, int reg_order, double k,
+int orc_loop4d_twopoint_dm2(double prefactor, int reg_kind, int reg_order, double k, double zk, double eta,
                             int nq, const double* xq, const double* wq,
                             int nc, const double* xc, const double* wc,
                             const double* Zv, int Z_nq, double Z_lo, double Z_hi, int Z_interp,
@@ -574,7 +584,7 @@ int orc_loop4d_twopoint_dm2(double prefactor, int reg_kind, int reg_order, doubl
       const double q = xq[i];
       const double sq = q * q;
       double Rq, Rdq;
-      regulator(reg_kind, reg_order, k, sq, &Rq, &Rdq);
+      regulator(reg_kind, reg_order, k, zk, eta, sq, &Rq, &Rdq);
       const double Dq = table_lookup(Zv, Z_nq, Z_lo, Z_hi, Z_interp, sq) * sq + Rq + mm;
       const double Gq = 1.0 / Dq;
       const double condq = (std::fabs(Dq - mm) + std::fabs(mm)) / std::fabs(Dq);
@@ -583,7 +593,7 @@ int orc_loop4d_twopoint_dm2(double prefactor, int reg_kind, int reg_order, doubl
         const double c = xc[j];
         const double s = clamp0(sq + p * p + 2.0 * q * p * c);
         double R, Rd;
-        regulator(reg_kind, reg_order, k, s, &R, &Rd);
+        regulator(reg_kind, reg_order, k, zk, eta, s, &R, &Rd);
         const double D = table_lookup(Zv, Z_nq, Z_lo, Z_hi, Z_interp, s) * s + R + mm;
         const double G = 1.0 / D;
         const double poly = coef[0] + coef[1] * (q * p * c / k2);
@@ -606,7 +616,7 @@ int orc_loop4d_twopoint_dm2(double prefactor, int reg_kind, int reg_order, doubl
 
 // dpsi[p][j][f] = d out / d m2_psi_f = C T sum_n sum_q w q^2 Rdot (-2 G_psi^3) sum_c w P G_phi
 // dphi[p][j][f] = d out / d m2_phi_f = C T sum_n sum_q w q^2 Rdot G_psi^2 sum_c w P (-G_phi^2)
-int orc_matsubara3d_dm2(double T, int n_max, double prefactor, int reg_kind, int reg_order, double k,
+int orc_matsubara3d_dm2(double T, int n_max, double prefactor, int reg_kind, int reg_order, double k, double zk, double eta,
                         int nq, const double* xq, const double* wq,
                         int nc, const double* xc, const double* wc,
                         const double* Zpsi, const double* Zphi, int t_nq, int t_nfreq,
@@ -640,7 +650,7 @@ int orc_matsubara3d_dm2(double T, int n_max, double prefactor, int reg_kind, int
         const double q = xq[i];
         const double spsi = nun * nun + q * q;
         double Rp, Rdp;
-        regulator(reg_kind, reg_order, k, spsi, &Rp, &Rdp);
+        regulator(reg_kind, reg_order, k, zk, eta, spsi, &Rp, &Rdp);
         const double Dpsi =
             table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q) * spsi + Rp + m2psi[f];
         const double Gpsi = 1.0 / Dpsi;
@@ -651,7 +661,7 @@ int orc_matsubara3d_dm2(double T, int n_max, double prefactor, int reg_kind, int
           const double r2 = clamp0(p * p + q * q - 2.0 * p * q * c);
           const double sphi = om * om + r2;
           double Rb, Rdb;
-          regulator(reg_kind, reg_order, k, sphi, &Rb, &Rdb);
+          regulator(reg_kind, reg_order, k, zk, eta, sphi, &Rb, &Rdb);
           const double Dphi =
               table_lookup(Zphi + (size_t)mabs * t_nq, t_nq, t_lo, t_hi, t_interp, r2) * sphi + Rb + m2phi[f];
           const double Gphi = 1.0 / Dphi;

@@ -29,7 +29,7 @@ _vp = C.c_void_p
 
 
 class Regulator(C.Structure):
-    _fields_ = [("kind", C.c_int), ("order", C.c_int), ("k", C.c_double)]
+    _fields_ = [("kind", C.c_int), ("order", C.c_int), ("k", C.c_double), ("zk", C.c_double), ("eta", C.c_double)]
 
 
 class Rule(C.Structure):
@@ -150,15 +150,15 @@ def dfrg_quad_nodes(n, a, b, rule_kind=RULE_GAUSS_LEGENDRE):
 
 
 # ---- LPA ------------------------------------------------------------------------------------------
-def _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, device, dchan=None):
+def _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, device, dchan=None, reg_zk=1.0, reg_eta=0.0):
     return LpaDesc(int(d), float(T), int(n_max), int(reg_arg4d), float(N), float(prefactor),
-                   Regulator(int(reg_kind), int(reg_order), float(k)), _rule(rule_q, device), _ptr(dchan, device))
+                   Regulator(int(reg_kind), int(reg_order), float(k), float(reg_zk), float(reg_eta)), _rule(rule_q, device), _ptr(dchan, device))
 
 
 def dfrg_integrate_lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, rho, u, du,
-                       flow, chan=None, dmin=None, dchan=None):
+                       flow, chan=None, dmin=None, dchan=None, reg_zk=1.0, reg_eta=0.0):
     """dchan (optional, [2, n_field]): dI/dm2 per channel (include/dfrg.h, "Mass derivatives")."""
-    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, True, dchan)
+    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, True, dchan, reg_zk, reg_eta)
     _check(lib().dfrg_integrate_lpa(C.byref(D), int(rho.numel()), _ptr(rho, True), _ptr(u, True), _ptr(du, True),
                                     _ptr(flow, True), _ptr(chan, True), _ptr(dmin, True), _stream()),
            "dfrg_integrate_lpa")
@@ -166,8 +166,8 @@ def dfrg_integrate_lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order
 
 
 def dfrg_integrate_lpa_host(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, rho, u, du,
-                            flow, chan=None, dmin=None, dchan=None):
-    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, False, dchan)
+                            flow, chan=None, dmin=None, dchan=None, reg_zk=1.0, reg_eta=0.0):
+    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, False, dchan, reg_zk, reg_eta)
     n_field = rho.numel() if hasattr(rho, "numel") else rho.size
     _check(lib().dfrg_integrate_lpa_host(C.byref(D), int(n_field), _ptr(rho, False), _ptr(u, False),
                                          _ptr(du, False), _ptr(flow, False), _ptr(chan, False), _ptr(dmin, False)),
@@ -177,11 +177,11 @@ def dfrg_integrate_lpa_host(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_
 
 # ---- loop4d ---------------------------------------------------------------------------------------
 def _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
-                 lnq_hi, interp, coef, device, ext_outer=0, dout_dm2=None):
+                 lnq_hi, interp, coef, device, ext_outer=0, dout_dm2=None, reg_zk=1.0, reg_eta=0.0):
     T3 = Table * 3
     tt = [_table(t, lnq_lo, lnq_hi, interp, device) for t in tabs] + [_table(None, 0, 0, 0, device)] * (3 - len(tabs))
     n_coef = coef.numel() if hasattr(coef, "numel") else coef.size
-    return Loop4dDesc(int(family), float(prefactor), Regulator(int(reg_kind), int(reg_order), float(k)),
+    return Loop4dDesc(int(family), float(prefactor), Regulator(int(reg_kind), int(reg_order), float(k), float(reg_zk), float(reg_eta)),
                       _rule(rule_q, device), _rule(rule_c1, device), _rule(rule_c2, device), _rule(rule_phi, device),
                       T3(*tt), _ptr(coef, device), int(n_coef), int(ext_outer), _ptr(dout_dm2, device))
 
@@ -191,11 +191,11 @@ def _n(a):
 
 
 def dfrg_integrate_loop4d(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs,
-                          lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0, dout_dm2=None):
+                          lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0, dout_dm2=None, reg_zk=1.0, reg_eta=0.0):
     """two-point: tabs=(Z,), m2=[n_field], ext=[n_ext] -> out [n_ext, n_field];
     three-point: tabs=(Z_A, Z_c, lambda3), m2=None, ext=[n_ext, 3] -> out [n_ext]; ext_outer: dfrg_loop4d_desc."""
     D = _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
-                     lnq_hi, interp, coef, True, ext_outer, dout_dm2)
+                     lnq_hi, interp, coef, True, ext_outer, dout_dm2, reg_zk, reg_eta)
     n_ext = _n(ext) if family == LOOP_TWOPOINT else _n(ext) // 3
     _check(lib().dfrg_integrate_loop4d(C.byref(D), _n(m2), _ptr(m2, True), n_ext, _ptr(ext, True),
                                        _ptr(out, True), _ptr(dmin, True), _stream()), "dfrg_integrate_loop4d")
@@ -203,9 +203,9 @@ def dfrg_integrate_loop4d(family, prefactor, reg_kind, reg_order, k, rule_q, rul
 
 
 def dfrg_integrate_loop4d_host(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs,
-                               lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0, dout_dm2=None):
+                               lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0, dout_dm2=None, reg_zk=1.0, reg_eta=0.0):
     D = _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
-                     lnq_hi, interp, coef, False, ext_outer, dout_dm2)
+                     lnq_hi, interp, coef, False, ext_outer, dout_dm2, reg_zk, reg_eta)
     n_ext = _n(ext) if family == LOOP_TWOPOINT else _n(ext) // 3
     _check(lib().dfrg_integrate_loop4d_host(C.byref(D), _n(m2), _ptr(m2, False), n_ext, _ptr(ext, False),
                                             _ptr(out, False), _ptr(dmin, False)), "dfrg_integrate_loop4d_host")
@@ -214,8 +214,8 @@ def dfrg_integrate_loop4d_host(family, prefactor, reg_kind, reg_order, k, rule_q
 
 # ---- matsubara3d ----------------------------------------------------------------------------------
 def _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp, coef,
-               device, dpsi=None, dphi=None):
-    return Mats3dDesc(float(T), int(n_max), float(prefactor), Regulator(int(reg_kind), int(reg_order), float(k)),
+               device, dpsi=None, dphi=None, reg_zk=1.0, reg_eta=0.0):
+    return Mats3dDesc(float(T), int(n_max), float(prefactor), Regulator(int(reg_kind), int(reg_order), float(k), float(reg_zk), float(reg_eta)),
                       _rule(rule_q, device), _rule(rule_c, device),
                       _table(Zpsi, lnq_lo, lnq_hi, interp, device), _table(Zphi, lnq_lo, lnq_hi, interp, device),
                       _ptr(coef, device), _n(coef), _ptr(dpsi, device), _ptr(dphi, device))
@@ -223,10 +223,10 @@ def _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi
 
 def dfrg_integrate_matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo,
                                lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, out, dmin=None,
-                               dout_dm2_psi=None, dout_dm2_phi=None):
+                               dout_dm2_psi=None, dout_dm2_phi=None, reg_zk=1.0, reg_eta=0.0):
     """out: [n_p, n_jext, n_field]."""
     D = _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp,
-                   coef, True, dout_dm2_psi, dout_dm2_phi)
+                   coef, True, dout_dm2_psi, dout_dm2_phi, reg_zk, reg_eta)
     _check(lib().dfrg_integrate_matsubara3d(C.byref(D), _n(m2psi), _ptr(m2psi, True), _ptr(m2phi, True), _n(pext),
                                             _ptr(pext, True), int(n_jext), _ptr(out, True), _ptr(dmin, True),
                                             _stream()), "dfrg_integrate_matsubara3d")
@@ -235,9 +235,9 @@ def dfrg_integrate_matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, rule
 
 def dfrg_integrate_matsubara3d_host(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo,
                                     lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, out, dmin=None,
-                               dout_dm2_psi=None, dout_dm2_phi=None):
+                               dout_dm2_psi=None, dout_dm2_phi=None, reg_zk=1.0, reg_eta=0.0):
     D = _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp,
-                   coef, False, dout_dm2_psi, dout_dm2_phi)
+                   coef, False, dout_dm2_psi, dout_dm2_phi, reg_zk, reg_eta)
     _check(lib().dfrg_integrate_matsubara3d_host(C.byref(D), _n(m2psi), _ptr(m2psi, False), _ptr(m2phi, False),
                                                  _n(pext), _ptr(pext, False), int(n_jext), _ptr(out, False),
                                                  _ptr(dmin, False)), "dfrg_integrate_matsubara3d_host")

@@ -128,13 +128,22 @@ struct RegParams {
   int order;
   double k2;      // k^2
   double inv_k2;  // 1/k^2
+  double zk;      // wave-function renormalisation: R = zk R_shape
+  double eta;     // anomalous dimension: Rdot = zk (Rdot_shape - eta R_shape)
 };
+// host side: RegParams from the ABI struct
+inline RegParams reg_params(int kind, int order, double k, double zk, double eta) {
+  RegParams rp;
+  rp.kind = kind; rp.order = order; rp.k2 = k * k; rp.inv_k2 = 1.0 / rp.k2; rp.zk = zk; rp.eta = eta;
+  return rp;
+}
 
 __device__ __forceinline__ void regulator(const RegParams& rp, const FastMath& fm, double s, double& R, double& Rdot) {
   if (rp.kind == 0) {
     const bool in = s < rp.k2;
-    R = in ? rp.k2 - s : 0.0;
-    Rdot = in ? 2.0 * rp.k2 : 0.0;
+    const double Rs = in ? rp.k2 - s : 0.0;
+    R = rp.zk * Rs;
+    Rdot = rp.zk * ((in ? 2.0 * rp.k2 : 0.0) - rp.eta * Rs);
     return;
   }
   const double x = s * rp.inv_k2;
@@ -148,8 +157,8 @@ __device__ __forceinline__ void regulator(const RegParams& rp, const FastMath& f
     }
   }
   const double r = rp.k2 * fm_exp_neg(fm, expo);
-  R = r;
-  Rdot = 2.0 * r * (1.0 + geo);
+  R = rp.zk * r;
+  Rdot = rp.zk * (2.0 * r * (1.0 + geo) - rp.eta * r);
 }
 
 // ---- log-grid table look-up --------------------------------------------------------------------

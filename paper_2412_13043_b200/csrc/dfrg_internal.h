@@ -20,7 +20,7 @@ inline int check_cuda(cudaError_t e) {
 int require_sm100(int* sm_count);
 
 inline bool valid_regulator(const dfrg_regulator& r) {
-  if (!(r.k > 0.0)) return false;
+  if (!(r.k > 0.0) || !(r.zk > 0.0) || !(r.eta == r.eta)) return false;
   if (r.kind == DFRG_REG_LITIM) return true;
   return r.kind == DFRG_REG_EXP_POLY && r.order >= 1 && r.order <= 16;
 }

@@ -332,7 +332,7 @@ template <int REGK>  // 0 Litim, 1 EXP_POLY(1), 2 EXP_POLY(order)
 __device__ __forceinline__ double t3_reg_R(const RegParams& rp, const double* __restrict__ fxtab,
                                            const double* __restrict__ kc, const double s) {
   if constexpr (REGK == 0) {
-    return s < rp.k2 ? rp.k2 - s : 0.0;
+    return s < rp.k2 ? rp.zk * (rp.k2 - s) : 0.0;
   } else if constexpr (REGK == 1) {
     return fx_exp_neg(fxtab, kc, s * rp.inv_k2);
   } else {
@@ -382,7 +382,7 @@ __global__ void __launch_bounds__(T3V2_THREADS, 1) threepoint_kernel_v2(const Th
     stage_to_smem(L, &bar, 0);
   }
   const FastMath fm = fm_build(fmmem, P.fmc);
-  const double* fxtab = fx_build(fxmem, P.reg.k2);
+  const double* fxtab = fx_build(fxmem, P.reg.zk * P.reg.k2);
   const LogGrid lg = lg_build(lgmem, P.grid.lo, P.grid.inv_h, nt);
   const double* kc = P.fmc.c;
   const double2* cZA = cells_build_guarded(cZA_all, sZA, nt, P.grid.interp);
@@ -582,7 +582,7 @@ __global__ void __launch_bounds__(T3G_THREADS, 1) t3g_prepass_kernel(const Three
     stage_to_smem(L, &bar, 0);
   }
   const FastMath fm = fm_build(sm.fmmem, P.fmc);
-  const double* fxtab = fx_build(sm.fxmem, P.reg.k2);
+  const double* fxtab = fx_build(sm.fxmem, P.reg.zk * P.reg.k2);
   const LogGrid lg = lg_build(sm.lgmem, P.grid.lo, P.grid.inv_h, nt);
   const double* kc = P.fmc.c;
   const double2* cZA = cells_build_guarded(sm.cZA_all, sm.sZA, nt, P.grid.interp);
@@ -680,7 +680,7 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
     L.add(sm.sZA, P.ZA, nt); L.add(sm.sL3, P.L3, nt);
     stage_to_smem(L, &bar, 0);
   }
-  const double* fxtab = fx_build(sm.fxmem, P.reg.k2);
+  const double* fxtab = fx_build(sm.fxmem, P.reg.zk * P.reg.k2);
   const LogGrid lg = lg_build(sm.lgmem, P.grid.lo, P.grid.inv_h, nt);
   const double* kc = P.fmc.c;
   const double2* cZA = cells_build_guarded(sm.cZA_all, sm.sZA, nt, P.grid.interp);
@@ -850,7 +850,7 @@ static int loop4d_validate(const dfrg_loop4d_desc* D, int n_field, const double*
 }
 
 static void fill_common(const dfrg_regulator& r, const dfrg_table& t, RegParams* rp, GridParams* gp) {
-  rp->kind = r.kind; rp->order = r.order; rp->k2 = r.k * r.k; rp->inv_k2 = 1.0 / rp->k2;
+  *rp = reg_params(r.kind, r.order, r.k, r.zk, r.eta);
   gp->lo = t.lnq_lo; gp->inv_h = (double)(t.n_q - 1) / (t.lnq_hi - t.lnq_lo); gp->n = t.n_q; gp->interp = t.interp;
 }
 

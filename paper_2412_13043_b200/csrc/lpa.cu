@@ -139,8 +139,7 @@ static int lpa_launch(const dfrg_lpa_desc* D, int n_field, const double* rho, co
   LpaParams P;
   P.d = D->d; P.n_max = D->n_max; P.reg_arg4d = D->reg_arg4d; P.nq = D->q.n; P.n_field = n_field;
   P.T = D->T; P.N = D->N; P.prefactor = D->prefactor;
-  P.reg.kind = D->reg.kind; P.reg.order = D->reg.order;
-  P.reg.k2 = D->reg.k * D->reg.k; P.reg.inv_k2 = 1.0 / P.reg.k2;
+  P.reg = reg_params(D->reg.kind, D->reg.order, D->reg.k, D->reg.zk, D->reg.eta);
   P.fmc = fm_consts();
   P.xq = D->q.x; P.wq = D->q.w; P.rho = rho; P.u = u; P.du = du;
   P.flow = flow; P.chan = chan; P.dmin = dmin; P.dchan = D->dchan;

@@ -815,7 +815,7 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   P.chunk_stride = (P.n_rows * P.nc + 1) & ~1;
   P.psi_stride = P.nq;
   P.T = D->T; P.prefactor = D->prefactor;
-  P.reg.kind = D->reg.kind; P.reg.order = D->reg.order; P.reg.k2 = D->reg.k * D->reg.k; P.reg.inv_k2 = 1.0 / P.reg.k2;
+  P.reg = reg_params(D->reg.kind, D->reg.order, D->reg.k, D->reg.zk, D->reg.eta);
   P.grid.lo = D->tab_psi.lnq_lo; P.grid.n = D->tab_psi.n_q; P.grid.interp = D->tab_psi.interp;
   P.grid.inv_h = (double)(P.grid.n - 1) / (D->tab_psi.lnq_hi - D->tab_psi.lnq_lo);
   P.fmc = fm_consts();

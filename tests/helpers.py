@@ -21,28 +21,33 @@ def make_rules(c, gen):
     return {key[5:]: gen(*val) for key, val in c.items() if key.startswith("rule_")}
 
 
+def _dress(c):
+    """Dressed-regulator parameters of a workload (reading A20); absent = plain shapes."""
+    return dict(zk=c.get("reg_zk", 1.0), eta=c.get("reg_eta", 0.0))
+
+
 def oracle_run(c, R, sel=None):
     """-> (out, dmin, sens); lpa: out = flow[n_field], extra channels under key 'chan' are returned via dict."""
     kd = kind_of(c)
     if kd == "lpa":
         flow, chan, dmin, sens = oracle.lpa(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["N"], c["prefactor"],
                                             c["reg_kind"], c["reg_order"], c["k"], *R["q"], c["rho"], c["u"], c["du"],
-                                            want_sens=True)
+                                            want_sens=True, **_dress(c))
         return dict(out=flow, chan=chan, dmin=dmin, sens=(c["N"] - 1.0) * sens[0] + sens[1], sens_chan=sens)
     if kd == "twopoint":
         out, dmin, sens = oracle.loop4d_twopoint(c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], *R["q"], *R["c"],
                                                  c["Z"], c["lnq_lo"], c["lnq_hi"], c["interp"], c["coef"], c["m2"],
-                                                 c["pext"], sel=sel, want_sens=True)
+                                                 c["pext"], sel=sel, want_sens=True, **_dress(c))
     elif kd == "threepoint":
         out, dmin, sens = oracle.loop4d_threepoint(c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], *R["q"],
                                                    *R["c1"], *R["c2"], *R["phi"], c["ZA"], c["Zc"], c["L3"],
                                                    c["lnq_lo"], c["lnq_hi"], c["interp"], c["coef"], c["ext"],
-                                                   sel=sel, want_sens=True)
+                                                   sel=sel, want_sens=True, **_dress(c))
     else:
         out, dmin, sens = oracle.matsubara3d(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
                                              *R["q"], *R["c"], c["Zpsi"], c["Zphi"], c["lnq_lo"], c["lnq_hi"],
                                              c["interp"], c["coef"], c["m2psi"], c["m2phi"], c["pext"], c["n_jext"],
-                                             sel=sel, want_sens=True)
+                                             sel=sel, want_sens=True, **_dress(c))
     return dict(out=out, dmin=dmin, sens=sens)
 
 
@@ -51,17 +56,17 @@ def oracle_run_dm2(c, R, sel=None):
     kd = kind_of(c)
     if kd == "lpa":
         d, s = oracle.lpa_dm2(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["prefactor"], c["reg_kind"], c["reg_order"],
-                              c["k"], *R["q"], c["rho"], c["u"], c["du"])
+                              c["k"], *R["q"], c["rho"], c["u"], c["du"], **_dress(c))
         return dict(dchan=(d, s))
     if kd == "twopoint":
         d, s = oracle.loop4d_twopoint_dm2(c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], *R["q"], *R["c"],
                                           c["Z"], c["lnq_lo"], c["lnq_hi"], c["interp"], c["coef"], c["m2"], c["pext"],
-                                          sel=sel)
+                                          sel=sel, **_dress(c))
         return dict(dout=(d, s))
     assert kd == "matsubara3d"
     a, b, sa, sb = oracle.matsubara3d_dm2(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
                                           *R["q"], *R["c"], c["Zpsi"], c["Zphi"], c["lnq_lo"], c["lnq_hi"], c["interp"],
-                                          c["coef"], c["m2psi"], c["m2phi"], c["pext"], c["n_jext"], sel=sel)
+                                          c["coef"], c["m2psi"], c["m2phi"], c["pext"], c["n_jext"], sel=sel, **_dress(c))
     return dict(dpsi=(a, sa), dphi=(b, sb))
 
 
@@ -82,13 +87,14 @@ def gpu_run(c, R, host=False, want_dmin=True, want_d=False):
     rule = lambda key: (up(R[key][0]), up(R[key][1]))
     kd = kind_of(c)
     res = {}
+    dress = dict(reg_zk=c.get("reg_zk", 1.0), reg_eta=c.get("reg_eta", 0.0))
     if kd == "lpa":
         nf = c["rho"].size
         flow, chan, dmin = new(nf), new(2, nf), new(nf) if want_dmin else None
         dchan = new(2, nf) if want_d else None
         fn = B.dfrg_integrate_lpa_host if host else B.dfrg_integrate_lpa
         fn(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["N"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
-           rule("q"), up(c["rho"]), up(c["u"]), up(c["du"]), flow, chan, dmin, dchan=dchan)
+           rule("q"), up(c["rho"]), up(c["u"]), up(c["du"]), flow, chan, dmin, dchan=dchan, **dress)
         res = dict(out=flow, chan=chan, dmin=dmin, dchan=dchan)
     elif kd == "twopoint":
         out = new(c["pext"].size, c["m2"].size)
@@ -97,7 +103,7 @@ def gpu_run(c, R, host=False, want_dmin=True, want_d=False):
         fn = B.dfrg_integrate_loop4d_host if host else B.dfrg_integrate_loop4d
         fn(B.LOOP_TWOPOINT, c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], rule("q"), rule("c"), None, None,
            (up(c["Z"]),), c["lnq_lo"], c["lnq_hi"], c["interp"], up(c["coef"]), up(c["m2"]), up(c["pext"]), out, dmin,
-           dout_dm2=dout)
+           dout_dm2=dout, **dress)
         res = dict(out=out, dmin=dmin, dout=dout)
     elif kd == "threepoint":
         ne = c["ext"].shape[0]
@@ -105,7 +111,7 @@ def gpu_run(c, R, host=False, want_dmin=True, want_d=False):
         fn = B.dfrg_integrate_loop4d_host if host else B.dfrg_integrate_loop4d
         fn(B.LOOP_THREEPOINT, c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], rule("q"), rule("c1"),
            rule("c2"), rule("phi"), (up(c["ZA"]), up(c["Zc"]), up(c["L3"])), c["lnq_lo"], c["lnq_hi"], c["interp"],
-           up(c["coef"]), None, up(c["ext"]), out, dmin, ext_outer=c.get("ext_outer", 0))
+           up(c["coef"]), None, up(c["ext"]), out, dmin, ext_outer=c.get("ext_outer", 0), **dress)
         res = dict(out=out, dmin=dmin)
     else:
         shape = (c["pext"].size, c["n_jext"], c["m2psi"].size)
@@ -114,7 +120,7 @@ def gpu_run(c, R, host=False, want_dmin=True, want_d=False):
         fn = B.dfrg_integrate_matsubara3d_host if host else B.dfrg_integrate_matsubara3d
         fn(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], rule("q"), rule("c"),
            up(c["Zpsi"]), up(c["Zphi"]), c["lnq_lo"], c["lnq_hi"], c["interp"], up(c["coef"]), up(c["m2psi"]),
-           up(c["m2phi"]), up(c["pext"]), c["n_jext"], out, dmin, dout_dm2_psi=dpsi, dout_dm2_phi=dphi)
+           up(c["m2phi"]), up(c["pext"]), c["n_jext"], out, dmin, dout_dm2_psi=dpsi, dout_dm2_phi=dphi, **dress)
         res = dict(out=out, dmin=dmin, dpsi=dpsi, dphi=dphi)
     if not host:
         torch.cuda.synchronize()

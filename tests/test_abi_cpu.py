@@ -83,7 +83,7 @@ def test_quad_nodes_validation(lib):
 def test_integrators_validate_before_touching_the_device(lib):
     # fake non-null pointers: validation must reject these calls without dereferencing anything
     p = 0x1000
-    reg = B.Regulator(B.REG_EXP_POLY, 1, 1.0)
+    reg = B.Regulator(B.REG_EXP_POLY, 1, 1.0, 1.0, 0.0)
     rule = B.Rule(p, p, 8)
     D = B.LpaDesc(4, 0.0, 0, 1, 4.0, 1.0, reg, rule)
     f = lib.dfrg_integrate_lpa
@@ -92,9 +92,11 @@ def test_integrators_validate_before_touching_the_device(lib):
     assert f(C.byref(D), 4, None, p, p, p, None, None, None) == B.DFRG_EINVAL
     bad = B.LpaDesc(4, -1.0, 0, 1, 4.0, 1.0, reg, rule)
     assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
-    bad = B.LpaDesc(4, 0.0, 0, 1, 4.0, 1.0, B.Regulator(1, 1, 0.0), rule)
+    bad = B.LpaDesc(4, 0.0, 0, 1, 4.0, 1.0, B.Regulator(1, 1, 0.0, 1.0, 0.0), rule)
     assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
-    bad = B.LpaDesc(4, 0.0, 0, 1, 4.0, 1.0, B.Regulator(7, 1, 1.0), rule)
+    bad = B.LpaDesc(4, 0.0, 0, 1, 4.0, 1.0, B.Regulator(7, 1, 1.0, 1.0, 0.0), rule)
+    assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
+    bad = B.LpaDesc(4, 0.0, 0, 1, 4.0, 1.0, B.Regulator(1, 1, 1.0), rule)            # zk = 0 (zero-initialised): rejected
     assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
     bad = B.LpaDesc(9, 0.0, 0, 1, 4.0, 1.0, reg, rule)
     assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EUNSUPPORTED
