@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     lpa,
     loop4d_twopoint,
     loop4d_threepoint,
+    loop4d_fourpoint,
     matsubara3d,
     lpa_dm2,
     loop4d_twopoint_dm2,

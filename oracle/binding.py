@@ -59,6 +59,12 @@ def _load():
                                                _dp, _dp, _dp, C.c_int, C.c_double, C.c_double, C.c_int,
                                                _dp, C.c_int, C.c_int, _dp,
                                                C.c_longlong, _lp, C.c_int, _dp, _dp, _dp]
+        _lib.orc_loop4d_fourpoint.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                              C.c_int, _dp, _dp, C.c_int, _dp, _dp,
+                                              C.c_int, _dp, _dp, C.c_int, _dp, _dp,
+                                              _dp, _dp, _dp, C.c_int, C.c_double, C.c_double, C.c_int,
+                                              _dp, C.c_int, C.c_int, _dp,
+                                              C.c_longlong, _lp, _dp, _dp, _dp]
         _lib.orc_matsubara3d.argtypes = [C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                          C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                          _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
@@ -170,6 +176,29 @@ def loop4d_threepoint(prefactor, reg_kind, reg_order, k, xq, wq, x1, w1, x2, w2,
                                        ns, selp, int(bool(literal_phi)), _d(out), _d(dmin), _d(sens))
     if rc:
         raise ValueError("orc_loop4d_threepoint: bad arguments")
+    return (out, dmin, sens) if want_sens else (out, dmin)
+
+
+def loop4d_fourpoint(prefactor, reg_kind, reg_order, k, xq, wq, x1, w1, x2, w2, xphi, wphi,
+                     ZA, Zc, L3, lnq_lo, lnq_hi, interp, coef, ext, sel=None, want_sens=False, zk=1.0, eta=0.0):
+    """ext: [n_ext, 6] = (|p1|, |p2|, |p3|, alpha, beta, gamma); coef: 70 = [gluon box | ghost box].
+    Returns (out[n_ext or n_sel], dmin)."""
+    xq, wq, x1, w1, x2, w2, xphi, wphi, ZA, Zc, L3, coef, ext = map(
+        _arr, (xq, wq, x1, w1, x2, w2, xphi, wphi, ZA, Zc, L3, coef, ext))
+    n_ext = ext.size // 6
+    ns, selp, _keep = _sel(sel)
+    n_out = ns if sel is not None else n_ext
+    out = np.empty(n_out)
+    dmin = np.empty(n_out)
+    sens = np.empty(n_out)
+    rc = _load().orc_loop4d_fourpoint(float(prefactor), int(reg_kind), int(reg_order), float(k), float(zk), float(eta),
+                                      int(xq.size), _d(xq), _d(wq), int(x1.size), _d(x1), _d(w1),
+                                      int(x2.size), _d(x2), _d(w2), int(xphi.size), _d(xphi), _d(wphi),
+                                      _d(ZA), _d(Zc), _d(L3), int(ZA.size), float(lnq_lo), float(lnq_hi),
+                                      int(interp), _d(coef), int(coef.size), int(n_ext), _d(ext),
+                                      ns, selp, _d(out), _d(dmin), _d(sens))
+    if rc:
+        raise ValueError("orc_loop4d_fourpoint: bad arguments")
     return (out, dmin, sens) if want_sens else (out, dmin)
 
 

@@ -431,6 +431,128 @@ int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double 
   return 0;
 }
 
+// ---- 4-D vacuum four-point box loop: genuine three-angle kinematics + ghost loop ----
+// "Angles -> 3": cos1, cos2, phi; four-gluon vertex configurations.  Reading A21.
+// ext = (|p1|, |p2|, |p3|, alpha, beta, gamma)[e]:
+//   p1 = |p1| (1, 0, 0, 0),  p2 = |p2| (cos al, sin al, 0, 0),  p3 = |p3| (cos be, sin be cos ga, sin be sin ga, 0),
+//   q  = q (c1, s1 c2, s1 s2 cos phi, s1 s2 sin phi),  s1 = sqrt(1-c1^2), s2 = sqrt(1-c2^2)
+//   u1 = q.p1 = q|p1| c1,  u2 = q.p2 = q|p2| (cos al c1 + sin al s1 c2),
+//   u3 = q.p3 = q|p3| (cos be c1 + sin be cos ga s1 c2 + sin be sin ga s1 s2 cos phi)
+// Box routing: internal lines q, q+p1, q+p1+p2, q+p1+p2+p3:
+//   s12 = |p1+p2|^2,  s123 = |p1+p2+p3|^2 (= p4^2),
+//   s_a = q^2 + p1^2 + 2 u1,  s_b = q^2 + s12 + 2 (u1 + u2),  s_d = q^2 + s123 + 2 (u1 + u2 + u3)
+// Gluon box: four three-gluon vertices, each dressed at the mean squared momentum of its legs,
+//   l1 = (q^2 + p1^2 + s_a)/3, l2 = (s_a + p2^2 + s_b)/3, l3 = (s_b + p3^2 + s_d)/3, l4 = (s_d + s123 + q^2)/3
+//   T_A = G_A(q^2) G_A(s_a) G_A(s_b) G_A(s_d) l3(l1) l3(l2) l3(l3) l3(l4) P_A,   G_A(s) = 1/(Z_A(s) s + R(s))
+// Ghost box (undressed ghost-gluon vertices):
+//   T_c = G_c(q^2) G_c(s_a) G_c(s_b) G_c(s_d) P_c,                                 G_c(s) = 1/(Z_c(s) s + R(s))
+// P_X = sum_{a+b+c+d<=3} kap^X_abcd (q^2/k^2)^a (u1/k^2)^b (u2/k^2)^c (u3/k^2)^d, a outermost, then b, c, d, ascending
+//   (35 coefficients each; coef = [kap^A | kap^c], n_coef = 70).
+// out[e] = C sum_q w q^3 Rdot(q^2) sum_c1 w sqrt(1-c1^2) sum_c2 w sum_phi w (T_A + T_c)
+int orc_loop4d_fourpoint(double prefactor, int reg_kind, int reg_order, double k, double zk, double eta,
+                         int nq, const double* xq, const double* wq,
+                         int n1, const double* x1, const double* w1,
+                         int n2, const double* x2, const double* w2,
+                         int nphi, const double* xphi, const double* wphi,
+                         const double* ZA, const double* Zc, const double* L3,
+                         int t_nq, double t_lo, double t_hi, int t_interp,
+                         const double* coef, int n_coef,
+                         int n_ext, const double* ext,
+                         long long n_sel, const long long* sel,
+                         double* out, double* dmin, double* sens) {
+  if (n_coef != 70 || nq < 1 || n1 < 1 || n2 < 1 || nphi < 1 || n_ext < 1 || k <= 0) return -1;
+  const double k2 = k * k;
+  const long long n_out = sel ? n_sel : (long long)n_ext;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (long long o = 0; o < n_out; ++o) {
+    const long long e = sel ? sel[o] : o;
+    const double p1 = ext[6 * e], p2 = ext[6 * e + 1], p3 = ext[6 * e + 2];
+    const double al = ext[6 * e + 3], be = ext[6 * e + 4], ga = ext[6 * e + 5];
+    const double ca = std::cos(al), sa = std::sin(al), cb = std::cos(be), sb = std::sin(be);
+    const double cg = std::cos(ga), sg = std::sin(ga);
+    const double p1p2 = p1 * p2 * ca, p1p3 = p1 * p3 * cb, p2p3 = p2 * p3 * (ca * cb + sa * sb * cg);
+    const double s12 = clamp0(p1 * p1 + p2 * p2 + 2.0 * p1p2);
+    const double s123 = clamp0(p1 * p1 + p2 * p2 + p3 * p3 + 2.0 * (p1p2 + p1p3 + p2p3));
+    double dm = kInf;
+    acc_t acc_q = 0.0L, sn_q = 0.0L;
+    for (int i = 0; i < nq; ++i) {
+      const double q = xq[i];
+      const double sq = q * q;
+      double Rq, Rdq;
+      regulator(reg_kind, reg_order, k, zk, eta, sq, &Rq, &Rdq);
+      const double DqA = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, sq) * sq + Rq;
+      const double Dqc = table_lookup(Zc, t_nq, t_lo, t_hi, t_interp, sq) * sq + Rq;
+      if (DqA / k2 < dm) dm = DqA / k2;
+      if (Dqc / k2 < dm) dm = Dqc / k2;
+      acc_t acc_1 = 0.0L, sn_1 = 0.0L;
+      for (int j1 = 0; j1 < n1; ++j1) {
+        const double c1 = x1[j1];
+        const double sin1 = std::sqrt((1.0 - c1) * (1.0 + c1));
+        acc_t acc_2 = 0.0L, sn_2 = 0.0L;
+        for (int j2 = 0; j2 < n2; ++j2) {
+          const double c2 = x2[j2];
+          const double sin2 = std::sqrt((1.0 - c2) * (1.0 + c2));
+          acc_t acc_phi = 0.0L, sn_phi = 0.0L;
+          for (int jp = 0; jp < nphi; ++jp) {
+            const double cphi = std::cos(xphi[jp]);
+            const double u1 = q * p1 * c1;
+            const double u2 = q * p2 * (ca * c1 + sa * sin1 * c2);
+            const double u3 = q * p3 * (cb * c1 + sb * cg * sin1 * c2 + sb * sg * sin1 * sin2 * cphi);
+            const double s_a = clamp0(sq + p1 * p1 + 2.0 * u1);
+            const double s_b = clamp0(sq + s12 + 2.0 * (u1 + u2));
+            const double s_d = clamp0(sq + s123 + 2.0 * (u1 + u2 + u3));
+            double Ra, Rb, Rd, dummy;
+            regulator(reg_kind, reg_order, k, zk, eta, s_a, &Ra, &dummy);
+            regulator(reg_kind, reg_order, k, zk, eta, s_b, &Rb, &dummy);
+            regulator(reg_kind, reg_order, k, zk, eta, s_d, &Rd, &dummy);
+            const double DaA = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, s_a) * s_a + Ra;
+            const double DbA = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, s_b) * s_b + Rb;
+            const double DdA = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, s_d) * s_d + Rd;
+            const double Dac = table_lookup(Zc, t_nq, t_lo, t_hi, t_interp, s_a) * s_a + Ra;
+            const double Dbc = table_lookup(Zc, t_nq, t_lo, t_hi, t_interp, s_b) * s_b + Rb;
+            const double Ddc = table_lookup(Zc, t_nq, t_lo, t_hi, t_interp, s_d) * s_d + Rd;
+            const double Dall[6] = {DaA, DbA, DdA, Dac, Dbc, Ddc};
+            for (int t = 0; t < 6; ++t)
+              if (Dall[t] / k2 < dm) dm = Dall[t] / k2;
+            const double lam =
+                table_lookup(L3, t_nq, t_lo, t_hi, t_interp, (sq + p1 * p1 + s_a) / 3.0) *
+                table_lookup(L3, t_nq, t_lo, t_hi, t_interp, (s_a + p2 * p2 + s_b) / 3.0) *
+                table_lookup(L3, t_nq, t_lo, t_hi, t_interp, (s_b + p3 * p3 + s_d) / 3.0) *
+                table_lookup(L3, t_nq, t_lo, t_hi, t_interp, (s_d + s123 + sq) / 3.0);
+            double PA = 0.0, PAabs = 0.0, Pc = 0.0, Pcabs = 0.0;
+            int idx = 0;
+            for (int a = 0; a <= 3; ++a)
+              for (int b = 0; a + b <= 3; ++b)
+                for (int c = 0; a + b + c <= 3; ++c)
+                  for (int d = 0; a + b + c + d <= 3; ++d) {
+                    const double mono = ipow(sq / k2, a) * ipow(u1 / k2, b) * ipow(u2 / k2, c) * ipow(u3 / k2, d);
+                    PA += coef[idx] * mono;
+                    PAabs += std::fabs(coef[idx] * mono);
+                    Pc += coef[35 + idx] * mono;
+                    Pcabs += std::fabs(coef[35 + idx] * mono);
+                    ++idx;
+                  }
+            const double gA = (1.0 / DqA) * (1.0 / DaA) * (1.0 / DbA) * (1.0 / DdA) * lam;
+            const double gc = (1.0 / Dqc) * (1.0 / Dac) * (1.0 / Dbc) * (1.0 / Ddc);
+            acc_phi += (acc_t)(wphi[jp] * (gA * PA + gc * Pc));
+            sn_phi += (acc_t)(wphi[jp] * (std::fabs(gA) * PAabs + std::fabs(gc) * Pcabs));
+          }
+          acc_2 += (acc_t)w2[j2] * acc_phi;
+          sn_2 += (acc_t)w2[j2] * sn_phi;
+        }
+        acc_1 += (acc_t)(w1[j1] * sin1) * acc_2;
+        sn_1 += (acc_t)(w1[j1] * sin1) * sn_2;
+      }
+      acc_q += (acc_t)(wq[i] * q * q * q * Rdq) * acc_1;
+      sn_q += (acc_t)std::fabs(wq[i] * q * q * q * Rdq) * sn_1;
+    }
+    out[o] = (double)((acc_t)prefactor * acc_q);
+    if (dmin) dmin[o] = dm;
+    if (sens) sens[o] = (double)((acc_t)std::fabs(prefactor) * sn_q);
+  }
+  return 0;
+}
+
 // ---- 3-D spatial + Matsubara loop (config 4) -----------------------------------------
 // nu_n = (2n+1) pi T (fermionic, loop n = -n_max..n_max, external j = 0..n_jext-1),
 // boson line (nu_j - nu_n, p - q): m = j - n, om_m = 2 pi m T, r^2 = p^2 + q^2 - 2 p q c.

@@ -135,6 +135,32 @@ def config3(n_p=32, n_alpha=8, n_q=96, n_c1=32, n_c2=16, n_phi=16, n_tab=128, k=
                 coef=coef, ext=ext.reshape(-1, 3), ext_outer=n_p)  # product grid: |p1| outermost
 
 
+def config5(n_s=16, n_ang=8, n_q=96, n_c1=32, n_c2=16, n_phi=16, n_tab=128, k=1.0, seed=11, interp=3):
+    """Four-point box loop in 4D at T=0 with genuine three-angle kinematics and a ghost loop (SURVEY 8(f) item 3,
+    DESIGN.md reading A21; not a BASELINE.json config).  Quadrature and tables as config 3; externals: n_s scales S
+    log-spaced in [1e-2, 1e2] k with (|p1|, |p2|, |p3|) = (S, 0.7 S, 1.3 S), times n_ang seeded angle triples
+    (alpha, beta, gamma) in (0.1 pi, 0.9 pi)."""
+    qt, lo, hi = table_grid(n_tab, k)
+    U = splitmix64_uniform(seed, 15 + 70 + 3 * n_ang)
+    ZA = _rational(qt, k, 0.5 + U[0:5])
+    Zc = _rational(qt, k, 0.5 + U[5:10])
+    L3 = _rational(qt, k, 0.5 + U[10:15])
+    coef = 2.0 * U[15:85] - 1.0
+    ang = math.pi * (0.1 + 0.8 * U[85:85 + 3 * n_ang].reshape(n_ang, 3))
+    S = logspace(1e-2 * k, 1e2 * k, n_s)
+    ext = np.empty((n_s, n_ang, 6))
+    ext[..., 0] = S[:, None]
+    ext[..., 1] = 0.7 * S[:, None]
+    ext[..., 2] = 1.3 * S[:, None]
+    ext[..., 3:6] = ang[None, :, :]
+    return dict(name="cfg5_fourpoint", family=2, prefactor=1.0 / (2.0 * math.pi) ** 4,
+                reg_kind=REG_EXP_POLY, reg_order=1, k=k,
+                rule_q=(n_q, 0.0, 8.0 * k), rule_c1=(n_c1, -1.0, 1.0), rule_c2=(n_c2, -1.0, 1.0),
+                rule_phi=(n_phi, 0.0, 2.0 * math.pi),
+                ZA=ZA, Zc=Zc, L3=L3, lnq_lo=lo, lnq_hi=hi, interp=interp,
+                coef=coef, ext=ext.reshape(-1, 6))
+
+
 def config4(n_field=512, n_p=64, n_jext=16, n_q=96, n_c=24, n_tab=128, n_freq=64,
             T_over_k=0.15, cut=10.0, k=1.0, seed=4, interp=3):
     """Finite-T momentum-dependent loop, quark-meson-like (BASELINE.json configs[4])."""
