@@ -195,6 +195,19 @@ def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
                    "nominal_evals_per_s": uniq * rr["phi"][0].numel() / ms * 1e3,
                    "integrals_per_s": o3.numel() / ms * 1e3,
                    "launches": 4}   # product-grid path: pre-pass, main, fix-up, and the general kernel returning at once
+    # cfg5 (four-point box, genuine three-angle kinematics + ghost loop; SURVEY 8(f) item 3 -- not a BASELINE config)
+    c = inputs.config5()
+    R = make_rules(c, B.dfrg_quad_nodes)
+    rr = {k_: (up(v[0]), up(v[1])) for k_, v in R.items()}
+    tabs = (up(c["ZA"]), up(c["Zc"]), up(c["L3"]))
+    coef, ext = up(c["coef"]), up(c["ext"])
+    o5 = torch.empty(ext.shape[0], dtype=torch.float64, device="cuda")
+    ms = timeit(lambda: B.dfrg_integrate_loop4d(B.LOOP_FOURPOINT, c["prefactor"], c["reg_kind"], c["reg_order"],
+                                                c["k"], rr["q"], rr["c1"], rr["c2"], rr["phi"], tabs, c["lnq_lo"],
+                                                c["lnq_hi"], c["interp"], coef, None, ext, o5), n=3)
+    ev = o5.numel() * rr["q"][0].numel() * rr["c1"][0].numel() * rr["c2"][0].numel() * rr["phi"][0].numel()
+    out["cfg5_fourpoint"] = {"ms": ms, "evals_per_s": ev / ms * 1e3, "integrals_per_s": o5.numel() / ms * 1e3,
+                             "launches": 2}
     # cfg4 with both mass derivatives (three passes of the moment kernel: value, d/dm2_psi, d/dm2_phi)
     c = inputs.config4()
     R = make_rules(c, B.dfrg_quad_nodes)

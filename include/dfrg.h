@@ -144,9 +144,23 @@ int dfrg_integrate_lpa_host(const dfrg_lpa_desc* D, int n_field, const double* r
  *   P = sum_{a+b+c<=4} coef[idx(a,b,c)] (q^2/k^2)^a (q.p1/k^2)^b (q.p2/k^2)^c,  idx: a outermost, then b, then c, ascending
  *   out[e] = prefactor sum_q w q^3 Rdot(q^2) G_A(q^2) sum_c1 w sqrt(1-c1^2) sum_c2 w sum_phi w  G_A(s_a) G_A(s_b) Lam P
  *   (the integrand is phi-independent: the phi axis contributes sum_phi w; Z_c is accepted and not used.)
+ * DFRG_LOOP_FOURPOINT (tab = Z_A, Z_c, lambda3 sharing one grid, n_coef = 70, axes q, cos1, cos2, phi; n_field = 0): a box
+ *   with genuine three-angle kinematics ("Angles" -> 3: cos1, cos2, phi; four-gluon vertex configurations,
+ *   PAPER.md:334) plus a ghost box; every node of the (q, c1, c2, phi) grid is a distinct evaluation.  DESIGN.md reading A21.
+ *   ext = (|p1|, |p2|, |p3|, alpha, beta, gamma)[n_ext]:
+ *     p1 = |p1| (1,0,0,0), p2 = |p2| (cos al, sin al, 0, 0), p3 = |p3| (cos be, sin be cos ga, sin be sin ga, 0)
+ *     q = q (c1, s1 c2, s1 s2 cos phi, s1 s2 sin phi), s_i = sqrt(1 - c_i^2);  u_i = q.p_i
+ *   internal lines q, q+p1, q+p1+p2, q+p1+p2+p3:  s_a = q^2 + p1^2 + 2 u1,  s_b = q^2 + |p1+p2|^2 + 2 (u1+u2),
+ *     s_d = q^2 + |p1+p2+p3|^2 + 2 (u1+u2+u3)   (each clamped at 0)
+ *   T_A = G_A(q^2) G_A(s_a) G_A(s_b) G_A(s_d) l3((q^2+p1^2+s_a)/3) l3((s_a+p2^2+s_b)/3) l3((s_b+p3^2+s_d)/3)
+ *         l3((s_d+|p1+p2+p3|^2+q^2)/3) P_A,        G_X(s) = 1/(Z_X(s) s + R(s))
+ *   T_c = G_c(q^2) G_c(s_a) G_c(s_b) G_c(s_d) P_c
+ *   P_X = sum_{a+b+c+d<=3} coef_X[idx(a,b,c,d)] (q^2/k^2)^a (u1/k^2)^b (u2/k^2)^c (u3/k^2)^d, idx: a outermost, then b, c, d,
+ *         ascending; coef = [coef_A (35) | coef_c (35)]
+ *   out[e] = prefactor sum_q w q^3 Rdot(q^2) sum_c1 w sqrt(1-c1^2) sum_c2 w sum_phi w (T_A + T_c)
  * out, dmin (nullable): [n_ext][max(n_field, 1)].
- * Limits: two-point q.n * cos1.n <= 12288; three-point q.n * cos1.n <= 65536, every tab[i].n_q <= 1024. */
-typedef enum { DFRG_LOOP_TWOPOINT = 0, DFRG_LOOP_THREEPOINT = 1 } dfrg_loop_family;
+ * Limits: four-point cos2.n <= 512, phi.n <= 4096, q.n * cos1.n <= 65536; two-point q.n * cos1.n <= 12288; three-point q.n * cos1.n <= 65536, every tab[i].n_q <= 1024. */
+typedef enum { DFRG_LOOP_TWOPOINT = 0, DFRG_LOOP_THREEPOINT = 1, DFRG_LOOP_FOURPOINT = 2 } dfrg_loop_family;
 typedef struct {
   int family;
   double prefactor;
@@ -162,7 +176,7 @@ typedef struct {
                     path runs and the results are the same.  Ignored (general path) if G > 256 or cos2.n > 512. */
   double* dout_dm2; /* two-point only, nullable output [n_ext][n_field]: d out[e][f] / d m2[f] (the same m2 sits in all
                        three propagators):  prefactor sum_i wq q^3 Rdot [-2 G(q)^3 A_i - G(q)^2 B_i],
-                       A_i = sum_j W'_ij G(s_ij), B_i = sum_j W'_ij G(s_ij)^2.  Must be NULL for the three-point family. */
+                       A_i = sum_j W'_ij G(s_ij), B_i = sum_j W'_ij G(s_ij)^2.  Must be NULL for the three- and four-point families. */
 } dfrg_loop4d_desc;
 
 int dfrg_integrate_loop4d(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext, const double* ext,

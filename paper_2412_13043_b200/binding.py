@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libdfrg.so")
 
 DFRG_OK, DFRG_EINVAL, DFRG_EUNSUPPORTED, DFRG_ECUDA, DFRG_ENOMEM = 0, -1, -2, -3, -4
 REG_LITIM, REG_EXP_POLY = 0, 1
-LOOP_TWOPOINT, LOOP_THREEPOINT = 0, 1
+LOOP_TWOPOINT, LOOP_THREEPOINT, LOOP_FOURPOINT = 0, 1, 2
 RULE_GAUSS_LEGENDRE = 0
 
 EXPORTS = (
@@ -193,10 +193,11 @@ def _n(a):
 def dfrg_integrate_loop4d(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs,
                           lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0, dout_dm2=None, reg_zk=1.0, reg_eta=0.0):
     """two-point: tabs=(Z,), m2=[n_field], ext=[n_ext] -> out [n_ext, n_field];
-    three-point: tabs=(Z_A, Z_c, lambda3), m2=None, ext=[n_ext, 3] -> out [n_ext]; ext_outer: dfrg_loop4d_desc."""
+    three-point: tabs=(Z_A, Z_c, lambda3), m2=None, ext=[n_ext, 3] -> out [n_ext]; ext_outer: dfrg_loop4d_desc;
+    four-point: tabs=(Z_A, Z_c, lambda3), m2=None, ext=[n_ext, 6], coef[70] -> out [n_ext]."""
     D = _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
                      lnq_hi, interp, coef, True, ext_outer, dout_dm2, reg_zk, reg_eta)
-    n_ext = _n(ext) if family == LOOP_TWOPOINT else _n(ext) // 3
+    n_ext = _n(ext) // {LOOP_TWOPOINT: 1, LOOP_THREEPOINT: 3, LOOP_FOURPOINT: 6}[family]
     _check(lib().dfrg_integrate_loop4d(C.byref(D), _n(m2), _ptr(m2, True), n_ext, _ptr(ext, True),
                                        _ptr(out, True), _ptr(dmin, True), _stream()), "dfrg_integrate_loop4d")
     return out
@@ -206,7 +207,7 @@ def dfrg_integrate_loop4d_host(family, prefactor, reg_kind, reg_order, k, rule_q
                                lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0, dout_dm2=None, reg_zk=1.0, reg_eta=0.0):
     D = _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
                      lnq_hi, interp, coef, False, ext_outer, dout_dm2, reg_zk, reg_eta)
-    n_ext = _n(ext) if family == LOOP_TWOPOINT else _n(ext) // 3
+    n_ext = _n(ext) // {LOOP_TWOPOINT: 1, LOOP_THREEPOINT: 3, LOOP_FOURPOINT: 6}[family]
     _check(lib().dfrg_integrate_loop4d_host(C.byref(D), _n(m2), _ptr(m2, False), n_ext, _ptr(ext, False),
                                             _ptr(out, False), _ptr(dmin, False)), "dfrg_integrate_loop4d_host")
     return out

@@ -130,6 +130,12 @@ def test_integrators_validate_before_touching_the_device(lib):
     assert g(C.byref(D3), 3, None, 4, p, p, None, None) == B.DFRG_EINVAL        # three-point has no field axis
     D3.family = 5
     assert g(C.byref(D3), 0, None, 4, p, p, None, None) == B.DFRG_EINVAL
+    D3.family = B.LOOP_FOURPOINT
+    assert g(C.byref(D3), 0, None, 4, p, p, None, None) == B.DFRG_EINVAL        # four-point needs n_coef == 70
+    D3.n_coef = 70
+    big = B.Rule(p, p, 600)
+    D5 = B.Loop4dDesc(B.LOOP_FOURPOINT, 1.0, reg, rule, rule, big, rule, T3(tab, tab, tab), p, 70)
+    assert g(C.byref(D5), 0, None, 4, p, p, None, None) == B.DFRG_EUNSUPPORTED  # cos2 rule longer than a CTA
 
     h = lib.dfrg_integrate_matsubara3d
     stack = B.Table(p, 128, 64, -9.0, 5.0, 3)
