@@ -41,13 +41,14 @@ def cfg4_counts(c, rules):
     nq, nc = rules["q"][0].size, rules["c"][0].size
     evals = n_out * n_terms * nq * nc
     # algorithmic FP64 work of the moment factorisation, per (p, radial node, field point):
-    #   (n_j + n_max) nc x 8   angular moments of the boson line   (DADD, 3 DFMA reciprocal, 4 DFMA)
+    #   (n_j + n_max) nc x 7   angular moments of the boson line   (DADD, 3 DFMA reciprocal, and per symmetric node
+    #                          pair (c, -c) 2 DADD + 4 DFMA: M_b += w c^b (r+ +- r-))
     # + (n_max + 1) x 5        fermion line G_psi^2                (DADD, 3 DFMA, DMUL)
     # + n_j n_terms x 5        acc_j += H (beta' . M)              (DMUL, 3 DFMA, DFMA)
     # flops = DFMA-slot equivalents (2 per instruction); strict = FMA 2, add/mul 1.
     rows = n_j + c["n_max"]
-    per_pif = rows * nc * 8 + (c["n_max"] + 1) * 5 + n_j * n_terms * 5
-    per_pif_strict = rows * nc * 15 + (c["n_max"] + 1) * 8 + n_j * n_terms * 9
+    per_pif = rows * nc * 7 + (c["n_max"] + 1) * 5 + n_j * n_terms * 5
+    per_pif_strict = rows * nc * 12 + (c["n_max"] + 1) * 8 + n_j * n_terms * 9
     units = n_p * nq * n_f
     return n_out, evals, (2.0 * units * per_pif, float(units * per_pif_strict))
 

@@ -51,6 +51,8 @@ struct Mats3dParams {
   int max_slots;     // partial sums per (field tile, p) in part[]
   int grid_main;     // CTAs of the moment kernel (the fix-up kernel re-derives the unit ownership from it)
   double *part;      // [max_slots][n_p][n_jext][n_field]
+  int sym_try;       // host: the cos rule is long enough for the symmetric-pair moment loop (nc % 8 == 0)
+  int* symflag;      // device: 1 if the cos rule is exactly symmetric (x_c = -x_{nc-1-c}, equal weights), set by the pre-pass
   int mode;          // 0: value;  1: d/dm2_psi (G_psi^2 -> -2 G_psi^3);  2: d/dm2_phi (G_phi -> -G_phi^2, kernels with SQ)
 };
 
@@ -63,6 +65,16 @@ __global__ void __launch_bounds__(M3_PRE_THREADS) mats3d_phi_rows_kernel(const M
   const FastMath fm = fm_build(fmmem, P.fmc);
   cells_build(cells, P.Zphi + (size_t)m * P.grid.n, P.grid);
   __syncthreads();
+  // Symmetric cos rule (Gauss-Legendre on [-1,1] is: x_c = -x_{nc-1-c}, equal weights)?  Then the moment path stores
+  // each row as (node c, node nc-1-c) pairs, and the moment loop works on r+ + r-, r+ - r- (see mats3d_moment_kernel).
+  int sym = 0;
+  if (P.sym_try && P.phi_layout == 1) {
+    int ok = 1;
+    for (int c = threadIdx.x; c < P.nc / 2; c += M3_PRE_THREADS)
+      if (P.xc[c] != -P.xc[P.nc - 1 - c] || P.wc[c] != P.wc[P.nc - 1 - c]) ok = 0;
+    sym = __syncthreads_and(ok);
+  }
+  if (m == 0 && e == 0 && threadIdx.x == 0 && P.symflag) *P.symflag = sym;
   const double p = P.pext[e];
   const double om = 2.0 * 3.14159265358979323846 * (double)m * P.T;
   const int npairs = P.nq * P.nc;
@@ -79,7 +91,7 @@ __global__ void __launch_bounds__(M3_PRE_THREADS) mats3d_phi_rows_kernel(const M
     regulator(P.reg, fm, sphi, R, Rd);
     const double D0 = table_lookup(cells, P.grid, fm, r2) * sphi + R;
     if (P.phi_layout == 0) dst[t] = D0;
-    else dst1[(size_t)i * P.chunk_stride + jc] = D0;
+    else dst1[(size_t)i * P.chunk_stride + (sym ? (2 * jc < P.nc ? 2 * jc : 2 * (P.nc - 1 - jc) + 1) : jc)] = D0;
     dmin = fmin(dmin, D0);
   }
   if (P.phi_layout == 0) {
@@ -446,6 +458,31 @@ __device__ __forceinline__ void mats3d_moment_accumulate(const double4* __restri
     }
 }
 
+// Symmetric cos rule: the batch holds two (x-, x+) pairs, x- = -x+, equal weights, so with s = r+ + r-, d = r+ - r-
+//   M_0 += w s,  M_1 += w x+ d,  M_2 += w x+^2 s,  M_3 += w x+^3 d :  6 FP64 instructions per pair and field point instead
+// of 8, and one weight vector per pair instead of per node.  w4[p] = (w, w x+, w x+^2, w x+^3) of the pair's positive node.
+template <int MF>
+__device__ __forceinline__ void mats3d_moment_accumulate_sym(const double4* __restrict__ w4,
+                                                             const double (&r)[M3_NBAT][MF], double (&M)[4][MF]) {
+  double4 w[M3_NBAT / 2];
+#pragma unroll
+  for (int p = 0; p < M3_NBAT / 2; ++p) w[p] = w4[p];
+  double sm[M3_NBAT / 2][MF], df[M3_NBAT / 2][MF];
+#pragma unroll
+  for (int p = 0; p < M3_NBAT / 2; ++p)
+#pragma unroll
+    for (int k = 0; k < MF; ++k) { sm[p][k] = r[2 * p + 1][k] + r[2 * p][k]; df[p][k] = r[2 * p + 1][k] - r[2 * p][k]; }
+#pragma unroll
+  for (int p = 0; p < M3_NBAT / 2; ++p)
+#pragma unroll
+    for (int k = 0; k < MF; ++k) {
+      M[0][k] = fma(w[p].x, sm[p][k], M[0][k]);
+      M[1][k] = fma(w[p].y, df[p][k], M[1][k]);
+      M[2][k] = fma(w[p].z, sm[p][k], M[2][k]);
+      M[3][k] = fma(w[p].w, df[p][k], M[3][k]);
+    }
+}
+
 // The (j, n) pairs with |j - n| = m of the moment kernel:  acc[j] += H[nbar(n)] (beta'[j][n] . M),  in groups of
 // four (two j x two signs), written stage by stage so that each stage is a set of independent instructions.
 template <int m, int NMAX, int NJ, int MF>
@@ -507,8 +544,10 @@ __device__ __forceinline__ void mats3d_pairs(const double4* __restrict__ bet4, c
   }
 }
 
-template <int NMAX, int NJ, int MF, int NTC, bool SQ>
+template <int NMAX, int NJ, int MF, int NTC, bool SQ, bool SYM>
 __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParams P) {
+  // two instantiations are enqueued when the symmetric-pair loop is possible; the pre-pass decided which one works
+  if (P.sym_try && (*P.symflag != 0) != SYM) return;
   constexpr int NT = 2 * NMAX + 1, NROWS = NJ + NMAX, NB = NJ * NT * 4, NPS = NMAX + 1;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t full[2];
@@ -537,8 +576,9 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
   }
   if (tid < 20) skap[tid] = P.coef[tid];
   for (int i = tid; i < nq; i += NTC) sxq[i] = P.xq[i];
-  for (int c = tid; c < nc; c += NTC) {
-    const double x = P.xc[c], w = P.wc[c];
+  for (int c = tid; c < (SYM ? nc / 2 : nc); c += NTC) {
+    const int cn = SYM ? nc - 1 - c : c;   // SYM: pair c = (node c, node nc-1-c), weights of the positive node
+    const double x = P.xc[cn], w = P.wc[cn];
     numbuf[4 * c] = w; numbuf[4 * c + 1] = w * x; numbuf[4 * c + 2] = w * x * x; numbuf[4 * c + 3] = w * x * x * x;
   }
   __syncthreads();
@@ -648,11 +688,13 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
         for (int c = 0; c < nc; c += 2 * M3_NBAT) {
           const int L = m * nc + c;
           mats3d_recip_batch<MF, SQ>(d0 + L + M3_NBAT, m2phi, rb);
-          mats3d_moment_accumulate<MF>(num4 + c, ra, M);
+          if constexpr (SYM) mats3d_moment_accumulate_sym<MF>(num4 + c / 2, ra, M);
+          else mats3d_moment_accumulate<MF>(num4 + c, ra, M);
           int Ln = L + 2 * M3_NBAT;
           Ln = Ln < l_last ? Ln : l_last;   // past the end of the chunk: recompute the last batch (result unused)
           mats3d_recip_batch<MF, SQ>(d0 + Ln, m2phi, ra);
-          mats3d_moment_accumulate<MF>(num4 + c + M3_NBAT, rb, M);
+          if constexpr (SYM) mats3d_moment_accumulate_sym<MF>(num4 + (c + M3_NBAT) / 2, rb, M);
+          else mats3d_moment_accumulate<MF>(num4 + c + M3_NBAT, rb, M);
         }
       } else {
         const double* drow = d0 + m * nc;
@@ -767,13 +809,13 @@ struct MomentPlan {
   size_t smem;
 };
 
-template <int NMAX, int NJ>
+template <int NMAX, int NJ, bool SYM>
 static int mats3d_moment_go(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream) {
   cudaError_t e;
 #define DFRG_M3_GO(MF, NTC)                                                                                          \
   {                                                                                                                  \
-    auto kern = P.mode == 2 ? mats3d_moment_kernel<NMAX, NJ, MF, NTC, true>                                          \
-                            : mats3d_moment_kernel<NMAX, NJ, MF, NTC, false>;                                        \
+    auto kern = P.mode == 2 ? mats3d_moment_kernel<NMAX, NJ, MF, NTC, true, SYM>                                     \
+                            : mats3d_moment_kernel<NMAX, NJ, MF, NTC, false, SYM>;                                   \
     e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);                       \
     if (e != cudaSuccess) return check_cuda(e);                                                                      \
     kern<<<pl.grid, NTC, pl.smem, stream>>>(P);                                                                      \
@@ -799,7 +841,15 @@ static bool mats3d_moment_shape(int n_max, int n_jext) {
   return false;
 }
 static int mats3d_moment_dispatch(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream) {
-#define X(a, b) if (P.n_max == a && P.n_jext == b) return mats3d_moment_go<a, b>(P, pl, stream);
+  // symmetric-pair instantiation first (runs iff the pre-pass found the cos rule symmetric), then the plain one
+#define X(a, b)                                                                    \
+  if (P.n_max == a && P.n_jext == b) {                                             \
+    if (P.sym_try) {                                                               \
+      const int rc = mats3d_moment_go<a, b, true>(P, pl, stream);                  \
+      if (rc != DFRG_OK) return rc;                                                \
+    }                                                                              \
+    return mats3d_moment_go<a, b, false>(P, pl, stream);                           \
+  }
   DFRG_M3_SHAPES(X)
 #undef X
   return DFRG_EUNSUPPORTED;
@@ -822,7 +872,7 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   P.xq = D->q.x; P.wq = D->q.w; P.xc = D->cos1.x; P.wc = D->cos1.w;
   P.Zpsi = D->tab_psi.v; P.Zphi = D->tab_phi.v; P.coef = D->coef;
   P.m2psi = m2_psi; P.m2phi = m2_phi; P.pext = p; P.out = out; P.dmin = dmin;
-  P.part = nullptr; P.tile_fields = 0; P.max_slots = 0; P.grid_main = 0; P.mode = 0;
+  P.part = nullptr; P.tile_fields = 0; P.max_slots = 0; P.grid_main = 0; P.mode = 0; P.sym_try = 0; P.symflag = nullptr;
 
   // ---- path: moment factorisation where an instantiation exists (DFRG_M3_PATH=generic forces the other one) ----
   const char* vpath = getenv("DFRG_M3_PATH");
@@ -845,6 +895,10 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
     if (pl.smem > 220 * 1024) moment = false;
   }
   P.phi_layout = moment ? 1 : 0;
+  {
+    const char* vs = getenv("DFRG_M3_SYM");
+    P.sym_try = (moment && (P.nc % (2 * M3_NBAT)) == 0 && !(vs && vs[0] == '0')) ? 1 : 0;
+  }
   P.tile_fields = pl.tile; P.max_slots = pl.max_slots; P.grid_main = pl.grid;
 
   const int n_terms = 2 * D->n_max + 1;
@@ -854,13 +908,14 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   const size_t n_psimin = ((size_t)n_terms + 1) & ~(size_t)1;
   const size_t n_part = moment ? (size_t)pl.max_slots * n_p * n_jext * n_field : 0;
   void* scratch = nullptr;
-  int rc = scratch_alloc(&scratch, (n_d0 + n_rowmin + n_psi + n_psimin + n_part) * sizeof(double), stream);
+  int rc = scratch_alloc(&scratch, (n_d0 + n_rowmin + n_psi + n_psimin + n_part + 2) * sizeof(double), stream);
   if (rc != DFRG_OK) return rc;
   P.d0phi = (double*)scratch;
   P.psi = (double2*)(P.d0phi + n_d0);
   P.rowmin = (double*)(P.psi) + n_psi;
   P.psimin = P.rowmin + n_rowmin;
   P.part = P.psimin + n_psimin;
+  P.symflag = (int*)(P.part + n_part);
 
   mats3d_phi_rows_kernel<<<dim3(P.n_rows, n_p), M3_PRE_THREADS, 0, stream>>>(P);
   rc = check_cuda(cudaGetLastError());

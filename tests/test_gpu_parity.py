@@ -202,6 +202,32 @@ def test_matsubara_moment_path_small(n_field, n_p, n_jext, n_q, n_c, n_max, inte
         del os.environ["DFRG_M3_MF"]
 
 
+@pytest.mark.parametrize("n_field,n_p,n_jext,n_q,n_c,n_max", [(700, 2, 3, 10, 8, 3), (1030, 3, 2, 7, 16, 11),
+                                                              (130, 2, 2, 9, 24, 2)])
+def test_matsubara_symmetric_pair_moments(n_field, n_p, n_jext, n_q, n_c, n_max):
+    # cos rules of 8 k nodes take the symmetric-pair moment loop (pairs (c, nc-1-c): r+ + r-, r+ - r-); the same inputs
+    # through the plain loop (DFRG_M3_SYM=0), and a rule that is NOT symmetric (Gauss-Legendre on [-1, 0.5]), which the
+    # device-side check must send to the plain loop
+    c = inputs.config4(n_field=n_field, n_p=n_p, n_jext=n_jext, n_q=n_q, n_c=n_c)
+    c["n_max"] = n_max
+    what = "mats_sym_%d_%d_%d_%d_%d_%d" % (n_field, n_p, n_jext, n_q, n_c, n_max)
+    g, o, _ = run_both(c, what=what)
+    os.environ["DFRG_M3_SYM"] = "0"
+    try:
+        g2, _, _ = run_both(c, what=what + "_plain")
+    finally:
+        del os.environ["DFRG_M3_SYM"]
+    assert not np.array_equal(g["out"], g2["out"])                       # two different loops ran
+    c["rule_c"] = (n_c, -1.0, 0.5)
+    g3, _, _ = run_both(c, what=what + "_asymmetric_rule")
+    os.environ["DFRG_M3_SYM"] = "0"
+    try:
+        g4, _, _ = run_both(c, what=what + "_asymmetric_rule_plain")
+    finally:
+        del os.environ["DFRG_M3_SYM"]
+    assert np.array_equal(g3["out"], g4["out"])                          # the fallback is the plain loop, bit for bit
+
+
 def test_matsubara_full_config4_sampled():
     c = inputs.config4()
     n_out = 64 * 16 * 512
