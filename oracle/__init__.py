@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     regulator,
     table_lookup,
     lpa,
+    lpa_fermion,
     loop4d_twopoint,
     loop4d_threepoint,
     loop4d_fourpoint,

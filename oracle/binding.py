@@ -59,6 +59,9 @@ def _load():
                                                _dp, _dp, _dp, C.c_int, C.c_double, C.c_double, C.c_int,
                                                _dp, C.c_int, C.c_int, _dp,
                                                C.c_longlong, _lp, C.c_int, _dp, _dp, _dp]
+        _lib.orc_lpa_fermion.argtypes = [C.c_int, C.c_double, C.c_int, C.c_double, C.c_double,
+                                         C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                         C.c_int, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp]
         _lib.orc_loop4d_fourpoint.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                               C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                               C.c_int, _dp, _dp, C.c_int, _dp, _dp,
@@ -136,6 +139,19 @@ def lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, xq, wq, rh
     if rc:
         raise ValueError("orc_lpa: bad arguments")
     return (flow, chan, dmin, sens) if want_sens else (flow, chan, dmin)
+
+
+def lpa_fermion(d, T, n_max, mu, prefactor, reg_kind, reg_order, k, xq, wq, m2, zk=1.0, eta=0.0):
+    """Fermionic LPA loop at chemical potential mu (spatial regulator).  Returns (I, dI, dmin, sens, sens_d), each [m2.size]."""
+    xq, wq, m2 = map(_arr, (xq, wq, m2))
+    I, dI, dmin, sens, sens_d = (np.empty(m2.shape) for _ in range(5))
+    rc = _load().orc_lpa_fermion(int(d), float(T), int(n_max), float(mu), float(prefactor),
+                                 int(reg_kind), int(reg_order), float(k), float(zk), float(eta),
+                                 int(xq.size), _d(xq), _d(wq), int(m2.size), _d(m2),
+                                 _d(I), _d(dI), _d(dmin), _d(sens), _d(sens_d))
+    if rc:
+        raise ValueError("orc_lpa_fermion: bad arguments")
+    return I, dI, dmin, sens, sens_d
 
 
 def loop4d_twopoint(prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Z, lnq_lo, lnq_hi, interp,

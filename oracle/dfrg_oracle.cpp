@@ -271,6 +271,59 @@ int orc_lpa(int d, double T, int n_max, int reg_arg4d, double N, double prefacto
   return 0;
 }
 
+// ---- fermionic LPA loop at finite temperature and chemical potential -------------
+// Fermionic Matsubara frequencies nu_n = (2n+1) pi T shifted by the chemical potential, p0 -> nu_n + i mu
+// (external fermion legs carry p0f - i mu_q; "T" and "muq"), spatial ("3D")
+// regulator R(q^2) as in the paper's finite-density example.  Reading A22:
+//   I_F(m2) = C T sum_{n=-n_max-1..n_max} sum_i w_i q_i^(d-1) Rdot(q_i^2) Re[ 1 / ((nu_n + i mu)^2 + q_i^2 + R(q_i^2) + m2) ]
+// (the sum over n = -n_max-1 .. n_max is symmetric under nu -> -nu, which makes it real; the real part is written out:
+//  D = a + i b, a = nu^2 - mu^2 + q^2 + R + m2, b = 2 nu mu, Re 1/D = a/(a^2+b^2)).
+//   dI[j] = d I_F / d m2 = -C T sum sum w q^(d-1) Rdot Re[1/D^2],  Re 1/D^2 = (a^2 - b^2)/(a^2+b^2)^2
+//   dmin[j] = min over nodes of |D| / k^2;   sens, sens_d: sum |term| (1 + (|D - m2| + |m2|)/|D| per power of 1/D)
+int orc_lpa_fermion(int d, double T, int n_max, double mu, double prefactor,
+                    int reg_kind, int reg_order, double k, double zk, double eta,
+                    int nq, const double* xq, const double* wq,
+                    int n_m2, const double* m2v,
+                    double* I, double* dI, double* dmin, double* sens, double* sens_d) {
+  if (d < 1 || nq < 1 || n_m2 < 0 || !(T > 0) || n_max < 0 || k <= 0) return -1;
+  const double pi = 3.14159265358979323846;
+  const double k2 = k * k;
+#pragma omp parallel for schedule(static)
+  for (int j = 0; j < n_m2; ++j) {
+    const double m2 = m2v[j];
+    acc_t acc = 0.0L, accd = 0.0L, sn = 0.0L, snd = 0.0L;
+    double dm = kInf;
+    for (int n = -n_max - 1; n <= n_max; ++n) {
+      const double nu = (2.0 * (double)n + 1.0) * pi * T;
+      for (int i = 0; i < nq; ++i) {
+        const double q = xq[i];
+        double R, Rd;
+        regulator(reg_kind, reg_order, k, zk, eta, q * q, &R, &Rd);
+        const double a0 = nu * nu - mu * mu + q * q + R;      // Re(D - m2)
+        const double a = a0 + m2, b = 2.0 * nu * mu;
+        const double den = a * a + b * b;                      // |D|^2
+        const double absD = std::sqrt(den);
+        if (absD / k2 < dm) dm = absD / k2;
+        const double w = wq[i] * ipow(q, d - 1) * Rd;
+        const double term = w * (a / den);
+        const double termd = w * ((a * a - b * b) / (den * den));
+        const double cond = (std::sqrt(a0 * a0 + b * b) + std::fabs(m2)) / absD;
+        acc += (acc_t)term;
+        accd += (acc_t)termd;
+        sn += (acc_t)(std::fabs(w) / absD * (1.0 + cond));
+        snd += (acc_t)(std::fabs(w) / den * (1.0 + 2.0 * cond));
+      }
+    }
+    const acc_t sc = (acc_t)prefactor * (acc_t)T;
+    I[j] = (double)(sc * acc);
+    if (dI) dI[j] = (double)(-sc * accd);
+    if (dmin) dmin[j] = dm;
+    if (sens) sens[j] = (double)(fabsl(sc) * sn);
+    if (sens_d) sens_d[j] = (double)(fabsl(sc) * snd);
+  }
+  return 0;
+}
+
 // ---- 4-D vacuum two-point loop (config 2) --------------------------------------------
 // out[e][f] = C sum_i wq_i q_i^3 Rdot(q_i^2) G(q_i^2;f)^2
 //               sum_j wc_j sqrt(1-c_j^2) (coef0 + coef1 q_i p_e c_j / k^2) G(s_ij;f),
