@@ -114,7 +114,23 @@ typedef struct {
  * flow [n_field]; chan nullable [2][n_field] = I_pi, I_sigma; dmin nullable [n_field].
  * dchan (in the descriptor, nullable) [2][n_field] = dI/dm2 at m2 = u and at m2 = u + 2 rho du, from which
  *   dflow/du = (N-1) dchan[0] + dchan[1],  dflow/d(du) = 2 rho dchan[1].
- * Limits: (n_max + 1) * q.n <= 12288. */
+ * Limits: (n_max + 1) * q.n <= 12288.
+ * Fermionic statistics at chemical potential mu (statistics = DFRG_STAT_FERMION; requires T > 0 and reg_arg4d = 0,
+ * the spatial "3D" regulators of the paper's finite-density example; the time component of a fermion
+ * momentum is nu_n + i mu, PAPER.md:1947-1952 -- the paper writes p0f - i mu_q, the real part below is even in mu;
+ * DESIGN.md reading A22):  nu_n = (2n+1) pi T,
+ *   I(m2) = prefactor T sum_{n=-n_max-1..n_max} sum_i w_i q_i^(d-1) Rdot(q_i^2) Re[ 1/((nu_n + i mu)^2 + q_i^2 + R(q_i^2) + m2) ]
+ * in the same combination flow = (N-1) I(u) + I(u + 2 rho du) (a single quark loop: N = 1, du = 0; signs and
+ * degeneracies go into prefactor); dchan = dI/dm2 = -prefactor T sum sum w q^(d-1) Rdot Re[1/(...)^2];
+ * dmin = min over nodes and both channels of |denominator| / k^2.  Limit: (n_max + 1) * q.n <= 6144. */
+typedef enum { DFRG_STAT_BOSON = 0, DFRG_STAT_FERMION = 1 } dfrg_statistics;
+/* Number of Matsubara terms on either side for a cut-off in the time direction:
+ *   DFRG_DOMAIN_X0 ("Quadraturex0": the domain scales with k):   n_max = ceil(extent * k / (2 pi T)),  extent in units of k
+ *   DFRG_DOMAIN_Q0 ("Quadratureq0": fixed, bounded domain):       n_max = ceil(extent / (2 pi T)),      extent in units of T's
+ * Host function.  Returns n_max >= 0, or DFRG_EINVAL (T <= 0, k <= 0, extent < 0, unknown domain, n_max beyond 2^30). */
+typedef enum { DFRG_DOMAIN_X0 = 0, DFRG_DOMAIN_Q0 = 1 } dfrg_time_domain;
+int dfrg_matsubara_n_max(int domain, double T, double k, double extent);
+
 typedef struct {
   int d;
   double T;
@@ -125,6 +141,8 @@ typedef struct {
   dfrg_regulator reg;
   dfrg_rule q;
   double* dchan; /* nullable output [2][n_field] */
+  int statistics; /* DFRG_STAT_BOSON (0): the sums above.  DFRG_STAT_FERMION (1): see below */
+  double mu;      /* chemical potential (fermionic statistics only; must be 0 otherwise) */
 } dfrg_lpa_desc;
 
 int dfrg_integrate_lpa(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u, const double* du,

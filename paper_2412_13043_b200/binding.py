@@ -14,11 +14,14 @@ LIB_PATH = os.path.join(_HERE, "libdfrg.so")
 
 DFRG_OK, DFRG_EINVAL, DFRG_EUNSUPPORTED, DFRG_ECUDA, DFRG_ENOMEM = 0, -1, -2, -3, -4
 REG_LITIM, REG_EXP_POLY = 0, 1
+STAT_BOSON, STAT_FERMION = 0, 1
+DOMAIN_X0, DOMAIN_Q0 = 0, 1
 LOOP_TWOPOINT, LOOP_THREEPOINT, LOOP_FOURPOINT = 0, 1, 2
 RULE_GAUSS_LEGENDRE = 0
 
 EXPORTS = (
     "dfrg_strerror", "dfrg_last_cuda_error", "dfrg_version", "dfrg_shutdown", "dfrg_quad_nodes",
+    "dfrg_matsubara_n_max",
     "dfrg_integrate_lpa", "dfrg_integrate_lpa_host",
     "dfrg_integrate_loop4d", "dfrg_integrate_loop4d_host",
     "dfrg_integrate_matsubara3d", "dfrg_integrate_matsubara3d_host",
@@ -43,7 +46,8 @@ class Table(C.Structure):
 
 class LpaDesc(C.Structure):
     _fields_ = [("d", C.c_int), ("T", C.c_double), ("n_max", C.c_int), ("reg_arg4d", C.c_int), ("N", C.c_double),
-                ("prefactor", C.c_double), ("reg", Regulator), ("q", Rule), ("dchan", _vp)]
+                ("prefactor", C.c_double), ("reg", Regulator), ("q", Rule), ("dchan", _vp),
+                ("statistics", C.c_int), ("mu", C.c_double)]
 
 
 class Loop4dDesc(C.Structure):
@@ -82,6 +86,7 @@ def lib():
         L.dfrg_strerror.restype = C.c_char_p
         L.dfrg_strerror.argtypes = [C.c_int]
         L.dfrg_shutdown.restype = None
+        L.dfrg_matsubara_n_max.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double]
         L.dfrg_quad_nodes.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, _vp, _vp]
         L.dfrg_integrate_lpa.argtypes = [C.POINTER(LpaDesc), C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
         L.dfrg_integrate_lpa_host.argtypes = [C.POINTER(LpaDesc), C.c_int, _vp, _vp, _vp, _vp, _vp, _vp]
@@ -149,16 +154,26 @@ def dfrg_quad_nodes(n, a, b, rule_kind=RULE_GAUSS_LEGENDRE):
     return x, w
 
 
+def dfrg_matsubara_n_max(domain, T, k, extent):
+    """Number of Matsubara terms on either side for a time-direction cut-off (Quadraturex0 / Quadratureq0)."""
+    n = lib().dfrg_matsubara_n_max(int(domain), float(T), float(k), float(extent))
+    if n < 0:
+        raise DfrgError(n, "dfrg_matsubara_n_max")
+    return n
+
+
 # ---- LPA ------------------------------------------------------------------------------------------
-def _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, device, dchan=None, reg_zk=1.0, reg_eta=0.0):
+def _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, device, dchan=None, reg_zk=1.0, reg_eta=0.0,
+              statistics=STAT_BOSON, mu=0.0):
     return LpaDesc(int(d), float(T), int(n_max), int(reg_arg4d), float(N), float(prefactor),
-                   Regulator(int(reg_kind), int(reg_order), float(k), float(reg_zk), float(reg_eta)), _rule(rule_q, device), _ptr(dchan, device))
+                   Regulator(int(reg_kind), int(reg_order), float(k), float(reg_zk), float(reg_eta)), _rule(rule_q, device),
+                   _ptr(dchan, device), int(statistics), float(mu))
 
 
 def dfrg_integrate_lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, rho, u, du,
-                       flow, chan=None, dmin=None, dchan=None, reg_zk=1.0, reg_eta=0.0):
+                       flow, chan=None, dmin=None, dchan=None, reg_zk=1.0, reg_eta=0.0, statistics=STAT_BOSON, mu=0.0):
     """dchan (optional, [2, n_field]): dI/dm2 per channel (include/dfrg.h, "Mass derivatives")."""
-    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, True, dchan, reg_zk, reg_eta)
+    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, True, dchan, reg_zk, reg_eta, statistics, mu)
     _check(lib().dfrg_integrate_lpa(C.byref(D), int(rho.numel()), _ptr(rho, True), _ptr(u, True), _ptr(du, True),
                                     _ptr(flow, True), _ptr(chan, True), _ptr(dmin, True), _stream()),
            "dfrg_integrate_lpa")
@@ -166,8 +181,8 @@ def dfrg_integrate_lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order
 
 
 def dfrg_integrate_lpa_host(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, rho, u, du,
-                            flow, chan=None, dmin=None, dchan=None, reg_zk=1.0, reg_eta=0.0):
-    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, False, dchan, reg_zk, reg_eta)
+                            flow, chan=None, dmin=None, dchan=None, reg_zk=1.0, reg_eta=0.0, statistics=STAT_BOSON, mu=0.0):
+    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, False, dchan, reg_zk, reg_eta, statistics, mu)
     n_field = rho.numel() if hasattr(rho, "numel") else rho.size
     _check(lib().dfrg_integrate_lpa_host(C.byref(D), int(n_field), _ptr(rho, False), _ptr(u, False),
                                          _ptr(du, False), _ptr(flow, False), _ptr(chan, False), _ptr(dmin, False)),

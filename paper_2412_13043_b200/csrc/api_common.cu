@@ -162,6 +162,15 @@ void dfrg_shutdown(void) { thread_arena().release(); scratch_shutdown(); }
 
 // S1: Gauss-Legendre nodes.  Half the roots from the Tricomi initial guess, Newton on P_n with the
 // three-term recurrence in long double, mirrored; derivative from P_n' = n (P_{n-1} - x P_n)/(1 - x^2).
+int dfrg_matsubara_n_max(int domain, double T, double k, double extent) {
+  if (!(T > 0.0) || !(k > 0.0) || !(extent >= 0.0) || !isfinite(extent)) return DFRG_EINVAL;
+  if (domain != DFRG_DOMAIN_X0 && domain != DFRG_DOMAIN_Q0) return DFRG_EINVAL;
+  const double cut = domain == DFRG_DOMAIN_X0 ? extent * k : extent;
+  const double n = ceil(cut / (2.0 * 3.14159265358979323846 * T));
+  if (!(n <= 1073741824.0)) return DFRG_EINVAL;
+  return (int)n;
+}
+
 int dfrg_quad_nodes(int rule_kind, int n, double a, double b, double* x_host, double* w_host) {
   if (rule_kind != DFRG_RULE_GAUSS_LEGENDRE || n < 1 || n > 4096 || !x_host || !w_host) return DFRG_EINVAL;
   if (!(b > a) || !isfinite(a) || !isfinite(b)) return DFRG_EINVAL;

@@ -21,7 +21,7 @@ constexpr int LPA_MAX_PAIRS = 12288;
 
 struct LpaParams {
   int d, n_max, reg_arg4d, nq, n_field;
-  double T, N, prefactor;
+  double T, N, prefactor, mu;
   RegParams reg;
   FastMathConsts fmc;
   const double *xq, *wq, *rho, *u, *du;
@@ -134,18 +134,106 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_kernel(const LpaParams P) {
   }
 }
 
+// ---- fermionic statistics at chemical potential mu (dfrg_lpa_desc::statistics == 1; include/dfrg.h) ----
+// nu_n = (2n+1) pi T, p0 = nu_n + i mu, spatial regulator:  D = a + i b,  a = nu^2 - mu^2 + q^2 + R(q^2) + m2,  b = 2 nu mu,
+//   I_F(m2) = C T sum_{n=-n_max-1..n_max} sum_i w q^(d-1) Rdot(q^2) Re(1/D),   Re 1/D = a/(a^2+b^2),  Re 1/D^2 = (a^2-b^2)/(a^2+b^2)^2.
+// The terms are even in nu, so n and -n-1 are folded (weight 2).  Same mapping as lpa_kernel; the field-independent
+// table holds (a - m2, W, b^2) per (n >= 0, radial node).  dmin = min over nodes of |D|/k^2, tracked in the hot loop.
+template <bool WANT_D>
+__global__ void __launch_bounds__(LPA_THREADS) lpa_fermion_kernel(const LpaParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t bar;
+  __shared__ double part[2][LPA_SLICES][LPA_FTILE];
+  __shared__ double dpart[2][LPA_SLICES][LPA_FTILE];
+  __shared__ double mpart[2][LPA_SLICES][LPA_FTILE];
+
+  const int n_pairs = (P.n_max + 1) * P.nq;
+  double4* tab = reinterpret_cast<double4*>(smem_raw);                      // [n_pairs] (a0, W, b^2, -)
+  double* sx = reinterpret_cast<double*>(smem_raw + (size_t)n_pairs * 32);  // [nq]
+  double* sw = sx + ((P.nq + 1) & ~1);
+  const FastMath fm = fm_build(sw + ((P.nq + 1) & ~1), P.fmc);
+
+  if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
+  __syncthreads();
+  StageList L;
+  L.add(sx, P.xq, P.nq);
+  L.add(sw, P.wq, P.nq);
+  stage_to_smem(L, &bar, 0);
+
+  const double pi_T = 3.14159265358979323846 * P.T;
+  for (int t = threadIdx.x; t < n_pairs; t += LPA_THREADS) {
+    const int n = t / P.nq, i = t - n * P.nq;
+    const double q = sx[i];
+    const double nu = (2.0 * (double)n + 1.0) * pi_T;
+    double R, Rd;
+    regulator(P.reg, fm, q * q, R, Rd);
+    const double b = 2.0 * nu * P.mu;
+    tab[t] = make_double4(nu * nu - P.mu * P.mu + q * q + R, 2.0 * (sw[i] * ipow(q, P.d - 1) * Rd), b * b, 0.0);
+  }
+  __syncthreads();
+
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int ch = wid & 1, slice = wid >> 1;
+  const int f = blockIdx.x * LPA_FTILE + lane;
+  const bool live = f < P.n_field;
+  double m2 = 1.0;
+  if (live) m2 = ch ? P.u[f] + 2.0 * P.rho[f] * P.du[f] : P.u[f];
+  const bool want_dmin = P.dmin != nullptr;
+  double acc = 0.0, accd = 0.0, den_min = __longlong_as_double(0x7ff0000000000000LL);
+#pragma unroll 4
+  for (int t = slice; t < n_pairs; t += LPA_SLICES) {
+    const double4 e = tab[t];
+    const double a = e.x + m2;
+    const double den = fma(a, a, e.z);
+    const double r = fast_rcp(den);
+    const double wr = e.y * r;
+    acc = fma(wr, a, acc);
+    if constexpr (WANT_D) accd = fma(wr * r, fma(a, a, -e.z), accd);
+    if (want_dmin) den_min = fmin(den_min, den);
+  }
+  part[ch][slice][lane] = acc;
+  dpart[ch][slice][lane] = accd;
+  mpart[ch][slice][lane] = den_min;
+  __syncthreads();
+  if (wid == 0 && live) {
+    const double scale = P.prefactor * P.T;
+    double I[2];
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+      I[c] = scale * ((part[c][0][lane] + part[c][1][lane]) + (part[c][2][lane] + part[c][3][lane]));
+    P.flow[f] = (P.N - 1.0) * I[0] + I[1];
+    if (P.chan) { P.chan[f] = I[0]; P.chan[P.n_field + f] = I[1]; }
+    if (want_dmin) {
+      double dm = mpart[0][0][lane];
+#pragma unroll
+      for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int sl = 0; sl < LPA_SLICES; ++sl) dm = fmin(dm, mpart[c][sl][lane]);
+      P.dmin[f] = sqrt(dm) * P.reg.inv_k2;
+    }
+    if constexpr (WANT_D) {
+#pragma unroll
+      for (int c = 0; c < 2; ++c)
+        P.dchan[c * P.n_field + f] =
+            -scale * ((dpart[c][0][lane] + dpart[c][1][lane]) + (dpart[c][2][lane] + dpart[c][3][lane]));
+    }
+  }
+}
+
 static int lpa_launch(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u, const double* du,
                       double* flow, double* chan, double* dmin, cudaStream_t stream) {
   LpaParams P;
   P.d = D->d; P.n_max = D->n_max; P.reg_arg4d = D->reg_arg4d; P.nq = D->q.n; P.n_field = n_field;
-  P.T = D->T; P.N = D->N; P.prefactor = D->prefactor;
+  P.T = D->T; P.N = D->N; P.prefactor = D->prefactor; P.mu = D->mu;
   P.reg = reg_params(D->reg.kind, D->reg.order, D->reg.k, D->reg.zk, D->reg.eta);
   P.fmc = fm_consts();
   P.xq = D->q.x; P.wq = D->q.w; P.rho = rho; P.u = u; P.du = du;
   P.flow = flow; P.chan = chan; P.dmin = dmin; P.dchan = D->dchan;
   const int n_terms = (D->T > 0.0) ? D->n_max + 1 : 1;
-  const size_t smem = (size_t)n_terms * D->q.n * 16 + (2 * (size_t)((D->q.n + 1) & ~1) + FM_DOUBLES) * 8;
-  auto kern = D->dchan ? lpa_kernel<true> : lpa_kernel<false>;
+  const bool fermi = D->statistics == DFRG_STAT_FERMION;
+  const size_t smem = (size_t)n_terms * D->q.n * (fermi ? 32 : 16) + (2 * (size_t)((D->q.n + 1) & ~1) + FM_DOUBLES) * 8;
+  auto kern = fermi ? (D->dchan ? lpa_fermion_kernel<true> : lpa_fermion_kernel<false>)
+                    : (D->dchan ? lpa_kernel<true> : lpa_kernel<false>);
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return check_cuda(e);
   const int grid = (n_field + LPA_FTILE - 1) / LPA_FTILE;
@@ -160,6 +248,14 @@ static int lpa_validate(const dfrg_lpa_desc* D, int n_field, const double* rho, 
   if (!(D->T >= 0.0) || D->n_max < 0 || !(D->N == D->N)) return DFRG_EINVAL;
   if (D->d < 1 || D->d > 8) return DFRG_EUNSUPPORTED;
   const long long n_terms = (D->T > 0.0) ? (long long)D->n_max + 1 : 1;
+  if (D->statistics != DFRG_STAT_BOSON && D->statistics != DFRG_STAT_FERMION) return DFRG_EINVAL;
+  if (D->statistics == DFRG_STAT_FERMION) {
+    // fermionic frequencies need T > 0; with a chemical potential the time component is complex: spatial regulator only
+    if (!(D->T > 0.0) || D->reg_arg4d != 0 || !(D->mu == D->mu)) return DFRG_EINVAL;
+    if (n_terms * D->q.n > LPA_MAX_PAIRS / 2) return DFRG_EUNSUPPORTED;
+  } else if (D->mu != 0.0) {
+    return DFRG_EINVAL;
+  }
   if (n_terms * D->q.n > LPA_MAX_PAIRS) return DFRG_EUNSUPPORTED;
   return DFRG_OK;
 }

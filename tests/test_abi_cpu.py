@@ -98,6 +98,14 @@ def test_integrators_validate_before_touching_the_device(lib):
     assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
     bad = B.LpaDesc(4, 0.0, 0, 1, 4.0, 1.0, B.Regulator(1, 1, 1.0), rule)            # zk = 0 (zero-initialised): rejected
     assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
+    bad = B.LpaDesc(3, 0.1, 4, 1, 4.0, 1.0, reg, rule, None, B.STAT_FERMION, 0.3)    # fermions + mu: spatial regulator only
+    assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
+    bad = B.LpaDesc(3, 0.0, 4, 0, 4.0, 1.0, reg, rule, None, B.STAT_FERMION, 0.3)    # fermionic frequencies need T > 0
+    assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
+    bad = B.LpaDesc(3, 0.1, 4, 0, 4.0, 1.0, reg, rule, None, B.STAT_BOSON, 0.3)      # no chemical potential for bosons
+    assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
+    bad = B.LpaDesc(3, 0.1, 4, 0, 4.0, 1.0, reg, rule, None, 7, 0.0)
+    assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
     bad = B.LpaDesc(9, 0.0, 0, 1, 4.0, 1.0, reg, rule)
     assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EUNSUPPORTED
     bad = B.LpaDesc(3, 0.1, 4000, 1, 4.0, 1.0, reg, rule)
@@ -160,3 +168,21 @@ def test_no_cpu_fallback_without_gpu(lib):
     with pytest.raises(B.DfrgError):
         B.dfrg_integrate_lpa_host(4, 0.0, 0, 1, 4.0, 1.0, B.REG_EXP_POLY, 1, 1.0, (x, w), rho, rho.copy(), rho.copy(), flow)
     assert np.all(np.isnan(flow))
+
+
+def test_matsubara_n_max_domains(lib):
+    """Quadraturex0 (domain scales with k) and Quadratureq0 (fixed domain); BASELINE.json's
+    N_max = ceil(6k/(2 pi T)) = 20, 10, 5, 2 for T/k = 0.05, 0.1, 0.2, 0.5 and ceil(10k/(2 pi T)) = 11 for T = 0.15k."""
+    for T, want in ((0.05, 20), (0.1, 10), (0.2, 5), (0.5, 2)):
+        assert B.dfrg_matsubara_n_max(B.DOMAIN_X0, T, 1.0, 6.0) == want
+        assert B.dfrg_matsubara_n_max(B.DOMAIN_X0, 1.7 * T, 1.7, 6.0) == want      # scales with k
+        assert B.dfrg_matsubara_n_max(B.DOMAIN_Q0, T, 1.0, 6.0) == want
+        assert B.dfrg_matsubara_n_max(B.DOMAIN_Q0, T, 0.01, 6.0) == want            # fixed domain: independent of k
+    assert B.dfrg_matsubara_n_max(B.DOMAIN_X0, 0.15, 1.0, 10.0) == 11
+    assert B.dfrg_matsubara_n_max(B.DOMAIN_Q0, 0.15, 1.0, 0.0) == 0
+    for bad in ((0, 0.0, 1.0, 6.0), (0, 0.1, 0.0, 6.0), (0, 0.1, 1.0, -1.0), (5, 0.1, 1.0, 6.0), (1, 1e-12, 1.0, 1e3)):
+        assert lib.dfrg_matsubara_n_max(*bad) == B.DFRG_EINVAL
+    from paper_2412_13043_b200 import inputs
+    for T in inputs.CONFIG1_TEMPERATURES:
+        assert inputs.config1(T)["n_max"] == B.dfrg_matsubara_n_max(B.DOMAIN_X0, T, 1.0, 6.0)
+    assert inputs.config4()["n_max"] == B.dfrg_matsubara_n_max(B.DOMAIN_X0, 0.15, 1.0, 10.0)
