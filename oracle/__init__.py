@@ -15,6 +15,9 @@ from .binding import (  # noqa: F401
     loop4d_twopoint,
     loop4d_threepoint,
     loop4d_fourpoint,
+    loop4d_threepoint_tab3d,
+    table3d_lookup,
+    vertex_coords,
     matsubara3d,
     lpa_dm2,
     loop4d_twopoint_dm2,

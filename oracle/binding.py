@@ -62,6 +62,18 @@ def _load():
         _lib.orc_lpa_fermion.argtypes = [C.c_int, C.c_double, C.c_int, C.c_double, C.c_double,
                                          C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                          C.c_int, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp]
+        _ip = C.POINTER(C.c_int)
+        _lib.orc_table3d_lookup.restype = C.c_double
+        _lib.orc_table3d_lookup.argtypes = [_dp, _ip, _dp, _dp, _ip, C.c_double, C.c_double, C.c_double]
+        _lib.orc_vertex_coords.restype = None
+        _lib.orc_vertex_coords.argtypes = [C.c_double, C.c_double, C.c_double, _dp, _dp, _dp]
+        _lib.orc_loop4d_threepoint_tab3d.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                                     C.c_int, _dp, _dp, C.c_int, _dp, _dp, C.c_int, _dp, _dp,
+                                                     C.c_int, _dp,
+                                                     _dp, C.c_int, C.c_double, C.c_double, C.c_int,
+                                                     _dp, _ip, _dp, _dp, _ip,
+                                                     _dp, C.c_int, C.c_int, _dp,
+                                                     C.c_longlong, _lp, _dp, _dp, _dp]
         _lib.orc_loop4d_fourpoint.argtypes = [C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                               C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                               C.c_int, _dp, _dp, C.c_int, _dp, _dp,
@@ -192,6 +204,49 @@ def loop4d_threepoint(prefactor, reg_kind, reg_order, k, xq, wq, x1, w1, x2, w2,
                                        ns, selp, int(bool(literal_phi)), _d(out), _d(dmin), _d(sens))
     if rc:
         raise ValueError("orc_loop4d_threepoint: bad arguments")
+    return (out, dmin, sens) if want_sens else (out, dmin)
+
+
+def _tab3d(v3, lo3, hi3, log3):
+    v3 = _arr(v3)
+    assert v3.ndim == 3
+    n3 = np.ascontiguousarray(v3.shape, dtype=np.int32)
+    lo3, hi3 = _arr(lo3), _arr(hi3)
+    log3 = np.ascontiguousarray(log3, dtype=np.int32)
+    ip = lambda a: a.ctypes.data_as(C.POINTER(C.c_int))
+    return v3, n3, lo3, hi3, log3, (_d(v3), ip(n3), _d(lo3), _d(hi3), ip(log3))
+
+
+def table3d_lookup(v3, lo3, hi3, log3, x0, x1, x2):
+    """Trilinear look-up in a 3-D table v3[n0, n1, n2]; logarithmic axes take the squared momentum."""
+    *_keep, args = _tab3d(v3, lo3, hi3, log3)
+    return float(_load().orc_table3d_lookup(*args, float(x0), float(x1), float(x2)))
+
+
+def vertex_coords(k1sq, k2sq, k3sq):
+    """(S0^2, a, s) of a three-point function with squared leg momenta k1sq, k2sq, k3sq."""
+    S, a, s = C.c_double(), C.c_double(), C.c_double()
+    _load().orc_vertex_coords(float(k1sq), float(k2sq), float(k3sq), C.byref(S), C.byref(a), C.byref(s))
+    return S.value, a.value, s.value
+
+
+def loop4d_threepoint_tab3d(prefactor, reg_kind, reg_order, k, xq, wq, x1, w1, x2, w2, wphi, ZA, lnq_lo, lnq_hi, interp,
+                            v3, lo3, hi3, log3, coef, ext, sel=None, want_sens=False, zk=1.0, eta=0.0):
+    """Three-point loop with the vertex dressing from a 3-D table l3(S0^2, a, s).  Returns (out, dmin[, sens])."""
+    xq, wq, x1, w1, x2, w2, wphi, ZA, coef, ext = map(_arr, (xq, wq, x1, w1, x2, w2, wphi, ZA, coef, ext))
+    *_keep, targs = _tab3d(v3, lo3, hi3, log3)
+    n_ext = ext.size // 3
+    ns, selp, _keep2 = _sel(sel)
+    n_out = ns if sel is not None else n_ext
+    out, dmin, sens = np.empty(n_out), np.empty(n_out), np.empty(n_out)
+    rc = _load().orc_loop4d_threepoint_tab3d(float(prefactor), int(reg_kind), int(reg_order), float(k), float(zk),
+                                             float(eta), int(xq.size), _d(xq), _d(wq), int(x1.size), _d(x1), _d(w1),
+                                             int(x2.size), _d(x2), _d(w2), int(wphi.size), _d(wphi),
+                                             _d(ZA), int(ZA.size), float(lnq_lo), float(lnq_hi), int(interp),
+                                             *targs, _d(coef), int(coef.size), int(n_ext), _d(ext),
+                                             ns, selp, _d(out), _d(dmin), _d(sens))
+    if rc:
+        raise ValueError("orc_loop4d_threepoint_tab3d: bad arguments")
     return (out, dmin, sens) if want_sens else (out, dmin)
 
 

@@ -125,6 +125,59 @@ double table_lookup(const double* v, int n, double lo, double hi, int interp, do
   return v[i] * (1.0 - tau) + v[i + 1] * tau;
 }
 
+// ---- 3-D dressing tables, trilinear: PAPER.md:1860-1896 (LinearInterpolator3D with Log x Log x Lin or
+// Log x Lin x Lin coordinates) -------------------------------------------------------------------------
+// v is row-major [n0][n1][n2].  Axis a has n_a >= 2 points on a uniform grid in its coordinate c_a between lo_a and
+// hi_a; c_a = log(x_a)/2 for a logarithmic axis (x_a = SQUARED momentum, as for the 1-D tables) and c_a = x_a for a
+// linear one.  t_a = clamp((c_a - lo_a)/h_a, 0, n_a - 1), cell i_a = min(floor(t_a), n_a - 2), tau_a = t_a - i_a, and
+// the value is the trilinear combination of the 8 corners.  Outside the grid the edge value is returned.
+struct Table3D {
+  const double* v;
+  int n[3];
+  double lo[3], hi[3];
+  int is_log[3];
+};
+double table3d_lookup(const Table3D& tb, double x0, double x1, double x2) {
+  const double x[3] = {x0, x1, x2};
+  int i[3];
+  double tau[3];
+  for (int a = 0; a < 3; ++a) {
+    const double h = (tb.hi[a] - tb.lo[a]) / (double)(tb.n[a] - 1);
+    const double c = tb.is_log[a] ? 0.5 * std::log(x[a]) : x[a];
+    double t = (c - tb.lo[a]) / h;
+    if (!(t > 0.0)) t = 0.0;
+    if (t > (double)(tb.n[a] - 1)) t = (double)(tb.n[a] - 1);
+    i[a] = (int)std::floor(t);
+    if (i[a] > tb.n[a] - 2) i[a] = tb.n[a] - 2;
+    tau[a] = t - (double)i[a];
+  }
+  double val = 0.0;
+  for (int d0 = 0; d0 < 2; ++d0)
+    for (int d1 = 0; d1 < 2; ++d1)
+      for (int d2 = 0; d2 < 2; ++d2) {
+        const double w = (d0 ? tau[0] : 1.0 - tau[0]) * (d1 ? tau[1] : 1.0 - tau[1]) * (d2 ? tau[2] : 1.0 - tau[2]);
+        val += w * tb.v[((size_t)(i[0] + d0) * tb.n[1] + (i[1] + d1)) * tb.n[2] + (i[2] + d2)];
+      }
+  return val;
+}
+
+// Vertex coordinates of a three-point function with squared leg momenta (k1, k2, k3) = (k1^2, k2^2, k3^2): the
+// permutation-group variables used for the paper's 96 x 8 x 7 vertex grids ("average momentum S0 and two angles a, s,
+// in a parametrisation as introduced in [34]"; reading A23):
+//   S0^2 = (k1 + k2 + k3)/6,   a = sqrt(3) (k2 - k1)/(6 S0^2),   s = (k1 + k2 - 2 k3)/(6 S0^2);   S0 = 0: a = s = 0.
+// Momentum conservation confines (a, s) to the unit disc.
+void vertex_coords(double k1, double k2, double k3, double* S0sq, double* a, double* s) {
+  const double six_s0 = k1 + k2 + k3;
+  *S0sq = six_s0 / 6.0;
+  if (six_s0 > 0.0) {
+    *a = std::sqrt(3.0) * (k2 - k1) / six_s0;
+    *s = (k1 + k2 - 2.0 * k3) / six_s0;
+  } else {
+    *a = 0.0;
+    *s = 0.0;
+  }
+}
+
 inline double ipow(double x, int e) {
   double r = 1.0;
   for (int i = 0; i < e; ++i) r *= x;
@@ -482,6 +535,112 @@ int orc_loop4d_threepoint(double prefactor, int reg_kind, int reg_order, double 
     }
   }
   return 0;
+}
+
+// ---- three-point vertex loop with a 3-D vertex dressing table ---------------------
+// As orc_loop4d_threepoint (same kinematics, propagators, polynomial, measure), but every three-gluon vertex is
+// dressed by lambda3(S0, a, s) from a 3-D table at the vertex coordinates of its legs (vertex_coords above):
+//   Lam = l3d(p1^2, q^2, s_a) l3d(p2^2, q^2, s_b) l3d(s_c, s_a, s_b)      (leg order as written)
+// Table axes: 0 = S0^2 (logarithmic or linear), 1 = a, 2 = s.
+int orc_loop4d_threepoint_tab3d(double prefactor, int reg_kind, int reg_order, double k, double zk, double eta,
+                                int nq, const double* xq, const double* wq,
+                                int n1, const double* x1, const double* w1,
+                                int n2, const double* x2, const double* w2,
+                                int nphi, const double* wphi,
+                                const double* ZA, int t_nq, double t_lo, double t_hi, int t_interp,
+                                const double* v3, const int* n3, const double* lo3, const double* hi3, const int* log3,
+                                const double* coef, int n_coef,
+                                int n_ext, const double* ext,
+                                long long n_sel, const long long* sel,
+                                double* out, double* dmin, double* sens) {
+  if (n_coef != 35 || nq < 1 || n1 < 1 || n2 < 1 || nphi < 1 || n_ext < 1 || k <= 0) return -1;
+  Table3D tb;
+  tb.v = v3;
+  for (int a = 0; a < 3; ++a) {
+    tb.n[a] = n3[a]; tb.lo[a] = lo3[a]; tb.hi[a] = hi3[a]; tb.is_log[a] = log3[a];
+    if (n3[a] < 2 || !(hi3[a] > lo3[a])) return -1;
+  }
+  const double k2 = k * k;
+  acc_t sw = 0.0L;
+  for (int jp = 0; jp < nphi; ++jp) sw += (acc_t)wphi[jp];
+  const long long n_out = sel ? n_sel : (long long)n_ext;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (long long o = 0; o < n_out; ++o) {
+    const long long e = sel ? sel[o] : o;
+    const double p1 = ext[3 * e], p2 = ext[3 * e + 1], al = ext[3 * e + 2];
+    const double ca = std::cos(al), sa = std::sin(al);
+    const double sc = clamp0(p1 * p1 + p2 * p2 + 2.0 * p1 * p2 * ca);
+    double dm = kInf;
+    acc_t acc_q = 0.0L, sn_q = 0.0L;
+    for (int i = 0; i < nq; ++i) {
+      const double q = xq[i];
+      const double sq = q * q;
+      double Rq, Rdq;
+      regulator(reg_kind, reg_order, k, zk, eta, sq, &Rq, &Rdq);
+      const double Dq = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, sq) * sq + Rq;
+      if (Dq / k2 < dm) dm = Dq / k2;
+      acc_t acc_1 = 0.0L, sn_1 = 0.0L;
+      for (int j1 = 0; j1 < n1; ++j1) {
+        const double c1 = x1[j1];
+        const double sin1 = std::sqrt((1.0 - c1) * (1.0 + c1));
+        acc_t acc_2 = 0.0L, sn_2 = 0.0L;
+        for (int j2 = 0; j2 < n2; ++j2) {
+          const double c2 = x2[j2];
+          const double qp1 = q * p1 * c1;
+          const double qp2 = q * p2 * (ca * c1 + sa * sin1 * c2);
+          const double s_a = clamp0(sq + p1 * p1 + 2.0 * qp1);
+          const double s_b = clamp0(sq + p2 * p2 - 2.0 * qp2);
+          double Ra, Rb, dummy;
+          regulator(reg_kind, reg_order, k, zk, eta, s_a, &Ra, &dummy);
+          regulator(reg_kind, reg_order, k, zk, eta, s_b, &Rb, &dummy);
+          const double Da = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, s_a) * s_a + Ra;
+          const double Db = table_lookup(ZA, t_nq, t_lo, t_hi, t_interp, s_b) * s_b + Rb;
+          if (Da / k2 < dm) dm = Da / k2;
+          if (Db / k2 < dm) dm = Db / k2;
+          double lam = 1.0;
+          const double legs[3][3] = {{p1 * p1, sq, s_a}, {p2 * p2, sq, s_b}, {sc, s_a, s_b}};
+          for (int v = 0; v < 3; ++v) {
+            double S0sq, a_, s_;
+            vertex_coords(legs[v][0], legs[v][1], legs[v][2], &S0sq, &a_, &s_);
+            lam *= table3d_lookup(tb, S0sq, a_, s_);
+          }
+          double P = 0.0, Pabs = 0.0;
+          int idx = 0;
+          for (int a = 0; a <= 4; ++a)
+            for (int b = 0; a + b <= 4; ++b)
+              for (int c = 0; a + b + c <= 4; ++c) {
+                const double mono = coef[idx++] * ipow(sq / k2, a) * ipow(qp1 / k2, b) * ipow(qp2 / k2, c);
+                P += mono;
+                Pabs += std::fabs(mono);
+              }
+          const double F = (1.0 / Da) * (1.0 / Db) * lam * P;
+          const double Fabs = std::fabs((1.0 / Da) * (1.0 / Db) * lam) * Pabs;
+          acc_2 += (acc_t)w2[j2] * (sw * (acc_t)F);
+          sn_2 += (acc_t)(w2[j2] * Fabs);
+        }
+        acc_1 += (acc_t)(w1[j1] * sin1) * acc_2;
+        sn_1 += (acc_t)(w1[j1] * sin1) * sn_2;
+      }
+      acc_q += (acc_t)(wq[i] * q * q * q * Rdq / Dq) * acc_1;
+      sn_q += (acc_t)std::fabs(wq[i] * q * q * q * Rdq / Dq) * sn_1;
+    }
+    out[o] = (double)((acc_t)prefactor * acc_q);
+    if (dmin) dmin[o] = dm;
+    if (sens) sens[o] = (double)((acc_t)std::fabs(prefactor) * sw * sn_q);
+  }
+  return 0;
+}
+
+double orc_table3d_lookup(const double* v3, const int* n3, const double* lo3, const double* hi3, const int* log3,
+                          double x0, double x1, double x2) {
+  Table3D tb;
+  tb.v = v3;
+  for (int a = 0; a < 3; ++a) { tb.n[a] = n3[a]; tb.lo[a] = lo3[a]; tb.hi[a] = hi3[a]; tb.is_log[a] = log3[a]; }
+  return table3d_lookup(tb, x0, x1, x2);
+}
+
+void orc_vertex_coords(double k1, double k2, double k3, double* S0sq, double* a, double* s) {
+  vertex_coords(k1, k2, k3, S0sq, a, s);
 }
 
 // ---- 4-D vacuum four-point box loop: genuine three-angle kinematics + ghost loop ----
