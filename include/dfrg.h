@@ -176,9 +176,31 @@ int dfrg_integrate_lpa_host(const dfrg_lpa_desc* D, int n_field, const double* r
  *   P_X = sum_{a+b+c+d<=3} coef_X[idx(a,b,c,d)] (q^2/k^2)^a (u1/k^2)^b (u2/k^2)^c (u3/k^2)^d, idx: a outermost, then b, c, d,
  *         ascending; coef = [coef_A (35) | coef_c (35)]
  *   out[e] = prefactor sum_q w q^3 Rdot(q^2) sum_c1 w sqrt(1-c1^2) sum_c2 w sum_phi w (T_A + T_c)
+ * DFRG_LOOP_THREEPOINT_TAB3D (tab[0] = Z_A, tab3d = lambda3(S0^2, a, s); n_coef = 35; n_field = 0): the three-point family
+ *   above with every vertex factor looked up in the 3-D table at the vertex coordinates of its squared leg momenta
+ *   (k1, k2, k3) (the paper's vertex grids "for the average momentum S0 and two angles a, s"; reading A23):
+ *     S0^2 = (k1 + k2 + k3)/6,  a = sqrt(3) (k2 - k1)/(6 S0^2),  s = (k1 + k2 - 2 k3)/(6 S0^2)   (S0 = 0: a = s = 0)
+ *     Lam = l3(p1^2, q^2, s_a) l3(p2^2, q^2, s_b) l3(s_c, s_a, s_b)      table axes: 0 = S0^2, 1 = a, 2 = s
+ *   tab[1], tab[2] and ext_outer are ignored.
  * out, dmin (nullable): [n_ext][max(n_field, 1)].
  * Limits: four-point cos2.n <= 512, phi.n <= 4096, q.n * cos1.n <= 65536; two-point q.n * cos1.n <= 12288; three-point q.n * cos1.n <= 65536, every tab[i].n_q <= 1024. */
-typedef enum { DFRG_LOOP_TWOPOINT = 0, DFRG_LOOP_THREEPOINT = 1, DFRG_LOOP_FOURPOINT = 2 } dfrg_loop_family;
+typedef enum {
+  DFRG_LOOP_TWOPOINT = 0,
+  DFRG_LOOP_THREEPOINT = 1,
+  DFRG_LOOP_FOURPOINT = 2,
+  DFRG_LOOP_THREEPOINT_TAB3D = 3
+} dfrg_loop_family;
+/* Dressing function on a 3-D grid, trilinear (the paper's LinearInterpolator3D with Log x Lin x Lin or Log x Log x Lin
+ * coordinates): v row-major [n[0]][n[1]][n[2]], axis a uniform in its coordinate c_a between lo[a]
+ * and hi[a] with n[a] >= 2 points; c_a = log(x_a)/2 for a logarithmic axis (x_a = SQUARED momentum, as dfrg_table) and
+ * c_a = x_a for a linear one.  t_a = clamp((c_a - lo_a)/h_a, 0, n_a - 1), cell min(floor(t_a), n_a - 2); the value is the
+ * trilinear combination of the 8 corners; outside the grid the edge value.  n[0] n[1] n[2] <= 12288. */
+typedef struct {
+  const double* v;
+  int n[3];
+  double lo[3], hi[3];
+  int is_log[3];
+} dfrg_table3d;
 typedef struct {
   int family;
   double prefactor;
@@ -195,6 +217,7 @@ typedef struct {
   double* dout_dm2; /* two-point only, nullable output [n_ext][n_field]: d out[e][f] / d m2[f] (the same m2 sits in all
                        three propagators):  prefactor sum_i wq q^3 Rdot [-2 G(q)^3 A_i - G(q)^2 B_i],
                        A_i = sum_j W'_ij G(s_ij), B_i = sum_j W'_ij G(s_ij)^2.  Must be NULL for the three- and four-point families. */
+  dfrg_table3d tab3d; /* DFRG_LOOP_THREEPOINT_TAB3D only */
 } dfrg_loop4d_desc;
 
 int dfrg_integrate_loop4d(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext, const double* ext,

@@ -16,7 +16,7 @@ DFRG_OK, DFRG_EINVAL, DFRG_EUNSUPPORTED, DFRG_ECUDA, DFRG_ENOMEM = 0, -1, -2, -3
 REG_LITIM, REG_EXP_POLY = 0, 1
 STAT_BOSON, STAT_FERMION = 0, 1
 DOMAIN_X0, DOMAIN_Q0 = 0, 1
-LOOP_TWOPOINT, LOOP_THREEPOINT, LOOP_FOURPOINT = 0, 1, 2
+LOOP_TWOPOINT, LOOP_THREEPOINT, LOOP_FOURPOINT, LOOP_THREEPOINT_TAB3D = 0, 1, 2, 3
 RULE_GAUSS_LEGENDRE = 0
 
 EXPORTS = (
@@ -44,6 +44,10 @@ class Table(C.Structure):
                 ("interp", C.c_int)]
 
 
+class Table3D(C.Structure):
+    _fields_ = [("v", _vp), ("n", C.c_int * 3), ("lo", C.c_double * 3), ("hi", C.c_double * 3), ("is_log", C.c_int * 3)]
+
+
 class LpaDesc(C.Structure):
     _fields_ = [("d", C.c_int), ("T", C.c_double), ("n_max", C.c_int), ("reg_arg4d", C.c_int), ("N", C.c_double),
                 ("prefactor", C.c_double), ("reg", Regulator), ("q", Rule), ("dchan", _vp),
@@ -54,7 +58,7 @@ class Loop4dDesc(C.Structure):
     _fields_ = [("family", C.c_int), ("prefactor", C.c_double), ("reg", Regulator),
                 ("q", Rule), ("cos1", Rule), ("cos2", Rule), ("phi", Rule),
                 ("tab", Table * 3), ("coef", _vp), ("n_coef", C.c_int), ("ext_outer", C.c_int),
-                ("dout_dm2", _vp)]
+                ("dout_dm2", _vp), ("tab3d", Table3D)]
 
 
 class Mats3dDesc(C.Structure):
@@ -192,13 +196,19 @@ def dfrg_integrate_lpa_host(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_
 
 # ---- loop4d ---------------------------------------------------------------------------------------
 def _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
-                 lnq_hi, interp, coef, device, ext_outer=0, dout_dm2=None, reg_zk=1.0, reg_eta=0.0):
+                 lnq_hi, interp, coef, device, ext_outer=0, dout_dm2=None, reg_zk=1.0, reg_eta=0.0, tab3d=None):
     T3 = Table * 3
+    if tab3d is None:
+        t3d = Table3D(None, (C.c_int * 3)(), (C.c_double * 3)(), (C.c_double * 3)(), (C.c_int * 3)())
+    else:
+        v3, lo3, hi3, log3 = tab3d
+        t3d = Table3D(_ptr(v3, device), (C.c_int * 3)(*[int(x) for x in v3.shape]), (C.c_double * 3)(*map(float, lo3)),
+                      (C.c_double * 3)(*map(float, hi3)), (C.c_int * 3)(*map(int, log3)))
     tt = [_table(t, lnq_lo, lnq_hi, interp, device) for t in tabs] + [_table(None, 0, 0, 0, device)] * (3 - len(tabs))
     n_coef = coef.numel() if hasattr(coef, "numel") else coef.size
     return Loop4dDesc(int(family), float(prefactor), Regulator(int(reg_kind), int(reg_order), float(k), float(reg_zk), float(reg_eta)),
                       _rule(rule_q, device), _rule(rule_c1, device), _rule(rule_c2, device), _rule(rule_phi, device),
-                      T3(*tt), _ptr(coef, device), int(n_coef), int(ext_outer), _ptr(dout_dm2, device))
+                      T3(*tt), _ptr(coef, device), int(n_coef), int(ext_outer), _ptr(dout_dm2, device), t3d)
 
 
 def _n(a):
@@ -206,23 +216,24 @@ def _n(a):
 
 
 def dfrg_integrate_loop4d(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs,
-                          lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0, dout_dm2=None, reg_zk=1.0, reg_eta=0.0):
+                          lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0, dout_dm2=None, reg_zk=1.0, reg_eta=0.0, tab3d=None):
     """two-point: tabs=(Z,), m2=[n_field], ext=[n_ext] -> out [n_ext, n_field];
     three-point: tabs=(Z_A, Z_c, lambda3), m2=None, ext=[n_ext, 3] -> out [n_ext]; ext_outer: dfrg_loop4d_desc;
-    four-point: tabs=(Z_A, Z_c, lambda3), m2=None, ext=[n_ext, 6], coef[70] -> out [n_ext]."""
+    four-point: tabs=(Z_A, Z_c, lambda3), m2=None, ext=[n_ext, 6], coef[70] -> out [n_ext];
+    three-point with a 3-D vertex table: tabs=(Z_A,), tab3d=(v3[n0,n1,n2], lo3, hi3, is_log3), ext=[n_ext, 3]."""
     D = _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
-                     lnq_hi, interp, coef, True, ext_outer, dout_dm2, reg_zk, reg_eta)
-    n_ext = _n(ext) // {LOOP_TWOPOINT: 1, LOOP_THREEPOINT: 3, LOOP_FOURPOINT: 6}[family]
+                     lnq_hi, interp, coef, True, ext_outer, dout_dm2, reg_zk, reg_eta, tab3d)
+    n_ext = _n(ext) // {LOOP_TWOPOINT: 1, LOOP_THREEPOINT: 3, LOOP_FOURPOINT: 6, LOOP_THREEPOINT_TAB3D: 3}[family]
     _check(lib().dfrg_integrate_loop4d(C.byref(D), _n(m2), _ptr(m2, True), n_ext, _ptr(ext, True),
                                        _ptr(out, True), _ptr(dmin, True), _stream()), "dfrg_integrate_loop4d")
     return out
 
 
 def dfrg_integrate_loop4d_host(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs,
-                               lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0, dout_dm2=None, reg_zk=1.0, reg_eta=0.0):
+                               lnq_lo, lnq_hi, interp, coef, m2, ext, out, dmin=None, ext_outer=0, dout_dm2=None, reg_zk=1.0, reg_eta=0.0, tab3d=None):
     D = _loop4d_desc(family, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, rule_c2, rule_phi, tabs, lnq_lo,
-                     lnq_hi, interp, coef, False, ext_outer, dout_dm2, reg_zk, reg_eta)
-    n_ext = _n(ext) // {LOOP_TWOPOINT: 1, LOOP_THREEPOINT: 3, LOOP_FOURPOINT: 6}[family]
+                     lnq_hi, interp, coef, False, ext_outer, dout_dm2, reg_zk, reg_eta, tab3d)
+    n_ext = _n(ext) // {LOOP_TWOPOINT: 1, LOOP_THREEPOINT: 3, LOOP_FOURPOINT: 6, LOOP_THREEPOINT_TAB3D: 3}[family]
     _check(lib().dfrg_integrate_loop4d_host(C.byref(D), _n(m2), _ptr(m2, False), n_ext, _ptr(ext, False),
                                             _ptr(out, False), _ptr(dmin, False)), "dfrg_integrate_loop4d_host")
     return out

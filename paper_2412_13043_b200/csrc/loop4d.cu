@@ -821,6 +821,196 @@ __global__ void __launch_bounds__(256) t3g_fixup_kernel(const ThreeGridParams Q)
 }
 
 // =====================================================================================================
+// three-point with a 3-D vertex dressing table (include/dfrg.h, DFRG_LOOP_THREEPOINT_TAB3D)
+// =====================================================================================================
+// The kinematics, propagators, polynomial and mapping of the general three-point kernel (thread = (q, c1) pairs, c2 loop
+// inside, persistent CTAs over the external configurations); every vertex factor is a trilinear look-up in
+// lambda3(S0^2, a, s) (the paper's 96 x 8 x 7 vertex grids): the whole table sits in
+// shared memory (43 KB for 96 x 8 x 7), a look-up gathers its 8 corners with plain 64-bit loads -- the first family
+// whose table traffic competes with the arithmetic.  The vertex at (p1, q, q+p1) is hoisted out of the c2 loop.
+struct Tab3DParams {
+  int n[3];
+  int is_log[3];
+  double lo[3], inv_h[3];
+};
+struct ThreePoint3DParams {
+  ThreePointParams B;   // L3 unused
+  Tab3DParams T;
+  const double* v3;
+};
+constexpr int T3D_MAX_TABLE = 12288;  // doubles (96 KB of shared memory)
+
+__device__ __forceinline__ double tab3d_eval(const double* __restrict__ v, const Tab3DParams& T, const FastMath& fm,
+                                             const double x0, const double x1, const double x2) {
+  const double x[3] = {x0, x1, x2};
+  int i[3];
+  double tau[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const double c = T.is_log[a] ? 0.5 * fm_log(fm, x[a]) : x[a];
+    double t = (c - T.lo[a]) * T.inv_h[a];
+    t = clamp_lo(t, 0.0);  // NaN -> 0
+    t = clamp_hi(t, (double)(T.n[a] - 1));
+    int ii = (int)t;
+    ii = min(ii, T.n[a] - 2);
+    i[a] = ii;
+    tau[a] = t - (double)ii;
+  }
+  const int s1 = T.n[2], s0 = T.n[1] * T.n[2];
+  const double* b = v + (i[0] * s0 + i[1] * s1 + i[2]);
+  // lerp along axis 2, then 1, then 0
+  const double v00 = fma(tau[2], b[1] - b[0], b[0]);
+  const double v01 = fma(tau[2], b[s1 + 1] - b[s1], b[s1]);
+  const double v10 = fma(tau[2], b[s0 + 1] - b[s0], b[s0]);
+  const double v11 = fma(tau[2], b[s0 + s1 + 1] - b[s0 + s1], b[s0 + s1]);
+  const double w0 = fma(tau[1], v01 - v00, v00);
+  const double w1 = fma(tau[1], v11 - v10, v10);
+  return fma(tau[0], w1 - w0, w0);
+}
+
+// lambda3 at the vertex with squared leg momenta (k1, k2, k3):  S0^2 = (k1+k2+k3)/6, a = sqrt3 (k2-k1)/(6 S0^2),
+// s = (k1+k2-2 k3)/(6 S0^2);  S0 = 0: a = s = 0.
+__device__ __forceinline__ double tab3d_vertex(const double* __restrict__ v, const Tab3DParams& T, const FastMath& fm,
+                                               const double k1, const double k2, const double k3) {
+  const double six = k1 + k2 + k3;
+  const double r = six > 0.0 ? fast_rcp(six) : 0.0;
+  return tab3d_eval(v, T, fm, six * (1.0 / 6.0), 1.7320508075688772 * (k2 - k1) * r, (k1 + k2 - 2.0 * k3) * r);
+}
+
+static size_t t3d_smem(int nq, int n1, int n2, int nt, int ntab3) {
+  return 8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((n1 + 1) & ~1) + 2 * ((n2 + 1) & ~1) + ((nt + 1) & ~1) + 36 +
+                      FM_DOUBLES + FX_DOUBLES + LG_DOUBLES + cells_guarded_size(nt) * 2 + 2 * nq + 2 * n2 +
+                      ((ntab3 + 1) & ~1));
+}
+
+template <int REGK, bool WANT_DMIN>
+__global__ void __launch_bounds__(256, 1) t3d_kernel(const ThreePoint3DParams Q) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t bar;
+  __shared__ double red[32];
+  constexpr int NT = 256;
+  const ThreePointParams& P = Q.B;
+  const Tab3DParams& T = Q.T;
+  const int nq = P.nq, n1 = P.n1, n2 = P.n2, nt = P.grid.n;
+  const int ntab3 = T.n[0] * T.n[1] * T.n[2];
+  double* sxq = reinterpret_cast<double*>(smem_raw);
+  double* swq = sxq + ((nq + 1) & ~1);
+  double* sx1 = swq + ((nq + 1) & ~1);
+  double* sw1 = sx1 + ((n1 + 1) & ~1);
+  double* sx2 = sw1 + ((n1 + 1) & ~1);
+  double* sw2 = sx2 + ((n2 + 1) & ~1);
+  double* sZA = sw2 + ((n2 + 1) & ~1);
+  double* skap = sZA + ((nt + 1) & ~1);  // 36
+  double* fmmem = skap + 36;
+  double* fxmem = fmmem + FM_DOUBLES;
+  double* lgmem = fxmem + FX_DOUBLES;
+  double2* cZA_all = reinterpret_cast<double2*>(lgmem + LG_DOUBLES);
+  double2* qtab = cZA_all + cells_guarded_size(nt);                   // [nq]
+  double2* xw2 = qtab + nq;                                           // [n2]
+  double* stab3 = reinterpret_cast<double*>(xw2 + n2);                // [ntab3]
+
+  if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
+  __syncthreads();
+  {
+    StageList L;
+    L.add(sxq, P.xq, nq); L.add(swq, P.wq, nq);
+    L.add(sx1, P.x1, n1); L.add(sw1, P.w1, n1);
+    L.add(sx2, P.x2, n2); L.add(sw2, P.w2, n2);
+    L.add(sZA, P.ZA, nt); L.add(stab3, Q.v3, ntab3);   // the whole 3-D table: one TMA bulk copy
+    stage_to_smem(L, &bar, 0);
+  }
+  const FastMath fm = fm_build(fmmem, P.fmc);
+  const double* fxtab = fx_build(fxmem, P.reg.zk * P.reg.k2);
+  const LogGrid lg = lg_build(lgmem, P.grid.lo, P.grid.inv_h, nt);
+  const double* kc = P.fmc.c;
+  const double2* cZA = cells_build_guarded(cZA_all, sZA, nt, P.grid.interp);
+  if (threadIdx.x < 35) skap[threadIdx.x] = P.coef[threadIdx.x];
+  for (int j = threadIdx.x; j < n2; j += NT) xw2[j] = make_double2(sx2[j], sw2[j]);
+  __syncthreads();
+
+  const double ik2 = P.reg.inv_k2;
+  const double inf = __longlong_as_double(0x7ff0000000000000LL);
+  double dmq = inf;
+  for (int i = threadIdx.x; i < nq; i += NT) {
+    const double q = sxq[i], sq = q * q;
+    double Rq, Rdq;
+    regulator(P.reg, fm, sq, Rq, Rdq);
+    const double Dq = lg_lookup(cZA, lg, kc, sq) * sq + Rq;
+    qtab[i] = make_double2((swq[i] * q * q * q * Rdq) * fast_rcp(Dq), Dq);
+    dmq = fmin(dmq, Dq);
+  }
+  dmq = block_min(dmq, red);  // also publishes qtab
+  double sum_wphi = 0.0;
+  for (int jp = 0; jp < P.nphi; ++jp) sum_wphi += P.wphi[jp];
+
+  const int npairs = nq * n1;
+  for (int e = blockIdx.x; e < P.n_ext; e += gridDim.x) {
+    const double p1 = P.ext[3 * e], p2 = P.ext[3 * e + 1], al = P.ext[3 * e + 2];
+    double sa_, ca_;
+    sincos(al, &sa_, &ca_);
+    double scc = p1 * p1 + p2 * p2 + 2.0 * p1 * p2 * ca_;
+    scc = scc > 0.0 ? scc : 0.0;
+    double dm = dmq;
+    double acc = 0.0;
+    for (int t = threadIdx.x; t < npairs; t += NT) {
+      const int i = t / n1, j1 = t - i * n1;
+      const double q = sxq[i], c1 = sx1[j1];
+      const double sq = q * q;
+      const double sin1 = sqrt((1.0 - c1) * (1.0 + c1));
+      const double wpair = qtab[i].x * (sw1[j1] * sin1);
+      const double qp1 = q * p1 * c1;
+      double s_a = sq + p1 * p1 + 2.0 * qp1;
+      s_a = clamp_lo(s_a, 0.0);
+      const double Da = fma(lg_lookup(cZA, lg, kc, s_a), s_a, t3_reg_R<REGK>(P.reg, fxtab, kc, s_a));
+      if (WANT_DMIN) dm = fmin(dm, Da);
+      const double lam1 = tab3d_vertex(stab3, T, fm, p1 * p1, sq, s_a);
+      const double X = sq * ik2, Y = qp1 * ik2;
+      double gam[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      {
+        int idx = 0;
+        double Xa = 1.0;
+#pragma unroll
+        for (int a = 0; a <= 4; ++a) {
+          double XaYb = Xa;
+#pragma unroll
+          for (int b = 0; b <= 4 - a; ++b) {
+#pragma unroll
+            for (int c = 0; c <= 4 - a - b; ++c) gam[c] = fma(skap[idx++], XaYb, gam[c]);
+            XaYb *= Y;
+          }
+          Xa *= X;
+        }
+      }
+      const double zc = q * p2 * ca_ * c1 * ik2;
+      const double zs = q * p2 * sa_ * sin1 * ik2;
+      const double sb0 = sq + p2 * p2;
+      const double m2k2 = -2.0 * P.reg.k2;
+      const double w0 = wpair * (fast_rcp(Da) * lam1);
+      double acc2 = 0.0;
+      for (int j2 = 0; j2 < n2; ++j2) {
+        const double2 xw = xw2[j2];
+        const double z = fma(zs, xw.x, zc);
+        double s_b = fma(m2k2, z, sb0);
+        s_b = clamp_lo(s_b, 0.0);
+        const double Db = fma(lg_lookup(cZA, lg, kc, s_b), s_b, t3_reg_R<REGK>(P.reg, fxtab, kc, s_b));
+        if (WANT_DMIN) dm = fmin(dm, Db);
+        const double lam2 = tab3d_vertex(stab3, T, fm, p2 * p2, sq, s_b);
+        const double lam3 = tab3d_vertex(stab3, T, fm, scc, s_a, s_b);
+        const double poly = fma(fma(fma(fma(gam[4], z, gam[3]), z, gam[2]), z, gam[1]), z, gam[0]);
+        acc2 = fma(xw.y * poly, fast_rcp(Db) * (lam2 * lam3), acc2);
+      }
+      acc = fma(w0, acc2, acc);
+    }
+    const double total = block_sum(acc, red);
+    const double dmin_b = WANT_DMIN ? block_min(dm, red) : 0.0;
+    if (threadIdx.x == 0) {
+      P.out[e] = P.prefactor * sum_wphi * total;
+      if (WANT_DMIN) P.dmin[e] = dmin_b * ik2;
+    }
+  }
+}
+
+// =====================================================================================================
 // four-point box: genuine three-angle kinematics + ghost loop (include/dfrg.h, DFRG_LOOP_FOURPOINT)
 // =====================================================================================================
 // Every node of the (q, c1, c2, phi) grid is a distinct evaluation.  Persistent CTAs; work unit = (external
@@ -1075,6 +1265,21 @@ static int loop4d_validate(const dfrg_loop4d_desc* D, int n_field, const double*
       return DFRG_EUNSUPPORTED;
     return DFRG_OK;
   }
+  if (D->family == DFRG_LOOP_THREEPOINT_TAB3D) {
+    if (n_field != 0 || D->n_coef != 35 || !valid_rule(D->cos2) || !valid_rule(D->phi) || D->dout_dm2) return DFRG_EINVAL;
+    if (!valid_table(D->tab[0], 1) || !D->tab3d.v) return DFRG_EINVAL;
+    long long ntab3 = 1;
+    for (int a = 0; a < 3; ++a) {
+      if (D->tab3d.n[a] < 2 || !(D->tab3d.hi[a] > D->tab3d.lo[a]) || (D->tab3d.is_log[a] != 0 && D->tab3d.is_log[a] != 1))
+        return DFRG_EINVAL;
+      ntab3 *= D->tab3d.n[a];
+      if (ntab3 > T3D_MAX_TABLE) return DFRG_EUNSUPPORTED;
+    }
+    if ((long long)D->q.n * D->cos1.n > 65536 || D->tab[0].n_q > 1024 || D->q.n > 4096 || D->cos1.n > 4096 ||
+        D->cos2.n > 4096)
+      return DFRG_EUNSUPPORTED;
+    return DFRG_OK;
+  }
   if (D->family == DFRG_LOOP_THREEPOINT || D->family == DFRG_LOOP_FOURPOINT) {
     const bool four = D->family == DFRG_LOOP_FOURPOINT;
     if (n_field != 0 || D->n_coef != (four ? 70 : 35) || !valid_rule(D->cos2) || !valid_rule(D->phi) || D->dout_dm2)
@@ -1196,6 +1401,29 @@ static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m
   P.xq = D->q.x; P.wq = D->q.w; P.x1 = D->cos1.x; P.w1 = D->cos1.w; P.x2 = D->cos2.x; P.w2 = D->cos2.w; P.wphi = D->phi.w;
   P.ZA = D->tab[0].v; P.L3 = D->tab[2].v; P.coef = D->coef; P.ext = ext; P.out = out; P.dmin = dmin;
   P.skip_flag = nullptr;
+  if (D->family == DFRG_LOOP_THREEPOINT_TAB3D) {
+    ThreePoint3DParams Q3;
+    Q3.B = P;
+    Q3.v3 = D->tab3d.v;
+    int ntab3 = 1;
+    for (int a = 0; a < 3; ++a) {
+      Q3.T.n[a] = D->tab3d.n[a]; Q3.T.is_log[a] = D->tab3d.is_log[a]; Q3.T.lo[a] = D->tab3d.lo[a];
+      Q3.T.inv_h[a] = (double)(D->tab3d.n[a] - 1) / (D->tab3d.hi[a] - D->tab3d.lo[a]);
+      ntab3 *= D->tab3d.n[a];
+    }
+    const size_t smem3 = t3d_smem(P.nq, P.n1, P.n2, P.grid.n, ntab3);
+    if (smem3 > 227 * 1024) return DFRG_EUNSUPPORTED;
+    const int regk3 = D->reg.kind == DFRG_REG_LITIM ? 0 : (D->reg.order == 1 ? 1 : 2);
+    void (*k3)(const ThreePoint3DParams) = nullptr;
+#define DFRG_T3D_PICK(K) if (regk3 == K) k3 = dmin ? t3d_kernel<K, true> : t3d_kernel<K, false>;
+    DFRG_T3D_PICK(0) DFRG_T3D_PICK(1) DFRG_T3D_PICK(2)
+#undef DFRG_T3D_PICK
+    cudaError_t e3 = cudaFuncSetAttribute(k3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3);
+    if (e3 != cudaSuccess) return check_cuda(e3);
+    const int grid3 = n_ext < sm_count ? n_ext : sm_count;
+    k3<<<grid3, 256, smem3, stream>>>(Q3);
+    return check_cuda(cudaGetLastError());
+  }
   const int regk = D->reg.kind == DFRG_REG_LITIM ? 0 : (D->reg.order == 1 ? 1 : 2);
   void* scratch = nullptr;
   // ---- product-grid path (ext_outer = G promised by the caller, checked on the device) ----
@@ -1281,6 +1509,7 @@ extern "C" int dfrg_integrate_loop4d_host(const dfrg_loop4d_desc* D, int n_field
   const size_t nf = two ? (size_t)n_field : 1, ne = (size_t)n_ext,
                next_d = two ? ne : (D->family == DFRG_LOOP_FOURPOINT ? 6 * ne : 3 * ne);
   size_t need = 2 * ((size_t)D->q.n + D->cos1.n + D->cos2.n + D->phi.n) + 3 * (size_t)D->tab[0].n_q + 128 + nf + next_d +
+                (D->family == DFRG_LOOP_THREEPOINT_TAB3D ? (size_t)T3D_MAX_TABLE + 16 : 0) +
                 3 * ne * nf;
   rc = A.begin(need * sizeof(double) + 32 * 256);
   if (rc != DFRG_OK) return rc;
@@ -1291,7 +1520,9 @@ extern "C" int dfrg_integrate_loop4d_host(const dfrg_loop4d_desc* D, int n_field
     Dd.cos2.x = A.put(D->cos2.x, D->cos2.n); Dd.cos2.w = A.put(D->cos2.w, D->cos2.n);
     Dd.phi.x = A.put(D->phi.x, D->phi.n); Dd.phi.w = A.put(D->phi.w, D->phi.n);
   }
-  for (int t = 0; t < (two ? 1 : 3); ++t) Dd.tab[t].v = A.put(D->tab[t].v, D->tab[t].n_q);
+  const bool tab3d = D->family == DFRG_LOOP_THREEPOINT_TAB3D;
+  for (int t = 0; t < ((two || tab3d) ? 1 : 3); ++t) Dd.tab[t].v = A.put(D->tab[t].v, D->tab[t].n_q);
+  if (tab3d) Dd.tab3d.v = A.put(D->tab3d.v, (size_t)D->tab3d.n[0] * D->tab3d.n[1] * D->tab3d.n[2]);
   Dd.coef = A.put(D->coef, D->n_coef);
   const double* d_m2 = two ? A.put(m2, nf) : nullptr;
   const double* d_ext = A.put(ext, next_d);

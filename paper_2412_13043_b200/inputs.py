@@ -161,6 +161,27 @@ def config5(n_s=16, n_ang=8, n_q=96, n_c1=32, n_c2=16, n_phi=16, n_tab=128, k=1.
                 coef=coef, ext=ext.reshape(-1, 6))
 
 
+def config6(n_p=32, n_alpha=8, n_q=96, n_c1=32, n_c2=16, n_phi=16, n_tab=128, n3=(96, 8, 7), k=1.0, seed=13, interp=3):
+    """Three-point vertex loop with a 3-D vertex dressing table lambda3(S0, a, s) (DESIGN.md reading
+    A23; not a BASELINE.json config).  Externals, quadrature, Z_A and the polynomial as config 3 (own seed); the vertex
+    table has the paper's 96 x 8 x 7 shape: S0 log-spaced over the 1-D grid's range, a and s uniform in
+    [-1, 1];  lambda3 = X(S0) (1 + c1 a^2 + c2 s + c3 a s) with X the rational function of config 3 and c_i seeded."""
+    c = config3(n_p=n_p, n_alpha=n_alpha, n_q=n_q, n_c1=n_c1, n_c2=n_c2, n_phi=n_phi, n_tab=n_tab, k=k, seed=seed,
+                interp=interp)
+    U = splitmix64_uniform(seed + 1000, 8)
+    lo, hi = c["lnq_lo"], c["lnq_hi"]
+    S0 = np.exp(np.linspace(lo, hi, n3[0]))
+    a = np.linspace(-1.0, 1.0, n3[1])
+    s_ = np.linspace(-1.0, 1.0, n3[2])
+    X = _rational(S0, k, 0.5 + U[0:5])
+    c1, c2, c3 = 0.3 * (U[5] - 0.5), 0.3 * (U[6] - 0.5), 0.3 * (U[7] - 0.5)
+    v3 = X[:, None, None] * (1.0 + c1 * a[None, :, None] ** 2 + c2 * s_[None, None, :] + c3 * a[None, :, None] * s_[None, None, :])
+    c.update(name="cfg6_threepoint3d", family=3, v3=np.ascontiguousarray(v3), lo3=(lo, -1.0, -1.0), hi3=(hi, 1.0, 1.0),
+             log3=(1, 0, 0), ext_outer=0)
+    del c["L3"], c["Zc"]
+    return c
+
+
 def config4(n_field=512, n_p=64, n_jext=16, n_q=96, n_c=24, n_tab=128, n_freq=64,
             T_over_k=0.15, cut=10.0, k=1.0, seed=4, interp=3):
     """Finite-T momentum-dependent loop, quark-meson-like (BASELINE.json configs[4])."""

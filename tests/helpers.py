@@ -38,6 +38,11 @@ def oracle_run(c, R, sel=None):
         out, dmin, sens = oracle.loop4d_twopoint(c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], *R["q"], *R["c"],
                                                  c["Z"], c["lnq_lo"], c["lnq_hi"], c["interp"], c["coef"], c["m2"],
                                                  c["pext"], sel=sel, want_sens=True, **_dress(c))
+    elif kd == "threepoint3d":
+        out, dmin, sens = oracle.loop4d_threepoint_tab3d(c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], *R["q"],
+                                                         *R["c1"], *R["c2"], R["phi"][1], c["ZA"], c["lnq_lo"],
+                                                         c["lnq_hi"], c["interp"], c["v3"], c["lo3"], c["hi3"], c["log3"],
+                                                         c["coef"], c["ext"], sel=sel, want_sens=True, **_dress(c))
     elif kd == "fourpoint":
         out, dmin, sens = oracle.loop4d_fourpoint(c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], *R["q"],
                                                   *R["c1"], *R["c2"], *R["phi"], c["ZA"], c["Zc"], c["L3"],
@@ -110,6 +115,14 @@ def gpu_run(c, R, host=False, want_dmin=True, want_d=False):
            (up(c["Z"]),), c["lnq_lo"], c["lnq_hi"], c["interp"], up(c["coef"]), up(c["m2"]), up(c["pext"]), out, dmin,
            dout_dm2=dout, **dress)
         res = dict(out=out, dmin=dmin, dout=dout)
+    elif kd == "threepoint3d":
+        ne = c["ext"].shape[0]
+        out, dmin = new(ne), new(ne) if want_dmin else None
+        fn = B.dfrg_integrate_loop4d_host if host else B.dfrg_integrate_loop4d
+        fn(B.LOOP_THREEPOINT_TAB3D, c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], rule("q"), rule("c1"),
+           rule("c2"), rule("phi"), (up(c["ZA"]),), c["lnq_lo"], c["lnq_hi"], c["interp"], up(c["coef"]), None,
+           up(c["ext"]), out, dmin, tab3d=(up(c["v3"]), c["lo3"], c["hi3"], c["log3"]), **dress)
+        res = dict(out=out, dmin=dmin)
     elif kd == "fourpoint":
         ne = c["ext"].shape[0]
         out, dmin = new(ne), new(ne) if want_dmin else None

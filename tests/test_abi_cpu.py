@@ -145,6 +145,22 @@ def test_integrators_validate_before_touching_the_device(lib):
     D5 = B.Loop4dDesc(B.LOOP_FOURPOINT, 1.0, reg, rule, rule, big, rule, T3(tab, tab, tab), p, 70)
     assert g(C.byref(D5), 0, None, 4, p, p, None, None) == B.DFRG_EUNSUPPORTED  # cos2 rule longer than a CTA
 
+    i3, d3 = C.c_int * 3, C.c_double * 3
+    t3 = B.Table3D(p, i3(96, 8, 7), d3(-9.0, -1.0, -1.0), d3(5.0, 1.0, 1.0), i3(1, 0, 0))
+    D6 = B.Loop4dDesc(B.LOOP_THREEPOINT_TAB3D, 1.0, reg, rule, rule, rule, rule, T3(tab, tab, tab), p, 35, 0, None, t3)
+    assert g(C.byref(D6), 1, None, 4, p, p, None, None) == B.DFRG_EINVAL        # no field axis
+    D6.tab3d.n[1] = 1
+    assert g(C.byref(D6), 0, None, 4, p, p, None, None) == B.DFRG_EINVAL        # every axis needs >= 2 points
+    D6.tab3d.n[1] = 8
+    D6.tab3d.hi[2] = -1.0
+    assert g(C.byref(D6), 0, None, 4, p, p, None, None) == B.DFRG_EINVAL        # empty axis range
+    D6.tab3d.hi[2] = 1.0
+    D6.tab3d.n[0] = 4000
+    assert g(C.byref(D6), 0, None, 4, p, p, None, None) == B.DFRG_EUNSUPPORTED  # table beyond the shared-memory budget
+    D6.tab3d.n[0] = 96
+    D6.tab3d.v = None
+    assert g(C.byref(D6), 0, None, 4, p, p, None, None) == B.DFRG_EINVAL
+
     h = lib.dfrg_integrate_matsubara3d
     stack = B.Table(p, 128, 64, -9.0, 5.0, 3)
     D4 = B.Mats3dDesc(0.15, 11, 1.0, reg, rule, rule, stack, stack, p, 20)
