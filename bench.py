@@ -30,8 +30,8 @@ WORKLOAD = "cfg4_matsubara3d: 64 p x 16 j x 512 field points, 23 Matsubara terms
 
 # FP64 roofline denominator: 148 SMs x 64 FP64 lanes x 2 flop/DFMA x 1.965 GHz
 FP64_LANES_PER_SM = 64
-# dram__bytes_read.sum + dram__bytes_write.sum of the moment kernel per launch on this workload (profiles/r1d_current_kernels.md)
-NCU_DRAM_BYTES_PER_LAUNCH = 31980800 + 3840
+# dram__bytes_read.sum + dram__bytes_write.sum of the moment kernel per launch on this workload (profiles/r1g_moment_kernel_symmetric_pairs.md)
+NCU_DRAM_BYTES_PER_LAUNCH = 31981056 + 2048
 
 
 def cfg4_counts(c, rules):
@@ -382,13 +382,13 @@ def main():
                        "parallelism": "external momenta sharded over GPUs (64 per GPU), no collective",
                        "integrals_per_step_per_gpu": n_out, "nominal_evals_per_step_per_gpu": evals},
             "integrals_per_s": world * n_out / (ms * 1e-3),
-            "clocks": clocks, "gpu_launches": 4 * args.steps,  # phi-rows pre-pass, psi pre-pass, moment kernel, fix-up kernel per step
+            "clocks": clocks, "gpu_launches": 5 * args.steps,  # phi-rows pre-pass, psi pre-pass, the two moment kernels (one returns at once), fix-up
             "e2e": {"value": world * evals / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_s * 1e3, "s1_host_ms": t_s1 * 1e3},
             "roofline": {"bound": "alu", "kernel": "mats3d_moment_kernel (+ the two pre-pass kernels and the fix-up kernel, timed together)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                          "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH if world == 1 else None,
                          "traffic_kind": "dram__bytes_read.sum + dram__bytes_write.sum of mats3d_moment_kernel, one ncu --set full "
-                                         "capture of this workload (profiles/r1d_current_kernels.md); algorithmic bytes: "
+                                         "capture of this workload (profiles/r1g_moment_kernel_symmetric_pairs.md); algorithmic bytes: "
                                          "31.85 MB of D0phi chunks read once",
                          "achieved_kind": "algorithmic FP64 instructions x 2 (DFMA-slot equivalents) / event time",
                          "achieved_strict": flops_strict / (ms_local * 1e-3) * 1e-12,
