@@ -228,6 +228,29 @@ def test_matsubara_symmetric_pair_moments(n_field, n_p, n_jext, n_q, n_c, n_max)
     assert np.array_equal(g3["out"], g4["out"])                          # the fallback is the plain loop, bit for bit
 
 
+@pytest.mark.parametrize("n_field,n_p,n_jext,n_q,n_c,n_max", [(530, 2, 5, 9, 8, 4), (300, 2, 17, 6, 6, 3), (100, 3, 1, 7, 5, 0),
+                                                              (64, 1, 32, 5, 4, 30), (700, 2, 3, 10, 16, 3),
+                                                              (200, 1, 16, 4, 8, 11)])
+def test_matsubara_any_shape_moment_kernel(n_field, n_p, n_jext, n_q, n_c, n_max):
+    # (n_max, n_jext) without a specialised instantiation take the any-shape moment kernel (n_jext padded up to the next
+    # compiled NJ, n_max at run time); shapes that have one ((3,3), (11,16)) are forced through it and must agree with the
+    # specialised kernel; everything against the oracle
+    c = inputs.config4(n_field=n_field, n_p=n_p, n_jext=n_jext, n_q=n_q, n_c=n_c, n_freq=64)
+    c["n_max"] = n_max
+    what = "mats_anyshape_%d_%d_%d_%d_%d_%d" % (n_field, n_p, n_jext, n_q, n_c, n_max)
+    os.environ["DFRG_M3_PATH"] = "moment-generic"
+    try:
+        g, o, _ = run_both(c, what=what)
+    finally:
+        del os.environ["DFRG_M3_PATH"]
+    g2, _, _ = run_both(c, what=what + "_default")
+    if (n_max, n_jext) in ((3, 3), (11, 16)):        # specialised kernel by default: same sums, possibly another rounding
+        fin = np.isfinite(g2["out"])
+        assert np.all(np.abs(g["out"] - g2["out"])[fin] <= 1e-13 * np.max(np.abs(g2["out"][fin])) + 1e-12 * np.abs(g2["out"][fin]))
+    else:                                            # the any-shape kernel is the default here
+        assert np.array_equal(g["out"], g2["out"], equal_nan=True)
+
+
 def test_matsubara_full_config4_sampled():
     c = inputs.config4()
     n_out = 64 * 16 * 512
