@@ -106,9 +106,9 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   if (moment) {
     const char* vm = getenv("DFRG_M3_MF");
     pl.generic = !mats3d_moment_shape(D->n_max, n_jext) || (vpath && vpath[0] == 'm');
-    pl.variant = (n_field <= 256 || (vm && atoi(vm) == 1)) ? 2 : 0;   // MF 2 x 256 threads, or MF 1 x 256 threads
-    if (pl.generic && n_jext > 16) pl.variant = 2;                    // 32 accumulators: one field point per thread
-    pl.tile = pl.variant == 0 ? 512 : 256;
+    pl.variant = n_field <= 256 ? 2 : ((vm && atoi(vm) == 1) ? 1 : 0);   // MF 2 x 256, MF 1 x 512 (knob), MF 1 x 256 threads
+    if (pl.generic && (n_jext > 16 || pl.variant == 1)) pl.variant = 2;  // any-shape kernel: 256 threads only
+    pl.tile = pl.variant == 2 ? 256 : 512;
     const int n_ftiles = (n_field + pl.tile - 1) / pl.tile;
     const long long upp = (long long)n_p * P.nq, U = (long long)n_ftiles * upp;
     pl.grid = (int)(U < sm_count ? U : sm_count);

@@ -381,19 +381,27 @@ __device__ __forceinline__ void mats3d_recip_batch(const double* __restrict__ dp
     for (int k = 0; k < MF; ++k) { d[t][k] = D0.x + m2[k]; d[t + 1][k] = D0.y + m2[k]; }
   }
   if constexpr (MF == 2) {
-    double pr[M3_NBAT], R[M3_NBAT];
+    // one hardware seed per TWO nodes x two field points: R = 1/((d00 d01)(d10 d11)), 1/(d00 d01) = R (d10 d11), ...
+    // 16 FP64 instructions per 4 reciprocals (as four separate Newton reciprocals) and a quarter of the MUFU.RCP64H
+    double pr[M3_NBAT], R[M3_NBAT / 2], q[M3_NBAT / 2];
 #pragma unroll
     for (int t = 0; t < M3_NBAT; ++t) pr[t] = d[t][0] * d[t][1];
 #pragma unroll
-    for (int t = 0; t < M3_NBAT; ++t) R[t] = rcp_seed(pr[t]);
+    for (int h = 0; h < M3_NBAT / 2; ++h) q[h] = pr[2 * h] * pr[2 * h + 1];
 #pragma unroll
-    for (int t = 0; t < M3_NBAT; ++t) pr[t] = fma(-pr[t], R[t], 1.0);
+    for (int h = 0; h < M3_NBAT / 2; ++h) R[h] = rcp_seed(q[h]);
 #pragma unroll
-    for (int t = 0; t < M3_NBAT; ++t) pr[t] = fma(pr[t], pr[t], pr[t]);
+    for (int h = 0; h < M3_NBAT / 2; ++h) q[h] = fma(-q[h], R[h], 1.0);
 #pragma unroll
-    for (int t = 0; t < M3_NBAT; ++t) R[t] = fma(R[t], pr[t], R[t]);
+    for (int h = 0; h < M3_NBAT / 2; ++h) q[h] = fma(q[h], q[h], q[h]);
 #pragma unroll
-    for (int t = 0; t < M3_NBAT; ++t) { r[t][0] = R[t] * d[t][1]; r[t][1] = R[t] * d[t][0]; }
+    for (int h = 0; h < M3_NBAT / 2; ++h) R[h] = fma(R[h], q[h], R[h]);
+#pragma unroll
+    for (int h = 0; h < M3_NBAT / 2; ++h) {
+      const double ra_ = R[h] * pr[2 * h + 1], rb_ = R[h] * pr[2 * h];   // 1/(d d) of node 2h, of node 2h+1
+      r[2 * h][0] = ra_ * d[2 * h][1]; r[2 * h][1] = ra_ * d[2 * h][0];
+      r[2 * h + 1][0] = rb_ * d[2 * h + 1][1]; r[2 * h + 1][1] = rb_ * d[2 * h + 1][0];
+    }
   } else {
 #pragma unroll
     for (int t = 0; t < M3_NBAT; ++t)
