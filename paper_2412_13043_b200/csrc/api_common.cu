@@ -171,48 +171,83 @@ int dfrg_matsubara_n_max(int domain, double T, double k, double extent) {
   return (int)n;
 }
 
+// Gauss-Legendre rule: roots of P_n by Newton on the three-term recurrence
+//   P_j = x P_{j-1} + c_j (x P_{j-1} - P_{j-2}),  c_j = (j-1)/j      (= ((2j-1) x P_{j-1} - (j-1) P_{j-2})/j, no division)
+// (1) Tricomi's initial guesses;  (2) three Newton iterations in double, eight roots side by side (independent chains:
+// the recurrence is latency bound);  (3) per root two passes in long double: one Newton correction at the double root
+// (d ~ 1e-16, so the corrected root is converged in long double), one evaluation of P_n' at the corrected root for the
+// weight 2/((1-x^2) P_n'^2).  Only the non-negative half is computed; the rule is mirrored, hence exactly symmetric.
 int dfrg_quad_nodes(int rule_kind, int n, double a, double b, double* x_host, double* w_host) {
   if (rule_kind != DFRG_RULE_GAUSS_LEGENDRE || n < 1 || n > 4096 || !x_host || !w_host) return DFRG_EINVAL;
   if (!(b > a) || !isfinite(a) || !isfinite(b)) return DFRG_EINVAL;
-  const long double PI_L = 3.14159265358979323846264338327950288L;
+  const double PI_D = 3.14159265358979323846;
   const long double hw = ((long double)b - (long double)a) / 2.0L, mid = ((long double)b + (long double)a) / 2.0L;
   const int half = (n + 1) / 2;
   const long double nn = (long double)n;
-  for (int r = 0; r < half; ++r) {  // r-th largest root
-    const long double theta = PI_L * (4.0L * r + 3.0L) / (4.0L * nn + 2.0L);
-    const long double sn = sinl(theta);
-    long double x = (1.0L - (nn - 1.0L) / (8.0L * nn * nn * nn) -
-                     (39.0L - 28.0L / (sn * sn)) / (384.0L * nn * nn * nn * nn)) * cosl(theta);
-    long double pn = 0.0L, pm = 0.0L, dpn = 1.0L;
-    for (int it = 0; it < 64; ++it) {
-      pm = 1.0L;  // P_0
-      pn = x;     // P_1
-      for (int j = 2; j <= n; ++j) {
-        const long double pj = ((2.0L * j - 1.0L) * x * pn - (j - 1.0L) * pm) / (long double)j;
-        pm = pn;
-        pn = pj;
-      }
-      if (n == 1) pm = 1.0L;
-      dpn = nn * (pm - x * pn) / ((1.0L - x) * (1.0L + x));
-      const long double step = pn / dpn;
-      x -= step;
-      if (fabsl(step) <= 4e-20L) break;
+  static thread_local long double cj[4097];
+  static thread_local double cjd[4097], xr[2048 + 8];
+  for (int j = 2; j <= n; ++j) { cj[j] = ((long double)j - 1.0L) / (long double)j; cjd[j] = (double)cj[j]; }
+  {  // (1) r-th largest root
+    const double nd = (double)n;
+    for (int r = 0; r < half; ++r) {
+      const double theta = PI_D * (4.0 * r + 3.0) / (4.0 * nd + 2.0);
+      const double sn = sin(theta);
+      xr[r] = (1.0 - (nd - 1.0) / (8.0 * nd * nd * nd) - (39.0 - 28.0 / (sn * sn)) / (384.0 * nd * nd * nd * nd)) * cos(theta);
     }
-    if (n % 2 == 1 && r == half - 1) x = 0.0L;
-    {  // P_{n-1} at the final x for the weight
-      pm = 1.0L; pn = x;
+    for (int r = half; r < half + 8; ++r) xr[r] = 0.5;  // padding of the last block
+  }
+  constexpr int NB = 8;
+  for (int r0 = 0; r0 < half && n > 1; r0 += NB) {  // (2)
+    for (int it = 0; it < 3; ++it) {
+      double x[NB], qm[NB], qn[NB];
+      for (int t = 0; t < NB; ++t) { x[t] = xr[r0 + t]; qm[t] = 1.0; qn[t] = x[t]; }
       for (int j = 2; j <= n; ++j) {
-        const long double pj = ((2.0L * j - 1.0L) * x * pn - (j - 1.0L) * pm) / (long double)j;
-        pm = pn; pn = pj;
+        const double c = cjd[j];
+        for (int t = 0; t < NB; ++t) {
+          const double xq = x[t] * qn[t];
+          const double qj = xq + c * (xq - qm[t]);
+          qm[t] = qn[t];
+          qn[t] = qj;
+        }
       }
-      if (n == 1) pm = 1.0L;
-      dpn = nn * (pm - x * pn) / ((1.0L - x) * (1.0L + x));
+      for (int t = 0; t < NB; ++t) {
+        const double dq = (double)n * (qm[t] - x[t] * qn[t]) / ((1.0 - x[t]) * (1.0 + x[t]));
+        xr[r0 + t] = x[t] - qn[t] / dq;
+      }
     }
-    const long double w = 2.0L / ((1.0L - x) * (1.0L + x) * dpn * dpn);
-    x_host[n - 1 - r] = (double)(mid + hw * x);
-    w_host[n - 1 - r] = (double)(hw * w);
-    x_host[r] = (double)(mid - hw * x);
-    w_host[r] = (double)(hw * w);
+  }
+  constexpr int LB = 4;   // (3) four roots side by side (independent long-double chains)
+  for (int r0 = 0; r0 < half; r0 += LB) {
+    long double x[LB], pm[LB], pn[LB], dp[LB];
+    for (int t = 0; t < LB; ++t) {
+      x[t] = (long double)xr[r0 + t];
+      if (n % 2 == 1 && r0 + t == half - 1) x[t] = 0.0L;   // the middle root of an odd rule is 0 exactly
+    }
+    for (int pass = 0; pass < 2; ++pass) {   // pass 0: Newton correction at the double root; pass 1: P_n' at the final root
+      for (int t = 0; t < LB; ++t) { pm[t] = 1.0L; pn[t] = x[t]; }
+      for (int j = 2; j <= n; ++j) {
+        const long double c = cj[j];
+        for (int t = 0; t < LB; ++t) {
+          const long double xp = x[t] * pn[t];
+          const long double pj = xp + c * (xp - pm[t]);
+          pm[t] = pn[t];
+          pn[t] = pj;
+        }
+      }
+      for (int t = 0; t < LB; ++t) {
+        if (n == 1) pm[t] = 1.0L;
+        dp[t] = nn * (pm[t] - x[t] * pn[t]) / ((1.0L - x[t]) * (1.0L + x[t]));
+        if (pass == 0 && !(n % 2 == 1 && r0 + t == half - 1)) x[t] -= pn[t] / dp[t];
+      }
+    }
+    for (int t = 0; t < LB && r0 + t < half; ++t) {
+      const int r = r0 + t;
+      const long double w = 2.0L / ((1.0L - x[t]) * (1.0L + x[t]) * dp[t] * dp[t]);
+      x_host[n - 1 - r] = (double)(mid + hw * x[t]);
+      w_host[n - 1 - r] = (double)(hw * w);
+      x_host[r] = (double)(mid - hw * x[t]);
+      w_host[r] = (double)(hw * w);
+    }
   }
   return DFRG_OK;
 }
