@@ -44,9 +44,12 @@
 // Mass derivatives (orc_*_dm2, at the end of the file): pinned by the derivatives of the Litim closed forms
 // (T = 0 and truncated Matsubara sum), the m2 -> inf weight integrals, and five-point finite differences of
 // the pinned value functions.
-// Parity unpinned: the *readings* of config 3 and config 4 (which integrand
-// the words of BASELINE.json mean) have no value outside this text to compare
-// with; their arithmetic is pinned by the independent mpmath restatement only.
+// Further families: dressed regulator (tests/test_oracle_pins_dressed.py), four-point box (..._fourpoint.py),
+// fermionic loop at chemical potential (..._fermion.py), 3-D tables and vertex coordinates (..._tab3d.py).
+// Every function here has a pin from outside this file.  What no pin can fix is the choice of READING where the
+// words of BASELINE.json / the paper leave an integrand open (configs 3, 4 and the 8(f) families): those readings
+// are stated in DESIGN.md section 2; the arithmetic of each reading is pinned by scipy/mpmath adaptive quadrature of
+// the continuum integrand it states, unit-monomial runs, Cartesian restatements and closed forms.
 
 #include <cmath>
 #include <cstddef>
