@@ -80,11 +80,18 @@ def oracle_run_dm2(c, R, sel=None):
     return dict(dpsi=(a, sa), dphi=(b, sb))
 
 
-def gpu_run(c, R, host=False, want_dmin=True, want_d=False):
+CANARY = -7.25e77       # sentinel around every output buffer of gpu_run(..., canary=True)
+CANARY_PAD = 64
+
+
+def gpu_run(c, R, host=False, want_dmin=True, want_d=False, canary=False):
     """Runs the workload through the C ABI (device entry point on torch CUDA tensors, or the *_host entry
-    point on numpy arrays).  -> dict(out=, dmin=, [chan=], [dchan= | dout= | dpsi=, dphi=]) of numpy arrays."""
+    point on numpy arrays).  -> dict(out=, dmin=, [chan=], [dchan= | dout= | dpsi=, dphi=]) of numpy arrays.
+    canary=True (device entry points): every output lives inside a larger buffer whose margins hold a sentinel; the
+    margins are checked after the call (an out-of-bounds write of the library fails the test)."""
     import torch
     from paper_2412_13043_b200 import binding as B
+    guards = []
 
     if host:
         up = lambda a: np.ascontiguousarray(a, dtype=np.float64)
@@ -92,8 +99,16 @@ def gpu_run(c, R, host=False, want_dmin=True, want_d=False):
         down = lambda a: a
     else:
         up = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).cuda()
-        new = lambda *shape: torch.full(shape, float("nan"), dtype=torch.float64, device="cuda")
         down = lambda a: a.cpu().numpy()
+
+        def new(*shape):
+            if not canary:
+                return torch.full(shape, float("nan"), dtype=torch.float64, device="cuda")
+            n = int(np.prod(shape))
+            big = torch.full((n + 2 * CANARY_PAD,), CANARY, dtype=torch.float64, device="cuda")
+            big[CANARY_PAD:CANARY_PAD + n] = float("nan")
+            guards.append((big, n))
+            return big[CANARY_PAD:CANARY_PAD + n].view(*shape)
     rule = lambda key: (up(R[key][0]), up(R[key][1]))
     kd = kind_of(c)
     res = {}
@@ -150,6 +165,9 @@ def gpu_run(c, R, host=False, want_dmin=True, want_d=False):
         res = dict(out=out, dmin=dmin, dpsi=dpsi, dphi=dphi)
     if not host:
         torch.cuda.synchronize()
+    for big, n in guards:
+        edge = torch.cat([big[:CANARY_PAD], big[CANARY_PAD + n:]]).cpu().numpy()
+        assert np.all(edge == CANARY), "the library wrote outside an output buffer (%s)" % c["name"]
     return {k_: (None if v is None else down(v)) for k_, v in res.items() if v is not None or k_ == "dmin"}
 
 
@@ -163,7 +181,7 @@ def parity_report(gpu, orc, dmin_orc, sens):
     diff = np.abs(gpu - orc)
     with np.errstate(divide="ignore", invalid="ignore"):
         rel = np.where(orc != 0, diff / np.abs(orc), np.where(diff == 0, 0.0, np.inf))
-        ratio = diff / sens
+        ratio = np.where(diff == 0, 0.0, diff / sens)      # 0/0: both sides are exactly zero (e.g. Rdot = 0 at every node)
     both_nonfinite = ~np.isfinite(gpu) & ~np.isfinite(orc)
     rep = dict(n=gpu.size, n_regular=int(regular.sum()), n_singular=int((~regular).sum()),
                n_pole=int((dmin_orc < REGULAR_DMIN).sum()), n_cancelling=int(((dmin_orc >= REGULAR_DMIN) & ~regular).sum()),
