@@ -19,6 +19,7 @@ from .binding import (  # noqa: F401
     table3d_lookup,
     vertex_coords,
     matsubara3d,
+    matsubara3d_mu,
     lpa_dm2,
     loop4d_twopoint_dm2,
     matsubara3d_dm2,

@@ -52,6 +52,7 @@
 // the continuum integrand it states, unit-monomial runs, Cartesian restatements and closed forms.
 
 #include <cmath>
+#include <complex>
 #include <cstddef>
 #include <cstdint>
 #include <limits>
@@ -847,6 +848,107 @@ int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg
       }
     }
     out[o] = (double)((acc_t)prefactor * (acc_t)T * acc_n);
+    if (dmin) dmin[o] = dm;
+    if (sens) sens[o] = (double)((acc_t)std::fabs(prefactor) * (acc_t)T * sn_n);
+  }
+  return 0;
+}
+
+// ---- 3-D spatial + Matsubara loop at finite chemical potential, spatial regulators ----
+// As orc_matsubara3d, with (reading A24):
+//   * spatial ("3D") regulators, as the paper's finite-density example: R(q^2), Rdot(q^2) on the fermion
+//     line, R(r^2) on the boson line;
+//   * every fermion leg carries the time component nu + i mu (PAPER.md:1947-1952 writes p0f - i mu_q: the complex
+//     conjugate convention; out(-mu) = conj(out(mu))): loop fermion nu_n + i mu, external fermion nu_j + i mu; the boson
+//     line carries their difference nu_j - nu_n, so mu drops out of it;
+//   s_psi = (nu_n + i mu)^2 + q^2 (complex),  G_psi = 1/(Z_psi(q^2; nbar) s_psi + R(q^2) + m2_psi)
+//   s_phi = om_m^2 + r^2,                      G_phi = 1/(Z_phi(r^2; |m|) s_phi + R(r^2) + m2_phi)
+//   y1 = (nu_n + i mu)(nu_j + i mu)/k^2,  y2 = p q c/k^2,  y3 = s_psi/k^2
+//   out[p][j][f] = C T sum_n sum_q w q^2 Rdot(q^2) G_psi^2 sum_c w P(y1, y2, y3) G_phi        (complex: out_re, out_im)
+// mu = 0 gives the real spatial-regulator variant of the family (out_im = 0 exactly).
+// dmin = min over nodes of min(|D_psi|, D_phi)/k^2;  sens as orc_matsubara3d with moduli.
+int orc_matsubara3d_mu(double T, int n_max, double mu, double prefactor, int reg_kind, int reg_order, double k,
+                       double zk, double eta,
+                       int nq, const double* xq, const double* wq,
+                       int nc, const double* xc, const double* wc,
+                       const double* Zpsi, const double* Zphi, int t_nq, int t_nfreq,
+                       double t_lo, double t_hi, int t_interp,
+                       const double* coef, int n_coef,
+                       int n_field, const double* m2psi, const double* m2phi,
+                       int n_p, const double* pext, int n_jext,
+                       long long n_sel, const long long* sel,
+                       double* out_re, double* out_im, double* dmin, double* sens) {
+  typedef std::complex<double> cd;
+  typedef std::complex<long double> cld;
+  if (n_coef != 20 || nq < 1 || nc < 1 || n_field < 1 || n_p < 1 || n_jext < 1 || k <= 0 || T <= 0) return -1;
+  if (n_max + 1 > t_nfreq || n_jext - 1 + n_max + 1 > t_nfreq) return -1;
+  const double pi = 3.14159265358979323846;
+  const double k2 = k * k;
+  const long long n_out = sel ? n_sel : (long long)n_p * n_jext * n_field;
+#pragma omp parallel for schedule(static)
+  for (long long o = 0; o < n_out; ++o) {
+    const long long flat = sel ? sel[o] : o;
+    const int f = (int)(flat % n_field);
+    const int j = (int)((flat / n_field) % n_jext);
+    const int e = (int)(flat / ((long long)n_field * n_jext));
+    const double p = pext[e];
+    const cd p0j((2.0 * j + 1.0) * pi * T, mu);
+    double dm = kInf;
+    cld acc_n(0.0L, 0.0L);
+    acc_t sn_n = 0.0L;
+    for (int n = -n_max; n <= n_max; ++n) {
+      const cd p0n((2.0 * n + 1.0) * pi * T, mu);
+      const int nbar = n >= 0 ? n : -n - 1;
+      const int m = j - n;
+      const int mabs = m >= 0 ? m : -m;
+      const double om = 2.0 * pi * (double)m * T;
+      for (int i = 0; i < nq; ++i) {
+        const double q = xq[i];
+        const cd spsi = p0n * p0n + q * q;
+        double Rp, Rdp;
+        regulator(reg_kind, reg_order, k, zk, eta, q * q, &Rp, &Rdp);
+        const cd Dpsi = table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q) * spsi + Rp + m2psi[f];
+        if (std::abs(Dpsi) / k2 < dm) dm = std::abs(Dpsi) / k2;
+        const cd Gpsi = 1.0 / Dpsi;
+        const double condpsi = 2.0 * (std::abs(Dpsi - m2psi[f]) + std::fabs(m2psi[f])) / std::abs(Dpsi);
+        cld acc_c(0.0L, 0.0L);
+        acc_t sn_c = 0.0L;
+        for (int jc = 0; jc < nc; ++jc) {
+          const double c = xc[jc];
+          const double r2 = clamp0(p * p + q * q - 2.0 * p * q * c);
+          const double sphi = om * om + r2;
+          double Rb, Rdb;
+          regulator(reg_kind, reg_order, k, zk, eta, r2, &Rb, &Rdb);
+          const double Dphi =
+              table_lookup(Zphi + (size_t)mabs * t_nq, t_nq, t_lo, t_hi, t_interp, r2) * sphi + Rb + m2phi[f];
+          if (Dphi / k2 < dm) dm = Dphi / k2;
+          const cd y1 = p0n * p0j / k2, y3 = spsi / k2;
+          const double y2 = p * q * c / k2;
+          cd P(0.0, 0.0);
+          double Pabs = 0.0;
+          int idx = 0;
+          for (int a = 0; a <= 3; ++a)
+            for (int b = 0; a + b <= 3; ++b)
+              for (int cc = 0; a + b + cc <= 3; ++cc) {
+                cd mono(coef[idx++], 0.0);
+                for (int t = 0; t < a; ++t) mono *= y1;
+                for (int t = 0; t < b; ++t) mono *= y2;
+                for (int t = 0; t < cc; ++t) mono *= y3;
+                P += mono;
+                Pabs += std::abs(mono);
+              }
+          const cd term = wc[jc] * P / Dphi;
+          acc_c += cld(term.real(), term.imag());
+          sn_c += (acc_t)(std::fabs(wc[jc] * Pabs / Dphi) *
+                          (1.0 + condpsi + (std::fabs(Dphi - m2phi[f]) + std::fabs(m2phi[f])) / std::fabs(Dphi)));
+        }
+        const cd wgt = wq[i] * q * q * Rdp * Gpsi * Gpsi;
+        acc_n += cld(wgt.real(), wgt.imag()) * acc_c;
+        sn_n += (acc_t)std::abs(wgt) * sn_c;
+      }
+    }
+    out_re[o] = (double)((acc_t)prefactor * (acc_t)T * acc_n.real());
+    out_im[o] = (double)((acc_t)prefactor * (acc_t)T * acc_n.imag());
     if (dmin) dmin[o] = dm;
     if (sens) sens[o] = (double)((acc_t)std::fabs(prefactor) * (acc_t)T * sn_n);
   }
