@@ -234,6 +234,15 @@ def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
                                                      c["k"], rq, rc, Zpsi, Zphi, c["lnq_lo"], c["lnq_hi"], c["interp"],
                                                      coef, m2psi, m2phi, pext, c["n_jext"], o4[0], dout_dm2_psi=o4[1],
                                                      dout_dm2_phi=o4[2]), n=3)
+    o_im = torch.empty_like(o4[0])
+    ms_mu = timeit(lambda: B.dfrg_integrate_matsubara3d(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"],
+                                                        c["k"], rq, rc, Zpsi, Zphi, c["lnq_lo"], c["lnq_hi"], c["interp"],
+                                                        coef, m2psi, m2phi, pext, c["n_jext"], o4[0], reg_arg4d=0, mu=0.3,
+                                                        out_im=o_im), n=3)
+    ev4 = o4[0].numel() * (2 * c["n_max"] + 1) * rq[0].numel() * rc[0].numel()
+    out["cfg4_chemical_potential"] = {"ms": ms_mu, "evals_per_s": ev4 / ms_mu * 1e3,
+                                      "integrals_per_s": o4[0].numel() / ms_mu * 1e3, "launches": 6,
+                                      "note": "mu = 0.3 k, spatial regulators, complex result (SURVEY 8(f) item 4)"}
     out["cfg4_with_mass_derivatives"] = {"ms": ms, "integrals_and_derivatives_per_s": 3 * o4[0].numel() / ms * 1e3,
                                          "launches": 8}
     return out

@@ -248,6 +248,16 @@ typedef struct {
   int n_coef;
   double* dout_dm2_psi; /* nullable output [n_p][n_jext][n_field]: d out / d m2_psi[f]  (G_psi^2 -> -2 G_psi^3) */
   double* dout_dm2_phi; /* nullable output [n_p][n_jext][n_field]: d out / d m2_phi[f]  (G_phi   -> -G_phi^2)   */
+  int reg_arg4d;        /* 1: R, Rdot at the 4-momentum squared (s_psi, s_phi) as written above (BASELINE.json config 4);
+                           0: spatial ("3D") regulators R(q^2), Rdot(q^2) on the fermion line and R(r^2) on the boson line */
+  double mu;            /* chemical potential (reading A24).  mu != 0 needs reg_arg4d = 0 and out_im:
+                           every fermion leg carries nu + i mu (loop nu_n + i mu, external nu_j + i mu; the boson line carries
+                           their difference and is unchanged), so s_psi = (nu_n + i mu)^2 + q^2, y1 = (nu_n + i mu)(nu_j + i mu)/k^2
+                           and y3 = s_psi/k^2 are complex and so is the result: out = real part, out_im = imaginary part
+                           (out(-mu) = conj out(mu): the paper writes p0f - i mu_q).  dmin = min(|D_psi|, D_phi)/k^2.
+                           Mass derivatives are not available with mu != 0 (DFRG_EUNSUPPORTED); n_jext <= 32 and
+                           128 n_jext (2 n_max + 1) + 4096 (n_max + 1) bytes of shared memory must fit (else DFRG_EUNSUPPORTED). */
+  double* out_im;       /* nullable unless mu != 0; output [n_p][n_jext][n_field] (zero-filled when mu == 0) */
 } dfrg_mats3d_desc;
 
 int dfrg_integrate_matsubara3d(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi, const double* m2_phi,

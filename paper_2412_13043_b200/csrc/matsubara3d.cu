@@ -37,6 +37,11 @@ static int mats3d_validate(const dfrg_mats3d_desc* D, int n_field, const double*
     return DFRG_EINVAL;
   if ((long long)D->q.n * D->cos1.n > M3_MAX_PAIRS || D->tab_psi.n_q > 1024) return DFRG_EUNSUPPORTED;
   if ((long long)n_p * n_jext > 2147483647LL || n_p > 65535) return DFRG_EUNSUPPORTED;
+  if ((D->reg_arg4d != 0 && D->reg_arg4d != 1) || !(D->mu == D->mu)) return DFRG_EINVAL;
+  if (D->mu != 0.0) {
+    if (D->reg_arg4d != 0 || !D->out_im) return DFRG_EINVAL;   // complex time component: spatial regulators only
+    if (D->dout_dm2_psi || D->dout_dm2_phi || n_jext > 32) return DFRG_EUNSUPPORTED;
+  }
   return DFRG_OK;
 }
 
@@ -78,6 +83,7 @@ static int mats3d_moment_dispatch(Mats3dParams& P, const MomentPlan& pl, cudaStr
 // any-shape moment kernel: compiled in matsubara3d_anyshape.cu (its own translation unit: the two sets of kernel
 // instantiations build side by side)
 int mats3d_gmoment_dispatch(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream);
+int mats3d_cmoment_dispatch(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream);   // mu != 0 (complex fermion line)
 
 static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi, const double* m2_phi, int n_p,
                          const double* p, int n_jext, double* out, double* dmin, int sm_count, cudaStream_t stream) {
@@ -97,17 +103,21 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   P.Zpsi = D->tab_psi.v; P.Zphi = D->tab_phi.v; P.coef = D->coef;
   P.m2psi = m2_psi; P.m2phi = m2_phi; P.pext = p; P.out = out; P.dmin = dmin;
   P.part = nullptr; P.tile_fields = 0; P.max_slots = 0; P.grid_main = 0; P.mode = 0; P.sym_try = 0; P.symflag = nullptr;
+  P.reg_arg4d = D->reg_arg4d; P.mu = D->mu;
+  P.psi_im = nullptr; P.psimin_f = nullptr; P.out_im = nullptr; P.part_im = nullptr;
+  const bool cplx = D->mu != 0.0;
 
   // ---- path: moment factorisation where an instantiation exists (DFRG_M3_PATH=generic forces the other one) ----
   const char* vpath = getenv("DFRG_M3_PATH");
   // DFRG_M3_PATH: "generic" forces the row-streaming kernel, "moment-generic" the any-shape moment kernel (tuning knobs)
-  bool moment = n_jext <= 32 && !(vpath && vpath[0] == 'g');
+  bool moment = n_jext <= 32 && (cplx || !(vpath && vpath[0] == 'g'));
   MomentPlan pl = {};
   if (moment) {
     const char* vm = getenv("DFRG_M3_MF");
     pl.generic = !mats3d_moment_shape(D->n_max, n_jext) || (vpath && vpath[0] == 'm');
     pl.variant = n_field <= 256 ? 2 : ((vm && atoi(vm) == 1) ? 1 : 0);   // MF 2 x 256, MF 1 x 512 (knob), MF 1 x 256 threads
     if (pl.generic && (n_jext > 16 || pl.variant == 1)) pl.variant = 2;  // any-shape kernel: 256 threads only
+    if (cplx) { pl.generic = true; pl.variant = 2; }                     // complex kernel: one field point per thread
     pl.tile = pl.variant == 2 ? 256 : 512;
     const int n_ftiles = (n_field + pl.tile - 1) / pl.tile;
     const long long upp = (long long)n_p * P.nq, U = (long long)n_ftiles * upp;
@@ -121,7 +131,13 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
     pl.smem = 8 * (size_t)(2 * P.chunk_stride + 2 * n_jext * (2 * D->n_max + 1) * 4 + 4 * (D->n_max + 1) + 4 * P.nc + P.nq);
     if (pl.generic)   // + the thread-private columns of H
       pl.smem += 8 * ((size_t)(D->n_max + 1) * 256 * (pl.variant == 0 ? 2 : 1) + 2);
-    if (pl.smem > 220 * 1024) moment = false;
+    if (cplx)         // beta' and H are complex: twice the shared memory for both
+      pl.smem = 8 * (size_t)(2 * P.chunk_stride + 2 * n_jext * (2 * D->n_max + 1) * 8 + 4 * (D->n_max + 1) + 4 * P.nc +
+                             ((P.nq + 1) & ~1) + 2 * (size_t)(D->n_max + 1) * 256 + 2);
+    if (pl.smem > 220 * 1024) {
+      if (cplx) return DFRG_EUNSUPPORTED;
+      moment = false;
+    }
   }
   P.phi_layout = moment ? 1 : 0;
   {
@@ -136,8 +152,9 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   const size_t n_psi = (size_t)n_terms * P.psi_stride * 2;
   const size_t n_psimin = ((size_t)n_terms + 1) & ~(size_t)1;
   const size_t n_part = moment ? (size_t)pl.max_slots * n_p * n_jext * n_field : 0;
+  const size_t n_cplx = cplx ? n_part + (size_t)n_terms * P.psi_stride + (((size_t)n_field + 1) & ~(size_t)1) : 0;
   void* scratch = nullptr;
-  int rc = scratch_alloc(&scratch, (n_d0 + n_rowmin + n_psi + n_psimin + n_part + 2) * sizeof(double), stream);
+  int rc = scratch_alloc(&scratch, (n_d0 + n_rowmin + n_psi + n_psimin + n_part + 2 + n_cplx) * sizeof(double), stream);
   if (rc != DFRG_OK) return rc;
   P.d0phi = (double*)scratch;
   P.psi = (double2*)(P.d0phi + n_d0);
@@ -145,11 +162,24 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   P.psimin = P.rowmin + n_rowmin;
   P.part = P.psimin + n_psimin;
   P.symflag = (int*)(P.part + n_part);
+  if (cplx) {
+    P.part_im = P.part + n_part + 2;
+    P.psi_im = P.part_im + n_part;
+    P.psimin_f = P.psi_im + (size_t)n_terms * P.psi_stride;
+    P.out_im = D->out_im;
+  } else if (D->out_im) {   // real result: the imaginary part is zero
+    rc = check_cuda(cudaMemsetAsync(D->out_im, 0, (size_t)n_p * n_jext * n_field * sizeof(double), stream));
+    if (rc != DFRG_OK) { scratch_free(scratch, stream); return rc; }
+  }
 
   mats3d_phi_rows_kernel<<<dim3(P.n_rows, n_p), M3_PRE_THREADS, 0, stream>>>(P);
   rc = check_cuda(cudaGetLastError());
   if (rc == DFRG_OK) {
     mats3d_psi_kernel<<<n_terms, 128, 0, stream>>>(P);
+    rc = check_cuda(cudaGetLastError());
+  }
+  if (rc == DFRG_OK && cplx && dmin) {
+    mats3d_psimin_cplx_kernel<<<(n_field + 127) / 128, 128, 0, stream>>>(P);
     rc = check_cuda(cudaGetLastError());
   }
   // one pass for the values, one more for each requested mass derivative (same kernels, mode 1 / 2)
@@ -160,7 +190,8 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
     P.out = pass_out[mode];
     P.dmin = mode == 0 ? dmin : nullptr;
     if (moment) {
-      rc = pl.generic ? mats3d_gmoment_dispatch(P, pl, stream) : mats3d_moment_dispatch(P, pl, stream);
+      rc = cplx ? mats3d_cmoment_dispatch(P, pl, stream)
+                : (pl.generic ? mats3d_gmoment_dispatch(P, pl, stream) : mats3d_moment_dispatch(P, pl, stream));
       if (rc == DFRG_OK) {
         const long long n_out = (long long)n_p * n_jext * n_field;
         mats3d_fixup_kernel<<<(unsigned)((n_out + 255) / 256), 256, 0, stream>>>(P);
@@ -217,7 +248,7 @@ extern "C" int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_
   Arena& A = thread_arena();
   const size_t nf = (size_t)n_field, n_out = (size_t)n_p * n_jext * nf;
   const size_t rows_psi = (size_t)D->n_max + 1, rows_phi = (size_t)n_jext + D->n_max, nt = (size_t)D->tab_psi.n_q;
-  const size_t need = 2 * ((size_t)D->q.n + D->cos1.n) + (rows_psi + rows_phi) * nt + 20 + 2 * nf + n_p + 4 * n_out;
+  const size_t need = 2 * ((size_t)D->q.n + D->cos1.n) + (rows_psi + rows_phi) * nt + 20 + 2 * nf + n_p + 5 * n_out;
   rc = A.begin(need * sizeof(double) + 32 * 256);
   if (rc != DFRG_OK) return rc;
   dfrg_mats3d_desc Dd = *D;
@@ -233,6 +264,7 @@ extern "C" int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_
   double* d_dmin = dmin ? A.reserve(n_out) : nullptr;
   Dd.dout_dm2_psi = D->dout_dm2_psi ? A.reserve(n_out) : nullptr;
   Dd.dout_dm2_phi = D->dout_dm2_phi ? A.reserve(n_out) : nullptr;
+  Dd.out_im = D->out_im ? A.reserve(n_out) : nullptr;
   if (A.status() != DFRG_OK) return A.status();
   rc = mats3d_launch(&Dd, n_field, d_mpsi, d_mphi, n_p, d_p, n_jext, d_out, d_dmin, sms, A.stream());
   if (rc != DFRG_OK) return rc;
@@ -240,5 +272,6 @@ extern "C" int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_
   if (dmin) A.fetch(dmin, d_dmin, n_out);
   if (D->dout_dm2_psi) A.fetch(D->dout_dm2_psi, Dd.dout_dm2_psi, n_out);
   if (D->dout_dm2_phi) A.fetch(D->dout_dm2_phi, Dd.dout_dm2_phi, n_out);
+  if (D->out_im) A.fetch(D->out_im, Dd.out_im, n_out);
   return A.finish();
 }

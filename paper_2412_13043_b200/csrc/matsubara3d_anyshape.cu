@@ -38,4 +38,27 @@ int mats3d_gmoment_dispatch(Mats3dParams& P, const MomentPlan& pl, cudaStream_t 
   return DFRG_EUNSUPPORTED;
 }
 
+
+// complex (mu != 0) moment kernel: one field point per thread, NJ = the smallest compiled value >= n_jext
+template <int NJ, bool SYM>
+static int mats3d_cmoment_go(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream) {
+  auto kern = mats3d_cmoment_kernel<NJ, SYM>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+  if (e != cudaSuccess) return check_cuda(e);
+  kern<<<pl.grid, 256, pl.smem, stream>>>(P);
+  return check_cuda(cudaGetLastError());
+}
+int mats3d_cmoment_dispatch(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream) {
+#define X(NJ)                                                                      \
+  if (P.n_jext <= NJ) {                                                            \
+    if (P.sym_try) {                                                               \
+      const int rc = mats3d_cmoment_go<NJ, true>(P, pl, stream);                   \
+      if (rc != DFRG_OK) return rc;                                                \
+    }                                                                              \
+    return mats3d_cmoment_go<NJ, false>(P, pl, stream);                            \
+  }
+  X(2) X(4) X(8) X(16) X(32)
+#undef X
+  return DFRG_EUNSUPPORTED;
+}
 }  // namespace dfrg

@@ -33,6 +33,11 @@ struct Mats3dParams {
   double *part;      // [max_slots][n_p][n_jext][n_field]
   int sym_try;       // host: the cos rule is long enough for the symmetric-pair moment loop (nc % 8 == 0)
   int* symflag;      // device: 1 if the cos rule is exactly symmetric (x_c = -x_{nc-1-c}, equal weights), set by the pre-pass
+  int reg_arg4d;     // 1: regulators at the 4-momentum squared; 0: spatial regulators
+  double mu;         // chemical potential (complex fermion line when != 0)
+  double *psi_im;    // [2 n_max + 1][psi_stride]  Im D0psi (mu != 0)
+  double *psimin_f;  // [n_field]  min over (n, q) of |D0psi + m2psi_f| (mu != 0)
+  double *out_im, *part_im;
   int mode;          // 0: value;  1: d/dm2_psi (G_psi^2 -> -2 G_psi^3);  2: d/dm2_phi (G_phi -> -G_phi^2, kernels with SQ)
 };
 
@@ -68,7 +73,7 @@ static __global__ void __launch_bounds__(M3_PRE_THREADS) mats3d_phi_rows_kernel(
     r2 = clamp_lo(r2, 0.0);
     const double sphi = om * om + r2;
     double R, Rd;
-    regulator(P.reg, fm, sphi, R, Rd);
+    regulator(P.reg, fm, P.reg_arg4d ? sphi : r2, R, Rd);
     const double D0 = table_lookup(cells, P.grid, fm, r2) * sphi + R;
     if (P.phi_layout == 0) dst[t] = D0;
     else dst1[(size_t)i * P.chunk_stride + (sym ? (2 * jc < P.nc ? 2 * jc : 2 * (P.nc - 1 - jc) + 1) : jc)] = D0;
@@ -98,11 +103,13 @@ static __global__ void __launch_bounds__(128) mats3d_psi_kernel(const Mats3dPara
   double dmin = __longlong_as_double(0x7ff0000000000000LL);
   for (int i = threadIdx.x; i < P.nq; i += 128) {
     const double q = P.xq[i];
-    const double spsi = nun * nun + q * q;
+    const double spsi = nun * nun - P.mu * P.mu + q * q;   // Re (nu + i mu)^2 + q^2
     double R, Rd;
-    regulator(P.reg, fm, spsi, R, Rd);
-    const double D0 = table_lookup(cells, P.grid, fm, q * q) * spsi + R;
+    regulator(P.reg, fm, P.reg_arg4d ? spsi : q * q, R, Rd);
+    const double Z = table_lookup(cells, P.grid, fm, q * q);
+    const double D0 = Z * spsi + R;
     P.psi[(size_t)it * P.psi_stride + i] = make_double2(D0, P.wq[i] * q * q * Rd);
+    if (P.psi_im) P.psi_im[(size_t)it * P.psi_stride + i] = Z * (2.0 * nun * P.mu);
     dmin = fmin(dmin, D0);
   }
   dmin = block_min(dmin, red);
@@ -983,6 +990,233 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_gmoment_kernel(const Mats3dPara
   }
 }
 
+// ---- (3d) moment kernel at finite chemical potential (complex fermion line) ------------------------------------
+// mu != 0 (include/dfrg.h, dfrg_mats3d_desc::mu; reading A24): the boson line and hence the angular moments
+// M_b stay real; the fermion line H = G_psi^2 and the polynomial coefficients beta'_b(j, n) are complex, and so are the
+// accumulators.  Same unit walk, staging and moment loop as mats3d_gmoment_kernel (one field point per thread):
+//   H[nbar] = 1/(D0re + m2 + i D0im)^2 per field point (thread-private shared-memory column; H(n < 0) = conj H(nbar)),
+//   beta' = (re[4], im[4]) per (j, n) in shared memory,  t = beta' . M (8 FP64),  acc[j] += H t (4 FP64).
+struct cplx_t { double re, im; };
+__device__ __forceinline__ cplx_t cmul(const cplx_t a, const cplx_t b) {
+  cplx_t r; r.re = a.re * b.re - a.im * b.im; r.im = a.re * b.im + a.im * b.re; return r;
+}
+template <int NJ, bool SYM>
+__global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dParams P) {
+  constexpr int NTC = 256, MF = 1;
+  if (P.sym_try && (*P.symflag != 0) != SYM) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t full[2];
+  __shared__ double skap[20];
+
+  const int nq = P.nq, nc = P.nc, cs = P.chunk_stride, ps = P.psi_stride;
+  const int n_max = P.n_max, n_jext = P.n_jext;
+  const int NT = 2 * n_max + 1, NROWS = n_jext + n_max, NB = n_jext * NT * 8, NPS = n_max + 1;
+  double* d0buf = reinterpret_cast<double*>(smem_raw);             // [2][cs]
+  double* betabuf = d0buf + 2 * cs;                                // [2][NB]  (re[4], im[4]) per (j, n)
+  double* psibuf = betabuf + 2 * NB;                               // [2][NPS][2] (Re D0psi, Im D0psi)
+  double* numbuf = psibuf + 4 * NPS;                               // [nc][4]  wc c^b
+  double* sxq = numbuf + 4 * nc;                                   // [nq]
+  double* Hs = sxq + ((nq + 1) & ~1);                              // [NPS][NTC][2]
+
+  const int tid = threadIdx.x;
+  const int n_ftiles = (P.n_field + NTC - 1) / NTC;
+  const long long upp = (long long)P.n_p * nq;
+  const long long U = (long long)n_ftiles * upp;
+  const long long u0 = (long long)blockIdx.x * U / gridDim.x, u1 = (long long)(blockIdx.x + 1) * U / gridDim.x;
+  const double pi = 3.14159265358979323846;
+  const double ik2 = P.reg.inv_k2;
+
+  if (tid == 0) {
+    mbar_init(&full[0], 1);
+    mbar_init(&full[1], 1);
+    mbar_fence_init();
+  }
+  if (tid < 20) skap[tid] = P.coef[tid];
+  for (int i = tid; i < nq; i += NTC) sxq[i] = P.xq[i];
+  for (int c = tid; c < (SYM ? nc / 2 : nc); c += NTC) {
+    const int cn = SYM ? nc - 1 - c : c;
+    const double x = P.xc[cn], w = P.wc[cn];
+    numbuf[4 * c] = w; numbuf[4 * c + 1] = w * x; numbuf[4 * c + 2] = w * x * x; numbuf[4 * c + 3] = w * x * x * x;
+  }
+  __syncthreads();
+
+  auto produce = [&](long long u, int b) {
+    const long long rem = u % upp;
+    const int e = (int)(rem / nq), i = (int)(rem - (long long)e * nq);
+    if (tid == 0) {
+      mbar_expect_tx(&full[b], (uint32_t)cs * 8u);
+      tma_bulk_g2s(d0buf + (size_t)b * cs, P.d0phi + ((size_t)e * nq + i) * cs, (uint32_t)cs * 8u, &full[b]);
+    }
+    for (int t = tid; t < NPS; t += NTC) {
+      const size_t at = (size_t)(t + n_max) * ps + i;
+      psibuf[(b * NPS + t) * 2] = P.psi[at].x;
+      psibuf[(b * NPS + t) * 2 + 1] = P.psi_im[at];
+    }
+    const double q = sxq[i];
+    const double pq = P.pext[e] * q * ik2;
+    double* bet = betabuf + (size_t)b * NB;
+    for (int t = tid; t < n_jext * NT; t += NTC) {
+      const int j = t / NT, n = t - j * NT - n_max;
+      const int nbar = n >= 0 ? n : -n - 1;
+      const double nun = (2.0 * n + 1.0) * pi * P.T, nuj = (2.0 * j + 1.0) * pi * P.T;
+      cplx_t p0n, p0j, y1, y3;
+      p0n.re = nun; p0n.im = P.mu; p0j.re = nuj; p0j.im = P.mu;
+      y1 = cmul(p0n, p0j); y1.re *= ik2; y1.im *= ik2;
+      y3 = cmul(p0n, p0n); y3.re = (y3.re + q * q) * ik2; y3.im *= ik2;
+      // P = sum_b y2^b beta_b,  beta_b = sum_{a+c<=3-b} kap_abc y1^a y3^c   (idx: a outermost, then b, then c)
+      cplx_t be[4];
+#pragma unroll
+      for (int bb = 0; bb < 4; ++bb) { be[bb].re = 0.0; be[bb].im = 0.0; }
+      int idx = 0;
+      cplx_t y1a; y1a.re = 1.0; y1a.im = 0.0;
+#pragma unroll
+      for (int a = 0; a <= 3; ++a) {
+#pragma unroll
+        for (int bb = 0; bb <= 3 - a; ++bb) {
+          cplx_t y3c = y1a;
+#pragma unroll
+          for (int c = 0; c <= 3 - a - bb; ++c) {
+            const double kap = skap[idx++];
+            be[bb].re = fma(kap, y3c.re, be[bb].re);
+            be[bb].im = fma(kap, y3c.im, be[bb].im);
+            y3c = cmul(y3c, y3);
+          }
+        }
+        y1a = cmul(y1a, y1);
+      }
+      const double W = P.psi[(size_t)(nbar + n_max) * ps + i].y;
+      double sc = W;
+#pragma unroll
+      for (int bb = 0; bb < 4; ++bb) {
+        bet[8 * t + bb] = be[bb].re * sc;
+        bet[8 * t + 4 + bb] = be[bb].im * sc;
+        sc *= pq;
+      }
+    }
+  };
+
+  const double4* num4 = reinterpret_cast<const double4*>(numbuf);
+  double* myH = Hs + (size_t)tid * 2;
+  double m2psi[MF], m2phi[MF], accr[NJ], acci[NJ];
+  int cur_ft = -1;
+  uint32_t g = 0;
+  if (u0 < u1) produce(u0, 0);
+  __syncthreads();
+  for (long long u = u0; u < u1; ++u, ++g) {
+    const int ft = (int)(u / upp);
+    const long long rem = u - (long long)ft * upp;
+    const int e = (int)(rem / nq), i = (int)(rem - (long long)e * nq);
+    const int f = ft * NTC + tid;
+    const int b = g & 1;
+    if (u + 1 < u1) produce(u + 1, b ^ 1);
+    if (ft != cur_ft) {
+      cur_ft = ft;
+      m2psi[0] = (f < P.n_field) ? P.m2psi[f] : 1.0;
+      m2phi[0] = (f < P.n_field) ? P.m2phi[f] : 1.0;
+    }
+    if (u == u0 || i == 0) {
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) { accr[j] = 0.0; acci[j] = 0.0; }
+    }
+    mbar_wait(&full[b], (g >> 1) & 1);
+    const double* d0 = d0buf + (size_t)b * cs;
+    const double4* bet4 = reinterpret_cast<const double4*>(betabuf + (size_t)b * NB);
+    const double* psb = psibuf + (size_t)b * NPS * 2;
+
+    for (int nb = 0; nb < NPS; ++nb) {   // H = G_psi^2, G_psi = conj(D)/|D|^2, D = a + i bb
+      const double a = psb[2 * nb] + m2psi[0], bb = psb[2 * nb + 1];
+      const double r = fast_rcp(fma(a, a, bb * bb));
+      const double gr = a * r, gi = -(bb * r);
+      myH[(size_t)nb * NTC * 2] = gr * gr - gi * gi;
+      myH[(size_t)nb * NTC * 2 + 1] = 2.0 * gr * gi;
+    }
+    const bool pipelined = (nc % (2 * M3_NBAT)) == 0;
+    const int l_last = NROWS * nc - M3_NBAT;
+    double ra[M3_NBAT][MF], rb[M3_NBAT][MF];
+    if (pipelined) mats3d_recip_batch<MF, false>(d0, m2phi, ra);
+#pragma unroll 1
+    for (int m = 0; m < NROWS; ++m) {
+      double M[4][MF];
+      M[0][0] = 0.0; M[1][0] = 0.0; M[2][0] = 0.0; M[3][0] = 0.0;
+      if (pipelined) {
+        for (int c = 0; c < nc; c += 2 * M3_NBAT) {
+          const int L = m * nc + c;
+          mats3d_recip_batch<MF, false>(d0 + L + M3_NBAT, m2phi, rb);
+          if constexpr (SYM) mats3d_moment_accumulate_sym<MF>(num4 + c / 2, ra, M);
+          else mats3d_moment_accumulate<MF>(num4 + c, ra, M);
+          int Ln = L + 2 * M3_NBAT;
+          Ln = Ln < l_last ? Ln : l_last;
+          mats3d_recip_batch<MF, false>(d0 + Ln, m2phi, ra);
+          if constexpr (SYM) mats3d_moment_accumulate_sym<MF>(num4 + (c + M3_NBAT) / 2, rb, M);
+          else mats3d_moment_accumulate<MF>(num4 + c + M3_NBAT, rb, M);
+        }
+      } else {
+        const double* drow = d0 + m * nc;
+#pragma unroll 1
+        for (int c = 0; c < nc; ++c) {
+          const double r = fast_rcp(drow[c] + m2phi[0]);
+          const double4 w = num4[c];
+          M[0][0] = fma(w.x, r, M[0][0]);
+          M[1][0] = fma(w.y, r, M[1][0]);
+          M[2][0] = fma(w.z, r, M[2][0]);
+          M[3][0] = fma(w.w, r, M[3][0]);
+        }
+      }
+      // ---- the (j, n) pairs with |j - n| = m ----
+      const int jlo1 = max(0, m - n_max), jhi1 = min(n_jext - 1, n_max + m);
+      const int jhi2 = m > 0 ? min(n_jext - 1, n_max - m) : -1;
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) {
+#pragma unroll
+        for (int side = 0; side < 2; ++side) {
+          const bool valid = side == 0 ? (j >= jlo1 && j <= jhi1) : (j <= jhi2);
+          if (valid) {
+            const int n = side == 0 ? j - m : j + m;
+            const int nbar = n >= 0 ? n : -n - 1;
+            const double4 Br = bet4[(j * NT + n + n_max) * 2], Bi = bet4[(j * NT + n + n_max) * 2 + 1];
+            const double hr = myH[(size_t)nbar * NTC * 2];
+            const double hi = n >= 0 ? myH[(size_t)nbar * NTC * 2 + 1] : -myH[(size_t)nbar * NTC * 2 + 1];
+            const double tr = fma(Br.w, M[3][0], fma(Br.z, M[2][0], fma(Br.y, M[1][0], Br.x * M[0][0])));
+            const double ti = fma(Bi.w, M[3][0], fma(Bi.z, M[2][0], fma(Bi.y, M[1][0], Bi.x * M[0][0])));
+            accr[j] = fma(hr, tr, fma(-hi, ti, accr[j]));
+            acci[j] = fma(hr, ti, fma(hi, tr, acci[j]));
+          }
+        }
+      }
+    }
+    if (i == nq - 1 || u == u1 - 1) {
+      const long long ufirst = (long long)ft * upp + (long long)e * nq;
+      const int c_first = (int)(((ufirst + 1) * gridDim.x - 1) / U);
+      const int slot = (int)blockIdx.x - c_first;
+      if (f < P.n_field) {
+#pragma unroll
+        for (int j = 0; j < NJ; ++j)
+          if (j < n_jext) {
+            const size_t at = (((size_t)slot * P.n_p + e) * n_jext + j) * P.n_field + f;
+            P.part[at] = accr[j];
+            P.part_im[at] = acci[j];
+          }
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// mu != 0: min over (n >= 0, q) of |D0psi + m2psi_f| per field point (the rows n < 0 are the complex conjugates).
+static __global__ void __launch_bounds__(128) mats3d_psimin_cplx_kernel(const Mats3dParams P) {
+  const int f = blockIdx.x * 128 + threadIdx.x;
+  if (f >= P.n_field) return;
+  const double m2 = P.m2psi[f];
+  double best = __longlong_as_double(0x7ff0000000000000LL);
+  for (int nb = 0; nb <= P.n_max; ++nb)
+    for (int i = 0; i < P.nq; ++i) {
+      const size_t at = (size_t)(nb + P.n_max) * P.psi_stride + i;
+      const double a = P.psi[at].x + m2, b = P.psi_im[at];
+      best = fmin(best, fma(a, a, b * b));
+    }
+  P.psimin_f[f] = sqrt(best);
+}
+
 // S5/S6 of the moment path: out = prefactor T sum_slots part, dmin from the row minima.
 static __global__ void __launch_bounds__(256) mats3d_fixup_kernel(const Mats3dParams P) {
   const long long idx = (long long)blockIdx.x * 256 + threadIdx.x;
@@ -999,7 +1233,23 @@ static __global__ void __launch_bounds__(256) mats3d_fixup_kernel(const Mats3dPa
   double r = P.part[idx];
   for (int s = 1; s <= c_last - c_first; ++s) r += P.part[(size_t)s * stride + idx];
   P.out[idx] = P.prefactor * P.T * r;
-  if (P.dmin) {
+  if (P.out_im) {
+    double ri = 0.0;
+    if (P.part_im) {
+      ri = P.part_im[idx];
+      for (int s = 1; s <= c_last - c_first; ++s) ri += P.part_im[(size_t)s * stride + idx];
+    }
+    P.out_im[idx] = P.prefactor * P.T * ri;
+  }
+  if (P.dmin && P.psimin_f) {   // complex fermion line: |D_psi| does not split into (min D0) + m2
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    double dphi = inf;
+    for (int it = 0; it < 2 * P.n_max + 1; ++it) {
+      const int mm = j - (it - P.n_max), mabs = mm >= 0 ? mm : -mm;
+      dphi = fmin(dphi, P.rowmin[(size_t)e * P.n_rows + mabs]);
+    }
+    P.dmin[idx] = fmin(P.psimin_f[f], dphi + P.m2phi[f]) * P.reg.inv_k2;
+  } else if (P.dmin) {
     const double inf = __longlong_as_double(0x7ff0000000000000LL);
     double dpsi = inf, dphi = inf;
     for (int it = 0; it < 2 * P.n_max + 1; ++it) {
