@@ -218,11 +218,12 @@ def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
     ms = timeit(lambda: B.dfrg_integrate_loop4d(B.LOOP_THREEPOINT_TAB3D, c["prefactor"], c["reg_kind"], c["reg_order"],
                                                 c["k"], rr["q"], rr["c1"], rr["c2"], rr["phi"], (ZA,), c["lnq_lo"],
                                                 c["lnq_hi"], c["interp"], coef, None, ext, o6,
-                                                tab3d=(v3, c["lo3"], c["hi3"], c["log3"])), n=3)
+                                                tab3d=(v3, c["lo3"], c["hi3"], c["log3"]),
+                                                ext_outer=c["ext_outer"]), n=3)
     uniq = o6.numel() * rr["q"][0].numel() * rr["c1"][0].numel() * rr["c2"][0].numel()
     out["cfg6_threepoint_tab3d"] = {"ms": ms, "unique_evals_per_s": uniq / ms * 1e3,
                                     "table_lookups_per_s": uniq * (2 + 1.0 / rr["c2"][0].numel()) / ms * 1e3,
-                                    "integrals_per_s": o6.numel() / ms * 1e3, "launches": 1}
+                                    "integrals_per_s": o6.numel() / ms * 1e3, "launches": 4}
     # cfg4 with both mass derivatives (three passes of the moment kernel: value, d/dm2_psi, d/dm2_phi)
     c = inputs.config4()
     R = make_rules(c, B.dfrg_quad_nodes)

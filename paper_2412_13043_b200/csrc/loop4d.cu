@@ -488,6 +488,57 @@ static size_t threepoint_v2_smem(int nq, int n1, int n2, int nt) {
                       FM_DOUBLES + FX_DOUBLES + LG_DOUBLES + 2 * cells_guarded_size(nt) * 2 + 2 * nq + 2 * n2);
 }
 
+// ---- 3-D vertex dressing table (dfrg_table3d): device-side look-up, used by the product-grid kernels below and by
+// t3d_kernel further down ----
+struct Tab3DParams {
+  int n[3];
+  int is_log[3];
+  double lo[3], inv_h[3];
+};
+struct ThreePoint3DParams {
+  ThreePointParams B;   // L3 unused
+  Tab3DParams T;
+  const double* v3;
+};
+constexpr int T3D_MAX_TABLE = 12288;  // doubles (96 KB of shared memory)
+
+__device__ __forceinline__ double tab3d_eval(const double* __restrict__ v, const Tab3DParams& T, const FastMath& fm,
+                                             const double x0, const double x1, const double x2) {
+  const double x[3] = {x0, x1, x2};
+  int i[3];
+  double tau[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const double c = T.is_log[a] ? 0.5 * fm_log(fm, x[a]) : x[a];
+    double t = (c - T.lo[a]) * T.inv_h[a];
+    t = clamp_lo(t, 0.0);  // NaN -> 0
+    t = clamp_hi(t, (double)(T.n[a] - 1));
+    int ii = (int)t;
+    ii = min(ii, T.n[a] - 2);
+    i[a] = ii;
+    tau[a] = t - (double)ii;
+  }
+  const int s1 = T.n[2], s0 = T.n[1] * T.n[2];
+  const double* b = v + (i[0] * s0 + i[1] * s1 + i[2]);
+  // lerp along axis 2, then 1, then 0
+  const double v00 = fma(tau[2], b[1] - b[0], b[0]);
+  const double v01 = fma(tau[2], b[s1 + 1] - b[s1], b[s1]);
+  const double v10 = fma(tau[2], b[s0 + 1] - b[s0], b[s0]);
+  const double v11 = fma(tau[2], b[s0 + s1 + 1] - b[s0 + s1], b[s0 + s1]);
+  const double w0 = fma(tau[1], v01 - v00, v00);
+  const double w1 = fma(tau[1], v11 - v10, v10);
+  return fma(tau[0], w1 - w0, w0);
+}
+
+// lambda3 at the vertex with squared leg momenta (k1, k2, k3):  S0^2 = (k1+k2+k3)/6, a = sqrt3 (k2-k1)/(6 S0^2),
+// s = (k1+k2-2 k3)/(6 S0^2);  S0 = 0: a = s = 0.
+__device__ __forceinline__ double tab3d_vertex(const double* __restrict__ v, const Tab3DParams& T, const FastMath& fm,
+                                               const double k1, const double k2, const double k3) {
+  const double six = k1 + k2 + k3;
+  const double r = six > 0.0 ? fast_rcp(six) : 0.0;
+  return tab3d_eval(v, T, fm, six * (1.0 / 6.0), 1.7320508075688772 * (k2 - k1) * r, (k1 + k2 - 2.0 * k3) * r);
+}
+
 // =====================================================================================================
 // three-point on a product grid of external momenta
 // =====================================================================================================
@@ -522,6 +573,9 @@ struct ThreeGridParams {
   int* flag;       // [1]   != 0: the layout promise does not hold
   double* part;    // [max_slots][n_ext]
   double* partB;   // [max_slots][S]  min over the slot's nodes of D_b
+  Tab3DParams T3;  // TAB3D instantiations: lambda3(S0^2, a, s) instead of the 1-D table
+  const double* v3;
+  int ntab3;
 };
 
 constexpr int T3G_THREADS = 256;
@@ -532,7 +586,7 @@ constexpr int T3G_MAXT = 512;   // threads of the main kernel (126 registers eac
 struct T3GShared {
   double *sxq, *swq, *sx1, *sw1, *sx2, *sw2, *sZA, *sL3, *skap, *fmmem, *fxmem, *lgmem;
   double2 *cZA_all, *cL3_all, *qtab, *xw2, *nodeA;
-  double *nodeZ, *red;
+  double *nodeZ, *red, *stab3;
 };
 __device__ __forceinline__ T3GShared t3g_carve(unsigned char* raw, int nq, int n1, int n2, int nt) {
   T3GShared s;
@@ -555,15 +609,16 @@ __device__ __forceinline__ T3GShared t3g_carve(unsigned char* raw, int nq, int n
   s.nodeA = s.xw2 + n2;                                          // [2][T3G_NODES]
   s.nodeZ = reinterpret_cast<double*>(s.nodeA + 2 * T3G_NODES);  // [2][T3G_NODES]
   s.red = s.nodeZ + 2 * T3G_NODES;                               // [T3G_MAXT]
+  s.stab3 = s.red + T3G_MAXT;                                    // [ntab3]  (TAB3D only)
   return s;
 }
-static size_t t3g_smem(int nq, int n1, int n2, int nt) {
+static size_t t3g_smem(int nq, int n1, int n2, int nt, int ntab3 = 0) {
   return 8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((n1 + 1) & ~1) + 2 * ((n2 + 1) & ~1) + 2 * ((nt + 1) & ~1) + 36 +
                       FM_DOUBLES + FX_DOUBLES + LG_DOUBLES + 2 * cells_guarded_size(nt) * 2 + 2 * nq + 2 * n2 +
-                      2 * 2 * T3G_NODES + 2 * T3G_NODES + T3G_MAXT);
+                      2 * 2 * T3G_NODES + 2 * T3G_NODES + T3G_MAXT + ((ntab3 + 1) & ~1));
 }
 
-template <int REGK>
+template <int REGK, bool TAB3D>
 __global__ void __launch_bounds__(T3G_THREADS, 1) t3g_prepass_kernel(const ThreeGridParams Q) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar;
@@ -578,7 +633,8 @@ __global__ void __launch_bounds__(T3G_THREADS, 1) t3g_prepass_kernel(const Three
     StageList L;
     L.add(sm.sxq, P.xq, nq); L.add(sm.swq, P.wq, nq);
     L.add(sm.sx1, P.x1, n1); L.add(sm.sw1, P.w1, n1);
-    L.add(sm.sZA, P.ZA, nt); L.add(sm.sL3, P.L3, nt);
+    L.add(sm.sZA, P.ZA, nt);
+    if (TAB3D) L.add(sm.stab3, Q.v3, Q.ntab3); else L.add(sm.sL3, P.L3, nt);
     stage_to_smem(L, &bar, 0);
   }
   const FastMath fm = fm_build(sm.fmmem, P.fmc);
@@ -586,7 +642,7 @@ __global__ void __launch_bounds__(T3G_THREADS, 1) t3g_prepass_kernel(const Three
   const LogGrid lg = lg_build(sm.lgmem, P.grid.lo, P.grid.inv_h, nt);
   const double* kc = P.fmc.c;
   const double2* cZA = cells_build_guarded(sm.cZA_all, sm.sZA, nt, P.grid.interp);
-  const double2* cL3 = cells_build_guarded(sm.cL3_all, sm.sL3, nt, P.grid.interp);
+  const double2* cL3 = TAB3D ? nullptr : cells_build_guarded(sm.cL3_all, sm.sL3, nt, P.grid.interp);
   if (threadIdx.x < 35) sm.skap[threadIdx.x] = P.coef[threadIdx.x];
   __syncthreads();
 
@@ -631,7 +687,8 @@ __global__ void __launch_bounds__(T3G_THREADS, 1) t3g_prepass_kernel(const Three
     s_a = clamp_lo(s_a, 0.0);
     const double Da = fma(lg_lookup(cZA, lg, kc, s_a), s_a, t3_reg_R<REGK>(P.reg, fxtab, kc, s_a));
     const double Ga = fast_rcp(Da);
-    const double lam1 = lg_lookup(cL3, lg, kc, (p1 * p1 + sq + s_a) * third);
+    const double lam1 = TAB3D ? tab3d_vertex(sm.stab3, Q.T3, fm, p1 * p1, sq, s_a)
+                              : lg_lookup(cL3, lg, kc, (p1 * p1 + sq + s_a) * third);
     const double X = sq * ik2, Y = qp1 * ik2;
     double gam[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     {
@@ -651,14 +708,14 @@ __global__ void __launch_bounds__(T3G_THREADS, 1) t3g_prepass_kernel(const Three
     }
     double* ta = Q.tabA + ((size_t)pair * 8) * G + a;
     ta[0] = wpair * (Ga * lam1);
-    ta[(size_t)G] = s_a * third;
+    ta[(size_t)G] = TAB3D ? s_a : s_a * third;
 #pragma unroll
     for (int c = 0; c < 5; ++c) ta[(size_t)(2 + c) * G] = gam[c];
     ta[(size_t)7 * G] = Da;
   }
 }
 
-template <int REGK, int NT, int UNR>
+template <int REGK, int NT, int UNR, bool TAB3D>
 __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ __align__(8) uint64_t bar;
@@ -677,14 +734,16 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
     L.add(sm.sxq, P.xq, nq);
     L.add(sm.sx1, P.x1, n1);
     L.add(sm.sx2, P.x2, n2); L.add(sm.sw2, P.w2, n2);
-    L.add(sm.sZA, P.ZA, nt); L.add(sm.sL3, P.L3, nt);
+    L.add(sm.sZA, P.ZA, nt);
+    if (TAB3D) L.add(sm.stab3, Q.v3, Q.ntab3); else L.add(sm.sL3, P.L3, nt);
     stage_to_smem(L, &bar, 0);
   }
+  const FastMath fm = fm_build(sm.fmmem, P.fmc);   // the S0 axis of the 3-D table (TAB3D)
   const double* fxtab = fx_build(sm.fxmem, P.reg.zk * P.reg.k2);
   const LogGrid lg = lg_build(sm.lgmem, P.grid.lo, P.grid.inv_h, nt);
   const double* kc = P.fmc.c;
   const double2* cZA = cells_build_guarded(sm.cZA_all, sm.sZA, nt, P.grid.interp);
-  const double2* cL3 = cells_build_guarded(sm.cL3_all, sm.sL3, nt, P.grid.interp);
+  const double2* cL3 = TAB3D ? nullptr : cells_build_guarded(sm.cL3_all, sm.sL3, nt, P.grid.interp);
   for (int j = tid; j < n2; j += NT) sm.xw2[j] = make_double2(sm.sx2[j], sm.sw2[j]);
   __syncthreads();
 
@@ -722,8 +781,9 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
       s_b = clamp_lo(s_b, 0.0);
       const double Db = fma(lg_lookup(cZA, lg, kc, s_b), s_b, t3_reg_R<REGK>(P.reg, fxtab, kc, s_b));
       dmB = fmin(dmB, Db);
-      const double lam2 = lg_lookup(cL3, lg, kc, fma(s_b, third, sb0 * third));
-      nA[n] = make_double2(xw.y * (fast_rcp(Db) * lam2), s_b * third);
+      const double lam2 = TAB3D ? tab3d_vertex(sm.stab3, Q.T3, fm, p2 * p2, sq, s_b)
+                                : lg_lookup(cL3, lg, kc, fma(s_b, third, sb0 * third));
+      nA[n] = make_double2(xw.y * (fast_rcp(Db) * lam2), TAB3D ? s_b : s_b * third);
       nZ[n] = z;
     }
   };
@@ -766,7 +826,8 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
         for (int j2 = 0; j2 < n2; ++j2) {
           const double2 bs = na[j2];
           const double z = nz[j2];
-          const double lam3 = lg_lookup(cL3, lg, kc, bs.y + l30);
+          const double lam3 = TAB3D ? tab3d_vertex(sm.stab3, Q.T3, fm, scc, cur[1], bs.y)
+                                    : lg_lookup(cL3, lg, kc, bs.y + l30);
           const double poly = fma(fma(fma(fma(cur[6], z, cur[5]), z, cur[4]), z, cur[3]), z, cur[2]);
           acc2 = fma(bs.x * poly, lam3, acc2);
         }
@@ -828,55 +889,6 @@ __global__ void __launch_bounds__(256) t3g_fixup_kernel(const ThreeGridParams Q)
 // lambda3(S0^2, a, s) (the paper's 96 x 8 x 7 vertex grids): the whole table sits in
 // shared memory (43 KB for 96 x 8 x 7), a look-up gathers its 8 corners with plain 64-bit loads -- the first family
 // whose table traffic competes with the arithmetic.  The vertex at (p1, q, q+p1) is hoisted out of the c2 loop.
-struct Tab3DParams {
-  int n[3];
-  int is_log[3];
-  double lo[3], inv_h[3];
-};
-struct ThreePoint3DParams {
-  ThreePointParams B;   // L3 unused
-  Tab3DParams T;
-  const double* v3;
-};
-constexpr int T3D_MAX_TABLE = 12288;  // doubles (96 KB of shared memory)
-
-__device__ __forceinline__ double tab3d_eval(const double* __restrict__ v, const Tab3DParams& T, const FastMath& fm,
-                                             const double x0, const double x1, const double x2) {
-  const double x[3] = {x0, x1, x2};
-  int i[3];
-  double tau[3];
-#pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    const double c = T.is_log[a] ? 0.5 * fm_log(fm, x[a]) : x[a];
-    double t = (c - T.lo[a]) * T.inv_h[a];
-    t = clamp_lo(t, 0.0);  // NaN -> 0
-    t = clamp_hi(t, (double)(T.n[a] - 1));
-    int ii = (int)t;
-    ii = min(ii, T.n[a] - 2);
-    i[a] = ii;
-    tau[a] = t - (double)ii;
-  }
-  const int s1 = T.n[2], s0 = T.n[1] * T.n[2];
-  const double* b = v + (i[0] * s0 + i[1] * s1 + i[2]);
-  // lerp along axis 2, then 1, then 0
-  const double v00 = fma(tau[2], b[1] - b[0], b[0]);
-  const double v01 = fma(tau[2], b[s1 + 1] - b[s1], b[s1]);
-  const double v10 = fma(tau[2], b[s0 + 1] - b[s0], b[s0]);
-  const double v11 = fma(tau[2], b[s0 + s1 + 1] - b[s0 + s1], b[s0 + s1]);
-  const double w0 = fma(tau[1], v01 - v00, v00);
-  const double w1 = fma(tau[1], v11 - v10, v10);
-  return fma(tau[0], w1 - w0, w0);
-}
-
-// lambda3 at the vertex with squared leg momenta (k1, k2, k3):  S0^2 = (k1+k2+k3)/6, a = sqrt3 (k2-k1)/(6 S0^2),
-// s = (k1+k2-2 k3)/(6 S0^2);  S0 = 0: a = s = 0.
-__device__ __forceinline__ double tab3d_vertex(const double* __restrict__ v, const Tab3DParams& T, const FastMath& fm,
-                                               const double k1, const double k2, const double k3) {
-  const double six = k1 + k2 + k3;
-  const double r = six > 0.0 ? fast_rcp(six) : 0.0;
-  return tab3d_eval(v, T, fm, six * (1.0 / 6.0), 1.7320508075688772 * (k2 - k1) * r, (k1 + k2 - 2.0 * k3) * r);
-}
-
 static size_t t3d_smem(int nq, int n1, int n2, int nt, int ntab3) {
   return 8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((n1 + 1) & ~1) + 2 * ((n2 + 1) & ~1) + ((nt + 1) & ~1) + 36 +
                       FM_DOUBLES + FX_DOUBLES + LG_DOUBLES + cells_guarded_size(nt) * 2 + 2 * nq + 2 * n2 +
@@ -891,6 +903,7 @@ __global__ void __launch_bounds__(256, 1) t3d_kernel(const ThreePoint3DParams Q)
   constexpr int NT = 256;
   const ThreePointParams& P = Q.B;
   const Tab3DParams& T = Q.T;
+  if (P.skip_flag && *P.skip_flag == 0) return;   // the product-grid kernels did the work
   const int nq = P.nq, n1 = P.n1, n2 = P.n2, nt = P.grid.n;
   const int ntab3 = T.n[0] * T.n[1] * T.n[2];
   double* sxq = reinterpret_cast<double*>(smem_raw);
@@ -1304,6 +1317,64 @@ static void fill_common(const dfrg_regulator& r, const dfrg_table& t, RegParams*
   gp->lo = t.lnq_lo; gp->inv_h = (double)(t.n_q - 1) / (t.lnq_hi - t.lnq_lo); gp->n = t.n_q; gp->interp = t.interp;
 }
 
+// Enqueues the product-grid kernels if the caller promised a product grid (G >= 2) and the shapes allow it; then
+// P.skip_flag points at the device flag the general kernel must consult.  T3 != nullptr: 3-D vertex table.
+static int t3g_launch(ThreePointParams& P, int G, int regk, const Tab3DParams* T3, const double* v3, int ntab3,
+                      int sm_count, cudaStream_t stream, void** scratch_out) {
+  const int n_ext = P.n_ext;
+  if (!(G >= 2 && G <= 256 && n_ext % G == 0 && P.n2 <= T3G_NODES)) return DFRG_OK;
+  const size_t smem_g = t3g_smem(P.nq, P.n1, P.n2, P.grid.n, T3 ? ntab3 : 0);
+  if (smem_g > 227 * 1024) return DFRG_OK;   // (large 3-D tables: the general kernel)
+  ThreeGridParams Q;
+  Q.B = P;
+  Q.G = G; Q.S = n_ext / G;
+  Q.v3 = v3; Q.ntab3 = ntab3;
+  if (T3) Q.T3 = *T3;
+  const int npairs = P.nq * P.n1;
+  Q.KP = T3G_NODES / P.n2 < npairs ? T3G_NODES / P.n2 : npairs;
+  Q.NCH = (npairs + Q.KP - 1) / Q.KP;
+  const long long U = (long long)Q.S * Q.NCH;
+  Q.grid_main = (int)(U < sm_count ? U : sm_count);
+  Q.max_slots = 1;
+  for (int r = 0; r < Q.S; ++r) {
+    const long long ufirst = (long long)r * Q.NCH, ulast = ufirst + Q.NCH - 1;
+    const int c0 = (int)(((ufirst + 1) * Q.grid_main - 1) / U), c1 = (int)(((ulast + 1) * Q.grid_main - 1) / U);
+    if (c1 - c0 + 1 > Q.max_slots) Q.max_slots = c1 - c0 + 1;
+  }
+  const size_t n_tabA = (size_t)npairs * 8 * G, n_tabR = 4 * (size_t)Q.S, n_part = (size_t)Q.max_slots * n_ext,
+               n_partB = (size_t)Q.max_slots * Q.S;
+  void* scratch = nullptr;
+  int rc = scratch_alloc(&scratch, (n_tabA + n_tabR + n_part + n_partB + 4) * sizeof(double), stream);
+  if (rc != DFRG_OK) return rc;
+  *scratch_out = scratch;
+  Q.tabA = (double*)scratch;
+  Q.tabR = Q.tabA + n_tabA;
+  Q.part = Q.tabR + n_tabR;
+  Q.partB = Q.part + n_part;
+  Q.qmin = Q.partB + n_partB;
+  Q.flag = (int*)(Q.qmin + 2);
+  cudaError_t e = cudaMemsetAsync(Q.flag, 0, sizeof(int), stream);
+  void (*kpre)(const ThreeGridParams) = nullptr;
+  void (*kmain)(const ThreeGridParams) = nullptr;
+#define DFRG_T3G_PICK(K)                                                                                  \
+  if (regk == K) {                                                                                        \
+    kpre = T3 ? t3g_prepass_kernel<K, true> : t3g_prepass_kernel<K, false>;                               \
+    kmain = T3 ? t3g_main_kernel<K, T3G_MAXT, 8, true> : t3g_main_kernel<K, T3G_MAXT, 8, false>;          \
+  }
+  DFRG_T3G_PICK(0) DFRG_T3G_PICK(1) DFRG_T3G_PICK(2)
+#undef DFRG_T3G_PICK
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(kpre, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(kmain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g);
+  if (e != cudaSuccess) { scratch_free(scratch, stream); *scratch_out = nullptr; return check_cuda(e); }
+  kpre<<<sm_count, T3G_THREADS, smem_g, stream>>>(Q);
+  kmain<<<Q.grid_main, T3G_MAXT, smem_g, stream>>>(Q);
+  t3g_fixup_kernel<<<(n_ext + 255) / 256, 256, 0, stream>>>(Q);
+  rc = check_cuda(cudaGetLastError());
+  if (rc != DFRG_OK) { scratch_free(scratch, stream); *scratch_out = nullptr; return rc; }
+  P.skip_flag = Q.flag;
+  return DFRG_OK;
+}
+
 static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext, const double* ext,
                          double* out, double* dmin, int sm_count, cudaStream_t stream) {
   if (D->family == DFRG_LOOP_TWOPOINT) {
@@ -1414,59 +1485,29 @@ static int loop4d_launch(const dfrg_loop4d_desc* D, int n_field, const double* m
     const size_t smem3 = t3d_smem(P.nq, P.n1, P.n2, P.grid.n, ntab3);
     if (smem3 > 227 * 1024) return DFRG_EUNSUPPORTED;
     const int regk3 = D->reg.kind == DFRG_REG_LITIM ? 0 : (D->reg.order == 1 ? 1 : 2);
+    void* scratch3 = nullptr;
+    {  // product grid promised (ext_outer): share the |p1|-only and (|p2|, alpha)-only vertices as the 1-D family does
+      const int rcg = t3g_launch(Q3.B, D->ext_outer, regk3, &Q3.T, Q3.v3, ntab3, sm_count, stream, &scratch3);
+      if (rcg != DFRG_OK) return rcg;
+    }
     void (*k3)(const ThreePoint3DParams) = nullptr;
 #define DFRG_T3D_PICK(K) if (regk3 == K) k3 = dmin ? t3d_kernel<K, true> : t3d_kernel<K, false>;
     DFRG_T3D_PICK(0) DFRG_T3D_PICK(1) DFRG_T3D_PICK(2)
 #undef DFRG_T3D_PICK
     cudaError_t e3 = cudaFuncSetAttribute(k3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem3);
-    if (e3 != cudaSuccess) return check_cuda(e3);
+    if (e3 != cudaSuccess) { scratch_free(scratch3, stream); return check_cuda(e3); }
     const int grid3 = n_ext < sm_count ? n_ext : sm_count;
     k3<<<grid3, 256, smem3, stream>>>(Q3);
-    return check_cuda(cudaGetLastError());
+    const int rc3 = check_cuda(cudaGetLastError());
+    scratch_free(scratch3, stream);
+    return rc3;
   }
   const int regk = D->reg.kind == DFRG_REG_LITIM ? 0 : (D->reg.order == 1 ? 1 : 2);
   void* scratch = nullptr;
   // ---- product-grid path (ext_outer = G promised by the caller, checked on the device) ----
-  const int G = D->ext_outer;
-  if (G >= 2 && G <= 256 && n_ext % G == 0 && P.n2 <= T3G_NODES) {
-    ThreeGridParams Q;
-    Q.B = P;
-    Q.G = G; Q.S = n_ext / G;
-    const int npairs = P.nq * P.n1;
-    Q.KP = T3G_NODES / P.n2 < npairs ? T3G_NODES / P.n2 : npairs;
-    Q.NCH = (npairs + Q.KP - 1) / Q.KP;
-    const long long U = (long long)Q.S * Q.NCH;
-    Q.grid_main = (int)(U < sm_count ? U : sm_count);
-    Q.max_slots = 1;
-    for (int r = 0; r < Q.S; ++r) {
-      const long long ufirst = (long long)r * Q.NCH, ulast = ufirst + Q.NCH - 1;
-      const int c0 = (int)(((ufirst + 1) * Q.grid_main - 1) / U), c1 = (int)(((ulast + 1) * Q.grid_main - 1) / U);
-      if (c1 - c0 + 1 > Q.max_slots) Q.max_slots = c1 - c0 + 1;
-    }
-    const size_t n_tabA = (size_t)npairs * 8 * G, n_tabR = 4 * (size_t)Q.S, n_part = (size_t)Q.max_slots * n_ext,
-                 n_partB = (size_t)Q.max_slots * Q.S;
-    int rc = scratch_alloc(&scratch, (n_tabA + n_tabR + n_part + n_partB + 4) * sizeof(double), stream);
-    if (rc != DFRG_OK) return rc;
-    Q.tabA = (double*)scratch;
-    Q.tabR = Q.tabA + n_tabA;
-    Q.part = Q.tabR + n_tabR;
-    Q.partB = Q.part + n_part;
-    Q.qmin = Q.partB + n_partB;
-    Q.flag = (int*)(Q.qmin + 2);
-    cudaError_t e = cudaMemsetAsync(Q.flag, 0, sizeof(int), stream);
-    const size_t smem_g = t3g_smem(P.nq, P.n1, P.n2, P.grid.n);
-    void (*kpre)(const ThreeGridParams) = regk == 0 ? t3g_prepass_kernel<0> : (regk == 1 ? t3g_prepass_kernel<1> : t3g_prepass_kernel<2>);
-    void (*kmain)(const ThreeGridParams) = regk == 0 ? t3g_main_kernel<0, T3G_MAXT, 8> : (regk == 1 ? t3g_main_kernel<1, T3G_MAXT, 8> : t3g_main_kernel<2, T3G_MAXT, 8>);
-    const int nt_main = T3G_MAXT;
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(kpre, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(kmain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_g);
-    if (e != cudaSuccess) { scratch_free(scratch, stream); return check_cuda(e); }
-    kpre<<<sm_count, T3G_THREADS, smem_g, stream>>>(Q);
-    kmain<<<Q.grid_main, nt_main, smem_g, stream>>>(Q);
-    t3g_fixup_kernel<<<(n_ext + 255) / 256, 256, 0, stream>>>(Q);
-    rc = check_cuda(cudaGetLastError());
-    if (rc != DFRG_OK) { scratch_free(scratch, stream); return rc; }
-    P.skip_flag = Q.flag;  // the general kernel below runs only if the promise turned out false
+  {
+    const int rc = t3g_launch(P, D->ext_outer, regk, nullptr, nullptr, 0, sm_count, stream, &scratch);
+    if (rc != DFRG_OK) return rc;   // P.skip_flag is set if the product-grid kernels were enqueued
   }
   const size_t smem = threepoint_v2_smem(P.nq, P.n1, P.n2, P.grid.n);
   void (*kern)(const ThreePointParams) = nullptr;

@@ -177,7 +177,7 @@ def config6(n_p=32, n_alpha=8, n_q=96, n_c1=32, n_c2=16, n_phi=16, n_tab=128, n3
     c1, c2, c3 = 0.3 * (U[5] - 0.5), 0.3 * (U[6] - 0.5), 0.3 * (U[7] - 0.5)
     v3 = X[:, None, None] * (1.0 + c1 * a[None, :, None] ** 2 + c2 * s_[None, None, :] + c3 * a[None, :, None] * s_[None, None, :])
     c.update(name="cfg6_threepoint3d", family=3, v3=np.ascontiguousarray(v3), lo3=(lo, -1.0, -1.0), hi3=(hi, 1.0, 1.0),
-             log3=(1, 0, 0), ext_outer=0)
+             log3=(1, 0, 0))   # ext_outer = n_p from config 3: the externals are a product grid
     del c["L3"], c["Zc"]
     return c
 

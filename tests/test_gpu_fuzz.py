@@ -47,6 +47,8 @@ def draw(rng):
                            n_c1=int(rng.integers(1, 8)), n_c2=int(rng.integers(1, 6)),
                            n3=(int(rng.integers(2, 40)), int(rng.integers(2, 9)), int(rng.integers(2, 9))),
                            interp=int(pick(rng, 1, 3)))
+        if rng.integers(2):
+            c["ext_outer"] = 0
     else:
         n_jext = int(pick(rng, 1, 2, 3, 5, 8, 16, 17, 33))
         n_max = int(pick(rng, 0, 1, 2, 3, 7, 11))

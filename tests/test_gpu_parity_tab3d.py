@@ -30,7 +30,19 @@ def both(c, sel=None, host=False):
                                    dict(n_p=14, n_alpha=12, n_q=7, n_c1=5, n_c2=3, n3=(33, 5, 9)),     # more outputs than SMs
                                    dict(n_p=2, n_alpha=2, n_q=40, n_c1=9, n_c2=6, n3=(128, 12, 8))])   # 12288-entry table
 def test_tab3d_small(shape):
-    both(inputs.config6(**shape))
+    c = inputs.config6(**shape)
+    g, _, _ = both(c)                               # product-grid kernels (ext_outer = n_p, checked on the device)
+    c["ext_outer"] = 0
+    g0, _, _ = both(c)                              # general kernel
+    if int(np.prod(shape["n3"])) <= 6000:           # (larger tables do not fit beside the product-grid tables: general kernel)
+        assert not np.array_equal(g["out"], g0["out"]) or g["out"].size <= 2
+    c["ext_outer"] = shape["n_p"]
+    c["ext"] = c["ext"].copy()
+    c["ext"][-1, 1] *= 1.5                          # the promise is broken: the device check must send it to the general kernel
+    gb, _, _ = both(c)
+    c["ext_outer"] = 0
+    gb0, _, _ = both(c)
+    assert np.array_equal(gb["out"], gb0["out"])
 
 
 def test_tab3d_regulators_coordinate_packs_host_and_edges():
@@ -52,6 +64,7 @@ def test_tab3d_regulators_coordinate_packs_host_and_edges():
     h, _, _ = both(c, host=True)
     assert np.array_equal(g["out"], h["out"])
     c = inputs.config6(n_p=1, n_alpha=1, n_q=12, n_c1=6, n_c2=4)
+    c["ext_outer"] = 0
     c["ext"] = np.array([[0.0, 0.0, 1.0], [1e-5, 1e3, 0.0], [2.0, 2.0, np.pi]])     # S0 -> 0, far off the table, p2 = -p1
     both(c)
 
