@@ -1000,6 +1000,39 @@ struct cplx_t { double re, im; };
 __device__ __forceinline__ cplx_t cmul(const cplx_t a, const cplx_t b) {
   cplx_t r; r.re = a.re * b.re - a.im * b.im; r.im = a.re * b.im + a.im * b.re; return r;
 }
+// JB consecutive j of one side of row m, complex:  acc[j0+t] += H(n0+t) (beta'[j0+t][n0+t] . M), H(n < 0) = conj H(nbar);
+// stage-wise (loads, then 2 JB independent chains).  b: first beta' entry (re, then im), bstride in double4 per j.
+template <int JB, int NJ>
+__device__ __forceinline__ void gm_cpair_block(const double4* __restrict__ b, const int bstride,
+                                               const double* __restrict__ H, const int hstride, const int n0,
+                                               const double (&M)[4][1], double (&accr)[NJ], double (&acci)[NJ],
+                                               const int j0) {
+  double4 Br[JB], Bi[JB];
+  double hr[JB], hi[JB], tr[JB], ti[JB];
+#pragma unroll
+  for (int q = 0; q < JB; ++q) {
+    Br[q] = b[q * bstride];
+    Bi[q] = b[q * bstride + 1];
+    const int n = n0 + q, nbar = n >= 0 ? n : -n - 1;
+    hr[q] = H[(size_t)nbar * hstride];
+    const double him = H[(size_t)nbar * hstride + 1];
+    hi[q] = n >= 0 ? him : -him;
+  }
+#pragma unroll
+  for (int q = 0; q < JB; ++q) { tr[q] = Br[q].x * M[0][0]; ti[q] = Bi[q].x * M[0][0]; }
+#pragma unroll
+  for (int q = 0; q < JB; ++q) { tr[q] = fma(Br[q].y, M[1][0], tr[q]); ti[q] = fma(Bi[q].y, M[1][0], ti[q]); }
+#pragma unroll
+  for (int q = 0; q < JB; ++q) { tr[q] = fma(Br[q].z, M[2][0], tr[q]); ti[q] = fma(Bi[q].z, M[2][0], ti[q]); }
+#pragma unroll
+  for (int q = 0; q < JB; ++q) { tr[q] = fma(Br[q].w, M[3][0], tr[q]); ti[q] = fma(Bi[q].w, M[3][0], ti[q]); }
+#pragma unroll
+  for (int q = 0; q < JB; ++q) {
+    accr[j0 + q] = fma(hr[q], tr[q], fma(-hi[q], ti[q], accr[j0 + q]));
+    acci[j0 + q] = fma(hr[q], ti[q], fma(hi[q], tr[q], acci[j0 + q]));
+  }
+}
+
 template <int NJ, bool SYM>
 __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dParams P) {
   constexpr int NTC = 256, MF = 1;
@@ -1165,22 +1198,28 @@ __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dPara
       // ---- the (j, n) pairs with |j - n| = m ----
       const int jlo1 = max(0, m - n_max), jhi1 = min(n_jext - 1, n_max + m);
       const int jhi2 = m > 0 ? min(n_jext - 1, n_max - m) : -1;
+      const double4* brow1 = bet4 + 2 * (n_max - m);   // entry (j, n = j - m) at brow1[2 j (NT + 1)] (re), +1 (im)
+      const double4* brow2 = bet4 + 2 * (n_max + m);
+      constexpr int JB = NJ < 4 ? NJ : 4;
 #pragma unroll
-      for (int j = 0; j < NJ; ++j) {
+      for (int j0 = 0; j0 < NJ; j0 += JB) {
+        if (j0 >= jlo1 && j0 + JB - 1 <= jhi1) {
+          gm_cpair_block<JB, NJ>(brow1 + 2 * j0 * (NT + 1), 2 * (NT + 1), myH, NTC * 2, j0 - m, M, accr, acci, j0);
+        } else if (j0 <= jhi1 && j0 + JB - 1 >= jlo1) {
 #pragma unroll
-        for (int side = 0; side < 2; ++side) {
-          const bool valid = side == 0 ? (j >= jlo1 && j <= jhi1) : (j <= jhi2);
-          if (valid) {
-            const int n = side == 0 ? j - m : j + m;
-            const int nbar = n >= 0 ? n : -n - 1;
-            const double4 Br = bet4[(j * NT + n + n_max) * 2], Bi = bet4[(j * NT + n + n_max) * 2 + 1];
-            const double hr = myH[(size_t)nbar * NTC * 2];
-            const double hi = n >= 0 ? myH[(size_t)nbar * NTC * 2 + 1] : -myH[(size_t)nbar * NTC * 2 + 1];
-            const double tr = fma(Br.w, M[3][0], fma(Br.z, M[2][0], fma(Br.y, M[1][0], Br.x * M[0][0])));
-            const double ti = fma(Bi.w, M[3][0], fma(Bi.z, M[2][0], fma(Bi.y, M[1][0], Bi.x * M[0][0])));
-            accr[j] = fma(hr, tr, fma(-hi, ti, accr[j]));
-            acci[j] = fma(hr, ti, fma(hi, tr, acci[j]));
-          }
+          for (int jj = 0; jj < JB; ++jj)
+            if (j0 + jj >= jlo1 && j0 + jj <= jhi1)
+              gm_cpair_block<1, NJ>(brow1 + 2 * (j0 + jj) * (NT + 1), 2 * (NT + 1), myH, NTC * 2, j0 + jj - m, M, accr, acci,
+                                    j0 + jj);
+        }
+        if (j0 + JB - 1 <= jhi2) {
+          gm_cpair_block<JB, NJ>(brow2 + 2 * j0 * (NT + 1), 2 * (NT + 1), myH, NTC * 2, j0 + m, M, accr, acci, j0);
+        } else if (j0 <= jhi2) {
+#pragma unroll
+          for (int jj = 0; jj < JB; ++jj)
+            if (j0 + jj <= jhi2)
+              gm_cpair_block<1, NJ>(brow2 + 2 * (j0 + jj) * (NT + 1), 2 * (NT + 1), myH, NTC * 2, j0 + jj + m, M, accr, acci,
+                                    j0 + jj);
         }
       }
     }
