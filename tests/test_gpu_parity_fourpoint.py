@@ -69,8 +69,8 @@ def test_fourpoint_edge_momenta():
     both(c)
 
 
-def test_fourpoint_full_quadrature_sampled_outputs():
-    """BASELINE-sized quadrature (as config 3: 96 x 32 x 16 x 16 = 786 432 distinct nodes per output) on 6 outputs."""
-    c = inputs.config5(n_s=3, n_ang=2)
+def test_fourpoint_full_config5():
+    """The bench workload in full: 128 outputs x 786 432 distinct nodes (quadrature as BASELINE config 3), ~2 s of oracle."""
+    c = inputs.config5()
     _, _, rep = both(c)
-    assert rep["max_rel_regular"] <= 1e-12
+    assert rep["n"] == 128 and rep["max_rel_regular"] <= 1e-12
