@@ -784,7 +784,7 @@ __device__ __forceinline__ void gm_pair_block(const double4* __restrict__ b, con
 // is read from shared memory here: H sits in a thread-private column Hs[nbar][tid] (no synchronisation needed), and the
 // (j, n) pairs of row m are enumerated by two warp-uniform range tests per j
 //     n = j - m:  max(0, m - n_max) <= j <= min(n_jext - 1, n_max + m);     n = j + m (m > 0):  j <= min(n_jext - 1, n_max - m).
-// Cost against the specialised kernel: one LDS per pair and two uniform branches per (j, side) slot.
+// Cost against the specialised kernel: one LDS per pair and two uniform range tests per block of eight j.
 template <int NJ, int MF, int NTC, bool SQ, bool SYM>
 __global__ void __launch_bounds__(NTC, 1) mats3d_gmoment_kernel(const Mats3dParams P) {
   if (P.sym_try && (*P.symflag != 0) != SYM) return;
@@ -950,7 +950,7 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_gmoment_kernel(const Mats3dPara
       const int jhi2 = m > 0 ? min(n_jext - 1, n_max - m) : -1;
       const double4* brow1 = bet4 + (n_max - m);   // entry (j, n = j - m) at brow1[j (NT + 1)]
       const double4* brow2 = bet4 + (n_max + m);   // entry (j, n = j + m) at brow2[j (NT + 1)]
-      constexpr int JB = NJ < 4 ? NJ : 4;          // blocks of JB values of j: one range test per block when it is
+      constexpr int JB = NJ < 8 ? NJ : 8;          // blocks of JB values of j: one range test per block when it is
 #pragma unroll                                     // entirely inside the valid range (stage-wise code: JB x MF chains)
       for (int j0 = 0; j0 < NJ; j0 += JB) {
         if (j0 >= jlo1 && j0 + JB - 1 <= jhi1) {
