@@ -46,8 +46,9 @@ void scratch_shutdown();
 class Arena {
  public:
   int begin(size_t bytes_needed);  // DFRG_OK / DFRG_ENOMEM / DFRG_ECUDA
-  double* put(const double* host, size_t n);
+  double* put(const double* host, size_t n);   // small arrays are gathered in a pinned staging block (see upload())
   double* reserve(size_t n);
+  int upload();                                // one H2D copy of everything put() gathered; call before the launch
   int fetch(double* host, const double* dev, size_t n);  // async D2H
   int finish();                                          // synchronise the arena stream
   cudaStream_t stream() const { return stream_; }
@@ -57,6 +58,8 @@ class Arena {
  private:
   char* base_ = nullptr;
   size_t cap_ = 0, off_ = 0;
+  char* hstage_ = nullptr;                     // pinned mirror of the first hcap_ bytes of the arena
+  size_t hcap_ = 0, up_lo_ = 0, up_hi_ = 0;
   cudaStream_t stream_ = nullptr;
   int status_ = DFRG_OK;
 };

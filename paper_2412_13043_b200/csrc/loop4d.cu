@@ -1570,7 +1570,7 @@ extern "C" int dfrg_integrate_loop4d_host(const dfrg_loop4d_desc* D, int n_field
   double* d_out = A.reserve(ne * nf);
   double* d_dmin = dmin ? A.reserve(ne * nf) : nullptr;
   Dd.dout_dm2 = D->dout_dm2 ? A.reserve(ne * nf) : nullptr;
-  if (A.status() != DFRG_OK) return A.status();
+  if (A.upload() != DFRG_OK) return A.status();
   rc = loop4d_launch(&Dd, n_field, d_m2, n_ext, d_ext, d_out, d_dmin, sms, A.stream());
   if (rc != DFRG_OK) return rc;
   A.fetch(out, d_out, ne * nf);

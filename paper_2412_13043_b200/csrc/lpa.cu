@@ -293,7 +293,7 @@ extern "C" int dfrg_integrate_lpa_host(const dfrg_lpa_desc* D, int n_field, cons
   double* d_chan = chan ? A.reserve(2 * nf) : nullptr;
   double* d_dmin = dmin ? A.reserve(nf) : nullptr;
   Dd.dchan = D->dchan ? A.reserve(2 * nf) : nullptr;
-  if (A.status() != DFRG_OK) return A.status();
+  if (A.upload() != DFRG_OK) return A.status();
   rc = lpa_launch(&Dd, n_field, d_rho, d_u, d_du, d_flow, d_chan, d_dmin, A.stream());
   if (rc != DFRG_OK) return rc;
   A.fetch(flow, d_flow, nf);

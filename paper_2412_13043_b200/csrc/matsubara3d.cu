@@ -265,7 +265,7 @@ extern "C" int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_
   Dd.dout_dm2_psi = D->dout_dm2_psi ? A.reserve(n_out) : nullptr;
   Dd.dout_dm2_phi = D->dout_dm2_phi ? A.reserve(n_out) : nullptr;
   Dd.out_im = D->out_im ? A.reserve(n_out) : nullptr;
-  if (A.status() != DFRG_OK) return A.status();
+  if (A.upload() != DFRG_OK) return A.status();
   rc = mats3d_launch(&Dd, n_field, d_mpsi, d_mphi, n_p, d_p, n_jext, d_out, d_dmin, sms, A.stream());
   if (rc != DFRG_OK) return rc;
   A.fetch(out, d_out, n_out);
