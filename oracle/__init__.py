@@ -20,6 +20,7 @@ from .binding import (  # noqa: F401
     vertex_coords,
     matsubara3d,
     matsubara3d_mu,
+    matsubara3d_mu_dm2,
     lpa_dm2,
     loop4d_twopoint_dm2,
     matsubara3d_dm2,

@@ -91,6 +91,12 @@ def _load():
                                             _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
                                             _dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int,
                                             C.c_longlong, _lp, _dp, _dp, _dp, _dp]
+        _lib.orc_matsubara3d_mu_dm2.argtypes = [C.c_double, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double,
+                                                C.c_double, C.c_double,
+                                                C.c_int, _dp, _dp, C.c_int, _dp, _dp,
+                                                _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
+                                                _dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int,
+                                                C.c_longlong, _lp, _dp, _dp, _dp, _dp, _dp, _dp]
         _lib.orc_lpa_dm2.argtypes = [C.c_int, C.c_double, C.c_int, C.c_int, C.c_double,
                                      C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                      C.c_int, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp]
@@ -322,6 +328,27 @@ def matsubara3d_mu(T, n_max, mu, prefactor, reg_kind, reg_order, k, xq, wq, xc, 
         raise ValueError("orc_matsubara3d_mu: bad arguments")
     out = o_re + 1j * o_im
     return (out, dmin, sens) if want_sens else (out, dmin)
+
+
+def matsubara3d_mu_dm2(T, n_max, mu, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zpsi, Zphi,
+                       lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, zk=1.0, eta=0.0):
+    """Mass derivatives of matsubara3d_mu.  Returns (dpsi, dphi, sens_psi, sens_phi), dpsi / dphi complex128."""
+    xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext = map(
+        _arr, (xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext))
+    nfreq, tnq = Zpsi.shape
+    ns, selp, _keep = _sel(sel)
+    shape = (ns,) if sel is not None else (pext.size, int(n_jext), m2psi.size)
+    a_re, a_im, b_re, b_im, sa, sb = (np.empty(shape) for _ in range(6))
+    rc = _load().orc_matsubara3d_mu_dm2(float(T), int(n_max), float(mu), float(prefactor), int(reg_kind),
+                                        int(reg_order), float(k), float(zk), float(eta),
+                                        int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
+                                        _d(Zpsi), _d(Zphi), int(tnq), int(nfreq), float(lnq_lo), float(lnq_hi),
+                                        int(interp), _d(coef), int(coef.size), int(m2psi.size), _d(m2psi), _d(m2phi),
+                                        int(pext.size), _d(pext), int(n_jext), ns, selp,
+                                        _d(a_re), _d(a_im), _d(b_re), _d(b_im), _d(sa), _d(sb))
+    if rc:
+        raise ValueError("orc_matsubara3d_mu_dm2: bad arguments")
+    return a_re + 1j * a_im, b_re + 1j * b_im, sa, sb
 
 
 # ---- mass derivatives (Jacobian support) ------------------------------------------------------------

@@ -955,6 +955,103 @@ int orc_matsubara3d_mu(double T, int n_max, double mu, double prefactor, int reg
   return 0;
 }
 
+// Mass derivatives of orc_matsubara3d_mu (spatial regulators, any mu), term by term on the same nodes:
+//   dpsi = d out / d m2_psi = C T sum_n sum_q w q^2 Rdot(q^2) (-2 G_psi^3) sum_c w P G_phi
+//   dphi = d out / d m2_phi = C T sum_n sum_q w q^2 Rdot(q^2) G_psi^2 sum_c w P (-G_phi^2)
+// (complex for mu != 0: *_re, *_im).  sens_* as orc_matsubara3d_dm2 with moduli.
+int orc_matsubara3d_mu_dm2(double T, int n_max, double mu, double prefactor, int reg_kind, int reg_order, double k,
+                           double zk, double eta,
+                           int nq, const double* xq, const double* wq,
+                           int nc, const double* xc, const double* wc,
+                           const double* Zpsi, const double* Zphi, int t_nq, int t_nfreq,
+                           double t_lo, double t_hi, int t_interp,
+                           const double* coef, int n_coef,
+                           int n_field, const double* m2psi, const double* m2phi,
+                           int n_p, const double* pext, int n_jext,
+                           long long n_sel, const long long* sel,
+                           double* dpsi_re, double* dpsi_im, double* dphi_re, double* dphi_im,
+                           double* sens_psi, double* sens_phi) {
+  typedef std::complex<double> cd;
+  typedef std::complex<long double> cld;
+  if (n_coef != 20 || nq < 1 || nc < 1 || n_field < 1 || n_p < 1 || n_jext < 1 || k <= 0 || T <= 0) return -1;
+  if (n_max + 1 > t_nfreq || n_jext - 1 + n_max + 1 > t_nfreq) return -1;
+  const double pi = 3.14159265358979323846;
+  const double k2 = k * k;
+  const long long n_out = sel ? n_sel : (long long)n_p * n_jext * n_field;
+#pragma omp parallel for schedule(static)
+  for (long long o = 0; o < n_out; ++o) {
+    const long long flat = sel ? sel[o] : o;
+    const int f = (int)(flat % n_field);
+    const int j = (int)((flat / n_field) % n_jext);
+    const int e = (int)(flat / ((long long)n_field * n_jext));
+    const double p = pext[e];
+    const cd p0j((2.0 * j + 1.0) * pi * T, mu);
+    cld a_psi(0.0L, 0.0L), a_phi(0.0L, 0.0L);
+    acc_t s_psi = 0.0L, s_phi = 0.0L;
+    for (int n = -n_max; n <= n_max; ++n) {
+      const cd p0n((2.0 * n + 1.0) * pi * T, mu);
+      const int nbar = n >= 0 ? n : -n - 1;
+      const int m = j - n;
+      const int mabs = m >= 0 ? m : -m;
+      const double om = 2.0 * pi * (double)m * T;
+      for (int i = 0; i < nq; ++i) {
+        const double q = xq[i];
+        const cd spsi = p0n * p0n + q * q;
+        double Rp, Rdp;
+        regulator(reg_kind, reg_order, k, zk, eta, q * q, &Rp, &Rdp);
+        const cd Dpsi = table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q) * spsi + Rp + m2psi[f];
+        const cd Gpsi = 1.0 / Dpsi;
+        const double condpsi = (std::abs(Dpsi - m2psi[f]) + std::fabs(m2psi[f])) / std::abs(Dpsi);
+        cld c_psi(0.0L, 0.0L), c_phi(0.0L, 0.0L);
+        acc_t sc_psi = 0.0L, sc_phi = 0.0L;
+        for (int jc = 0; jc < nc; ++jc) {
+          const double c = xc[jc];
+          const double r2 = clamp0(p * p + q * q - 2.0 * p * q * c);
+          const double sphi = om * om + r2;
+          double Rb, Rdb;
+          regulator(reg_kind, reg_order, k, zk, eta, r2, &Rb, &Rdb);
+          const double Dphi =
+              table_lookup(Zphi + (size_t)mabs * t_nq, t_nq, t_lo, t_hi, t_interp, r2) * sphi + Rb + m2phi[f];
+          const double Gphi = 1.0 / Dphi;
+          const double condphi = (std::fabs(Dphi - m2phi[f]) + std::fabs(m2phi[f])) / std::fabs(Dphi);
+          const cd y1 = p0n * p0j / k2, y3 = spsi / k2;
+          const double y2 = p * q * c / k2;
+          cd P(0.0, 0.0);
+          double Pabs = 0.0;
+          int idx = 0;
+          for (int a = 0; a <= 3; ++a)
+            for (int b = 0; a + b <= 3; ++b)
+              for (int cc = 0; a + b + cc <= 3; ++cc) {
+                cd mono(coef[idx++], 0.0);
+                for (int t = 0; t < a; ++t) mono *= y1;
+                for (int t = 0; t < b; ++t) mono *= y2;
+                for (int t = 0; t < cc; ++t) mono *= y3;
+                P += mono;
+                Pabs += std::abs(mono);
+              }
+          const cd t_psi = wc[jc] * P * Gphi, t_phi = -wc[jc] * P * Gphi * Gphi;
+          c_psi += cld(t_psi.real(), t_psi.imag());
+          c_phi += cld(t_phi.real(), t_phi.imag());
+          sc_psi += (acc_t)(std::fabs(wc[jc] * Pabs * Gphi) * (1.0 + 3.0 * condpsi + condphi));
+          sc_phi += (acc_t)(std::fabs(wc[jc] * Pabs * Gphi * Gphi) * (1.0 + 2.0 * condpsi + 2.0 * condphi));
+        }
+        const double W = wq[i] * q * q * Rdp;
+        const cd w_psi = -2.0 * W * Gpsi * Gpsi * Gpsi, w_phi = W * Gpsi * Gpsi;
+        a_psi += cld(w_psi.real(), w_psi.imag()) * c_psi;
+        a_phi += cld(w_phi.real(), w_phi.imag()) * c_phi;
+        s_psi += (acc_t)std::abs(w_psi) * sc_psi;
+        s_phi += (acc_t)std::abs(w_phi) * sc_phi;
+      }
+    }
+    const acc_t sc = (acc_t)prefactor * (acc_t)T;
+    dpsi_re[o] = (double)(sc * a_psi.real()); dpsi_im[o] = (double)(sc * a_psi.imag());
+    dphi_re[o] = (double)(sc * a_phi.real()); dphi_im[o] = (double)(sc * a_phi.imag());
+    if (sens_psi) sens_psi[o] = (double)(fabsl(sc) * s_psi);
+    if (sens_phi) sens_phi[o] = (double)(fabsl(sc) * s_phi);
+  }
+  return 0;
+}
+
 // =====================================================================================================
 // Mass derivatives (Jacobian support).  Implicit time-steppers need dR_i/du_j (eq. 27;
 // kernel option "AD"): for the loop integrals that is the derivative of the quadrature

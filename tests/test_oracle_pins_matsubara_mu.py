@@ -131,3 +131,57 @@ def test_matsubara_mu_conjugation_and_mu0_is_real():
     sel = np.array([0, 5, 17, 9])
     s, _, _ = run(c, rq, rc, 0.3, n_max=2, sel=sel)
     assert np.array_equal(s, a.ravel()[sel])
+
+
+# ---- mass derivatives at chemical potential (orc_matsubara3d_mu_dm2) -------------------------------------------
+def _dm2(c, rq, rc, mu, **over):
+    a = dict(c)
+    a.update(over)
+    return oracle.matsubara3d_mu_dm2(a["T"], a["n_max"], mu, a["prefactor"], a["reg_kind"], a["reg_order"], a["k"], *rq, *rc,
+                                     a["Zpsi"], a["Zphi"], a["lnq_lo"], a["lnq_hi"], a["interp"], a["coef"],
+                                     a["m2psi"], a["m2phi"], a["pext"], a["n_jext"], sel=a.get("sel"))
+
+
+def test_matsubara_mu_dm2_vs_finite_differences_of_the_pinned_value_function():
+    """Five-point central differences of orc_matsubara3d_mu (pinned above) in m2_psi and in m2_phi, mu != 0 and mu = 0."""
+    c = inputs.config4(n_field=4, n_p=2, n_jext=3)
+    rq, rc = oracle.gl_rule(10, 0, 10), oracle.gl_rule(6, -1, 1)
+    mpsi, mphi = np.array([0.2, 0.6, 1.1, 2.0]), np.array([0.3, 0.8, 1.5, 3.0])
+    h = 1e-3
+    fd5 = lambda fun: (fun(-2 * h) - 8 * fun(-h) + 8 * fun(h) - fun(2 * h)) / (12 * h)
+    for mu in (0.4, 0.0):
+        dpsi, dphi, spsi, sphi = _dm2(c, rq, rc, mu, n_max=2, m2psi=mpsi, m2phi=mphi)
+        val = lambda dpsi_, dphi_: run(c, rq, rc, mu, n_max=2, m2psi=mpsi + dpsi_, m2phi=mphi + dphi_)[0]
+        fpsi = fd5(lambda t: val(t, 0.0))
+        fphi = fd5(lambda t: val(0.0, t))
+        scale = np.abs(run(c, rq, rc, mu, n_max=2, m2psi=mpsi, m2phi=mphi)[0])
+        assert np.all(np.abs(dpsi - fpsi) <= 1e-8 * (np.abs(dpsi) + scale))
+        assert np.all(np.abs(dphi - fphi) <= 1e-8 * (np.abs(dphi) + scale))
+        assert np.all(spsi >= np.abs(dpsi)) and np.all(sphi >= np.abs(dphi))
+        if mu == 0.0:
+            assert np.all(dpsi.imag == 0) and np.all(dphi.imag == 0)
+
+
+def test_matsubara_mu_dm2_flat_regulator_closed_form():
+    """As test_matsubara_mu_flat_regulator_closed_form: d/dm2_psi (A + m)^-2 = -2 (A + m)^-3, d/dm2_phi (B + m)^-1 = -(B + m)^-2."""
+    k, T, n_max, mu = 1.2, 0.2, 4, 0.5
+    c = inputs.config4(n_field=3, n_p=1, n_jext=3, T_over_k=T / k, k=k)
+    ones = np.ones_like(c["Zpsi"])
+    coef = np.zeros(20)
+    coef[0] = 1.0
+    rq, rc = oracle.gl_rule(16, 0, k), oracle.gl_rule(4, -1, 1)
+    mpsi, mphi = np.array([0.1, 0.7, 2.0]), np.array([0.4, -0.3, 1.5])
+    dpsi, dphi, _, _ = _dm2(c, rq, rc, mu, n_max=n_max, reg_kind=oracle.REG_LITIM, Zpsi=ones, Zphi=ones, coef=coef,
+                            m2psi=mpsi, m2phi=mphi, pext=np.zeros(1), n_jext=3)
+    for j in range(3):
+        for f in range(3):
+            tpsi = tphi = 0.0
+            for n in range(-n_max, n_max + 1):
+                p0n = complex((2 * n + 1) * PI * c["T"], mu)
+                A = p0n * p0n + k * k + mpsi[f]
+                Bq = (2 * PI * (j - n) * c["T"]) ** 2 + k * k + mphi[f]
+                tpsi += -2.0 / (A ** 3 * Bq)
+                tphi += -1.0 / (A ** 2 * Bq ** 2)
+            pref = c["prefactor"] * c["T"] * (2 * k ** 5 / 3) * 2
+            assert abs(dpsi[0, j, f] / (pref * tpsi) - 1) < 1e-12
+            assert abs(dphi[0, j, f] / (pref * tphi) - 1) < 1e-12
