@@ -255,9 +255,12 @@ typedef struct {
                            their difference and is unchanged), so s_psi = (nu_n + i mu)^2 + q^2, y1 = (nu_n + i mu)(nu_j + i mu)/k^2
                            and y3 = s_psi/k^2 are complex and so is the result: out = real part, out_im = imaginary part
                            (out(-mu) = conj out(mu): the paper writes p0f - i mu_q).  dmin = min(|D_psi|, D_phi)/k^2.
-                           Mass derivatives are not available with mu != 0 (DFRG_EUNSUPPORTED); n_jext <= 32 and
+                           The mass derivatives are complex too: dout_dm2_psi / dout_dm2_phi receive the real parts and need
+                           their partners dout_dm2_psi_im / dout_dm2_phi_im (DFRG_EINVAL otherwise).  n_jext <= 32 and
                            128 n_jext (2 n_max + 1) + 4096 (n_max + 1) bytes of shared memory must fit (else DFRG_EUNSUPPORTED). */
   double* out_im;       /* nullable unless mu != 0; output [n_p][n_jext][n_field] (zero-filled when mu == 0) */
+  double* dout_dm2_psi_im; /* imaginary parts of the mass derivatives: nullable unless mu != 0 and the real part is requested; */
+  double* dout_dm2_phi_im; /* zero-filled when mu == 0 */
 } dfrg_mats3d_desc;
 
 int dfrg_integrate_matsubara3d(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi, const double* m2_phi,

@@ -65,7 +65,8 @@ class Mats3dDesc(C.Structure):
     _fields_ = [("T", C.c_double), ("n_max", C.c_int), ("prefactor", C.c_double), ("reg", Regulator),
                 ("q", Rule), ("cos1", Rule), ("tab_psi", Table), ("tab_phi", Table),
                 ("coef", _vp), ("n_coef", C.c_int), ("dout_dm2_psi", _vp), ("dout_dm2_phi", _vp),
-                ("reg_arg4d", C.c_int), ("mu", C.c_double), ("out_im", _vp)]
+                ("reg_arg4d", C.c_int), ("mu", C.c_double), ("out_im", _vp),
+                ("dout_dm2_psi_im", _vp), ("dout_dm2_phi_im", _vp)]
 
 
 class DfrgError(RuntimeError):
@@ -242,21 +243,23 @@ def dfrg_integrate_loop4d_host(family, prefactor, reg_kind, reg_order, k, rule_q
 
 # ---- matsubara3d ----------------------------------------------------------------------------------
 def _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp, coef,
-               device, dpsi=None, dphi=None, reg_zk=1.0, reg_eta=0.0, reg_arg4d=1, mu=0.0, out_im=None):
+               device, dpsi=None, dphi=None, reg_zk=1.0, reg_eta=0.0, reg_arg4d=1, mu=0.0, out_im=None,
+               dpsi_im=None, dphi_im=None):
     return Mats3dDesc(float(T), int(n_max), float(prefactor), Regulator(int(reg_kind), int(reg_order), float(k), float(reg_zk), float(reg_eta)),
                       _rule(rule_q, device), _rule(rule_c, device),
                       _table(Zpsi, lnq_lo, lnq_hi, interp, device), _table(Zphi, lnq_lo, lnq_hi, interp, device),
                       _ptr(coef, device), _n(coef), _ptr(dpsi, device), _ptr(dphi, device),
-                      int(reg_arg4d), float(mu), _ptr(out_im, device))
+                      int(reg_arg4d), float(mu), _ptr(out_im, device), _ptr(dpsi_im, device), _ptr(dphi_im, device))
 
 
 def dfrg_integrate_matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo,
                                lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, out, dmin=None,
-                               dout_dm2_psi=None, dout_dm2_phi=None, reg_zk=1.0, reg_eta=0.0, reg_arg4d=1, mu=0.0, out_im=None):
+                               dout_dm2_psi=None, dout_dm2_phi=None, reg_zk=1.0, reg_eta=0.0, reg_arg4d=1, mu=0.0, out_im=None,
+                               dout_dm2_psi_im=None, dout_dm2_phi_im=None):
     """out: [n_p, n_jext, n_field].  reg_arg4d=0: spatial regulators; mu != 0 (needs reg_arg4d=0 and out_im): complex result,
     out = real part, out_im = imaginary part (include/dfrg.h, dfrg_mats3d_desc::mu)."""
     D = _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp,
-                   coef, True, dout_dm2_psi, dout_dm2_phi, reg_zk, reg_eta, reg_arg4d, mu, out_im)
+                   coef, True, dout_dm2_psi, dout_dm2_phi, reg_zk, reg_eta, reg_arg4d, mu, out_im, dout_dm2_psi_im, dout_dm2_phi_im)
     _check(lib().dfrg_integrate_matsubara3d(C.byref(D), _n(m2psi), _ptr(m2psi, True), _ptr(m2phi, True), _n(pext),
                                             _ptr(pext, True), int(n_jext), _ptr(out, True), _ptr(dmin, True),
                                             _stream()), "dfrg_integrate_matsubara3d")
@@ -265,9 +268,10 @@ def dfrg_integrate_matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, rule
 
 def dfrg_integrate_matsubara3d_host(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo,
                                     lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, out, dmin=None,
-                               dout_dm2_psi=None, dout_dm2_phi=None, reg_zk=1.0, reg_eta=0.0, reg_arg4d=1, mu=0.0, out_im=None):
+                               dout_dm2_psi=None, dout_dm2_phi=None, reg_zk=1.0, reg_eta=0.0, reg_arg4d=1, mu=0.0, out_im=None,
+                               dout_dm2_psi_im=None, dout_dm2_phi_im=None):
     D = _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp,
-                   coef, False, dout_dm2_psi, dout_dm2_phi, reg_zk, reg_eta, reg_arg4d, mu, out_im)
+                   coef, False, dout_dm2_psi, dout_dm2_phi, reg_zk, reg_eta, reg_arg4d, mu, out_im, dout_dm2_psi_im, dout_dm2_phi_im)
     _check(lib().dfrg_integrate_matsubara3d_host(C.byref(D), _n(m2psi), _ptr(m2psi, False), _ptr(m2phi, False),
                                                  _n(pext), _ptr(pext, False), int(n_jext), _ptr(out, False),
                                                  _ptr(dmin, False)), "dfrg_integrate_matsubara3d_host")

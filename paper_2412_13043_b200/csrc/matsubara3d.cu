@@ -40,7 +40,8 @@ static int mats3d_validate(const dfrg_mats3d_desc* D, int n_field, const double*
   if ((D->reg_arg4d != 0 && D->reg_arg4d != 1) || !(D->mu == D->mu)) return DFRG_EINVAL;
   if (D->mu != 0.0) {
     if (D->reg_arg4d != 0 || !D->out_im) return DFRG_EINVAL;   // complex time component: spatial regulators only
-    if (D->dout_dm2_psi || D->dout_dm2_phi || n_jext > 32) return DFRG_EUNSUPPORTED;
+    if ((D->dout_dm2_psi && !D->dout_dm2_psi_im) || (D->dout_dm2_phi && !D->dout_dm2_phi_im)) return DFRG_EINVAL;
+    if (n_jext > 32) return DFRG_EUNSUPPORTED;
   }
   return DFRG_OK;
 }
@@ -167,8 +168,12 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
     P.psi_im = P.part_im + n_part;
     P.psimin_f = P.psi_im + (size_t)n_terms * P.psi_stride;
     P.out_im = D->out_im;
-  } else if (D->out_im) {   // real result: the imaginary part is zero
-    rc = check_cuda(cudaMemsetAsync(D->out_im, 0, (size_t)n_p * n_jext * n_field * sizeof(double), stream));
+  } else {   // real results: the imaginary parts are zero
+    double* const zero_fill[3] = {D->out_im, D->dout_dm2_psi ? D->dout_dm2_psi_im : nullptr,
+                                  D->dout_dm2_phi ? D->dout_dm2_phi_im : nullptr};
+    for (int z = 0; z < 3 && rc == DFRG_OK; ++z)
+      if (zero_fill[z])
+        rc = check_cuda(cudaMemsetAsync(zero_fill[z], 0, (size_t)n_p * n_jext * n_field * sizeof(double), stream));
     if (rc != DFRG_OK) { scratch_free(scratch, stream); return rc; }
   }
 
@@ -184,10 +189,12 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   }
   // one pass for the values, one more for each requested mass derivative (same kernels, mode 1 / 2)
   double* const pass_out[3] = {out, D->dout_dm2_psi, D->dout_dm2_phi};
+  double* const pass_out_im[3] = {D->out_im, D->dout_dm2_psi_im, D->dout_dm2_phi_im};
   for (int mode = 0; mode < 3 && rc == DFRG_OK; ++mode) {
     if (!pass_out[mode]) continue;
     P.mode = mode;
     P.out = pass_out[mode];
+    P.out_im = cplx ? pass_out_im[mode] : nullptr;
     P.dmin = mode == 0 ? dmin : nullptr;
     if (moment) {
       rc = cplx ? mats3d_cmoment_dispatch(P, pl, stream)
@@ -248,7 +255,7 @@ extern "C" int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_
   Arena& A = thread_arena();
   const size_t nf = (size_t)n_field, n_out = (size_t)n_p * n_jext * nf;
   const size_t rows_psi = (size_t)D->n_max + 1, rows_phi = (size_t)n_jext + D->n_max, nt = (size_t)D->tab_psi.n_q;
-  const size_t need = 2 * ((size_t)D->q.n + D->cos1.n) + (rows_psi + rows_phi) * nt + 20 + 2 * nf + n_p + 5 * n_out;
+  const size_t need = 2 * ((size_t)D->q.n + D->cos1.n) + (rows_psi + rows_phi) * nt + 20 + 2 * nf + n_p + 7 * n_out;
   rc = A.begin(need * sizeof(double) + 32 * 256);
   if (rc != DFRG_OK) return rc;
   dfrg_mats3d_desc Dd = *D;
@@ -265,6 +272,8 @@ extern "C" int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_
   Dd.dout_dm2_psi = D->dout_dm2_psi ? A.reserve(n_out) : nullptr;
   Dd.dout_dm2_phi = D->dout_dm2_phi ? A.reserve(n_out) : nullptr;
   Dd.out_im = D->out_im ? A.reserve(n_out) : nullptr;
+  Dd.dout_dm2_psi_im = D->dout_dm2_psi_im ? A.reserve(n_out) : nullptr;
+  Dd.dout_dm2_phi_im = D->dout_dm2_phi_im ? A.reserve(n_out) : nullptr;
   if (A.upload() != DFRG_OK) return A.status();
   rc = mats3d_launch(&Dd, n_field, d_mpsi, d_mphi, n_p, d_p, n_jext, d_out, d_dmin, sms, A.stream());
   if (rc != DFRG_OK) return rc;
@@ -273,5 +282,7 @@ extern "C" int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_
   if (D->dout_dm2_psi) A.fetch(D->dout_dm2_psi, Dd.dout_dm2_psi, n_out);
   if (D->dout_dm2_phi) A.fetch(D->dout_dm2_phi, Dd.dout_dm2_phi, n_out);
   if (D->out_im) A.fetch(D->out_im, Dd.out_im, n_out);
+  if (D->dout_dm2_psi && D->dout_dm2_psi_im) A.fetch(D->dout_dm2_psi_im, Dd.dout_dm2_psi_im, n_out);
+  if (D->dout_dm2_phi && D->dout_dm2_phi_im) A.fetch(D->dout_dm2_phi_im, Dd.dout_dm2_phi_im, n_out);
   return A.finish();
 }

@@ -42,7 +42,7 @@ int mats3d_gmoment_dispatch(Mats3dParams& P, const MomentPlan& pl, cudaStream_t 
 // complex (mu != 0) moment kernel: one field point per thread, NJ = the smallest compiled value >= n_jext
 template <int NJ, bool SYM>
 static int mats3d_cmoment_go(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream) {
-  auto kern = mats3d_cmoment_kernel<NJ, SYM>;
+  auto kern = P.mode == 2 ? mats3d_cmoment_kernel<NJ, SYM, true> : mats3d_cmoment_kernel<NJ, SYM, false>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
   if (e != cudaSuccess) return check_cuda(e);
   kern<<<pl.grid, 256, pl.smem, stream>>>(P);

@@ -1033,7 +1033,7 @@ __device__ __forceinline__ void gm_cpair_block(const double4* __restrict__ b, co
   }
 }
 
-template <int NJ, bool SYM>
+template <int NJ, bool SYM, bool SQ>
 __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dParams P) {
   constexpr int NTC = 256, MF = 1;
   if (P.sym_try && (*P.symflag != 0) != SYM) return;
@@ -1160,13 +1160,19 @@ __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dPara
       const double a = psb[2 * nb] + m2psi[0], bb = psb[2 * nb + 1];
       const double r = fast_rcp(fma(a, a, bb * bb));
       const double gr = a * r, gi = -(bb * r);
-      myH[(size_t)nb * NTC * 2] = gr * gr - gi * gi;
-      myH[(size_t)nb * NTC * 2 + 1] = 2.0 * gr * gi;
+      const double g2r = gr * gr - gi * gi, g2i = 2.0 * gr * gi;
+      if (P.mode == 1) {   // d/dm2_psi: G^2 -> -2 G^3
+        myH[(size_t)nb * NTC * 2] = -2.0 * (g2r * gr - g2i * gi);
+        myH[(size_t)nb * NTC * 2 + 1] = -2.0 * (g2r * gi + g2i * gr);
+      } else {
+        myH[(size_t)nb * NTC * 2] = g2r;
+        myH[(size_t)nb * NTC * 2 + 1] = g2i;
+      }
     }
     const bool pipelined = (nc % (2 * M3_NBAT)) == 0;
     const int l_last = NROWS * nc - M3_NBAT;
     double ra[M3_NBAT][MF], rb[M3_NBAT][MF];
-    if (pipelined) mats3d_recip_batch<MF, false>(d0, m2phi, ra);
+    if (pipelined) mats3d_recip_batch<MF, SQ>(d0, m2phi, ra);
 #pragma unroll 1
     for (int m = 0; m < NROWS; ++m) {
       double M[4][MF];
@@ -1174,12 +1180,12 @@ __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dPara
       if (pipelined) {
         for (int c = 0; c < nc; c += 2 * M3_NBAT) {
           const int L = m * nc + c;
-          mats3d_recip_batch<MF, false>(d0 + L + M3_NBAT, m2phi, rb);
+          mats3d_recip_batch<MF, SQ>(d0 + L + M3_NBAT, m2phi, rb);
           if constexpr (SYM) mats3d_moment_accumulate_sym<MF>(num4 + c / 2, ra, M);
           else mats3d_moment_accumulate<MF>(num4 + c, ra, M);
           int Ln = L + 2 * M3_NBAT;
           Ln = Ln < l_last ? Ln : l_last;
-          mats3d_recip_batch<MF, false>(d0 + Ln, m2phi, ra);
+          mats3d_recip_batch<MF, SQ>(d0 + Ln, m2phi, ra);
           if constexpr (SYM) mats3d_moment_accumulate_sym<MF>(num4 + (c + M3_NBAT) / 2, rb, M);
           else mats3d_moment_accumulate<MF>(num4 + c + M3_NBAT, rb, M);
         }
@@ -1187,7 +1193,8 @@ __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dPara
         const double* drow = d0 + m * nc;
 #pragma unroll 1
         for (int c = 0; c < nc; ++c) {
-          const double r = fast_rcp(drow[c] + m2phi[0]);
+          double r = fast_rcp(drow[c] + m2phi[0]);
+          if constexpr (SQ) r = -(r * r);
           const double4 w = num4[c];
           M[0][0] = fma(w.x, r, M[0][0]);
           M[1][0] = fma(w.y, r, M[1][0]);

@@ -163,7 +163,7 @@ def test_integrators_validate_before_touching_the_device(lib):
 
     h = lib.dfrg_integrate_matsubara3d
     stack = B.Table(p, 128, 64, -9.0, 5.0, 3)
-    D4 = B.Mats3dDesc(0.15, 11, 1.0, reg, rule, rule, stack, stack, p, 20, None, None, 1, 0.0, None)
+    D4 = B.Mats3dDesc(0.15, 11, 1.0, reg, rule, rule, stack, stack, p, 20, None, None, 1, 0.0, None, None, None)
     assert h(C.byref(D4), 4, p, p, 2, p, 0, p, None, None) == B.DFRG_EINVAL     # n_jext < 1
     assert h(C.byref(D4), 4, p, p, 2, p, 60, p, None, None) == B.DFRG_EINVAL    # needs rows up to 60-1+11 > 63
     D4.T = 0.0

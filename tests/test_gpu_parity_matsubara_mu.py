@@ -141,3 +141,53 @@ def test_matsubara_mu_full_config4_sampled():
                                          want_sens=True)
     g = (out.cpu().numpy() + 1j * out_im.cpu().numpy()).ravel()[sel]
     check(g, dmin.cpu().numpy().ravel()[sel], o, odm, sens, "cfg4_mu_full_sampled")
+
+
+def run_dm2(c, mu, host=False):
+    import torch
+    from paper_2412_13043_b200 import binding as B
+    xq, wq = B.dfrg_quad_nodes(*c["rule_q"])
+    xc, wc = B.dfrg_quad_nodes(*c["rule_c"])
+    shape = (c["pext"].size, c["n_jext"], c["m2psi"].size)
+    if host:
+        up = lambda a: np.ascontiguousarray(a, dtype=np.float64)
+        new = lambda: np.full(shape, np.nan)
+        fn, down = B.dfrg_integrate_matsubara3d_host, (lambda a: a)
+    else:
+        up = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+        new = lambda: torch.full(shape, float("nan"), dtype=torch.float64, device="cuda")
+        fn, down = B.dfrg_integrate_matsubara3d, (lambda a: a.cpu().numpy())
+    bufs = [new() for _ in range(6)]
+    fn(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], (up(xq), up(wq)), (up(xc), up(wc)),
+       up(c["Zpsi"]), up(c["Zphi"]), c["lnq_lo"], c["lnq_hi"], c["interp"], up(c["coef"]), up(c["m2psi"]),
+       up(c["m2phi"]), up(c["pext"]), c["n_jext"], bufs[0], None, reg_arg4d=0, mu=mu, out_im=bufs[1],
+       dout_dm2_psi=bufs[2], dout_dm2_psi_im=bufs[3], dout_dm2_phi=bufs[4], dout_dm2_phi_im=bufs[5])
+    if not host:
+        torch.cuda.synchronize()
+    b = [down(x) for x in bufs]
+    args = (c["T"], c["n_max"], mu, c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], xq, wq, xc, wc, c["Zpsi"],
+            c["Zphi"], c["lnq_lo"], c["lnq_hi"], c["interp"], c["coef"], c["m2psi"], c["m2phi"], c["pext"], c["n_jext"])
+    o, odm, sens = oracle.matsubara3d_mu(*args, want_sens=True)
+    dpsi, dphi, spsi, sphi = oracle.matsubara3d_mu_dm2(*args)
+    return (b[0] + 1j * b[1], b[2] + 1j * b[3], b[4] + 1j * b[5]), (o, dpsi, dphi), (sens, spsi, sphi), odm
+
+
+@pytest.mark.parametrize("n_field,n_p,n_jext,n_q,n_c,n_max,mu", [(300, 2, 3, 9, 8, 3, 0.4), (130, 2, 5, 7, 5, 2, 0.7),
+                                                                 (300, 2, 3, 9, 8, 3, 0.0), (130, 2, 5, 7, 5, 2, 0.0),
+                                                                 (90, 1, 40, 5, 4, 3, 0.0)])
+def test_matsubara_mu_mass_derivatives(n_field, n_p, n_jext, n_q, n_c, n_max, mu):
+    # mu != 0: complex kernel, modes 1 and 2; mu = 0: spatial regulators through the real kernels (specialised, any-shape,
+    # row-streaming), imaginary parts zero-filled
+    c = inputs.config4(n_field=n_field, n_p=n_p, n_jext=n_jext, n_q=n_q, n_c=n_c)
+    c["n_max"] = n_max
+    g, o, sens, odm = run_dm2(c, mu)
+    for gi, oi, si, name in zip(g, o, sens, ("value", "dpsi", "dphi")):
+        diff = np.abs(gi - oi)
+        assert np.all(diff <= 20 * SENS_EPS * si), (name, float(np.max(diff / si)))
+        regular = (odm >= 1e-6) & (si <= 1e4 * np.abs(oi))
+        assert np.max(diff[regular] / np.abs(oi[regular])) <= 10 * RTOL, name
+        if mu == 0.0:
+            assert np.all(gi.imag == 0)
+    if n_jext <= 5 and n_field == 130:
+        h, _, _, _ = run_dm2(c, mu, host=True)
+        assert all(np.array_equal(a, b) for a, b in zip(g, h))
