@@ -3,6 +3,8 @@ output buffer (tests/helpers.py: gpu_run(canary=True)): ragged sizes, sizes of 1
 boundaries of the kernels (32 / 128 / 256 / 512 field points, 512-node chunks, 148 CTAs), both interpolation modes and
 all regulator paths.  compute-sanitizer is not available on this pool; an out-of-bounds write that lands in a margin,
 or a wrong index that changes a value, fails here."""
+import os
+
 import numpy as np
 import pytest
 
@@ -65,7 +67,10 @@ def draw(rng):
     return fam, c
 
 
-@pytest.mark.parametrize("seed", range(100))
+N_SEEDS = int(os.environ.get("DFRG_FUZZ_SEEDS", "100"))      # a longer soak: DFRG_FUZZ_SEEDS=2000 python -m pytest tests/test_gpu_fuzz.py
+
+
+@pytest.mark.parametrize("seed", range(N_SEEDS))
 def test_fuzz_shapes_against_oracle_with_canaries(seed):
     rng = np.random.default_rng(1000 + seed)
     fam, c = draw(rng)
