@@ -29,6 +29,19 @@ def _dress(c):
 def oracle_run(c, R, sel=None):
     """-> (out, dmin, sens); lpa: out = flow[n_field], extra channels under key 'chan' are returned via dict."""
     kd = kind_of(c)
+    if kd == "lpa" and c.get("statistics", 0) == 1:     # fermionic loop at chemical potential (reading A22)
+        m2 = np.stack([c["u"], c["u"] + 2.0 * c["rho"] * c["du"]])
+        I, dI, dm, sn, snd = oracle.lpa_fermion(c["d"], c["T"], c["n_max"], c.get("mu", 0.0), c["prefactor"], c["reg_kind"],
+                                                c["reg_order"], c["k"], *R["q"], m2.ravel(), **_dress(c))
+        I, dm, sn = (a.reshape(2, -1) for a in (I, dm, sn))
+        return dict(out=(c["N"] - 1.0) * I[0] + I[1], chan=I, dmin=np.minimum(dm[0], dm[1]),
+                    sens=abs(c["N"] - 1.0) * sn[0] + sn[1], sens_chan=sn)
+    if kd == "matsubara3d" and c.get("reg_arg4d", 1) == 0:   # spatial regulators / chemical potential (reading A24)
+        out, dmin, sens = oracle.matsubara3d_mu(c["T"], c["n_max"], c.get("mu", 0.0), c["prefactor"], c["reg_kind"],
+                                                c["reg_order"], c["k"], *R["q"], *R["c"], c["Zpsi"], c["Zphi"],
+                                                c["lnq_lo"], c["lnq_hi"], c["interp"], c["coef"], c["m2psi"], c["m2phi"],
+                                                c["pext"], c["n_jext"], sel=sel, want_sens=True, **_dress(c))
+        return dict(out=out, dmin=dmin, sens=sens)
     if kd == "lpa":
         flow, chan, dmin, sens = oracle.lpa(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["N"], c["prefactor"],
                                             c["reg_kind"], c["reg_order"], c["k"], *R["q"], c["rho"], c["u"], c["du"],
@@ -119,7 +132,8 @@ def gpu_run(c, R, host=False, want_dmin=True, want_d=False, canary=False):
         dchan = new(2, nf) if want_d else None
         fn = B.dfrg_integrate_lpa_host if host else B.dfrg_integrate_lpa
         fn(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["N"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
-           rule("q"), up(c["rho"]), up(c["u"]), up(c["du"]), flow, chan, dmin, dchan=dchan, **dress)
+           rule("q"), up(c["rho"]), up(c["u"]), up(c["du"]), flow, chan, dmin, dchan=dchan,
+           statistics=c.get("statistics", 0), mu=c.get("mu", 0.0) if c.get("statistics", 0) == 1 else 0.0, **dress)
         res = dict(out=flow, chan=chan, dmin=dmin, dchan=dchan)
     elif kd == "twopoint":
         out = new(c["pext"].size, c["m2"].size)
@@ -159,11 +173,14 @@ def gpu_run(c, R, host=False, want_dmin=True, want_d=False, canary=False):
         shape = (c["pext"].size, c["n_jext"], c["m2psi"].size)
         out, dmin = new(*shape), new(*shape) if want_dmin else None
         dpsi, dphi = (new(*shape), new(*shape)) if want_d else (None, None)
+        spatial = c.get("reg_arg4d", 1) == 0
+        out_im = new(*shape) if spatial else None
         fn = B.dfrg_integrate_matsubara3d_host if host else B.dfrg_integrate_matsubara3d
         fn(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"], rule("q"), rule("c"),
            up(c["Zpsi"]), up(c["Zphi"]), c["lnq_lo"], c["lnq_hi"], c["interp"], up(c["coef"]), up(c["m2psi"]),
-           up(c["m2phi"]), up(c["pext"]), c["n_jext"], out, dmin, dout_dm2_psi=dpsi, dout_dm2_phi=dphi, **dress)
-        res = dict(out=out, dmin=dmin, dpsi=dpsi, dphi=dphi)
+           up(c["m2phi"]), up(c["pext"]), c["n_jext"], out, dmin, dout_dm2_psi=dpsi, dout_dm2_phi=dphi,
+           reg_arg4d=c.get("reg_arg4d", 1), mu=c.get("mu", 0.0) if spatial else 0.0, out_im=out_im, **dress)
+        res = dict(out=out, dmin=dmin, dpsi=dpsi, dphi=dphi, out_im=out_im)
     if not host:
         torch.cuda.synchronize()
     for big, n in guards:

@@ -25,12 +25,16 @@ def pick(rng, *choices):
 
 
 def draw(rng):
-    fam = pick(rng, "lpa0", "lpa1", "two", "three", "four", "tab3d", "mats")
+    fam = pick(rng, "lpa0", "lpa1", "lpaF", "two", "three", "four", "tab3d", "mats", "matsmu")
     edge_f = lambda: int(pick(rng, 1, 2, 31, 32, 33, 127, 128, 129, 255, 256, 257, 300, 511, 513, int(rng.integers(1, 700))))
     if fam == "lpa0":
         c = inputs.config0(n_field=edge_f(), n_q=int(rng.integers(1, 70)), d=int(pick(rng, 3, 4)))
     elif fam == "lpa1":
         c = inputs.config1(float(pick(rng, 0.05, 0.1, 0.2, 0.5)), n_field=edge_f(), n_q=int(rng.integers(1, 70)))
+    elif fam == "lpaF":                              # fermionic loop at chemical potential: spatial regulator
+        c = inputs.config1(float(pick(rng, 0.05, 0.1, 0.2, 0.5)), n_field=edge_f(), n_q=int(rng.integers(1, 70)))
+        c["reg_arg4d"], c["statistics"], c["mu"] = 0, 1, float(pick(rng, 0.0, 0.3, 0.9))
+        c["N"] = float(pick(rng, 1.0, 4.0))
     elif fam == "two":
         c = inputs.config2(n_field=edge_f(), n_ext=int(rng.integers(1, 9)), n_q=int(rng.integers(1, 50)),
                            n_c=int(rng.integers(1, 20)), interp=int(pick(rng, 1, 3)))
@@ -57,6 +61,10 @@ def draw(rng):
         c = inputs.config4(n_field=edge_f(), n_p=int(rng.integers(1, 4)), n_jext=n_jext, n_q=int(rng.integers(1, 14)),
                            n_c=int(pick(rng, 1, 3, 4, 6, 8, 16)), interp=int(pick(rng, 1, 3)))
         c["n_max"] = n_max
+        if fam == "matsmu":                          # spatial regulators; mu = 0 runs the real kernels, mu != 0 the complex one
+            c["reg_arg4d"], c["mu"] = 0, float(pick(rng, 0.0, 0.35, -0.8))
+            if c["mu"] != 0.0 and n_jext > 32:
+                c["mu"] = 0.0
     reg = pick(rng, "exp1", "exp1", "exp3", "litim")
     if reg == "litim":
         c["reg_kind"] = 0
@@ -78,7 +86,12 @@ def test_fuzz_shapes_against_oracle_with_canaries(seed):
     want_d = fam in ("lpa0", "lpa1", "two", "mats") and bool(rng.integers(2))
     g = gpu_run(c, R, want_d=want_d, canary=True)
     o = oracle_run(c, R)
-    assert_parity(g["out"], o["out"], o["dmin"], o["sens"], "%s seed %d" % (c["name"], seed))
+    what = "%s %s seed %d" % (c["name"], fam, seed)
+    if fam == "matsmu":                              # complex result: both parts against the same yardstick
+        assert_parity(g["out"], o["out"].real, o["dmin"], o["sens"], what + " re")
+        assert_parity(g["out_im"], o["out"].imag, o["dmin"], o["sens"], what + " im")
+        return
+    assert_parity(g["out"], o["out"], o["dmin"], o["sens"], what)
     if want_d:
         od = oracle_run_dm2(c, R)
         for key, (val, sens) in od.items():
