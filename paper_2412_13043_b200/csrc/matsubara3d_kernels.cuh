@@ -1207,7 +1207,7 @@ __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dPara
       const int jhi2 = m > 0 ? min(n_jext - 1, n_max - m) : -1;
       const double4* brow1 = bet4 + 2 * (n_max - m);   // entry (j, n = j - m) at brow1[2 j (NT + 1)] (re), +1 (im)
       const double4* brow2 = bet4 + 2 * (n_max + m);
-      constexpr int JB = NJ < 4 ? NJ : 4;
+      constexpr int JB = NJ < 8 ? NJ : 8;
 #pragma unroll
       for (int j0 = 0; j0 < NJ; j0 += JB) {
         if (j0 >= jlo1 && j0 + JB - 1 <= jhi1) {
