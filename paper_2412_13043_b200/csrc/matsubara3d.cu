@@ -1,26 +1,21 @@
-// matsubara3d.cu -- dfrg_integrate_matsubara3d: 3-D spatial loop + Matsubara sum (BASELINE.json config 4).
+// matsubara3d.cu -- dfrg_integrate_matsubara3d: 3-D spatial loop + Matsubara sum (BASELINE.json config 4): host side
+// (validation, plan, scratch, launches) and the C entry points.  Kernels: matsubara3d_kernels.cuh.
 //
-// Three launches per call, all on the caller's stream:
-//
-//  (1) mats3d_phi_rows_kernel  (S3, field independent, once per call)
-//        D0phi[p][m][i][c] = Z_phi(r^2; row m) s_phi + R(s_phi),  m = 0 .. n_jext-1+n_max
-//      The boson denominator depends on the external and loop Matsubara indices only through
-//      |j - n|, so the 16 x 23 (j, n) combinations of config 4 share 27 rows per momentum p.
-//      Rows go to a stream-ordered scratch buffer (31 MB for config 4: L2 resident) together with
-//      their minima (for dmin).
-//  (2) mats3d_psi_kernel       (S3, once per call)
-//        psi[n][i] = (D0psi, Wpsi) = (Z_psi(q_i^2; row nbar) s_psi + R(s_psi),  wq_i q_i^2 Rdot(s_psi))
-//  (3) mats3d_main_kernel      (S2 + S3 remainder + S4 + S5 + S6): persistent, one CTA per SM, warp-specialised
-//      (see the comment at the kernel).  Row |j-n| of D0phi and row n of psi arrive by TMA bulk copy into a
-//      double-buffered shared-memory stage; a producer warp builds the numerator row Nw[i][c] = wc_c P(y1, y2, y3)
-//      (P as a cubic in y2 = p q c/k^2 by Horner, its four coefficients depending on (n, i) only).  Hot loop:
-//      thread = MF field points; per node  d_f = D0 + m2phi_f;  two-way batched inversion
-//      r = 1/(d_a d_b), 1/d_a = r d_b, 1/d_b = r d_a  (one MUFU.RCP64H seed + cubic Newton step per two
-//      evaluations: 10 FP64 instructions per two evaluations, the same as two separate reciprocals, but
-//      half the load on the XU pipe);  a_f += Nw / d_f  on two accumulators per field point.
-//      Every lane of a warp reads the same table entries (shared-memory broadcast).
-//      Then acc_f += Wpsi G_psi(f)^2 a_f.
-// dmin: fl(D0 + m2) is monotone in D0, so the minimum over nodes is (min D0) + m2: no hot-loop work.
+// Launches per call, all on the caller's stream:
+//  (1) mats3d_phi_rows_kernel  (S3, field independent)   D0phi[p][i][m][c] = Z_phi(r^2; row m) s_phi + R,  m = 0 .. n_jext-1+n_max
+//      The boson denominator depends on the external and loop Matsubara indices only through |j - n|: the 16 x 23 (j, n)
+//      combinations of config 4 share 27 rows per momentum p.  Also checks whether the cos rule is exactly symmetric.
+//  (2) mats3d_psi_kernel       (S3)   psi[n][i] = (D0psi, Wpsi)  (+ Im D0psi at mu != 0)
+//  (3) one moment kernel per requested output (value, d/dm2_psi, d/dm2_phi), chosen by the plan below:
+//        mats3d_moment_kernel   specialised (n_max, n_jext) = (11,16), (3,3): compile-time pair code behind a jump table
+//        mats3d_gmoment_kernel  any (n_max, n_jext <= 32)
+//        mats3d_cmoment_kernel  mu != 0: complex fermion line
+//        mats3d_main_kernel     n_jext > 32: row-streaming kernel without the moment factorisation
+//      The symmetric-pair and the plain instantiation of a moment kernel are both enqueued; the one that does not match
+//      the device-side symmetry flag returns at once.
+//  (4) mats3d_fixup_kernel     (S5/S6) adds the per-CTA partial sums in slot order, writes out (and out_im), dmin.
+// dmin: fl(D0 + m2) is monotone in D0, so the minimum over nodes is (min D0) + m2: no hot-loop work (|D_psi| per field
+// point at mu != 0: mats3d_psimin_cplx_kernel).
 #include "matsubara3d_kernels.cuh"
 
 namespace dfrg {
