@@ -1,4 +1,4 @@
-// loop4d.cu -- dfrg_integrate_loop4d: 4-D vacuum loops (BASELINE.json configs 2 and 3).
+// loop4d.cu -- dfrg_integrate_loop4d: 4-D vacuum loops (BASELINE.json configs 2 and 3, and the SURVEY 8(f) families).
 //
 // Two-point family.  One persistent warp-specialised kernel: producer warps build the field-independent (D0, W') of
 //   the next chunk of radial nodes while the consumers do add -> reciprocal -> FMA over (field point x node), two
@@ -12,6 +12,11 @@
 //               comes from a pre-pass table, what depends on (|p2|, alpha) alone is built once per work unit in shared
 //               memory; one look-up and one Horner evaluation remain per (a, r, node).
 //   The integrand has no phi dependence: the phi axis contributes sum_phi w.  Fixed-order sums.
+//   With a 3-D vertex table lambda3(S0, a, s) (DFRG_LOOP_THREEPOINT_TAB3D): the same two paths (t3d_kernel for a general
+//   list, the product-grid kernels instantiated with TAB3D), the table in shared memory, trilinear look-ups.
+//
+// Four-point family (DFRG_LOOP_FOURPOINT).  Genuine three-angle kinematics + ghost box: fp4_main_kernel, thread =
+//   (q, c1, c2) triple with the phi loop inside (see the comment at the kernel).
 #include "dfrg_device.cuh"
 #include "dfrg_internal.h"
 
