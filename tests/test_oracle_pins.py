@@ -655,3 +655,28 @@ def test_p9_matsubara_scaling():
     ob = _mats(b, (k * rq[0], k * rq[1]), rc, Zpsi=one, Zphi=one)[0]
     # T sum int q^2 dq Rdot G^2 G ~ k^(1+3+2-6) = k^0
     np.testing.assert_allclose(ob, oa, rtol=3e-12)
+
+
+def test_oracle_regression_fixture():
+    """The oracle's arithmetic is frozen by tests/golden/oracle_regression.txt (written by the committed script beside it,
+    which calls only oracle/): a change of the oracle's numbers has to be deliberate -- regenerate the fixture and say why
+    in the commit message.  (Not a pin: the pins are the tests above.)"""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_oracle_regression", os.path.join(here, "make_oracle_regression.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    stored = {}
+    for line in open(os.path.join(here, "oracle_regression.txt")):
+        if line.startswith("#"):
+            continue
+        name, idx, hx, _ = line.split(None, 3)
+        stored[(name, int(idx))] = float.fromhex(hx)
+    n = 0
+    for name, vals in mod.cases():
+        for i, v in enumerate(np.asarray(vals, dtype=np.float64)):
+            ref = stored[(name, i)]
+            assert abs(v - ref) <= 1e-14 * abs(ref) + 1e-300, (name, i, v, ref)
+            n += 1
+    assert n == len(stored) and n >= 30
