@@ -30,8 +30,8 @@ WORKLOAD = "cfg4_matsubara3d: 64 p x 16 j x 512 field points, 23 Matsubara terms
 
 # FP64 roofline denominator: 148 SMs x 64 FP64 lanes x 2 flop/DFMA x 1.965 GHz
 FP64_LANES_PER_SM = 64
-# dram__bytes_read.sum + dram__bytes_write.sum of the moment kernel per launch on this workload (profiles/r1g_moment_kernel_symmetric_pairs.md)
-NCU_DRAM_BYTES_PER_LAUNCH = 31981056 + 2048
+# dram__bytes_read.sum + dram__bytes_write.sum of the moment kernel per launch on this workload (profiles/r1k_bench_kernel_final.md)
+NCU_DRAM_BYTES_PER_LAUNCH = 31980288 + 2048
 
 
 def cfg4_counts(c, rules):
@@ -408,7 +408,7 @@ def main():
             "roofline": {"bound": "alu", "kernel": "mats3d_moment_kernel (+ the two pre-pass kernels and the fix-up kernel, timed together)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                          "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH if world == 1 else None,
                          "traffic_kind": "dram__bytes_read.sum + dram__bytes_write.sum of mats3d_moment_kernel, one ncu --set full "
-                                         "capture of this workload (profiles/r1g_moment_kernel_symmetric_pairs.md); algorithmic bytes: "
+                                         "capture of this workload (profiles/r1k_bench_kernel_final.md); algorithmic bytes: "
                                          "31.85 MB of D0phi chunks read once",
                          "achieved_kind": "algorithmic FP64 instructions x 2 (DFMA-slot equivalents) / event time",
                          "achieved_strict": flops_strict / (ms_local * 1e-3) * 1e-12,
