@@ -43,6 +43,11 @@ int mats3d_gmoment_dispatch(Mats3dParams& P, const MomentPlan& pl, cudaStream_t 
 template <int NJ, bool SYM>
 static int mats3d_cmoment_go(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream) {
   auto kern = P.mode == 2 ? mats3d_cmoment_kernel<NJ, SYM, true> : mats3d_cmoment_kernel<NJ, SYM, false>;
+  if constexpr (NJ == 16) {   // BASELINE config 4's shape: pair code enumerated at compile time
+    const char* vpath = getenv("DFRG_M3_PATH");
+    if (P.n_max == 11 && P.n_jext == 16 && !(vpath && vpath[0] == 'm'))
+      kern = P.mode == 2 ? mats3d_cmoment_kernel<16, SYM, true, 11> : mats3d_cmoment_kernel<16, SYM, false, 11>;
+  }
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
   if (e != cudaSuccess) return check_cuda(e);
   kern<<<pl.grid, 256, pl.smem, stream>>>(P);

@@ -1033,7 +1033,23 @@ __device__ __forceinline__ void gm_cpair_block(const double4* __restrict__ b, co
   }
 }
 
-template <int NJ, bool SYM, bool SQ>
+// Row m of the complex pair section with (n_max, n_jext) = (NMAX, NJ) known at compile time: the valid (j, n) pairs are
+// enumerated by the compiler (no range tests), as the jump-table pair code of the specialised real kernel.
+template <int m, int NMAX, int NJ>
+__device__ __forceinline__ void gm_cpairs_static(const double4* __restrict__ bet4, const double* __restrict__ H,
+                                                 const int hstride, const double (&M)[4][1], double (&accr)[NJ],
+                                                 double (&acci)[NJ]) {
+  constexpr int NT = 2 * NMAX + 1;
+#pragma unroll
+  for (int j = 0; j < NJ; ++j) {
+    const int n1 = j - m, n2 = j + m;
+    if (n1 >= -NMAX && n1 <= NMAX) gm_cpair_block<1, NJ>(bet4 + 2 * (j * NT + n1 + NMAX), 0, H, hstride, n1, M, accr, acci, j);
+    if (m > 0 && n2 <= NMAX) gm_cpair_block<1, NJ>(bet4 + 2 * (j * NT + n2 + NMAX), 0, H, hstride, n2, M, accr, acci, j);
+  }
+}
+
+// NMAX_T >= 0: (n_max, n_jext) = (NMAX_T, NJ) exactly, pair code per row behind a jump table; NMAX_T < 0: any n_max, n_jext <= NJ.
+template <int NJ, bool SYM, bool SQ, int NMAX_T = -1>
 __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dParams P) {
   constexpr int NTC = 256, MF = 1;
   if (P.sym_try && (*P.symflag != 0) != SYM) return;
@@ -1203,6 +1219,19 @@ __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dPara
         }
       }
       // ---- the (j, n) pairs with |j - n| = m ----
+      if constexpr (NMAX_T >= 0) {
+        switch (m) {
+#define DFRG_M3C_CASE(k) case k: if constexpr (k < NJ + NMAX_T) gm_cpairs_static<(k < NJ + NMAX_T ? k : 0), NMAX_T, NJ>(bet4, myH, NTC * 2, M, accr, acci); break;
+          DFRG_M3C_CASE(0) DFRG_M3C_CASE(1) DFRG_M3C_CASE(2) DFRG_M3C_CASE(3) DFRG_M3C_CASE(4) DFRG_M3C_CASE(5) DFRG_M3C_CASE(6)
+          DFRG_M3C_CASE(7) DFRG_M3C_CASE(8) DFRG_M3C_CASE(9) DFRG_M3C_CASE(10) DFRG_M3C_CASE(11) DFRG_M3C_CASE(12)
+          DFRG_M3C_CASE(13) DFRG_M3C_CASE(14) DFRG_M3C_CASE(15) DFRG_M3C_CASE(16) DFRG_M3C_CASE(17) DFRG_M3C_CASE(18)
+          DFRG_M3C_CASE(19) DFRG_M3C_CASE(20) DFRG_M3C_CASE(21) DFRG_M3C_CASE(22) DFRG_M3C_CASE(23) DFRG_M3C_CASE(24)
+          DFRG_M3C_CASE(25) DFRG_M3C_CASE(26) DFRG_M3C_CASE(27) DFRG_M3C_CASE(28) DFRG_M3C_CASE(29) DFRG_M3C_CASE(30)
+          DFRG_M3C_CASE(31)
+#undef DFRG_M3C_CASE
+          default: break;
+        }
+      } else {
       const int jlo1 = max(0, m - n_max), jhi1 = min(n_jext - 1, n_max + m);
       const int jhi2 = m > 0 ? min(n_jext - 1, n_max - m) : -1;
       const double4* brow1 = bet4 + 2 * (n_max - m);   // entry (j, n = j - m) at brow1[2 j (NT + 1)] (re), +1 (im)
@@ -1229,6 +1258,7 @@ __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dPara
                                     j0 + jj);
         }
       }
+          }
     }
     if (i == nq - 1 || u == u1 - 1) {
       const long long ufirst = (long long)ft * upp + (long long)e * nq;

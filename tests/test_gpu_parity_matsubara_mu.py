@@ -191,3 +191,18 @@ def test_matsubara_mu_mass_derivatives(n_field, n_p, n_jext, n_q, n_c, n_max, mu
     if n_jext <= 5 and n_field == 130:
         h, _, _, _ = run_dm2(c, mu, host=True)
         assert all(np.array_equal(a, b) for a, b in zip(g, h))
+
+
+def test_matsubara_mu_static_and_runtime_pair_enumeration_agree():
+    """(n_max, n_jext) = (11, 16) takes the complex kernel whose pair code is enumerated at compile time; forced through the
+    run-time enumeration (DFRG_M3_PATH=moment-generic) it must give the same sums (same order per accumulator: bit for bit)."""
+    import os
+    c = inputs.config4(n_field=300, n_p=2, n_jext=16, n_q=6, n_c=8)
+    g, gdm, o, odm, sens = run(c, 0.3)
+    check(g, gdm, o, odm, sens, "mats_mu_static_11_16")
+    os.environ["DFRG_M3_PATH"] = "moment-generic"
+    try:
+        g2, _, _, _, _ = run(c, 0.3)
+    finally:
+        del os.environ["DFRG_M3_PATH"]
+    assert np.array_equal(g, g2)
