@@ -318,11 +318,12 @@ def main():
 
     # ---- FP64 peak probe (register-only DFMA chains), before the timed region ----
     sink = torch.zeros(8, dtype=torch.float64, device="cuda")
-    B.dfrg_fp64_peak_probe(2000, 2, sink)
+    from paper_2412_13043_b200 import probe
+    probe.fp64_peak(2000, 2, sink)
     torch.cuda.synchronize()
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record()
-    probe_flops = B.dfrg_fp64_peak_probe(40000, 2, sink)
+    probe_flops = probe.fp64_peak(40000, 2, sink)
     b.record()
     b.synchronize()
     probe_tflops = probe_flops / (a.elapsed_time(b) * 1e-3) * 1e-12

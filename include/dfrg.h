@@ -263,19 +263,25 @@ typedef struct {
   double* out_im;       /* nullable unless mu != 0; output [n_p][n_jext][n_field] (zero-filled when mu == 0) */
   double* dout_dm2_psi_im; /* imaginary parts of the mass derivatives: nullable unless mu != 0 and the real part is requested; */
   double* dout_dm2_phi_im; /* zero-filled when mu == 0 */
+  int path;             /* kernel-path selection, an OR of dfrg_mats3d_path bits; 0 = the library's own choice.  Every path
+                           computes the same sums (the tests run them all on the same inputs); the field exists for testing
+                           and tuning and is part of the descriptor so that the call stays free of global state. */
 } dfrg_mats3d_desc;
+typedef enum {
+  DFRG_M3_AUTO = 0,
+  DFRG_M3_ROW_STREAMING = 1,      /* the kernel without the moment factorisation (the library's choice for n_jext > 32) */
+  DFRG_M3_ANY_SHAPE = 2,          /* the any-shape moment kernel even where a compile-time-specialised one exists */
+  DFRG_M3_PLAIN_MOMENTS = 4,      /* plain moment loop even if the cos rule is exactly symmetric */
+  DFRG_M3_ONE_FIELD = 8,          /* one field point per thread (512-thread CTAs) where the default is two */
+  DFRG_M3_GROUPS_4 = 16,          /* row-streaming kernel: 4 consumer groups per CTA (default 6) */
+  DFRG_M3_GROUPS_7 = 32           /* row-streaming kernel: 7 consumer groups per CTA */
+} dfrg_mats3d_path;
 
 int dfrg_integrate_matsubara3d(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi, const double* m2_phi,
                                int n_p, const double* p, int n_jext, double* out, double* dmin, void* cuda_stream);
 int dfrg_integrate_matsubara3d_host(const dfrg_mats3d_desc* D, int n_field, const double* m2_psi,
                                     const double* m2_phi, int n_p, const double* p, int n_jext, double* out,
                                     double* dmin);
-
-/* ---- measurement aid (bench.py roofline denominator; not part of the paper's path) -----------------------
- * Runs a register-only kernel of independent DFMA chains (n_iter x 64 DFMA per thread, one CTA of 512 threads
- * per SM x ctas_per_sm) on cuda_stream; *flops_out (host) receives the number of FP64 flops it executes
- * (2 per DFMA).  sink: device array of at least 1 double. */
-int dfrg_fp64_peak_probe(int n_iter, int ctas_per_sm, double* sink, double* flops_out, void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -1,0 +1,37 @@
+// fp64_probe.cu -- measurement aid of bench.py, NOT part of the library: the denominator of the FP64 roofline.
+// Built into its own shared object (libdfrg_probe.so) by paper_2412_13043_b200/build.py; the product ABI
+// (include/dfrg.h, libdfrg.so) does not contain it.
+//
+//   int dfrg_probe_fp64_peak(int n_iter, int ctas_per_sm, double* sink_dev, double* flops_out_host, void* cuda_stream)
+// runs a register-only kernel of 8 independent DFMA chains per thread (n_iter x 64 DFMA per thread, one CTA of 512
+// threads per SM x ctas_per_sm) on cuda_stream; *flops_out_host receives the FP64 flops it executes (2 per DFMA).
+// Returns 0, -1 (bad argument) or -3 (CUDA error).
+#include <cuda_runtime.h>
+
+namespace {
+__global__ void __launch_bounds__(512) fp64_peak_kernel(int n_iter, double* sink) {
+  double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 0.1, a2 = a0 + 0.2, a3 = a0 + 0.3;
+  double a4 = a0 + 0.4, a5 = a0 + 0.5, a6 = a0 + 0.6, a7 = a0 + 0.7;
+  const double m = 0.999999, c = 1e-7;
+  for (int it = 0; it < n_iter; ++it) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+      a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+  }
+  const double s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  if (s == 123456.789) sink[0] = s;  // never true; keeps the chains alive
+}
+}  // namespace
+
+extern "C" int dfrg_probe_fp64_peak(int n_iter, int ctas_per_sm, double* sink, double* flops_out, void* cuda_stream) {
+  if (n_iter < 1 || ctas_per_sm < 1 || ctas_per_sm > 4 || !sink) return -1;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return -3;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -3;
+  const int grid = sms * ctas_per_sm;
+  fp64_peak_kernel<<<grid, 512, 0, (cudaStream_t)cuda_stream>>>(n_iter, sink);
+  if (flops_out) *flops_out = 2.0 * 64.0 * (double)n_iter * 512.0 * (double)grid;
+  return cudaGetLastError() == cudaSuccess ? 0 : -3;
+}

@@ -17,6 +17,8 @@ REG_LITIM, REG_EXP_POLY = 0, 1
 STAT_BOSON, STAT_FERMION = 0, 1
 DOMAIN_X0, DOMAIN_Q0 = 0, 1
 LOOP_TWOPOINT, LOOP_THREEPOINT, LOOP_FOURPOINT, LOOP_THREEPOINT_TAB3D = 0, 1, 2, 3
+# dfrg_mats3d_desc::path bits (kernel-path selection; 0 = the library's own choice)
+M3_AUTO, M3_ROW_STREAMING, M3_ANY_SHAPE, M3_PLAIN_MOMENTS, M3_ONE_FIELD, M3_GROUPS_4, M3_GROUPS_7 = 0, 1, 2, 4, 8, 16, 32
 RULE_GAUSS_LEGENDRE = 0
 
 EXPORTS = (
@@ -25,7 +27,6 @@ EXPORTS = (
     "dfrg_integrate_lpa", "dfrg_integrate_lpa_host",
     "dfrg_integrate_loop4d", "dfrg_integrate_loop4d_host",
     "dfrg_integrate_matsubara3d", "dfrg_integrate_matsubara3d_host",
-    "dfrg_fp64_peak_probe",
 )
 
 _vp = C.c_void_p
@@ -66,7 +67,7 @@ class Mats3dDesc(C.Structure):
                 ("q", Rule), ("cos1", Rule), ("tab_psi", Table), ("tab_phi", Table),
                 ("coef", _vp), ("n_coef", C.c_int), ("dout_dm2_psi", _vp), ("dout_dm2_phi", _vp),
                 ("reg_arg4d", C.c_int), ("mu", C.c_double), ("out_im", _vp),
-                ("dout_dm2_psi_im", _vp), ("dout_dm2_phi_im", _vp)]
+                ("dout_dm2_psi_im", _vp), ("dout_dm2_phi_im", _vp), ("path", C.c_int)]
 
 
 class DfrgError(RuntimeError):
@@ -102,7 +103,6 @@ def lib():
                                                  _vp, _vp, _vp]
         L.dfrg_integrate_matsubara3d_host.argtypes = [C.POINTER(Mats3dDesc), C.c_int, _vp, _vp, C.c_int, _vp,
                                                       C.c_int, _vp, _vp]
-        L.dfrg_fp64_peak_probe.argtypes = [C.c_int, C.c_int, _vp, C.POINTER(C.c_double), _vp]
         _lib = L
     return _lib
 
@@ -244,22 +244,24 @@ def dfrg_integrate_loop4d_host(family, prefactor, reg_kind, reg_order, k, rule_q
 # ---- matsubara3d ----------------------------------------------------------------------------------
 def _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp, coef,
                device, dpsi=None, dphi=None, reg_zk=1.0, reg_eta=0.0, reg_arg4d=1, mu=0.0, out_im=None,
-               dpsi_im=None, dphi_im=None):
+               dpsi_im=None, dphi_im=None, path=0):
     return Mats3dDesc(float(T), int(n_max), float(prefactor), Regulator(int(reg_kind), int(reg_order), float(k), float(reg_zk), float(reg_eta)),
                       _rule(rule_q, device), _rule(rule_c, device),
                       _table(Zpsi, lnq_lo, lnq_hi, interp, device), _table(Zphi, lnq_lo, lnq_hi, interp, device),
                       _ptr(coef, device), _n(coef), _ptr(dpsi, device), _ptr(dphi, device),
-                      int(reg_arg4d), float(mu), _ptr(out_im, device), _ptr(dpsi_im, device), _ptr(dphi_im, device))
+                      int(reg_arg4d), float(mu), _ptr(out_im, device), _ptr(dpsi_im, device), _ptr(dphi_im, device),
+                      int(path))
 
 
 def dfrg_integrate_matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo,
                                lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, out, dmin=None,
                                dout_dm2_psi=None, dout_dm2_phi=None, reg_zk=1.0, reg_eta=0.0, reg_arg4d=1, mu=0.0, out_im=None,
-                               dout_dm2_psi_im=None, dout_dm2_phi_im=None):
+                               dout_dm2_psi_im=None, dout_dm2_phi_im=None, path=0):
     """out: [n_p, n_jext, n_field].  reg_arg4d=0: spatial regulators; mu != 0 (needs reg_arg4d=0 and out_im): complex result,
     out = real part, out_im = imaginary part (include/dfrg.h, dfrg_mats3d_desc::mu)."""
     D = _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp,
-                   coef, True, dout_dm2_psi, dout_dm2_phi, reg_zk, reg_eta, reg_arg4d, mu, out_im, dout_dm2_psi_im, dout_dm2_phi_im)
+                   coef, True, dout_dm2_psi, dout_dm2_phi, reg_zk, reg_eta, reg_arg4d, mu, out_im, dout_dm2_psi_im, dout_dm2_phi_im,
+                   path)
     _check(lib().dfrg_integrate_matsubara3d(C.byref(D), _n(m2psi), _ptr(m2psi, True), _ptr(m2phi, True), _n(pext),
                                             _ptr(pext, True), int(n_jext), _ptr(out, True), _ptr(dmin, True),
                                             _stream()), "dfrg_integrate_matsubara3d")
@@ -269,19 +271,11 @@ def dfrg_integrate_matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, rule
 def dfrg_integrate_matsubara3d_host(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo,
                                     lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, out, dmin=None,
                                dout_dm2_psi=None, dout_dm2_phi=None, reg_zk=1.0, reg_eta=0.0, reg_arg4d=1, mu=0.0, out_im=None,
-                               dout_dm2_psi_im=None, dout_dm2_phi_im=None):
+                               dout_dm2_psi_im=None, dout_dm2_phi_im=None, path=0):
     D = _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp,
-                   coef, False, dout_dm2_psi, dout_dm2_phi, reg_zk, reg_eta, reg_arg4d, mu, out_im, dout_dm2_psi_im, dout_dm2_phi_im)
+                   coef, False, dout_dm2_psi, dout_dm2_phi, reg_zk, reg_eta, reg_arg4d, mu, out_im, dout_dm2_psi_im, dout_dm2_phi_im,
+                   path)
     _check(lib().dfrg_integrate_matsubara3d_host(C.byref(D), _n(m2psi), _ptr(m2psi, False), _ptr(m2phi, False),
                                                  _n(pext), _ptr(pext, False), int(n_jext), _ptr(out, False),
                                                  _ptr(dmin, False)), "dfrg_integrate_matsubara3d_host")
     return out
-
-
-# ---- measurement aid ------------------------------------------------------------------------------
-def dfrg_fp64_peak_probe(n_iter, ctas_per_sm, sink):
-    """Enqueues the DFMA probe on the current stream; returns the FP64 flops it executes."""
-    flops = C.c_double()
-    _check(lib().dfrg_fp64_peak_probe(int(n_iter), int(ctas_per_sm), _ptr(sink, True), C.byref(flops), _stream()),
-           "dfrg_fp64_peak_probe")
-    return flops.value

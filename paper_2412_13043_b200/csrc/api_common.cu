@@ -1,10 +1,12 @@
-// api_common.cu -- status strings, error slot, device check, Gauss-Legendre nodes (S1, host),
-// the host-entry-point arena, and the FP64 peak probe kernel used by bench.py.
+// api_common.cu -- status strings, error slot, device check, Gauss-Legendre nodes (S1, host) and
+// the host-entry-point arena.
 #include <math.h>
 #include <stdint.h>
 #include <string.h>
 
 #include <mutex>
+#include <set>
+#include <utility>
 
 #include "dfrg_internal.h"
 
@@ -13,17 +15,52 @@ namespace dfrg {
 static thread_local int g_last_cuda_error = 0;
 void set_last_cuda_error(int e) { g_last_cuda_error = e; }
 
+// Per-device cache of (compute capability major, SM count): filled on first use of a device.
+static std::mutex g_dev_mutex;
+static int g_dev_major[64] = {}, g_dev_sms[64] = {};
 int require_sm100(int* sm_count) {
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) { set_last_cuda_error((int)e); return DFRG_ECUDA; }
-  int major = 0, sms = 0;
-  e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
-  if (e != cudaSuccess) { set_last_cuda_error((int)e); return DFRG_ECUDA; }
-  e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  if (e != cudaSuccess) { set_last_cuda_error((int)e); return DFRG_ECUDA; }
+  if (dev < 0 || dev >= 64) return DFRG_EUNSUPPORTED;
+  int major, sms;
+  {
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    if (g_dev_major[dev] == 0) {
+      int mj = 0, sm = 0;
+      e = cudaDeviceGetAttribute(&mj, cudaDevAttrComputeCapabilityMajor, dev);
+      if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev);
+      if (e != cudaSuccess) { set_last_cuda_error((int)e); return DFRG_ECUDA; }
+      g_dev_major[dev] = mj;
+      g_dev_sms[dev] = sm;
+    }
+    major = g_dev_major[dev];
+    sms = g_dev_sms[dev];
+  }
   if (major != 10) return DFRG_EUNSUPPORTED;
   if (sm_count) *sm_count = sms;
+  return DFRG_OK;
+}
+
+static std::mutex g_attr_mutex;
+static std::set<std::pair<int, const void*>> g_attr_done;
+int opt_in_max_smem_impl(const void* kernel) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return check_cuda(e);
+  std::lock_guard<std::mutex> lock(g_attr_mutex);
+  const std::pair<int, const void*> key(dev, kernel);
+  if (g_attr_done.count(key)) return DFRG_OK;
+  // the opt-in limit covers static + dynamic shared memory: leave room for the kernel's own static part
+  cudaFuncAttributes fa;
+  e = cudaFuncGetAttributes(&fa, kernel);
+  if (e != cudaSuccess) return check_cuda(e);
+  int optin = 0;
+  e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if (e != cudaSuccess) return check_cuda(e);
+  e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes);
+  if (e != cudaSuccess) return check_cuda(e);
+  g_attr_done.insert(key);
   return DFRG_OK;
 }
 
@@ -151,23 +188,6 @@ Arena& thread_arena() {
   return a;
 }
 
-// ---- FP64 peak probe ---------------------------------------------------------------------------
-// 8 independent DFMA chains per thread, 8 DFMA per chain per iteration: register-only, no memory.
-__global__ void __launch_bounds__(512) fp64_peak_kernel(int n_iter, double* sink) {
-  double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 0.1, a2 = a0 + 0.2, a3 = a0 + 0.3;
-  double a4 = a0 + 0.4, a5 = a0 + 0.5, a6 = a0 + 0.6, a7 = a0 + 0.7;
-  const double m = 0.999999, c = 1e-7;
-  for (int it = 0; it < n_iter; ++it) {
-#pragma unroll
-    for (int u = 0; u < 8; ++u) {
-      a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
-      a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
-    }
-  }
-  const double s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
-  if (s == 123456.789) sink[0] = s;  // never true; keeps the chains alive
-}
-
 }  // namespace dfrg
 
 using namespace dfrg;
@@ -186,7 +206,12 @@ const char* dfrg_strerror(int status) {
 }
 int dfrg_last_cuda_error(void) { return g_last_cuda_error; }
 int dfrg_version(void) { return 100; }
-void dfrg_shutdown(void) { thread_arena().release(); scratch_shutdown(); }
+void dfrg_shutdown(void) {
+  thread_arena().release();
+  scratch_shutdown();
+  std::lock_guard<std::mutex> lock(g_attr_mutex);
+  g_attr_done.clear();   // kernel attributes do not survive a device reset: set them again on the next call
+}
 
 // S1: Gauss-Legendre nodes.  Half the roots from the Tricomi initial guess, Newton on P_n with the
 // three-term recurrence in long double, mirrored; derivative from P_n' = n (P_{n-1} - x P_n)/(1 - x^2).
@@ -278,17 +303,6 @@ int dfrg_quad_nodes(int rule_kind, int n, double a, double b, double* x_host, do
     }
   }
   return DFRG_OK;
-}
-
-int dfrg_fp64_peak_probe(int n_iter, int ctas_per_sm, double* sink, double* flops_out, void* cuda_stream) {
-  if (n_iter < 1 || ctas_per_sm < 1 || ctas_per_sm > 4 || !sink) return DFRG_EINVAL;
-  int sms = 0;
-  int rc = require_sm100(&sms);
-  if (rc != DFRG_OK) return rc;
-  const int grid = sms * ctas_per_sm;
-  fp64_peak_kernel<<<grid, 512, 0, (cudaStream_t)cuda_stream>>>(n_iter, sink);
-  if (flops_out) *flops_out = 2.0 * 64.0 * (double)n_iter * 512.0 * (double)grid;
-  return check_cuda(cudaGetLastError());
 }
 
 }  // extern "C"

@@ -34,8 +34,8 @@ __device__ __forceinline__ double fast_rcp(double d) {
 //   fm_log(s):  s = 2^e m, m in [1,2); j = top 7 mantissa bits; r = m * (1/c_j) - 1, |r| <= 2^-8;
 //               ln s = e ln2 + ln c_j + (r - r^2/2 + ... - r^6/6)          abs. error <~ 3e-16 for |e| < 64
 //   fm_exp_neg(x) = e^-x, 0 <= x: n = rint(-64 x / ln2), r = -x - n ln2/64, |r| <= ln2/128;
-//               e^-x = 2^(n>>6) 2^((n&63)/64) (1 + r + ... + r^5/120)       rel. error <~ 2 ulp; x > 700 is clamped
-//               (e^-700 = 1e-304: the regulator is then 300 orders of magnitude below anything it is added to).
+//               e^-x = 2^(n>>6) 2^((n&63)/64) (1 + r + ... + r^5/120)       rel. error <~ 2 ulp; exactly 0 where libm's
+//               e^-x is 0 (x >= 745.1332191019412); 700 < x below that is clamped to 700 (1e-304 instead of a subnormal).
 // fm_log(0) = -709.8 (exponent field 0): every table coordinate derived from it clamps to the first grid point.
 struct FastMath {
   const double2* logtab;  // [128] (1/c_j, ln c_j)
@@ -105,7 +105,13 @@ __device__ __forceinline__ double fm_log(const FastMath& fm, double s) {
   return fma(ed, fm.k[5], T.y) + fma(ed, fm.k[6], lm);
 }
 
+// libm's e^-x is exactly 0 from x = 745.1332191019412 on (it rounds below half the smallest subnormal): the same here,
+// decided on the bits of x with integer compares (reading A17: 0 on both sides).  Below that the argument is clamped to 700.
+__device__ __forceinline__ bool exp_neg_underflows(const double x) {
+  return __double_as_longlong(x) > 0x40874910d52d3051LL;   // x >= 0 (NaN counts as underflow)
+}
 __device__ __forceinline__ double fm_exp_neg(const FastMath& fm, double x) {
+  const bool uf = exp_neg_underflows(x);
   x = clamp_hi(x, 700.0);
   const double MAGIC = fm.k[8];  // 1.5 * 2^52: the low word of y holds rint(-x * 64/ln2)
   const double y = fma(x, fm.k[7], MAGIC);
@@ -119,7 +125,7 @@ __device__ __forceinline__ double fm_exp_neg(const FastMath& fm, double x) {
   p = fma(r, p, fm.k[15]);
   p = fma(r, p, fm.k[15]);
   const double v = fm.exptab[n & 63] * p;
-  return __hiloint2double(__double2hiint(v) + ((n >> 6) << 20), __double2loint(v));
+  return __hiloint2double(uf ? 0 : __double2hiint(v) + ((n >> 6) << 20), uf ? 0 : __double2loint(v));
 }
 
 // ---- regulators --------------------------------------------------------------------------------
@@ -310,9 +316,107 @@ __device__ __forceinline__ double lg_lookup(const double2* __restrict__ cells, c
   return lg_cell_eval(cells, L, lg_coord(L, kc, s));
 }
 
+// ---- second-generation coordinate / cells for the hot product-grid loop (t3g_main_kernel) ---------------------
+// Same mathematics as lg_coord / lg_cell_eval, arranged for the fewest issue slots per look-up:
+//   * mant[j] = (inv_j, A ln c_j + B + 1): the reciprocal is NOT pre-multiplied by A, so 2^-e can be folded into its
+//     exponent field with one integer multiply-add (inv' = inv_j 2^-e; r = fma(x, inv', -1) is the same exact residual as
+//     m inv_j - 1 without building the mantissa m), and A moves into the series coefficients a1..a4;
+//   * the coordinate comes out as t' = t + 1 >= 0 for every s on or above the first grid point, so that one
+//     saturating float-to-unsigned conversion is floor AND the lower clamp: F' = min(cvt.rmi.u32(t'), n) in [0, n];
+//   * guarded cells are NOT replicated (32 bytes each, cell F' at byte 32 F'): the hot loop keeps the current cell in
+//     registers and reloads it only when F' changes (x is monotone along the c2 row, so this is rare).
+// x = 0 and subnormal x give t' << 0 -> cell 0 (the table's first value); valid for x < 2^1023.
+// The series coefficients travel in the kernel parameters (constant bank), so that every DFMA of the coordinate reads
+// its constant as an operand and no register holds them.
+struct LogGrid2Consts {
+  double a1, a2, a3, a4;  // A, -A/2, A/3, -A/4   (A = 1/(2h)):  A ln(1+r) = r (a1 + r (a2 + r (a3 + r a4)))
+  double ex1;             // A ln2
+  double bq;              // B + 1 = 1 - lo/h
+};
+inline LogGrid2Consts lg2_consts(const double lo, const double inv_h) {   // host side
+  const double A = 0.5 * inv_h;
+  LogGrid2Consts K;
+  K.a1 = A; K.a2 = -0.5 * A; K.a3 = A * (1.0 / 3.0); K.a4 = -0.25 * A;
+  K.ex1 = A * 0.6931471805599453;
+  K.bq = -lo * inv_h + 1.0;
+  return K;
+}
+struct LogGrid2 {
+  const char* mant;      // the table: entry j, replica r at byte 128 j + 16 r
+  unsigned rep16;        // 16 * (this thread's replica): OR-ed into the byte offset (the index bits start at bit 7)
+  unsigned n;            // grid points = index of the upper guard cell
+  const LogGrid2Consts* K;   // inside the kernel parameters
+};
+__device__ __forceinline__ LogGrid2 lg2_build(double* mem, const LogGrid2Consts& K, const int n) {
+  double2* mt = reinterpret_cast<double2*>(mem);
+  for (int j = threadIdx.x; j < LG_NM; j += blockDim.x) {
+    const double c = 1.0 + ((double)j + 0.5) * (1.0 / (double)LG_NM);
+    const double inv = 1.0 / c;                      // the rounded value defines the centre: c_j := 1 / inv
+    const double2 ent = make_double2(inv, fma(-K.a1, log(inv), K.bq));
+#pragma unroll
+    for (int r = 0; r < LG_REP; ++r) mt[j * LG_REP + r] = ent;
+  }
+  LogGrid2 L;
+  L.mant = reinterpret_cast<const char*>(mt);
+  L.rep16 = 16u * (threadIdx.x & (LG_REP - 1));
+  L.n = (unsigned)n;
+  L.K = &K;
+  return L;
+}
+__device__ __forceinline__ double lg2_coord(const LogGrid2& L, const double x) {
+  const int hi = __double2hiint(x);
+  unsigned off;                                   // 128 * (top 9 mantissa bits) + 16 * replica, as ONE three-input LOP3
+  asm("lop3.b32 %0, %1, 0xff80, %2, 0xEA;" : "=r"(off) : "r"((unsigned)hi >> 4), "r"(L.rep16));
+  const double2 T = *reinterpret_cast<const double2*>(L.mant + off);
+  const int e = (int)((unsigned)hi >> 20) - 1023;
+  const double inv = __hiloint2double(__double2hiint(T.x) - (e << 20), __double2loint(T.x));   // inv_j 2^-e
+  const double r = fma(x, inv, -1.0);
+  const double P = fma(r, fma(r, fma(r, L.K->a4, L.K->a3), L.K->a2), L.K->a1);
+  return fma((double)e, L.K->ex1, fma(r, P, T.y));
+}
+// Guarded cells, one copy: cell F' in [0, n] as double4 (value, d1, d2, d3) in tau = t' - F'.  (n + 1) double4.
+__device__ __forceinline__ void cells2_build(double4* cells, const double* __restrict__ v, const int n, const int interp) {
+  for (int c = threadIdx.x; c <= n; c += blockDim.x) {
+    const int F = c - 1;
+    double4 k;
+    if (F < 0) k = make_double4(v[0], 0.0, 0.0, 0.0);
+    else if (F >= n - 1) k = make_double4(v[n - 1], 0.0, 0.0, 0.0);
+    else if (interp == 3) {
+      int i0 = F - 1;
+      i0 = i0 < 0 ? 0 : i0;
+      i0 = i0 > n - 4 ? n - 4 : i0;
+      const int dl = F - i0;
+      const double v0 = v[i0], v1 = v[i0 + 1], v2 = v[i0 + 2], v3 = v[i0 + 3];
+      const double d3 = ((v3 - v0) + 3.0 * (v1 - v2)) * (1.0 / 6.0);
+      if (dl == 0)
+        k = make_double4(v0, (-11.0 * v0 + 18.0 * v1 - 9.0 * v2 + 2.0 * v3) * (1.0 / 6.0),
+                         (2.0 * v0 - 5.0 * v1 + 4.0 * v2 - v3) * 0.5, d3);
+      else if (dl == 1)
+        k = make_double4(v1, (-2.0 * v0 - 3.0 * v1 + 6.0 * v2 - v3) * (1.0 / 6.0), (v0 - 2.0 * v1 + v2) * 0.5, d3);
+      else
+        k = make_double4(v2, (v0 - 6.0 * v1 + 3.0 * v2 + 2.0 * v3) * (1.0 / 6.0), (v1 - 2.0 * v2 + v3) * 0.5, d3);
+    } else {
+      k = make_double4(v[F], v[F + 1] - v[F], 0.0, 0.0);
+    }
+    cells[c] = k;
+  }
+}
+__device__ __forceinline__ unsigned lg2_cell(const LogGrid2& L, const double tq) {
+  const unsigned F = __double2uint_rd(tq);   // F2I.U32.F64.FLOOR: negative and NaN -> 0
+  return min(F, L.n);
+}
+// stand-alone look-up (set-up code; the hot loop inlines the pieces around its cell cache)
+__device__ __forceinline__ double lg2_lookup(const double4* __restrict__ cells, const LogGrid2& L, const double x) {
+  const double tq = lg2_coord(L, x);
+  const unsigned F = lg2_cell(L, tq);
+  const double tau = tq - (double)F;
+  const double4 k = cells[F];
+  return fma(fma(fma(k.w, tau, k.z), tau, k.y), tau, k.x);
+}
+
 // k^2 e^-x from a table of k^2 2^(j/64), replicated 16 times (one copy per lane & 15: a 64-bit shared-memory load is
 // served in half-warps, so the look-up is conflict free):  n = rint(-64 x / ln2), r = -x - n ln2/64, |r| <= ln2/128,
-// e^r by its series to r^5/120.  x is clamped to 700 (e^-700 = 1e-304).
+// e^r by its series to r^5/120.  Exactly 0 where libm underflows to 0; 700 < x below that is clamped to 700.
 constexpr int FX_REP = 16;
 constexpr int FX_DOUBLES = 64 * FX_REP;
 __device__ __forceinline__ const double* fx_build(double* mem, const double k2) {
@@ -324,6 +428,7 @@ __device__ __forceinline__ const double* fx_build(double* mem, const double k2) 
   return mem + (threadIdx.x & (FX_REP - 1));
 }
 __device__ __forceinline__ double fx_exp_neg(const double* __restrict__ tab, const double* __restrict__ kc, double x) {
+  const bool uf = exp_neg_underflows(x);
   x = clamp_hi(x, 700.0);
   const double MAGIC = kc[8];
   const double y = fma(x, kc[7], MAGIC);
@@ -337,7 +442,7 @@ __device__ __forceinline__ double fx_exp_neg(const double* __restrict__ tab, con
   p = fma(r, p, kc[15]);
   p = fma(r, p, kc[15]);
   const double v = tab[(n & 63) * FX_REP] * p;
-  return __hiloint2double(__double2hiint(v) + ((n >> 6) << 20), __double2loint(v));
+  return __hiloint2double(uf ? 0 : __double2hiint(v) + ((n >> 6) << 20), uf ? 0 : __double2loint(v));
 }
 
 __device__ __forceinline__ double ipow(double x, int e) {

@@ -16,8 +16,19 @@ inline int check_cuda(cudaError_t e) {
   return DFRG_ECUDA;
 }
 
-// DFRG_EUNSUPPORTED unless the current device is compute capability 10.x.
+// DFRG_EUNSUPPORTED unless the current device is compute capability 10.x.  The device's attributes are queried once
+// per device and cached (one cudaGetDevice per call afterwards).
 int require_sm100(int* sm_count);
+
+// Largest dynamic shared memory the library asks for: the 227 KB a CTA may opt into on sm_100 minus 1 KB for the
+// kernels' static shared memory (barriers, reduction scratch).  Every kernel that needs more than the 48 KB default is
+// raised to its own limit (opt-in maximum - its static part) ONCE per device (kernel attributes are per device) --
+// never per call and never to a per-call size, so concurrent callers cannot lower each other's limit between the set
+// and the launch.
+constexpr size_t kMaxDynSmem = 226 * 1024;
+int opt_in_max_smem_impl(const void* kernel);   // DFRG_OK / DFRG_ECUDA; thread-safe, cached per (device, kernel)
+template <typename K>
+inline int opt_in_max_smem(K kernel) { return opt_in_max_smem_impl(reinterpret_cast<const void*>(kernel)); }
 
 inline bool valid_regulator(const dfrg_regulator& r) {
   if (!(r.k > 0.0) || !(r.zk > 0.0) || !(r.eta == r.eta)) return false;

@@ -1,0 +1,327 @@
+// loop4d_twopoint.cu -- two-point family of dfrg_integrate_loop4d (BASELINE.json config 2).
+#include "loop4d_kernels.cuh"
+
+namespace dfrg {
+
+// =====================================================================================================
+// two-point
+// =====================================================================================================
+// One persistent, warp-specialised kernel (one CTA per SM) and a small fix-up kernel.
+//  Work unit = (field tile, p, chunk of QC radial nodes); the units are dealt to the CTAs in contiguous ranges, so a
+//  consumer keeps its accumulators while the CTA stays inside one (field tile, p).
+//  Producer warps (S3, field independent), one unit ahead through a two-stage mbarrier ring (full[b] / empty[b]):
+//        chunk[i][j] = (D0, W'),  D0 = Z(s_ij) s_ij + R(s_ij),  W' = wc_j sqrt(1-c_j^2) (coef0 + coef1 q_i p c_j/k^2)
+//    and the chunk's minimum of D0 (for dmin).  outer[i] = (Z(q_i^2) q_i^2 + R(q_i^2), wq_i q_i^3 Rdot(q_i^2)) is built
+//    once per CTA.  S2: nodes, weights and the Z table arrive by TMA bulk copy.
+//  Consumers (S4 + S5): TP_GROUPS groups x TP_FT threads; a thread owns MF field points, a group every TP_GROUPS-th
+//    radial node of the chunk.  Per node:  d_f = D0 + m2_f;  MF = 2: one seed + Newton reciprocal of d_0 d_1 serves both
+//    field points (4.5 FP64 instructions per evaluation);  A_f += W'/d_f  (with mass derivatives also B_f += W'/d_f^2).
+//    Per radial node:  acc_f += Wq G(q)^2 A_f.  Every table read is a shared-memory broadcast.
+//    When (field tile, p) or the CTA's range ends, the groups are combined in fixed order and the partial sum goes to
+//    part[slot]; slot = rank of the CTA among the owners of that (field tile, p).
+//  tp_fixup_kernel (S5 + S6): out = prefactor sum_slots part in fixed order; dmin from the chunk minima
+//    (fl(D0 + m2) is monotone in D0, so the minimum over nodes is (min D0) + m2).
+
+// One batch of NB angular nodes for the MF field points of a thread.
+template <int MF, bool WANT_D, int NB>
+__device__ __forceinline__ void tp_batch(const double2* __restrict__ row, const double (&m2)[MF], double (&A)[MF],
+                                         double (&B)[MF]) {
+  double2 t[NB];
+#pragma unroll
+  for (int b = 0; b < NB; ++b) t[b] = row[b];
+  if constexpr (MF == 2) {
+    double d0[NB], d1[NB], R[NB], Rw[NB];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) { d0[b] = t[b].x + m2[0]; d1[b] = t[b].x + m2[1]; }
+#pragma unroll
+    for (int b = 0; b < NB; ++b) R[b] = fast_rcp(d0[b] * d1[b]);
+#pragma unroll
+    for (int b = 0; b < NB; ++b) Rw[b] = R[b] * t[b].y;
+#pragma unroll
+    for (int b = 0; b < NB; ++b) { A[0] = fma(Rw[b], d1[b], A[0]); A[1] = fma(Rw[b], d0[b], A[1]); }
+    if constexpr (WANT_D) {
+#pragma unroll
+      for (int b = 0; b < NB; ++b) {
+        B[0] = fma(Rw[b] * d1[b], R[b] * d1[b], B[0]);
+        B[1] = fma(Rw[b] * d0[b], R[b] * d0[b], B[1]);
+      }
+    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < MF; ++k) {
+      double r[NB];
+#pragma unroll
+      for (int b = 0; b < NB; ++b) r[b] = fast_rcp(t[b].x + m2[k]);
+#pragma unroll
+      for (int b = 0; b < NB; ++b) {
+        A[k] = fma(t[b].y, r[b], A[k]);
+        if constexpr (WANT_D) B[k] = fma(t[b].y * r[b], r[b], B[k]);
+      }
+    }
+  }
+}
+
+template <int MF, bool WANT_D>
+__global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t bar, full[2], empty[2];
+  __shared__ double red[32];
+  const int nq = P.nq, nc = P.nc, nt = P.grid.n, QC = P.QC, NCH = P.NCH;
+  const int chunk_nodes = QC * nc;
+  constexpr int ND = WANT_D ? 2 : 1;
+  double2* buf = reinterpret_cast<double2*>(smem_raw);                // [2][chunk_nodes]
+  double2* souter = buf + 2 * (size_t)chunk_nodes;                    // [nq]
+  double4* cZ = reinterpret_cast<double4*>(souter + nq);              // [nt] per-cell cubics of Z
+  double* sxq = reinterpret_cast<double*>(cZ + nt);
+  double* swq = sxq + ((nq + 1) & ~1);
+  double* sxc = swq + ((nq + 1) & ~1);
+  double* swc = sxc + ((nc + 1) & ~1);                                // wc_j sqrt(1 - c_j^2) after the set-up
+  double* sZ = swc + ((nc + 1) & ~1);
+  double* fmmem = sZ + ((nt + 1) & ~1);
+  double* comb = fmmem + FM_DOUBLES;                                  // [2][ND][TP_GROUPS][TP_FT * MF]
+
+  const int tid = threadIdx.x;
+  const int tile = TP_FT * MF;
+  const int n_ftiles = (P.n_field + tile - 1) / tile;
+  const long long upp = (long long)P.n_ext * NCH;                     // units per field tile
+  const long long U = (long long)n_ftiles * upp;
+  const long long u0 = (long long)blockIdx.x * U / gridDim.x, u1 = (long long)(blockIdx.x + 1) * U / gridDim.x;
+
+  if (tid == 0) {
+    mbar_init(&bar, 1);
+    mbar_init(&full[0], TP_NPROD / 32);
+    mbar_init(&full[1], TP_NPROD / 32);
+    mbar_init(&empty[0], TP_NCONS / 32);
+    mbar_init(&empty[1], TP_NCONS / 32);
+    mbar_fence_init();
+  }
+  __syncthreads();
+  StageList L;
+  L.add(sxq, P.xq, nq); L.add(swq, P.wq, nq);
+  L.add(sxc, P.xc, nc); L.add(swc, P.wc, nc);
+  L.add(sZ, P.Z, nt);
+  const FastMath fm = fm_build(fmmem, P.fmc);
+  stage_to_smem(L, &bar, 0);
+  cells_build(cZ, sZ, P.grid);
+  __syncthreads();
+  const double inf = __longlong_as_double(0x7ff0000000000000LL);
+  {
+    double dq = inf;
+    for (int i = tid; i < nq; i += TP_THREADS) {
+      const double q = sxq[i], s = q * q;
+      double R, Rd;
+      regulator(P.reg, fm, s, R, Rd);
+      const double D0 = table_lookup(cZ, P.grid, fm, s) * s + R;
+      souter[i] = make_double2(D0, swq[i] * q * q * q * Rd);
+      dq = fmin(dq, D0);
+    }
+    for (int j = tid; j < nc; j += TP_THREADS) {
+      const double c = sxc[j];
+      swc[j] *= sqrt((1.0 - c) * (1.0 + c));
+    }
+    dq = block_min(dq, red);  // also publishes souter and swc
+    if (blockIdx.x == 0 && tid == 0) P.chunkmin[(size_t)n_ftiles * P.n_ext * NCH * (TP_NPROD / 32)] = dq;
+  }
+
+  if (tid >= TP_NCONS) {
+    // =========================== producers ===========================
+    const int ptid = tid - TP_NCONS, lane = ptid & 31, pw = ptid >> 5;
+    const double coef0 = P.coef[0], coef1 = P.coef[1];
+    uint32_t g = 0;
+    for (long long u = u0; u < u1; ++u, ++g) {
+      const int b = g & 1;
+      const long long rem = u % upp;
+      const int e = (int)(rem / NCH), ch = (int)(rem - (long long)e * NCH);
+      const int i0 = ch * QC;
+      const int ni = min(QC, nq - i0);
+      const double p = P.pext[e];
+      mbar_wait(&empty[b], ((g >> 1) & 1) ^ 1);   // consumers drained this stage (passes at once for g < 2)
+      double2* dst = buf + (size_t)b * chunk_nodes;
+      double dmin0 = inf;
+      for (int t = ptid; t < ni * nc; t += TP_NPROD) {
+        const int il = t / nc, j = t - il * nc;
+        const double q = sxq[i0 + il], c = sxc[j];
+        double s = q * q + p * p + 2.0 * q * p * c;
+        s = clamp_lo(s, 0.0);
+        double R, Rd;
+        regulator(P.reg, fm, s, R, Rd);
+        const double D0 = table_lookup(cZ, P.grid, fm, s) * s + R;
+        const double poly = coef0 + coef1 * (q * p * c * P.reg.inv_k2);
+        dst[t] = make_double2(D0, swc[j] * poly);
+        dmin0 = fmin(dmin0, D0);
+      }
+      dmin0 = warp_min(dmin0);
+      __syncwarp();           // every lane's stores to the chunk precede lane 0's release-arrive below
+      if (lane == 0) {
+        P.chunkmin[(size_t)(u * (TP_NPROD / 32)) + pw] = dmin0;
+        mbar_arrive(&full[b]);  // release: the chunk is visible to whoever acquires full[b]
+      }
+    }
+    return;
+  }
+
+  // =============================== consumers ===============================
+  const int grp = tid / TP_FT, tf = tid - grp * TP_FT;
+  const bool warp_leader = (tid & 31) == 0;
+  double m2[MF], acc[MF], dacc[MF];
+  int cur_ft = -1, seg_parity = 0;
+  uint32_t g = 0;
+  for (long long u = u0; u < u1; ++u, ++g) {
+    const int ft = (int)(u / upp);
+    const long long rem = u - (long long)ft * upp;
+    const int e = (int)(rem / NCH), ch = (int)(rem - (long long)e * NCH);
+    const int f0 = ft * tile + tf;
+    const int b = g & 1;
+    if (ft != cur_ft) {
+      cur_ft = ft;
+#pragma unroll
+      for (int k = 0; k < MF; ++k) {
+        const int f = f0 + k * TP_FT;
+        m2[k] = (f < P.n_field) ? P.m2[f] : 1.0;
+      }
+    }
+    if (u == u0 || ch == 0) {
+#pragma unroll
+      for (int k = 0; k < MF; ++k) { acc[k] = 0.0; dacc[k] = 0.0; }
+    }
+    mbar_wait(&full[b], (g >> 1) & 1);
+    const double2* chunk = buf + (size_t)b * chunk_nodes;
+    const int i0 = ch * QC;
+    const int ni = min(QC, nq - i0);
+    for (int il = grp; il < ni; il += TP_GROUPS) {
+      const double2* row = chunk + il * nc;
+      double A[MF], B[MF];
+#pragma unroll
+      for (int k = 0; k < MF; ++k) { A[k] = 0.0; B[k] = 0.0; }
+      int j = 0;
+      for (; j + 4 <= nc; j += 4) tp_batch<MF, WANT_D, 4>(row + j, m2, A, B);
+      for (; j < nc; ++j) tp_batch<MF, WANT_D, 1>(row + j, m2, A, B);
+      const double2 o = souter[i0 + il];
+#pragma unroll
+      for (int k = 0; k < MF; ++k) {
+        const double gq = fast_rcp(o.x + m2[k]);
+        const double wg2 = o.y * (gq * gq);
+        acc[k] = fma(wg2, A[k], acc[k]);
+        if constexpr (WANT_D) dacc[k] = fma(wg2, fma(2.0 * gq, A[k], B[k]), dacc[k]);
+      }
+    }
+    __syncwarp();
+    if (warp_leader) mbar_arrive(&empty[b]);
+    if (ch == NCH - 1 || u == u1 - 1) {
+      // combine the groups in fixed order; partial sum of this CTA for (field tile, p)
+      double* cb = comb + (size_t)seg_parity * ND * TP_GROUPS * tile;
+      seg_parity ^= 1;
+#pragma unroll
+      for (int k = 0; k < MF; ++k) {
+        cb[grp * tile + k * TP_FT + tf] = acc[k];
+        if constexpr (WANT_D) cb[(TP_GROUPS + grp) * tile + k * TP_FT + tf] = dacc[k];
+      }
+      named_bar_sync(1, TP_NCONS);
+      if (grp == 0) {
+        const long long ufirst = (long long)ft * upp + (long long)e * NCH;
+        const int c_first = (int)(((ufirst + 1) * gridDim.x - 1) / U);
+        const int slot = (int)blockIdx.x - c_first;
+        const size_t plane = (size_t)P.n_ext * P.n_field;
+#pragma unroll
+        for (int k = 0; k < MF; ++k) {
+          const int f = f0 + k * TP_FT;
+          if (f < P.n_field) {
+            double r = cb[k * TP_FT + tf];
+#pragma unroll
+            for (int gg = 1; gg < TP_GROUPS; ++gg) r += cb[gg * tile + k * TP_FT + tf];
+            P.part[((size_t)slot * ND) * plane + (size_t)e * P.n_field + f] = r;
+            if constexpr (WANT_D) {
+              double dr = cb[TP_GROUPS * tile + k * TP_FT + tf];
+#pragma unroll
+              for (int gg = 1; gg < TP_GROUPS; ++gg) dr += cb[(TP_GROUPS + gg) * tile + k * TP_FT + tf];
+              P.part[((size_t)slot * 2 + 1) * plane + (size_t)e * P.n_field + f] = dr;
+            }
+          }
+        }
+      }
+    }
+  }
+}
+static size_t tp_main_smem(int nq, int nc, int nt, int chunk_nodes, int mf, bool want_d) {
+  return 16 * (2 * (size_t)chunk_nodes + nq) + 32 * (size_t)nt +
+         8 * (size_t)(2 * ((nq + 1) & ~1) + 2 * ((nc + 1) & ~1) + ((nt + 1) & ~1) + FM_DOUBLES +
+                      2 * (want_d ? 2 : 1) * TP_GROUPS * TP_FT * mf);
+}
+
+__global__ void __launch_bounds__(256) tp_fixup_kernel(const TwoPointParams P) {
+  const long long idx = (long long)blockIdx.x * 256 + threadIdx.x;
+  const long long n_out = (long long)P.n_ext * P.n_field;
+  if (idx >= n_out) return;
+  const int f = (int)(idx % P.n_field), e = (int)(idx / P.n_field);
+  const int n_ftiles = (P.n_field + P.tile - 1) / P.tile;
+  const long long upp = (long long)P.n_ext * P.NCH, U = (long long)n_ftiles * upp;
+  const long long ufirst = (long long)(f / P.tile) * upp + (long long)e * P.NCH, ulast = ufirst + P.NCH - 1;
+  const int c_first = (int)(((ufirst + 1) * P.grid_main - 1) / U), c_last = (int)(((ulast + 1) * P.grid_main - 1) / U);
+  const int nd = P.dout ? 2 : 1;
+  const size_t plane = (size_t)n_out;
+  double r = P.part[idx];
+  for (int s = 1; s <= c_last - c_first; ++s) r += P.part[(size_t)s * nd * plane + idx];
+  P.out[idx] = P.prefactor * r;
+  if (P.dout) {
+    double dr = P.part[plane + idx];
+    for (int s = 1; s <= c_last - c_first; ++s) dr += P.part[((size_t)s * 2 + 1) * plane + idx];
+    P.dout[idx] = -P.prefactor * dr;
+  }
+  if (P.dmin) {
+    constexpr int NW = TP_NPROD / 32;
+    double dm = P.chunkmin[(size_t)U * NW];
+    for (long long t = ufirst * NW; t < (ulast + 1) * NW; ++t) dm = fmin(dm, P.chunkmin[t]);
+    P.dmin[idx] = (dm + P.m2[f]) * P.reg.inv_k2;
+  }
+}
+
+int twopoint_launch(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext, const double* ext, double* out,
+                    double* dmin, int sm_count, cudaStream_t stream) {
+  TwoPointParams P;
+  P.nq = D->q.n; P.nc = D->cos1.n; P.n_field = n_field; P.n_ext = n_ext;
+  P.prefactor = D->prefactor;
+  fill_common(D->reg, D->tab[0], &P.reg, &P.grid);
+  P.fmc = fm_consts();
+  P.xq = D->q.x; P.wq = D->q.w; P.xc = D->cos1.x; P.wc = D->cos1.w; P.Z = D->tab[0].v;
+  P.coef = D->coef; P.m2 = m2; P.pext = ext; P.out = out; P.dmin = dmin; P.dout = D->dout_dm2;
+  // ---- plan: chunk of QC radial nodes per unit, contiguous unit ranges per CTA ----
+  const int mf = n_field > TP_FT ? 2 : 1;
+  P.tile = TP_FT * mf;
+  int qc = TP_CHUNK_NODES / P.nc;
+  qc = qc > 8 ? 8 : qc;
+  qc = qc > P.nq ? P.nq : qc;
+  P.QC = qc;
+  P.NCH = (P.nq + qc - 1) / qc;
+  const int n_ftiles = (n_field + P.tile - 1) / P.tile;
+  const long long upp = (long long)n_ext * P.NCH, U = (long long)n_ftiles * upp;
+  P.grid_main = (int)(U < sm_count ? U : sm_count);
+  P.max_slots = 1;
+  for (long long seg = 0; seg < (long long)n_ftiles * n_ext; ++seg) {
+    const long long ufirst = seg * P.NCH, ulast = ufirst + P.NCH - 1;
+    const int c0 = (int)(((ufirst + 1) * P.grid_main - 1) / U), c1 = (int)(((ulast + 1) * P.grid_main - 1) / U);
+    if (c1 - c0 + 1 > P.max_slots) P.max_slots = c1 - c0 + 1;
+  }
+  const bool want_d = D->dout_dm2 != nullptr;
+  const size_t n_chunkmin = ((size_t)U * (TP_NPROD / 32) + 2) & ~(size_t)1,
+               n_part = (size_t)P.max_slots * (want_d ? 2 : 1) * n_ext * n_field;
+  void* scratch = nullptr;
+  int rc = scratch_alloc(&scratch, (n_chunkmin + n_part) * sizeof(double), stream);
+  if (rc != DFRG_OK) return rc;
+  P.chunkmin = (double*)scratch;
+  P.part = P.chunkmin + n_chunkmin;
+  const size_t smem_main = tp_main_smem(P.nq, P.nc, P.grid.n, P.QC * P.nc, mf, want_d);
+  void (*kmain)(const TwoPointParams) =
+      mf == 2 ? (want_d ? tp_main_kernel<2, true> : tp_main_kernel<2, false>)
+              : (want_d ? tp_main_kernel<1, true> : tp_main_kernel<1, false>);
+  if (smem_main > kMaxDynSmem) { scratch_free(scratch, stream); return DFRG_EUNSUPPORTED; }
+  rc = opt_in_max_smem(kmain);
+  if (rc != DFRG_OK) { scratch_free(scratch, stream); return rc; }
+  kmain<<<P.grid_main, TP_THREADS, smem_main, stream>>>(P);
+  const long long n_out = (long long)n_ext * n_field;
+  tp_fixup_kernel<<<(unsigned)((n_out + 255) / 256), 256, 0, stream>>>(P);
+  rc = check_cuda(cudaGetLastError());
+  scratch_free(scratch, stream);
+  return rc;
+}
+
+}  // namespace dfrg

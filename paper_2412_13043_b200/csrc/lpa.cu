@@ -220,6 +220,13 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_fermion_kernel(const LpaParam
   }
 }
 
+// dynamic shared memory of one CTA: the (D0, W) table over (n >= 0, q) plus the staged rule and the log/exp tables
+static size_t lpa_smem(const dfrg_lpa_desc* D) {
+  const size_t n_terms = (D->T > 0.0) ? (size_t)D->n_max + 1 : 1;
+  const bool fermi = D->statistics == DFRG_STAT_FERMION;
+  return n_terms * D->q.n * (fermi ? 32 : 16) + (2 * (size_t)((D->q.n + 1) & ~1) + FM_DOUBLES) * 8;
+}
+
 static int lpa_launch(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u, const double* du,
                       double* flow, double* chan, double* dmin, cudaStream_t stream) {
   LpaParams P;
@@ -229,13 +236,13 @@ static int lpa_launch(const dfrg_lpa_desc* D, int n_field, const double* rho, co
   P.fmc = fm_consts();
   P.xq = D->q.x; P.wq = D->q.w; P.rho = rho; P.u = u; P.du = du;
   P.flow = flow; P.chan = chan; P.dmin = dmin; P.dchan = D->dchan;
-  const int n_terms = (D->T > 0.0) ? D->n_max + 1 : 1;
   const bool fermi = D->statistics == DFRG_STAT_FERMION;
-  const size_t smem = (size_t)n_terms * D->q.n * (fermi ? 32 : 16) + (2 * (size_t)((D->q.n + 1) & ~1) + FM_DOUBLES) * 8;
+  const size_t smem = lpa_smem(D);
   auto kern = fermi ? (D->dchan ? lpa_fermion_kernel<true> : lpa_fermion_kernel<false>)
                     : (D->dchan ? lpa_kernel<true> : lpa_kernel<false>);
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return check_cuda(e);
+  if (smem > kMaxDynSmem) return DFRG_EUNSUPPORTED;   // (lpa_validate bounds the table; this is the exact size)
+  const int rca = opt_in_max_smem(kern);
+  if (rca != DFRG_OK) return rca;
   const int grid = (n_field + LPA_FTILE - 1) / LPA_FTILE;
   kern<<<grid, LPA_THREADS, smem, stream>>>(P);
   return check_cuda(cudaGetLastError());
@@ -257,6 +264,7 @@ static int lpa_validate(const dfrg_lpa_desc* D, int n_field, const double* rho, 
     return DFRG_EINVAL;
   }
   if (n_terms * D->q.n > LPA_MAX_PAIRS) return DFRG_EUNSUPPORTED;
+  if (lpa_smem(D) > kMaxDynSmem) return DFRG_EUNSUPPORTED;   // the table, the rule and the log/exp tables must fit one CTA
   return DFRG_OK;
 }
 

@@ -33,6 +33,7 @@ static int mats3d_validate(const dfrg_mats3d_desc* D, int n_field, const double*
   if ((long long)D->q.n * D->cos1.n > M3_MAX_PAIRS || D->tab_psi.n_q > 1024) return DFRG_EUNSUPPORTED;
   if ((long long)n_p * n_jext > 2147483647LL || n_p > 65535) return DFRG_EUNSUPPORTED;
   if ((D->reg_arg4d != 0 && D->reg_arg4d != 1) || !(D->mu == D->mu)) return DFRG_EINVAL;
+  if (D->path < 0 || D->path > 63) return DFRG_EINVAL;
   if (D->mu != 0.0) {
     if (D->reg_arg4d != 0 || !D->out_im) return DFRG_EINVAL;   // complex time component: spatial regulators only
     if ((D->dout_dm2_psi && !D->dout_dm2_psi_im) || (D->dout_dm2_phi && !D->dout_dm2_phi_im)) return DFRG_EINVAL;
@@ -44,10 +45,10 @@ static int mats3d_validate(const dfrg_mats3d_desc* D, int n_field, const double*
 template <int GROUPS, int MF>
 static int mats3d_launch_main(const Mats3dParams& P, int sm_count, cudaStream_t stream) {
   const size_t smem = mats3d_main_smem(P.nq, P.nc, P.row_stride, P.psi_stride, GROUPS, MF);
-  if (smem > 227 * 1024) return DFRG_EUNSUPPORTED;
+  if (smem > kMaxDynSmem) return DFRG_EUNSUPPORTED;
   auto kern = P.mode == 2 ? mats3d_main_kernel<GROUPS, MF, true> : mats3d_main_kernel<GROUPS, MF, false>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return check_cuda(e);
+  const int rca = opt_in_max_smem(kern);
+  if (rca != DFRG_OK) return rca;
   const long long n_ftiles = (P.n_field + M3_FT * MF - 1) / (M3_FT * MF);
   const long long n_items = (long long)P.n_p * P.n_jext * n_ftiles;
   const int grid = (int)(n_items < sm_count ? n_items : sm_count);
@@ -103,15 +104,14 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   P.psi_im = nullptr; P.psimin_f = nullptr; P.out_im = nullptr; P.part_im = nullptr;
   const bool cplx = D->mu != 0.0;
 
-  // ---- path: moment factorisation where an instantiation exists (DFRG_M3_PATH=generic forces the other one) ----
-  const char* vpath = getenv("DFRG_M3_PATH");
-  // DFRG_M3_PATH: "generic" forces the row-streaming kernel, "moment-generic" the any-shape moment kernel (tuning knobs)
-  bool moment = n_jext <= 32 && (cplx || !(vpath && vpath[0] == 'g'));
+  // ---- path: moment factorisation wherever it applies; dfrg_mats3d_desc::path overrides (testing / tuning) ----
+  const int path = D->path;
+  bool moment = n_jext <= 32 && (cplx || !(path & DFRG_M3_ROW_STREAMING));
   MomentPlan pl = {};
+  pl.any_shape_forced = (path & DFRG_M3_ANY_SHAPE) != 0;
   if (moment) {
-    const char* vm = getenv("DFRG_M3_MF");
-    pl.generic = !mats3d_moment_shape(D->n_max, n_jext) || (vpath && vpath[0] == 'm');
-    pl.variant = n_field <= 256 ? 2 : ((vm && atoi(vm) == 1) ? 1 : 0);   // MF 2 x 256, MF 1 x 512 (knob), MF 1 x 256 threads
+    pl.generic = !mats3d_moment_shape(D->n_max, n_jext) || (path & DFRG_M3_ANY_SHAPE);
+    pl.variant = n_field <= 256 ? 2 : ((path & DFRG_M3_ONE_FIELD) ? 1 : 0);   // MF 2 x 256, MF 1 x 512, MF 1 x 256 threads
     if (pl.generic && (n_jext > 16 || pl.variant == 1)) pl.variant = 2;  // any-shape kernel: 256 threads only
     if (cplx) { pl.generic = true; pl.variant = 2; }                     // complex kernel: one field point per thread
     pl.tile = pl.variant == 2 ? 256 : 512;
@@ -136,10 +136,7 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
     }
   }
   P.phi_layout = moment ? 1 : 0;
-  {
-    const char* vs = getenv("DFRG_M3_SYM");
-    P.sym_try = (moment && (P.nc % (2 * M3_NBAT)) == 0 && !(vs && vs[0] == '0')) ? 1 : 0;
-  }
+  P.sym_try = (moment && (P.nc % (2 * M3_NBAT)) == 0 && !(path & DFRG_M3_PLAIN_MOMENTS)) ? 1 : 0;
   P.tile_fields = pl.tile; P.max_slots = pl.max_slots; P.grid_main = pl.grid;
 
   const int n_terms = 2 * D->n_max + 1;
@@ -200,13 +197,11 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
         rc = check_cuda(cudaGetLastError());
       }
     } else {
-      // generic path: consumer groups per CTA (radial nodes are dealt round-robin to the groups) and field points per
-      // thread; DFRG_M3_GROUPS / DFRG_M3_MF override the defaults (tuning knobs)
-      const char* vg = getenv("DFRG_M3_GROUPS");
-      const char* vm = getenv("DFRG_M3_MF");
+      // row-streaming path: consumer groups per CTA (radial nodes are dealt round-robin to the groups) and field points
+      // per thread; dfrg_mats3d_desc::path overrides the defaults
       int mf = n_field > 2 * M3_FT ? 4 : (n_field > M3_FT ? 2 : 1);
-      if (vm && atoi(vm) >= 1 && atoi(vm) < mf) mf = atoi(vm) == 3 ? 2 : atoi(vm);
-      const int groups = vg ? atoi(vg) : 6;
+      if (path & DFRG_M3_ONE_FIELD) mf = 1;
+      const int groups = (path & DFRG_M3_GROUPS_7) ? 7 : ((path & DFRG_M3_GROUPS_4) ? 4 : 6);
       if (mf == 4) {
         if (groups == 7) rc = mats3d_launch_main<7, 4>(P, sm_count, stream);
         else if (groups == 4) rc = mats3d_launch_main<4, 4>(P, sm_count, stream);

@@ -7,13 +7,12 @@ namespace dfrg {
 // generic-shape moment kernel: NJ = the smallest compiled value >= n_jext
 template <int NJ, bool SYM>
 static int mats3d_gmoment_go(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream) {
-  cudaError_t e;
 #define DFRG_M3_GGO(MF)                                                                                              \
   {                                                                                                                  \
     auto kern = P.mode == 2 ? mats3d_gmoment_kernel<NJ, MF, 256, true, SYM>                                          \
                             : mats3d_gmoment_kernel<NJ, MF, 256, false, SYM>;                                        \
-    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);                       \
-    if (e != cudaSuccess) return check_cuda(e);                                                                      \
+    const int rca = opt_in_max_smem(kern);                                                                           \
+    if (rca != DFRG_OK) return rca;                                                                                  \
     kern<<<pl.grid, 256, pl.smem, stream>>>(P);                                                                      \
   }
   if constexpr (NJ <= 16) {
@@ -44,12 +43,11 @@ template <int NJ, bool SYM>
 static int mats3d_cmoment_go(Mats3dParams& P, const MomentPlan& pl, cudaStream_t stream) {
   auto kern = P.mode == 2 ? mats3d_cmoment_kernel<NJ, SYM, true> : mats3d_cmoment_kernel<NJ, SYM, false>;
   if constexpr (NJ == 16) {   // BASELINE config 4's shape: pair code enumerated at compile time
-    const char* vpath = getenv("DFRG_M3_PATH");
-    if (P.n_max == 11 && P.n_jext == 16 && !(vpath && vpath[0] == 'm'))
+    if (P.n_max == 11 && P.n_jext == 16 && !pl.any_shape_forced)
       kern = P.mode == 2 ? mats3d_cmoment_kernel<16, SYM, true, 11> : mats3d_cmoment_kernel<16, SYM, false, 11>;
   }
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
-  if (e != cudaSuccess) return check_cuda(e);
+  const int rca = opt_in_max_smem(kern);
+  if (rca != DFRG_OK) return rca;
   kern<<<pl.grid, 256, pl.smem, stream>>>(P);
   return check_cuda(cudaGetLastError());
 }

@@ -1348,6 +1348,7 @@ struct MomentPlan {
   int tile, grid, max_slots;
   size_t smem;
   bool generic;    // mats3d_gmoment_kernel (any n_max, n_jext <= 32) instead of a specialised instantiation
+  bool any_shape_forced;   // dfrg_mats3d_desc::path & DFRG_M3_ANY_SHAPE: no compile-time-enumerated instantiation
 };
 
 }  // namespace dfrg

@@ -11,6 +11,7 @@ import os
 import numpy as np
 import pytest
 
+from paper_2412_13043_b200 import binding as B
 from paper_2412_13043_b200 import inputs
 
 from helpers import assert_dmin, assert_parity, gpu_run, make_rules, oracle_run
@@ -189,17 +190,13 @@ def test_matsubara_moment_path_small(n_field, n_p, n_jext, n_q, n_c, n_max, inte
     c["n_max"] = n_max
     what = "mats_moment_%d_%d_%d_%d_%d_%d_i%d" % (n_field, n_p, n_jext, n_q, n_c, n_max, interp)
     g, o, _ = run_both(c, what=what)
-    os.environ["DFRG_M3_PATH"] = "generic"
-    try:
-        g2, _, _ = run_both(c, what=what + "_generic")
-    finally:
-        del os.environ["DFRG_M3_PATH"]
+    c["path"] = B.M3_ROW_STREAMING
+    g2, _, _ = run_both(c, what=what + "_generic")
+    c["path"] = 0
     assert not np.array_equal(g["out"], g2["out"]) or n_field == 1      # two different kernels ran
-    os.environ["DFRG_M3_MF"] = "1"
-    try:
-        run_both(c, what=what + "_mf1")
-    finally:
-        del os.environ["DFRG_M3_MF"]
+    c["path"] = B.M3_ONE_FIELD
+    run_both(c, what=what + "_mf1")
+    c["path"] = 0
 
 
 @pytest.mark.parametrize("n_field,n_p,n_jext,n_q,n_c,n_max", [(700, 2, 3, 10, 8, 3), (1030, 3, 2, 7, 16, 11),
@@ -212,19 +209,15 @@ def test_matsubara_symmetric_pair_moments(n_field, n_p, n_jext, n_q, n_c, n_max)
     c["n_max"] = n_max
     what = "mats_sym_%d_%d_%d_%d_%d_%d" % (n_field, n_p, n_jext, n_q, n_c, n_max)
     g, o, _ = run_both(c, what=what)
-    os.environ["DFRG_M3_SYM"] = "0"
-    try:
-        g2, _, _ = run_both(c, what=what + "_plain")
-    finally:
-        del os.environ["DFRG_M3_SYM"]
+    c["path"] = B.M3_PLAIN_MOMENTS
+    g2, _, _ = run_both(c, what=what + "_plain")
+    c["path"] = 0
     assert not np.array_equal(g["out"], g2["out"])                       # two different loops ran
     c["rule_c"] = (n_c, -1.0, 0.5)
     g3, _, _ = run_both(c, what=what + "_asymmetric_rule")
-    os.environ["DFRG_M3_SYM"] = "0"
-    try:
-        g4, _, _ = run_both(c, what=what + "_asymmetric_rule_plain")
-    finally:
-        del os.environ["DFRG_M3_SYM"]
+    c["path"] = B.M3_PLAIN_MOMENTS
+    g4, _, _ = run_both(c, what=what + "_asymmetric_rule_plain")
+    c["path"] = 0
     assert np.array_equal(g3["out"], g4["out"])                          # the fallback is the plain loop, bit for bit
 
 
@@ -238,11 +231,9 @@ def test_matsubara_any_shape_moment_kernel(n_field, n_p, n_jext, n_q, n_c, n_max
     c = inputs.config4(n_field=n_field, n_p=n_p, n_jext=n_jext, n_q=n_q, n_c=n_c, n_freq=64)
     c["n_max"] = n_max
     what = "mats_anyshape_%d_%d_%d_%d_%d_%d" % (n_field, n_p, n_jext, n_q, n_c, n_max)
-    os.environ["DFRG_M3_PATH"] = "moment-generic"
-    try:
-        g, o, _ = run_both(c, what=what)
-    finally:
-        del os.environ["DFRG_M3_PATH"]
+    c["path"] = B.M3_ANY_SHAPE
+    g, o, _ = run_both(c, what=what)
+    c["path"] = 0
     g2, _, _ = run_both(c, what=what + "_default")
     if (n_max, n_jext) in ((3, 3), (11, 16)):        # specialised kernel by default: same sums, possibly another rounding
         fin = np.isfinite(g2["out"])

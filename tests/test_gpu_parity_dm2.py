@@ -6,6 +6,7 @@ import os
 import numpy as np
 import pytest
 
+from paper_2412_13043_b200 import binding as B
 from paper_2412_13043_b200 import inputs
 
 from helpers import assert_parity, gpu_run, make_rules, oracle_run, oracle_run_dm2
@@ -73,11 +74,9 @@ def test_matsubara_derivatives_small(n_field, n_p, n_jext, n_q, n_c, n_max, inte
     c["n_max"] = n_max
     what = "mats_dm2_%d_%d_%d_%d_%d_%d" % (n_field, n_p, n_jext, n_q, n_c, n_max)
     g, _ = check(c, ["dpsi", "dphi"], what=what)
-    os.environ["DFRG_M3_PATH"] = "generic"
-    try:
-        g2, _ = check(c, ["dpsi", "dphi"], what=what + "_generic")
-    finally:
-        del os.environ["DFRG_M3_PATH"]
+    c["path"] = B.M3_ROW_STREAMING
+    g2, _ = check(c, ["dpsi", "dphi"], what=what + "_generic")
+    c["path"] = 0
 
 
 def test_matsubara_derivatives_full_config4_sampled():
