@@ -1,6 +1,7 @@
 // loop4d_grid.cu -- three-point family of dfrg_integrate_loop4d on a product grid of external momenta
 // (dfrg_loop4d_desc::ext_outer; BASELINE.json config 3 as bench.py runs it), 1-D and 3-D vertex tables.
 #include "loop4d_kernels.cuh"
+#include <cstdlib>
 
 namespace dfrg {
 
@@ -152,12 +153,12 @@ __global__ void __launch_bounds__(T3G_THREADS, 1) t3g_prepass_kernel(const Three
         Xa *= X;
       }
     }
-    double* ta = Q.tabA + ((size_t)pair * 8) * G + a;
+    double2* ta = reinterpret_cast<double2*>(Q.tabA + ((size_t)pair * G + a) * 8);
     const double w0 = wpair * (Ga * lam1);
-    ta[0] = TAB3D ? s_a : s_a * third;
-#pragma unroll
-    for (int c = 0; c < 5; ++c) ta[(size_t)(1 + c) * G] = w0 * gam[c];
-    ta[(size_t)7 * G] = Da;
+    ta[0] = make_double2(TAB3D ? s_a : s_a * third, w0 * gam[0]);
+    ta[1] = make_double2(w0 * gam[1], w0 * gam[2]);
+    ta[2] = make_double2(w0 * gam[3], w0 * gam[4]);
+    ta[3] = make_double2(0.0, Da);
   }
 }
 
@@ -167,11 +168,13 @@ __global__ void __launch_bounds__(T3G_THREADS, 1) t3g_prepass_kernel(const Three
 struct T3MShared {
   double* lgmem;
   double4 *cL3, *cZA;
-  double *fxmem, *fmmem, *sxq, *sx1, *sx2, *sw2, *sZA, *sL3;
+  double *fxmem, *fmmem, *sxq, *sx1, *ssin1, *sx2, *sw2, *sZA, *sL3;
   double2 *xw2, *nodeA;
+  double4* ptab;
   double *rowc, *nodeS, *red, *stab3;
 };
-__device__ __forceinline__ T3MShared t3m_carve(unsigned char* raw, int nq, int n1, int n2, int nt, int nodes, int nt_thr) {
+__device__ __forceinline__ T3MShared t3m_carve(unsigned char* raw, int nq, int n1, int n2, int nt, int nodes, int kp,
+                                               int nt_thr) {
   T3MShared s;
   s.lgmem = reinterpret_cast<double*>(raw);
   s.cL3 = reinterpret_cast<double4*>(s.lgmem + LG_DOUBLES);
@@ -180,46 +183,48 @@ __device__ __forceinline__ T3MShared t3m_carve(unsigned char* raw, int nq, int n
   s.fmmem = s.fxmem + FX_DOUBLES;
   s.sxq = s.fmmem + FM_DOUBLES;
   s.sx1 = s.sxq + ((nq + 1) & ~1);
-  s.sx2 = s.sx1 + ((n1 + 1) & ~1);
+  s.ssin1 = s.sx1 + ((n1 + 1) & ~1);
+  s.sx2 = s.ssin1 + ((n1 + 1) & ~1);
   s.sw2 = s.sx2 + ((n2 + 1) & ~1);
   s.sZA = s.sw2 + ((n2 + 1) & ~1);
   s.sL3 = s.sZA + ((nt + 1) & ~1);
   s.xw2 = reinterpret_cast<double2*>(s.sL3 + ((nt + 1) & ~1));
   s.nodeA = s.xw2 + n2;                                       // [2][nodes] (w2 G_A(s_b) lambda3(.), z)
-  s.rowc = reinterpret_cast<double*>(s.nodeA + 2 * nodes);    // [2][nodes] (q^2 + p2^2)/3 of the row (one per pair)
-  s.nodeS = s.rowc + 2 * nodes;                               // [2][nodes] s_b        (TAB3D only)
+  s.ptab = reinterpret_cast<double4*>(s.nodeA + 2 * nodes);   // [2][kp]    (zc, zs, q^2, -) of a pair
+  s.rowc = reinterpret_cast<double*>(s.ptab + 2 * kp);        // [2][kp]    (q^2 + p2^2)/3 of the row (one per pair)
+  s.nodeS = s.rowc + 2 * kp;                                  // [2][nodes] s_b        (TAB3D only)
   s.red = s.nodeS + 2 * nodes;                                // [threads]
   s.stab3 = s.red + nt_thr;                                   // [ntab3]               (TAB3D only)
   return s;
 }
-static size_t t3m_smem(int nq, int n1, int n2, int nt, int nodes, int threads, int ntab3) {
-  return 8 * (size_t)(LG_DOUBLES + 2 * 4 * (nt + 1) + FX_DOUBLES + FM_DOUBLES + ((nq + 1) & ~1) + ((n1 + 1) & ~1) +
-                      2 * ((n2 + 1) & ~1) + 2 * ((nt + 1) & ~1) + 2 * n2 + 2 * 2 * nodes + 2 * nodes + 2 * nodes + threads +
-                      ((ntab3 + 1) & ~1));
+static size_t t3m_smem(int nq, int n1, int n2, int nt, int nodes, int kp, int threads, int ntab3) {
+  return 8 * (size_t)(LG_DOUBLES + 2 * 4 * (nt + 1) + FX_DOUBLES + FM_DOUBLES + ((nq + 1) & ~1) + 2 * ((n1 + 1) & ~1) +
+                      2 * ((n2 + 1) & ~1) + 2 * ((nt + 1) & ~1) + 2 * n2 + 2 * 2 * nodes + 2 * 4 * kp + 2 * kp +
+                      2 * nodes + threads + ((ntab3 + 1) & ~1));
 }
 
 // Hot loop (1-D vertex table), per (a, r, node):  x = (s_c + s_a + s_b)/3 = up + m2k23 z  with  up = (s_c + s_a + q^2 + p2^2)/3
 // per row and z the node's q.p2/k^2 (so the node record is one 16-byte broadcast (w, z)); t' = lg2_coord(x); the cell of
-// lambda3 lives in registers (kc, Fc, Fd) and is reloaded only when floor(t') changes; quartic Horner in z; two
-// multiply-adds.  17 FP64 instructions.  Along a row x is monotone in the c2 node (s_b is affine in c2), so when the two
-// end nodes of the row fall into the same cell for every lane of the warp (the common case: cells are 25 % wide in x)
-// the interior nodes skip floor / clamp / compare / reload altogether (FAST).  Both paths do the same arithmetic in the
-// same order: results are bit-identical whichever runs.
+// lambda3 lives in registers (cc.k, cc.Fd) and is reloaded only when t' leaves it: tau = t' - Fd lies in [0, 1) exactly when
+// the high word of tau, read as an unsigned integer, is below that of 1.0 (negative, >= 1 and NaN all fail), so the test is
+// one integer compare off the FP64 pipe; cubic in tau; quartic Horner in z; two multiply-adds.  17 FP64 instructions.
+// Along a row x is monotone in the c2 node (s_b is affine in c2) and a cell is 25 % wide in x, so 9 nodes in 10 stay in
+// the cell of their predecessor.  Whether the cell is reloaded or not, tau = t' - floor(t') (clamped) is the same number.
 struct CellCache {
   double4 k;
   double Fd;
-  unsigned Fc;
 };
-template <bool FAST>
 __device__ __forceinline__ double t3m_node(const double2 b, const double up, const double m2k23, const LogGrid2& lg,
                                            const double4* __restrict__ cL3, CellCache& cc, const double (&cur)[6],
                                            const double acc2) {
   const double tq = lg2_coord(lg, fma(b.y, m2k23, up));
-  if constexpr (!FAST) {
+  double tau = tq - cc.Fd;
+  if ((unsigned)__double2hiint(tau) >= 0x3ff00000u) {   // (predicated: a branch per node costs more than it saves)
     const unsigned F = lg2_cell(lg, tq);
-    if (F != cc.Fc) { cc.Fc = F; cc.Fd = (double)F; cc.k = cL3[F]; }
+    cc.Fd = (double)F;
+    cc.k = cL3[F];
+    tau = tq - cc.Fd;
   }
-  const double tau = tq - cc.Fd;
   const double lam3 = fma(fma(fma(cc.k.w, tau, cc.k.z), tau, cc.k.y), tau, cc.k.x);
   const double poly = fma(fma(fma(fma(cur[5], b.y, cur[4]), b.y, cur[3]), b.y, cur[2]), b.y, cur[1]);
   return fma(b.x * poly, lam3, acc2);
@@ -235,7 +240,7 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
   const int nq = P.nq, n1 = P.n1, n2 = N2 ? N2 : P.n2, nt = P.grid.n, G = Q.G, S = Q.S, KP = Q.KP, NCH = Q.NCH;
   const int NODES = Q.NODES;
   const int npairs = nq * n1;
-  const T3MShared sm = t3m_carve(smem_raw, nq, n1, n2, nt, NODES, NT);
+  const T3MShared sm = t3m_carve(smem_raw, nq, n1, n2, nt, NODES, KP, NT);
   const int tid = threadIdx.x;
 
   if (tid == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
@@ -256,13 +261,11 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
   cells2_build(sm.cZA, sm.sZA, nt, P.grid.interp);
   if (!TAB3D) cells2_build(sm.cL3, sm.sL3, nt, P.grid.interp);
   for (int j = tid; j < n2; j += NT) sm.xw2[j] = make_double2(sm.sx2[j], sm.sw2[j]);
-  // is the cos2 rule monotone?  (then x is monotone along a row and the row's end nodes bracket its cells)
-  bool mono_up = true, mono_dn = true;
-  for (int j = tid + 1; j < n2; j += NT) {
-    mono_up = mono_up && sm.sx2[j] > sm.sx2[j - 1];
-    mono_dn = mono_dn && sm.sx2[j] < sm.sx2[j - 1];
+  for (int j = tid; j < n1; j += NT) {
+    const double c1 = sm.sx1[j];
+    sm.ssin1[j] = sqrt((1.0 - c1) * (1.0 + c1));
   }
-  const bool mono = __syncthreads_and(mono_up) || __syncthreads_and(mono_dn);   // also publishes the tables
+  __syncthreads();   // publishes the tables
 
   const double ik2 = P.reg.inv_k2, third = 1.0 / 3.0, m2k2 = -2.0 * P.reg.k2;
   const double& m2k23 = Q.m2k23;   // straight from the kernel parameters: a constant-bank operand of the hot loop
@@ -275,77 +278,87 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
   const double p1 = P.ext[3 * ((long long)a * S)];
 
   double dmB_cur = inf, dmB_nxt = inf;
-  // Phase 1: shared node data of unit u into buffer b
-  auto phase1 = [&](long long u, int b, double& dmB) {
+  // Phase 0 (two units ahead): the pair data of unit u -- z = zc + zs c2,  s_b = q^2 + p2^2 - 2 k^2 z
+  auto phase0 = [&](long long u) {
     const int r = (int)(u / NCH), ch = (int)(u - (long long)r * NCH);
     const int pair0 = ch * KP;
     const int npl = min(KP, npairs - pair0);
     const double p2 = Q.tabR[4 * r], ca_ = Q.tabR[4 * r + 1], sa_ = Q.tabR[4 * r + 2];
+    const double pc = p2 * ca_ * ik2, ps = p2 * sa_ * ik2;
+    double4* pt = sm.ptab + (int)((u - u0) & 1) * KP;
+    for (int pl = tid; pl < npl; pl += NT) {
+      const int pair = pair0 + pl;
+      const int i = pair / n1, j1 = pair - i * n1;
+      const double q = sm.sxq[i];
+      pt[pl] = make_double4(q * sm.sx1[j1] * pc, q * sm.ssin1[j1] * ps, q * q, 0.0);
+    }
+  };
+  // Phase 1 (one unit ahead): shared node data of unit u into buffer b
+  auto phase1 = [&](long long u, int b, double& dmB) {
+    const int r = (int)(u / NCH), ch = (int)(u - (long long)r * NCH);
+    const int pair0 = ch * KP;
+    const int npl = min(KP, npairs - pair0);
+    const double p2sq = Q.tabR[4 * r] * Q.tabR[4 * r];
+    const double4* pt = sm.ptab + b * KP;
     double2* nA = sm.nodeA + b * NODES;
-    double* rc = sm.rowc + b * NODES;
+    double* rc = sm.rowc + b * KP;
     double* nS = sm.nodeS + b * NODES;
     for (int n = tid; n < npl * n2; n += NT) {
       const int pl = n / n2, j2 = n - pl * n2;
-      const int pair = pair0 + pl;
-      const int i = pair / n1, j1 = pair - i * n1;
-      const double q = sm.sxq[i], c1 = sm.sx1[j1];
-      const double sq = q * q;
-      const double sin1 = sqrt((1.0 - c1) * (1.0 + c1));
-      const double zc = q * p2 * ca_ * c1 * ik2;
-      const double zs = q * p2 * sa_ * sin1 * ik2;
-      const double sb0 = sq + p2 * p2;
+      const double4 pd = pt[pl];
       const double2 xw = sm.xw2[j2];
-      const double z = fma(zs, xw.x, zc);
+      const double z = fma(pd.y, xw.x, pd.x);
+      const double sb0 = pd.z + p2sq, sb03 = sb0 * third;
       double s_b = fma(m2k2, z, sb0);
       s_b = clamp_lo(s_b, 0.0);
       const double Db = fma(lg2_lookup(sm.cZA, lg, s_b), s_b, t3_reg_R<REGK>(P.reg, fxtab, kc, s_b));
       dmB = fmin(dmB, Db);
-      const double lam2 = TAB3D ? tab3d_vertex(sm.stab3, Q.T3, fm, p2 * p2, sq, s_b)
-                                : lg2_lookup(sm.cL3, lg, fma(s_b, third, sb0 * third));
+      const double lam2 = TAB3D ? tab3d_vertex(sm.stab3, Q.T3, fm, p2sq, pd.z, s_b)
+                                : lg2_lookup(sm.cL3, lg, fma(s_b, third, sb03));
       nA[n] = make_double2(xw.y * (fast_rcp(Db) * lam2), z);
       if (TAB3D) nS[n] = s_b;
-      if (j2 == 0) rc[pl] = sb0 * third;
+      if (j2 == 0) rc[pl] = sb03;
     }
   };
 
   double acc = 0.0;
   CellCache cc;
-  cc.Fc = 0xffffffffu; cc.Fd = 0.0; cc.k = make_double4(0.0, 0.0, 0.0, 0.0);
+  cc.Fd = inf; cc.k = make_double4(0.0, 0.0, 0.0, 0.0);   // tau = t' - inf fails the range test: the first node loads its cell
+  if (u0 < u1) phase0(u0);
+  __syncthreads();
   if (u0 < u1) phase1(u0, 0, dmB_cur);
+  if (u0 + 1 < u1) phase0(u0 + 1);
   __syncthreads();
   for (long long u = u0; u < u1; ++u) {
     const int b = (int)((u - u0) & 1);
     const int r = (int)(u / NCH), ch = (int)(u - (long long)r * NCH);
     const bool last_of_r = (u + 1 == u1) || ((u + 1) / NCH != r);
-    if (u + 1 < u1) phase1(u + 1, b ^ 1, last_of_r ? dmB_nxt : dmB_cur);
-    // ---- phase 2 ----
     const int pair0 = ch * KP;
     const int npl = min(KP, npairs - pair0);
+    // the first row's coefficients: in flight while phase 1 runs
+    double2 c01_first, c23_first, c45_first;
+    if (active && w < npl) {
+      const double2* ta = reinterpret_cast<const double2*>(Q.tabA) + ((size_t)(pair0 + w) * G + a) * 4;
+      c01_first = ta[0]; c23_first = ta[1]; c45_first = ta[2];
+    }
+    if (u + 1 < u1) phase1(u + 1, b ^ 1, last_of_r ? dmB_nxt : dmB_cur);
+    // ---- phase 2 ----
     {
       const double p2 = Q.tabR[4 * r], ca_ = Q.tabR[4 * r + 1];
       double scc = p1 * p1 + p2 * p2 + 2.0 * p1 * p2 * ca_;
       scc = scc > 0.0 ? scc : 0.0;
       const double scc3 = scc * third;
       const double2* nA = sm.nodeA + b * NODES;
-      const double* rc = sm.rowc + b * NODES;
+      const double* rc = sm.rowc + b * KP;
       const double* nS = sm.nodeS + b * NODES;
-      double cur[6], nxt[6];
-      if (active && w < npl) {
-        const double* ta = Q.tabA + ((size_t)(pair0 + w) * 8) * G + a;
-#pragma unroll
-        for (int c = 0; c < 6; ++c) cur[c] = ta[(size_t)c * G];
-      }
-      const int iters = (npl + nw - 1) / nw;   // the same for every thread: the votes below are warp-wide
-      for (int it = 0; it < iters; ++it) {
-        const int pl = w + it * nw;
-        const bool valid = active && pl < npl;
-        if (active && pl + nw < npl) {
-          const double* ta = Q.tabA + ((size_t)(pair0 + pl + nw) * 8) * G + a;
-#pragma unroll
-          for (int c = 0; c < 6; ++c) nxt[c] = ta[(size_t)c * G];
-        }
-        const unsigned vmask = __ballot_sync(0xffffffffu, valid);
-        if (valid) {
+      const double2* ta = reinterpret_cast<const double2*>(Q.tabA) + ((size_t)(pair0 + w) * G + a) * 4;
+      const size_t ta_step = (size_t)nw * G * 4;
+      double2 c01 = c01_first, c23 = c23_first, c45 = c45_first;
+      for (int pl = w; pl < npl; pl += nw) {
+        if (active) {
+          const double cur[6] = {c01.x, c01.y, c23.x, c23.y, c45.x, c45.y};
+          ta += ta_step;
+          if (pl + nw < npl) { c01 = ta[0]; c23 = ta[1]; c45 = ta[2]; }
           const double2* na = nA + pl * n2;
           double acc2 = acc;      // (w0 is folded into the quartic coefficients: the row adds straight into the running sum)
           if constexpr (TAB3D) {
@@ -359,52 +372,19 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
             }
           } else {
             const double up = (cur[0] + scc3) + rc[pl];
-            // the row's last node decides the path; its coordinate is kept for the end of the row
-            const double2 bL = na[n2 - 1];
-            const double tL = lg2_coord(lg, fma(bL.y, m2k23, up));
-            const unsigned FL = lg2_cell(lg, tL);
-            const double2 b0 = na[0];
-            const double t0 = lg2_coord(lg, fma(b0.y, m2k23, up));
-            const unsigned F0 = lg2_cell(lg, t0);
-            if (F0 != cc.Fc) { cc.Fc = F0; cc.Fd = (double)F0; cc.k = sm.cL3[F0]; }
-            {
-              const double tau = t0 - cc.Fd;
-              const double lam3 = fma(fma(fma(cc.k.w, tau, cc.k.z), tau, cc.k.y), tau, cc.k.x);
-              const double poly = fma(fma(fma(fma(cur[5], b0.y, cur[4]), b0.y, cur[3]), b0.y, cur[2]), b0.y, cur[1]);
-              acc2 = fma(b0.x * poly, lam3, acc2);
-            }
-            const bool fast = mono && __all_sync(vmask, F0 == FL);
-            if (fast) {
-              if constexpr (N2 > 0) {
+            if constexpr (N2 > 0) {
 #pragma unroll
-                for (int j2 = 1; j2 < N2 - 1; ++j2) acc2 = t3m_node<true>(na[j2], up, m2k23, lg, sm.cL3, cc, cur, acc2);
-              } else {
-#pragma unroll 4
-                for (int j2 = 1; j2 < n2 - 1; ++j2) acc2 = t3m_node<true>(na[j2], up, m2k23, lg, sm.cL3, cc, cur, acc2);
-              }
+              for (int j2 = 0; j2 < N2; ++j2) acc2 = t3m_node(na[j2], up, m2k23, lg, sm.cL3, cc, cur, acc2);
             } else {
-              if constexpr (N2 > 0) {
-#pragma unroll
-                for (int j2 = 1; j2 < N2 - 1; ++j2) acc2 = t3m_node<false>(na[j2], up, m2k23, lg, sm.cL3, cc, cur, acc2);
-              } else {
 #pragma unroll 4
-                for (int j2 = 1; j2 < n2 - 1; ++j2) acc2 = t3m_node<false>(na[j2], up, m2k23, lg, sm.cL3, cc, cur, acc2);
-              }
-            }
-            if (n2 > 1) {
-              if (FL != cc.Fc) { cc.Fc = FL; cc.Fd = (double)FL; cc.k = sm.cL3[FL]; }
-              const double tau = tL - cc.Fd;
-              const double lam3 = fma(fma(fma(cc.k.w, tau, cc.k.z), tau, cc.k.y), tau, cc.k.x);
-              const double poly = fma(fma(fma(fma(cur[5], bL.y, cur[4]), bL.y, cur[3]), bL.y, cur[2]), bL.y, cur[1]);
-              acc2 = fma(bL.x * poly, lam3, acc2);
+              for (int j2 = 0; j2 < n2; ++j2) acc2 = t3m_node(na[j2], up, m2k23, lg, sm.cL3, cc, cur, acc2);
             }
           }
           acc = acc2;
         }
-#pragma unroll
-        for (int c = 0; c < 6; ++c) cur[c] = nxt[c];
       }
     }
+    if (u + 2 < u1) phase0(u + 2);
     if (last_of_r) {
       // partial sums of this CTA for r: slot = rank of this CTA among the owners of r's units
       const long long ufirst = (long long)r * NCH;
@@ -445,7 +425,7 @@ __global__ void __launch_bounds__(256) t3g_fixup_kernel(const ThreeGridParams Q)
     double dm = *Q.qmin;
     for (int s = 0; s <= c_last - c_first; ++s) dm = fmin(dm, Q.partB[(size_t)s * S + r]);
     const int npairs = P.nq * P.n1;
-    for (int pair = 0; pair < npairs; ++pair) dm = fmin(dm, Q.tabA[((size_t)pair * 8 + 7) * G + a]);
+    for (int pair = 0; pair < npairs; ++pair) dm = fmin(dm, Q.tabA[((size_t)pair * G + a) * 8 + 7]);
     P.dmin[e] = dm * P.reg.inv_k2;
   }
 }
@@ -458,22 +438,32 @@ int t3g_launch(ThreePointParams& P, int G, int regk, const Tab3DParams* T3, cons
   const size_t smem_pre = t3g_smem(P.nq, P.n1, P.n2, P.grid.n, T3 ? ntab3 : 0);
   if (smem_pre > kMaxDynSmem) return DFRG_OK;   // (large 3-D tables: the general kernel)
   // node buffer of the main kernel: the largest of 2048 / 1024 / 512 nodes that fits (fewer, longer work units)
+  const int npairs = P.nq * P.n1;
+  int NTX = T3G_MAXT;
+  if (const char* ev = getenv("DFRG_T3G_NT")) NTX = atoi(ev);   // EXPERIMENT
+  const int nw = NTX / G;   // pair slots of the main kernel
+  auto pairs_per_unit = [&](int nodes_) {
+    int kp = nodes_ / P.n2 < npairs ? nodes_ / P.n2 : npairs;
+    if (kp > nw) kp -= kp % nw;   // whole rounds of the pair slots
+    return kp;
+  };
   int nodes = 2048;
   while (nodes > T3G_NODES && (nodes / 2 >= P.n2) &&
-         t3m_smem(P.nq, P.n1, P.n2, P.grid.n, nodes, T3G_MAXT, T3 ? ntab3 : 0) > 160 * 1024) nodes /= 2;
+         t3m_smem(P.nq, P.n1, P.n2, P.grid.n, nodes, pairs_per_unit(nodes), NTX, T3 ? ntab3 : 0) > 176 * 1024)
+    nodes /= 2;
   if (nodes < P.n2) nodes = T3G_NODES;
-  const size_t smem_main = t3m_smem(P.nq, P.n1, P.n2, P.grid.n, nodes, T3G_MAXT, T3 ? ntab3 : 0);
+  const int kp = pairs_per_unit(nodes);
+  const size_t smem_main = t3m_smem(P.nq, P.n1, P.n2, P.grid.n, nodes, kp, NTX, T3 ? ntab3 : 0);
   if (smem_main > kMaxDynSmem) return DFRG_OK;
   ThreeGridParams Q;
   Q.B = P;
   Q.G = G; Q.S = n_ext / G;
   Q.v3 = v3; Q.ntab3 = ntab3;
   if (T3) Q.T3 = *T3;
-  const int npairs = P.nq * P.n1;
   Q.NODES = nodes;
   Q.lgc = lg2_consts(P.grid.lo, P.grid.inv_h);
   Q.m2k23 = -2.0 * P.reg.k2 * (1.0 / 3.0);
-  Q.KP = nodes / P.n2 < npairs ? nodes / P.n2 : npairs;
+  Q.KP = kp;
   Q.NCH = (npairs + Q.KP - 1) / Q.KP;
   const long long U = (long long)Q.S * Q.NCH;
   Q.grid_main = (int)(U < sm_count ? U : sm_count);
@@ -507,12 +497,15 @@ int t3g_launch(ThreePointParams& P, int G, int regk, const Tab3DParams* T3, cons
   }
   DFRG_T3G_PICK(0) DFRG_T3G_PICK(1) DFRG_T3G_PICK(2)
 #undef DFRG_T3G_PICK
+  if (NTX == 768 && regk == 1 && !T3 && n2_16) kmain = t3g_main_kernel<1, 768, 16, false>;
+  if (NTX == 256 && regk == 1 && !T3 && n2_16) kmain = t3g_main_kernel<1, 256, 16, false>;
+  if (NTX == 384 && regk == 1 && !T3 && n2_16) kmain = t3g_main_kernel<1, 384, 16, false>;
   int rca = e == cudaSuccess ? DFRG_OK : check_cuda(e);
   if (rca == DFRG_OK) rca = opt_in_max_smem(kpre);
   if (rca == DFRG_OK) rca = opt_in_max_smem(kmain);
   if (rca != DFRG_OK) { scratch_free(scratch, stream); *scratch_out = nullptr; return rca; }
   kpre<<<sm_count, T3G_THREADS, smem_pre, stream>>>(Q);
-  kmain<<<Q.grid_main, T3G_MAXT, smem_main, stream>>>(Q);
+  kmain<<<Q.grid_main, NTX, smem_main, stream>>>(Q);
   t3g_fixup_kernel<<<(n_ext + 255) / 256, 256, 0, stream>>>(Q);
   rc = check_cuda(cudaGetLastError());
   if (rc != DFRG_OK) { scratch_free(scratch, stream); *scratch_out = nullptr; return rc; }
