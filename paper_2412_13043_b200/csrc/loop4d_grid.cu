@@ -1,7 +1,6 @@
 // loop4d_grid.cu -- three-point family of dfrg_integrate_loop4d on a product grid of external momenta
 // (dfrg_loop4d_desc::ext_outer; BASELINE.json config 3 as bench.py runs it), 1-D and 3-D vertex tables.
 #include "loop4d_kernels.cuh"
-#include <cstdlib>
 
 namespace dfrg {
 
@@ -19,14 +18,15 @@ namespace dfrg {
 // on the device and, if it does not hold, the product-grid kernels return at once and the general kernel runs instead
 // (both are enqueued; the one that is not needed exits after reading one flag).
 //
-//  (1) t3g_prepass_kernel: promise check; tabR[r] = (|p2|, cos alpha, sin alpha); tabA[pair][0..7][a] for every (q, c1) pair:
+//  (1) t3g_prepass_kernel: promise check; tabR[r] = (|p2|, cos alpha, sin alpha); tabA[pair][a][0..7] for every (q, c1) pair:
 //        s_a/3,  the five quartic coefficients times w0 = wq q^3 Rdot(q^2) G_A(q^2) w1 sqrt(1-c1^2) G_A(s_a) lambda3(.),  D_a.
 //  (2) t3g_main_kernel: persistent, one CTA per SM.  Work unit = (r, chunk of KP pairs); the units are dealt to the
-//      CTAs in contiguous ranges.  Phase 1 (all threads, one unit ahead, double buffered): the shared node data
-//      (w2 G_A(s_b) lambda3(.), s_b/3, z) of the unit's KP x n2 nodes into shared memory.  Phase 2: thread = (a, pair
-//      slot); per node one look-up, one Horner, two multiply-adds; the shared node data are warp-uniform broadcasts.
-//      A thread keeps the running sum of its a while the CTA stays inside one r; the partial sums of an output are
-//      written per CTA ("slot") and added in fixed order by
+//      CTAs in contiguous ranges.  Phase 0 (two units ahead): the unit's pair data (q.p2 split into its c2-independent and
+//      c2-proportional parts, q^2).  Phase 1 (all threads, one unit ahead, double buffered): the shared node data
+//      (w2 G_A(s_b) lambda3(.), z) of the unit's KP x n2 nodes into shared memory.  Phase 2: thread = (a, pair slot); per
+//      node one coordinate, the cell of lambda3 cached in registers, one Horner, two multiply-adds; the shared node data
+//      are warp-uniform broadcasts.  A thread keeps the running sum of its a while the CTA stays inside one r; the partial
+//      sums of an output are written per CTA ("slot") and added in fixed order by
 //  (3) t3g_fixup_kernel (deterministic: the ownership of units is a pure function of the grid size).
 
 // common shared-memory carve-up of the two product-grid kernels
@@ -279,13 +279,12 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
 
   double dmB_cur = inf, dmB_nxt = inf;
   // Phase 0 (two units ahead): the pair data of unit u -- z = zc + zs c2,  s_b = q^2 + p2^2 - 2 k^2 z
-  auto phase0 = [&](long long u) {
-    const int r = (int)(u / NCH), ch = (int)(u - (long long)r * NCH);
+  auto phase0 = [&](const int r, const int ch, const int b) {
     const int pair0 = ch * KP;
     const int npl = min(KP, npairs - pair0);
     const double p2 = Q.tabR[4 * r], ca_ = Q.tabR[4 * r + 1], sa_ = Q.tabR[4 * r + 2];
     const double pc = p2 * ca_ * ik2, ps = p2 * sa_ * ik2;
-    double4* pt = sm.ptab + (int)((u - u0) & 1) * KP;
+    double4* pt = sm.ptab + b * KP;
     for (int pl = tid; pl < npl; pl += NT) {
       const int pair = pair0 + pl;
       const int i = pair / n1, j1 = pair - i * n1;
@@ -294,8 +293,7 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
     }
   };
   // Phase 1 (one unit ahead): shared node data of unit u into buffer b
-  auto phase1 = [&](long long u, int b, double& dmB) {
-    const int r = (int)(u / NCH), ch = (int)(u - (long long)r * NCH);
+  auto phase1 = [&](const int r, const int ch, const int b, double& dmB) {
     const int pair0 = ch * KP;
     const int npl = min(KP, npairs - pair0);
     const double p2sq = Q.tabR[4 * r] * Q.tabR[4 * r];
@@ -324,24 +322,28 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
   double acc = 0.0;
   CellCache cc;
   cc.Fd = inf; cc.k = make_double4(0.0, 0.0, 0.0, 0.0);   // tau = t' - inf fails the range test: the first node loads its cell
-  if (u0 < u1) phase0(u0);
+  // (r, ch) of the units u, u + 1, u + 2, advanced without divisions
+  int r = (int)(u0 / NCH), ch = (int)(u0 - (long long)r * NCH);
+  auto next_unit = [&](int& rr, int& cc_) { if (++cc_ == NCH) { cc_ = 0; ++rr; } };
+  int r1 = r, ch1 = ch;
+  next_unit(r1, ch1);
+  int r2 = r1, ch2 = ch1;
+  next_unit(r2, ch2);
+  const int nu = (int)(u1 - u0);
+  if (nu > 0) phase0(r, ch, 0);
   __syncthreads();
-  if (u0 < u1) phase1(u0, 0, dmB_cur);
-  if (u0 + 1 < u1) phase0(u0 + 1);
+  if (nu > 0) phase1(r, ch, 0, dmB_cur);
+  if (nu > 1) phase0(r1, ch1, 1);
   __syncthreads();
-  for (long long u = u0; u < u1; ++u) {
-    const int b = (int)((u - u0) & 1);
-    const int r = (int)(u / NCH), ch = (int)(u - (long long)r * NCH);
-    const bool last_of_r = (u + 1 == u1) || ((u + 1) / NCH != r);
+  for (int iu = 0; iu < nu; ++iu) {
+    const int b = iu & 1;
+    const bool last_of_r = (iu + 1 == nu) || (r1 != r);
     const int pair0 = ch * KP;
     const int npl = min(KP, npairs - pair0);
-    // the first row's coefficients: in flight while phase 1 runs
-    double2 c01_first, c23_first, c45_first;
-    if (active && w < npl) {
-      const double2* ta = reinterpret_cast<const double2*>(Q.tabA) + ((size_t)(pair0 + w) * G + a) * 4;
-      c01_first = ta[0]; c23_first = ta[1]; c45_first = ta[2];
-    }
-    if (u + 1 < u1) phase1(u + 1, b ^ 1, last_of_r ? dmB_nxt : dmB_cur);
+    // the first row's coefficients: on their way into L1 while phase 1 runs
+    if (active && w < npl)
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(Q.tabA + ((size_t)(pair0 + w) * G + a) * 8));
+    if (iu + 1 < nu) phase1(r1, ch1, b ^ 1, last_of_r ? dmB_nxt : dmB_cur);
     // ---- phase 2 ----
     {
       const double p2 = Q.tabR[4 * r], ca_ = Q.tabR[4 * r + 1];
@@ -353,7 +355,7 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
       const double* nS = sm.nodeS + b * NODES;
       const double2* ta = reinterpret_cast<const double2*>(Q.tabA) + ((size_t)(pair0 + w) * G + a) * 4;
       const size_t ta_step = (size_t)nw * G * 4;
-      double2 c01 = c01_first, c23 = c23_first, c45 = c45_first;
+      double2 c01 = ta[0], c23 = ta[1], c45 = ta[2];
       for (int pl = w; pl < npl; pl += nw) {
         if (active) {
           const double cur[6] = {c01.x, c01.y, c23.x, c23.y, c45.x, c45.y};
@@ -384,7 +386,7 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
         }
       }
     }
-    if (u + 2 < u1) phase0(u + 2);
+    if (iu + 2 < nu) phase0(r2, ch2, b);
     if (last_of_r) {
       // partial sums of this CTA for r: slot = rank of this CTA among the owners of r's units
       const long long ufirst = (long long)r * NCH;
@@ -403,6 +405,8 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
       dmB_nxt = inf;
     }
     __syncthreads();  // unit u is drained: its buffer may be refilled; the stage of unit u+1 is complete
+    r = r1; ch = ch1; r1 = r2; ch1 = ch2;
+    next_unit(r2, ch2);
   }
 }
 
@@ -439,9 +443,7 @@ int t3g_launch(ThreePointParams& P, int G, int regk, const Tab3DParams* T3, cons
   if (smem_pre > kMaxDynSmem) return DFRG_OK;   // (large 3-D tables: the general kernel)
   // node buffer of the main kernel: the largest of 2048 / 1024 / 512 nodes that fits (fewer, longer work units)
   const int npairs = P.nq * P.n1;
-  int NTX = T3G_MAXT;
-  if (const char* ev = getenv("DFRG_T3G_NT")) NTX = atoi(ev);   // EXPERIMENT
-  const int nw = NTX / G;   // pair slots of the main kernel
+  const int nw = T3G_MAXT / G;   // pair slots of the main kernel
   auto pairs_per_unit = [&](int nodes_) {
     int kp = nodes_ / P.n2 < npairs ? nodes_ / P.n2 : npairs;
     if (kp > nw) kp -= kp % nw;   // whole rounds of the pair slots
@@ -449,11 +451,11 @@ int t3g_launch(ThreePointParams& P, int G, int regk, const Tab3DParams* T3, cons
   };
   int nodes = 2048;
   while (nodes > T3G_NODES && (nodes / 2 >= P.n2) &&
-         t3m_smem(P.nq, P.n1, P.n2, P.grid.n, nodes, pairs_per_unit(nodes), NTX, T3 ? ntab3 : 0) > 176 * 1024)
+         t3m_smem(P.nq, P.n1, P.n2, P.grid.n, nodes, pairs_per_unit(nodes), T3G_MAXT, T3 ? ntab3 : 0) > 176 * 1024)
     nodes /= 2;
   if (nodes < P.n2) nodes = T3G_NODES;
   const int kp = pairs_per_unit(nodes);
-  const size_t smem_main = t3m_smem(P.nq, P.n1, P.n2, P.grid.n, nodes, kp, NTX, T3 ? ntab3 : 0);
+  const size_t smem_main = t3m_smem(P.nq, P.n1, P.n2, P.grid.n, nodes, kp, T3G_MAXT, T3 ? ntab3 : 0);
   if (smem_main > kMaxDynSmem) return DFRG_OK;
   ThreeGridParams Q;
   Q.B = P;
@@ -497,15 +499,12 @@ int t3g_launch(ThreePointParams& P, int G, int regk, const Tab3DParams* T3, cons
   }
   DFRG_T3G_PICK(0) DFRG_T3G_PICK(1) DFRG_T3G_PICK(2)
 #undef DFRG_T3G_PICK
-  if (NTX == 768 && regk == 1 && !T3 && n2_16) kmain = t3g_main_kernel<1, 768, 16, false>;
-  if (NTX == 256 && regk == 1 && !T3 && n2_16) kmain = t3g_main_kernel<1, 256, 16, false>;
-  if (NTX == 384 && regk == 1 && !T3 && n2_16) kmain = t3g_main_kernel<1, 384, 16, false>;
   int rca = e == cudaSuccess ? DFRG_OK : check_cuda(e);
   if (rca == DFRG_OK) rca = opt_in_max_smem(kpre);
   if (rca == DFRG_OK) rca = opt_in_max_smem(kmain);
   if (rca != DFRG_OK) { scratch_free(scratch, stream); *scratch_out = nullptr; return rca; }
   kpre<<<sm_count, T3G_THREADS, smem_pre, stream>>>(Q);
-  kmain<<<Q.grid_main, NTX, smem_main, stream>>>(Q);
+  kmain<<<Q.grid_main, T3G_MAXT, smem_main, stream>>>(Q);
   t3g_fixup_kernel<<<(n_ext + 255) / 256, 256, 0, stream>>>(Q);
   rc = check_cuda(cudaGetLastError());
   if (rc != DFRG_OK) { scratch_free(scratch, stream); *scratch_out = nullptr; return rc; }

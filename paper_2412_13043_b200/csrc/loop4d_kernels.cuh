@@ -121,7 +121,7 @@ struct ThreeGridParams {
   int grid_main, max_slots;
   LogGrid2Consts lgc;   // series coefficients of lg2_coord (constant-bank operands of the hot loop)
   double m2k23;    // -2 k^2 / 3
-  double* tabA;    // [npairs][8][G]: s_a/3 (TAB3D: s_a), the five quartic coefficients times w0, (unused), D_a
+  double* tabA;    // [npairs][G][8]: s_a/3 (TAB3D: s_a), the five quartic coefficients times w0, (unused), D_a
   double* tabR;    // [S][4]
   double* qmin;    // [1]   min over radial nodes of D(q^2)
   int* flag;       // [1]   != 0: the layout promise does not hold
