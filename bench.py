@@ -1,13 +1,18 @@
 #!/usr/bin/env python
 """bench.py -- measures the loop-integral hot path on B200 (contract: see DESIGN.md "Measurement").
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-others]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-others] [--no-cpu-baseline]
+                    [--full] [--report FILE]
 
 A step is one pass of the whole hot path (S1..S6) over one batch: BASELINE.json configs[4], the
 finite-T momentum-dependent loop (64 p x 16 Matsubara indices x 512 field points = 524 288 integrals,
 52 992 quadrature nodes each), the largest single-GPU configuration.  `value` = nominal integrand
 evaluations per second with inputs resident in HBM; `e2e` = the same through the host-buffer C-ABI
 call (node generation + H2D + kernel + D2H in the timed region).  One JSON line on stdout.
+
+--full compares ALL outputs of the workload with the CPU oracle (about 2.5 minutes of host time on 16 cores) instead
+of the bounded sample of the default cpu_baseline leg; --report FILE also writes that comparison as JSON to FILE.
+The process exits 1 (after printing the line) if the comparison breaks a bar of DESIGN.md "Parity bar".
 """
 import argparse
 import json
@@ -22,7 +27,6 @@ import numpy as np
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
-sys.path.insert(0, os.path.join(ROOT, "tests"))
 
 METRIC = "fp64_integrand_evals_per_s"
 UNIT = "evals/s"
@@ -30,8 +34,24 @@ WORKLOAD = "cfg4_matsubara3d: 64 p x 16 j x 512 field points, 23 Matsubara terms
 
 # FP64 roofline denominator: 148 SMs x 64 FP64 lanes x 2 flop/DFMA x 1.965 GHz
 FP64_LANES_PER_SM = 64
-# dram__bytes_read.sum + dram__bytes_write.sum of the moment kernel per launch on this workload (profiles/r1k_bench_kernel_final.md)
-NCU_DRAM_BYTES_PER_LAUNCH = 31980288 + 2048
+# the committed `ncu --set full` capture of the bench kernel on this workload: roofline.traffic is read from it
+NCU_CAPTURE = os.path.join("profiles", "r2_bench_kernel.md")
+
+
+def ncu_dram_bytes_per_launch():
+    """dram__bytes_read.sum + dram__bytes_write.sum of the moment kernel, per launch, from the committed ncu summary
+    (a run under ncu is never a bench run, so the number cannot be measured here); None if the file is missing."""
+    unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    try:
+        tot, seen = 0.0, set()
+        for ln in open(os.path.join(ROOT, NCU_CAPTURE)):
+            f = [t.strip() for t in ln.strip().strip("|").split("|")]
+            if len(f) == 3 and f[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum") and f[0] not in seen:
+                seen.add(f[0])
+                tot += float(f[1]) * unit[f[2]]
+        return int(round(tot)) if len(seen) == 2 else None
+    except (OSError, KeyError, ValueError):
+        return None
 
 
 def cfg4_counts(c, rules):
@@ -97,10 +117,10 @@ def run_reference(args):
     if rank != 0:
         return 0
     import oracle
-    from helpers import make_rules, oracle_run
+    from oracle.harness import oracle_run
     from paper_2412_13043_b200 import inputs
     c = inputs.config4()
-    R = make_rules(c, oracle.gl_rule)
+    R = inputs.make_rules(c, oracle.gl_rule)
     n_out, evals, _ = cfg4_counts(c, R)
     stride = 512
     sel = np.arange(0, n_out, stride)                       # 1024 outputs per step
@@ -125,7 +145,17 @@ def run_reference(args):
     return 0
 
 
-def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
+def alu_roofline(alg_instr, alg_flops_strict, ms, peak, what):
+    """roofline block of an FP64-pipe-bound kernel: algorithmic FP64 instructions x 2 = DFMA-slot
+    equivalents (a DADD/DMUL holds the pipe as long as a DFMA) against the nominal FP64 peak; strict = FMA 2, add/mul 1."""
+    ach = 2.0 * alg_instr / (ms * 1e-3) * 1e-12
+    strict = alg_flops_strict / (ms * 1e-3) * 1e-12
+    return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+            "achieved_strict": strict, "frac_strict": strict / peak, "alg_fp64_instr_per_launch": alg_instr,
+            "achieved_kind": what}
+
+
+def time_other_configs(torch, B, inputs, make_rules, peak, iters=5):
     """Device-resident timings of configs 0-3 (context for the flagship loop4d kernels; not the bench line)."""
     out = {}
 
@@ -187,9 +217,13 @@ def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
                                                 rq, rc, None, None, (Z,), c["lnq_lo"], c["lnq_hi"], c["interp"], coef,
                                                 m2, pext, o2), reps=20)
     ev = o2.numel() * rq[0].numel() * rc[0].numel()
-    fl = o2.numel() * rq[0].numel() * (9 * rc[0].numel() + 11)
-    out["cfg2"] = {"ms": ms, "evals_per_s": ev / ms * 1e3, "integrals_per_s": o2.numel() / ms * 1e3,
-                   "alg_tflops": fl / ms * 1e-9, "launches": 1}
+    # per (p, q, field point) one pair inversion per two cos nodes (4.5 instr per node: DADD, 3 DFMA
+    # Newton, 1/2 DMUL + ... ) and 5.5 per radial node; strict flops: 8 per node + 10 per radial node
+    n_pqf = o2.numel() * rq[0].numel()
+    out["cfg2"] = {"ms": ms, "evals_per_s": ev / ms * 1e3, "integrals_per_s": o2.numel() / ms * 1e3, "launches": 1,
+                   "roofline": alu_roofline(n_pqf * (4.5 * rc[0].numel() + 5.5), n_pqf * (8.0 * rc[0].numel() + 10.0), ms,
+                                            peak, "tp_main_kernel: 4.5 FP64 instr per (p, q, c, field point) + 5.5 per "
+                                                  "(p, q, field point)")}
     # cfg3
     c = inputs.config3()
     R = make_rules(c, B.dfrg_quad_nodes)
@@ -202,10 +236,20 @@ def time_other_configs(torch, B, inputs, make_rules, gpu_inputs_fn, iters=5):
                                                 c["lnq_hi"], c["interp"], coef, None, ext, o3,
                                                 ext_outer=c["ext_outer"]), n=3)
     uniq = o3.numel() * rr["q"][0].numel() * rr["c1"][0].numel() * rr["c2"][0].numel()
+    # 17 FP64 instr per unique node (a, r, q, c1, c2); 45 per shared node (r, q, c1, c2) of phase 1
+    # (G_A(s_b) and its vertex); 85 per (|p1|, q, c1) of the pre-pass; 2 per row.  strict: 15 of the 17 are FMAs.
+    G = c["ext_outer"]
+    S = o3.numel() // G
+    npairs, n2 = rr["q"][0].numel() * rr["c1"][0].numel(), rr["c2"][0].numel()
+    alg3 = uniq * 17.0 + S * npairs * n2 * 45.0 + G * npairs * 85.0 + o3.numel() * npairs * 2.0
+    alg3s = uniq * 32.0 + S * npairs * n2 * 80.0 + G * npairs * 160.0 + o3.numel() * npairs * 2.0
     out["cfg3"] = {"ms": ms, "unique_evals_per_s": uniq / ms * 1e3,
                    "nominal_evals_per_s": uniq * rr["phi"][0].numel() / ms * 1e3,
                    "integrals_per_s": o3.numel() / ms * 1e3,
-                   "launches": 4}   # product-grid path: pre-pass, main, fix-up, and the general kernel returning at once
+                   "launches": 4,   # product-grid path: pre-pass, main, fix-up, and the general kernel returning at once
+                   "roofline": alu_roofline(alg3, alg3s, ms, peak, "t3g_main_kernel (+ pre-pass and fix-up, timed "
+                                            "together): 17 FP64 instr per unique node, 45 per shared node, 85 per "
+                                            "pre-pass entry")}
     # cfg5 (four-point box, genuine three-angle kinematics + ghost loop; SURVEY 8(f) item 3 -- not a BASELINE config)
     c = inputs.config5()
     R = make_rules(c, B.dfrg_quad_nodes)
@@ -267,15 +311,17 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-others", action="store_true", help="skip the context timings of configs 0-3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--full", action="store_true", help="compare every output of the workload with the CPU oracle")
+    ap.add_argument("--report", default=None, help="write the oracle comparison as JSON to this file")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
 
     import torch
-    from helpers import make_rules, oracle_run
     from paper_2412_13043_b200 import binding as B
     from paper_2412_13043_b200 import inputs
+    from paper_2412_13043_b200.inputs import make_rules
     from paper_2412_13043_b200.shard import shard_bounds
 
     rank = int(os.environ.get("RANK", "0"))
@@ -407,12 +453,15 @@ def main():
             "e2e": {"value": world * evals / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_s * 1e3, "s1_host_ms": t_s1 * 1e3},
             "roofline": {"bound": "alu", "kernel": "mats3d_moment_kernel (+ the two pre-pass kernels and the fix-up kernel, timed together)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                         "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH if world == 1 else None,
-                         "traffic_kind": "dram__bytes_read.sum + dram__bytes_write.sum of mats3d_moment_kernel, one ncu --set full "
-                                         "capture of this workload (profiles/r1k_bench_kernel_final.md); algorithmic bytes: "
-                                         "31.85 MB of D0phi chunks read once",
+                         "frac": achieved / peak, "traffic": ncu_dram_bytes_per_launch() if world == 1 else None,
+                         "traffic_kind": "dram__bytes_read.sum + dram__bytes_write.sum of mats3d_moment_kernel per launch, read "
+                                         "at run time from the committed ncu --set full capture of this workload (" +
+                                         NCU_CAPTURE + "); algorithmic bytes: the D0phi chunks [p][27 rows][q][c], read once",
+                         "alg_bytes_per_launch": 8 * c["pext"].size * rows_phi * R["q"][0].size * R["c"][0].size,
                          "achieved_kind": "algorithmic FP64 instructions x 2 (DFMA-slot equivalents) / event time",
                          "achieved_strict": flops_strict / (ms_local * 1e-3) * 1e-12,
+                         "frac_strict": flops_strict / (ms_local * 1e-3) * 1e-12 / peak,
+                         "alg_fp64_instr_per_nominal_eval": flops / 2.0 / evals,
                          "peak_kind": "nominal FP64: %d SMs x %d lanes x 2 x %.0f MHz (MEASURED_PEAKS.json has no FP64 "
                                       "entry)" % (sms, FP64_LANES_PER_SM, sm_max_mhz),
                          "peak_probe_tflops": probe_tflops, "frac_of_probe": achieved / probe_tflops,
@@ -420,33 +469,53 @@ def main():
             "wall_s_timed_region": t_wall}
 
     if not args.no_others and world == 1:
-        line["other_configs"] = time_other_configs(torch, B, inputs, make_rules, None)
+        line["other_configs"] = time_other_configs(torch, B, inputs, make_rules, peak)
 
-    if not args.no_cpu_baseline and world == 1:
+    parity_ok = True
+    if (args.full or not args.no_cpu_baseline) and world == 1:
+        # the oracle as it stands, on the host cores, on the SAME nodes the GPU used (R: the library's dfrg_quad_nodes)
         import oracle
-        Ro = make_rules(c, oracle.gl_rule)
+        from oracle.harness import RTOL, SENS_EPS, oracle_run, parity_report
         per_out = evals // n_out
-        probe_sel = np.arange(0, n_out, n_out // 256)[:256]
+        if args.full:
+            sel = np.arange(n_out, dtype=np.int64)
+        else:
+            probe_sel = np.arange(0, n_out, n_out // 256)[:256]
+            t0 = time.perf_counter()
+            oracle_run(c, R, sel=probe_sel)
+            rate = probe_sel.size / (time.perf_counter() - t0)                 # outputs per second
+            n_s = int(min(n_out // 4, max(256, rate * 15.0)))               # about 15 s of host time
+            stride = n_out // n_s
+            stride += 1 - stride % 2                                         # odd: the sample visits every field-point residue
+            sel = np.arange(n_s, dtype=np.int64) * stride
         t0 = time.perf_counter()
-        oracle_run(c, Ro, sel=probe_sel)
-        rate = probe_sel.size / (time.perf_counter() - t0)                 # outputs per second
-        n_s = int(min(n_out // 4, max(256, rate * 15.0)))               # about 15 s of host time
-        sel = np.arange(n_s, dtype=np.int64) * (n_out // n_s)
-        t0 = time.perf_counter()
-        o = oracle_run(c, Ro, sel=sel)
+        o = oracle_run(c, R, sel=sel)
         dt = time.perf_counter() - t0
         got = out.cpu().numpy().ravel()[sel]
-        reg = (o["dmin"] >= 1e-6) & (o["sens"] <= 1e4 * np.abs(o["out"]))
-        line["cpu_baseline"] = {"value": n_s * per_out / dt, "unit": UNIT, "cores": oracle.num_threads(),
+        rep = parity_report(got, o["out"], o["dmin"], o["sens"])
+        rep = {k_: v for k_, v in rep.items() if not k_.startswith("_")}
+        parity_ok = (rep["n_nonfinite_gpu_only"] == 0 and rep["max_rel_regular"] <= RTOL and
+                     rep["max_sens_ratio_regular"] <= SENS_EPS and rep["max_sens_ratio_singular"] <= SENS_EPS)
+        line["cpu_baseline"] = {"value": sel.size * per_out / dt, "unit": UNIT, "cores": oracle.num_threads(),
                                 "kind": "oracle", "seconds": dt,
-                                "sample": "%d of %d outputs (every %dth), %d nodes each" % (n_s, n_out, n_out // n_s,
-                                                                                           per_out),
-                                "max_rel_err_vs_gpu_regular": float(np.max(np.abs(got[reg] / o["out"][reg] - 1))),
-                                "max_abs_err_over_sens": float(np.max(np.abs(got - o["out"]) / o["sens"]))}
+                                "sample": ("all %d outputs" % n_out) if args.full else
+                                          "%d of %d outputs (every %dth), %d nodes each" % (sel.size, n_out, stride, per_out),
+                                "nodes": "the library's (dfrg_quad_nodes), the same arrays the GPU call used",
+                                "max_rel_err_vs_gpu_regular": rep["max_rel_regular"],
+                                "max_abs_err_over_sens": max(rep["max_sens_ratio_regular"], rep["max_sens_ratio_singular"]),
+                                "n_regular": rep["n_regular"], "n_pole": rep["n_pole"], "n_cancelling": rep["n_cancelling"],
+                                "max_rel_cancelling": rep["max_rel_cancelling"],
+                                "max_abs_err_over_sens_singular": rep["max_sens_ratio_singular"],
+                                "n_nonfinite_gpu_only": rep["n_nonfinite_gpu_only"],
+                                "bars": {"rel_regular": RTOL, "abs_over_sens": SENS_EPS}, "parity_ok": parity_ok}
+        if args.report:
+            with open(args.report, "w") as fh:
+                json.dump({"workload": WORKLOAD, "compared": int(sel.size), "of": n_out, "oracle_seconds": dt, **rep,
+                           "bars": {"rel_regular": RTOL, "abs_over_sens": SENS_EPS}, "parity_ok": parity_ok}, fh, indent=1)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
-    return 0
+    return 0 if parity_ok else 1
 
 
 if __name__ == "__main__":

@@ -205,3 +205,9 @@ def config4(n_field=512, n_p=64, n_jext=16, n_q=96, n_c=24, n_tab=128, n_freq=64
                 coef=2.0 * U[4:24] - 1.0,
                 m2psi=rho.copy(), m2phi=u,
                 pext=logspace(1e-2 * k, 20.0 * k, n_p), n_jext=n_jext)
+
+
+def make_rules(c, gen):
+    """gen(n, a, b) -> (x, w), the caller's node generator (the library's dfrg_quad_nodes or the oracle's);
+    returns {axis: (x, w)} for every rule_* entry of the workload."""
+    return {key[5:]: gen(*val) for key, val in c.items() if key.startswith("rule_")}
