@@ -487,7 +487,7 @@ def main():
             n_s = int(min(n_out // 4, max(256, rate * 15.0)))               # about 15 s of host time
             stride = n_out // n_s
             stride += 1 - stride % 2                                         # odd: the sample visits every field-point residue
-            sel = np.arange(n_s, dtype=np.int64) * stride
+            sel = np.arange(0, n_out, stride, dtype=np.int64)[:n_s]
         t0 = time.perf_counter()
         o = oracle_run(c, R, sel=sel)
         dt = time.perf_counter() - t0

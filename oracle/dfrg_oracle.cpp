@@ -100,6 +100,28 @@ void regulator_shape(int kind, int order, double k, double s, double* R, double*
   *Rdot = 2.0 * r * (1.0 + geo);
 }
 
+// ---- fermionic regulator RF / RFdot ------------------------------------------------------------------
+// The paper makes four functions available in every integration kernel, RB, RF, RBdot, RFdot, and
+// its finite-temperature / finite-density examples are fermionic; it prints no fermionic
+// shape.  Reading A25: the regulator of a Dirac operator, i pslash (1 + r_F), with the standard relation
+// (1 + r_F)^2 = 1 + r_B to the bosonic shape, i.e. with R_F = |p| r_F of momentum dimension one
+//   (sqrt(s) + R_F(s))^2 = s + R_B(s)   =>   R_F = sqrt(s + R_B) - sqrt(s),   k dR_F/dk = RBdot / (2 sqrt(s + R_B))
+// (flat shape: R_F = (k - sqrt(s)) Theta(k^2 - s), the flat fermionic regulator).  Dressed as the bosonic one:
+//   RF = zk R_F,   RFdot = k d(Z_k R_F)/dk = zk (k dR_F/dk - eta R_F).
+// A fermion line regulated this way has the scalar denominator of  Z (pslash + ...) + RF-slash + i m:
+//   D = Z^2 (s - sR) + (Z sqrt(sR) + RF(sR))^2 + m^2,   insertion  k dD/dk at fixed Z, m  =  2 (Z sqrt(sR) + RF) RFdot
+// where sR is the argument of the regulator (the 4-momentum squared, or the spatial part for "3D" regulators, in which
+// case s - sR is the squared time component) and m^2 the squared fermion mass.
+void regulator_fermion(int kind, int order, double k, double zk, double eta, double s, double* RF, double* RFdot) {
+  double Rb, Rbd;
+  regulator_shape(kind, order, k, s, &Rb, &Rbd);
+  const double root = std::sqrt(s + Rb);
+  const double rf = root - std::sqrt(s);
+  const double rfd = Rbd / (2.0 * root);
+  *RF = zk * rf;
+  *RFdot = zk * (rfd - eta * rf);
+}
+
 // ---- log-grid table look-up: PAPER.md:1854-1880; stacks PAPER.md:1898-1905 -----------
 // v[0..n-1] sits on ln q_i = lo + i h, h = (hi - lo)/(n - 1).  The argument is the
 // SQUARED momentum s; l = log(s)/2; t = clamp((l - lo)/h, 0, n-1).
@@ -257,6 +279,9 @@ void orc_regulator(int kind, int order, double k, double zk, double eta, double 
   regulator(kind, order, k, zk, eta, s, R, Rdot);
 }
 
+void orc_regulator_fermion(int kind, int order, double k, double zk, double eta, double s, double* RF, double* RFdot) {
+  regulator_fermion(kind, order, k, zk, eta, s, RF, RFdot);
+}
 double orc_table_lookup(const double* v, int n_q, double lnq_lo, double lnq_hi, int interp, double s) {
   return table_lookup(v, n_q, lnq_lo, lnq_hi, interp, s);
 }
@@ -337,8 +362,11 @@ int orc_lpa(int d, double T, int n_max, int reg_arg4d, double N, double prefacto
 //  D = a + i b, a = nu^2 - mu^2 + q^2 + R + m2, b = 2 nu mu, Re 1/D = a/(a^2+b^2)).
 //   dI[j] = d I_F / d m2 = -C T sum sum w q^(d-1) Rdot Re[1/D^2],  Re 1/D^2 = (a^2 - b^2)/(a^2+b^2)^2
 //   dmin[j] = min over nodes of |D| / k^2;   sens, sens_d: sum |term| (1 + (|D - m2| + |m2|)/|D| per power of 1/D)
+// freg != 0 (reading A25): the loop is regulated with RF / RFdot on the Dirac structure (Z = 1, spatial argument):
+//   D = (nu_n + i mu)^2 + (q + RF(q^2))^2 + m2,   Rdot(q^2) -> 2 (q + RF(q^2)) RFdot(q^2);
+// with zk = 1, eta = 0 this is the same function as freg = 0 ((q + R_F)^2 = q^2 + R_B, 2 (q + R_F) k dR_F/dk = RBdot).
 int orc_lpa_fermion(int d, double T, int n_max, double mu, double prefactor,
-                    int reg_kind, int reg_order, double k, double zk, double eta,
+                    int reg_kind, int reg_order, double k, double zk, double eta, int freg,
                     int nq, const double* xq, const double* wq,
                     int n_m2, const double* m2v,
                     double* I, double* dI, double* dmin, double* sens, double* sens_d) {
@@ -354,9 +382,18 @@ int orc_lpa_fermion(int d, double T, int n_max, double mu, double prefactor,
       const double nu = (2.0 * (double)n + 1.0) * pi * T;
       for (int i = 0; i < nq; ++i) {
         const double q = xq[i];
-        double R, Rd;
-        regulator(reg_kind, reg_order, k, zk, eta, q * q, &R, &Rd);
-        const double a0 = nu * nu - mu * mu + q * q + R;      // Re(D - m2)
+        double R, Rd;      // freg: R = (q + RF)^2 - q^2 is not formed; a0 is written with the kinetic term A = q + RF
+        double a0;                                             // Re(D - m2)
+        if (freg) {
+          double RF, RFd;
+          regulator_fermion(reg_kind, reg_order, k, zk, eta, q * q, &RF, &RFd);
+          const double A = q + RF;
+          a0 = nu * nu - mu * mu + A * A;
+          Rd = 2.0 * A * RFd;
+        } else {
+          regulator(reg_kind, reg_order, k, zk, eta, q * q, &R, &Rd);
+          a0 = nu * nu - mu * mu + q * q + R;
+        }
         const double a = a0 + m2, b = 2.0 * nu * mu;
         const double den = a * a + b * b;                      // |D|^2
         const double absD = std::sqrt(den);
@@ -778,7 +815,10 @@ int orc_loop4d_fourpoint(double prefactor, int reg_kind, int reg_order, double k
 // P = sum_{a+b+c<=3} kap_abc y1^a y2^b y3^c, y1 = nu_n nu_j/k^2, y2 = p q c/k^2, y3 = s_psi/k^2
 // out[p][j][f] = C T sum_n sum_q w q^2 Rdot(s_psi) G_psi^2 sum_c w P G_phi
 // Tables are row-major [n_freq][n_q]; the momentum argument is the spatial one (q^2, r^2).
+// freg != 0 (reading A25): the fermion line carries the fermionic regulator on its Dirac structure (4-D argument):
+//   A = Z_psi sqrt(s_psi) + RF(s_psi),  G_psi = 1/(A^2 + m2_psi),  Rdot(s_psi) -> 2 A RFdot(s_psi);  boson line unchanged.
 int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg_order, double k, double zk, double eta,
+                    int freg,
                     int nq, const double* xq, const double* wq,
                     int nc, const double* xc, const double* wc,
                     const double* Zpsi, const double* Zphi, int t_nq, int t_nfreq,
@@ -812,10 +852,18 @@ int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg
       for (int i = 0; i < nq; ++i) {
         const double q = xq[i];
         const double spsi = nun * nun + q * q;
-        double Rp, Rdp;
-        regulator(reg_kind, reg_order, k, zk, eta, spsi, &Rp, &Rdp);
-        const double Dpsi =
-            table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q) * spsi + Rp + m2psi[f];
+        double Rp, Rdp, Dpsi;
+        const double Zq = table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q);
+        if (freg) {
+          double RF, RFd;
+          regulator_fermion(reg_kind, reg_order, k, zk, eta, spsi, &RF, &RFd);
+          const double A = Zq * std::sqrt(spsi) + RF;
+          Dpsi = A * A + m2psi[f];
+          Rdp = 2.0 * A * RFd;
+        } else {
+          regulator(reg_kind, reg_order, k, zk, eta, spsi, &Rp, &Rdp);
+          Dpsi = Zq * spsi + Rp + m2psi[f];
+        }
         if (Dpsi / k2 < dm) dm = Dpsi / k2;
         const double Gpsi = 1.0 / Dpsi;
         const double condpsi = 2.0 * (std::fabs(Dpsi - m2psi[f]) + std::fabs(m2psi[f])) / std::fabs(Dpsi);
@@ -867,8 +915,10 @@ int orc_matsubara3d(double T, int n_max, double prefactor, int reg_kind, int reg
 //   out[p][j][f] = C T sum_n sum_q w q^2 Rdot(q^2) G_psi^2 sum_c w P(y1, y2, y3) G_phi        (complex: out_re, out_im)
 // mu = 0 gives the real spatial-regulator variant of the family (out_im = 0 exactly).
 // dmin = min over nodes of min(|D_psi|, D_phi)/k^2;  sens as orc_matsubara3d with moduli.
+// freg != 0 (reading A25): fermion line with the fermionic regulator on the Dirac structure, spatial argument:
+//   A = Z_psi q + RF(q^2),  G_psi = 1/(Z_psi^2 (nu_n + i mu)^2 + A^2 + m2_psi),  Rdot(q^2) -> 2 A RFdot(q^2).
 int orc_matsubara3d_mu(double T, int n_max, double mu, double prefactor, int reg_kind, int reg_order, double k,
-                       double zk, double eta,
+                       double zk, double eta, int freg,
                        int nq, const double* xq, const double* wq,
                        int nc, const double* xc, const double* wc,
                        const double* Zpsi, const double* Zphi, int t_nq, int t_nfreq,
@@ -906,8 +956,18 @@ int orc_matsubara3d_mu(double T, int n_max, double mu, double prefactor, int reg
         const double q = xq[i];
         const cd spsi = p0n * p0n + q * q;
         double Rp, Rdp;
-        regulator(reg_kind, reg_order, k, zk, eta, q * q, &Rp, &Rdp);
-        const cd Dpsi = table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q) * spsi + Rp + m2psi[f];
+        cd Dpsi;
+        const double Zq = table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q);
+        if (freg) {
+          double RF, RFd;
+          regulator_fermion(reg_kind, reg_order, k, zk, eta, q * q, &RF, &RFd);
+          const double A = Zq * q + RF;
+          Dpsi = (Zq * Zq) * (p0n * p0n) + A * A + m2psi[f];
+          Rdp = 2.0 * A * RFd;
+        } else {
+          regulator(reg_kind, reg_order, k, zk, eta, q * q, &Rp, &Rdp);
+          Dpsi = Zq * spsi + Rp + m2psi[f];
+        }
         if (std::abs(Dpsi) / k2 < dm) dm = std::abs(Dpsi) / k2;
         const cd Gpsi = 1.0 / Dpsi;
         const double condpsi = 2.0 * (std::abs(Dpsi - m2psi[f]) + std::fabs(m2psi[f])) / std::abs(Dpsi);
@@ -959,8 +1019,10 @@ int orc_matsubara3d_mu(double T, int n_max, double mu, double prefactor, int reg
 //   dpsi = d out / d m2_psi = C T sum_n sum_q w q^2 Rdot(q^2) (-2 G_psi^3) sum_c w P G_phi
 //   dphi = d out / d m2_phi = C T sum_n sum_q w q^2 Rdot(q^2) G_psi^2 sum_c w P (-G_phi^2)
 // (complex for mu != 0: *_re, *_im).  sens_* as orc_matsubara3d_dm2 with moduli.
+// freg != 0 (reading A25): fermion line with the fermionic regulator on the Dirac structure, spatial argument:
+//   A = Z_psi q + RF(q^2),  G_psi = 1/(Z_psi^2 (nu_n + i mu)^2 + A^2 + m2_psi),  Rdot(q^2) -> 2 A RFdot(q^2).
 int orc_matsubara3d_mu_dm2(double T, int n_max, double mu, double prefactor, int reg_kind, int reg_order, double k,
-                           double zk, double eta,
+                           double zk, double eta, int freg,
                            int nq, const double* xq, const double* wq,
                            int nc, const double* xc, const double* wc,
                            const double* Zpsi, const double* Zphi, int t_nq, int t_nfreq,
@@ -998,8 +1060,18 @@ int orc_matsubara3d_mu_dm2(double T, int n_max, double mu, double prefactor, int
         const double q = xq[i];
         const cd spsi = p0n * p0n + q * q;
         double Rp, Rdp;
-        regulator(reg_kind, reg_order, k, zk, eta, q * q, &Rp, &Rdp);
-        const cd Dpsi = table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q) * spsi + Rp + m2psi[f];
+        cd Dpsi;
+        const double Zq = table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q);
+        if (freg) {
+          double RF, RFd;
+          regulator_fermion(reg_kind, reg_order, k, zk, eta, q * q, &RF, &RFd);
+          const double A = Zq * q + RF;
+          Dpsi = (Zq * Zq) * (p0n * p0n) + A * A + m2psi[f];
+          Rdp = 2.0 * A * RFd;
+        } else {
+          regulator(reg_kind, reg_order, k, zk, eta, q * q, &Rp, &Rdp);
+          Dpsi = Zq * spsi + Rp + m2psi[f];
+        }
         const cd Gpsi = 1.0 / Dpsi;
         const double condpsi = (std::abs(Dpsi - m2psi[f]) + std::fabs(m2psi[f])) / std::abs(Dpsi);
         cld c_psi(0.0L, 0.0L), c_phi(0.0L, 0.0L);
@@ -1152,7 +1224,9 @@ int orc_loop4d_twopoint_dm2(double prefactor, int reg_kind, int reg_order, doubl
 
 // dpsi[p][j][f] = d out / d m2_psi_f = C T sum_n sum_q w q^2 Rdot (-2 G_psi^3) sum_c w P G_phi
 // dphi[p][j][f] = d out / d m2_phi_f = C T sum_n sum_q w q^2 Rdot G_psi^2 sum_c w P (-G_phi^2)
+// freg: as orc_matsubara3d.
 int orc_matsubara3d_dm2(double T, int n_max, double prefactor, int reg_kind, int reg_order, double k, double zk, double eta,
+                        int freg,
                         int nq, const double* xq, const double* wq,
                         int nc, const double* xc, const double* wc,
                         const double* Zpsi, const double* Zphi, int t_nq, int t_nfreq,
@@ -1185,10 +1259,18 @@ int orc_matsubara3d_dm2(double T, int n_max, double prefactor, int reg_kind, int
       for (int i = 0; i < nq; ++i) {
         const double q = xq[i];
         const double spsi = nun * nun + q * q;
-        double Rp, Rdp;
-        regulator(reg_kind, reg_order, k, zk, eta, spsi, &Rp, &Rdp);
-        const double Dpsi =
-            table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q) * spsi + Rp + m2psi[f];
+        double Rp, Rdp, Dpsi;
+        const double Zq = table_lookup(Zpsi + (size_t)nbar * t_nq, t_nq, t_lo, t_hi, t_interp, q * q);
+        if (freg) {
+          double RF, RFd;
+          regulator_fermion(reg_kind, reg_order, k, zk, eta, spsi, &RF, &RFd);
+          const double A = Zq * std::sqrt(spsi) + RF;
+          Dpsi = A * A + m2psi[f];
+          Rdp = 2.0 * A * RFd;
+        } else {
+          regulator(reg_kind, reg_order, k, zk, eta, spsi, &Rp, &Rdp);
+          Dpsi = Zq * spsi + Rp + m2psi[f];
+        }
         const double Gpsi = 1.0 / Dpsi;
         const double condpsi = (std::fabs(Dpsi - m2psi[f]) + std::fabs(m2psi[f])) / std::fabs(Dpsi);
         acc_t c_psi = 0.0L, c_phi = 0.0L, sc_psi = 0.0L, sc_phi = 0.0L;
