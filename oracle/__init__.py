@@ -9,6 +9,7 @@ from .binding import (  # noqa: F401
     build,
     gl_rule,
     regulator,
+    regulator_fermion,
     table_lookup,
     lpa,
     lpa_fermion,

@@ -44,6 +44,7 @@ def _load():
         _lib.orc_table_lookup.argtypes = [_dp, C.c_int, C.c_double, C.c_double, C.c_int, C.c_double]
         _lib.orc_regulator.restype = None
         _lib.orc_regulator.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, _dp, _dp]
+        _lib.orc_regulator_fermion.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, _dp, _dp]
         _lib.orc_gl_rule.argtypes = [C.c_int, C.c_double, C.c_double, _dp, _dp]
         _lib.orc_lpa.argtypes = [C.c_int, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
                                  C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
@@ -60,7 +61,7 @@ def _load():
                                                _dp, C.c_int, C.c_int, _dp,
                                                C.c_longlong, _lp, C.c_int, _dp, _dp, _dp]
         _lib.orc_lpa_fermion.argtypes = [C.c_int, C.c_double, C.c_int, C.c_double, C.c_double,
-                                         C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                         C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int,
                                          C.c_int, _dp, _dp, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp]
         _ip = C.POINTER(C.c_int)
         _lib.orc_table3d_lookup.restype = C.c_double
@@ -80,19 +81,19 @@ def _load():
                                               _dp, _dp, _dp, C.c_int, C.c_double, C.c_double, C.c_int,
                                               _dp, C.c_int, C.c_int, _dp,
                                               C.c_longlong, _lp, _dp, _dp, _dp]
-        _lib.orc_matsubara3d.argtypes = [C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+        _lib.orc_matsubara3d.argtypes = [C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int,
                                          C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                          _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
                                          _dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int,
                                          C.c_longlong, _lp, _dp, _dp, _dp]
         _lib.orc_matsubara3d_mu.argtypes = [C.c_double, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double,
-                                            C.c_double, C.c_double,
+                                            C.c_double, C.c_double, C.c_int,
                                             C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                             _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
                                             _dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int,
                                             C.c_longlong, _lp, _dp, _dp, _dp, _dp]
         _lib.orc_matsubara3d_mu_dm2.argtypes = [C.c_double, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double,
-                                                C.c_double, C.c_double,
+                                                C.c_double, C.c_double, C.c_int,
                                                 C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                                 _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
                                                 _dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int,
@@ -105,7 +106,7 @@ def _load():
                                                  _dp, C.c_int, C.c_double, C.c_double, C.c_int,
                                                  _dp, C.c_int, C.c_int, _dp, C.c_int, _dp,
                                                  C.c_longlong, _lp, _dp, _dp]
-        _lib.orc_matsubara3d_dm2.argtypes = [C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+        _lib.orc_matsubara3d_dm2.argtypes = [C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int,
                                              C.c_int, _dp, _dp, C.c_int, _dp, _dp,
                                              _dp, _dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
                                              _dp, C.c_int, C.c_int, _dp, _dp, C.c_int, _dp, C.c_int,
@@ -137,6 +138,14 @@ def regulator(kind, order, k, s, zk=1.0, eta=0.0):
     return R.value, Rd.value
 
 
+def regulator_fermion(kind, order, k, s, zk=1.0, eta=0.0):
+    """(RF, RFdot) of reading A25 at the squared momentum s."""
+    R = C.c_double()
+    Rd = C.c_double()
+    _load().orc_regulator_fermion(int(kind), int(order), float(k), float(zk), float(eta), float(s), C.byref(R), C.byref(Rd))
+    return R.value, Rd.value
+
+
 def table_lookup(v, lnq_lo, lnq_hi, interp, s):
     v = _arr(v)
     return float(_load().orc_table_lookup(_d(v), int(v.size), float(lnq_lo), float(lnq_hi), int(interp), float(s)))
@@ -165,12 +174,12 @@ def lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, xq, wq, rh
     return (flow, chan, dmin, sens) if want_sens else (flow, chan, dmin)
 
 
-def lpa_fermion(d, T, n_max, mu, prefactor, reg_kind, reg_order, k, xq, wq, m2, zk=1.0, eta=0.0):
+def lpa_fermion(d, T, n_max, mu, prefactor, reg_kind, reg_order, k, xq, wq, m2, zk=1.0, eta=0.0, freg=0):
     """Fermionic LPA loop at chemical potential mu (spatial regulator).  Returns (I, dI, dmin, sens, sens_d), each [m2.size]."""
     xq, wq, m2 = map(_arr, (xq, wq, m2))
     I, dI, dmin, sens, sens_d = (np.empty(m2.shape) for _ in range(5))
     rc = _load().orc_lpa_fermion(int(d), float(T), int(n_max), float(mu), float(prefactor),
-                                 int(reg_kind), int(reg_order), float(k), float(zk), float(eta),
+                                 int(reg_kind), int(reg_order), float(k), float(zk), float(eta), int(freg),
                                  int(xq.size), _d(xq), _d(wq), int(m2.size), _d(m2),
                                  _d(I), _d(dI), _d(dmin), _d(sens), _d(sens_d))
     if rc:
@@ -286,7 +295,7 @@ def loop4d_fourpoint(prefactor, reg_kind, reg_order, k, xq, wq, x1, w1, x2, w2, 
 
 
 def matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zpsi, Zphi,
-                lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, want_sens=False, zk=1.0, eta=0.0):
+                lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, want_sens=False, zk=1.0, eta=0.0, freg=0):
     """Zpsi, Zphi: [n_freq, n_q].  Returns (out, dmin): [n_p, n_jext, n_field] or [n_sel]
     for flat indices (e*n_jext + j)*n_field + f in sel."""
     xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext = map(
@@ -298,7 +307,7 @@ def matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zps
     out = np.empty(shape)
     dmin = np.empty(shape)
     sens = np.empty(shape)
-    rc = _load().orc_matsubara3d(float(T), int(n_max), float(prefactor), int(reg_kind), int(reg_order), float(k), float(zk), float(eta),
+    rc = _load().orc_matsubara3d(float(T), int(n_max), float(prefactor), int(reg_kind), int(reg_order), float(k), float(zk), float(eta), int(freg),
                                  int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
                                  _d(Zpsi), _d(Zphi), int(tnq), int(nfreq), float(lnq_lo), float(lnq_hi), int(interp),
                                  _d(coef), int(coef.size), int(m2psi.size), _d(m2psi), _d(m2phi),
@@ -309,7 +318,7 @@ def matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zps
 
 
 def matsubara3d_mu(T, n_max, mu, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zpsi, Zphi,
-                   lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, want_sens=False, zk=1.0, eta=0.0):
+                   lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, want_sens=False, zk=1.0, eta=0.0, freg=0):
     """Matsubara family at chemical potential mu with spatial regulators.  Returns (out complex128, dmin[, sens])."""
     xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext = map(
         _arr, (xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext))
@@ -318,7 +327,7 @@ def matsubara3d_mu(T, n_max, mu, prefactor, reg_kind, reg_order, k, xq, wq, xc, 
     shape = (ns,) if sel is not None else (pext.size, int(n_jext), m2psi.size)
     o_re, o_im, dmin, sens = (np.empty(shape) for _ in range(4))
     rc = _load().orc_matsubara3d_mu(float(T), int(n_max), float(mu), float(prefactor), int(reg_kind), int(reg_order),
-                                    float(k), float(zk), float(eta),
+                                    float(k), float(zk), float(eta), int(freg),
                                     int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
                                     _d(Zpsi), _d(Zphi), int(tnq), int(nfreq), float(lnq_lo), float(lnq_hi), int(interp),
                                     _d(coef), int(coef.size), int(m2psi.size), _d(m2psi), _d(m2phi),
@@ -331,7 +340,7 @@ def matsubara3d_mu(T, n_max, mu, prefactor, reg_kind, reg_order, k, xq, wq, xc, 
 
 
 def matsubara3d_mu_dm2(T, n_max, mu, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zpsi, Zphi,
-                       lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, zk=1.0, eta=0.0):
+                       lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, zk=1.0, eta=0.0, freg=0):
     """Mass derivatives of matsubara3d_mu.  Returns (dpsi, dphi, sens_psi, sens_phi), dpsi / dphi complex128."""
     xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext = map(
         _arr, (xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext))
@@ -340,7 +349,7 @@ def matsubara3d_mu_dm2(T, n_max, mu, prefactor, reg_kind, reg_order, k, xq, wq, 
     shape = (ns,) if sel is not None else (pext.size, int(n_jext), m2psi.size)
     a_re, a_im, b_re, b_im, sa, sb = (np.empty(shape) for _ in range(6))
     rc = _load().orc_matsubara3d_mu_dm2(float(T), int(n_max), float(mu), float(prefactor), int(reg_kind),
-                                        int(reg_order), float(k), float(zk), float(eta),
+                                        int(reg_order), float(k), float(zk), float(eta), int(freg),
                                         int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
                                         _d(Zpsi), _d(Zphi), int(tnq), int(nfreq), float(lnq_lo), float(lnq_hi),
                                         int(interp), _d(coef), int(coef.size), int(m2psi.size), _d(m2psi), _d(m2phi),
@@ -385,7 +394,7 @@ def loop4d_twopoint_dm2(prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Z, ln
 
 
 def matsubara3d_dm2(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc, Zpsi, Zphi,
-                    lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, zk=1.0, eta=0.0):
+                    lnq_lo, lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, sel=None, zk=1.0, eta=0.0, freg=0):
     """Returns (dpsi, dphi, sens_psi, sens_phi): d out / d m2_psi[f] and d out / d m2_phi[f]."""
     xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext = map(
         _arr, (xq, wq, xc, wc, Zpsi, Zphi, coef, m2psi, m2phi, pext))
@@ -393,7 +402,7 @@ def matsubara3d_dm2(T, n_max, prefactor, reg_kind, reg_order, k, xq, wq, xc, wc,
     ns, selp, _keep = _sel(sel)
     shape = (ns,) if sel is not None else (pext.size, int(n_jext), m2psi.size)
     dpsi, dphi, spsi, sphi = (np.empty(shape) for _ in range(4))
-    rc = _load().orc_matsubara3d_dm2(float(T), int(n_max), float(prefactor), int(reg_kind), int(reg_order), float(k), float(zk), float(eta),
+    rc = _load().orc_matsubara3d_dm2(float(T), int(n_max), float(prefactor), int(reg_kind), int(reg_order), float(k), float(zk), float(eta), int(freg),
                                      int(xq.size), _d(xq), _d(wq), int(xc.size), _d(xc), _d(wc),
                                      _d(Zpsi), _d(Zphi), int(tnq), int(nfreq), float(lnq_lo), float(lnq_hi),
                                      int(interp), _d(coef), int(coef.size), int(m2psi.size), _d(m2psi), _d(m2phi),

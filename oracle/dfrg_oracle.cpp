@@ -116,7 +116,7 @@ void regulator_fermion(int kind, int order, double k, double zk, double eta, dou
   double Rb, Rbd;
   regulator_shape(kind, order, k, s, &Rb, &Rbd);
   const double root = std::sqrt(s + Rb);
-  const double rf = root - std::sqrt(s);
+  const double rf = Rb / (root + std::sqrt(s));   // = root - sqrt(s), written without the cancellation at s >> R_B
   const double rfd = Rbd / (2.0 * root);
   *RF = zk * rf;
   *RFdot = zk * (rfd - eta * rf);

@@ -22,13 +22,18 @@ def _dress(c):
     return dict(zk=c.get("reg_zk", 1.0), eta=c.get("reg_eta", 0.0))
 
 
+def _fdress(c):
+    """... plus the fermionic-regulator switch of the families with a fermion line (reading A25)."""
+    return dict(freg=c.get("fermion_reg", 0), **_dress(c))
+
+
 def oracle_run(c, R, sel=None):
     """-> (out, dmin, sens); lpa: out = flow[n_field], extra channels under key 'chan' are returned via dict."""
     kd = kind_of(c)
     if kd == "lpa" and c.get("statistics", 0) == 1:     # fermionic loop at chemical potential (reading A22)
         m2 = np.stack([c["u"], c["u"] + 2.0 * c["rho"] * c["du"]])
         I, dI, dm, sn, snd = oracle.lpa_fermion(c["d"], c["T"], c["n_max"], c.get("mu", 0.0), c["prefactor"], c["reg_kind"],
-                                                c["reg_order"], c["k"], *R["q"], m2.ravel(), **_dress(c))
+                                                c["reg_order"], c["k"], *R["q"], m2.ravel(), **_fdress(c))
         I, dm, sn = (a.reshape(2, -1) for a in (I, dm, sn))
         return dict(out=(c["N"] - 1.0) * I[0] + I[1], chan=I, dmin=np.minimum(dm[0], dm[1]),
                     sens=abs(c["N"] - 1.0) * sn[0] + sn[1], sens_chan=sn)
@@ -36,7 +41,7 @@ def oracle_run(c, R, sel=None):
         out, dmin, sens = oracle.matsubara3d_mu(c["T"], c["n_max"], c.get("mu", 0.0), c["prefactor"], c["reg_kind"],
                                                 c["reg_order"], c["k"], *R["q"], *R["c"], c["Zpsi"], c["Zphi"],
                                                 c["lnq_lo"], c["lnq_hi"], c["interp"], c["coef"], c["m2psi"], c["m2phi"],
-                                                c["pext"], c["n_jext"], sel=sel, want_sens=True, **_dress(c))
+                                                c["pext"], c["n_jext"], sel=sel, want_sens=True, **_fdress(c))
         return dict(out=out, dmin=dmin, sens=sens)
     if kd == "lpa":
         flow, chan, dmin, sens = oracle.lpa(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["N"], c["prefactor"],
@@ -66,7 +71,7 @@ def oracle_run(c, R, sel=None):
         out, dmin, sens = oracle.matsubara3d(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
                                              *R["q"], *R["c"], c["Zpsi"], c["Zphi"], c["lnq_lo"], c["lnq_hi"],
                                              c["interp"], c["coef"], c["m2psi"], c["m2phi"], c["pext"], c["n_jext"],
-                                             sel=sel, want_sens=True, **_dress(c))
+                                             sel=sel, want_sens=True, **_fdress(c))
     return dict(out=out, dmin=dmin, sens=sens)
 
 
@@ -85,7 +90,7 @@ def oracle_run_dm2(c, R, sel=None):
     assert kd == "matsubara3d"
     a, b, sa, sb = oracle.matsubara3d_dm2(c["T"], c["n_max"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
                                           *R["q"], *R["c"], c["Zpsi"], c["Zphi"], c["lnq_lo"], c["lnq_hi"], c["interp"],
-                                          c["coef"], c["m2psi"], c["m2phi"], c["pext"], c["n_jext"], sel=sel, **_dress(c))
+                                          c["coef"], c["m2psi"], c["m2phi"], c["pext"], c["n_jext"], sel=sel, **_fdress(c))
     return dict(dpsi=(a, sa), dphi=(b, sb))
 
 
