@@ -69,6 +69,16 @@ void dfrg_shutdown(void);               /* frees the calling thread's device are
  *   R = zk R_shape,   Rdot = k d(Z_k R_shape)/dk = zk (Rdot_shape - eta R_shape)
  * in every propagator and in the insertion.  zk > 0 is required (DFRG_EINVAL otherwise: a zero-initialised struct is
  * rejected); zk = 1, eta = 0 gives the plain shapes.  Z_k dresses the regulator only, not the s term (reading A12/A20). */
+/* Fermionic regulator (the paper's RF / RFdot; its finite-temperature and finite-density examples are
+ * fermionic; the paper prints no fermionic shape -- DESIGN.md reading A25).  A fermion line of a
+ * descriptor with fermion_reg = 1 is regulated on its Dirac structure, i pslash (1 + r_F), with (1 + r_F)^2 = 1 + r_B:
+ *   R_F(s) = sqrt(s + R_shape(s)) - sqrt(s)      (momentum dimension one; flat shape: (k - sqrt(s)) Theta(k^2 - s))
+ *   k dR_F/dk = Rdot_shape(s) / (2 sqrt(s + R_shape(s)))
+ *   RF = zk R_F,  RFdot = zk (k dR_F/dk - eta R_F)
+ * and has the denominator  D = Z^2 (s - sR) + (Z sqrt(sR) + RF(sR))^2 + m2  with the insertion  2 (Z sqrt(sR) + RF(sR)) RFdot(sR)
+ * in place of  Z s + R(sR) + m2  and  Rdot(sR)   (sR = argument of the regulator: s, or its spatial part for "3D" regulators,
+ * s - sR then being the squared time component; Z = the line's dressing table; m2 = the squared fermion mass).
+ * With zk = 1, eta = 0 and Z = 1 the two switches describe the same function. */
 typedef enum { DFRG_REG_LITIM = 0, DFRG_REG_EXP_POLY = 1 } dfrg_reg_kind;
 typedef struct {
   int kind;
@@ -144,6 +154,9 @@ typedef struct {
   double* dchan; /* nullable output [2][n_field] */
   int statistics; /* DFRG_STAT_BOSON (0): the sums above.  DFRG_STAT_FERMION (1): see below */
   double mu;      /* chemical potential (fermionic statistics only; must be 0 otherwise) */
+  int fermion_reg; /* fermionic statistics only (must be 0 otherwise).  0: the loop is regulated with R / Rdot as written above.
+                      1: with RF / RFdot (see dfrg_regulator):  D = (nu_n + i mu)^2 + (q_i + RF(q_i^2))^2 + m2,
+                      Rdot(q_i^2) -> 2 (q_i + RF(q_i^2)) RFdot(q_i^2) */
 } dfrg_lpa_desc;
 
 int dfrg_integrate_lpa(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u, const double* du,
@@ -266,6 +279,11 @@ typedef struct {
   int path;             /* kernel-path selection, an OR of dfrg_mats3d_path bits; 0 = the library's own choice.  Every path
                            computes the same sums (the tests run them all on the same inputs); the field exists for testing
                            and tuning and is part of the descriptor so that the call stays free of global state. */
+  int fermion_reg;      /* 0: the fermion line is regulated with R / Rdot as written above (BASELINE.json config 4).
+                           1: with RF / RFdot on its Dirac structure (see dfrg_regulator; reading A25):
+                              A = Z_psi sqrt(sR) + RF(sR),  sR = s_psi (reg_arg4d = 1) or q^2 (reg_arg4d = 0)
+                              G_psi = 1/(Z_psi^2 (s_psi - sR) + A^2 + m2_psi[f]),   Rdot(sR) -> 2 A RFdot(sR)
+                              (s_psi - sR = (nu_n + i mu)^2 for spatial regulators, 0 otherwise); the boson line is unchanged. */
 } dfrg_mats3d_desc;
 typedef enum {
   DFRG_M3_AUTO = 0,

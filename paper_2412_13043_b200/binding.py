@@ -52,7 +52,7 @@ class Table3D(C.Structure):
 class LpaDesc(C.Structure):
     _fields_ = [("d", C.c_int), ("T", C.c_double), ("n_max", C.c_int), ("reg_arg4d", C.c_int), ("N", C.c_double),
                 ("prefactor", C.c_double), ("reg", Regulator), ("q", Rule), ("dchan", _vp),
-                ("statistics", C.c_int), ("mu", C.c_double)]
+                ("statistics", C.c_int), ("mu", C.c_double), ("fermion_reg", C.c_int)]
 
 
 class Loop4dDesc(C.Structure):
@@ -67,7 +67,7 @@ class Mats3dDesc(C.Structure):
                 ("q", Rule), ("cos1", Rule), ("tab_psi", Table), ("tab_phi", Table),
                 ("coef", _vp), ("n_coef", C.c_int), ("dout_dm2_psi", _vp), ("dout_dm2_phi", _vp),
                 ("reg_arg4d", C.c_int), ("mu", C.c_double), ("out_im", _vp),
-                ("dout_dm2_psi_im", _vp), ("dout_dm2_phi_im", _vp), ("path", C.c_int)]
+                ("dout_dm2_psi_im", _vp), ("dout_dm2_phi_im", _vp), ("path", C.c_int), ("fermion_reg", C.c_int)]
 
 
 class DfrgError(RuntimeError):
@@ -170,16 +170,17 @@ def dfrg_matsubara_n_max(domain, T, k, extent):
 
 # ---- LPA ------------------------------------------------------------------------------------------
 def _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, device, dchan=None, reg_zk=1.0, reg_eta=0.0,
-              statistics=STAT_BOSON, mu=0.0):
+              statistics=STAT_BOSON, mu=0.0, fermion_reg=0):
     return LpaDesc(int(d), float(T), int(n_max), int(reg_arg4d), float(N), float(prefactor),
                    Regulator(int(reg_kind), int(reg_order), float(k), float(reg_zk), float(reg_eta)), _rule(rule_q, device),
-                   _ptr(dchan, device), int(statistics), float(mu))
+                   _ptr(dchan, device), int(statistics), float(mu), int(fermion_reg))
 
 
 def dfrg_integrate_lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, rho, u, du,
-                       flow, chan=None, dmin=None, dchan=None, reg_zk=1.0, reg_eta=0.0, statistics=STAT_BOSON, mu=0.0):
+                       flow, chan=None, dmin=None, dchan=None, reg_zk=1.0, reg_eta=0.0, statistics=STAT_BOSON, mu=0.0,
+                       fermion_reg=0):
     """dchan (optional, [2, n_field]): dI/dm2 per channel (include/dfrg.h, "Mass derivatives")."""
-    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, True, dchan, reg_zk, reg_eta, statistics, mu)
+    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, True, dchan, reg_zk, reg_eta, statistics, mu, fermion_reg)
     _check(lib().dfrg_integrate_lpa(C.byref(D), int(rho.numel()), _ptr(rho, True), _ptr(u, True), _ptr(du, True),
                                     _ptr(flow, True), _ptr(chan, True), _ptr(dmin, True), _stream()),
            "dfrg_integrate_lpa")
@@ -187,8 +188,9 @@ def dfrg_integrate_lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order
 
 
 def dfrg_integrate_lpa_host(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, rho, u, du,
-                            flow, chan=None, dmin=None, dchan=None, reg_zk=1.0, reg_eta=0.0, statistics=STAT_BOSON, mu=0.0):
-    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, False, dchan, reg_zk, reg_eta, statistics, mu)
+                            flow, chan=None, dmin=None, dchan=None, reg_zk=1.0, reg_eta=0.0, statistics=STAT_BOSON, mu=0.0,
+                       fermion_reg=0):
+    D = _lpa_desc(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, False, dchan, reg_zk, reg_eta, statistics, mu, fermion_reg)
     n_field = rho.numel() if hasattr(rho, "numel") else rho.size
     _check(lib().dfrg_integrate_lpa_host(C.byref(D), int(n_field), _ptr(rho, False), _ptr(u, False),
                                          _ptr(du, False), _ptr(flow, False), _ptr(chan, False), _ptr(dmin, False)),
@@ -244,24 +246,24 @@ def dfrg_integrate_loop4d_host(family, prefactor, reg_kind, reg_order, k, rule_q
 # ---- matsubara3d ----------------------------------------------------------------------------------
 def _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp, coef,
                device, dpsi=None, dphi=None, reg_zk=1.0, reg_eta=0.0, reg_arg4d=1, mu=0.0, out_im=None,
-               dpsi_im=None, dphi_im=None, path=0):
+               dpsi_im=None, dphi_im=None, path=0, fermion_reg=0):
     return Mats3dDesc(float(T), int(n_max), float(prefactor), Regulator(int(reg_kind), int(reg_order), float(k), float(reg_zk), float(reg_eta)),
                       _rule(rule_q, device), _rule(rule_c, device),
                       _table(Zpsi, lnq_lo, lnq_hi, interp, device), _table(Zphi, lnq_lo, lnq_hi, interp, device),
                       _ptr(coef, device), _n(coef), _ptr(dpsi, device), _ptr(dphi, device),
                       int(reg_arg4d), float(mu), _ptr(out_im, device), _ptr(dpsi_im, device), _ptr(dphi_im, device),
-                      int(path))
+                      int(path), int(fermion_reg))
 
 
 def dfrg_integrate_matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo,
                                lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, out, dmin=None,
                                dout_dm2_psi=None, dout_dm2_phi=None, reg_zk=1.0, reg_eta=0.0, reg_arg4d=1, mu=0.0, out_im=None,
-                               dout_dm2_psi_im=None, dout_dm2_phi_im=None, path=0):
+                               dout_dm2_psi_im=None, dout_dm2_phi_im=None, path=0, fermion_reg=0):
     """out: [n_p, n_jext, n_field].  reg_arg4d=0: spatial regulators; mu != 0 (needs reg_arg4d=0 and out_im): complex result,
     out = real part, out_im = imaginary part (include/dfrg.h, dfrg_mats3d_desc::mu)."""
     D = _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp,
                    coef, True, dout_dm2_psi, dout_dm2_phi, reg_zk, reg_eta, reg_arg4d, mu, out_im, dout_dm2_psi_im, dout_dm2_phi_im,
-                   path)
+                   path, fermion_reg)
     _check(lib().dfrg_integrate_matsubara3d(C.byref(D), _n(m2psi), _ptr(m2psi, True), _ptr(m2phi, True), _n(pext),
                                             _ptr(pext, True), int(n_jext), _ptr(out, True), _ptr(dmin, True),
                                             _stream()), "dfrg_integrate_matsubara3d")
@@ -271,10 +273,10 @@ def dfrg_integrate_matsubara3d(T, n_max, prefactor, reg_kind, reg_order, k, rule
 def dfrg_integrate_matsubara3d_host(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo,
                                     lnq_hi, interp, coef, m2psi, m2phi, pext, n_jext, out, dmin=None,
                                dout_dm2_psi=None, dout_dm2_phi=None, reg_zk=1.0, reg_eta=0.0, reg_arg4d=1, mu=0.0, out_im=None,
-                               dout_dm2_psi_im=None, dout_dm2_phi_im=None, path=0):
+                               dout_dm2_psi_im=None, dout_dm2_phi_im=None, path=0, fermion_reg=0):
     D = _mats_desc(T, n_max, prefactor, reg_kind, reg_order, k, rule_q, rule_c, Zpsi, Zphi, lnq_lo, lnq_hi, interp,
                    coef, False, dout_dm2_psi, dout_dm2_phi, reg_zk, reg_eta, reg_arg4d, mu, out_im, dout_dm2_psi_im, dout_dm2_phi_im,
-                   path)
+                   path, fermion_reg)
     _check(lib().dfrg_integrate_matsubara3d_host(C.byref(D), _n(m2psi), _ptr(m2psi, False), _ptr(m2phi, False),
                                                  _n(pext), _ptr(pext, False), int(n_jext), _ptr(out, False),
                                                  _ptr(dmin, False)), "dfrg_integrate_matsubara3d_host")

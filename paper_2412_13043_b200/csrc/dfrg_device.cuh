@@ -167,6 +167,24 @@ __device__ __forceinline__ void regulator(const RegParams& rp, const FastMath& f
   Rdot = rp.zk * (2.0 * r * (1.0 + geo) - rp.eta * r);
 }
 
+// Fermion line regulated with the fermionic regulator RF / RFdot (reading A25):
+//   (sqrt(s) + R_F)^2 = s + R_B  =>  R_F = R_B/(sqrt(s + R_B) + sqrt(s)),  k dR_F/dk = RBdot/(2 sqrt(s + R_B)),
+//   RF = zk R_F,  RFdot = zk (k dR_F/dk - eta R_F);  kinetic term A = Z sqrt(sR) + RF(sR) at the regulator argument sR.
+// Returns A; ins = 2 A RFdot (what replaces Rdot in the insertion).  The line's denominator is Z^2 (s - sR) + A^2 + m^2.
+__device__ __forceinline__ double fermion_kinetic(const RegParams& rp, const FastMath& fm, const double Z, const double sR,
+                                                  double& ins) {
+  RegParams shape = rp;
+  shape.zk = 1.0; shape.eta = 0.0;
+  double Rb, Rbd;
+  regulator(shape, fm, sR, Rb, Rbd);
+  const double root = sqrt(sR + Rb), sq = sqrt(sR);
+  const double rf = Rb / (root + sq);
+  const double rfd = Rbd / (2.0 * root);
+  const double A = fma(Z, sq, rp.zk * rf);
+  ins = 2.0 * A * (rp.zk * (rfd - rp.eta * rf));
+  return A;
+}
+
 // ---- log-grid table look-up --------------------------------------------------------------------
 // A table row v[0..n-1] on ln q_i = lo + i h is turned, once per CTA, into per-cell cubics in shared memory:
 //   cubic mode (interp 3): cell c = stencil i0 = c, anchored at node c+1:  p(tau) = v[c+1] + tau (d1 + tau (d2 + tau d3)),

@@ -20,7 +20,7 @@ constexpr int LPA_FTILE = 32;
 constexpr int LPA_MAX_PAIRS = 12288;
 
 struct LpaParams {
-  int d, n_max, reg_arg4d, nq, n_field;
+  int d, n_max, reg_arg4d, nq, n_field, fermion_reg;
   double T, N, prefactor, mu;
   RegParams reg;
   FastMathConsts fmc;
@@ -165,10 +165,16 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_fermion_kernel(const LpaParam
     const int n = t / P.nq, i = t - n * P.nq;
     const double q = sx[i];
     const double nu = (2.0 * (double)n + 1.0) * pi_T;
-    double R, Rd;
-    regulator(P.reg, fm, q * q, R, Rd);
+    double K, Rd;   // K = q^2 + R(q^2), or (q + RF(q^2))^2 with the fermionic regulator (reading A25)
+    if (P.fermion_reg) {
+      const double A = fermion_kinetic(P.reg, fm, 1.0, q * q, Rd);
+      K = A * A;
+    } else {
+      regulator(P.reg, fm, q * q, K, Rd);
+      K += q * q;
+    }
     const double b = 2.0 * nu * P.mu;
-    tab[t] = make_double4(nu * nu - P.mu * P.mu + q * q + R, 2.0 * (sw[i] * ipow(q, P.d - 1) * Rd), b * b, 0.0);
+    tab[t] = make_double4(nu * nu - P.mu * P.mu + K, 2.0 * (sw[i] * ipow(q, P.d - 1) * Rd), b * b, 0.0);
   }
   __syncthreads();
 
@@ -231,6 +237,7 @@ static int lpa_launch(const dfrg_lpa_desc* D, int n_field, const double* rho, co
                       double* flow, double* chan, double* dmin, cudaStream_t stream) {
   LpaParams P;
   P.d = D->d; P.n_max = D->n_max; P.reg_arg4d = D->reg_arg4d; P.nq = D->q.n; P.n_field = n_field;
+  P.fermion_reg = D->fermion_reg;
   P.T = D->T; P.N = D->N; P.prefactor = D->prefactor; P.mu = D->mu;
   P.reg = reg_params(D->reg.kind, D->reg.order, D->reg.k, D->reg.zk, D->reg.eta);
   P.fmc = fm_consts();
@@ -260,7 +267,8 @@ static int lpa_validate(const dfrg_lpa_desc* D, int n_field, const double* rho, 
     // fermionic frequencies need T > 0; with a chemical potential the time component is complex: spatial regulator only
     if (!(D->T > 0.0) || D->reg_arg4d != 0 || !(D->mu == D->mu)) return DFRG_EINVAL;
     if (n_terms * D->q.n > LPA_MAX_PAIRS / 2) return DFRG_EUNSUPPORTED;
-  } else if (D->mu != 0.0) {
+    if (D->fermion_reg != 0 && D->fermion_reg != 1) return DFRG_EINVAL;
+  } else if (D->mu != 0.0 || D->fermion_reg != 0) {
     return DFRG_EINVAL;
   }
   if (n_terms * D->q.n > LPA_MAX_PAIRS) return DFRG_EUNSUPPORTED;

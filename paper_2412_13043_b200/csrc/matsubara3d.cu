@@ -33,6 +33,7 @@ static int mats3d_validate(const dfrg_mats3d_desc* D, int n_field, const double*
   if ((long long)D->q.n * D->cos1.n > M3_MAX_PAIRS || D->tab_psi.n_q > 1024) return DFRG_EUNSUPPORTED;
   if ((long long)n_p * n_jext > 2147483647LL || n_p > 65535) return DFRG_EUNSUPPORTED;
   if ((D->reg_arg4d != 0 && D->reg_arg4d != 1) || !(D->mu == D->mu)) return DFRG_EINVAL;
+  if (D->fermion_reg != 0 && D->fermion_reg != 1) return DFRG_EINVAL;
   if (D->path < 0 || D->path > 63) return DFRG_EINVAL;
   if (D->mu != 0.0) {
     if (D->reg_arg4d != 0 || !D->out_im) return DFRG_EINVAL;   // complex time component: spatial regulators only
@@ -100,7 +101,7 @@ static int mats3d_launch(const dfrg_mats3d_desc* D, int n_field, const double* m
   P.Zpsi = D->tab_psi.v; P.Zphi = D->tab_phi.v; P.coef = D->coef;
   P.m2psi = m2_psi; P.m2phi = m2_phi; P.pext = p; P.out = out; P.dmin = dmin;
   P.part = nullptr; P.tile_fields = 0; P.max_slots = 0; P.grid_main = 0; P.mode = 0; P.sym_try = 0; P.symflag = nullptr;
-  P.reg_arg4d = D->reg_arg4d; P.mu = D->mu;
+  P.reg_arg4d = D->reg_arg4d; P.mu = D->mu; P.fermion_reg = D->fermion_reg;
   P.psi_im = nullptr; P.psimin_f = nullptr; P.out_im = nullptr; P.part_im = nullptr;
   const bool cplx = D->mu != 0.0;
 

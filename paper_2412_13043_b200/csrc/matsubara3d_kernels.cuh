@@ -34,6 +34,7 @@ struct Mats3dParams {
   int sym_try;       // host: the cos rule is long enough for the symmetric-pair moment loop (nc % 8 == 0)
   int* symflag;      // device: 1 if the cos rule is exactly symmetric (x_c = -x_{nc-1-c}, equal weights), set by the pre-pass
   int reg_arg4d;     // 1: regulators at the 4-momentum squared; 0: spatial regulators
+  int fermion_reg;   // 1: fermion line regulated with RF / RFdot on its Dirac structure (reading A25)
   double mu;         // chemical potential (complex fermion line when != 0)
   double *psi_im;    // [2 n_max + 1][psi_stride]  Im D0psi (mu != 0)
   double *psimin_f;  // [n_field]  min over (n, q) of |D0psi + m2psi_f| (mu != 0)
@@ -104,12 +105,20 @@ static __global__ void __launch_bounds__(128) mats3d_psi_kernel(const Mats3dPara
   for (int i = threadIdx.x; i < P.nq; i += 128) {
     const double q = P.xq[i];
     const double spsi = nun * nun - P.mu * P.mu + q * q;   // Re (nu + i mu)^2 + q^2
-    double R, Rd;
-    regulator(P.reg, fm, P.reg_arg4d ? spsi : q * q, R, Rd);
     const double Z = table_lookup(cells, P.grid, fm, q * q);
-    const double D0 = Z * spsi + R;
+    double D0, Rd, Zt = Z;   // Zt: what multiplies the squared time component (nu + i mu)^2
+    if (P.fermion_reg) {     // reading A25: D = Z^2 (s - sR) + (Z sqrt(sR) + RF(sR))^2 + m2, insertion 2 A RFdot
+      const double sR = P.reg_arg4d ? spsi : q * q;   // (mu != 0 needs the spatial argument: spsi is real here)
+      const double A = fermion_kinetic(P.reg, fm, Z, sR, Rd);
+      Zt = Z * Z;
+      D0 = fma(Zt, spsi - sR, A * A);
+    } else {
+      double R;
+      regulator(P.reg, fm, P.reg_arg4d ? spsi : q * q, R, Rd);
+      D0 = Z * spsi + R;
+    }
     P.psi[(size_t)it * P.psi_stride + i] = make_double2(D0, P.wq[i] * q * q * Rd);
-    if (P.psi_im) P.psi_im[(size_t)it * P.psi_stride + i] = Z * (2.0 * nun * P.mu);
+    if (P.psi_im) P.psi_im[(size_t)it * P.psi_stride + i] = Zt * (2.0 * nun * P.mu);
     dmin = fmin(dmin, D0);
   }
   dmin = block_min(dmin, red);

@@ -49,7 +49,8 @@ def gpu_run(c, R, host=False, want_dmin=True, want_d=False, canary=False):
         fn = B.dfrg_integrate_lpa_host if host else B.dfrg_integrate_lpa
         fn(c["d"], c["T"], c["n_max"], c["reg_arg4d"], c["N"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
            rule("q"), up(c["rho"]), up(c["u"]), up(c["du"]), flow, chan, dmin, dchan=dchan,
-           statistics=c.get("statistics", 0), mu=c.get("mu", 0.0) if c.get("statistics", 0) == 1 else 0.0, **dress)
+           statistics=c.get("statistics", 0), mu=c.get("mu", 0.0) if c.get("statistics", 0) == 1 else 0.0,
+           fermion_reg=c.get("fermion_reg", 0), **dress)
         res = dict(out=flow, chan=chan, dmin=dmin, dchan=dchan)
     elif kd == "twopoint":
         out = new(c["pext"].size, c["m2"].size)
@@ -96,7 +97,7 @@ def gpu_run(c, R, host=False, want_dmin=True, want_d=False, canary=False):
            up(c["Zpsi"]), up(c["Zphi"]), c["lnq_lo"], c["lnq_hi"], c["interp"], up(c["coef"]), up(c["m2psi"]),
            up(c["m2phi"]), up(c["pext"]), c["n_jext"], out, dmin, dout_dm2_psi=dpsi, dout_dm2_phi=dphi,
            reg_arg4d=c.get("reg_arg4d", 1), mu=c.get("mu", 0.0) if spatial else 0.0, out_im=out_im,
-           path=c.get("path", 0), **dress)
+           path=c.get("path", 0), fermion_reg=c.get("fermion_reg", 0), **dress)
         res = dict(out=out, dmin=dmin, dpsi=dpsi, dphi=dphi, out_im=out_im)
     if not host:
         torch.cuda.synchronize()
