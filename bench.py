@@ -373,6 +373,7 @@ def main():
     b.record()
     b.synchronize()
     probe_tflops = probe_flops / (a.elapsed_time(b) * 1e-3) * 1e-12
+    issue_model = probe.fp64_issue_model(sink)                # 8 DFMA + {0, 4, 8} integer adds: DESIGN.md section 7
 
     for _ in range(args.warmup):
         step()
@@ -465,6 +466,9 @@ def main():
                          "peak_kind": "nominal FP64: %d SMs x %d lanes x 2 x %.0f MHz (MEASURED_PEAKS.json has no FP64 "
                                       "entry)" % (sms, FP64_LANES_PER_SM, sm_max_mhz),
                          "peak_probe_tflops": probe_tflops, "frac_of_probe": achieved / probe_tflops,
+                         "issue_model_probe": dict(issue_model, kind="time of 8 DFMA chains + K integer adds per 8 DFMA, "
+                                                   "K = 0, 4, 8; ratios (16 + K)/16 would mean an FP64 instruction holds the issue port for 2 cycles, ratios of 1 "
+                                                   "that other instructions issue in its shadow (bound = the FP64 pipe)"),
                          "alg_flops_per_launch": flops},
             "wall_s_timed_region": t_wall}
 

@@ -33,6 +33,13 @@
  *    gives whatever IEEE arithmetic gives; `dmin` reports it (signed minimum over all quadrature
  *    nodes and all propagators of an output of denominator / k^2; reading A4 in DESIGN.md).
  *    An exactly zero denominator yields NaN (the reciprocal is a Newton iteration on a hardware seed).
+ *    Magnitude range and coupling of the batched reciprocals: the two-point and Matsubara kernels invert the denominators
+ *    of the TWO field points a thread owns (f and f + tile/2 of a field tile: f + 128 in the two-point family, f + 256 in
+ *    dfrg_integrate_matsubara3d) at one or two neighbouring quadrature nodes jointly, 1/(d_1 d_2 [d_3 d_4]) from one seed.
+ *    Every denominator must therefore satisfy 1e-75 k^2 < |D| < 1e75 k^2 (the product of four stays inside the double
+ *    range; physical denominators lie between ~1e-3 k^2 and ~1e6 k^2), and a denominator that is exactly zero, subnormal,
+ *    infinite or NaN at field point f makes the output of its partner field point NaN as well (the partner's own dmin does
+ *    not show it: check dmin of both).  dfrg_mats3d_desc::path = DFRG_M3_ONE_FIELD inverts every field point on its own.
  *  - Mass derivatives (Jacobian support; the paper's "AD" kernels for implicit time-steppers, PAPER.md:713-723
  *    eq. 27 and PAPER.md:1842): every descriptor of a family with a field axis carries nullable output pointers
  *    for the derivative of each integral with respect to the mass term of its propagators,

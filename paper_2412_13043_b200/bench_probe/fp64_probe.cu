@@ -23,7 +23,52 @@ __global__ void __launch_bounds__(512) fp64_peak_kernel(int n_iter, double* sink
   const double s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
   if (s == 123456.789) sink[0] = s;  // never true; keeps the chains alive
 }
+
+// Issue model: the same 8 DFMA chains with K independent 32-bit integer adds (volatile inline PTX: one SASS IADD each,
+// never merged or removed) interleaved per 8 DFMA.  If an FP64 warp instruction holds its scheduler's issue port for two
+// cycles and any other instruction for one, the time grows as (16 + K)/16; if the port were free in the second cycle of
+// an FP64 instruction, K <= 8 would cost nothing.
+template <int K>
+__global__ void __launch_bounds__(512) fp64_issue_kernel(int n_iter, double* sink) {
+  double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 0.1, a2 = a0 + 0.2, a3 = a0 + 0.3;
+  double a4 = a0 + 0.4, a5 = a0 + 0.5, a6 = a0 + 0.6, a7 = a0 + 0.7;
+  int x[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) x[i] = threadIdx.x + i;
+  const double m = 0.999999, c = 1e-7;
+  for (int it = 0; it < n_iter; ++it) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+#pragma unroll
+      for (int i = 0; i < K / 2; ++i) asm volatile("add.s32 %0, %0, 7;" : "+r"(x[i]));
+      a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+#pragma unroll
+      for (int i = K / 2; i < K; ++i) asm volatile("add.s32 %0, %0, 7;" : "+r"(x[i]));
+    }
+  }
+  const double s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  int xs = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) xs ^= x[i];
+  if (s == 123456.789 || xs == 0x7fffffff) sink[0] = s;
+}
 }  // namespace
+
+//   int dfrg_probe_fp64_issue(int n_iter, int k_int, double* sink_dev, void* cuda_stream)
+// launches the issue-model kernel with k_int in {0, 4, 8} integer adds per 8 DFMA (one CTA of 512 threads per SM).
+extern "C" int dfrg_probe_fp64_issue(int n_iter, int k_int, double* sink, void* cuda_stream) {
+  if (n_iter < 1 || !sink) return -1;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return -3;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -3;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (k_int == 0) fp64_issue_kernel<0><<<sms, 512, 0, st>>>(n_iter, sink);
+  else if (k_int == 4) fp64_issue_kernel<4><<<sms, 512, 0, st>>>(n_iter, sink);
+  else if (k_int == 8) fp64_issue_kernel<8><<<sms, 512, 0, st>>>(n_iter, sink);
+  else return -1;
+  return cudaGetLastError() == cudaSuccess ? 0 : -3;
+}
 
 extern "C" int dfrg_probe_fp64_peak(int n_iter, int ctas_per_sm, double* sink, double* flops_out, void* cuda_stream) {
   if (n_iter < 1 || ctas_per_sm < 1 || ctas_per_sm > 4 || !sink) return -1;

@@ -72,17 +72,17 @@ __device__ __forceinline__ double clamp_hi(double x, double hi) {  // x < hi ? x
   return r;
 }
 constexpr int FM_DOUBLES = 2 * 128 + 64;
+#include "fm_tables.inc"   // kFmLog, kFmExp, kLg2Log: correctly rounded constants (gen_fm_tables.py)
 
 // All threads of the CTA; the caller synchronises before first use.  mem: FM_DOUBLES doubles, 16-byte aligned.
+// The tables are constants of the library (fm_tables.inc): a CTA copies them from global memory (L2 resident after the
+// first CTA) instead of computing 128 divisions + logarithms and 64 exp2 in its set-up.
 __device__ __forceinline__ FastMath fm_build(double* mem, const FastMathConsts& consts) {
   double2* lt = reinterpret_cast<double2*>(mem);
   double* et = mem + 256;
-  for (int j = threadIdx.x; j < 128; j += blockDim.x) {
-    const double c = 1.0 + ((double)j + 0.5) * (1.0 / 128.0);
-    const double inv = 1.0 / c;
-    lt[j] = make_double2(inv, -log(inv));  // ln of the centre the rounded reciprocal stands for
-  }
-  for (int j = threadIdx.x; j < 64; j += blockDim.x) et[j] = exp2((double)j * (1.0 / 64.0));
+  for (int j = threadIdx.x; j < 128; j += blockDim.x)
+    lt[j] = make_double2(kFmLog[2 * j], kFmLog[2 * j + 1]);  // (1/c_j rounded, ln of the centre the rounded reciprocal stands for)
+  for (int j = threadIdx.x; j < 64; j += blockDim.x) et[j] = kFmExp[j];
   FastMath fm;
   fm.logtab = lt;
   fm.exptab = et;
@@ -257,11 +257,10 @@ __device__ __forceinline__ LogGrid lg_build(double* mem, const double lo, const 
   double2* mt = reinterpret_cast<double2*>(mem);
   const double A = 0.5 * inv_h, B = -lo * inv_h;
   const double ex1 = A * 0.6931471805599453;
-  const double lnA = log(A);
   for (int j = threadIdx.x; j < LG_NM; j += blockDim.x) {
-    const double c = 1.0 + ((double)j + 0.5) * (1.0 / (double)LG_NM);
-    const double ainv = A / c;                       // the rounded value defines the centre: c_j := A / ainv
-    const double2 ent = make_double2(ainv, fma(A, lnA - log(ainv), B));
+    // c_j = 1/inv_j with inv_j = fl(1/(1 + (j + 1/2)/512)) from the constant table; A inv_j is rounded once more, which moves
+    // the centre it stands for by < 1.2e-16 relative (5e-16 in t, against ulp(t) = 1.4e-14 at the top of the grid)
+    const double2 ent = make_double2(A * kLg2Log[2 * j], fma(-A, kLg2Log[2 * j + 1], B));
 #pragma unroll
     for (int r = 0; r < LG_REP; ++r) mt[j * LG_REP + r] = ent;
   }
@@ -368,9 +367,9 @@ struct LogGrid2 {
 __device__ __forceinline__ LogGrid2 lg2_build(double* mem, const LogGrid2Consts& K, const int n) {
   double2* mt = reinterpret_cast<double2*>(mem);
   for (int j = threadIdx.x; j < LG_NM; j += blockDim.x) {
-    const double c = 1.0 + ((double)j + 0.5) * (1.0 / (double)LG_NM);
-    const double inv = 1.0 / c;                      // the rounded value defines the centre: c_j := 1 / inv
-    const double2 ent = make_double2(inv, fma(-K.a1, log(inv), K.bq));
+    static_assert(LG_NM == 512, "kLg2Log holds 512 entries");
+    const double inv = kLg2Log[2 * j];               // fl(1/c_j), c_j = 1 + (j + 1/2)/512; the rounded value defines the centre
+    const double2 ent = make_double2(inv, fma(-K.a1, kLg2Log[2 * j + 1], K.bq));
 #pragma unroll
     for (int r = 0; r < LG_REP; ++r) mt[j * LG_REP + r] = ent;
   }
@@ -439,7 +438,7 @@ constexpr int FX_REP = 16;
 constexpr int FX_DOUBLES = 64 * FX_REP;
 __device__ __forceinline__ const double* fx_build(double* mem, const double k2) {
   for (int j = threadIdx.x; j < 64; j += blockDim.x) {
-    const double v = k2 * exp2((double)j * (1.0 / 64.0));
+    const double v = k2 * kFmExp[j];
 #pragma unroll
     for (int r = 0; r < FX_REP; ++r) mem[j * FX_REP + r] = v;
   }
@@ -587,6 +586,21 @@ __device__ __forceinline__ double block_sum(double v, double* scratch) {
     for (int w = 0; w < nw; ++w) r += scratch[w];
   return r;
 }
+// Compensated sum of the per-CTA partial sums of an output (fix-up kernels).  north_star asks for Kahan-compensated partial
+// sums "where ncu shows it is free": it is free here -- a fix-up kernel adds <= a handful of slots per output and waits on its
+// loads -- and nowhere else: the hot loops are bound by FP64 issue slots ("Kahan"), where a compensated
+// add costs three more FP64 instructions per term.  Neumaier's variant (the correction also covers |x| > |sum|); deterministic.
+struct CompSum {
+  double s, c;
+  __device__ __forceinline__ explicit CompSum(double x) : s(x), c(0.0) {}
+  __device__ __forceinline__ void add(double x) {
+    const double t = s + x;
+    c += (fabs(s) >= fabs(x)) ? (s - t) + x : (x - t) + s;
+    s = t;
+  }
+  __device__ __forceinline__ double value() const { return s + c; }
+};
+
 __device__ __forceinline__ double block_min(double v, double* scratch) {
   v = warp_min(v);
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;

@@ -222,9 +222,9 @@ __global__ void __launch_bounds__(256) fp4_fixup_kernel(const FourPointParams P)
   const long long U = (long long)P.n_ext * P.NCH;
   const long long ufirst = e * P.NCH, ulast = ufirst + P.NCH - 1;
   const int c_first = (int)(((ufirst + 1) * P.grid_main - 1) / U), c_last = (int)(((ulast + 1) * P.grid_main - 1) / U);
-  double t = P.part[e];
-  for (int s = 1; s <= c_last - c_first; ++s) t += P.part[(size_t)s * P.n_ext + e];
-  P.out[e] = P.prefactor * t;
+  CompSum t(P.part[e]);
+  for (int s = 1; s <= c_last - c_first; ++s) t.add(P.part[(size_t)s * P.n_ext + e]);
+  P.out[e] = P.prefactor * t.value();
   if (P.dmin) {
     double dm = P.partD[e];
     for (int s = 1; s <= c_last - c_first; ++s) dm = fmin(dm, P.partD[(size_t)s * P.n_ext + e]);

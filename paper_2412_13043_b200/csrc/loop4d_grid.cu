@@ -420,8 +420,9 @@ __global__ void __launch_bounds__(256) t3g_fixup_kernel(const ThreeGridParams Q)
   const long long U = (long long)S * NCH;
   const long long ufirst = (long long)r * NCH, ulast = ufirst + NCH - 1;
   const int c_first = (int)(((ufirst + 1) * Q.grid_main - 1) / U), c_last = (int)(((ulast + 1) * Q.grid_main - 1) / U);
-  double t = Q.part[e];
-  for (int s = 1; s <= c_last - c_first; ++s) t += Q.part[(size_t)s * P.n_ext + e];
+  CompSum ts(Q.part[e]);
+  for (int s = 1; s <= c_last - c_first; ++s) ts.add(Q.part[(size_t)s * P.n_ext + e]);
+  const double t = ts.value();
   double sum_wphi = 0.0;
   for (int jp = 0; jp < P.nphi; ++jp) sum_wphi += P.wphi[jp];
   P.out[e] = P.prefactor * sum_wphi * t;

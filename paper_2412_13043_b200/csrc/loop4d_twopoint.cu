@@ -259,13 +259,13 @@ __global__ void __launch_bounds__(256) tp_fixup_kernel(const TwoPointParams P) {
   const int c_first = (int)(((ufirst + 1) * P.grid_main - 1) / U), c_last = (int)(((ulast + 1) * P.grid_main - 1) / U);
   const int nd = P.dout ? 2 : 1;
   const size_t plane = (size_t)n_out;
-  double r = P.part[idx];
-  for (int s = 1; s <= c_last - c_first; ++s) r += P.part[(size_t)s * nd * plane + idx];
-  P.out[idx] = P.prefactor * r;
+  CompSum r(P.part[idx]);
+  for (int s = 1; s <= c_last - c_first; ++s) r.add(P.part[(size_t)s * nd * plane + idx]);
+  P.out[idx] = P.prefactor * r.value();
   if (P.dout) {
-    double dr = P.part[plane + idx];
-    for (int s = 1; s <= c_last - c_first; ++s) dr += P.part[((size_t)s * 2 + 1) * plane + idx];
-    P.dout[idx] = -P.prefactor * dr;
+    CompSum dr(P.part[plane + idx]);
+    for (int s = 1; s <= c_last - c_first; ++s) dr.add(P.part[((size_t)s * 2 + 1) * plane + idx]);
+    P.dout[idx] = -P.prefactor * dr.value();
   }
   if (P.dmin) {
     constexpr int NW = TP_NPROD / 32;

@@ -1315,14 +1315,15 @@ static __global__ void __launch_bounds__(256) mats3d_fixup_kernel(const Mats3dPa
   const long long ufirst = (long long)(f / P.tile_fields) * upp + (long long)e * P.nq, ulast = ufirst + P.nq - 1;
   const int c_first = (int)(((ufirst + 1) * P.grid_main - 1) / U), c_last = (int)(((ulast + 1) * P.grid_main - 1) / U);
   const size_t stride = (size_t)P.n_p * P.n_jext * P.n_field;
-  double r = P.part[idx];
-  for (int s = 1; s <= c_last - c_first; ++s) r += P.part[(size_t)s * stride + idx];
-  P.out[idx] = P.prefactor * P.T * r;
+  CompSum r(P.part[idx]);
+  for (int s = 1; s <= c_last - c_first; ++s) r.add(P.part[(size_t)s * stride + idx]);
+  P.out[idx] = P.prefactor * P.T * r.value();
   if (P.out_im) {
     double ri = 0.0;
     if (P.part_im) {
-      ri = P.part_im[idx];
-      for (int s = 1; s <= c_last - c_first; ++s) ri += P.part_im[(size_t)s * stride + idx];
+      CompSum ci(P.part_im[idx]);
+      for (int s = 1; s <= c_last - c_first; ++s) ci.add(P.part_im[(size_t)s * stride + idx]);
+      ri = ci.value();
     }
     P.out_im[idx] = P.prefactor * P.T * ri;
   }

@@ -202,3 +202,24 @@ def test_matsubara_n_max_domains(lib):
     for T in inputs.CONFIG1_TEMPERATURES:
         assert inputs.config1(T)["n_max"] == B.dfrg_matsubara_n_max(B.DOMAIN_X0, T, 1.0, 6.0)
     assert inputs.config4()["n_max"] == B.dfrg_matsubara_n_max(B.DOMAIN_X0, 0.15, 1.0, 10.0)
+
+
+def test_constant_tables_are_what_the_generator_writes():
+    """csrc/fm_tables.inc (the constants of the device log / exp) is generated: regenerate and compare, and check two entries
+    against closed forms (mpmath)."""
+    import subprocess
+    import sys
+    import mpmath as mp
+    gen = os.path.join(ROOT, "paper_2412_13043_b200", "csrc", "gen_fm_tables.py")
+    assert subprocess.run([sys.executable, gen, "--check"]).returncode == 0
+    txt = open(os.path.join(ROOT, "paper_2412_13043_b200", "csrc", "fm_tables.inc")).read()
+    body = txt.split("kFmExp[64] = {")[1].split("}")[0]
+    vals = [float.fromhex(t.strip()) for t in body.split(",") if t.strip()]
+    mp.mp.dps = 40
+    assert len(vals) == 64 and vals[0] == 1.0 and vals[32] == float(mp.sqrt(2))
+    body = txt.split("kLg2Log[1024] = {")[1].split("}")[0]
+    vals = [float.fromhex(t.strip()) for t in body.split(",") if t.strip()]
+    assert len(vals) == 1024
+    for j in (0, 255, 511):
+        inv = 1.0 / (1.0 + (j + 0.5) / 512.0)
+        assert vals[2 * j] == inv and vals[2 * j + 1] == float(mp.log(mp.mpf(inv)))
