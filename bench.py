@@ -207,6 +207,16 @@ def time_other_configs(torch, B, inputs, make_rules, peak, iters=5):
             msg = timeit(graph.replay, reps=20)
             out["cfg1_cuda_graph"] = {"ms": msg, "evals_per_s": evals / msg * 1e3, "integrals_per_s": integrals / msg * 1e3,
                                       "launches": len(calls)}
+            # ... and as ONE launch through dfrg_integrate_lpa_batch (grid.y = temperature)
+            c0 = calls[0][0]
+            fb = torch.empty(len(calls), calls[0][2].numel(), dtype=torch.float64, device="cuda")
+            msb = timeit(lambda: B.dfrg_integrate_lpa_batch(c0["d"], [cc[0]["T"] for cc in calls], [cc[0]["n_max"] for cc in calls],
+                                                            c0["reg_arg4d"], c0["N"], c0["prefactor"], c0["reg_kind"],
+                                                            c0["reg_order"], c0["k"], calls[0][1], calls[0][2], calls[0][3],
+                                                            calls[0][4], fb), reps=20)
+            assert all(torch.equal(fb[t_], calls[t_][5]) for t_ in range(len(calls)))
+            out["cfg1_batched"] = {"ms": msb, "evals_per_s": evals / msb * 1e3, "integrals_per_s": integrals / msb * 1e3,
+                                   "launches": 1}
     # cfg2
     c = inputs.config2()
     R = make_rules(c, B.dfrg_quad_nodes)
@@ -466,9 +476,10 @@ def main():
                          "peak_kind": "nominal FP64: %d SMs x %d lanes x 2 x %.0f MHz (MEASURED_PEAKS.json has no FP64 "
                                       "entry)" % (sms, FP64_LANES_PER_SM, sm_max_mhz),
                          "peak_probe_tflops": probe_tflops, "frac_of_probe": achieved / probe_tflops,
-                         "issue_model_probe": dict(issue_model, kind="time of 8 DFMA chains + K integer adds per 8 DFMA, "
-                                                   "K = 0, 4, 8; ratios (16 + K)/16 would mean an FP64 instruction holds the issue port for 2 cycles, ratios of 1 "
-                                                   "that other instructions issue in its shadow (bound = the FP64 pipe)"),
+                         "issue_model_probe": dict(issue_model, kind="time of 8 DFMA chains + K instructions of another pipe per 8 DFMA "
+                                                   "(integer add, I2F.F64, LDS.128) relative to K = 0; integer-add ratios "
+                                                   "(16 + K)/16 would mean an FP64 instruction holds the issue port for 2 "
+                                                   "cycles, ratios of 1 that other instructions issue in its shadow"),
                          "alg_flops_per_launch": flops},
             "wall_s_timed_region": t_wall}
 

@@ -170,6 +170,14 @@ int dfrg_integrate_lpa(const dfrg_lpa_desc* D, int n_field, const double* rho, c
                        double* flow, double* chan, double* dmin, void* cuda_stream);
 int dfrg_integrate_lpa_host(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u,
                             const double* du, double* flow, double* chan, double* dmin);
+/* Several temperatures in ONE launch (BASELINE.json config 1 runs T in {0.05, 0.1, 0.2, 0.5} k on the same field grid):
+ * the integrals of dfrg_integrate_lpa with D->T, D->n_max replaced by T_host[t], n_max_host[t] for t < n_T (HOST arrays,
+ * read before the call returns; 1 <= n_T <= 16, else DFRG_EUNSUPPORTED; every entry must satisfy the limits above).
+ * Outputs gain a leading axis: flow [n_T][n_field]; chan, D->dchan (nullable) [n_T][2][n_field]; dmin (nullable)
+ * [n_T][n_field].  Entry t is bit-identical to a single call at (T_host[t], n_max_host[t]).  Device pointers, asynchronous. */
+int dfrg_integrate_lpa_batch(const dfrg_lpa_desc* D, int n_T, const double* T_host, const int* n_max_host, int n_field,
+                             const double* rho, const double* u, const double* du, double* flow, double* chan,
+                             double* dmin, void* cuda_stream);
 
 /* ---- 4-D vacuum loops (BASELINE.json configs 2 and 3; angles cos1, cos2, phi of PAPER.md:1837-1840) ------
  * DFRG_LOOP_TWOPOINT (tab[0] = Z, n_coef = 2, axes q, cos1; cos2/phi unused, their measure is in prefactor):

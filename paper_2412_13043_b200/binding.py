@@ -24,7 +24,7 @@ RULE_GAUSS_LEGENDRE = 0
 EXPORTS = (
     "dfrg_strerror", "dfrg_last_cuda_error", "dfrg_version", "dfrg_shutdown", "dfrg_quad_nodes",
     "dfrg_matsubara_n_max",
-    "dfrg_integrate_lpa", "dfrg_integrate_lpa_host",
+    "dfrg_integrate_lpa", "dfrg_integrate_lpa_host", "dfrg_integrate_lpa_batch",
     "dfrg_integrate_loop4d", "dfrg_integrate_loop4d_host",
     "dfrg_integrate_matsubara3d", "dfrg_integrate_matsubara3d_host",
 )
@@ -97,6 +97,8 @@ def lib():
         L.dfrg_quad_nodes.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, _vp, _vp]
         L.dfrg_integrate_lpa.argtypes = [C.POINTER(LpaDesc), C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
         L.dfrg_integrate_lpa_host.argtypes = [C.POINTER(LpaDesc), C.c_int, _vp, _vp, _vp, _vp, _vp, _vp]
+        L.dfrg_integrate_lpa_batch.argtypes = [C.POINTER(LpaDesc), C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_int,
+                                               _vp, _vp, _vp, _vp, _vp, _vp, _vp]
         L.dfrg_integrate_loop4d.argtypes = [C.POINTER(Loop4dDesc), C.c_int, _vp, C.c_int, _vp, _vp, _vp, _vp]
         L.dfrg_integrate_loop4d_host.argtypes = [C.POINTER(Loop4dDesc), C.c_int, _vp, C.c_int, _vp, _vp, _vp]
         L.dfrg_integrate_matsubara3d.argtypes = [C.POINTER(Mats3dDesc), C.c_int, _vp, _vp, C.c_int, _vp, C.c_int,
@@ -184,6 +186,22 @@ def dfrg_integrate_lpa(d, T, n_max, reg_arg4d, N, prefactor, reg_kind, reg_order
     _check(lib().dfrg_integrate_lpa(C.byref(D), int(rho.numel()), _ptr(rho, True), _ptr(u, True), _ptr(du, True),
                                     _ptr(flow, True), _ptr(chan, True), _ptr(dmin, True), _stream()),
            "dfrg_integrate_lpa")
+    return flow
+
+
+def dfrg_integrate_lpa_batch(d, Ts, n_maxs, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, rho, u, du,
+                             flow, chan=None, dmin=None, dchan=None, reg_zk=1.0, reg_eta=0.0, statistics=STAT_BOSON, mu=0.0,
+                             fermion_reg=0):
+    """Several temperatures in one launch: flow [n_T, n_field], chan / dchan [n_T, 2, n_field], dmin [n_T, n_field]."""
+    n_T = len(Ts)
+    assert len(n_maxs) == n_T
+    D = _lpa_desc(d, 0.0, 0, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, True, dchan, reg_zk, reg_eta, statistics,
+                  mu, fermion_reg)
+    Tv = (C.c_double * n_T)(*[float(t) for t in Ts])
+    nv = (C.c_int * n_T)(*[int(n) for n in n_maxs])
+    _check(lib().dfrg_integrate_lpa_batch(C.byref(D), n_T, Tv, nv, int(rho.numel()), _ptr(rho, True), _ptr(u, True),
+                                          _ptr(du, True), _ptr(flow, True), _ptr(chan, True), _ptr(dmin, True), _stream()),
+           "dfrg_integrate_lpa_batch")
     return flow
 
 

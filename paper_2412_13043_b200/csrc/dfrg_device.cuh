@@ -544,6 +544,27 @@ struct StageList {
   }
 };
 
+// stage_issue + stage_wait = stage_to_smem; work placed between the two overlaps the copies' flight time.
+__device__ __forceinline__ void stage_issue(const StageList& L, uint64_t* bar) {
+  // bar must have been initialised (count 1) and fenced before the first call
+  if (threadIdx.x == 0) {
+    uint32_t total = 0;
+    for (int a = 0; a < L.count; ++a)
+      if (tma_ok(L.src[a], (size_t)L.n[a] * 8) && tma_ok(L.dst[a], 16)) total += (uint32_t)L.n[a] * 8u;
+    mbar_expect_tx(bar, total);
+    for (int a = 0; a < L.count; ++a)
+      if (tma_ok(L.src[a], (size_t)L.n[a] * 8) && tma_ok(L.dst[a], 16))
+        tma_bulk_g2s(L.dst[a], L.src[a], (uint32_t)L.n[a] * 8u, bar);
+  }
+  for (int a = 0; a < L.count; ++a) {
+    if (!(tma_ok(L.src[a], (size_t)L.n[a] * 8) && tma_ok(L.dst[a], 16)))
+      for (int i = threadIdx.x; i < L.n[a]; i += blockDim.x) L.dst[a][i] = L.src[a][i];
+  }
+}
+__device__ __forceinline__ void stage_wait(uint64_t* bar, uint32_t parity) {
+  mbar_wait(bar, parity);
+  __syncthreads();
+}
 __device__ __forceinline__ void stage_to_smem(const StageList& L, uint64_t* bar, uint32_t parity) {
   // bar must have been initialised (count 1) and fenced before the first call
   if (threadIdx.x == 0) {
@@ -588,7 +609,7 @@ __device__ __forceinline__ double block_sum(double v, double* scratch) {
 }
 // Compensated sum of the per-CTA partial sums of an output (fix-up kernels).  north_star asks for Kahan-compensated partial
 // sums "where ncu shows it is free": it is free here -- a fix-up kernel adds <= a handful of slots per output and waits on its
-// loads -- and nowhere else: the hot loops are bound by FP64 issue slots ("Kahan"), where a compensated
+// loads -- and nowhere else: the hot loops are bound by the FP64 pipe ("Kahan"), where a compensated
 // add costs three more FP64 instructions per term.  Neumaier's variant (the correction also covers |x| > |sum|); deterministic.
 struct CompSum {
   double s, c;

@@ -100,38 +100,32 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
   L.add(sxq, P.xq, nq); L.add(swq, P.wq, nq);
   L.add(sxc, P.xc, nc); L.add(swc, P.wc, nc);
   L.add(sZ, P.Z, nt);
-  const FastMath fm = fm_build(fmmem, P.fmc);
-  stage_to_smem(L, &bar, 0);
+  stage_issue(L, &bar);
+  const FastMath fm = fm_build(fmmem, P.fmc);   // (its loads fly with the bulk copies)
+  stage_wait(&bar, 0);
   cells_build(cZ, sZ, P.grid);
-  __syncthreads();
-  const double inf = __longlong_as_double(0x7ff0000000000000LL);
-  {
-    double dq = inf;
-    for (int i = tid; i < nq; i += TP_THREADS) {
-      const double q = sxq[i], s = q * q;
-      double R, Rd;
-      regulator(P.reg, fm, s, R, Rd);
-      const double D0 = table_lookup(cZ, P.grid, fm, s) * s + R;
-      souter[i] = make_double2(D0, swq[i] * q * q * q * Rd);
-      dq = fmin(dq, D0);
-    }
-    for (int j = tid; j < nc; j += TP_THREADS) {
-      const double c = sxc[j];
-      swc[j] *= sqrt((1.0 - c) * (1.0 + c));
-    }
-    dq = block_min(dq, red);  // also publishes souter and swc
-    if (blockIdx.x == 0 && tid == 0) P.chunkmin[(size_t)n_ftiles * P.n_ext * NCH * (TP_NPROD / 32)] = dq;
+  for (int j = tid; j < nc; j += TP_THREADS) {
+    const double c = sxc[j];
+    swc[j] *= sqrt((1.0 - c) * (1.0 + c));
   }
+  __syncthreads();   // the producers start on their first chunk from here; the consumers build souter meanwhile
+  const double inf = __longlong_as_double(0x7ff0000000000000LL);
+  // unit u = (ft, e, ch); advanced without divisions
+  int ft_u = (int)(u0 / upp);
+  int e_u = (int)((u0 - (long long)ft_u * upp) / NCH);
+  int ch_u = (int)(u0 - (long long)ft_u * upp - (long long)e_u * NCH);
+  auto next_unit = [&]() {
+    if (++ch_u == NCH) { ch_u = 0; if (++e_u == P.n_ext) { e_u = 0; ++ft_u; } }
+  };
 
   if (tid >= TP_NCONS) {
     // =========================== producers ===========================
     const int ptid = tid - TP_NCONS, lane = ptid & 31, pw = ptid >> 5;
     const double coef0 = P.coef[0], coef1 = P.coef[1];
     uint32_t g = 0;
-    for (long long u = u0; u < u1; ++u, ++g) {
+    for (long long u = u0; u < u1; ++u, ++g, next_unit()) {
       const int b = g & 1;
-      const long long rem = u % upp;
-      const int e = (int)(rem / NCH), ch = (int)(rem - (long long)e * NCH);
+      const int e = e_u, ch = ch_u;
       const int i0 = ch * QC;
       const int ni = min(QC, nq - i0);
       const double p = P.pext[e];
@@ -161,15 +155,33 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
   }
 
   // =============================== consumers ===============================
+  {
+    // outer[i] = (Z(q^2) q^2 + R(q^2), wq q^3 Rdot(q^2)) and its minimum (for dmin), by the consumers while the
+    // producers are on the first chunk; published among the consumers by a named barrier
+    double dq = inf;
+    for (int i = tid; i < nq; i += TP_NCONS) {
+      const double q = sxq[i], s = q * q;
+      double R, Rd;
+      regulator(P.reg, fm, s, R, Rd);
+      const double D0 = table_lookup(cZ, P.grid, fm, s) * s + R;
+      souter[i] = make_double2(D0, swq[i] * q * q * q * Rd);
+      dq = fmin(dq, D0);
+    }
+    dq = warp_min(dq);
+    if ((tid & 31) == 0) red[tid >> 5] = dq;
+    named_bar_sync(1, TP_NCONS);
+    if (blockIdx.x == 0 && tid == 0) {
+      for (int w = 1; w < TP_NCONS / 32; ++w) dq = fmin(dq, red[w]);
+      P.chunkmin[(size_t)n_ftiles * P.n_ext * NCH * (TP_NPROD / 32)] = dq;
+    }
+  }
   const int grp = tid / TP_FT, tf = tid - grp * TP_FT;
   const bool warp_leader = (tid & 31) == 0;
   double m2[MF], acc[MF], dacc[MF];
   int cur_ft = -1, seg_parity = 0;
   uint32_t g = 0;
-  for (long long u = u0; u < u1; ++u, ++g) {
-    const int ft = (int)(u / upp);
-    const long long rem = u - (long long)ft * upp;
-    const int e = (int)(rem / NCH), ch = (int)(rem - (long long)e * NCH);
+  for (long long u = u0; u < u1; ++u, ++g, next_unit()) {
+    const int ft = ft_u, e = e_u, ch = ch_u;
     const int f0 = ft * tile + tf;
     const int b = g & 1;
     if (ft != cur_ft) {

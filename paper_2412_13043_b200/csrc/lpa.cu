@@ -18,10 +18,13 @@ constexpr int LPA_THREADS = 256;   // 8 warps: 2 channels x 4 node slices
 constexpr int LPA_SLICES = 4;
 constexpr int LPA_FTILE = 32;
 constexpr int LPA_MAX_PAIRS = 12288;
+constexpr int LPA_MAX_T = 16;      // temperatures per launch (dfrg_integrate_lpa_batch)
 
 struct LpaParams {
-  int d, n_max, reg_arg4d, nq, n_field, fermion_reg;
-  double T, N, prefactor, mu;
+  int d, reg_arg4d, nq, n_field, fermion_reg;
+  double N, prefactor, mu;
+  double Tv[LPA_MAX_T];     // temperature of batch entry blockIdx.y (a single call is a batch of one)
+  int nmaxv[LPA_MAX_T];     // its Matsubara cut-off
   RegParams reg;
   FastMathConsts fmc;
   const double *xq, *wq, *rho, *u, *du;
@@ -37,7 +40,9 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_kernel(const LpaParams P) {
   __shared__ double part[2][LPA_SLICES][LPA_FTILE];
   __shared__ double dpart[WANT_D ? 2 : 1][LPA_SLICES][LPA_FTILE];
 
-  const int n_terms = (P.T > 0.0) ? P.n_max + 1 : 1;
+  const int it = blockIdx.y;                      // batch entry: its own (T, n_max) and output planes
+  const double T = P.Tv[it];
+  const int n_terms = (T > 0.0) ? P.nmaxv[it] + 1 : 1;
   const int n_pairs = n_terms * P.nq;
   double2* tab = reinterpret_cast<double2*>(smem_raw);                 // [n_pairs] (D0, W)
   double* sx = reinterpret_cast<double*>(smem_raw + (size_t)n_pairs * 16);  // [nq]
@@ -52,7 +57,7 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_kernel(const LpaParams P) {
   stage_to_smem(L, &bar, 0);
 
   // ---- S3: field-independent table ----
-  const double two_pi_T = 2.0 * 3.14159265358979323846 * P.T;
+  const double two_pi_T = 2.0 * 3.14159265358979323846 * T;
   double dmin0 = __longlong_as_double(0x7ff0000000000000LL);
   for (int t = threadIdx.x; t < n_pairs; t += LPA_THREADS) {
     const int n = t / P.nq, i = t - n * P.nq;
@@ -117,18 +122,19 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_kernel(const LpaParams P) {
 
   // ---- S5/S6 ----
   if (wid == 0 && live) {
-    const double scale = (P.T > 0.0) ? P.prefactor * P.T : P.prefactor;
+    const double scale = (T > 0.0) ? P.prefactor * T : P.prefactor;
+    const size_t o1 = (size_t)it * P.n_field, o2 = 2 * o1;
     double I[2];
 #pragma unroll
     for (int c = 0; c < 2; ++c)
       I[c] = scale * ((part[c][0][lane] + part[c][1][lane]) + (part[c][2][lane] + part[c][3][lane]));
-    P.flow[f] = (P.N - 1.0) * I[0] + I[1];
-    if (P.chan) { P.chan[f] = I[0]; P.chan[P.n_field + f] = I[1]; }
-    if (P.dmin) P.dmin[f] = fmin(dmin0 + m2pi, dmin0 + m2sig) * P.reg.inv_k2;
+    P.flow[o1 + f] = (P.N - 1.0) * I[0] + I[1];
+    if (P.chan) { P.chan[o2 + f] = I[0]; P.chan[o2 + P.n_field + f] = I[1]; }
+    if (P.dmin) P.dmin[o1 + f] = fmin(dmin0 + m2pi, dmin0 + m2sig) * P.reg.inv_k2;
     if constexpr (WANT_D) {
 #pragma unroll
       for (int c = 0; c < 2; ++c)
-        P.dchan[c * P.n_field + f] =
+        P.dchan[o2 + c * P.n_field + f] =
             -scale * ((dpart[c][0][lane] + dpart[c][1][lane]) + (dpart[c][2][lane] + dpart[c][3][lane]));
     }
   }
@@ -147,7 +153,9 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_fermion_kernel(const LpaParam
   __shared__ double dpart[2][LPA_SLICES][LPA_FTILE];
   __shared__ double mpart[2][LPA_SLICES][LPA_FTILE];
 
-  const int n_pairs = (P.n_max + 1) * P.nq;
+  const int it = blockIdx.y;
+  const double T = P.Tv[it];
+  const int n_pairs = (P.nmaxv[it] + 1) * P.nq;
   double4* tab = reinterpret_cast<double4*>(smem_raw);                      // [n_pairs] (a0, W, b^2, -)
   double* sx = reinterpret_cast<double*>(smem_raw + (size_t)n_pairs * 32);  // [nq]
   double* sw = sx + ((P.nq + 1) & ~1);
@@ -160,7 +168,7 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_fermion_kernel(const LpaParam
   L.add(sw, P.wq, P.nq);
   stage_to_smem(L, &bar, 0);
 
-  const double pi_T = 3.14159265358979323846 * P.T;
+  const double pi_T = 3.14159265358979323846 * T;
   for (int t = threadIdx.x; t < n_pairs; t += LPA_THREADS) {
     const int n = t / P.nq, i = t - n * P.nq;
     const double q = sx[i];
@@ -202,25 +210,26 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_fermion_kernel(const LpaParam
   mpart[ch][slice][lane] = den_min;
   __syncthreads();
   if (wid == 0 && live) {
-    const double scale = P.prefactor * P.T;
+    const double scale = P.prefactor * T;
+    const size_t o1 = (size_t)it * P.n_field, o2 = 2 * o1;
     double I[2];
 #pragma unroll
     for (int c = 0; c < 2; ++c)
       I[c] = scale * ((part[c][0][lane] + part[c][1][lane]) + (part[c][2][lane] + part[c][3][lane]));
-    P.flow[f] = (P.N - 1.0) * I[0] + I[1];
-    if (P.chan) { P.chan[f] = I[0]; P.chan[P.n_field + f] = I[1]; }
+    P.flow[o1 + f] = (P.N - 1.0) * I[0] + I[1];
+    if (P.chan) { P.chan[o2 + f] = I[0]; P.chan[o2 + P.n_field + f] = I[1]; }
     if (want_dmin) {
       double dm = mpart[0][0][lane];
 #pragma unroll
       for (int c = 0; c < 2; ++c)
 #pragma unroll
         for (int sl = 0; sl < LPA_SLICES; ++sl) dm = fmin(dm, mpart[c][sl][lane]);
-      P.dmin[f] = sqrt(dm) * P.reg.inv_k2;
+      P.dmin[o1 + f] = sqrt(dm) * P.reg.inv_k2;
     }
     if constexpr (WANT_D) {
 #pragma unroll
       for (int c = 0; c < 2; ++c)
-        P.dchan[c * P.n_field + f] =
+        P.dchan[o2 + c * P.n_field + f] =
             -scale * ((dpart[c][0][lane] + dpart[c][1][lane]) + (dpart[c][2][lane] + dpart[c][3][lane]));
     }
   }
@@ -233,24 +242,35 @@ static size_t lpa_smem(const dfrg_lpa_desc* D) {
   return n_terms * D->q.n * (fermi ? 32 : 16) + (2 * (size_t)((D->q.n + 1) & ~1) + FM_DOUBLES) * 8;
 }
 
-static int lpa_launch(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u, const double* du,
-                      double* flow, double* chan, double* dmin, cudaStream_t stream) {
+// n_T batch entries (Tv, nmaxv; a single call is a batch of one): grid.y = n_T, outputs with a leading [n_T] axis
+static int lpa_launch(const dfrg_lpa_desc* D, int n_T, const double* Tv, const int* nmaxv, int n_field, const double* rho,
+                      const double* u, const double* du, double* flow, double* chan, double* dmin, cudaStream_t stream) {
   LpaParams P;
-  P.d = D->d; P.n_max = D->n_max; P.reg_arg4d = D->reg_arg4d; P.nq = D->q.n; P.n_field = n_field;
+  P.d = D->d; P.reg_arg4d = D->reg_arg4d; P.nq = D->q.n; P.n_field = n_field;
   P.fermion_reg = D->fermion_reg;
-  P.T = D->T; P.N = D->N; P.prefactor = D->prefactor; P.mu = D->mu;
+  P.N = D->N; P.prefactor = D->prefactor; P.mu = D->mu;
+  size_t smem = 0;
+  for (int t = 0; t < LPA_MAX_T; ++t) {
+    P.Tv[t] = t < n_T ? Tv[t] : 0.0;
+    P.nmaxv[t] = t < n_T ? nmaxv[t] : 0;
+    if (t < n_T) {
+      dfrg_lpa_desc Dt = *D;
+      Dt.T = Tv[t]; Dt.n_max = nmaxv[t];
+      const size_t st = lpa_smem(&Dt);
+      smem = st > smem ? st : smem;
+    }
+  }
   P.reg = reg_params(D->reg.kind, D->reg.order, D->reg.k, D->reg.zk, D->reg.eta);
   P.fmc = fm_consts();
   P.xq = D->q.x; P.wq = D->q.w; P.rho = rho; P.u = u; P.du = du;
   P.flow = flow; P.chan = chan; P.dmin = dmin; P.dchan = D->dchan;
   const bool fermi = D->statistics == DFRG_STAT_FERMION;
-  const size_t smem = lpa_smem(D);
   auto kern = fermi ? (D->dchan ? lpa_fermion_kernel<true> : lpa_fermion_kernel<false>)
                     : (D->dchan ? lpa_kernel<true> : lpa_kernel<false>);
   if (smem > kMaxDynSmem) return DFRG_EUNSUPPORTED;   // (lpa_validate bounds the table; this is the exact size)
   const int rca = opt_in_max_smem(kern);
   if (rca != DFRG_OK) return rca;
-  const int grid = (n_field + LPA_FTILE - 1) / LPA_FTILE;
+  const dim3 grid((n_field + LPA_FTILE - 1) / LPA_FTILE, n_T);
   kern<<<grid, LPA_THREADS, smem, stream>>>(P);
   return check_cuda(cudaGetLastError());
 }
@@ -276,9 +296,32 @@ static int lpa_validate(const dfrg_lpa_desc* D, int n_field, const double* rho, 
   return DFRG_OK;
 }
 
+static int lpa_validate_batch(const dfrg_lpa_desc* D, int n_T, const double* T, const int* n_max, int n_field,
+                              const double* rho, const double* u, const double* du, double* flow) {
+  if (!D || !T || !n_max || n_T < 1) return DFRG_EINVAL;
+  if (n_T > LPA_MAX_T) return DFRG_EUNSUPPORTED;
+  for (int t = 0; t < n_T; ++t) {
+    dfrg_lpa_desc Dt = *D;
+    Dt.T = T[t]; Dt.n_max = n_max[t];
+    const int rc = lpa_validate(&Dt, n_field, rho, u, du, flow);
+    if (rc != DFRG_OK) return rc;
+  }
+  return DFRG_OK;
+}
+
 }  // namespace dfrg
 
 using namespace dfrg;
+
+extern "C" int dfrg_integrate_lpa_batch(const dfrg_lpa_desc* D, int n_T, const double* T_host, const int* n_max_host,
+                                        int n_field, const double* rho, const double* u, const double* du, double* flow,
+                                        double* chan, double* dmin, void* cuda_stream) {
+  int rc = lpa_validate_batch(D, n_T, T_host, n_max_host, n_field, rho, u, du, flow);
+  if (rc != DFRG_OK) return rc;
+  rc = require_sm100(nullptr);
+  if (rc != DFRG_OK) return rc;
+  return lpa_launch(D, n_T, T_host, n_max_host, n_field, rho, u, du, flow, chan, dmin, (cudaStream_t)cuda_stream);
+}
 
 extern "C" int dfrg_integrate_lpa(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u,
                                   const double* du, double* flow, double* chan, double* dmin, void* cuda_stream) {
@@ -286,7 +329,7 @@ extern "C" int dfrg_integrate_lpa(const dfrg_lpa_desc* D, int n_field, const dou
   if (rc != DFRG_OK) return rc;
   rc = require_sm100(nullptr);
   if (rc != DFRG_OK) return rc;
-  return lpa_launch(D, n_field, rho, u, du, flow, chan, dmin, (cudaStream_t)cuda_stream);
+  return lpa_launch(D, 1, &D->T, &D->n_max, n_field, rho, u, du, flow, chan, dmin, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int dfrg_integrate_lpa_host(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u,
@@ -310,7 +353,7 @@ extern "C" int dfrg_integrate_lpa_host(const dfrg_lpa_desc* D, int n_field, cons
   double* d_dmin = dmin ? A.reserve(nf) : nullptr;
   Dd.dchan = D->dchan ? A.reserve(2 * nf) : nullptr;
   if (A.upload() != DFRG_OK) return A.status();
-  rc = lpa_launch(&Dd, n_field, d_rho, d_u, d_du, d_flow, d_chan, d_dmin, A.stream());
+  rc = lpa_launch(&Dd, 1, &Dd.T, &Dd.n_max, n_field, d_rho, d_u, d_du, d_flow, d_chan, d_dmin, A.stream());
   if (rc != DFRG_OK) return rc;
   A.fetch(flow, d_flow, nf);
   if (chan) A.fetch(chan, d_chan, 2 * nf);

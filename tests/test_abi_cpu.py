@@ -108,6 +108,17 @@ def test_integrators_validate_before_touching_the_device(lib):
     assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
     bad = B.LpaDesc(9, 0.0, 0, 1, 4.0, 1.0, reg, rule)
     assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EUNSUPPORTED
+    # batched temperatures: host arrays, 1 <= n_T <= 16, every entry validated like a single call
+    fb = lib.dfrg_integrate_lpa_batch
+    Tv, nv = (C.c_double * 17)(*([0.1] * 17)), (C.c_int * 17)(*([3] * 17))
+    Db = B.LpaDesc(3, 0.0, 0, 1, 4.0, 1.0, reg, rule)
+    assert fb(C.byref(Db), 0, Tv, nv, 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
+    assert fb(C.byref(Db), 2, None, nv, 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
+    assert fb(C.byref(Db), 17, Tv, nv, 4, p, p, p, p, None, None, None) == B.DFRG_EUNSUPPORTED
+    Tv[1] = -0.5
+    assert fb(C.byref(Db), 2, Tv, nv, 4, p, p, p, p, None, None, None) == B.DFRG_EINVAL
+    Tv[1], nv[1] = 0.1, 100000
+    assert fb(C.byref(Db), 2, Tv, nv, 4, p, p, p, p, None, None, None) == B.DFRG_EUNSUPPORTED
     bad = B.LpaDesc(3, 0.1, 4000, 1, 4.0, 1.0, reg, rule)
     assert f(C.byref(bad), 4, p, p, p, p, None, None, None) == B.DFRG_EUNSUPPORTED
 

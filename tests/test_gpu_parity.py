@@ -295,3 +295,29 @@ def test_runs_on_a_side_stream():
     with torch.cuda.stream(s):
         out = gpu_run(c, R)["out"]
     assert np.array_equal(ref, out)
+
+
+def test_lpa_batched_temperatures_are_the_single_calls():
+    """dfrg_integrate_lpa_batch: the four temperatures of BASELINE config 1 in one launch, bit-identical to four calls
+    (which test_lpa_full_config0_and_config1 compares with the oracle); fermionic statistics with the fermionic regulator too."""
+    import torch
+    from paper_2412_13043_b200 import binding as B
+    up = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+    for fermi in (False, True):
+        cs = [inputs.config1(T, n_field=1000) for T in inputs.CONFIG1_TEMPERATURES]
+        c0 = cs[0]
+        xq, wq = B.dfrg_quad_nodes(*c0["rule_q"])
+        rq = (up(xq), up(wq))
+        rho, u, du = up(c0["rho"]), up(c0["u"]), up(c0["du"])
+        nf, nT = rho.numel(), len(cs)
+        kw = dict(statistics=B.STAT_FERMION, mu=0.3, fermion_reg=1, reg_zk=1.2, reg_eta=0.1) if fermi else {}
+        arg4d = 0 if fermi else c0["reg_arg4d"]
+        new = lambda *s: torch.full(s, float("nan"), dtype=torch.float64, device="cuda")
+        flow, chan, dmin, dchan = new(nT, nf), new(nT, 2, nf), new(nT, nf), new(nT, 2, nf)
+        B.dfrg_integrate_lpa_batch(c0["d"], [c["T"] for c in cs], [c["n_max"] for c in cs], arg4d, c0["N"], c0["prefactor"],
+                                   c0["reg_kind"], c0["reg_order"], c0["k"], rq, rho, u, du, flow, chan, dmin, dchan=dchan, **kw)
+        for t, c in enumerate(cs):
+            f1, c1, d1, dc1 = new(nf), new(2, nf), new(nf), new(2, nf)
+            B.dfrg_integrate_lpa(c["d"], c["T"], c["n_max"], arg4d, c["N"], c["prefactor"], c["reg_kind"], c["reg_order"],
+                                 c["k"], rq, rho, u, du, f1, c1, d1, dchan=dc1, **kw)
+            assert torch.equal(flow[t], f1) and torch.equal(chan[t], c1) and torch.equal(dmin[t], d1) and torch.equal(dchan[t], dc1)
