@@ -90,6 +90,11 @@ __device__ __forceinline__ FastMath fm_build(double* mem, const FastMathConsts& 
   return fm;
 }
 
+// The same tables through a stage list (TMA bulk copies from the constant arrays: no instructions in the CTA's set-up).
+// Declared after StageList below; mem: FM_DOUBLES doubles, 16-byte aligned.
+struct StageList;
+__device__ __forceinline__ FastMath fm_stage(StageList& L, double* mem, const FastMathConsts& consts);
+
 __device__ __forceinline__ double fm_log(const FastMath& fm, double s) {
   const int hi = __double2hiint(s);
   const int e = (hi >> 20) - 1023;
@@ -544,20 +549,40 @@ struct StageList {
   }
 };
 
+__device__ __forceinline__ FastMath fm_stage(StageList& L, double* mem, const FastMathConsts& consts) {
+  L.add(mem, kFmLog, 256);
+  L.add(mem + 256, kFmExp, 64);
+  FastMath fm;
+  fm.logtab = reinterpret_cast<const double2*>(mem);
+  fm.exptab = mem + 256;
+  fm.k = consts.c;
+  return fm;
+}
+
 // stage_issue + stage_wait = stage_to_smem; work placed between the two overlaps the copies' flight time.
+// (The loops over the list are fully unrolled so that the list lives in registers: with run-time indices it sits in local
+// memory and thread 0 spends ~3000 cycles walking it.  Copy a is issued by lane 0 of warp a mod n_warps: a bulk-copy
+// instruction takes ~200 cycles to issue, five of them in one thread cost a microsecond at the head of a short kernel.  The
+// barrier cannot complete before thread 0's arrive.expect_tx, whatever the order in which the copies' complete_tx land.)
 __device__ __forceinline__ void stage_issue(const StageList& L, uint64_t* bar) {
   // bar must have been initialised (count 1) and fenced before the first call
-  if (threadIdx.x == 0) {
-    uint32_t total = 0;
-    for (int a = 0; a < L.count; ++a)
-      if (tma_ok(L.src[a], (size_t)L.n[a] * 8) && tma_ok(L.dst[a], 16)) total += (uint32_t)L.n[a] * 8u;
-    mbar_expect_tx(bar, total);
-    for (int a = 0; a < L.count; ++a)
-      if (tma_ok(L.src[a], (size_t)L.n[a] * 8) && tma_ok(L.dst[a], 16))
+  const int warp = threadIdx.x >> 5, n_warps = (blockDim.x + 31) >> 5;
+  if ((threadIdx.x & 31) == 0) {
+    if (threadIdx.x == 0) {
+      uint32_t total = 0;
+#pragma unroll
+      for (int a = 0; a < 8; ++a)
+        if (a < L.count && tma_ok(L.src[a], (size_t)L.n[a] * 8) && tma_ok(L.dst[a], 16)) total += (uint32_t)L.n[a] * 8u;
+      mbar_expect_tx(bar, total);
+    }
+#pragma unroll
+    for (int a = 0; a < 8; ++a)
+      if (a < L.count && warp == a % n_warps && tma_ok(L.src[a], (size_t)L.n[a] * 8) && tma_ok(L.dst[a], 16))
         tma_bulk_g2s(L.dst[a], L.src[a], (uint32_t)L.n[a] * 8u, bar);
   }
-  for (int a = 0; a < L.count; ++a) {
-    if (!(tma_ok(L.src[a], (size_t)L.n[a] * 8) && tma_ok(L.dst[a], 16)))
+#pragma unroll
+  for (int a = 0; a < 8; ++a) {
+    if (a < L.count && !(tma_ok(L.src[a], (size_t)L.n[a] * 8) && tma_ok(L.dst[a], 16)))
       for (int i = threadIdx.x; i < L.n[a]; i += blockDim.x) L.dst[a][i] = L.src[a][i];
   }
 }
@@ -566,22 +591,8 @@ __device__ __forceinline__ void stage_wait(uint64_t* bar, uint32_t parity) {
   __syncthreads();
 }
 __device__ __forceinline__ void stage_to_smem(const StageList& L, uint64_t* bar, uint32_t parity) {
-  // bar must have been initialised (count 1) and fenced before the first call
-  if (threadIdx.x == 0) {
-    uint32_t total = 0;
-    for (int a = 0; a < L.count; ++a)
-      if (tma_ok(L.src[a], (size_t)L.n[a] * 8) && tma_ok(L.dst[a], 16)) total += (uint32_t)L.n[a] * 8u;
-    mbar_expect_tx(bar, total);
-    for (int a = 0; a < L.count; ++a)
-      if (tma_ok(L.src[a], (size_t)L.n[a] * 8) && tma_ok(L.dst[a], 16))
-        tma_bulk_g2s(L.dst[a], L.src[a], (uint32_t)L.n[a] * 8u, bar);
-  }
-  for (int a = 0; a < L.count; ++a) {
-    if (!(tma_ok(L.src[a], (size_t)L.n[a] * 8) && tma_ok(L.dst[a], 16)))
-      for (int i = threadIdx.x; i < L.n[a]; i += blockDim.x) L.dst[a][i] = L.src[a][i];
-  }
-  mbar_wait(bar, parity);
-  __syncthreads();
+  stage_issue(L, bar);
+  stage_wait(bar, parity);
 }
 
 // ---- deterministic reductions ----------------------------------------------------------------------

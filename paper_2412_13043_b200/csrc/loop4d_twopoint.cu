@@ -85,7 +85,14 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
   const int n_ftiles = (P.n_field + tile - 1) / tile;
   const long long upp = (long long)P.n_ext * NCH;                     // units per field tile
   const long long U = (long long)n_ftiles * upp;
-  const long long u0 = (long long)blockIdx.x * U / gridDim.x, u1 = (long long)(blockIdx.x + 1) * U / gridDim.x;
+  long long u0, u1;
+  if ((long long)gridDim.x * U < (1ll << 32)) {   // (32-bit divisions where they suffice: ~300 cycles each otherwise)
+    u0 = (unsigned)(blockIdx.x * (unsigned)U) / gridDim.x;
+    u1 = (unsigned)((blockIdx.x + 1) * (unsigned)U) / gridDim.x;
+  } else {
+    u0 = (long long)blockIdx.x * U / gridDim.x;
+    u1 = (long long)(blockIdx.x + 1) * U / gridDim.x;
+  }
 
   if (tid == 0) {
     mbar_init(&bar, 1);
@@ -100,8 +107,9 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
   L.add(sxq, P.xq, nq); L.add(swq, P.wq, nq);
   L.add(sxc, P.xc, nc); L.add(swc, P.wc, nc);
   L.add(sZ, P.Z, nt);
+  const FastMath fm = fm_stage(L, fmmem, P.fmc);   // the constant log/exp tables travel with the inputs
+  const double coef0 = P.coef[0], coef1 = P.coef[1];   // (producers; loaded here so that the latency hides behind the staging)
   stage_issue(L, &bar);
-  const FastMath fm = fm_build(fmmem, P.fmc);   // (its loads fly with the bulk copies)
   stage_wait(&bar, 0);
   cells_build(cZ, sZ, P.grid);
   for (int j = tid; j < nc; j += TP_THREADS) {
@@ -111,9 +119,18 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
   __syncthreads();   // the producers start on their first chunk from here; the consumers build souter meanwhile
   const double inf = __longlong_as_double(0x7ff0000000000000LL);
   // unit u = (ft, e, ch); advanced without divisions
-  int ft_u = (int)(u0 / upp);
-  int e_u = (int)((u0 - (long long)ft_u * upp) / NCH);
-  int ch_u = (int)(u0 - (long long)ft_u * upp - (long long)e_u * NCH);
+  int ft_u, e_u, ch_u;
+  if (U < (1ll << 31)) {   // (32-bit divisions: the 64-bit ones cost ~1000 cycles at the head of every CTA)
+    const unsigned v = (unsigned)u0, uppu = (unsigned)upp;
+    ft_u = (int)(v / uppu);
+    const unsigned rem = v - (unsigned)ft_u * uppu;
+    e_u = (int)(rem / (unsigned)NCH);
+    ch_u = (int)(rem - (unsigned)e_u * (unsigned)NCH);
+  } else {
+    ft_u = (int)(u0 / upp);
+    e_u = (int)((u0 - (long long)ft_u * upp) / NCH);
+    ch_u = (int)(u0 - (long long)ft_u * upp - (long long)e_u * NCH);
+  }
   auto next_unit = [&]() {
     if (++ch_u == NCH) { ch_u = 0; if (++e_u == P.n_ext) { e_u = 0; ++ft_u; } }
   };
@@ -121,7 +138,6 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
   if (tid >= TP_NCONS) {
     // =========================== producers ===========================
     const int ptid = tid - TP_NCONS, lane = ptid & 31, pw = ptid >> 5;
-    const double coef0 = P.coef[0], coef1 = P.coef[1];
     uint32_t g = 0;
     for (long long u = u0; u < u1; ++u, ++g, next_unit()) {
       const int b = g & 1;
@@ -200,14 +216,8 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
     const double2* chunk = buf + (size_t)b * chunk_nodes;
     const int i0 = ch * QC;
     const int ni = min(QC, nq - i0);
-    for (int il = grp; il < ni; il += TP_GROUPS) {
-      const double2* row = chunk + il * nc;
-      double A[MF], B[MF];
-#pragma unroll
-      for (int k = 0; k < MF; ++k) { A[k] = 0.0; B[k] = 0.0; }
-      int j = 0;
-      for (; j + 4 <= nc; j += 4) tp_batch<MF, WANT_D, 4>(row + j, m2, A, B);
-      for (; j < nc; ++j) tp_batch<MF, WANT_D, 1>(row + j, m2, A, B);
+    // radial node il of the chunk:  acc_f += Wq G(q)^2 A_f
+    auto close_row = [&](const int il, const double (&A)[MF], const double (&B)[MF]) {
       const double2 o = souter[i0 + il];
 #pragma unroll
       for (int k = 0; k < MF; ++k) {
@@ -216,6 +226,37 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
         acc[k] = fma(wg2, A[k], acc[k]);
         if constexpr (WANT_D) dacc[k] = fma(wg2, fma(2.0 * gq, A[k], B[k]), dacc[k]);
       }
+    };
+    int il = grp;
+    // two radial nodes of the group at a time (their angular loops interleaved: the row set-up and the dependent chain that
+    // closes a row overlap with the other row's work); the rows are closed in the order of the single-row loop below
+    for (; il + TP_GROUPS < ni; il += 2 * TP_GROUPS) {
+      const double2* rowa = chunk + il * nc;
+      const double2* rowb = rowa + TP_GROUPS * nc;
+      double Aa[MF], Ba[MF], Ab[MF], Bb[MF];
+#pragma unroll
+      for (int k = 0; k < MF; ++k) { Aa[k] = 0.0; Ba[k] = 0.0; Ab[k] = 0.0; Bb[k] = 0.0; }
+      int j = 0;
+      for (; j + 4 <= nc; j += 4) {
+        tp_batch<MF, WANT_D, 4>(rowa + j, m2, Aa, Ba);
+        tp_batch<MF, WANT_D, 4>(rowb + j, m2, Ab, Bb);
+      }
+      for (; j < nc; ++j) {
+        tp_batch<MF, WANT_D, 1>(rowa + j, m2, Aa, Ba);
+        tp_batch<MF, WANT_D, 1>(rowb + j, m2, Ab, Bb);
+      }
+      close_row(il, Aa, Ba);
+      close_row(il + TP_GROUPS, Ab, Bb);
+    }
+    for (; il < ni; il += TP_GROUPS) {
+      const double2* row = chunk + il * nc;
+      double A[MF], B[MF];
+#pragma unroll
+      for (int k = 0; k < MF; ++k) { A[k] = 0.0; B[k] = 0.0; }
+      int j = 0;
+      for (; j + 4 <= nc; j += 4) tp_batch<MF, WANT_D, 4>(row + j, m2, A, B);
+      for (; j < nc; ++j) tp_batch<MF, WANT_D, 1>(row + j, m2, A, B);
+      close_row(il, A, B);
     }
     __syncwarp();
     if (warp_leader) mbar_arrive(&empty[b]);

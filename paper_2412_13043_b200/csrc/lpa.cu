@@ -47,13 +47,13 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_kernel(const LpaParams P) {
   double2* tab = reinterpret_cast<double2*>(smem_raw);                 // [n_pairs] (D0, W)
   double* sx = reinterpret_cast<double*>(smem_raw + (size_t)n_pairs * 16);  // [nq]
   double* sw = sx + ((P.nq + 1) & ~1);                                      // [nq]
-  const FastMath fm = fm_build(sw + ((P.nq + 1) & ~1), P.fmc);                     // [FM_DOUBLES]
 
   if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
   __syncthreads();
   StageList L;
   L.add(sx, P.xq, P.nq);
   L.add(sw, P.wq, P.nq);
+  const FastMath fm = fm_stage(L, sw + ((P.nq + 1) & ~1), P.fmc);                  // [FM_DOUBLES]
   stage_to_smem(L, &bar, 0);
 
   // ---- S3: field-independent table ----
@@ -159,13 +159,13 @@ __global__ void __launch_bounds__(LPA_THREADS) lpa_fermion_kernel(const LpaParam
   double4* tab = reinterpret_cast<double4*>(smem_raw);                      // [n_pairs] (a0, W, b^2, -)
   double* sx = reinterpret_cast<double*>(smem_raw + (size_t)n_pairs * 32);  // [nq]
   double* sw = sx + ((P.nq + 1) & ~1);
-  const FastMath fm = fm_build(sw + ((P.nq + 1) & ~1), P.fmc);
 
   if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
   __syncthreads();
   StageList L;
   L.add(sx, P.xq, P.nq);
   L.add(sw, P.wq, P.nq);
+  const FastMath fm = fm_stage(L, sw + ((P.nq + 1) & ~1), P.fmc);
   stage_to_smem(L, &bar, 0);
 
   const double pi_T = 3.14159265358979323846 * T;
