@@ -26,7 +26,8 @@ __global__ void __launch_bounds__(512) fp64_peak_kernel(int n_iter, double* sink
 
 // Issue model: the same 8 DFMA chains with K independent instructions of another pipe interleaved per 8 DFMA (volatile
 // inline PTX: one SASS instruction each, never merged or removed):
-//   KIND 0: 32-bit integer add (ALU)        KIND 1: cvt.rn.f64.s32 = I2F.F64 (XU)        KIND 2: 16-byte shared-memory load (LSU)
+//   KIND 0: 32-bit integer add (ALU)      KIND 1: I2F.F64 / F2I.F64 conversions (XU)      KIND 2: 16-byte shared-memory load (LSU)
+//   KIND 3: rcp.approx.ftz.f64 = MUFU.RCP64H (XU)
 // If an FP64 warp instruction held its scheduler's issue port for two cycles, the time would grow as (16 + K)/16 with K
 // integer adds; if the port is free in the second cycle, K <= 8 adds cost nothing.  The XU and LSU variants show whether
 // those pipes run beside the FP64 pipe (ratio 1 while their own throughput is not exceeded) or in turn with it.
@@ -41,13 +42,18 @@ __global__ void __launch_bounds__(512) fp64_issue_kernel(int n_iter, double* sin
   double y[8];
   double2 v[8];
 #pragma unroll
-  for (int i = 0; i < 8; ++i) { x[i] = threadIdx.x + i; y[i] = 0.0; v[i] = make_double2(0.0, 0.0); }
+  for (int i = 0; i < 8; ++i) { x[i] = threadIdx.x + i; y[i] = 1.5 + i; v[i] = make_double2(0.0, 0.0); }
   const unsigned saddr = (unsigned)__cvta_generic_to_shared(sh) + 16u * (threadIdx.x & 7);
   const double m = 0.999999, c = 1e-7;
   auto other = [&](int i) {
-    if (KIND == 0) asm volatile("add.s32 %0, %0, 7;" : "+r"(x[i]));
-    else if (KIND == 1) asm volatile("cvt.rn.f64.s32 %0, %1;" : "=d"(y[i]) : "r"(x[i]));
-    else asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[i].x), "=d"(v[i].y) : "r"(saddr));
+    // (ptxas folds a chain of adds of a constant and hoists a conversion of an unchanged register: every instruction below
+    // depends on the one before it in its own chain, by a value the assembler cannot know)
+    if (KIND == 0) asm volatile("add.s32 %0, %0, %1;" : "+r"(x[i]) : "r"(x[(i + 1) & 7]));
+    else if (KIND == 1) {
+      if (i & 1) asm volatile("cvt.rzi.s32.f64 %0, %1;" : "=r"(x[i >> 1]) : "d"(y[i >> 1]));
+      else asm volatile("cvt.rn.f64.s32 %0, %1;" : "=d"(y[i >> 1]) : "r"(x[i >> 1]));
+    } else if (KIND == 3) asm volatile("rcp.approx.ftz.f64 %0, %0;" : "+d"(y[i]));   // MUFU.RCP64H: y -> 1/y -> y ...
+    else asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[i].x), "=d"(v[i].y) : "r"(saddr));
   };
   for (int it = 0; it < n_iter; ++it) {
 #pragma unroll
@@ -79,8 +85,9 @@ extern "C" int dfrg_probe_fp64_issue(int n_iter, int kind, int k, double* sink, 
   void (*kern)(int, double*) = nullptr;
 #define DFRG_PROBE_PICK(KD, KK) if (kind == KD && k == KK) kern = fp64_issue_kernel<KD, KK>;
   DFRG_PROBE_PICK(0, 0) DFRG_PROBE_PICK(0, 4) DFRG_PROBE_PICK(0, 8)
-  DFRG_PROBE_PICK(1, 1) DFRG_PROBE_PICK(1, 2) DFRG_PROBE_PICK(1, 4)
+  DFRG_PROBE_PICK(1, 2) DFRG_PROBE_PICK(1, 4) DFRG_PROBE_PICK(1, 8)
   DFRG_PROBE_PICK(2, 2) DFRG_PROBE_PICK(2, 4) DFRG_PROBE_PICK(2, 8)
+  DFRG_PROBE_PICK(3, 1) DFRG_PROBE_PICK(3, 2) DFRG_PROBE_PICK(3, 4)
 #undef DFRG_PROBE_PICK
   if (!kern) return -1;
   kern<<<sms, 512, 0, st>>>(n_iter, sink);

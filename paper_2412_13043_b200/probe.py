@@ -21,7 +21,7 @@ def _load():
 
 def fp64_issue_model(sink, n_iter=20000):
     """Times 8 DFMA chains per thread with K instructions of another pipe interleaved per 8 DFMA (bench_probe/fp64_probe.cu).
-    Returns {"base_ms": t(K=0), "int_add": {K: t/t0}, "i2f_f64": {...}, "lds128": {...}}.  int_add ratios (16 + K)/16 = 1.25, 1.5
+    Returns {"base_ms": t(K=0), "int_add": {K: t/t0}, "cvt_f64": {...}, "lds128": {...}}.  int_add ratios (16 + K)/16 = 1.25, 1.5
     would mean an FP64 warp instruction holds the issue port for two cycles; ratios of 1 that other instructions issue in its
     shadow."""
     import torch
@@ -39,8 +39,8 @@ def fp64_issue_model(sink, n_iter=20000):
                 raise RuntimeError("dfrg_probe_fp64_issue failed (%d)" % rc)
         return a.elapsed_time(b)
     t0 = t(0, 0)
-    return {"base_ms": t0, "int_add": {k: t(0, k) / t0 for k in (4, 8)}, "i2f_f64": {k: t(1, k) / t0 for k in (1, 2, 4)},
-            "lds128": {k: t(2, k) / t0 for k in (2, 4, 8)}}
+    return {"base_ms": t0, "int_add": {k: t(0, k) / t0 for k in (4, 8)}, "cvt_f64": {k: t(1, k) / t0 for k in (2, 4, 8)},
+            "lds128": {k: t(2, k) / t0 for k in (2, 4, 8)}, "mufu_rcp64h": {k: t(3, k) / t0 for k in (1, 2, 4)}}
 
 
 def fp64_peak(n_iter, ctas_per_sm, sink):
