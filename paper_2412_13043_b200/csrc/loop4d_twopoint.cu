@@ -151,12 +151,15 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
       for (int t = ptid; t < ni * nc; t += TP_NPROD) {
         const int il = t / nc, j = t - il * nc;
         const double q = sxq[i0 + il], c = sxc[j];
-        double s = q * q + p * p + 2.0 * q * p * c;
+        // (explicit FMAs: left to the compiler, the contraction of a*b + c may differ between the template instantiations
+        //  of this kernel, and the values must not depend on whether derivatives were asked for)
+        const double qpc = q * p * c;
+        double s = fma(2.0, qpc, fma(q, q, p * p));
         s = clamp_lo(s, 0.0);
         double R, Rd;
         regulator(P.reg, fm, s, R, Rd);
-        const double D0 = table_lookup(cZ, P.grid, fm, s) * s + R;
-        const double poly = coef0 + coef1 * (q * p * c * P.reg.inv_k2);
+        const double D0 = fma(table_lookup(cZ, P.grid, fm, s), s, R);
+        const double poly = fma(coef1, qpc * P.reg.inv_k2, coef0);
         dst[t] = make_double2(D0, swc[j] * poly);
         dmin0 = fmin(dmin0, D0);
       }
@@ -179,7 +182,7 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
       const double q = sxq[i], s = q * q;
       double R, Rd;
       regulator(P.reg, fm, s, R, Rd);
-      const double D0 = table_lookup(cZ, P.grid, fm, s) * s + R;
+      const double D0 = fma(table_lookup(cZ, P.grid, fm, s), s, R);
       souter[i] = make_double2(D0, swq[i] * q * q * q * Rd);
       dq = fmin(dq, D0);
     }
