@@ -55,7 +55,7 @@ def check(g, o, N):
     flow_o = (N - 1.0) * o["chan"][0] + o["chan"][1]
     assert np.all(np.abs(g["flow"] - flow_o) <= SENS_EPS * ((abs(N - 1.0)) * o["sens"][0] + o["sens"][1]))
     if g["dchan"] is not None:
-        assert np.all(np.abs(g["dchan"] - o["dchan"]) <= 10 * SENS_EPS * o["sens_d"])
+        assert np.all(np.abs(g["dchan"] - o["dchan"]) <= SENS_EPS * o["sens_d"])
     if g["dmin"] is not None:
         dm = np.minimum(o["dmin"][0], o["dmin"][1])
         assert np.all(np.abs(g["dmin"] - dm) <= 1e-12 * (1 + dm))
