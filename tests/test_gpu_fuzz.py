@@ -72,6 +72,8 @@ def draw(rng):
         c["reg_order"] = 3
     if rng.integers(3) == 0:
         c["reg_zk"], c["reg_eta"] = 1.0 + 0.5 * float(rng.random()), float(rng.random()) - 0.3
+    if fam in ("lpaF", "mats", "matsmu") and rng.integers(2):
+        c["fermion_reg"] = 1                         # fermion line regulated with RF / RFdot (reading A25)
     return fam, c
 
 
