@@ -321,3 +321,38 @@ def test_lpa_batched_temperatures_are_the_single_calls():
             B.dfrg_integrate_lpa(c["d"], c["T"], c["n_max"], arg4d, c["N"], c["prefactor"], c["reg_kind"], c["reg_order"],
                                  c["k"], rq, rho, u, du, f1, c1, d1, dchan=dc1, **kw)
             assert torch.equal(flow[t], f1) and torch.equal(chan[t], c1) and torch.equal(dmin[t], d1) and torch.equal(dchan[t], dc1)
+
+
+def test_batched_reciprocal_range_and_coupling_are_as_documented():
+    """include/dfrg.h, "Magnitude range and coupling of the batched reciprocals": masses up to ~1e75 k^2 are fine everywhere;
+    a denominator beyond the range at field point f invalidates f and its partner (f + 256 in the Matsubara family, f + 128
+    in the two-point family) and nothing else; DFRG_M3_ONE_FIELD confines it to f."""
+    from paper_2412_13043_b200 import binding as B
+    # Matsubara family, 600 field points: tile 0 pairs f with f + 256
+    c = inputs.config4(n_field=600, n_p=1, n_jext=2, n_q=6, n_c=8)
+    c["n_max"] = 2
+    c["m2psi"], c["m2phi"] = c["m2psi"].copy(), c["m2phi"].copy()
+    c["m2psi"][10] = c["m2phi"][10] = 1e30                  # inside the documented range: correct, partner too
+    R = make_rules(c, B.dfrg_quad_nodes)
+    o = oracle_run(c, R)
+    g = gpu_run(c, R)
+    assert_parity(g["out"], o["out"], o["dmin"], o["sens"], "m2 = 1e30")
+    c["m2phi"][20] = 1e80                                   # outside: f = 20 and its partner f = 276 are lost, nothing else
+    o = oracle_run(c, R)
+    keep = np.ones(600, dtype=bool)
+    keep[[20, 276]] = False
+    g = gpu_run(c, R)
+    assert_parity(g["out"][..., keep], o["out"][..., keep], o["dmin"][..., keep], o["sens"][..., keep], "m2 = 1e80")
+    keep[276] = True
+    g = gpu_run(dict(c, path=B.M3_ONE_FIELD), R)            # every field point inverted on its own
+    assert_parity(g["out"][..., keep], o["out"][..., keep], o["dmin"][..., keep], o["sens"][..., keep], "m2 = 1e80, one field")
+    # two-point family, 300 field points: f pairs with f + 128
+    c = inputs.config2(n_field=300, n_ext=2, n_q=12, n_c=6)
+    c["m2"] = c["m2"].copy()
+    c["m2"][5] = 1e80
+    R = make_rules(c, B.dfrg_quad_nodes)
+    o = oracle_run(c, R)
+    keep = np.ones(300, dtype=bool)
+    keep[[5, 133]] = False
+    g = gpu_run(c, R)
+    assert_parity(g["out"][:, keep], o["out"][:, keep], o["dmin"][:, keep], o["sens"][:, keep], "two-point m2 = 1e80")
