@@ -252,8 +252,11 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
     L.add(sm.sx2, P.x2, n2); L.add(sm.sw2, P.w2, n2);
     L.add(sm.sZA, P.ZA, nt);
     if (TAB3D) L.add(sm.stab3, Q.v3, Q.ntab3); else L.add(sm.sL3, P.L3, nt);
+    // the shifted copy for the paired look-up of the hot loop (source not 16-byte aligned: plain loads)
+    if (TAB3D && Q.paired3) L.add(sm.stab3 + ((Q.ntab3 + 1) & ~1), Q.v3 + 1, Q.ntab3 - 1);
     stage_to_smem(L, &bar, 0);
   }
+  const double* stab3B = sm.stab3 + ((Q.ntab3 + 1) & ~1);
   const FastMath fm = fm_build(sm.fmmem, P.fmc);   // the S0 axis of the 3-D table (TAB3D)
   const double* fxtab = fx_build(sm.fxmem, P.reg.zk * P.reg.k2);
   const LogGrid2 lg = lg2_build(sm.lgmem, Q.lgc, nt);
@@ -365,12 +368,22 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
           double acc2 = acc;      // (w0 is folded into the quartic coefficients: the row adds straight into the running sum)
           if constexpr (TAB3D) {
             const double* ns = nS + pl * n2;
+            if (Q.paired3) {
 #pragma unroll 4
-            for (int j2 = 0; j2 < n2; ++j2) {
-              const double2 bs = na[j2];
-              const double lam3 = tab3d_vertex(sm.stab3, Q.T3, fm, scc, cur[0], ns[j2]);
-              const double poly = fma(fma(fma(fma(cur[5], bs.y, cur[4]), bs.y, cur[3]), bs.y, cur[2]), bs.y, cur[1]);
-              acc2 = fma(bs.x * poly, lam3, acc2);
+              for (int j2 = 0; j2 < n2; ++j2) {
+                const double2 bs = na[j2];
+                const double lam3 = tab3d_vertex_paired(sm.stab3, stab3B, Q.T3, fm, scc, cur[0], ns[j2]);
+                const double poly = fma(fma(fma(fma(cur[5], bs.y, cur[4]), bs.y, cur[3]), bs.y, cur[2]), bs.y, cur[1]);
+                acc2 = fma(bs.x * poly, lam3, acc2);
+              }
+            } else {
+#pragma unroll 4
+              for (int j2 = 0; j2 < n2; ++j2) {
+                const double2 bs = na[j2];
+                const double lam3 = tab3d_vertex(sm.stab3, Q.T3, fm, scc, cur[0], ns[j2]);
+                const double poly = fma(fma(fma(fma(cur[5], bs.y, cur[4]), bs.y, cur[3]), bs.y, cur[2]), bs.y, cur[1]);
+                acc2 = fma(bs.x * poly, lam3, acc2);
+              }
             }
           } else {
             const double up = (cur[0] + scc3) + rc[pl];
@@ -456,12 +469,16 @@ int t3g_launch(ThreePointParams& P, int G, int regk, const Tab3DParams* T3, cons
     nodes /= 2;
   if (nodes < P.n2) nodes = T3G_NODES;
   const int kp = pairs_per_unit(nodes);
-  const size_t smem_main = t3m_smem(P.nq, P.n1, P.n2, P.grid.n, nodes, kp, T3G_MAXT, T3 ? ntab3 : 0);
+  size_t smem_main = t3m_smem(P.nq, P.n1, P.n2, P.grid.n, nodes, kp, T3G_MAXT, T3 ? ntab3 : 0);
   if (smem_main > kMaxDynSmem) return DFRG_OK;
+  // a second, shifted copy of the 3-D table for the paired look-up of the hot loop, if it fits (n[2] >= 2 always holds)
+  const size_t smem_copy = 8 * (size_t)((ntab3 + 1) & ~1);
+  const bool paired3 = T3 != nullptr && smem_main + smem_copy <= kMaxDynSmem;
+  if (paired3) smem_main += smem_copy;
   ThreeGridParams Q;
   Q.B = P;
   Q.G = G; Q.S = n_ext / G;
-  Q.v3 = v3; Q.ntab3 = ntab3;
+  Q.v3 = v3; Q.ntab3 = ntab3; Q.paired3 = paired3 ? 1 : 0;
   if (T3) Q.T3 = *T3;
   Q.NODES = nodes;
   Q.lgc = lg2_consts(P.grid.lo, P.grid.inv_h);

@@ -103,6 +103,43 @@ __device__ __forceinline__ double tab3d_eval(const double* __restrict__ v, const
   return fma(tau[0], w1 - w0, w0);
 }
 
+// The same look-up with the eight corners fetched as four 16-byte loads.  The corners come in pairs adjacent along the last
+// axis, (i2, i2 + 1); vB is a second copy of the table shifted by one element (vB[j] = v[j + 1]), so that a pair starting at
+// an odd offset is read, aligned, from vB at offset - 1.  The look-up is bound by the shared-memory pipe (eight scattered
+// 8-byte loads per lane, each several wavefronts because of bank conflicts); four scattered 16-byte loads need fewer
+// wavefronts.  Same arithmetic as tab3d_eval, bit for bit.  v and vB are 16-byte aligned.
+__device__ __forceinline__ double tab3d_eval_paired(const double* __restrict__ v, const double* __restrict__ vB,
+                                                    const Tab3DParams& T, const FastMath& fm, const double x0,
+                                                    const double x1, const double x2) {
+  const double x[3] = {x0, x1, x2};
+  int i[3];
+  double tau[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const double c = T.is_log[a] ? 0.5 * fm_log(fm, x[a]) : x[a];
+    double t = (c - T.lo[a]) * T.inv_h[a];
+    t = clamp_lo(t, 0.0);  // NaN -> 0
+    t = clamp_hi(t, (double)(T.n[a] - 1));
+    int ii = (int)t;
+    ii = min(ii, T.n[a] - 2);
+    i[a] = ii;
+    tau[a] = t - (double)ii;
+  }
+  const int s1 = T.n[2], s0 = T.n[1] * T.n[2];
+  const int o = i[0] * s0 + i[1] * s1 + i[2];
+  auto pair_at = [&](const int off) {
+    return (off & 1) ? *reinterpret_cast<const double2*>(vB + off - 1) : *reinterpret_cast<const double2*>(v + off);
+  };
+  const double2 b00 = pair_at(o), b01 = pair_at(o + s1), b10 = pair_at(o + s0), b11 = pair_at(o + s0 + s1);
+  const double v00 = fma(tau[2], b00.y - b00.x, b00.x);
+  const double v01 = fma(tau[2], b01.y - b01.x, b01.x);
+  const double v10 = fma(tau[2], b10.y - b10.x, b10.x);
+  const double v11 = fma(tau[2], b11.y - b11.x, b11.x);
+  const double w0 = fma(tau[1], v01 - v00, v00);
+  const double w1 = fma(tau[1], v11 - v10, v10);
+  return fma(tau[0], w1 - w0, w0);
+}
+
 // lambda3 at the vertex with squared leg momenta (k1, k2, k3):  S0^2 = (k1+k2+k3)/6, a = sqrt3 (k2-k1)/(6 S0^2),
 // s = (k1+k2-2 k3)/(6 S0^2);  S0 = 0: a = s = 0.
 __device__ __forceinline__ double tab3d_vertex(const double* __restrict__ v, const Tab3DParams& T, const FastMath& fm,
@@ -110,6 +147,14 @@ __device__ __forceinline__ double tab3d_vertex(const double* __restrict__ v, con
   const double six = k1 + k2 + k3;
   const double r = six > 0.0 ? fast_rcp(six) : 0.0;
   return tab3d_eval(v, T, fm, six * (1.0 / 6.0), 1.7320508075688772 * (k2 - k1) * r, (k1 + k2 - 2.0 * k3) * r);
+}
+
+__device__ __forceinline__ double tab3d_vertex_paired(const double* __restrict__ v, const double* __restrict__ vB,
+                                                      const Tab3DParams& T, const FastMath& fm, const double k1,
+                                                      const double k2, const double k3) {
+  const double six = k1 + k2 + k3;
+  const double r = six > 0.0 ? fast_rcp(six) : 0.0;
+  return tab3d_eval_paired(v, vB, T, fm, six * (1.0 / 6.0), 1.7320508075688772 * (k2 - k1) * r, (k1 + k2 - 2.0 * k3) * r);
 }
 
 // ---- three-point on a product grid ----
@@ -130,6 +175,7 @@ struct ThreeGridParams {
   Tab3DParams T3;  // TAB3D instantiations: lambda3(S0^2, a, s) instead of the 1-D table
   const double* v3;
   int ntab3;
+  int paired3;     // TAB3D main kernel: a second, shifted copy of the table sits behind the first (tab3d_eval_paired)
 };
 
 constexpr int T3G_THREADS = 256;
