@@ -35,7 +35,7 @@ __device__ __forceinline__ double fast_rcp(double d) {
 //               ln s = e ln2 + ln c_j + (r - r^2/2 + ... - r^6/6)          abs. error <~ 3e-16 for |e| < 64
 //   fm_exp_neg(x) = e^-x, 0 <= x: n = rint(-64 x / ln2), r = -x - n ln2/64, |r| <= ln2/128;
 //               e^-x = 2^(n>>6) 2^((n&63)/64) (1 + r + ... + r^5/120)       rel. error <~ 2 ulp; exactly 0 where libm's
-//               e^-x is 0 (x >= 745.1332191019412); 700 < x below that is clamped to 700 (1e-304 instead of a subnormal).
+//               e^-x is 0 (x >= 745.1332191019412) and, flushed, where libm's is a subnormal (x >= 708.4).
 // fm_log(0) = -709.8 (exponent field 0): every table coordinate derived from it clamps to the first grid point.
 struct FastMath {
   const double2* logtab;  // [128] (1/c_j, ln c_j)
@@ -110,14 +110,18 @@ __device__ __forceinline__ double fm_log(const FastMath& fm, double s) {
   return fma(ed, fm.k[5], T.y) + fma(ed, fm.k[6], lm);
 }
 
-// libm's e^-x is exactly 0 from x = 745.1332191019412 on (it rounds below half the smallest subnormal): the same here,
-// decided on the bits of x with integer compares (reading A17: 0 on both sides).  Below that the argument is clamped to 700.
-__device__ __forceinline__ bool exp_neg_underflows(const double x) {
-  return __double_as_longlong(x) > 0x40874910d52d3051LL;   // x >= 0 (NaN counts as underflow)
+// libm's e^-x is exactly 0 from x = 745.1332191019412 on (reading A17: 0 on both sides).  Here the argument is clamped to 746
+// and the scaling by 2^(n >> 6) -- an integer add into the exponent field -- returns exactly 0 whenever the result would not
+// be a normal number: e^-x = 0 for x >= 708.4 (libm returns subnormals, < 2.3e-308, between 708.4 and 745.13).  One integer
+// compare and two selects on the result; a test on the bits of x itself (a 64-bit compare with x kept alive across the
+// series) cost the three- and four-point kernels 8-20 % of their time.
+__device__ __forceinline__ double exp_scale_flush(const double v, const int n) {
+  const int hi = __double2hiint(v) + ((n >> 6) << 20);
+  const bool sub = hi < 0x00100000;                 // exponent field <= 0 (or wrapped below it)
+  return __hiloint2double(sub ? 0 : hi, sub ? 0 : __double2loint(v));
 }
 __device__ __forceinline__ double fm_exp_neg(const FastMath& fm, double x) {
-  const bool uf = exp_neg_underflows(x);
-  x = clamp_hi(x, 700.0);
+  x = clamp_hi(x, 746.0);   // (NaN -> 746 -> 0)
   const double MAGIC = fm.k[8];  // 1.5 * 2^52: the low word of y holds rint(-x * 64/ln2)
   const double y = fma(x, fm.k[7], MAGIC);
   const int n = __double2loint(y);
@@ -130,7 +134,7 @@ __device__ __forceinline__ double fm_exp_neg(const FastMath& fm, double x) {
   p = fma(r, p, fm.k[15]);
   p = fma(r, p, fm.k[15]);
   const double v = fm.exptab[n & 63] * p;
-  return __hiloint2double(uf ? 0 : __double2hiint(v) + ((n >> 6) << 20), uf ? 0 : __double2loint(v));
+  return exp_scale_flush(v, n);
 }
 
 // ---- regulators --------------------------------------------------------------------------------
@@ -438,7 +442,7 @@ __device__ __forceinline__ double lg2_lookup(const double4* __restrict__ cells, 
 
 // k^2 e^-x from a table of k^2 2^(j/64), replicated 16 times (one copy per lane & 15: a 64-bit shared-memory load is
 // served in half-warps, so the look-up is conflict free):  n = rint(-64 x / ln2), r = -x - n ln2/64, |r| <= ln2/128,
-// e^r by its series to r^5/120.  Exactly 0 where libm underflows to 0; 700 < x below that is clamped to 700.
+// e^r by its series to r^5/120.  Exactly 0 where libm underflows to 0 and where its result is a subnormal.
 constexpr int FX_REP = 16;
 constexpr int FX_DOUBLES = 64 * FX_REP;
 __device__ __forceinline__ const double* fx_build(double* mem, const double k2) {
@@ -450,8 +454,7 @@ __device__ __forceinline__ const double* fx_build(double* mem, const double k2) 
   return mem + (threadIdx.x & (FX_REP - 1));
 }
 __device__ __forceinline__ double fx_exp_neg(const double* __restrict__ tab, const double* __restrict__ kc, double x) {
-  const bool uf = exp_neg_underflows(x);
-  x = clamp_hi(x, 700.0);
+  x = clamp_hi(x, 746.0);
   const double MAGIC = kc[8];
   const double y = fma(x, kc[7], MAGIC);
   const int n = __double2loint(y);
@@ -464,7 +467,7 @@ __device__ __forceinline__ double fx_exp_neg(const double* __restrict__ tab, con
   p = fma(r, p, kc[15]);
   p = fma(r, p, kc[15]);
   const double v = tab[(n & 63) * FX_REP] * p;
-  return __hiloint2double(uf ? 0 : __double2hiint(v) + ((n >> 6) << 20), uf ? 0 : __double2loint(v));
+  return exp_scale_flush(v, n);
 }
 
 __device__ __forceinline__ double ipow(double x, int e) {
