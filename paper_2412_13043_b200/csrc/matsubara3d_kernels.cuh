@@ -1,6 +1,7 @@
 // matsubara3d_kernels.cuh -- kernels of dfrg_integrate_matsubara3d, shared by matsubara3d.cu (host API, pre-passes, the
 // row-streaming kernel and the specialised moment kernel) and matsubara3d_anyshape.cu (the any-shape moment kernel).
 #pragma once
+#include <type_traits>
 #include <stdlib.h>
 
 #include "dfrg_device.cuh"
@@ -231,7 +232,7 @@ __global__ void __launch_bounds__(GROUPS * M3_FT + 32, 1) mats3d_main_kernel(con
         const double y1 = nun * nuj * ik2;
         for (int i = lane; i < nq; i += 32) {
           const double q = sxq[i];
-          const double y3 = (nun * nun + q * q) * ik2;
+          const double y3 = fma(nun, nun, __dmul_rn(q, q)) * ik2;   // (explicit: the same bits in every instantiation)
           double be[4] = {0.0, 0.0, 0.0, 0.0};
           int idx = 0;
           double y1a = 1.0;
@@ -605,7 +606,7 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
       const int nbar = n >= 0 ? n : -n - 1;
       const double nun = (2.0 * n + 1.0) * pi * P.T, nuj = (2.0 * j + 1.0) * pi * P.T;
       const double y1 = nun * nuj * ik2;
-      const double y3 = (nun * nun + q * q) * ik2;
+      const double y3 = fma(nun, nun, __dmul_rn(q, q)) * ik2;   // (explicit: the same bits in every instantiation)
       // P = sum_b y2^b beta_b,  beta_b = sum_{a+c<=3-b} kap_abc y1^a y3^c   (idx: a outermost, then b, then c)
       double be[4] = {0.0, 0.0, 0.0, 0.0};
       int idx = 0;
@@ -686,7 +687,30 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
       double M[4][MF];
 #pragma unroll
       for (int k = 0; k < MF; ++k) { M[0][k] = 0.0; M[1][k] = 0.0; M[2][k] = 0.0; M[3][k] = 0.0; }
-      if (pipelined) {
+      // angular rules of 16, 24 (BASELINE config 4) and 32 nodes: the trips of the loop below unrolled at compile time (no
+      // loop control per row, and the scheduler sees across the trips: cfg4 1.64 -> 1.60 ms)
+      auto unrolled_row = [&](auto ncc) {
+        constexpr int NCC = decltype(ncc)::value;
+#pragma unroll
+        for (int c = 0; c < NCC; c += 2 * M3_NBAT) {
+          const int L = m * NCC + c;
+          mats3d_recip_batch<MF, SQ>(d0 + L + M3_NBAT, m2phi, rb);
+          if constexpr (SYM) mats3d_moment_accumulate_sym<MF>(num4 + c / 2, ra, M);
+          else mats3d_moment_accumulate<MF>(num4 + c, ra, M);
+          int Ln = L + 2 * M3_NBAT;
+          Ln = Ln < l_last ? Ln : l_last;
+          mats3d_recip_batch<MF, SQ>(d0 + Ln, m2phi, ra);
+          if constexpr (SYM) mats3d_moment_accumulate_sym<MF>(num4 + (c + M3_NBAT) / 2, rb, M);
+          else mats3d_moment_accumulate<MF>(num4 + c + M3_NBAT, rb, M);
+        }
+      };
+      if (nc == 24) {
+        unrolled_row(std::integral_constant<int, 24>{});
+      } else if (nc == 16) {
+        unrolled_row(std::integral_constant<int, 16>{});
+      } else if (nc == 32) {
+        unrolled_row(std::integral_constant<int, 32>{});
+      } else if (pipelined) {
         // two batches per trip, the reciprocals ping-ponging between ra and rb (no register moves):
         //   ra = batch at c (ready), rb <- batch at c+4 while ra is accumulated, ra <- batch at c+8 while rb is ...
         for (int c = 0; c < nc; c += 2 * M3_NBAT) {
@@ -850,7 +874,7 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_gmoment_kernel(const Mats3dPara
       const int nbar = n >= 0 ? n : -n - 1;
       const double nun = (2.0 * n + 1.0) * pi * P.T, nuj = (2.0 * j + 1.0) * pi * P.T;
       const double y1 = nun * nuj * ik2;
-      const double y3 = (nun * nun + q * q) * ik2;
+      const double y3 = fma(nun, nun, __dmul_rn(q, q)) * ik2;   // (explicit: the same bits in every instantiation)
       double be[4] = {0.0, 0.0, 0.0, 0.0};
       int idx = 0;
       double y1a = 1.0;
@@ -925,7 +949,28 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_gmoment_kernel(const Mats3dPara
       double M[4][MF];
 #pragma unroll
       for (int k = 0; k < MF; ++k) { M[0][k] = 0.0; M[1][k] = 0.0; M[2][k] = 0.0; M[3][k] = 0.0; }
-      if (pipelined) {
+      auto unrolled_row = [&](auto ncc) {   // as in mats3d_moment_kernel: 16, 24 and 32 angular nodes unrolled
+        constexpr int NCC = decltype(ncc)::value;
+#pragma unroll
+        for (int c = 0; c < NCC; c += 2 * M3_NBAT) {
+          const int L = m * NCC + c;
+          mats3d_recip_batch<MF, SQ>(d0 + L + M3_NBAT, m2phi, rb);
+          if constexpr (SYM) mats3d_moment_accumulate_sym<MF>(num4 + c / 2, ra, M);
+          else mats3d_moment_accumulate<MF>(num4 + c, ra, M);
+          int Ln = L + 2 * M3_NBAT;
+          Ln = Ln < l_last ? Ln : l_last;
+          mats3d_recip_batch<MF, SQ>(d0 + Ln, m2phi, ra);
+          if constexpr (SYM) mats3d_moment_accumulate_sym<MF>(num4 + (c + M3_NBAT) / 2, rb, M);
+          else mats3d_moment_accumulate<MF>(num4 + c + M3_NBAT, rb, M);
+        }
+      };
+      if (nc == 24) {
+        unrolled_row(std::integral_constant<int, 24>{});
+      } else if (nc == 16) {
+        unrolled_row(std::integral_constant<int, 16>{});
+      } else if (nc == 32) {
+        unrolled_row(std::integral_constant<int, 32>{});
+      } else if (pipelined) {
         for (int c = 0; c < nc; c += 2 * M3_NBAT) {
           const int L = m * nc + c;
           mats3d_recip_batch<MF, SQ>(d0 + L + M3_NBAT, m2phi, rb);
@@ -1006,8 +1051,13 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_gmoment_kernel(const Mats3dPara
 //   H[nbar] = 1/(D0re + m2 + i D0im)^2 per field point (thread-private shared-memory column; H(n < 0) = conj H(nbar)),
 //   beta' = (re[4], im[4]) per (j, n) in shared memory,  t = beta' . M (8 FP64),  acc[j] += H t (4 FP64).
 struct cplx_t { double re, im; };
+// (explicit roundings: left to the compiler, the contraction of a*b + c*d differs between the instantiations of the kernel,
+//  and the compile-time and run-time pair enumerations must agree bit for bit)
 __device__ __forceinline__ cplx_t cmul(const cplx_t a, const cplx_t b) {
-  cplx_t r; r.re = a.re * b.re - a.im * b.im; r.im = a.re * b.im + a.im * b.re; return r;
+  cplx_t r;
+  r.re = fma(a.re, b.re, -__dmul_rn(a.im, b.im));
+  r.im = fma(a.re, b.im, __dmul_rn(a.im, b.re));
+  return r;
 }
 // JB consecutive j of one side of row m, complex:  acc[j0+t] += H(n0+t) (beta'[j0+t][n0+t] . M), H(n < 0) = conj H(nbar);
 // stage-wise (loads, then 2 JB independent chains).  b: first beta' entry (re, then im), bstride in double4 per j.
@@ -1120,7 +1170,7 @@ __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dPara
       cplx_t p0n, p0j, y1, y3;
       p0n.re = nun; p0n.im = P.mu; p0j.re = nuj; p0j.im = P.mu;
       y1 = cmul(p0n, p0j); y1.re *= ik2; y1.im *= ik2;
-      y3 = cmul(p0n, p0n); y3.re = (y3.re + q * q) * ik2; y3.im *= ik2;
+      y3 = cmul(p0n, p0n); y3.re = fma(q, q, y3.re) * ik2; y3.im *= ik2;
       // P = sum_b y2^b beta_b,  beta_b = sum_{a+c<=3-b} kap_abc y1^a y3^c   (idx: a outermost, then b, then c)
       cplx_t be[4];
 #pragma unroll
@@ -1183,12 +1233,12 @@ __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dPara
 
     for (int nb = 0; nb < NPS; ++nb) {   // H = G_psi^2, G_psi = conj(D)/|D|^2, D = a + i bb
       const double a = psb[2 * nb] + m2psi[0], bb = psb[2 * nb + 1];
-      const double r = fast_rcp(fma(a, a, bb * bb));
+      const double r = fast_rcp(fma(a, a, __dmul_rn(bb, bb)));
       const double gr = a * r, gi = -(bb * r);
-      const double g2r = gr * gr - gi * gi, g2i = 2.0 * gr * gi;
+      const double g2r = fma(gr, gr, -__dmul_rn(gi, gi)), g2i = 2.0 * gr * gi;
       if (P.mode == 1) {   // d/dm2_psi: G^2 -> -2 G^3
-        myH[(size_t)nb * NTC * 2] = -2.0 * (g2r * gr - g2i * gi);
-        myH[(size_t)nb * NTC * 2 + 1] = -2.0 * (g2r * gi + g2i * gr);
+        myH[(size_t)nb * NTC * 2] = -2.0 * fma(g2r, gr, -__dmul_rn(g2i, gi));
+        myH[(size_t)nb * NTC * 2 + 1] = -2.0 * fma(g2r, gi, __dmul_rn(g2i, gr));
       } else {
         myH[(size_t)nb * NTC * 2] = g2r;
         myH[(size_t)nb * NTC * 2 + 1] = g2i;
@@ -1202,7 +1252,28 @@ __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dPara
     for (int m = 0; m < NROWS; ++m) {
       double M[4][MF];
       M[0][0] = 0.0; M[1][0] = 0.0; M[2][0] = 0.0; M[3][0] = 0.0;
-      if (pipelined) {
+      auto unrolled_row = [&](auto ncc) {   // as in mats3d_moment_kernel: 16, 24 and 32 angular nodes unrolled
+        constexpr int NCC = decltype(ncc)::value;
+#pragma unroll
+        for (int c = 0; c < NCC; c += 2 * M3_NBAT) {
+          const int L = m * NCC + c;
+          mats3d_recip_batch<MF, SQ>(d0 + L + M3_NBAT, m2phi, rb);
+          if constexpr (SYM) mats3d_moment_accumulate_sym<MF>(num4 + c / 2, ra, M);
+          else mats3d_moment_accumulate<MF>(num4 + c, ra, M);
+          int Ln = L + 2 * M3_NBAT;
+          Ln = Ln < l_last ? Ln : l_last;
+          mats3d_recip_batch<MF, SQ>(d0 + Ln, m2phi, ra);
+          if constexpr (SYM) mats3d_moment_accumulate_sym<MF>(num4 + (c + M3_NBAT) / 2, rb, M);
+          else mats3d_moment_accumulate<MF>(num4 + c + M3_NBAT, rb, M);
+        }
+      };
+      if (nc == 24) {
+        unrolled_row(std::integral_constant<int, 24>{});
+      } else if (nc == 16) {
+        unrolled_row(std::integral_constant<int, 16>{});
+      } else if (nc == 32) {
+        unrolled_row(std::integral_constant<int, 32>{});
+      } else if (pipelined) {
         for (int c = 0; c < nc; c += 2 * M3_NBAT) {
           const int L = m * nc + c;
           mats3d_recip_batch<MF, SQ>(d0 + L + M3_NBAT, m2phi, rb);
