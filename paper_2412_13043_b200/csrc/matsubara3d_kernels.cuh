@@ -590,9 +590,7 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
 
   // Stage of unit u into buffer b (S2 + the field-independent S3 remainder), by all threads of the CTA: the TMA
   // bulk copy of the unit's D0phi chunk, the fermion denominators, and beta'[j][n].  Called one unit ahead.
-  auto produce = [&](long long u, int b) {
-    const long long rem = u % upp;
-    const int e = (int)(rem / nq), i = (int)(rem - (long long)e * nq);
+  auto produce = [&](const int e, const int i, int b) {   // unit (., e, i); the caller advances (ft, e, i) without divisions
     if (tid == 0) {
       mbar_expect_tx(&full[b], (uint32_t)cs * 8u);
       tma_bulk_g2s(d0buf + (size_t)b * cs, P.d0phi + ((size_t)e * nq + i) * cs, (uint32_t)cs * 8u, &full[b]);
@@ -634,15 +632,18 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
   double m2psi[MF], m2phi[MF], acc[NJ][MF];
   int cur_ft = -1;
   uint32_t g = 0;
-  if (u0 < u1) produce(u0, 0);
+  // unit u = (ft, e, i), decoded once (64-bit divisions cost ~100 instructions each) and advanced incrementally
+  int ft_u = (int)(u0 / upp);
+  int e_u = (int)((u0 - (long long)ft_u * upp) / nq);
+  int i_u = (int)(u0 - (long long)ft_u * upp - (long long)e_u * nq);
+  if (u0 < u1) produce(e_u, i_u, 0);
   __syncthreads();
   for (long long u = u0; u < u1; ++u, ++g) {
-    const int ft = (int)(u / upp);
-    const long long rem = u - (long long)ft * upp;
-    const int e = (int)(rem / nq), i = (int)(rem - (long long)e * nq);
+    const int ft = ft_u, e = e_u, i = i_u;
+    if (++i_u == nq) { i_u = 0; if (++e_u == P.n_p) { e_u = 0; ++ft_u; } }   // (ft_u, e_u, i_u): unit u + 1
     const int f0 = ft * tile + tid;
     const int b = g & 1;
-    if (u + 1 < u1) produce(u + 1, b ^ 1);   // buffer b^1 was drained before the barrier that ended unit u-1
+    if (u + 1 < u1) produce(e_u, i_u, b ^ 1);   // buffer b^1 was drained before the barrier that ended unit u-1
     if (ft != cur_ft) {
       cur_ft = ft;
 #pragma unroll
@@ -858,9 +859,7 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_gmoment_kernel(const Mats3dPara
   }
   __syncthreads();
 
-  auto produce = [&](long long u, int b) {
-    const long long rem = u % upp;
-    const int e = (int)(rem / nq), i = (int)(rem - (long long)e * nq);
+  auto produce = [&](const int e, const int i, int b) {   // unit (., e, i); the caller advances (ft, e, i) without divisions
     if (tid == 0) {
       mbar_expect_tx(&full[b], (uint32_t)cs * 8u);
       tma_bulk_g2s(d0buf + (size_t)b * cs, P.d0phi + ((size_t)e * nq + i) * cs, (uint32_t)cs * 8u, &full[b]);
@@ -902,15 +901,18 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_gmoment_kernel(const Mats3dPara
   double m2psi[MF], m2phi[MF], acc[NJ][MF];
   int cur_ft = -1;
   uint32_t g = 0;
-  if (u0 < u1) produce(u0, 0);
+  // unit u = (ft, e, i), decoded once (64-bit divisions cost ~100 instructions each) and advanced incrementally
+  int ft_u = (int)(u0 / upp);
+  int e_u = (int)((u0 - (long long)ft_u * upp) / nq);
+  int i_u = (int)(u0 - (long long)ft_u * upp - (long long)e_u * nq);
+  if (u0 < u1) produce(e_u, i_u, 0);
   __syncthreads();
   for (long long u = u0; u < u1; ++u, ++g) {
-    const int ft = (int)(u / upp);
-    const long long rem = u - (long long)ft * upp;
-    const int e = (int)(rem / nq), i = (int)(rem - (long long)e * nq);
+    const int ft = ft_u, e = e_u, i = i_u;
+    if (++i_u == nq) { i_u = 0; if (++e_u == P.n_p) { e_u = 0; ++ft_u; } }   // (ft_u, e_u, i_u): unit u + 1
     const int f0 = ft * tile + tid;
     const int b = g & 1;
-    if (u + 1 < u1) produce(u + 1, b ^ 1);
+    if (u + 1 < u1) produce(e_u, i_u, b ^ 1);
     if (ft != cur_ft) {
       cur_ft = ft;
 #pragma unroll
@@ -1148,9 +1150,7 @@ __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dPara
   }
   __syncthreads();
 
-  auto produce = [&](long long u, int b) {
-    const long long rem = u % upp;
-    const int e = (int)(rem / nq), i = (int)(rem - (long long)e * nq);
+  auto produce = [&](const int e, const int i, int b) {   // unit (., e, i); the caller advances (ft, e, i) without divisions
     if (tid == 0) {
       mbar_expect_tx(&full[b], (uint32_t)cs * 8u);
       tma_bulk_g2s(d0buf + (size_t)b * cs, P.d0phi + ((size_t)e * nq + i) * cs, (uint32_t)cs * 8u, &full[b]);
@@ -1208,15 +1208,18 @@ __global__ void __launch_bounds__(256, 1) mats3d_cmoment_kernel(const Mats3dPara
   double m2psi[MF], m2phi[MF], accr[NJ], acci[NJ];
   int cur_ft = -1;
   uint32_t g = 0;
-  if (u0 < u1) produce(u0, 0);
+  // unit u = (ft, e, i), decoded once (64-bit divisions cost ~100 instructions each) and advanced incrementally
+  int ft_u = (int)(u0 / upp);
+  int e_u = (int)((u0 - (long long)ft_u * upp) / nq);
+  int i_u = (int)(u0 - (long long)ft_u * upp - (long long)e_u * nq);
+  if (u0 < u1) produce(e_u, i_u, 0);
   __syncthreads();
   for (long long u = u0; u < u1; ++u, ++g) {
-    const int ft = (int)(u / upp);
-    const long long rem = u - (long long)ft * upp;
-    const int e = (int)(rem / nq), i = (int)(rem - (long long)e * nq);
+    const int ft = ft_u, e = e_u, i = i_u;
+    if (++i_u == nq) { i_u = 0; if (++e_u == P.n_p) { e_u = 0; ++ft_u; } }   // (ft_u, e_u, i_u): unit u + 1
     const int f = ft * NTC + tid;
     const int b = g & 1;
-    if (u + 1 < u1) produce(u + 1, b ^ 1);
+    if (u + 1 < u1) produce(e_u, i_u, b ^ 1);
     if (ft != cur_ft) {
       cur_ft = ft;
       m2psi[0] = (f < P.n_field) ? P.m2psi[f] : 1.0;
