@@ -178,6 +178,9 @@ int dfrg_integrate_lpa_host(const dfrg_lpa_desc* D, int n_field, const double* r
 int dfrg_integrate_lpa_batch(const dfrg_lpa_desc* D, int n_T, const double* T_host, const int* n_max_host, int n_field,
                              const double* rho, const double* u, const double* du, double* flow, double* chan,
                              double* dmin, void* cuda_stream);
+int dfrg_integrate_lpa_batch_host(const dfrg_lpa_desc* D, int n_T, const double* T_host, const int* n_max_host, int n_field,
+                                  const double* rho, const double* u, const double* du, double* flow, double* chan,
+                                  double* dmin);   /* host pointers throughout; returns when the outputs have landed */
 
 /* ---- 4-D vacuum loops (BASELINE.json configs 2 and 3; angles cos1, cos2, phi of PAPER.md:1837-1840) ------
  * DFRG_LOOP_TWOPOINT (tab[0] = Z, n_coef = 2, axes q, cos1; cos2/phi unused, their measure is in prefactor):

@@ -24,7 +24,7 @@ RULE_GAUSS_LEGENDRE = 0
 EXPORTS = (
     "dfrg_strerror", "dfrg_last_cuda_error", "dfrg_version", "dfrg_shutdown", "dfrg_quad_nodes",
     "dfrg_matsubara_n_max",
-    "dfrg_integrate_lpa", "dfrg_integrate_lpa_host", "dfrg_integrate_lpa_batch",
+    "dfrg_integrate_lpa", "dfrg_integrate_lpa_host", "dfrg_integrate_lpa_batch", "dfrg_integrate_lpa_batch_host",
     "dfrg_integrate_loop4d", "dfrg_integrate_loop4d_host",
     "dfrg_integrate_matsubara3d", "dfrg_integrate_matsubara3d_host",
 )
@@ -99,6 +99,8 @@ def lib():
         L.dfrg_integrate_lpa_host.argtypes = [C.POINTER(LpaDesc), C.c_int, _vp, _vp, _vp, _vp, _vp, _vp]
         L.dfrg_integrate_lpa_batch.argtypes = [C.POINTER(LpaDesc), C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_int,
                                                _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+        L.dfrg_integrate_lpa_batch_host.argtypes = [C.POINTER(LpaDesc), C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int),
+                                                    C.c_int, _vp, _vp, _vp, _vp, _vp, _vp]
         L.dfrg_integrate_loop4d.argtypes = [C.POINTER(Loop4dDesc), C.c_int, _vp, C.c_int, _vp, _vp, _vp, _vp]
         L.dfrg_integrate_loop4d_host.argtypes = [C.POINTER(Loop4dDesc), C.c_int, _vp, C.c_int, _vp, _vp, _vp]
         L.dfrg_integrate_matsubara3d.argtypes = [C.POINTER(Mats3dDesc), C.c_int, _vp, _vp, C.c_int, _vp, C.c_int,
@@ -202,6 +204,22 @@ def dfrg_integrate_lpa_batch(d, Ts, n_maxs, reg_arg4d, N, prefactor, reg_kind, r
     _check(lib().dfrg_integrate_lpa_batch(C.byref(D), n_T, Tv, nv, int(rho.numel()), _ptr(rho, True), _ptr(u, True),
                                           _ptr(du, True), _ptr(flow, True), _ptr(chan, True), _ptr(dmin, True), _stream()),
            "dfrg_integrate_lpa_batch")
+    return flow
+
+
+def dfrg_integrate_lpa_batch_host(d, Ts, n_maxs, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, rho, u, du,
+                                  flow, chan=None, dmin=None, dchan=None, reg_zk=1.0, reg_eta=0.0, statistics=STAT_BOSON, mu=0.0,
+                                  fermion_reg=0):
+    """dfrg_integrate_lpa_batch on host (numpy) arrays."""
+    n_T = len(Ts)
+    D = _lpa_desc(d, 0.0, 0, reg_arg4d, N, prefactor, reg_kind, reg_order, k, rule_q, False, dchan, reg_zk, reg_eta, statistics,
+                  mu, fermion_reg)
+    Tv = (C.c_double * n_T)(*[float(t) for t in Ts])
+    nv = (C.c_int * n_T)(*[int(n) for n in n_maxs])
+    n_field = rho.numel() if hasattr(rho, "numel") else rho.size
+    _check(lib().dfrg_integrate_lpa_batch_host(C.byref(D), n_T, Tv, nv, int(n_field), _ptr(rho, False), _ptr(u, False),
+                                               _ptr(du, False), _ptr(flow, False), _ptr(chan, False), _ptr(dmin, False)),
+           "dfrg_integrate_lpa_batch_host")
     return flow
 
 

@@ -332,6 +332,37 @@ extern "C" int dfrg_integrate_lpa(const dfrg_lpa_desc* D, int n_field, const dou
   return lpa_launch(D, 1, &D->T, &D->n_max, n_field, rho, u, du, flow, chan, dmin, (cudaStream_t)cuda_stream);
 }
 
+extern "C" int dfrg_integrate_lpa_batch_host(const dfrg_lpa_desc* D, int n_T, const double* T_host, const int* n_max_host,
+                                             int n_field, const double* rho, const double* u, const double* du,
+                                             double* flow, double* chan, double* dmin) {
+  int rc = lpa_validate_batch(D, n_T, T_host, n_max_host, n_field, rho, u, du, flow);
+  if (rc != DFRG_OK) return rc;
+  rc = require_sm100(nullptr);
+  if (rc != DFRG_OK) return rc;
+  Arena& A = thread_arena();
+  const size_t nf = (size_t)n_field, nq = (size_t)D->q.n, nt = (size_t)n_T;
+  rc = A.begin((2 * nq + 3 * nf + 6 * nf * nt) * sizeof(double) + 16 * 256);
+  if (rc != DFRG_OK) return rc;
+  dfrg_lpa_desc Dd = *D;
+  Dd.q.x = A.put(D->q.x, nq);
+  Dd.q.w = A.put(D->q.w, nq);
+  const double* d_rho = A.put(rho, nf);
+  const double* d_u = A.put(u, nf);
+  const double* d_du = A.put(du, nf);
+  double* d_flow = A.reserve(nt * nf);
+  double* d_chan = chan ? A.reserve(2 * nt * nf) : nullptr;
+  double* d_dmin = dmin ? A.reserve(nt * nf) : nullptr;
+  Dd.dchan = D->dchan ? A.reserve(2 * nt * nf) : nullptr;
+  if (A.upload() != DFRG_OK) return A.status();
+  rc = lpa_launch(&Dd, n_T, T_host, n_max_host, n_field, d_rho, d_u, d_du, d_flow, d_chan, d_dmin, A.stream());
+  if (rc != DFRG_OK) return rc;
+  A.fetch(flow, d_flow, nt * nf);
+  if (chan) A.fetch(chan, d_chan, 2 * nt * nf);
+  if (dmin) A.fetch(dmin, d_dmin, nt * nf);
+  if (D->dchan) A.fetch(D->dchan, Dd.dchan, 2 * nt * nf);
+  return A.finish();
+}
+
 extern "C" int dfrg_integrate_lpa_host(const dfrg_lpa_desc* D, int n_field, const double* rho, const double* u,
                                        const double* du, double* flow, double* chan, double* dmin) {
   int rc = lpa_validate(D, n_field, rho, u, du, flow);

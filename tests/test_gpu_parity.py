@@ -321,6 +321,11 @@ def test_lpa_batched_temperatures_are_the_single_calls():
             B.dfrg_integrate_lpa(c["d"], c["T"], c["n_max"], arg4d, c["N"], c["prefactor"], c["reg_kind"], c["reg_order"],
                                  c["k"], rq, rho, u, du, f1, c1, d1, dchan=dc1, **kw)
             assert torch.equal(flow[t], f1) and torch.equal(chan[t], c1) and torch.equal(dmin[t], d1) and torch.equal(dchan[t], dc1)
+        if not fermi:   # the host entry point: the same numbers
+            hf, hc = np.full((nT, nf), np.nan), np.full((nT, 2, nf), np.nan)
+            B.dfrg_integrate_lpa_batch_host(c0["d"], [c["T"] for c in cs], [c["n_max"] for c in cs], arg4d, c0["N"], c0["prefactor"],
+                                            c0["reg_kind"], c0["reg_order"], c0["k"], (xq, wq), c0["rho"], c0["u"], c0["du"], hf, hc)
+            assert np.array_equal(hf, flow.cpu().numpy()) and np.array_equal(hc, chan.cpu().numpy())
 
 
 def test_batched_reciprocal_range_and_coupling_are_as_documented():
