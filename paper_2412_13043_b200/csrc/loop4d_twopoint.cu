@@ -1,4 +1,6 @@
 // loop4d_twopoint.cu -- two-point family of dfrg_integrate_loop4d (BASELINE.json config 2).
+#include <type_traits>
+
 #include "loop4d_kernels.cuh"
 
 namespace dfrg {
@@ -239,14 +241,32 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
       double Aa[MF], Ba[MF], Ab[MF], Bb[MF];
 #pragma unroll
       for (int k = 0; k < MF; ++k) { Aa[k] = 0.0; Ba[k] = 0.0; Ab[k] = 0.0; Bb[k] = 0.0; }
-      int j = 0;
-      for (; j + 4 <= nc; j += 4) {
-        tp_batch<MF, WANT_D, 4>(rowa + j, m2, Aa, Ba);
-        tp_batch<MF, WANT_D, 4>(rowb + j, m2, Ab, Bb);
-      }
-      for (; j < nc; ++j) {
-        tp_batch<MF, WANT_D, 1>(rowa + j, m2, Aa, Ba);
-        tp_batch<MF, WANT_D, 1>(rowb + j, m2, Ab, Bb);
+      // angular rules of 16, 24 and 32 (BASELINE config 2) nodes: unrolled at compile time, same order of operations
+      // (cfg2 33.1 -> 31.6 us: no loop control, and the scheduler sees across the batches)
+      auto unrolled_rows = [&](auto ncc) {
+        constexpr int NCC = decltype(ncc)::value;
+#pragma unroll
+        for (int j = 0; j < NCC; j += 4) {
+          tp_batch<MF, WANT_D, 4>(rowa + j, m2, Aa, Ba);
+          tp_batch<MF, WANT_D, 4>(rowb + j, m2, Ab, Bb);
+        }
+      };
+      if (nc == 32) {
+        unrolled_rows(std::integral_constant<int, 32>{});
+      } else if (nc == 24) {
+        unrolled_rows(std::integral_constant<int, 24>{});
+      } else if (nc == 16) {
+        unrolled_rows(std::integral_constant<int, 16>{});
+      } else {
+        int j = 0;
+        for (; j + 4 <= nc; j += 4) {
+          tp_batch<MF, WANT_D, 4>(rowa + j, m2, Aa, Ba);
+          tp_batch<MF, WANT_D, 4>(rowb + j, m2, Ab, Bb);
+        }
+        for (; j < nc; ++j) {
+          tp_batch<MF, WANT_D, 1>(rowa + j, m2, Aa, Ba);
+          tp_batch<MF, WANT_D, 1>(rowb + j, m2, Ab, Bb);
+        }
       }
       close_row(il, Aa, Ba);
       close_row(il + TP_GROUPS, Ab, Bb);
