@@ -74,7 +74,9 @@ def cfg4_counts(c, rules):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 20 ms under load.  The timed region of a default run lasts tens of
+    milliseconds -- shorter than nvidia-smi takes to start -- so the sampler is started before an untimed pre-load phase of the
+    same steps (0.3 s) that runs straight into the timed steps; the samples cover pre-load + timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -87,7 +89,7 @@ class ClockSampler:
     def start(self):
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                       "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.f,
                                       stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -108,6 +110,7 @@ class ClockSampler:
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         reasons = [nm for i, nm in enumerate(names) if any("Active" in r[3 + i] and "Not" not in r[3 + i] for r in rows)]
         return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "samples": len(rows),
+                "window": "untimed pre-load of the same steps (0.3 s) + the timed region, sampled every 20 ms",
                 "power_w_max": max(float(r[2]) for r in rows), "reasons": reasons}
 
 
@@ -400,6 +403,11 @@ def main():
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
+    t_pre = time.perf_counter()
+    while time.perf_counter() - t_pre < 0.3:                  # untimed pre-load: the GPU is under the same load when the
+        for _ in range(8):                                     # timed steps start, and the clock sampler is up
+            step()
+        torch.cuda.synchronize()
     evs = []
     barrier()
     t_wall = time.perf_counter()
