@@ -323,6 +323,8 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
   };
 
   double acc = 0.0;
+  Tab3Cell cell3;
+  cell3.o = -1;
   CellCache cc;
   cc.Fd = inf; cc.k = make_double4(0.0, 0.0, 0.0, 0.0);   // tau = t' - inf fails the range test: the first node loads its cell
   // (r, ch) of the units u, u + 1, u + 2, advanced without divisions
@@ -372,7 +374,7 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
 #pragma unroll 4
               for (int j2 = 0; j2 < n2; ++j2) {
                 const double2 bs = na[j2];
-                const double lam3 = tab3d_vertex_paired(sm.stab3, stab3B, Q.T3, fm, scc, cur[0], ns[j2]);
+                const double lam3 = tab3d_vertex_cached(sm.stab3, stab3B, Q.T3, fm, cell3, scc, cur[0], ns[j2]);
                 const double poly = fma(fma(fma(fma(cur[5], bs.y, cur[4]), bs.y, cur[3]), bs.y, cur[2]), bs.y, cur[1]);
                 acc2 = fma(bs.x * poly, lam3, acc2);
               }

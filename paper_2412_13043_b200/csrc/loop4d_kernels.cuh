@@ -140,6 +140,55 @@ __device__ __forceinline__ double tab3d_eval_paired(const double* __restrict__ v
   return fma(tau[0], w1 - w0, w0);
 }
 
+// ... and with the eight corners of the current cell kept in registers: consecutive nodes of a cos2 row move the vertex
+// coordinates slowly, so most look-ups fall into the cell of their predecessor and need no load at all (the reload is
+// predicated on the flat cell offset; the arithmetic is that of tab3d_eval, bit for bit).
+struct Tab3Cell {
+  int o;                        // flat offset of the cached cell's first corner; -1 = empty
+  double2 b00, b01, b10, b11;   // the corner pairs along the last axis
+};
+__device__ __forceinline__ double tab3d_eval_cached(const double* __restrict__ v, const double* __restrict__ vB,
+                                                    const Tab3DParams& T, const FastMath& fm, Tab3Cell& cell,
+                                                    const double x0, const double x1, const double x2) {
+  const double x[3] = {x0, x1, x2};
+  int i[3];
+  double tau[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const double c = T.is_log[a] ? 0.5 * fm_log(fm, x[a]) : x[a];
+    double t = (c - T.lo[a]) * T.inv_h[a];
+    t = clamp_lo(t, 0.0);  // NaN -> 0
+    t = clamp_hi(t, (double)(T.n[a] - 1));
+    int ii = (int)t;
+    ii = min(ii, T.n[a] - 2);
+    i[a] = ii;
+    tau[a] = t - (double)ii;
+  }
+  const int s1 = T.n[2], s0 = T.n[1] * T.n[2];
+  const int o = i[0] * s0 + i[1] * s1 + i[2];
+  if (o != cell.o) {
+    auto pair_at = [&](const int off) {
+      return (off & 1) ? *reinterpret_cast<const double2*>(vB + off - 1) : *reinterpret_cast<const double2*>(v + off);
+    };
+    cell.b00 = pair_at(o); cell.b01 = pair_at(o + s1); cell.b10 = pair_at(o + s0); cell.b11 = pair_at(o + s0 + s1);
+    cell.o = o;
+  }
+  const double v00 = fma(tau[2], cell.b00.y - cell.b00.x, cell.b00.x);
+  const double v01 = fma(tau[2], cell.b01.y - cell.b01.x, cell.b01.x);
+  const double v10 = fma(tau[2], cell.b10.y - cell.b10.x, cell.b10.x);
+  const double v11 = fma(tau[2], cell.b11.y - cell.b11.x, cell.b11.x);
+  const double w0 = fma(tau[1], v01 - v00, v00);
+  const double w1 = fma(tau[1], v11 - v10, v10);
+  return fma(tau[0], w1 - w0, w0);
+}
+__device__ __forceinline__ double tab3d_vertex_cached(const double* __restrict__ v, const double* __restrict__ vB,
+                                                      const Tab3DParams& T, const FastMath& fm, Tab3Cell& cell,
+                                                      const double k1, const double k2, const double k3) {
+  const double six = k1 + k2 + k3;
+  const double r = six > 0.0 ? fast_rcp(six) : 0.0;
+  return tab3d_eval_cached(v, vB, T, fm, cell, six * (1.0 / 6.0), 1.7320508075688772 * (k2 - k1) * r, (k1 + k2 - 2.0 * k3) * r);
+}
+
 // lambda3 at the vertex with squared leg momenta (k1, k2, k3):  S0^2 = (k1+k2+k3)/6, a = sqrt3 (k2-k1)/(6 S0^2),
 // s = (k1+k2-2 k3)/(6 S0^2);  S0 = 0: a = s = 0.
 __device__ __forceinline__ double tab3d_vertex(const double* __restrict__ v, const Tab3DParams& T, const FastMath& fm,
