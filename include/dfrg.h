@@ -59,7 +59,8 @@ typedef enum {
   DFRG_EINVAL = -1,       /* null required pointer, non-positive size, T < 0, k <= 0, bad interp, wrong n_coef ... */
   DFRG_EUNSUPPORTED = -2, /* sizes beyond the shared-memory budget, unsupported dimension, not an sm_100 device */
   DFRG_ECUDA = -3,        /* CUDA runtime / launch error; see dfrg_last_cuda_error() */
-  DFRG_ENOMEM = -4        /* device arena allocation failed (host entry points only) */
+  DFRG_ENOMEM = -4,       /* device arena allocation failed (host entry points only) */
+  DFRG_ESCRATCH = -5      /* dfrg_integrate_twopoint_noalloc only: the call needs more scratch than the fixed array holds */
 } dfrg_status;
 
 const char* dfrg_strerror(int status);  /* static string */
@@ -256,6 +257,41 @@ int dfrg_integrate_loop4d(const dfrg_loop4d_desc* D, int n_field, const double* 
                           double* out, double* dmin, void* cuda_stream);
 int dfrg_integrate_loop4d_host(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext,
                                const double* ext, double* out, double* dmin);
+
+/* ---- Two-point loop for callers that cannot allocate device memory ------------------------------------------
+ * Every other device entry point of this library takes the scratch of its kernels (partial sums of the fixed-order
+ * reduction, denominator minima) from a library-owned CUDA memory pool, which now and then has to grow, i.e. allocate.
+ * That is not acceptable to every caller: a solver that has given all device memory to its own allocator and wants no
+ * second one beside it, a thread that must never block on the driver's allocation lock (callbacks, latency-bound
+ * loops), a job under a device-memory cap where an allocation in the middle of a flow may fail.  This entry point is
+ * the two-point family (DFRG_LOOP_TWOPOINT; same descriptor, same arguments, same integrand, PAPER.md:1007-1030 and the
+ * "Two-point" block above) with NO allocation of any kind on the device: it calls neither cudaMalloc / cudaFree nor
+ * their stream-ordered or pooled relatives, nor any library routine that does.  The kernels and the launch plan are the
+ * ones dfrg_integrate_loop4d uses, so out / dmin / D->dout_dm2 are bit-identical to that call's.
+ *
+ * Where the scratch lives: in a fixed array of DFRG_NOALLOC_SCRATCH_BYTES that is part of the library image.  Every GPU
+ * on which the library is loaded carries it from load to process exit, used or not; that is the price of the guarantee.
+ * The limit: the call needs
+ *     8 * ( 4 U + 2  +  slots * (dout_dm2 ? 2 : 1) * n_ext * n_field )  bytes,
+ *     U = ceil(n_field / tile) * n_ext * ceil(q.n / QC),  tile = 256 (128 if n_field <= 128),
+ *     QC = min(8, q.n, floor(2048 / cos1.n)),  slots <= 2 + ceil(q.n / QC) * (number of SMs) / U  (CTAs sharing one output),
+ * about 0.6 MB for BASELINE.json config 2 with derivatives (64 momenta x 256 field points, 128 x 32 nodes).  A call
+ * that needs more returns DFRG_ESCRATCH before anything is enqueued and writes nothing; use dfrg_integrate_loop4d then.
+ *
+ * First call on a device: looks up the device address of the array and raises the kernels' shared-memory limit (two
+ * CUDA runtime queries, a few host-side table entries).  Make this first call outside any stream capture; later calls
+ * only enqueue the two kernels.
+ *
+ * Sharing: there is ONE array per device, and every call on that device uses it from its start.  Two calls whose kernels
+ * can overlap on the GPU (different streams without an ordering between them, or two host threads) race on it and both
+ * results are garbage: order such calls on one stream or with events.  The array keeps whatever the last call left in
+ * it; no call depends on its contents (every entry that is read has been written by the same call before), so there is
+ * nothing to clear between calls.
+ *
+ * Other return values as dfrg_integrate_loop4d; D->family must be DFRG_LOOP_TWOPOINT (DFRG_EINVAL otherwise). */
+#define DFRG_NOALLOC_SCRATCH_BYTES (8u * 1024u * 1024u)
+int dfrg_integrate_twopoint_noalloc(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext,
+                                    const double* ext, double* out, double* dmin, void* cuda_stream);
 
 /* ---- 3-D spatial momentum + Matsubara sum (BASELINE.json config 4; "Quadraturex0") -------
  *   nu_n = (2n+1) pi T (loop fermion, n = -n_max..n_max; external fermion index j = 0..n_jext-1)

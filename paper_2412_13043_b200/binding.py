@@ -12,7 +12,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdfrg.so")
 
-DFRG_OK, DFRG_EINVAL, DFRG_EUNSUPPORTED, DFRG_ECUDA, DFRG_ENOMEM = 0, -1, -2, -3, -4
+DFRG_OK, DFRG_EINVAL, DFRG_EUNSUPPORTED, DFRG_ECUDA, DFRG_ENOMEM, DFRG_ESCRATCH = 0, -1, -2, -3, -4, -5
+NOALLOC_SCRATCH_BYTES = 8 * 1024 * 1024   # DFRG_NOALLOC_SCRATCH_BYTES of include/dfrg.h
 REG_LITIM, REG_EXP_POLY = 0, 1
 STAT_BOSON, STAT_FERMION = 0, 1
 DOMAIN_X0, DOMAIN_Q0 = 0, 1
@@ -25,7 +26,7 @@ EXPORTS = (
     "dfrg_strerror", "dfrg_last_cuda_error", "dfrg_version", "dfrg_shutdown", "dfrg_quad_nodes",
     "dfrg_matsubara_n_max",
     "dfrg_integrate_lpa", "dfrg_integrate_lpa_host", "dfrg_integrate_lpa_batch", "dfrg_integrate_lpa_batch_host",
-    "dfrg_integrate_loop4d", "dfrg_integrate_loop4d_host",
+    "dfrg_integrate_loop4d", "dfrg_integrate_loop4d_host", "dfrg_integrate_twopoint_noalloc",
     "dfrg_integrate_matsubara3d", "dfrg_integrate_matsubara3d_host",
 )
 
@@ -103,6 +104,7 @@ def lib():
                                                     C.c_int, _vp, _vp, _vp, _vp, _vp, _vp]
         L.dfrg_integrate_loop4d.argtypes = [C.POINTER(Loop4dDesc), C.c_int, _vp, C.c_int, _vp, _vp, _vp, _vp]
         L.dfrg_integrate_loop4d_host.argtypes = [C.POINTER(Loop4dDesc), C.c_int, _vp, C.c_int, _vp, _vp, _vp]
+        L.dfrg_integrate_twopoint_noalloc.argtypes = [C.POINTER(Loop4dDesc), C.c_int, _vp, C.c_int, _vp, _vp, _vp, _vp]
         L.dfrg_integrate_matsubara3d.argtypes = [C.POINTER(Mats3dDesc), C.c_int, _vp, _vp, C.c_int, _vp, C.c_int,
                                                  _vp, _vp, _vp]
         L.dfrg_integrate_matsubara3d_host.argtypes = [C.POINTER(Mats3dDesc), C.c_int, _vp, _vp, C.c_int, _vp,
@@ -266,6 +268,22 @@ def dfrg_integrate_loop4d(family, prefactor, reg_kind, reg_order, k, rule_q, rul
     n_ext = _n(ext) // {LOOP_TWOPOINT: 1, LOOP_THREEPOINT: 3, LOOP_FOURPOINT: 6, LOOP_THREEPOINT_TAB3D: 3}[family]
     _check(lib().dfrg_integrate_loop4d(C.byref(D), _n(m2), _ptr(m2, True), n_ext, _ptr(ext, True),
                                        _ptr(out, True), _ptr(dmin, True), _stream()), "dfrg_integrate_loop4d")
+    return out
+
+
+def dfrg_integrate_twopoint_noalloc(prefactor, reg_kind, reg_order, k, rule_q, rule_c1, Z, lnq_lo, lnq_hi, interp, coef,
+                                    m2, ext, out, dmin=None, dout_dm2=None, reg_zk=1.0, reg_eta=0.0):
+    """Two-point loop without any device allocation inside the library (include/dfrg.h, dfrg_integrate_twopoint_noalloc):
+    for hosts that may not call cudaMalloc -- all memory owned by another allocator, allocation-lock-free threads, jobs
+    under a memory cap.  The kernels' scratch is a fixed NOALLOC_SCRATCH_BYTES array inside libdfrg.so; a call that needs
+    more raises DfrgError with status DFRG_ESCRATCH.  Same arguments and bit-identical results as the two-point case of
+    dfrg_integrate_loop4d.  One array per device: do not let two such calls overlap on the GPU.  Make the first call on a
+    device outside stream capture (it looks the array's address up)."""
+    D = _loop4d_desc(LOOP_TWOPOINT, prefactor, reg_kind, reg_order, k, rule_q, rule_c1, None, None, (Z,), lnq_lo, lnq_hi,
+                     interp, coef, True, 0, dout_dm2, reg_zk, reg_eta, None)
+    _check(lib().dfrg_integrate_twopoint_noalloc(C.byref(D), _n(m2), _ptr(m2, True), _n(ext), _ptr(ext, True),
+                                                 _ptr(out, True), _ptr(dmin, True), _stream()),
+           "dfrg_integrate_twopoint_noalloc")
     return out
 
 

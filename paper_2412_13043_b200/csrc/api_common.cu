@@ -201,6 +201,7 @@ const char* dfrg_strerror(int status) {
     case DFRG_EUNSUPPORTED: return "unsupported size, dimension or device";
     case DFRG_ECUDA: return "CUDA runtime error (see dfrg_last_cuda_error)";
     case DFRG_ENOMEM: return "device arena allocation failed";
+    case DFRG_ESCRATCH: return "call needs more scratch than the fixed array of the no-allocation entry point holds";
     default: return "unknown status";
   }
 }

@@ -1,4 +1,5 @@
 // loop4d_twopoint.cu -- two-point family of dfrg_integrate_loop4d (BASELINE.json config 2).
+#include <mutex>
 #include <type_traits>
 
 #include "loop4d_kernels.cuh"
@@ -400,4 +401,109 @@ int twopoint_launch(const dfrg_loop4d_desc* D, int n_field, const double* m2, in
   return rc;
 }
 
+
+// ---- the entry point that allocates nothing -------------------------------------------------------------------------
+// twopoint_launch() above takes its scratch (per-chunk denominator minima and per-CTA partial sums) from the library's
+// stream-ordered memory pool.  Some hosts of this library may not allocate device memory at the moment they call it: a
+// flow-equation right-hand side evaluated inside a solver that has already handed the whole GPU to its own allocator, a
+// call made from a thread that must not take the driver's allocation lock (a real-time or callback context), or a process
+// running under a memory cap where any cudaMalloc may fail.  For those callers the same two kernels run here with their
+// scratch in an array that is part of the library image: it is there from the moment the library is loaded on a device
+// until the process exits, on EVERY device that loads the library, whether or not this entry point is ever called
+// (DFRG_NOALLOC_SCRATCH_BYTES each).
+//
+// In host code the name g_tp_fixed_scratch is only a handle for the runtime, not a device address; the address the
+// kernels need is asked for once per device with cudaGetSymbolAddress (with that device current) and cached.
+static __device__ __align__(256) double g_tp_fixed_scratch[DFRG_NOALLOC_SCRATCH_BYTES / sizeof(double)];
+
+static std::mutex g_fixed_mutex;
+static double* g_fixed_addr[64] = {};   // per device: device address of g_tp_fixed_scratch, nullptr = not asked yet
+
+static int fixed_scratch_address(double** addr) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return check_cuda(e);
+  if (dev < 0 || dev >= 64) return DFRG_EUNSUPPORTED;
+  std::lock_guard<std::mutex> lock(g_fixed_mutex);
+  if (!g_fixed_addr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_tp_fixed_scratch);   // the current device's copy of the array
+    if (e != cudaSuccess) return check_cuda(e);
+    if (!p) return DFRG_ECUDA;
+    g_fixed_addr[dev] = (double*)p;
+  }
+  *addr = g_fixed_addr[dev];
+  return DFRG_OK;
+}
+
+// Same plan, same kernels, same launch configuration as twopoint_launch (the GPU test asserts bit-identical outputs);
+// only the origin of P.chunkmin / P.part differs.  Keep the two plans in step.
+static int twopoint_launch_fixed_scratch(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext,
+                                         const double* ext, double* out, double* dmin, int sm_count,
+                                         cudaStream_t stream) {
+  TwoPointParams P;
+  P.nq = D->q.n; P.nc = D->cos1.n; P.n_field = n_field; P.n_ext = n_ext;
+  P.prefactor = D->prefactor;
+  fill_common(D->reg, D->tab[0], &P.reg, &P.grid);
+  P.fmc = fm_consts();
+  P.xq = D->q.x; P.wq = D->q.w; P.xc = D->cos1.x; P.wc = D->cos1.w; P.Z = D->tab[0].v;
+  P.coef = D->coef; P.m2 = m2; P.pext = ext; P.out = out; P.dmin = dmin; P.dout = D->dout_dm2;
+  const int mf = n_field > TP_FT ? 2 : 1;
+  P.tile = TP_FT * mf;
+  int qc = TP_CHUNK_NODES / P.nc;
+  qc = qc > 8 ? 8 : qc;
+  qc = qc > P.nq ? P.nq : qc;
+  P.QC = qc;
+  P.NCH = (P.nq + qc - 1) / qc;
+  const int n_ftiles = (n_field + P.tile - 1) / P.tile;
+  const long long upp = (long long)n_ext * P.NCH, U = (long long)n_ftiles * upp;
+  P.grid_main = (int)(U < sm_count ? U : sm_count);
+  P.max_slots = 1;
+  for (long long seg = 0; seg < (long long)n_ftiles * n_ext; ++seg) {
+    const long long ufirst = seg * P.NCH, ulast = ufirst + P.NCH - 1;
+    const int c0 = (int)(((ufirst + 1) * P.grid_main - 1) / U), c1 = (int)(((ulast + 1) * P.grid_main - 1) / U);
+    if (c1 - c0 + 1 > P.max_slots) P.max_slots = c1 - c0 + 1;
+  }
+  const bool want_d = D->dout_dm2 != nullptr;
+  const size_t n_chunkmin = ((size_t)U * (TP_NPROD / 32) + 2) & ~(size_t)1,
+               n_part = (size_t)P.max_slots * (want_d ? 2 : 1) * n_ext * n_field;
+  if (n_chunkmin + n_part > DFRG_NOALLOC_SCRATCH_BYTES / sizeof(double)) return DFRG_ESCRATCH;   // nothing enqueued
+  const size_t smem_main = tp_main_smem(P.nq, P.nc, P.grid.n, P.QC * P.nc, mf, want_d);
+  if (smem_main > kMaxDynSmem) return DFRG_EUNSUPPORTED;
+  double* fixed = nullptr;
+  int rc = fixed_scratch_address(&fixed);
+  if (rc != DFRG_OK) return rc;
+  // Nothing in the scratch has to start at zero: the main kernel writes every chunkmin entry and every partial-sum slot
+  // that the fix-up kernel reads, so what the previous call left behind is never looked at.
+  P.chunkmin = fixed;
+  P.part = fixed + n_chunkmin;
+  void (*kmain)(const TwoPointParams) =
+      mf == 2 ? (want_d ? tp_main_kernel<2, true> : tp_main_kernel<2, false>)
+              : (want_d ? tp_main_kernel<1, true> : tp_main_kernel<1, false>);
+  rc = opt_in_max_smem(kmain);
+  if (rc != DFRG_OK) return rc;
+  kmain<<<P.grid_main, TP_THREADS, smem_main, stream>>>(P);
+  const long long n_out = (long long)n_ext * n_field;
+  tp_fixup_kernel<<<(unsigned)((n_out + 255) / 256), 256, 0, stream>>>(P);
+  return check_cuda(cudaGetLastError());
+}
+
 }  // namespace dfrg
+
+using namespace dfrg;
+
+// See include/dfrg.h.  Validation is the two-point branch of dfrg_integrate_loop4d's.
+extern "C" int dfrg_integrate_twopoint_noalloc(const dfrg_loop4d_desc* D, int n_field, const double* m2, int n_ext,
+                                               const double* ext, double* out, double* dmin, void* cuda_stream) {
+  if (!D || !ext || !out || n_ext < 1 || n_field < 1 || !m2) return DFRG_EINVAL;
+  if (D->family != DFRG_LOOP_TWOPOINT) return DFRG_EINVAL;
+  if (!valid_regulator(D->reg) || !valid_rule(D->q) || !valid_rule(D->cos1) || !D->coef || D->n_coef != 2 ||
+      !valid_table(D->tab[0], 1))
+    return DFRG_EINVAL;
+  if ((long long)D->q.n * D->cos1.n > TP_MAX_PAIRS || D->cos1.n > TP_CHUNK_NODES || D->tab[0].n_q > 1024)
+    return DFRG_EUNSUPPORTED;
+  int sms = 0;
+  int rc = require_sm100(&sms);
+  if (rc != DFRG_OK) return rc;
+  return twopoint_launch_fixed_scratch(D, n_field, m2, n_ext, ext, out, dmin, sms, (cudaStream_t)cuda_stream);
+}
