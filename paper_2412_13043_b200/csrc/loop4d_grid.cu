@@ -360,7 +360,8 @@ __global__ void __launch_bounds__(NT, 1) t3g_main_kernel(const ThreeGridParams Q
       const double* nS = sm.nodeS + b * NODES;
       const double2* ta = reinterpret_cast<const double2*>(Q.tabA) + ((size_t)(pair0 + w) * G + a) * 4;
       const size_t ta_step = (size_t)nw * G * 4;
-      double2 c01 = ta[0], c23 = ta[1], c45 = ta[2];
+      double2 c01 = make_double2(0.0, 0.0), c23 = c01, c45 = c01;
+      if (active && w < npl) { c01 = ta[0]; c23 = ta[1]; c45 = ta[2]; }   // (idle threads and pair slots beyond the chunk: ta points past tabA)
       for (int pl = w; pl < npl; pl += nw) {
         if (active) {
           const double cur[6] = {c01.x, c01.y, c23.x, c23.y, c45.x, c45.y};

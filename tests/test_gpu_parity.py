@@ -146,7 +146,8 @@ def test_threepoint_small(n_p, n_alpha, n_q, n1, n2, interp):
 
 
 @pytest.mark.parametrize("n_p,n_alpha,n_q,n1,n2,interp", [(3, 2, 20, 10, 6, 3), (5, 3, 33, 9, 5, 1), (7, 1, 40, 12, 16, 3),
-                                                          (2, 2, 6, 3, 200, 3)])
+                                                          (2, 2, 6, 3, 200, 3),
+                                                          (2, 1, 3, 3, 4, 3)])   # 9 (q, c1) pairs: most pair slots of the main kernel idle
 def test_threepoint_product_grid_path(n_p, n_alpha, n_q, n1, n2, interp):
     # the product-grid kernels (ext_outer = n_p promised), the general kernel on the same inputs (no promise), and a
     # false promise (shuffled ext): all three against the oracle; the first two must come from different kernels
