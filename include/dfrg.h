@@ -33,6 +33,9 @@
  *    gives whatever IEEE arithmetic gives; `dmin` reports it (signed minimum over all quadrature
  *    nodes and all propagators of an output of denominator / k^2; reading A4 in DESIGN.md).
  *    An exactly zero denominator yields NaN (the reciprocal is a Newton iteration on a hardware seed).
+ *    NaN inputs: a NaN momentum or mass reaches the output through the Z s + m^2 terms of its denominators; the regulator
+ *    term alone does not carry it (the device e^-x maps a NaN argument to 0, so R(NaN) = 0), which matters only where a
+ *    caller inspects intermediate quantities -- the outputs that depend on the NaN input are NaN either way.
  *    Magnitude range and coupling of the batched reciprocals: the two-point and Matsubara kernels invert the denominators
  *    of the TWO field points a thread owns (f and f + tile/2 of a field tile: f + 128 in the two-point family, f + 256 in
  *    dfrg_integrate_matsubara3d) at one or two neighbouring quadrature nodes jointly, 1/(d_1 d_2 [d_3 d_4]) from one seed.

@@ -30,7 +30,7 @@ __device__ __forceinline__ double fast_rcp(double d) {
 // ---- table-driven FP64 log and exp --------------------------------------------------------------------------
 // The S3 pre-computation is dominated by log (table coordinate) and exp (regulator).  libdevice's versions
 // cost ~100 SASS instructions each, two thirds of them integer/constant traffic.  These versions keep two small
-// tables in shared memory (built once per CTA from libdevice log/exp2, fm_build) and need ~10 FP64 instructions:
+// tables in shared memory (copied per CTA from the correctly rounded literals of fm_tables.inc, fm_build / TMA) and need ~10 FP64 instructions:
 //   fm_log(s):  s = 2^e m, m in [1,2); j = top 7 mantissa bits; r = m * (1/c_j) - 1, |r| <= 2^-8;
 //               ln s = e ln2 + ln c_j + (r - r^2/2 + ... - r^6/6)          abs. error <~ 3e-16 for |e| < 64
 //   fm_exp_neg(x) = e^-x, 0 <= x: n = rint(-64 x / ln2), r = -x - n ln2/64, |r| <= ln2/128;
@@ -389,6 +389,12 @@ __device__ __forceinline__ LogGrid2 lg2_build(double* mem, const LogGrid2Consts&
   L.K = &K;
   return L;
 }
+// Precondition: x >= 0 (or NaN).  The exponent is taken from the high word WITHOUT masking the sign bit (one integer
+// instruction less in the three-point hot loop), so a negative x -- even -0.0 or a rounding-sized negative value -- would
+// come out as a huge t' and land in the LAST cell, where reading A16 (max(s, 0): log 0 clamps to the first entry) wants the
+// first.  Every caller guarantees it: set-up code clamps s at 0 before the call; the product-grid hot loop feeds
+// x = (s_a + s_b + s_c)/3 with s_a, s_c >= 0 fixed per row and s_b = |q + p2|^2 at Gauss-Legendre nodes (|cos| < 1
+// strictly), where the unclamped s_b >= (q - p2)^2 (1 - |cos|) stays far above rounding size relative to the sum.
 __device__ __forceinline__ double lg2_coord(const LogGrid2& L, const double x) {
   const int hi = __double2hiint(x);
   unsigned off;                                   // 128 * (top 9 mantissa bits) + 16 * replica, as ONE three-input LOP3
