@@ -2,7 +2,12 @@
 """bench.py -- measures the loop-integral hot path on B200 (contract: see DESIGN.md "Measurement").
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-others] [--no-cpu-baseline]
-                    [--full] [--report FILE]
+                    [--full] [--report FILE] [--issue-model]
+
+--gpus N > 1: one rank per GPU, weak scaling (64 external momenta per rank, no data-path collective).  Either start the
+ranks yourself (`python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P
+bench.py --gpus N ...`) or run `python bench.py --gpus N ...` plainly: without a launcher environment the script starts
+the N ranks itself, and it refuses to run if fewer than N devices are visible.  Rank 0 prints the line.
 
 A step is one pass of the whole hot path (S1..S6) over one batch: BASELINE.json configs[4], the
 finite-T momentum-dependent loop (64 p x 16 Matsubara indices x 512 field points = 524 288 integrals,
@@ -71,6 +76,14 @@ def cfg4_counts(c, rules):
     per_pif_strict = rows * nc * 12 + (c["n_max"] + 1) * 8 + n_j * n_terms * 9
     units = n_p * nq * n_f
     return n_out, evals, (2.0 * units * per_pif, float(units * per_pif_strict))
+
+
+def cfg4_reciprocals(c, rules):
+    """Reciprocals the moment factorisation executes per step: per (p, radial node, field point) one per boson-line row
+    and cos node and one per fermion-line term (the nominal count `evals` has one propagator pair per (n, q, c) node of
+    every output; the factorisation shares the boson-line reciprocals over the (j, n) pairs with equal |j - n|)."""
+    nq, nc = rules["q"][0].size, rules["c"][0].size
+    return c["pext"].size * nq * c["m2psi"].size * ((c["n_jext"] + c["n_max"]) * nc + c["n_max"] + 1)
 
 
 class ClockSampler:
@@ -149,13 +162,16 @@ def run_reference(args):
 
 
 def alu_roofline(alg_instr, alg_flops_strict, ms, peak, what):
-    """roofline block of an FP64-pipe-bound kernel: algorithmic FP64 instructions x 2 = DFMA-slot
-    equivalents (a DADD/DMUL holds the pipe as long as a DFMA) against the nominal FP64 peak; strict = FMA 2, add/mul 1."""
-    ach = 2.0 * alg_instr / (ms * 1e-3) * 1e-12
+    """roofline block of an FP64-pipe-bound kernel.  `achieved` / `frac`: algorithmic flops counted strictly (FMA 2,
+    add / mul 1) against the nominal FP64 peak in TFLOP/s.  `fp64_pipe_utilisation`: algorithmic FP64
+    instructions / the pipe's issue slots in the measured time (a DADD or DMUL holds the pipe as long as a DFMA) -- the
+    figure ncu's sm__pipe_fp64_cycles_active measures, and the one the >= 50 % target of SURVEY 8(d) is worded on."""
     strict = alg_flops_strict / (ms * 1e-3) * 1e-12
-    return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-            "achieved_strict": strict, "frac_strict": strict / peak, "alg_fp64_instr_per_launch": alg_instr,
-            "achieved_kind": what}
+    slots = 2.0 * alg_instr / (ms * 1e-3) * 1e-12
+    return {"bound": "alu", "achieved": strict, "peak": peak, "unit": "TFLOP/s", "frac": strict / peak,
+            "achieved_kind": "algorithmic flops, FMA = 2, add / mul = 1 (" + what + ")",
+            "fp64_pipe_utilisation": slots / peak, "alg_fp64_instr_per_launch": alg_instr,
+            "alg_fp64_instr_per_s": alg_instr / (ms * 1e-3), "alg_flops_per_launch": alg_flops_strict}
 
 
 def time_other_configs(torch, B, inputs, make_rules, peak, iters=5):
@@ -326,6 +342,64 @@ def time_other_configs(torch, B, inputs, make_rules, peak, iters=5):
     return out
 
 
+def rank_env(n_gpus_arg):
+    """(rank, world, local rank) of this process from the launcher's environment (torchrun sets RANK / WORLD_SIZE /
+    LOCAL_RANK); a plain single-process run is rank 0 of 1.  --gpus must agree with the world size."""
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", str(rank)))
+    if not (0 <= rank < world):
+        raise SystemExit("bench.py: RANK %d outside WORLD_SIZE %d" % (rank, world))
+    if n_gpus_arg != world:
+        raise SystemExit("bench.py: --gpus %d but the launcher started %d rank(s)" % (n_gpus_arg, world))
+    return rank, world, local
+
+
+def rank_workload(inputs, shard_bounds, world, rank):
+    """This rank's share of the global batch.  Weak scaling: the global batch has 64 x world external momenta on the same
+    log range; rank r integrates its contiguous block; no data-path collective."""
+    c = inputs.config4(n_p=64 * world)
+    lo_p, hi_p = shard_bounds(c["pext"].size, world, rank)
+    c["pext_global_range"] = (lo_p, hi_p)
+    c["pext"] = np.ascontiguousarray(c["pext"][lo_p:hi_p])
+    return c
+
+
+def max_over_ranks(x, dist, device):
+    """MAX over ranks of a per-rank time (the job is as slow as its slowest rank); dist = None: single process."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(world, units_per_rank, ms):
+    """units per second over ALL ranks: every rank processed units_per_rank in the (max-over-ranks) time ms."""
+    return world * units_per_rank / (ms * 1e-3)
+
+
+def launch_ranks(n, argv):
+    """`python bench.py --gpus N` with N > 1 and no launcher environment: starts N ranks (one per GPU) of this script under
+    torch.distributed.run on 127.0.0.1 and returns its exit code.  Rank 0 prints the JSON line.  NCCL's communicator set-up
+    lines go to stderr (NCCL_DEBUG=INFO, INIT subsystem) unless the caller has set NCCL_DEBUG."""
+    import socket
+    import torch
+    have = torch.cuda.device_count()
+    if have < n:
+        raise SystemExit("bench.py --gpus %d: only %d CUDA device(s) visible; refusing to run fewer ranks than asked" % (n, have))
+    with socket.socket() as sock:
+        sock.bind(("127.0.0.1", 0))
+        port = sock.getsockname()[1]
+    env = dict(os.environ)
+    if "NCCL_DEBUG" not in env:
+        env.update(NCCL_DEBUG="INFO", NCCL_DEBUG_SUBSYS="INIT", NCCL_DEBUG_FILE="/dev/stderr")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n), "--master-addr",
+           "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+    return subprocess.call(cmd, env=env)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -336,10 +410,14 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--full", action="store_true", help="compare every output of the workload with the CPU oracle")
     ap.add_argument("--report", default=None, help="write the oracle comparison as JSON to this file")
+    ap.add_argument("--issue-model", action="store_true",
+                    help="also run the FP64 issue-model probe (DESIGN.md section 7) and add it to the roofline block")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return launch_ranks(args.gpus, sys.argv[1:])         # `python bench.py --gpus N`: start the N ranks ourselves
 
     import torch
     from paper_2412_13043_b200 import binding as B
@@ -347,11 +425,12 @@ def main():
     from paper_2412_13043_b200.inputs import make_rules
     from paper_2412_13043_b200.shard import shard_bounds
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = rank_env(args.gpus)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    if torch.cuda.device_count() <= local:
+        raise SystemExit("bench.py: rank %d wants cuda:%d but only %d device(s) are visible" %
+                         (rank, local, torch.cuda.device_count()))
     torch.cuda.set_device(local)
     dist = None
     if world > 1:
@@ -361,9 +440,7 @@ def main():
 
     # ---- workload (weak scaling: the global batch has 64 x N external momenta on the same log range; every
     # rank integrates its contiguous block of 64; no data-path collective) ----
-    c = inputs.config4(n_p=64 * world)
-    lo_p, hi_p = shard_bounds(c["pext"].size, world, rank)
-    c["pext"] = np.ascontiguousarray(c["pext"][lo_p:hi_p])
+    c = rank_workload(inputs, shard_bounds, world, rank)
     t_s1 = time.perf_counter()
     R = make_rules(c, B.dfrg_quad_nodes)                     # S1, host
     t_s1 = time.perf_counter() - t_s1
@@ -396,7 +473,7 @@ def main():
     b.record()
     b.synchronize()
     probe_tflops = probe_flops / (a.elapsed_time(b) * 1e-3) * 1e-12
-    issue_model = probe.fp64_issue_model(sink)                # 8 DFMA + {0, 4, 8} integer adds: DESIGN.md section 7
+    issue_model = probe.fp64_issue_model(sink) if args.issue_model else None   # 8 DFMA + K other instructions: DESIGN.md section 7
 
     for _ in range(args.warmup):
         step()
@@ -422,12 +499,8 @@ def main():
     t_wall = time.perf_counter() - t_wall
     clocks = sampler.stop()
     ms_local = sum(e0.elapsed_time(e1) for e0, e1 in evs) / args.steps
-    ms = ms_local
-    if dist is not None:
-        t = torch.tensor([ms_local], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * evals / (ms * 1e-3)
+    ms = max_over_ranks(ms_local, dist, "cuda")
+    value = whole_job_rate(world, evals, ms)
 
     # ---- e2e: host buffers through the C ABI, S1 + H2D + kernel + D2H inside the timed region ----
     pin = lambda a: torch.as_tensor(np.ascontiguousarray(a)).pin_memory()
@@ -452,10 +525,7 @@ def main():
         e2e_step()
     barrier()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
-    if dist is not None:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, dist, "cuda")
     rows_psi, rows_phi = c["n_max"] + 1, c["n_jext"] + c["n_max"]
     h2d = 8 * (2 * (R["q"][0].size + R["c"][0].size) + (rows_psi + rows_phi) * c["Zpsi"].shape[1] + 20 +
                2 * c["m2psi"].size + c["pext"].size)
@@ -470,35 +540,47 @@ def main():
     sm_max_mhz = clocks.get("sm_max_mhz") or 1965.0
     sms = torch.cuda.get_device_properties(local).multi_processor_count
     peak = sms * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 * 1e-12          # TFLOP/s at max clock
-    achieved = flops / (ms_local * 1e-3) * 1e-12
+    roof = alu_roofline(flops / 2.0, flops_strict, ms_local, peak,
+                        "moment factorisation: 7 FP64 instr per (boson row, cos node), 5 per fermion term, 5 per (j, n), "
+                        "each per (p, radial node, field point)")
+    alg_bytes = 8 * c["pext"].size * rows_phi * R["q"][0].size * R["c"][0].size
+    roof.update({
+        "kernel": "mats3d_moment_kernel (+ the two pre-pass kernels and the fix-up kernel, timed together)",
+        "traffic": ncu_dram_bytes_per_launch() if world == 1 else None,
+        "traffic_kind": "MOMENT KERNEL ONLY: dram__bytes_read.sum + dram__bytes_write.sum of mats3d_moment_kernel per launch, a "
+                        "constant read at run time from the committed ncu --set full capture of this workload (" + NCU_CAPTURE +
+                        "), not measured by this run; its algorithmic bytes are the D0phi chunks [p][27 rows][q][c], read once",
+        "alg_bytes_per_launch": alg_bytes,
+        "alg_bytes_per_step": 2 * alg_bytes + 8 * n_out,
+        "alg_bytes_per_step_kind": "the pre-pass writes the D0phi table, the moment kernel reads it once, the fix-up writes the "
+                                   "outputs (partial sums and the small tables stay in L2): about 68 MB, 1 % of the HBM "
+                                   "bandwidth at this step time",
+        "alg_fp64_instr_per_nominal_eval": flops / 2.0 / evals,
+        "peak_kind": "nominal FP64: %d SMs x %d lanes x 2 x %.0f MHz (MEASURED_PEAKS.json has no FP64 "
+                     "entry)" % (sms, FP64_LANES_PER_SM, sm_max_mhz),
+        "peak_probe_tflops": probe_tflops, "frac_of_probe": roof["achieved"] / probe_tflops})
+    if issue_model is not None:
+        roof["issue_model_probe"] = dict(issue_model, kind="time of 8 DFMA chains + K instructions of another pipe per 8 DFMA "
+                                         "(integer add, I2F.F64, LDS.128) relative to K = 0; integer-add ratios "
+                                         "(16 + K)/16 would mean an FP64 instruction holds the issue port for 2 "
+                                         "cycles, ratios of 1 that other instructions issue in its shadow")
+    n_recip = cfg4_reciprocals(c, R)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
+            "value_kind": "NOMINAL integrand evaluations (one per output and (n, q, c) node, the count BASELINE.json's metric "
+                          "names); the executed work after the exact moment factorisation is in executed_reciprocals_per_s "
+                          "and alg_fp64_instr_per_s",
+            "executed_reciprocals_per_s": whole_job_rate(world, n_recip, ms),
+            "alg_fp64_instr_per_s": whole_job_rate(world, flops / 2.0, ms),
             "config": {"workload": WORKLOAD, "l2": "flushed between timed steps (256 MiB fill)",
                        "parallelism": "external momenta sharded over GPUs (64 per GPU), no collective",
                        "integrals_per_step_per_gpu": n_out, "nominal_evals_per_step_per_gpu": evals},
-            "integrals_per_s": world * n_out / (ms * 1e-3),
+            "integrals_per_s": whole_job_rate(world, n_out, ms),
             "clocks": clocks, "gpu_launches": 5 * args.steps,  # phi-rows pre-pass, psi pre-pass, the two moment kernels (one returns at once), fix-up
-            "e2e": {"value": world * evals / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "ms_per_step": e2e_s * 1e3, "s1_host_ms": t_s1 * 1e3},
-            "roofline": {"bound": "alu", "kernel": "mats3d_moment_kernel (+ the two pre-pass kernels and the fix-up kernel, timed together)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                         "frac": achieved / peak, "traffic": ncu_dram_bytes_per_launch() if world == 1 else None,
-                         "traffic_kind": "dram__bytes_read.sum + dram__bytes_write.sum of mats3d_moment_kernel per launch, read "
-                                         "at run time from the committed ncu --set full capture of this workload (" +
-                                         NCU_CAPTURE + "); algorithmic bytes: the D0phi chunks [p][27 rows][q][c], read once",
-                         "alg_bytes_per_launch": 8 * c["pext"].size * rows_phi * R["q"][0].size * R["c"][0].size,
-                         "achieved_kind": "algorithmic FP64 instructions x 2 (DFMA-slot equivalents) / event time",
-                         "achieved_strict": flops_strict / (ms_local * 1e-3) * 1e-12,
-                         "frac_strict": flops_strict / (ms_local * 1e-3) * 1e-12 / peak,
-                         "alg_fp64_instr_per_nominal_eval": flops / 2.0 / evals,
-                         "peak_kind": "nominal FP64: %d SMs x %d lanes x 2 x %.0f MHz (MEASURED_PEAKS.json has no FP64 "
-                                      "entry)" % (sms, FP64_LANES_PER_SM, sm_max_mhz),
-                         "peak_probe_tflops": probe_tflops, "frac_of_probe": achieved / probe_tflops,
-                         "issue_model_probe": dict(issue_model, kind="time of 8 DFMA chains + K instructions of another pipe per 8 DFMA "
-                                                   "(integer add, I2F.F64, LDS.128) relative to K = 0; integer-add ratios "
-                                                   "(16 + K)/16 would mean an FP64 instruction holds the issue port for 2 "
-                                                   "cycles, ratios of 1 that other instructions issue in its shadow"),
-                         "alg_flops_per_launch": flops},
+            "e2e": {"value": whole_job_rate(world, evals, e2e_s * 1e3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "s1_host_ms": t_s1 * 1e3},
+            "roofline": roof,
             "wall_s_timed_region": t_wall}
 
     if not args.no_others and world == 1:
