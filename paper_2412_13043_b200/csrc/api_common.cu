@@ -4,8 +4,8 @@
 #include <stdint.h>
 #include <string.h>
 
+#include <map>
 #include <mutex>
-#include <set>
 #include <utility>
 
 #include "dfrg_internal.h"
@@ -43,14 +43,18 @@ int require_sm100(int* sm_count) {
 }
 
 static std::mutex g_attr_mutex;
-static std::set<std::pair<int, const void*>> g_attr_done;
-int opt_in_max_smem_impl(const void* kernel) {
+static std::map<std::pair<int, const void*>, size_t> g_attr_done;   // (device, kernel) -> its dynamic shared-memory limit
+int opt_in_max_smem_impl(const void* kernel, size_t* limit) {
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return check_cuda(e);
   std::lock_guard<std::mutex> lock(g_attr_mutex);
   const std::pair<int, const void*> key(dev, kernel);
-  if (g_attr_done.count(key)) return DFRG_OK;
+  const auto it = g_attr_done.find(key);
+  if (it != g_attr_done.end()) {
+    if (limit) *limit = it->second;
+    return DFRG_OK;
+  }
   // the opt-in limit covers static + dynamic shared memory: leave room for the kernel's own static part
   cudaFuncAttributes fa;
   e = cudaFuncGetAttributes(&fa, kernel);
@@ -58,9 +62,11 @@ int opt_in_max_smem_impl(const void* kernel) {
   int optin = 0;
   e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   if (e != cudaSuccess) return check_cuda(e);
-  e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes);
+  const int dyn = optin - (int)fa.sharedSizeBytes;
+  e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn);
   if (e != cudaSuccess) return check_cuda(e);
-  g_attr_done.insert(key);
+  g_attr_done[key] = (size_t)dyn;
+  if (limit) *limit = (size_t)dyn;
   return DFRG_OK;
 }
 

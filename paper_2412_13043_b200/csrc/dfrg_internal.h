@@ -25,10 +25,14 @@ int require_sm100(int* sm_count);
 // raised to its own limit (opt-in maximum - its static part) ONCE per device (kernel attributes are per device) --
 // never per call and never to a per-call size, so concurrent callers cannot lower each other's limit between the set
 // and the launch.
+// A kernel with more than 1 KB of static shared memory (the LPA kernels' reduction scratch: 3-6 KB) has a smaller limit
+// than kMaxDynSmem: its launcher asks for the exact figure (`limit`) and compares before it launches.
 constexpr size_t kMaxDynSmem = 226 * 1024;
-int opt_in_max_smem_impl(const void* kernel);   // DFRG_OK / DFRG_ECUDA; thread-safe, cached per (device, kernel)
+int opt_in_max_smem_impl(const void* kernel, size_t* limit);   // DFRG_OK / DFRG_ECUDA; thread-safe, cached per (device, kernel)
 template <typename K>
-inline int opt_in_max_smem(K kernel) { return opt_in_max_smem_impl(reinterpret_cast<const void*>(kernel)); }
+inline int opt_in_max_smem(K kernel, size_t* limit = nullptr) {   // *limit: the most dynamic shared memory `kernel` may be launched with
+  return opt_in_max_smem_impl(reinterpret_cast<const void*>(kernel), limit);
+}
 
 inline bool valid_regulator(const dfrg_regulator& r) {
   if (!(r.k > 0.0) || !(r.zk > 0.0) || !(r.eta == r.eta)) return false;

@@ -268,8 +268,10 @@ static int lpa_launch(const dfrg_lpa_desc* D, int n_T, const double* Tv, const i
   auto kern = fermi ? (D->dchan ? lpa_fermion_kernel<true> : lpa_fermion_kernel<false>)
                     : (D->dchan ? lpa_kernel<true> : lpa_kernel<false>);
   if (smem > kMaxDynSmem) return DFRG_EUNSUPPORTED;   // (lpa_validate bounds the table; this is the exact size)
-  const int rca = opt_in_max_smem(kern);
+  size_t smem_limit = 0;   // 227 KB minus this kernel's static shared memory (3-6 KB of reduction scratch)
+  const int rca = opt_in_max_smem(kern, &smem_limit);
   if (rca != DFRG_OK) return rca;
+  if (smem > smem_limit) return DFRG_EUNSUPPORTED;    // nothing enqueued
   const dim3 grid((n_field + LPA_FTILE - 1) / LPA_FTILE, n_T);
   kern<<<grid, LPA_THREADS, smem, stream>>>(P);
   return check_cuda(cudaGetLastError());

@@ -102,3 +102,32 @@ def test_fermion_litim_fermi_function_closed_form_on_gpu():
     tail = c["prefactor"] * (2.0 / 3.0) / (2 * math.pi ** 2 * T * c["n_max"])
     assert np.all(np.abs(g["chan"][ok] - ref) <= 1.5 * tail)
     assert np.max(np.abs(g["chan"][ok] - ref)) > 0.2 * tail     # and the tail is really there (truncated sum, as the oracle)
+
+
+def test_lpa_table_between_the_kernel_limit_and_the_library_limit_is_unsupported():
+    # The LPA kernels hold 3-6 KB of static shared memory, so their dynamic limit lies below the library-wide 226 KB
+    # bound that validation applies: 48 n_q + 2560 bytes (fermionic, one Matsubara term) fit the bound up to n_q = 4768
+    # but the kernel only up to ~4660.  In between the call used to fail at launch (DFRG_ECUDA); the header promises
+    # DFRG_EUNSUPPORTED with nothing written.  Just below the kernel's limit the call works.
+    import torch
+    from paper_2412_13043_b200 import binding as B
+
+    def call(n_q, statistics):
+        c = inputs.config1(0.2, n_field=9, n_q=n_q)
+        _, a, b = c["rule_q"]                    # dfrg_quad_nodes stops at 4096 nodes: a composite rule of two panels
+        halves = [B.dfrg_quad_nodes(n_q // 2, a, 0.5 * (a + b)), B.dfrg_quad_nodes(n_q - n_q // 2, 0.5 * (a + b), b)]
+        xq, wq = (np.concatenate([h[i] for h in halves]) for i in (0, 1))
+        up = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+        flow = torch.full((9,), -3.5, dtype=torch.float64, device="cuda")
+        B.dfrg_integrate_lpa(c["d"], c["T"], 0, 0, c["N"], c["prefactor"], c["reg_kind"], c["reg_order"], c["k"],
+                             (up(xq), up(wq)), up(c["rho"]), up(c["u"]), up(c["du"]), flow, None, None,
+                             statistics=statistics, mu=0.0)
+        torch.cuda.synchronize()
+        return flow
+
+    for stat, n_fits, n_between in ((B.STAT_FERMION, 4600, 4720), (B.STAT_BOSON, 6800, 7120)):
+        assert bool(torch.isfinite(call(n_fits, stat)).all())
+        with pytest.raises(B.DfrgError) as err:
+            call(n_between, stat)
+        assert err.value.status == B.DFRG_EUNSUPPORTED
+    assert bool(torch.isfinite(call(64, B.STAT_FERMION)).all())     # the library is still usable afterwards
