@@ -36,13 +36,18 @@
  *    NaN inputs: a NaN momentum or mass reaches the output through the Z s + m^2 terms of its denominators; the regulator
  *    term alone does not carry it (the device e^-x maps a NaN argument to 0, so R(NaN) = 0), which matters only where a
  *    caller inspects intermediate quantities -- the outputs that depend on the NaN input are NaN either way.
- *    Magnitude range and coupling of the batched reciprocals: the two-point and Matsubara kernels invert the denominators
- *    of the TWO field points a thread owns (f and f + tile/2 of a field tile: f + 128 in the two-point family, f + 256 in
- *    dfrg_integrate_matsubara3d) at one or two neighbouring quadrature nodes jointly, 1/(d_1 d_2 [d_3 d_4]) from one seed.
- *    Every denominator must therefore satisfy 1e-75 k^2 < |D| < 1e75 k^2 (the product of four stays inside the double
- *    range; physical denominators lie between ~1e-3 k^2 and ~1e6 k^2), and a denominator that is exactly zero, subnormal,
- *    infinite or NaN at field point f makes the output of its partner field point NaN as well (the partner's own dmin does
- *    not show it: check dmin of both).  dfrg_mats3d_desc::path = DFRG_M3_ONE_FIELD inverts every field point on its own.
+ *    Field points are independent outputs, also where the kernels batch: the two-point and Matsubara kernels invert the
+ *    denominators of the TWO field points a thread owns (f and f + 128, resp. f + 256 of a field tile) through one product,
+ *    1/(d_1 d_2 [d_3 d_4]) from one hardware seed.  A field point whose mass term has blown up -- NaN, infinite, or beyond
+ *    1e150 (two-point) / 1e70 (Matsubara) in magnitude, where the product would overflow -- is detected from the masses
+ *    before the loop starts and its thread inverts every denominator on its own: that field point gets what IEEE arithmetic
+ *    gives for it, its partner its own regular value, as in the oracle
+ *    (tests/test_gpu_parity.py::test_field_points_are_independent_outputs_also_where_reciprocals_are_batched).
+ *    What remains coupled: a denominator D0 + m2 that is EXACTLY zero at a quadrature node (D0 and -m2 equal bit for bit;
+ *    a mere sign change between nodes is not this case) yields NaN for the partner field point as well, and the partner's
+ *    own dmin does not show it (data-dependent tests inside the hot loop were measured at 2-4 % of the kernel time and left
+ *    out).  The field-independent part D0 of every denominator must stay below ~1e75 in magnitude (physical values lie
+ *    between ~1e-3 k^2 and ~1e6 k^2).  dfrg_mats3d_desc::path = DFRG_M3_ONE_FIELD never batches across field points.
  *  - Mass derivatives (Jacobian support; the paper's "AD" kernels for implicit time-steppers, PAPER.md:713-723
  *    eq. 27 and PAPER.md:1842): every descriptor of a family with a field axis carries nullable output pointers
  *    for the derivative of each integral with respect to the mass term of its propagators,

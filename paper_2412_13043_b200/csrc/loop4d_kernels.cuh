@@ -14,6 +14,7 @@ constexpr int TP_NCONS = TP_FT * TP_GROUPS;   // 512
 constexpr int TP_NPROD = 128;                 // 4 producer warps
 constexpr int TP_THREADS = TP_NCONS + TP_NPROD;
 constexpr int TP_MAX_PAIRS = 12288;
+constexpr double TP_JOINT_MASS_MAX = 1e150;   // (1e150 + |D0|)^2 stays finite for every |D0| < 1e153
 constexpr int TP_CHUNK_NODES = 2048;          // most (radial x angular) nodes of a unit: 32 KB per stage
 
 struct TwoPointParams {

@@ -201,6 +201,7 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
   const bool warp_leader = (tid & 31) == 0;
   double m2[MF], acc[MF], dacc[MF];
   int cur_ft = -1, seg_parity = 0;
+  bool solo = false;   // this thread inverts every denominator on its own (close_row)
   uint32_t g = 0;
   for (long long u = u0; u < u1; ++u, ++g, next_unit()) {
     const int ft = ft_u, e = e_u, ch = ch_u;
@@ -213,6 +214,9 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
         const int f = f0 + k * TP_FT;
         m2[k] = (f < P.n_field) ? P.m2[f] : 1.0;
       }
+      if constexpr (MF == 2)   // a padding lane beside a real field point: the real one's mass (its joint products are then its own)
+        if (f0 + TP_FT >= P.n_field && f0 < P.n_field) m2[1] = m2[0];
+      if constexpr (MF == 2) solo = !(fabs(m2[0]) < TP_JOINT_MASS_MAX) || !(fabs(m2[1]) < TP_JOINT_MASS_MAX);
     }
     if (u == u0 || ch == 0) {
 #pragma unroll
@@ -223,14 +227,41 @@ __global__ void __launch_bounds__(TP_THREADS, 1) tp_main_kernel(const TwoPointPa
     const int i0 = ch * QC;
     const int ni = min(QC, nq - i0);
     // radial node il of the chunk:  acc_f += Wq G(q)^2 A_f
-    auto close_row = [&](const int il, const double (&A)[MF], const double (&B)[MF]) {
+    auto close_row = [&](const int il, double (&A)[MF], double (&B)[MF]) {
       const double2 o = souter[i0 + il];
+      double gq[MF], wg2[MF];
 #pragma unroll
       for (int k = 0; k < MF; ++k) {
-        const double gq = fast_rcp(o.x + m2[k]);
-        const double wg2 = o.y * (gq * gq);
-        acc[k] = fma(wg2, A[k], acc[k]);
-        if constexpr (WANT_D) dacc[k] = fma(wg2, fma(2.0 * gq, A[k], B[k]), dacc[k]);
+        gq[k] = fast_rcp(o.x + m2[k]);
+        wg2[k] = o.y * (gq[k] * gq[k]);
+      }
+      if constexpr (MF == 2) {
+        // Field points are independent outputs (reading A4), but tp_batch inverts the denominators of the thread's two
+        // field points at a node through their product.  A field point whose mass term has blown up (NaN, infinite, or so
+        // large that the product overflows) would spoil its partner's reciprocals too; the masses are fixed per thread, so
+        // such a thread (`solo`, known long before the row ends: no cost) redoes each row with one reciprocal per
+        // denominator.  The blown-up field point gets what IEEE arithmetic gives for it, its partner its own regular
+        // value.  Not covered: a denominator that is EXACTLY zero at a node still costs the partner's output as well.
+        if (solo) {
+          const double2* row = chunk + il * nc;
+#pragma unroll
+          for (int k = 0; k < MF; ++k) { A[k] = 0.0; B[k] = 0.0; }
+#pragma unroll 1
+          for (int j = 0; j < nc; ++j) {
+            const double2 t = row[j];
+#pragma unroll
+            for (int k = 0; k < MF; ++k) {
+              const double r = fast_rcp(t.x + m2[k]);
+              A[k] = fma(t.y, r, A[k]);
+              if constexpr (WANT_D) B[k] = fma(t.y * r, r, B[k]);
+            }
+          }
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < MF; ++k) {
+        acc[k] = fma(wg2[k], A[k], acc[k]);
+        if constexpr (WANT_D) dacc[k] = fma(wg2[k], fma(2.0 * gq[k], A[k], B[k]), dacc[k]);
       }
     };
     int il = grp;

@@ -445,6 +445,50 @@ __device__ __forceinline__ void mats3d_recip_batch(const double* __restrict__ dp
   }
 }
 
+// Field points are independent outputs (reading A4: whatever IEEE arithmetic gives, PER OUTPUT), but mats3d_recip_batch
+// inverts the denominators of a thread's two field points at two neighbouring nodes through ONE product.  A field point
+// whose mass term has blown up (NaN, infinite, or so large that the product of four denominators overflows) would spoil
+// the reciprocals of its partner as well.  The masses are fixed per thread and field tile, so this is known before the
+// unit starts: `solo` is set where either mass is not below M3_JOINT_MASS_MAX in magnitude, and such a thread redoes every
+// row with one Newton reciprocal per denominator, as the one-field-point kernels do (a branch on a flag that has long
+// been known: measured cost nil.  Flags derived from the data inside the loop -- the hardware seeds of the products, or
+// the finished moments -- cost 4.2 % and 2.3 % of the bench kernel's time: integer work and a branch at the end of the
+// dependent chain are not free at two warps per scheduler).  The blown-up field point gets what IEEE arithmetic gives
+// for it, its partner its own regular value.  Not covered: a denominator D0 + m2 that is EXACTLY zero at a node (D0 and
+// -m2 equal bit for bit) still costs the partner's output too; include/dfrg.h says so.
+constexpr double M3_JOINT_MASS_MAX = 1e70;   // (1e70 + |D0|)^4 stays finite for every |D0| < 1e76
+template <int MF, bool SQ, bool SYM>
+__device__ __forceinline__ void mats3d_row_decouple(const double* __restrict__ drow, const double4* __restrict__ num4,
+                                                    const int nc, const double (&m2phi)[MF], double (&M)[4][MF],
+                                                    const bool solo) {
+  if constexpr (MF == 2) {
+    if (solo) {
+#pragma unroll
+      for (int k = 0; k < MF; ++k) { M[0][k] = 0.0; M[1][k] = 0.0; M[2][k] = 0.0; M[3][k] = 0.0; }
+#pragma unroll 1
+      for (int c = 0; c < nc; ++c) {
+        const double D0 = drow[c];
+        double4 w;
+        if constexpr (SYM) {   // pair-ordered chunk (x-, x+), one weight vector (w, w x+, w x+^2, w x+^3) per pair
+          w = num4[c >> 1];
+          if (!(c & 1)) { w.y = -w.y; w.w = -w.w; }
+        } else {
+          w = num4[c];
+        }
+#pragma unroll
+        for (int k = 0; k < MF; ++k) {
+          double r = fast_rcp(D0 + m2phi[k]);
+          if constexpr (SQ) r = -(r * r);
+          M[0][k] = fma(w.x, r, M[0][k]);
+          M[1][k] = fma(w.y, r, M[1][k]);
+          M[2][k] = fma(w.z, r, M[2][k]);
+          M[3][k] = fma(w.w, r, M[3][k]);
+        }
+      }
+    }
+  }
+}
+
 // M_b += sum_t w[t].b r[t]  for a batch of M3_NBAT nodes (w = wc c^b, broadcast from shared memory).
 template <int MF>
 __device__ __forceinline__ void mats3d_moment_accumulate(const double4* __restrict__ w4, const double (&r)[M3_NBAT][MF],
@@ -631,6 +675,7 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
   const double4* num4 = reinterpret_cast<const double4*>(numbuf);
   double m2psi[MF], m2phi[MF], acc[NJ][MF];
   int cur_ft = -1;
+  bool solo = false;   // this thread inverts every denominator on its own (mats3d_row_decouple)
   uint32_t g = 0;
   // unit u = (ft, e, i), decoded once (64-bit divisions cost ~100 instructions each) and advanced incrementally
   int ft_u = (int)(u0 / upp);
@@ -652,6 +697,9 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
         m2psi[k] = (f < P.n_field) ? P.m2psi[f] : 1.0;
         m2phi[k] = (f < P.n_field) ? P.m2phi[f] : 1.0;
       }
+      if constexpr (MF == 2)   // a padding lane beside a real field point: the real one's masses (its joint products are then its own)
+        if (f0 + NTC >= P.n_field && f0 < P.n_field) { m2psi[1] = m2psi[0]; m2phi[1] = m2phi[0]; }
+      if constexpr (MF == 2) solo = !(fabs(m2phi[0]) < M3_JOINT_MASS_MAX) || !(fabs(m2phi[1]) < M3_JOINT_MASS_MAX);
     }
     if (u == u0 || i == 0) {
 #pragma unroll
@@ -742,6 +790,7 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_moment_kernel(const Mats3dParam
           }
         }
       }
+      if (pipelined) mats3d_row_decouple<MF, SQ, SYM>(d0 + m * nc, num4, nc, m2phi, M, solo);
       // ---- the (j, n) pairs with |j - n| = m: compile-time code per m (static register indices), reached through
       // a jump table so that the moment loop above exists once in the instruction stream ----
       switch (m) {
@@ -900,6 +949,7 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_gmoment_kernel(const Mats3dPara
   double* myH = Hs + (size_t)tid * MF;
   double m2psi[MF], m2phi[MF], acc[NJ][MF];
   int cur_ft = -1;
+  bool solo = false;   // this thread inverts every denominator on its own (mats3d_row_decouple)
   uint32_t g = 0;
   // unit u = (ft, e, i), decoded once (64-bit divisions cost ~100 instructions each) and advanced incrementally
   int ft_u = (int)(u0 / upp);
@@ -921,6 +971,9 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_gmoment_kernel(const Mats3dPara
         m2psi[k] = (f < P.n_field) ? P.m2psi[f] : 1.0;
         m2phi[k] = (f < P.n_field) ? P.m2phi[f] : 1.0;
       }
+      if constexpr (MF == 2)   // a padding lane beside a real field point: the real one's masses (its joint products are then its own)
+        if (f0 + NTC >= P.n_field && f0 < P.n_field) { m2psi[1] = m2psi[0]; m2phi[1] = m2phi[0]; }
+      if constexpr (MF == 2) solo = !(fabs(m2phi[0]) < M3_JOINT_MASS_MAX) || !(fabs(m2phi[1]) < M3_JOINT_MASS_MAX);
     }
     if (u == u0 || i == 0) {
 #pragma unroll
@@ -1001,6 +1054,7 @@ __global__ void __launch_bounds__(NTC, 1) mats3d_gmoment_kernel(const Mats3dPara
           }
         }
       }
+      if (pipelined) mats3d_row_decouple<MF, SQ, SYM>(d0 + m * nc, num4, nc, m2phi, M, solo);
       // ---- the (j, n) pairs with |j - n| = m ----
       const int jlo1 = max(0, m - n_max), jhi1 = min(n_jext - 1, n_max + m);
       const int jhi2 = m > 0 ? min(n_jext - 1, n_max - m) : -1;

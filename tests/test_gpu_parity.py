@@ -329,36 +329,59 @@ def test_lpa_batched_temperatures_are_the_single_calls():
             assert np.array_equal(hf, flow.cpu().numpy()) and np.array_equal(hc, chan.cpu().numpy())
 
 
-def test_batched_reciprocal_range_and_coupling_are_as_documented():
-    """include/dfrg.h, "Magnitude range and coupling of the batched reciprocals": masses up to ~1e75 k^2 are fine everywhere;
-    a denominator beyond the range at field point f invalidates f and its partner (f + 256 in the Matsubara family, f + 128
-    in the two-point family) and nothing else; DFRG_M3_ONE_FIELD confines it to f."""
+def test_field_points_are_independent_outputs_also_where_reciprocals_are_batched():
+    """Reading A4 / include/dfrg.h "numerical special cases": what IEEE arithmetic gives, PER OUTPUT -- as the oracle, whose
+    outputs are independent.  The two-point and Matsubara kernels invert the denominators of the two field points of a thread
+    (f and f + 256, resp. f + 128) through one product; a mass that takes that product out of the double range (1e80, 1e200)
+    or is NaN at field point f must cost nothing but f's own output where that is NaN in the oracle too: the partner, and f
+    itself for the huge masses, agree with the oracle at the usual bars.  Also with DFRG_M3_ONE_FIELD (no batching).
+    (Blown-up masses are what a diverging flow produces; the one documented residue, a denominator that is exactly zero at
+    a node, cannot be constructed from outside and is not tested.)"""
     from paper_2412_13043_b200 import binding as B
-    # Matsubara family, 600 field points: tile 0 pairs f with f + 256
+    # Matsubara family, 600 field points: tile 0 pairs f with f + 256; tile 1 (f >= 512) has padding lanes as partners
     c = inputs.config4(n_field=600, n_p=1, n_jext=2, n_q=6, n_c=8)
     c["n_max"] = 2
     c["m2psi"], c["m2phi"] = c["m2psi"].copy(), c["m2phi"].copy()
-    c["m2psi"][10] = c["m2phi"][10] = 1e30                  # inside the documented range: correct, partner too
+    c["m2psi"][10] = c["m2phi"][10] = 1e30
+    c["m2phi"][20] = 1e80                                   # the product of four denominators overflows
+    c["m2phi"][50] = 1e200                                  # the product of two overflows
+    c["m2phi"][530] = 1e80                                  # partner is a padding lane
+    c["m2phi"][300] = 1e-300                                # partner (f = 44) regular; harmless either way
     R = make_rules(c, B.dfrg_quad_nodes)
     o = oracle_run(c, R)
-    g = gpu_run(c, R)
-    assert_parity(g["out"], o["out"], o["dmin"], o["sens"], "m2 = 1e30")
-    c["m2phi"][20] = 1e80                                   # outside: f = 20 and its partner f = 276 are lost, nothing else
+    assert np.all(np.isfinite(o["out"]))
+    for path in (0, B.M3_ONE_FIELD, B.M3_ANY_SHAPE, B.M3_PLAIN_MOMENTS):
+        g = gpu_run(dict(c, path=path), R)
+        assert_parity(g["out"], o["out"], o["dmin"], o["sens"], "huge masses, path %d" % path)
+    c["m2phi"][30] = np.nan                                 # f = 30 is lost (NaN in the oracle as well), f = 286 is not
+    c["m2psi"][70] = np.nan                                 # fermion line: inverted per field point anyway
     o = oracle_run(c, R)
     keep = np.ones(600, dtype=bool)
-    keep[[20, 276]] = False
-    g = gpu_run(c, R)
-    assert_parity(g["out"][..., keep], o["out"][..., keep], o["dmin"][..., keep], o["sens"][..., keep], "m2 = 1e80")
-    keep[276] = True
-    g = gpu_run(dict(c, path=B.M3_ONE_FIELD), R)            # every field point inverted on its own
-    assert_parity(g["out"][..., keep], o["out"][..., keep], o["dmin"][..., keep], o["sens"][..., keep], "m2 = 1e80, one field")
-    # two-point family, 300 field points: f pairs with f + 128
+    keep[[30, 70]] = False
+    assert np.all(np.isnan(o["out"][..., ~keep])) and np.all(np.isfinite(o["out"][..., keep]))
+    for path in (0, B.M3_ONE_FIELD, B.M3_ANY_SHAPE):
+        g = gpu_run(dict(c, path=path), R)
+        assert np.all(np.isnan(g["out"][..., ~keep]))
+        assert_parity(g["out"][..., keep], o["out"][..., keep], o["dmin"][..., keep], o["sens"][..., keep],
+                      "NaN mass, path %d" % path)
+    # two-point family, 300 field points: f pairs with f + 128; f >= 256 + 44 = 300 are padding lanes
     c = inputs.config2(n_field=300, n_ext=2, n_q=12, n_c=6)
     c["m2"] = c["m2"].copy()
     c["m2"][5] = 1e80
+    c["m2"][9] = 1e200
+    c["m2"][290] = 1e200                                    # partner is a padding lane
     R = make_rules(c, B.dfrg_quad_nodes)
     o = oracle_run(c, R)
-    keep = np.ones(300, dtype=bool)
-    keep[[5, 133]] = False
+    assert np.all(np.isfinite(o["out"]))
     g = gpu_run(c, R)
-    assert_parity(g["out"][:, keep], o["out"][:, keep], o["dmin"][:, keep], o["sens"][:, keep], "two-point m2 = 1e80")
+    assert_parity(g["out"], o["out"], o["dmin"], o["sens"], "two-point huge masses")
+    d = gpu_run(c, R, want_d=True)
+    assert np.array_equal(d["out"], g["out"])               # values do not depend on whether derivatives were asked for
+    c["m2"][7] = np.nan
+    o = oracle_run(c, R)
+    keep = np.ones(300, dtype=bool)
+    keep[7] = False
+    assert np.all(np.isnan(o["out"][:, 7])) and np.all(np.isfinite(o["out"][:, keep]))
+    g = gpu_run(c, R)
+    assert np.all(np.isnan(g["out"][:, 7]))
+    assert_parity(g["out"][:, keep], o["out"][:, keep], o["dmin"][:, keep], o["sens"][:, keep], "two-point NaN mass")
