@@ -40,7 +40,7 @@ WORKLOAD = "cfg4_matsubara3d: 64 p x 16 j x 512 field points, 23 Matsubara terms
 # FP64 roofline denominator: 148 SMs x 64 FP64 lanes x 2 flop/DFMA x 1.965 GHz
 FP64_LANES_PER_SM = 64
 # the committed `ncu --set full` capture of the bench kernel on this workload: roofline.traffic is read from it
-NCU_CAPTURE = os.path.join("profiles", "r2_bench_kernel.md")
+NCU_CAPTURE = os.path.join("profiles", "r3_bench_kernel.md")
 
 
 def ncu_dram_bytes_per_launch():
