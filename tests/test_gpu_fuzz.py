@@ -77,7 +77,7 @@ def draw(rng):
     return fam, c
 
 
-N_SEEDS = int(os.environ.get("DFRG_FUZZ_SEEDS", "100"))      # a longer soak: DFRG_FUZZ_SEEDS=2000 python -m pytest tests/test_gpu_fuzz.py
+N_SEEDS = int(os.environ.get("DFRG_FUZZ_SEEDS", "400"))      # a longer soak: DFRG_FUZZ_SEEDS=2000 python -m pytest tests/test_gpu_fuzz.py
 
 
 @pytest.mark.parametrize("seed", range(N_SEEDS))
